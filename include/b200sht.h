@@ -1,0 +1,134 @@
+/* b200sht.h -- C ABI of the B200-native spin spherical harmonic / Wigner transform library.
+ *
+ * Implements the hot path of arXiv 2311.14670 (Price & McEwen): forward and inverse spin-s spherical harmonic
+ * transforms and Wigner (SO(3)) transforms, computed with the paper's Wigner d-function recursion along the
+ * harmonic order m (Eq. 25-27; renormalised on the fly, Sec. 3.4) fused with
+ * the separable theta-ring contraction (Eq. 30 / Eq. 33; Sec. 4.4).
+ * The four maps are the paper's problem statement:
+ *     F : B_L(S^2) -> C^{L^2},  F^-1,   W : B_L(SO(3)) -> C^{(4L^3-L)/3},  W^-1.
+ *
+ * Conventions (all entry points)
+ *   - Pointers named `f`, `flm`, `flmn`, `work` are DEVICE pointers owned by the caller.  Inputs are never
+ *     modified; outputs are fully overwritten (coefficients outside the support |m| <= l, l >= |spin|, |n| <= l
+ *     are written as 0).  The library never frees or keeps caller memory beyond the plan's workspace.
+ *   - All work is enqueued on `stream`; no entry point synchronises the device except sht_plan_timings().
+ *   - Errors are return codes; nothing throws across the ABI.  sht_status_string() names them.
+ *   - Layouts are row-major, last index fastest; complex = interleaved (re, im) doubles.
+ *       flm  [L][2L-1]            (l, m+L-1)                              embeds C^{L^2}
+ *       MW map   f[L][2L-1]       (theta_t, phi_p), theta_t=(2t+1)pi/(2L-1), phi_p=2 pi p/(2L-1)   (Eq. 37-38)
+ *       HEALPix  f[12 nside^2]    ring-ordered: rings north to south, phi increasing within a ring
+ *       SO(3)    f[2N-1][L][2L-1] (gamma_g, beta_b, alpha_a), MW in (beta, alpha), gamma_g = 2 pi g/(2N-1)
+ *       flmn [2N-1][L][2L-1]      (n+N-1, l, m+L-1)
+ *     With reality = 1 (spin 0 only) maps are arrays of real doubles of the same shape, and the m < 0 half of
+ *     flm is ignored on input / filled with (-1)^m conj(f_{l,-m}) on output.
+ *   - dtype: SHT_F64 only in this version (SHT_F32 returns SHT_EUNSUPPORTED).
+ */
+#ifndef B200SHT_H
+#define B200SHT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SHT_OK = 0,
+    SHT_EINVAL = 1,        /* bad argument (L < 1, |spin| >= L, N > L, reality with spin != 0, null pointer ...) */
+    SHT_EUNSUPPORTED = 2,  /* valid request this build does not implement (fp32, batch > 1) */
+    SHT_EWORKSPACE = 3,    /* workspace missing or too small */
+    SHT_ECUDA = 4,         /* a CUDA runtime call failed (cudaGetLastError text via sht_last_error()) */
+    SHT_ECUFFT = 5         /* a cuFFT call failed */
+} sht_status;
+
+enum { SHT_MW = 0, SHT_HEALPIX = 1 };   /* sampling */
+enum { SHT_F64 = 0, SHT_F32 = 1 };      /* dtype    */
+
+typedef struct sht_plan sht_plan;       /* opaque; host object holding sizes, cuFFT handles and table pointers */
+typedef void* sht_stream;               /* a cudaStream_t */
+
+const char* sht_status_string(sht_status s);
+const char* sht_last_error(void);       /* text of the last CUDA / cuFFT failure on this thread ("" if none) */
+
+/* ---- plans ------------------------------------------------------------------------------------------------
+ * A plan fixes (L, spin, sampling, nside, reality) for S^2 or (L, N) for SO(3).  It owns no device memory:
+ * the caller provides one workspace of sht_plan_workspace_bytes() bytes (tables + scratch), which
+ * sht_plan_set_workspace() fills with the O(L^2) ring / start-value tables ("optionally precompute some
+ * additional internal terms ... O(L^2)"; Eq. 27 start values in mantissa/exponent form).
+ * The workspace must stay valid and untouched while the plan is used.  One plan = one stream at a time.
+ * nside is used for HEALPix only (the band-limit L is independent of it).
+ */
+sht_status sht_plan_s2(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype);
+sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);
+size_t     sht_plan_workspace_bytes(const sht_plan* plan);
+sht_status sht_plan_set_workspace(sht_plan* plan, void* work, size_t work_bytes, sht_stream stream);
+sht_status sht_plan_destroy(sht_plan* plan);
+
+/* ---- transforms through a plan (device pointers) -----------------------------------------------------------
+ * s2_forward : map f -> flm.  MW: FFT in phi (Eq. 31), extension to the torus and 2x upsampling in theta
+ *              (PAPER.md:379-381), quadrature weights Eq. 41-44 at band-limit 2L, then the fused recursion +
+ *              theta contraction of Eq. 30.  HEALPix: ring FFTs with phase shift and periodic extension
+ *              (PAPER.md:403-407), weights 4 pi/Npix, Eq. 30.
+ * s2_inverse : flm -> map f.  Fused recursion + l contraction of Eq. 33, then ring synthesis Eq. 32 (HEALPix:
+ *              aliasing fold of F_m onto m mod nphi).
+ * so3_forward / so3_inverse : Eq. 15-18: FFT in gamma and one spin -n transform per
+ *              n = -(N-1)..N-1, all n batched in the same kernel launches.
+ */
+sht_status s2_forward_plan(sht_plan* plan, const void* f, void* flm, sht_stream stream);
+sht_status s2_inverse_plan(sht_plan* plan, const void* flm, void* f, sht_stream stream);
+sht_status so3_forward_plan(sht_plan* plan, const void* f, void* flmn, sht_stream stream);
+sht_status so3_inverse_plan(sht_plan* plan, const void* flmn, void* f, sht_stream stream);
+
+/* The hot path alone (the fused recursion + contraction kernels and their pole-ring companions), for timing and
+ * for sampled parity at sizes where the full map is too large for the oracle:
+ *   s2_theta_inverse_plan: flm -> Fm[2L-1][ntheta] (row m+L-1; ntheta = sht_plan_ntheta(plan, 0)); Eq. 33.
+ *   s2_theta_forward_plan: Wm[2L-1][ntheta_q] (row m+L-1; already weighted; ntheta_q = sht_plan_ntheta(plan, 1),
+ *                          2L on MW) -> flm; Eq. 30.
+ */
+int        sht_plan_ntheta(const sht_plan* plan, int forward);
+sht_status s2_theta_inverse_plan(sht_plan* plan, const void* flm, void* Fm, sht_stream stream);
+sht_status s2_theta_forward_plan(sht_plan* plan, const void* Wm, void* flm, sht_stream stream);
+
+/* Stage timing.  After sht_plan_enable_timing(plan, 1) every transform records CUDA events between its stages;
+ * sht_plan_timings() synchronises on the last transform's final event and returns milliseconds:
+ *   ms[0] = hot kernels (fused recursion + contraction, incl. pole ring)   -- FP64-pipe bound
+ *   ms[1] = FFTs (cuFFT: phi, theta-upsampling, gamma)                     -- HBM bound
+ *   ms[2] = staging kernels (transposes, scaling, phases, extension, fold) -- HBM bound
+ *   ms[3] = total.
+ */
+sht_status sht_plan_enable_timing(sht_plan* plan, int on);
+sht_status sht_plan_timings(sht_plan* plan, float ms[4]);
+
+/* ---- the north-star calls: fp64, batch 1, plan + workspace cached inside the library ------------------------
+ * (device pointers; the cache allocates its workspaces with cudaMalloc on first use of an argument set and
+ * sht_cache_clear() releases them).  HEALPix uses nside = L/2 here (L even).
+ */
+sht_status s2_forward(int L, int spin, int sampling, int reality, const void* f, void* flm, sht_stream stream);
+sht_status s2_inverse(int L, int spin, int sampling, int reality, const void* flm, void* f, sht_stream stream);
+sht_status so3_forward(int L, int N, const void* f, void* flmn, sht_stream stream);
+sht_status so3_inverse(int L, int N, const void* flmn, void* f, sht_stream stream);
+sht_status sht_cache_clear(void);
+
+/* ---- host-buffer convenience (end-to-end path): HOST pointers, copies in and out on `stream`, then a stream
+ * synchronise.  Same semantics and layouts as above.
+ */
+sht_status s2_forward_host(int L, int spin, int sampling, int reality, const void* f_host, void* flm_host, sht_stream stream);
+sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const void* flm_host, void* f_host, sht_stream stream);
+sht_status so3_forward_host(int L, int N, const void* f_host, void* flmn_host, sht_stream stream);
+sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, sht_stream stream);
+
+/* ---- measurement helper: register-only DFMA chain, returns achieved FP64 TFLOP/s and kernel ms (used by
+ * bench.py for the FP64 roofline denominator, since MEASURED_PEAKS.json has no FP64 entry). */
+sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream);
+
+/* ---- introspection --------------------------------------------------------------------------------------- */
+/* number of kernels of this library launched by the calling thread since the last reset (bench: gpu_launches) */
+long       sht_launch_count(int reset);
+/* number of d-steps (one Eq. 25 evaluation for one (l, theta, pass)) one transform of this plan performs */
+double     sht_plan_dsteps(const sht_plan* plan, int forward);
+const char* sht_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* B200SHT_H */

@@ -1,0 +1,71 @@
+"""ctypes loader of libb200sht.so (built in-tree by paper_2311_14670_b200/build.py).  No fallback: a missing or
+unloadable library is an error."""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libb200sht.so")
+
+SHT_MW, SHT_HEALPIX = 0, 1
+SHT_F64, SHT_F32 = 0, 1
+
+# every symbol include/b200sht.h declares: name -> (restype, argtypes)
+_vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
+SIGNATURES = {
+    "sht_status_string": (C.c_char_p, [_i]),
+    "sht_last_error": (C.c_char_p, []),
+    "sht_plan_s2": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i]),
+    "sht_plan_so3": (_i, [C.POINTER(_vp), _i, _i, _i]),
+    "sht_plan_workspace_bytes": (_sz, [_vp]),
+    "sht_plan_set_workspace": (_i, [_vp, _vp, _sz, _vp]),
+    "sht_plan_destroy": (_i, [_vp]),
+    "s2_forward_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "s2_inverse_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "so3_forward_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "so3_inverse_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "sht_plan_ntheta": (_i, [_vp, _i]),
+    "s2_theta_inverse_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "s2_theta_forward_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "sht_plan_enable_timing": (_i, [_vp, _i]),
+    "sht_plan_timings": (_i, [_vp, C.POINTER(C.c_float)]),
+    "s2_forward": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
+    "s2_inverse": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
+    "so3_forward": (_i, [_i, _i, _vp, _vp, _vp]),
+    "so3_inverse": (_i, [_i, _i, _vp, _vp, _vp]),
+    "sht_cache_clear": (_i, []),
+    "s2_forward_host": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
+    "s2_inverse_host": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
+    "so3_forward_host": (_i, [_i, _i, _vp, _vp, _vp]),
+    "so3_inverse_host": (_i, [_i, _i, _vp, _vp, _vp]),
+    "sht_fp64_peak": (_i, [_i, C.POINTER(C.c_double), C.POINTER(C.c_float), _vp]),
+    "sht_launch_count": (C.c_long, [_i]),
+    "sht_plan_dsteps": (C.c_double, [_vp, _i]),
+    "sht_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library (once).  Raises if it has not been built -- there is no CPU path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2311_14670_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+class ShtError(RuntimeError):
+    pass
+
+
+def check(status):
+    if status != 0:
+        L = lib()
+        raise ShtError(f"{L.sht_status_string(status).decode()} [{L.sht_last_error().decode()}]")

@@ -1,0 +1,191 @@
+"""Python binding of include/b200sht.h -- argument marshalling only; every step of the transforms runs in the CUDA
+library.  PyTorch supplies device memory and the current CUDA stream, nothing else.
+
+Layouts (see include/b200sht.h): flm[L, 2L-1] complex128 (column m+L-1); MW maps f[L, 2L-1]; HEALPix maps
+f[12 nside^2] ring-ordered; SO(3) f[2N-1, L, 2L-1] = (gamma, beta, alpha); flmn[2N-1, L, 2L-1] = (n+N-1, l, m+L-1).
+With reality=True maps are float64.
+"""
+import ctypes as C
+
+import numpy as np
+import torch
+
+from ._lib import SHT_F64, SHT_HEALPIX, SHT_MW, check, lib
+
+MW, HEALPIX = SHT_MW, SHT_HEALPIX
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t, dtype, shape, what):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda):
+        raise TypeError(f"{what} must be a CUDA tensor")
+    if t.dtype != dtype or tuple(t.shape) != tuple(shape) or not t.is_contiguous():
+        raise ValueError(f"{what}: expected contiguous {dtype} of shape {tuple(shape)}, got {t.dtype} {tuple(t.shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+def map_shape(L, sampling=MW, nside=0):
+    return (L, 2 * L - 1) if sampling == MW else (12 * nside * nside,)
+
+
+class Plan:
+    """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
+
+    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0"):
+        self._h = C.c_void_p()
+        self.L, self.spin, self.sampling, self.nside, self.reality, self.N = L, spin, sampling, nside, bool(reality), N
+        self.device = torch.device(device)
+        L_ = lib()
+        with torch.cuda.device(self.device):
+            if N is None:
+                check(L_.sht_plan_s2(C.byref(self._h), L, spin, sampling, nside, int(self.reality), SHT_F64))
+            else:
+                check(L_.sht_plan_so3(C.byref(self._h), L, N, SHT_F64))
+            nbytes = L_.sht_plan_workspace_bytes(self._h)
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            check(L_.sht_plan_set_workspace(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes, _stream()))
+        self.map_dtype = torch.float64 if self.reality else torch.complex128
+        self.coef_shape = (L, 2 * L - 1) if N is None else (2 * N - 1, L, 2 * L - 1)
+        self.map_shape = map_shape(L, sampling, nside) if N is None else (2 * N - 1, L, 2 * L - 1)
+
+    def __del__(self):
+        try:
+            if self._h:
+                lib().sht_plan_destroy(self._h)
+                self._h = C.c_void_p()
+        except Exception:
+            pass
+
+    # -- transforms (device tensors in, device tensors out) --
+    def forward(self, f, out=None):
+        out = torch.empty(self.coef_shape, dtype=torch.complex128, device=self.device) if out is None else out
+        fn = lib().s2_forward_plan if self.N is None else lib().so3_forward_plan
+        check(fn(self._h, _dev(f, self.map_dtype, self.map_shape, "f"), _dev(out, torch.complex128, self.coef_shape, "flm"), _stream()))
+        return out
+
+    def inverse(self, flm, out=None):
+        out = torch.empty(self.map_shape, dtype=self.map_dtype, device=self.device) if out is None else out
+        fn = lib().s2_inverse_plan if self.N is None else lib().so3_inverse_plan
+        check(fn(self._h, _dev(flm, torch.complex128, self.coef_shape, "flm"), _dev(out, self.map_dtype, self.map_shape, "f"), _stream()))
+        return out
+
+    def ntheta(self, forward):
+        return int(lib().sht_plan_ntheta(self._h, int(forward)))
+
+    def theta_inverse(self, flm):
+        """Hot path only (Eq. 33): flm -> F[2L-1, ntheta], row m+L-1."""
+        out = torch.empty((2 * self.L - 1, self.ntheta(False)), dtype=torch.complex128, device=self.device)
+        check(lib().s2_theta_inverse_plan(self._h, _dev(flm, torch.complex128, self.coef_shape, "flm"), C.c_void_p(out.data_ptr()), _stream()))
+        return out
+
+    def theta_forward(self, W):
+        """Hot path only (Eq. 30): weighted W[2L-1, ntheta_q] (row m+L-1) -> flm."""
+        shape = (2 * self.L - 1, self.ntheta(True))
+        out = torch.empty(self.coef_shape, dtype=torch.complex128, device=self.device)
+        check(lib().s2_theta_forward_plan(self._h, _dev(W, torch.complex128, shape, "W"), C.c_void_p(out.data_ptr()), _stream()))
+        return out
+
+    def enable_timing(self, on=True):
+        check(lib().sht_plan_enable_timing(self._h, int(on)))
+
+    def timings(self):
+        """dict(hot, fft, staging, total) in ms for the last transform (synchronises)."""
+        ms = (C.c_float * 4)()
+        check(lib().sht_plan_timings(self._h, ms))
+        return dict(hot=ms[0], fft=ms[1], staging=ms[2], total=ms[3])
+
+    def dsteps(self, forward):
+        return float(lib().sht_plan_dsteps(self._h, int(forward)))
+
+
+# -- the north-star calls (library-side plan cache; device tensors) --
+def s2_forward(f, L, spin=0, sampling=MW, reality=False):
+    nside = L // 2 if sampling == HEALPIX else 0
+    dt = torch.float64 if reality else torch.complex128
+    flm = torch.empty((L, 2 * L - 1), dtype=torch.complex128, device=f.device)
+    with torch.cuda.device(f.device):
+        check(lib().s2_forward(L, spin, sampling, int(reality), _dev(f, dt, map_shape(L, sampling, nside), "f"), C.c_void_p(flm.data_ptr()), _stream()))
+    return flm
+
+
+def s2_inverse(flm, L, spin=0, sampling=MW, reality=False):
+    nside = L // 2 if sampling == HEALPIX else 0
+    dt = torch.float64 if reality else torch.complex128
+    f = torch.empty(map_shape(L, sampling, nside), dtype=dt, device=flm.device)
+    with torch.cuda.device(flm.device):
+        check(lib().s2_inverse(L, spin, sampling, int(reality), _dev(flm, torch.complex128, (L, 2 * L - 1), "flm"), C.c_void_p(f.data_ptr()), _stream()))
+    return f
+
+
+def so3_forward(f, L, N):
+    shape = (2 * N - 1, L, 2 * L - 1)
+    flmn = torch.empty(shape, dtype=torch.complex128, device=f.device)
+    with torch.cuda.device(f.device):
+        check(lib().so3_forward(L, N, _dev(f, torch.complex128, shape, "f"), C.c_void_p(flmn.data_ptr()), _stream()))
+    return flmn
+
+
+def so3_inverse(flmn, L, N):
+    shape = (2 * N - 1, L, 2 * L - 1)
+    f = torch.empty(shape, dtype=torch.complex128, device=flmn.device)
+    with torch.cuda.device(flmn.device):
+        check(lib().so3_inverse(L, N, _dev(flmn, torch.complex128, shape, "flmn"), C.c_void_p(f.data_ptr()), _stream()))
+    return f
+
+
+# -- end-to-end through HOST buffers (numpy arrays; copies happen inside the C call) --
+def _host(a, dtype, shape, what):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if tuple(a.shape) != tuple(shape):
+        raise ValueError(f"{what}: expected shape {tuple(shape)}, got {a.shape}")
+    return a
+
+
+def s2_forward_host(f, L, spin=0, sampling=MW, reality=False, out=None):
+    nside = L // 2 if sampling == HEALPIX else 0
+    f = _host(f, np.float64 if reality else np.complex128, map_shape(L, sampling, nside), "f")
+    out = np.empty((L, 2 * L - 1), np.complex128) if out is None else out
+    check(lib().s2_forward_host(L, spin, sampling, int(reality), f.ctypes.data, out.ctypes.data, _stream()))
+    return out
+
+
+def s2_inverse_host(flm, L, spin=0, sampling=MW, reality=False, out=None):
+    nside = L // 2 if sampling == HEALPIX else 0
+    flm = _host(flm, np.complex128, (L, 2 * L - 1), "flm")
+    out = np.empty(map_shape(L, sampling, nside), np.float64 if reality else np.complex128) if out is None else out
+    check(lib().s2_inverse_host(L, spin, sampling, int(reality), flm.ctypes.data, out.ctypes.data, _stream()))
+    return out
+
+
+def so3_forward_host(f, L, N, out=None):
+    shape = (2 * N - 1, L, 2 * L - 1)
+    f = _host(f, np.complex128, shape, "f")
+    out = np.empty(shape, np.complex128) if out is None else out
+    check(lib().so3_forward_host(L, N, f.ctypes.data, out.ctypes.data, _stream()))
+    return out
+
+
+def so3_inverse_host(flmn, L, N, out=None):
+    shape = (2 * N - 1, L, 2 * L - 1)
+    flmn = _host(flmn, np.complex128, shape, "flmn")
+    out = np.empty(shape, np.complex128) if out is None else out
+    check(lib().so3_inverse_host(L, N, flmn.ctypes.data, out.ctypes.data, _stream()))
+    return out
+
+
+def fp64_peak(iters=20000):
+    """Measured FP64 FMA throughput of this GPU (register-only DFMA chains): (TFLOP/s, ms)."""
+    tf, ms = C.c_double(), C.c_float()
+    check(lib().sht_fp64_peak(iters, C.byref(tf), C.byref(ms), _stream()))
+    return tf.value, ms.value
+
+
+def launch_count(reset=False):
+    return int(lib().sht_launch_count(int(reset)))
+
+
+def cache_clear():
+    check(lib().sht_cache_clear())

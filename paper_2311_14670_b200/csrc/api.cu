@@ -1,0 +1,776 @@
+// api.cu -- the C ABI of include/b200sht.h: plans, workspace layout, stage orchestration, cuFFT calls.
+//
+// Data flow; everything is m-major so that the hot kernels read contiguous tiles:
+//   inverse:  coef[l][m] --prep--> G[pass][m][l]  ==theta_inverse==>  F[m mod NB][ring]  --cuFFT(phi)--> map
+//   forward:  map --cuFFT(phi)--> Fa[m][ring] --MW extend / theta-FFT / pad / theta-iFFT--> U[m][ring']
+//             --weight_split--> W[pass][m][ring']  ==theta_forward==>  H[m][l]  --finalize--> coef[l][m]
+#include "../../include/b200sht.h"
+#include "internal.h"
+#include "staging.h"
+
+#include <cufft.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <map>
+#include <mutex>
+#include <string>
+#include <tuple>
+#include <vector>
+
+namespace {
+
+thread_local long g_launches = 0;
+thread_local std::string g_err;
+
+typedef long double ld;
+const ld PI_L = 3.14159265358979323846264338327950288L;
+
+inline size_t rup(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            g_err = std::string(#call) + ": " + cudaGetErrorString(e__);                           \
+            return SHT_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)
+#define CF(call)                                                                                   \
+    do {                                                                                           \
+        cufftResult r__ = (call);                                                                  \
+        if (r__ != CUFFT_SUCCESS) {                                                                \
+            g_err = std::string(#call) + ": cufft error " + std::to_string((int)r__);              \
+            return SHT_ECUFFT;                                                                     \
+        }                                                                                          \
+    } while (0)
+#define CS(call)                                                                                   \
+    do {                                                                                           \
+        sht_status s__ = (call);                                                                   \
+        if (s__ != SHT_OK) return s__;                                                             \
+    } while (0)
+
+// ---- one set of iso-latitude rings the theta kernels run on -----------------------------------------------------
+struct RingSet {
+    int nth = 0, ntp = 0;      // regular rings, padded count (multiple of 128; > nth so a pole ring fits)
+    bool pole = false;         // a theta = pi ring at index nth (MW, Eq. 29)
+    std::vector<ld> ct, c2, s2;  // host: cos(theta), cos(theta/2), sin(theta/2) of the regular rings
+    double *csc = nullptr, *tau = nullptr, *sig = nullptr, *c2hi = nullptr, *c2lo = nullptr, *s2hi = nullptr, *s2lo = nullptr;
+    double* wq = nullptr;      // [ntp] forward quadrature weight per ring (incl. the pole ring at index nth)
+    struct Start { double* val; uint8_t* k; };
+    std::map<int, Start> start;   // second index n -> windowed start values [Lp][ntp]
+    std::map<int, int*> mlo;      // key 2n (pass A) / 2n+1 (pass B) -> per-ring first served step
+};
+
+struct PassHost {
+    ThetaPass p;
+    int mode;                  // 0 PM, 1 P
+};
+
+enum { CAT_HOT = 0, CAT_FFT = 1, CAT_STAGE = 2 };
+
+}  // namespace
+
+struct sht_plan {
+    int kind = 0;              // 0 S^2, 1 SO(3)
+    int L = 0, spin = 0, sampling = 0, nside = 0, reality = 0, N = 1;
+    int Lp = 0, NB = 0;        // padded L; 2L-1
+    int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
+    std::vector<int> slab_n;   // second index n of d^l_{m,n} per slab
+    RingSet inv, fwd;          // rings of the inverse theta step / of the forward quadrature
+    int kmin = 0, kstride = 0, krows = 0;
+    int8_t* kexp = nullptr;
+    double* rsq = nullptr;
+    double *scale_inv = nullptr, *scale_fwd = nullptr;   // [Lp] l-dependent factors
+    // pass lists (host copies + device arrays), split by kernel mode
+    std::vector<PassHost> pinv, pfwd;
+    ThetaPass *d_inv_pm = nullptr, *d_inv_p = nullptr, *d_fwd_pm = nullptr, *d_fwd_p = nullptr;
+    int n_inv_pm = 0, n_inv_p = 0, n_fwd_pm = 0, n_fwd_p = 0;
+    // scratch
+    double2 *F = nullptr, *Fa = nullptr, *X = nullptr, *Z = nullptr, *H = nullptr, *cplx = nullptr, *fn = nullptr;
+    double2* polev = nullptr;  // [nslab] pole-ring values of the inverse
+    double* tmp = nullptr;     // [2*Lp] plan-time scratch
+    double* unit_wq = nullptr; // [fwd.ntp] ones (theta-stage entry point takes already weighted rows)
+    size_t F_slab = 0, Fa_slab = 0, X_slab = 0, Z_slab = 0, H_slab = 0;
+    int Ltp = 0;               // padded ring count of Fa rows
+    void* fft_work = nullptr; size_t fft_work_bytes = 0;
+    cufftHandle fft_phi_inv = 0, fft_phi_fwd = 0, fft_th1 = 0, fft_th2 = 0, fft_gamma = 0;
+    bool have_fft = false;
+    // workspace
+    void* work = nullptr; size_t work_bytes = 0, need_bytes = 0;
+    bool ready = false;
+    // timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev; std::vector<int> ev_cat; int ev_n = 0;
+    double dsteps_inv = 0, dsteps_fwd = 0;
+};
+
+namespace {
+
+// ---- host-side ring geometry (long double; the GPU tables are split into hi/lo doubles where it matters) ---------
+void rings_mw(RingSet& R, int Lt) {      // Eq. 37: theta_t = (2t+1)pi/(2Lt-1); ring Lt-1 is theta = pi
+    R.nth = Lt - 1; R.pole = true;
+    R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
+    for (int t = 0; t < R.nth; ++t) {
+        ld th = PI_L * (ld)(2 * t + 1) / (ld)(2 * Lt - 1);
+        R.ct[t] = cosl(th); R.c2[t] = cosl(th / 2); R.s2[t] = sinl(th / 2);
+    }
+    R.ntp = (int)rup((size_t)R.nth + 1, 128);
+}
+
+struct Bump {
+    size_t off = 0; char* base = nullptr;
+    template <class T> T* take(size_t n) {
+        off = rup(off, 256);
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+void stage(sht_plan* P, int cat, cudaStream_t st) {
+    if (!P->timing) return;
+    if (P->ev_n >= (int)P->ev.size()) return;
+    cudaEventRecord(P->ev[P->ev_n], st);
+    P->ev_cat[P->ev_n] = cat;
+    P->ev_n++;
+}
+
+// Walks the workspace layout.  With base == nullptr it only measures; otherwise it assigns every pointer.
+void layout(sht_plan* P, char* base) {
+    Bump B; B.base = base;
+    const int L = P->L, Lp = P->Lp, NB = P->NB;
+    P->rsq = B.take<double>(2 * (size_t)Lp + 64);
+    P->kexp = B.take<int8_t>((size_t)P->krows * P->kstride);
+    P->scale_inv = B.take<double>(Lp);
+    P->scale_fwd = B.take<double>(Lp);
+    for (RingSet* R : {&P->inv, &P->fwd}) {
+        R->csc = B.take<double>(R->ntp); R->tau = B.take<double>(R->ntp); R->sig = B.take<double>(R->ntp);
+        R->c2hi = B.take<double>(R->ntp); R->c2lo = B.take<double>(R->ntp);
+        R->s2hi = B.take<double>(R->ntp); R->s2lo = B.take<double>(R->ntp);
+        R->wq = B.take<double>(R->ntp);
+        for (auto& kv : R->start) {
+            kv.second.val = B.take<double>((size_t)Lp * R->ntp);
+            kv.second.k = B.take<uint8_t>((size_t)Lp * R->ntp);
+        }
+        for (auto& kv : R->mlo) kv.second = B.take<int>(R->ntp);
+    }
+    P->d_inv_pm = B.take<ThetaPass>(P->pinv.size() + 1); P->d_inv_p = B.take<ThetaPass>(P->pinv.size() + 1);
+    P->d_fwd_pm = B.take<ThetaPass>(P->pfwd.size() + 1); P->d_fwd_p = B.take<ThetaPass>(P->pfwd.size() + 1);
+    // per-pass operand buffers
+    for (auto& ph : P->pinv) ph.p.in = B.take<double2>((size_t)(L - ph.p.m_end) * Lp * (ph.mode == 0 ? 2 : 1));
+    for (auto& ph : P->pfwd) ph.p.in = B.take<double2>((size_t)(L - ph.p.m_end) * P->fwd.ntp * (ph.mode == 0 ? 2 : 1));
+    // scratch arrays
+    P->F_slab = (size_t)NB * P->inv.ntp;
+    P->F = B.take<double2>(P->F_slab * P->nslab);
+    P->polev = B.take<double2>(P->nslab);
+    P->tmp = B.take<double>(2 * (size_t)Lp);
+    P->unit_wq = B.take<double>(P->fwd.ntp);
+    P->Ltp = P->inv.ntp;
+    P->Fa_slab = (size_t)NB * P->Ltp;
+    P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
+    P->X_slab = (size_t)NB * NB;
+    P->X = B.take<double2>(P->X_slab * P->nslab);
+    P->Z_slab = (size_t)NB * (4 * L - 1);
+    P->Z = B.take<double2>(P->Z_slab * P->nslab);
+    P->H_slab = (size_t)NB * Lp;
+    P->H = B.take<double2>(P->H_slab * P->nslab);
+    if (P->reality) P->cplx = B.take<double2>((size_t)L * NB);
+    if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
+    P->fft_work = B.take<char>(P->fft_work_bytes);
+    // route every pass to its slab's output array
+    for (auto& ph : P->pinv) ph.p.out = P->F ? P->F + P->F_slab * ph.p.slab : nullptr;
+    for (auto& ph : P->pfwd) ph.p.out = P->H ? P->H + P->H_slab * ph.p.slab : nullptr;
+    P->need_bytes = rup(B.off, 256);
+}
+
+void add_passes(sht_plan* P, int slab, int n, bool real) {
+    auto mk = [&](int nn, int sgn, int m_end, int mode, int mlo_key) {
+        PassHost a{}; a.mode = mode;
+        a.p.n = nn; a.p.sgn_out = sgn; a.p.m_end = m_end; a.p.slab = slab;
+        (void)mlo_key;
+        return a;
+    };
+    if (n == 0) {
+        PassHost a = mk(0, +1, 0, real ? 1 : 0, -1);
+        P->pinv.push_back(a); P->pfwd.push_back(a);
+        P->inv.start[0]; P->fwd.start[0];
+    } else {
+        int an = n < 0 ? -n : n;
+        PassHost a = mk(n, +1, -an, 1, 2 * n), b = mk(-n, -1, 1 - an, 1, 2 * n + 1);
+        P->pinv.push_back(a); P->pinv.push_back(b);
+        P->pfwd.push_back(a); P->pfwd.push_back(b);
+        for (RingSet* R : {&P->inv, &P->fwd}) { R->start[n]; R->start[-n]; R->mlo[2 * n]; R->mlo[2 * n + 1]; }
+    }
+}
+
+sht_status make_fft_plans(sht_plan* P) {
+    const int L = P->L, NB = P->NB;
+    size_t ws = 0, w;
+    int n1[1] = {NB};
+    CF(cufftCreate(&P->fft_phi_inv)); CF(cufftSetAutoAllocation(P->fft_phi_inv, 0));
+    { int inembed[1] = {NB}, onembed[1] = {NB};
+      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, P->inv.ntp, 1, onembed, 1, NB, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
+    CF(cufftCreate(&P->fft_phi_fwd)); CF(cufftSetAutoAllocation(P->fft_phi_fwd, 0));
+    { int inembed[1] = {NB}, onembed[1] = {NB};
+      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, P->inv.ntp, 1, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
+    CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
+    { int inembed[1] = {NB};
+      CF(cufftMakePlanMany(P->fft_th1, 1, n1, inembed, 1, NB, inembed, 1, NB, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
+    int n2[1] = {4 * L - 1};
+    CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
+    { int inembed[1] = {4 * L - 1};
+      CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L - 1, inembed, 1, 4 * L - 1, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
+    if (P->kind == 1) {
+        int n3[1] = {2 * P->N - 1};
+        CF(cufftCreate(&P->fft_gamma)); CF(cufftSetAutoAllocation(P->fft_gamma, 0));
+        int emb[1] = {2 * P->N - 1};
+        CF(cufftMakePlanMany(P->fft_gamma, 1, n3, emb, L * NB, 1, emb, L * NB, 1, CUFFT_Z2Z, L * NB, &w)); ws = w > ws ? w : ws;
+    }
+    P->fft_work_bytes = ws + 256;
+    P->have_fft = true;
+    return SHT_OK;
+}
+
+sht_status plan_common(sht_plan* P) {
+    const int L = P->L;
+    P->Lp = (int)rup(L, 128); P->NB = 2 * L - 1;
+    int nmax = 0;
+    for (int n : P->slab_n) nmax = (n < 0 ? -n : n) > nmax ? (n < 0 ? -n : n) : nmax;
+    P->kmin = -(nmax + 2);
+    P->kstride = (int)rup((size_t)P->Lp + SHT_TQ + (size_t)(-P->kmin) + 2, 16);
+    P->krows = P->Lp / SHT_TQ + 1;
+    for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
+    // d-step counts: rings * sum over l of the steps each pass runs
+    for (int dir = 0; dir < 2; ++dir) {
+        double tot = 0; const RingSet& R = dir ? P->fwd : P->inv;
+        for (auto& ph : (dir ? P->pfwd : P->pinv)) {
+            int an = ph.p.n < 0 ? -ph.p.n : ph.p.n;
+            for (int l = an; l < L; ++l) tot += (double)(l - ph.p.m_end + 1);
+        }
+        (dir ? P->dsteps_fwd : P->dsteps_inv) = tot * R.nth;
+    }
+    CS(make_fft_plans(P));
+    layout(P, nullptr);
+    return SHT_OK;
+}
+
+// upload a host vector<double> through a staging copy (synchronous wrt the host buffer)
+sht_status up(const std::vector<double>& h, double* d, cudaStream_t st) {
+    CK(cudaMemcpyAsync(d, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return SHT_OK;
+}
+
+sht_status fill_ringset(sht_plan* P, RingSet& R, cudaStream_t st) {
+    const int L = P->L, Lp = P->Lp;
+    std::vector<double> csc(R.ntp, 1.0), tau(R.ntp, 0.0), sig(R.ntp, 1.0), c2h(R.ntp, 0.0), c2l(R.ntp, 0.0), s2h(R.ntp, 0.0), s2l(R.ntp, 0.0);
+    for (int t = 0; t < R.nth; ++t) {
+        ld c2 = R.c2[t], s2 = R.s2[t], st_ = 2 * c2 * s2;
+        bool north = R.ct[t] >= 0;
+        csc[t] = (double)(1 / st_);
+        tau[t] = north ? (double)(s2 / c2) : (double)(-c2 / s2);
+        sig[t] = north ? 1.0 : -1.0;
+        c2h[t] = (double)c2; c2l[t] = (double)(c2 - (ld)c2h[t]);
+        s2h[t] = (double)s2; s2l[t] = (double)(s2 - (ld)s2h[t]);
+    }
+    CS(up(csc, R.csc, st)); CS(up(tau, R.tau, st)); CS(up(sig, R.sig, st));
+    CS(up(c2h, R.c2hi, st)); CS(up(c2l, R.c2lo, st)); CS(up(s2h, R.s2hi, st)); CS(up(s2l, R.s2lo, st));
+    // start values per second index
+    double* rtab = P->tmp;
+    for (auto& kv : R.start) {
+        int n = kv.first, an = n < 0 ? -n : n;
+        std::vector<double> r(2 * (size_t)Lp, 0.0);
+        for (int l = an + 1; l < L; ++l) {
+            ld v = sqrtl((ld)(2 * l) * (ld)(2 * l - 1) / ((ld)(l + n) * (ld)(l - n)));
+            r[l] = (double)v; r[Lp + l] = (double)(v - (ld)r[l]);
+        }
+        CS(up(r, rtab, st));
+        CK(cudaMemsetAsync(kv.second.val, 0, sizeof(double) * (size_t)Lp * R.ntp, st));
+        CK(cudaMemsetAsync(kv.second.k, 0, (size_t)Lp * R.ntp, st));
+        CK(st_start_values(L, n, R.nth, R.ntp, R.c2hi, R.c2lo, R.s2hi, R.s2lo, rtab, rtab + Lp, kv.second.val, kv.second.k, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    // peak split (R5): pass A serves m >= m_s = round(n cos theta), pass B serves m' >= 1 - m_s
+    for (auto& kv : R.mlo) {
+        int key = kv.first, n = (key - (key & 1)) / 2, passB = key & 1;
+        std::vector<int> h(R.ntp, 1 << 30);
+        for (int t = 0; t < R.nth; ++t) {
+            int ms = (int)llroundl((ld)n * R.ct[t]);
+            h[t] = passB ? 1 - ms : ms;
+        }
+        CK(cudaMemcpyAsync(kv.second, h.data(), sizeof(int) * R.ntp, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return SHT_OK;
+}
+
+sht_status upload_passes(sht_plan* P, cudaStream_t st) {
+    for (int dir = 0; dir < 2; ++dir) {
+        RingSet& R = dir ? P->fwd : P->inv;
+        std::vector<ThetaPass> pm, p;
+        for (auto& ph : (dir ? P->pfwd : P->pinv)) {
+            ThetaPass t = ph.p;
+            t.st_val = R.start[t.n].val; t.st_k = R.start[t.n].k;
+            if (t.n != 0) {
+                int n_slab = t.sgn_out > 0 ? t.n : -t.n;
+                t.m_lo = R.mlo[2 * n_slab + (t.sgn_out > 0 ? 0 : 1)];
+            } else t.m_lo = nullptr;
+            ph.p = t;
+            (ph.mode == 0 ? pm : p).push_back(t);
+        }
+        ThetaPass* dpm = dir ? P->d_fwd_pm : P->d_inv_pm; ThetaPass* dp = dir ? P->d_fwd_p : P->d_inv_p;
+        if (!pm.empty()) CK(cudaMemcpyAsync(dpm, pm.data(), pm.size() * sizeof(ThetaPass), cudaMemcpyHostToDevice, st));
+        if (!p.empty()) CK(cudaMemcpyAsync(dp, p.data(), p.size() * sizeof(ThetaPass), cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+        (dir ? P->n_fwd_pm : P->n_inv_pm) = (int)pm.size();
+        (dir ? P->n_fwd_p : P->n_inv_p) = (int)p.size();
+    }
+    return SHT_OK;
+}
+
+ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
+    const RingSet& R = fwd ? P->fwd : P->inv;
+    ThetaArgs a{};
+    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.NB = P->NB;
+    a.csc = R.csc; a.tau = R.tau; a.sig = R.sig;
+    a.kexp = P->kexp; a.kstride = P->kstride; a.kmin = P->kmin; a.rsq = P->rsq;
+    a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
+    a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
+    return a;
+}
+
+// ---- the stages --------------------------------------------------------------------------------------------------
+// coef: nslab slabs of [L][NB] in *slab order*.  Leaves F[slab][row][ring] complete (all rows, incl. the pole ring).
+sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) {
+    const int L = P->L;
+    stage(P, CAT_STAGE, st);
+    for (auto& ph : P->pinv)
+        CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, coef + (size_t)ph.p.slab * L * P->NB,
+                           P->scale_inv, const_cast<double2*>(ph.p.in), st));
+    CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab * P->nslab, st));
+    stage(P, CAT_HOT, st);
+    CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
+    CK(launch_theta_inverse(theta_args(P, false, false), 1, st));
+    if (P->inv.pole) {
+        for (int s = 0; s < P->nslab; ++s) {
+            int n = P->slab_n[s];
+            int row = (-n) < 0 ? -n + P->NB : -n;
+            CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->inv.ntp + P->inv.nth, st));
+        }
+    }
+    stage(P, CAT_STAGE, st);
+    if (P->reality)
+        for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->inv.ntp, P->inv.nth + (P->inv.pole ? 1 : 0), P->F + P->F_slab * s, st));
+    return SHT_OK;
+}
+// U: [slab][bin][ldu] samples of F_m on the forward ring set (weights not yet applied).  Leaves H complete.
+sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int ldu, cudaStream_t st) {
+    const int L = P->L;
+    stage(P, CAT_STAGE, st);
+    for (auto& ph : P->pfwd) {
+        int n_slab = P->slab_n[ph.p.slab];
+        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.m_lo,
+                           P->fwd.wq, U + U_slab * ph.p.slab, const_cast<double2*>(ph.p.in), st));
+    }
+    CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
+    stage(P, CAT_HOT, st);
+    CK(launch_theta_forward(theta_args(P, true, true), 0, st));
+    CK(launch_theta_forward(theta_args(P, true, false), 1, st));
+    if (P->fwd.pole) {
+        for (int s = 0; s < P->nslab; ++s)
+            CK(st_pole_forward(L, P->Lp, P->slab_n[s], P->NB, ldu, P->fwd.nth, P->fwd.wq, U + U_slab * s, P->H + P->H_slab * s, st));
+    }
+    return SHT_OK;
+}
+
+sht_status check_ready(const sht_plan* P) {
+    if (!P) return SHT_EINVAL;
+    if (!P->ready) { g_err = "plan has no workspace (call sht_plan_set_workspace)"; return SHT_EWORKSPACE; }
+    return SHT_OK;
+}
+
+// MW: F_m(theta_t) on L rings (Fa, [bin][Ltp]) -> U[bin][4L-1] on the MW(2L) rings (in Z)
+sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
+    const int L = P->L, NB = P->NB, T2 = 4 * L - 1;
+    stage(P, CAT_STAGE, st);
+    for (int s = 0; s < P->nslab; ++s) CK(st_mw_extend(L, P->slab_n[s], P->Ltp, NB, P->Fa + P->Fa_slab * s, P->X + P->X_slab * s, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_th1, st)); CF(cufftExecZ2Z(P->fft_th1, P->X, P->X, CUFFT_FORWARD));
+    stage(P, CAT_STAGE, st);
+    for (int s = 0; s < P->nslab; ++s) CK(st_mw_pad_phase(L, NB, T2, P->X + P->X_slab * s, P->Z + P->Z_slab * s, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_th2, st)); CF(cufftExecZ2Z(P->fft_th2, P->Z, P->Z, CUFFT_INVERSE));
+    return SHT_OK;
+}
+
+}  // namespace
+
+void count_launch(int n) { g_launches += n; }
+
+extern "C" {
+
+const char* sht_status_string(sht_status s) {
+    switch (s) {
+        case SHT_OK: return "SHT_OK";
+        case SHT_EINVAL: return "SHT_EINVAL: invalid argument";
+        case SHT_EUNSUPPORTED: return "SHT_EUNSUPPORTED: not implemented in this build";
+        case SHT_EWORKSPACE: return "SHT_EWORKSPACE: workspace missing or too small";
+        case SHT_ECUDA: return "SHT_ECUDA: CUDA runtime failure";
+        case SHT_ECUFFT: return "SHT_ECUFFT: cuFFT failure";
+    }
+    return "unknown status";
+}
+const char* sht_last_error(void) { return g_err.c_str(); }
+const char* sht_version(void) { return "b200sht 0.1 (sm_100a)"; }
+long sht_launch_count(int reset) { long v = g_launches; if (reset) g_launches = 0; return v; }
+
+sht_status sht_plan_s2(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype) {
+    if (!out) return SHT_EINVAL;
+    *out = nullptr;
+    if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || (sampling != SHT_MW && sampling != SHT_HEALPIX)) return SHT_EINVAL;
+    if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
+    if (dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (sampling == SHT_HEALPIX) return SHT_EUNSUPPORTED;
+    sht_plan* P = new sht_plan();
+    P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = nside; P->reality = reality ? 1 : 0;
+    P->nslab = 1; P->slab_n = {-spin};        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
+    rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L);
+    sht_status s = plan_common(P);
+    if (s != SHT_OK) { sht_plan_destroy(P); return s; }
+    *out = P;
+    return SHT_OK;
+}
+sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
+    if (!out) return SHT_EINVAL;
+    *out = nullptr;
+    if (L < 1 || L > 16384 || N < 1 || N > L) return SHT_EINVAL;
+    if (dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    sht_plan* P = new sht_plan();
+    P->kind = 1; P->L = L; P->N = N; P->sampling = SHT_MW;
+    P->nslab = 2 * N - 1;
+    for (int b = 0; b < P->nslab; ++b) P->slab_n.push_back(b < N ? b : b - (2 * N - 1));   // gamma-FFT bin order
+    rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L);
+    sht_status s = plan_common(P);
+    if (s != SHT_OK) { sht_plan_destroy(P); return s; }
+    *out = P;
+    return SHT_OK;
+}
+size_t sht_plan_workspace_bytes(const sht_plan* P) { return P ? P->need_bytes : 0; }
+int sht_plan_ntheta(const sht_plan* P, int forward) {
+    if (!P) return 0;
+    const RingSet& R = forward ? P->fwd : P->inv;
+    return R.nth + (R.pole ? 1 : 0);
+}
+double sht_plan_dsteps(const sht_plan* P, int forward) { return P ? (forward ? P->dsteps_fwd : P->dsteps_inv) : 0.0; }
+
+sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sht_stream stream) {
+    if (!P || !work) return SHT_EINVAL;
+    if (work_bytes < P->need_bytes) { g_err = "workspace too small"; return SHT_EWORKSPACE; }
+    cudaStream_t st = (cudaStream_t)stream;
+    P->work = work; P->work_bytes = work_bytes;
+    layout(P, (char*)work);
+    const int L = P->L, Lp = P->Lp;
+    CK(st_rsq(2 * Lp + 64, P->rsq, st));
+    CK(st_kexp(P->krows, P->kstride, P->kmin, P->kexp, st));
+    std::vector<double> si(Lp, 0.0), sf(Lp, 0.0);
+    for (int l = 0; l < L; ++l) {
+        if (P->kind == 0) {
+            double pref = ((P->spin & 1) ? -1.0 : 1.0) * (double)sqrtl((ld)(2 * l + 1) / (4 * PI_L));     // Eq. 30 / 33
+            si[l] = pref; sf[l] = pref;
+        } else {
+            si[l] = (double)((ld)(2 * l + 1) / (8 * PI_L * PI_L));                                        // Eq. 13
+            sf[l] = (double)(2 * PI_L / (ld)(2 * P->N - 1));                                              // q_Gamma
+        }
+    }
+    CS(up(si, P->scale_inv, st)); CS(up(sf, P->scale_fwd, st));
+    CS(fill_ringset(P, P->inv, st)); CS(fill_ringset(P, P->fwd, st));
+    // forward quadrature weights on MW(2L): q_u = (2 pi/(2L-1)) v_u   (Eq. 41-44 at band-limit 2L)
+    CK(cudaMemsetAsync(P->fwd.wq, 0, sizeof(double) * P->fwd.ntp, st));
+    CK(st_mw_weights(2 * L, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
+    { std::vector<double> ones(P->fwd.ntp, 1.0); CS(up(ones, P->unit_wq, st)); }
+    CS(upload_passes(P, st));
+    for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));
+    if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
+    CK(cudaStreamSynchronize(st));
+    P->ready = true;
+    return SHT_OK;
+}
+
+sht_status sht_plan_destroy(sht_plan* P) {
+    if (!P) return SHT_OK;
+    if (P->have_fft || P->fft_phi_inv) {
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma})
+            if (h) cufftDestroy(h);
+    }
+    for (auto e : P->ev) cudaEventDestroy(e);
+    delete P;
+    return SHT_OK;
+}
+
+sht_status sht_plan_enable_timing(sht_plan* P, int on) {
+    if (!P) return SHT_EINVAL;
+    if (on && P->ev.empty()) {
+        P->ev.resize(96); P->ev_cat.assign(96, 0);
+        for (auto& e : P->ev) CK(cudaEventCreate(&e));
+    }
+    P->timing = on != 0;
+    return SHT_OK;
+}
+sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
+    if (!P || !ms) return SHT_EINVAL;
+    ms[0] = ms[1] = ms[2] = ms[3] = 0.f;
+    if (P->ev_n < 2) return SHT_OK;
+    CK(cudaEventSynchronize(P->ev[P->ev_n - 1]));
+    for (int i = 0; i + 1 < P->ev_n; ++i) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, P->ev[i], P->ev[i + 1]));
+        ms[P->ev_cat[i]] += t; ms[3] += t;
+    }
+    return SHT_OK;
+}
+
+// ---- S^2 ----------------------------------------------------------------------------------------------------------
+sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    P->ev_n = 0;
+    CS(run_theta_inverse(P, (const double2*)flm, st));
+    int nt = sht_plan_ntheta(P, 0);
+    CK(st_rows_reorder(P->L, P->NB, nt, P->inv.ntp, nt, 1, P->F, (double2*)Fm, st));
+    stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!Wm || !flm || P->kind != 0) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    P->ev_n = 0;
+    // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
+    int nt = sht_plan_ntheta(P, 1), T2 = 4 * P->L - 1;
+    CK(st_rows_reorder(P->L, P->NB, nt, nt, T2, 0, (const double2*)Wm, P->Z, st));
+    double* saved = P->fwd.wq;
+    P->fwd.wq = P->unit_wq;
+    sht_status s = run_theta_forward(P, P->Z, P->Z_slab, T2, st);
+    P->fwd.wq = saved;
+    if (s == SHT_OK) {
+        stage(P, CAT_STAGE, st);
+        cudaError_t e = st_finalize_forward(P->L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H, (double2*)flm, st);
+        if (e != cudaSuccess) s = SHT_ECUDA;
+        stage(P, CAT_STAGE, st);
+    }
+    return s;
+}
+
+sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int L = P->L, NB = P->NB;
+    P->ev_n = 0;
+    CS(run_theta_inverse(P, (const double2*)flm, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_phi_inv, st));
+    double2* outc = P->reality ? P->cplx : (double2*)f;
+    CF(cufftExecZ2Z(P->fft_phi_inv, P->F, outc, CUFFT_INVERSE));                      // Eq. 32
+    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_complex_to_real((size_t)L * NB, P->cplx, (double*)f, st)); }
+    stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int L = P->L, NB = P->NB;
+    P->ev_n = 0;
+    const double2* fin = (const double2*)f;
+    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex((size_t)L * NB, (const double*)f, P->cplx, st)); fin = P->cplx; }
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_phi_fwd, st));
+    CF(cufftExecZ2Z(P->fft_phi_fwd, const_cast<double2*>(fin), P->Fa, CUFFT_FORWARD)); // Eq. 31 (weight folded into q_u)
+    CS(mw_upsample(P, st));
+    CS(run_theta_forward(P, P->Z, P->Z_slab, 4 * L - 1, st));
+    stage(P, CAT_STAGE, st);
+    CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H, (double2*)flm, st));
+    stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+
+// ---- SO(3) (Eq. 15-18) ----------------------------------------------------------------------------
+sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int L = P->L, NB = P->NB, N = P->N;
+    const size_t slab = (size_t)L * NB;
+    P->ev_n = 0;
+    stage(P, CAT_STAGE, st);
+    // coefficient slabs from n order (n+N-1) to gamma-FFT bin order
+    for (int b = 0; b < P->nslab; ++b)
+        CK(cudaMemcpyAsync(P->fn + slab * b, (const double2*)flmn + slab * (P->slab_n[b] + N - 1), sizeof(double2) * slab, cudaMemcpyDeviceToDevice, st));
+    CS(run_theta_inverse(P, P->fn, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_phi_inv, st));
+    for (int b = 0; b < P->nslab; ++b) CF(cufftExecZ2Z(P->fft_phi_inv, P->F + P->F_slab * b, (double2*)f + slab * b, CUFFT_INVERSE));
+    CF(cufftSetStream(P->fft_gamma, st));
+    CF(cufftExecZ2Z(P->fft_gamma, (double2*)f, (double2*)f, CUFFT_INVERSE));          // Eq. 17
+    stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int L = P->L, NB = P->NB, N = P->N;
+    const size_t slab = (size_t)L * NB;
+    P->ev_n = 0;
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_gamma, st));
+    CF(cufftExecZ2Z(P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD));   // Eq. 16 (q_Gamma in scale_fwd)
+    CF(cufftSetStream(P->fft_phi_fwd, st));
+    for (int b = 0; b < P->nslab; ++b) CF(cufftExecZ2Z(P->fft_phi_fwd, P->fn + slab * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD));
+    CS(mw_upsample(P, st));
+    CS(run_theta_forward(P, P->Z, P->Z_slab, 4 * L - 1, st));
+    stage(P, CAT_STAGE, st);
+    for (int b = 0; b < P->nslab; ++b)
+        CK(st_finalize_forward(L, P->Lp, P->slab_n[b], 0, P->scale_fwd, P->H + P->H_slab * b, (double2*)flmn + slab * (P->slab_n[b] + N - 1), st));
+    stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+
+// ---- cached convenience calls ------------------------------------------------------------------------------------------
+}  // extern "C"
+
+namespace {
+struct CacheEntry { sht_plan* plan = nullptr; void* work = nullptr; void* d_in = nullptr; void* d_out = nullptr; size_t in_bytes = 0, out_bytes = 0; };
+std::map<std::tuple<int, int, int, int, int, int>, CacheEntry> g_cache;
+std::mutex g_cache_mu;
+
+sht_status cache_get(int kind, int L, int a, int sampling, int nside, int reality, cudaStream_t st, CacheEntry** out) {
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    auto key = std::make_tuple(kind, L, a, sampling, nside, reality);
+    auto it = g_cache.find(key);
+    if (it == g_cache.end()) {
+        CacheEntry e;
+        sht_status s = kind == 0 ? sht_plan_s2(&e.plan, L, a, sampling, nside, reality, SHT_F64) : sht_plan_so3(&e.plan, L, a, SHT_F64);
+        if (s != SHT_OK) return s;
+        size_t nb = sht_plan_workspace_bytes(e.plan);
+        cudaError_t ce = cudaMalloc(&e.work, nb);
+        if (ce != cudaSuccess) { g_err = std::string("cudaMalloc workspace: ") + cudaGetErrorString(ce); sht_plan_destroy(e.plan); return SHT_ECUDA; }
+        s = sht_plan_set_workspace(e.plan, e.work, nb, st);
+        if (s != SHT_OK) { cudaFree(e.work); sht_plan_destroy(e.plan); return s; }
+        it = g_cache.emplace(key, e).first;
+    }
+    *out = &it->second;
+    return SHT_OK;
+}
+size_t s2_map_bytes(int L, int sampling, int nside, int reality) {
+    size_t n = sampling == SHT_MW ? (size_t)L * (2 * L - 1) : (size_t)12 * nside * nside;
+    return n * (reality ? 8 : 16);
+}
+sht_status host_io(CacheEntry* e, size_t in_bytes, size_t out_bytes) {
+    if (e->in_bytes < in_bytes) { if (e->d_in) cudaFree(e->d_in); CK(cudaMalloc(&e->d_in, in_bytes)); e->in_bytes = in_bytes; }
+    if (e->out_bytes < out_bytes) { if (e->d_out) cudaFree(e->d_out); CK(cudaMalloc(&e->d_out, out_bytes)); e->out_bytes = out_bytes; }
+    return SHT_OK;
+}
+}  // namespace
+
+extern "C" {
+
+sht_status s2_forward(int L, int spin, int sampling, int reality, const void* f, void* flm, sht_stream stream) {
+    CacheEntry* e; CS(cache_get(0, L, spin, sampling, sampling == SHT_HEALPIX ? L / 2 : 0, reality, (cudaStream_t)stream, &e));
+    return s2_forward_plan(e->plan, f, flm, stream);
+}
+sht_status s2_inverse(int L, int spin, int sampling, int reality, const void* flm, void* f, sht_stream stream) {
+    CacheEntry* e; CS(cache_get(0, L, spin, sampling, sampling == SHT_HEALPIX ? L / 2 : 0, reality, (cudaStream_t)stream, &e));
+    return s2_inverse_plan(e->plan, flm, f, stream);
+}
+sht_status so3_forward(int L, int N, const void* f, void* flmn, sht_stream stream) {
+    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, (cudaStream_t)stream, &e));
+    return so3_forward_plan(e->plan, f, flmn, stream);
+}
+sht_status so3_inverse(int L, int N, const void* flmn, void* f, sht_stream stream) {
+    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, (cudaStream_t)stream, &e));
+    return so3_inverse_plan(e->plan, flmn, f, stream);
+}
+sht_status sht_cache_clear(void) {
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    for (auto& kv : g_cache) {
+        sht_plan_destroy(kv.second.plan);
+        if (kv.second.work) cudaFree(kv.second.work);
+        if (kv.second.d_in) cudaFree(kv.second.d_in);
+        if (kv.second.d_out) cudaFree(kv.second.d_out);
+    }
+    g_cache.clear();
+    return SHT_OK;
+}
+
+sht_status s2_forward_host(int L, int spin, int sampling, int reality, const void* f_host, void* flm_host, sht_stream stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    int nside = sampling == SHT_HEALPIX ? L / 2 : 0;
+    CacheEntry* e; CS(cache_get(0, L, spin, sampling, nside, reality, st, &e));
+    size_t mb = s2_map_bytes(L, sampling, nside, reality), cb = (size_t)L * (2 * L - 1) * 16;
+    CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
+    CK(cudaMemcpyAsync(e->d_in, f_host, mb, cudaMemcpyHostToDevice, st));
+    CS(s2_forward_plan(e->plan, e->d_in, e->d_out, stream));
+    CK(cudaMemcpyAsync(flm_host, e->d_out, cb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SHT_OK;
+}
+sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const void* flm_host, void* f_host, sht_stream stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    int nside = sampling == SHT_HEALPIX ? L / 2 : 0;
+    CacheEntry* e; CS(cache_get(0, L, spin, sampling, nside, reality, st, &e));
+    size_t mb = s2_map_bytes(L, sampling, nside, reality), cb = (size_t)L * (2 * L - 1) * 16;
+    CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
+    CK(cudaMemcpyAsync(e->d_in, flm_host, cb, cudaMemcpyHostToDevice, st));
+    CS(s2_inverse_plan(e->plan, e->d_in, e->d_out, stream));
+    CK(cudaMemcpyAsync(f_host, e->d_out, mb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SHT_OK;
+}
+sht_status so3_forward_host(int L, int N, const void* f_host, void* flmn_host, sht_stream stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, st, &e));
+    size_t b = (size_t)(2 * N - 1) * L * (2 * L - 1) * 16;
+    CS(host_io(e, b, b));
+    CK(cudaMemcpyAsync(e->d_in, f_host, b, cudaMemcpyHostToDevice, st));
+    CS(so3_forward_plan(e->plan, e->d_in, e->d_out, stream));
+    CK(cudaMemcpyAsync(flmn_host, e->d_out, b, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SHT_OK;
+}
+sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, sht_stream stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, st, &e));
+    size_t b = (size_t)(2 * N - 1) * L * (2 * L - 1) * 16;
+    CS(host_io(e, b, b));
+    CK(cudaMemcpyAsync(e->d_in, flmn_host, b, cudaMemcpyHostToDevice, st));
+    CS(so3_inverse_plan(e->plan, e->d_in, e->d_out, stream));
+    CK(cudaMemcpyAsync(f_host, e->d_out, b, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SHT_OK;
+}
+
+sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream) {
+    if (!tflops || !ms || iters < 1) return SHT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* sink = nullptr;
+    CK(cudaMalloc(&sink, 8));
+    cudaEvent_t a, b;
+    CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+    int blocks, threads, per;
+    CK(launch_fp64_peak(iters / 8 + 1, sink, st, &blocks, &threads, &per));       // warm-up
+    CK(cudaEventRecord(a, st));
+    CK(launch_fp64_peak(iters, sink, st, &blocks, &threads, &per));
+    CK(cudaEventRecord(b, st));
+    CK(cudaEventSynchronize(b));
+    CK(cudaEventElapsedTime(ms, a, b));
+    *tflops = 2.0 * (double)iters * per * (double)blocks * threads / (*ms * 1e-3) / 1e12;
+    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
+    return SHT_OK;
+}
+
+}  // extern "C"

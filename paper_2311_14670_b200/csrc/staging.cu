@@ -1,0 +1,344 @@
+// staging.cu -- everything around the hot kernels that is O(L^2): plan-time tables (ring constants, Eq. 27 start
+// values in windowed mantissa/exponent form, kappa exponents, quadrature weights) and the per-transform staging
+// kernels (layout changes, l-scaling, MW torus extension / upsampling phases, pole ring
+// (Eq. 28-29), Hermitian fills).  All of it is HBM-bound and timed separately from the hot path.
+#include "staging.h"
+
+#include <math.h>
+
+namespace {
+
+__device__ __forceinline__ double sgn_pow(int k) { return (k & 1) ? -1.0 : 1.0; }
+
+// ---- double-double helpers for the start-value product -------------------------------------------------------
+struct dd { double hi, lo; };
+__device__ __forceinline__ dd dd_mul(dd a, dd b) {
+    double p = a.hi * b.hi;
+    double e = fma(a.hi, b.hi, -p);
+    e = fma(a.hi, b.lo, e);
+    e = fma(a.lo, b.hi, e);
+    double s = p + e;
+    return {s, e - (s - p)};
+}
+
+// Eq. 27 for all l at one ring, as the running product
+//   d^l_{l,n} = d^{l-1}_{l-1,n} * ( -sqrt(2l(2l-1)/((l+n)(l-n))) * sin(b/2)cos(b/2) ),   d^{|n|}_{|n|,n} = c2^{2n} or s2^{-2n},
+// carried as double-double mantissa * 2^e so that neither the 1e-35000 magnitudes nor l-fold rounding matter
+// (R7).  Output: windowed value val = d * 2^(SWIN*k), k = floor((TWIN - e)/SWIN) if e < TWIN else 0.
+__global__ void k_start_values(int L, int n, int nth, int ntp, const double* __restrict__ c2hi, const double* __restrict__ c2lo,
+                               const double* __restrict__ s2hi, const double* __restrict__ s2lo, const double* __restrict__ rhi,
+                               const double* __restrict__ rlo, double* __restrict__ st_val, uint8_t* __restrict__ st_k) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x;
+    if (th >= nth) return;
+    const int an = n < 0 ? -n : n;
+    dd c = {c2hi[th], c2lo[th]}, s = {s2hi[th], s2lo[th]};
+    dd q = dd_mul(c, s);
+    q.hi = -q.hi; q.lo = -q.lo;
+    dd base = n >= 0 ? c : s;
+    dd v = {1.0, 0.0};
+    long e = 0;
+    for (int i = 0; i < 2 * an; ++i) {
+        v = dd_mul(v, base);
+        int ex; double f = frexp(v.hi, &ex);
+        v.hi = f; v.lo = ldexp(v.lo, -ex); e += ex;
+    }
+    for (int l = an; l < L; ++l) {
+        if (l > an) {
+            dd r = {rhi[l], rlo[l]};
+            v = dd_mul(dd_mul(v, r), q);
+            int ex; double f = frexp(v.hi, &ex);
+            v.hi = f; v.lo = ldexp(v.lo, -ex); e += ex;
+        }
+        long k = 0;
+        if (e < SHT_TWIN) k = (SHT_TWIN - e) / SHT_SWIN;
+        if (k > 255) { st_val[(size_t)l * ntp + th] = 0.0; st_k[(size_t)l * ntp + th] = 0; continue; }   // < 2^-143000: never matters
+        st_val[(size_t)l * ntp + th] = ldexp(v.hi + v.lo, (int)(e + k * SHT_SWIN));
+        st_k[(size_t)l * ntp + th] = (uint8_t)k;
+    }
+}
+
+// kappa exponents: for a tile with l_top = TQ*(row+1): k_m chosen greedily so that c_m(l_top) = prod a_{j-1}(l_top) 2^{k_j}
+// stays in [1,2).  Entry for m = l_top is 0.
+__global__ void k_kexp(int nrows, int kstride, int kmin, int8_t* __restrict__ kexp) {
+    int row = blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= nrows) return;
+    const int ltop = SHT_TQ * (row + 1);
+    int8_t* kr = kexp + (size_t)row * kstride - kmin;
+    for (int m = kmin; m <= kmin + kstride - 1; ++m) kr[m] = 0;
+    double P = 1.0;
+    for (int m = ltop; m > kmin && m > -ltop; --m) {
+        double x = (double)(ltop - m + 1) * (double)(ltop + m);
+        if (x <= 0.0) break;
+        P *= 2.0 / sqrt(x);
+        int ex; (void)frexp(P, &ex);
+        int kk = -(ex - 1);
+        if (m <= ltop - 1 || true) kr[m] = (int8_t)kk;
+        P = ldexp(P, kk);
+    }
+}
+
+__global__ void k_rsq(int n, double* __restrict__ rsq) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) rsq[k] = k > 0 ? 1.0 / sqrt((double)k) : 0.0;
+}
+
+// MW theta-quadrature weights at band-limit Lq (closed form of Eq. 41-44 with reflection sign +1, R9):
+//   v_u = (zeta_u/(2Lq-1)) sum_{|2j|<=Lq-1} 4 cos(2j theta_u)/(1-4j^2),  theta_u = (2u+1)pi/(2Lq-1);  times qphi.
+__global__ void k_mw_weights(int Lq, double qphi, double* __restrict__ w) {
+    int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= Lq) return;
+    const int T = 2 * Lq - 1, jmax = (Lq - 1) / 2;
+    double acc = 2.0;                               // j = 0 term: 2/(1-0) * 2 * ... /2 handled below
+    acc = 0.0;
+    for (int j = jmax; j >= 1; --j) {               // small terms first
+        long r = ((long)2 * j * (2 * u + 1)) % (2L * T);
+        acc += 4.0 / (1.0 - 4.0 * (double)j * (double)j) * cospi((double)r / (double)T);
+    }
+    acc = 2.0 * acc + 4.0;                          // +-j pairs, plus j = 0
+    double v = acc / (double)T;
+    if (u == Lq - 1) v *= 0.5;
+    w[u] = v * qphi;
+}
+
+// ---- per-transform staging ------------------------------------------------------------------------------------
+// inverse prep: coef[slab_in][L][NB] -> G[m-m_end][Lp][NC] of one pass, scaled by scale[l] and the pass sign.
+__global__ void k_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, const double2* __restrict__ coef,
+                               const double* __restrict__ scale, double2* __restrict__ G) {
+    int l = blockIdx.x * blockDim.x + threadIdx.x;
+    int m = m_end + blockIdx.y;
+    if (l >= Lp) return;
+    const int an = n < 0 ? -n : n, am = m < 0 ? -m : m, NB = 2 * L - 1;
+    for (int c = 0; c < NC; ++c) {
+        double2 v = {0.0, 0.0};
+        if (l < L && l >= an && l >= am && !(c == 1 && m == 0)) {
+            int m_out = (c == 1 || sgn_out < 0) ? -m : m;
+            double s = scale[l];
+            if (c == 1) s *= sgn_pow(m);
+            else if (sgn_out < 0) s *= sgn_pow(m + n);
+            double2 x = coef[(size_t)l * NB + m_out + L - 1];
+            v.x = s * x.x; v.y = s * x.y;
+        }
+        G[((size_t)(m - m_end) * Lp + l) * NC + c] = v;
+    }
+}
+// pole ring theta = pi, inverse (Eq. 29): F_{-n}(pi) = sum_l scale(l) f_{l,-n} (-1)^{l-n}.  One block per slab.
+__global__ void k_pole_inverse(int L, int n, const double2* __restrict__ coef, const double* __restrict__ scale, double2* __restrict__ out) {
+    __shared__ double sre[256], sim[256];
+    const int an = n < 0 ? -n : n, NB = 2 * L - 1;
+    double re = 0, im = 0;
+    for (int l = an + threadIdx.x; l < L; l += blockDim.x) {
+        double2 x = coef[(size_t)l * NB + (-n) + L - 1];
+        double s = scale[l] * sgn_pow(l - n);
+        re += s * x.x; im += s * x.y;
+    }
+    sre[threadIdx.x] = re; sim[threadIdx.x] = im;
+    __syncthreads();
+    for (int k = blockDim.x / 2; k > 0; k >>= 1) {
+        if ((int)threadIdx.x < k) { sre[threadIdx.x] += sre[threadIdx.x + k]; sim[threadIdx.x] += sim[threadIdx.x + k]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out->x = sre[0]; out->y = sim[0]; }
+}
+// real signals: rows m < 0 of F from rows m > 0:  F_{-m}(theta) = conj(F_m(theta))
+__global__ void k_hermitian_rows(int L, int NB, int ntp, int nth, double2* __restrict__ F) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x, m = 1 + blockIdx.y;
+    if (th >= nth || m >= L) return;
+    double2 v = F[(size_t)m * ntp + th];
+    F[(size_t)(NB - m) * ntp + th] = make_double2(v.x, -v.y);
+}
+__global__ void k_real_to_complex(size_t n, const double* __restrict__ in, double2* __restrict__ out) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = make_double2(in[i], 0.0);
+}
+__global__ void k_complex_to_real(size_t n, const double2* __restrict__ in, double* __restrict__ out) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = in[i].x;
+}
+
+// MW forward (ii): extension of F_m(theta_t) to the torus, t = L..2L-2: F_m(theta_t) = (-1)^{m-n} F_m(theta_{2L-2-t})
+__global__ void k_mw_extend(int L, int n, int ldin, int ldout, const double2* __restrict__ Fa, double2* __restrict__ X) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const int T = 2 * L - 1;
+    if (t >= T) return;
+    int m = b < L ? b : b - T;
+    double2 v;
+    if (t < L) v = Fa[(size_t)b * ldin + t];
+    else { v = Fa[(size_t)b * ldin + (2 * L - 2 - t)]; double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
+    X[(size_t)b * ldout + t] = v;
+}
+// MW forward (iii)->(iv): F_{mm'} = (1/T) e^{-i m' pi/T} Y[m' mod T]; Z[m' mod T2] = F_{mm'} e^{+i m' pi/T2}; zero elsewhere.
+__global__ void k_mw_pad_phase(int L, int ldin, int ldout, const double2* __restrict__ Y, double2* __restrict__ Z) {
+    int k2 = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const int T = 2 * L - 1, T2 = 4 * L - 1;
+    if (k2 >= T2) return;
+    int mp = k2 < L ? k2 : (k2 > T2 - L ? k2 - T2 : T2);      // |m'| <= L-1, else none
+    double2 v = {0.0, 0.0};
+    if (mp != T2) {
+        double2 y = Y[(size_t)b * ldin + (mp < 0 ? mp + T : mp)];
+        double s1, c1, s2, c2;
+        sincospi(-(double)mp / (double)T, &s1, &c1);
+        sincospi((double)mp / (double)T2, &s2, &c2);
+        double pr = c1 * c2 - s1 * s2, pi_ = c1 * s2 + s1 * c2;
+        double inv = 1.0 / (double)T;
+        v.x = (y.x * pr - y.y * pi_) * inv; v.y = (y.x * pi_ + y.y * pr) * inv;
+    }
+    Z[(size_t)b * ldout + k2] = v;
+}
+// forward split: U[bin][u] (upsampled F_m(theta'_u), or the ring-FFT output on other samplings) -> weighted operand
+// tiles W[m-m_end][ntp][NC] of one pass; rings not served by the pass at step m get 0 (peak split, R5).
+__global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end,
+                               const int* __restrict__ m_lo, const double* __restrict__ wq, const double2* __restrict__ U,
+                               double2* __restrict__ W) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x;
+    int m = m_end + blockIdx.y;
+    if (th >= ntp) return;
+    for (int c = 0; c < NC; ++c) {
+        double2 v = {0.0, 0.0};
+        bool ok = th < nth && !(c == 1 && m == 0) && (m < L) && (m > -L);
+        if (ok && m_lo) ok = m >= m_lo[th];
+        if (ok) {
+            int m_out = (c == 1 || sgn_out < 0) ? -m : m;
+            double s = wq[th];
+            if (c == 1) s *= sgn_pow(m);
+            else if (sgn_out < 0) s *= sgn_pow(m + n);
+            double2 x = U[(size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + th];
+            v.x = s * x.x; v.y = s * x.y;
+        }
+        W[((size_t)(m - m_end) * ntp + th) * NC + c] = v;
+    }
+}
+// pole ring theta = pi, forward (Eq. 29): H[-n+L-1][l] += (-1)^{l-n} * wq_pole * U_{-n}(pi)
+__global__ void k_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* __restrict__ wq,
+                               const double2* __restrict__ U, double2* __restrict__ H) {
+    int l = blockIdx.x * blockDim.x + threadIdx.x;
+    const int an = n < 0 ? -n : n;
+    if (l >= L || l < an) return;
+    int mo = -n;
+    double2 x = U[(size_t)(mo < 0 ? mo + NBin : mo) * ldin + upole];
+    double s = wq[upole] * sgn_pow(l - n);
+    double2* h = H + (size_t)(mo + L - 1) * Lp + l;
+    h->x += s * x.x; h->y += s * x.y;
+}
+// forward finalize: H[m+L-1][Lp] -> coef[l][m+L-1] = scale(l) * H on the support, 0 elsewhere; real: fill m<0.
+__global__ void k_finalize_forward(int L, int Lp, int n, int real, const double* __restrict__ scale, const double2* __restrict__ H,
+                                   double2* __restrict__ coef) {
+    __shared__ double2 tile[32][33];
+    const int NB = 2 * L - 1, an = n < 0 ? -n : n;
+    int mi0 = blockIdx.x * 32, l0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {      // read H rows (mi), coalesced along l
+        int mi = mi0 + r, l = l0 + threadIdx.x;
+        double2 v = {0.0, 0.0};
+        if (mi < NB && l < L) {
+            int m = mi - (L - 1), am = m < 0 ? -m : m;
+            if (l >= an && l >= am) {
+                if (real && m < 0) { double2 h = H[(size_t)(-m + L - 1) * Lp + l]; double s = scale[l] * sgn_pow(m); v.x = s * h.x; v.y = -s * h.y; }
+                else { double2 h = H[(size_t)mi * Lp + l]; v.x = scale[l] * h.x; v.y = scale[l] * h.y; }
+            }
+        }
+        tile[r][threadIdx.x] = v;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {      // write coef rows (l), coalesced along mi
+        int l = l0 + r, mi = mi0 + threadIdx.x;
+        if (l < L && mi < NB) coef[(size_t)l * NB + mi] = tile[threadIdx.x][r];
+    }
+}
+// generic strided row copy used by the theta-stage entry points: dst[r][c] = src[map(r)][c]
+__global__ void k_rows_bin_to_mi(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* __restrict__ src,
+                                 double2* __restrict__ dst) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y;
+    if (c >= ncol) return;
+    int m = r - (L - 1);
+    int b = m < 0 ? m + NB : m;
+    if (to_mi) dst[(size_t)r * lddst + c] = src[(size_t)b * ldsrc + c];
+    else dst[(size_t)b * lddst + c] = src[(size_t)r * ldsrc + c];
+}
+// SO(3): coefficient slabs are stored in n order (n+N-1); internal slabs are in gamma-FFT bin order (n mod 2N-1)
+__global__ void k_scale_copy(size_t n, double s, const double2* __restrict__ in, double2* __restrict__ out) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = make_double2(s * in[i].x, s * in[i].y);
+}
+
+inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+
+}  // namespace
+
+#define LAUNCHED() do { count_launch(); cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return e_; } while (0)
+
+cudaError_t st_start_values(int L, int n, int nth, int ntp, const double* c2hi, const double* c2lo, const double* s2hi,
+                            const double* s2lo, const double* rhi, const double* rlo, double* st_val, uint8_t* st_k, cudaStream_t st) {
+    if (nth <= 0) return cudaSuccess;
+    k_start_values<<<cdiv(nth, 64), 64, 0, st>>>(L, n, nth, ntp, c2hi, c2lo, s2hi, s2lo, rhi, rlo, st_val, st_k);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t st) {
+    k_kexp<<<cdiv(nrows, 32), 32, 0, st>>>(nrows, kstride, kmin, kexp);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_rsq(int n, double* rsq, cudaStream_t st) {
+    k_rsq<<<cdiv(n, 256), 256, 0, st>>>(n, rsq);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st) {
+    k_mw_weights<<<cdiv(Lq, 128), 128, 0, st>>>(Lq, qphi, w);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, const double2* coef, const double* scale,
+                            double2* G, cudaStream_t st) {
+    dim3 grid(cdiv(Lp, 128), L - m_end);
+    k_prep_inverse<<<grid, 128, 0, st>>>(L, Lp, NC, n, sgn_out, m_end, coef, scale, G);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_pole_inverse(int L, int n, const double2* coef, const double* scale, double2* out, cudaStream_t st) {
+    k_pole_inverse<<<1, 256, 0, st>>>(L, n, coef, scale, out);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st) {
+    if (L < 2) return cudaSuccess;
+    dim3 grid(cdiv(nth, 128), L - 1);
+    k_hermitian_rows<<<grid, 128, 0, st>>>(L, NB, ntp, nth, F);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStream_t st) {
+    k_real_to_complex<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st) {
+    k_complex_to_real<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st) {
+    dim3 grid(cdiv(2 * L - 1, 128), 2 * L - 1);
+    k_mw_extend<<<grid, 128, 0, st>>>(L, n, ldin, ldout, Fa, X);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st) {
+    dim3 grid(cdiv(4 * L - 1, 128), 2 * L - 1);
+    k_mw_pad_phase<<<grid, 128, 0, st>>>(L, ldin, ldout, Y, Z);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, const int* m_lo,
+                            const double* wq, const double2* U, double2* W, cudaStream_t st) {
+    dim3 grid(cdiv(ntp, 128), L - m_end);
+    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, m_lo, wq, U, W);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
+                            cudaStream_t st) {
+    k_pole_forward<<<cdiv(L, 128), 128, 0, st>>>(L, Lp, n, NBin, ldin, upole, wq, U, H);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st) {
+    dim3 grid(cdiv(2 * L - 1, 32), cdiv(L, 32)), block(32, 8);
+    k_finalize_forward<<<grid, block, 0, st>>>(L, Lp, n, real, scale, H, coef);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st) {
+    dim3 grid(cdiv(ncol, 128), NB);
+    k_rows_bin_to_mi<<<grid, 128, 0, st>>>(L, NB, ncol, ldsrc, lddst, to_mi, src, dst);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st) {
+    k_scale_copy<<<cdiv(n, 256), 256, 0, st>>>(n, s, in, out);
+    LAUNCHED(); return cudaSuccess;
+}

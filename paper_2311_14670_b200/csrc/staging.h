@@ -1,0 +1,24 @@
+// staging.h -- launchers of the table-setup and staging kernels (staging.cu).  Internal.
+#pragma once
+#include "internal.h"
+
+cudaError_t st_start_values(int L, int n, int nth, int ntp, const double* c2hi, const double* c2lo, const double* s2hi,
+                            const double* s2lo, const double* rhi, const double* rlo, double* st_val, uint8_t* st_k, cudaStream_t st);
+cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t st);
+cudaError_t st_rsq(int n, double* rsq, cudaStream_t st);
+cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st);
+cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, const double2* coef, const double* scale,
+                            double2* G, cudaStream_t st);
+cudaError_t st_pole_inverse(int L, int n, const double2* coef, const double* scale, double2* out, cudaStream_t st);
+cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st);
+cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStream_t st);
+cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st);
+cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st);
+cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
+cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, const int* m_lo,
+                            const double* wq, const double2* U, double2* W, cudaStream_t st);
+cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
+                            cudaStream_t st);
+cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st);
+cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st);
+cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st);
