@@ -1,0 +1,163 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on seeded inputs.
+
+Tolerance: fp64 max|delta| / max|ref| <= 1e-11 (BASELINE.json north_star) -- asserted here at 1e-12 for L <= 256,
+which is still > 50x the errors observed (~3.5e-16 L)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2311_14670_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+@pytest.fixture(scope="module")
+def api():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_14670_b200 import api as A
+    return A
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# sizes span several kernel tiles (128 degrees / 32 rings inverse; 32 degrees / 128 rings forward) plus ragged tails
+@pytest.mark.parametrize("L,spin", [(1, 0), (2, 0), (3, 1), (8, 0), (33, 0), (64, 0), (64, 2), (48, -3), (130, 1), (131, -2), (200, 0), (257, 2)])
+def test_s2_mw_inverse_forward_vs_oracle(api, orc, L, spin):
+    flm = synth.random_flm(L, spin, seed=L + 7 * spin)
+    P = api.Plan(L, spin)
+    f = P.inverse(dev(flm)).cpu().numpy()
+    f_ref = orc.s2_inverse(L, spin, orc.MW, flm)
+    assert rel(f, f_ref) < TOL
+    # forward of the oracle's map, against the oracle's forward AND against the generating coefficients (pin 6)
+    back = P.forward(dev(f_ref)).cpu().numpy()
+    assert rel(back, orc.s2_forward(L, spin, orc.MW, f_ref)) < TOL
+    assert rel(back, flm) < TOL
+    # coefficients outside the support are written as exact zeros
+    el = np.arange(L)[:, None]
+    m = np.arange(-(L - 1), L)[None, :]
+    assert np.all(back[(np.abs(m) > el) | (el < abs(spin))] == 0)
+
+
+def test_config1_L64_spin0_round_trip_and_forward(api, orc):
+    """BASELINE.json configs[0]: spin-0 complex, MW L=64, flm iid complex N(0,1), seed 0."""
+    L = 64
+    flm = synth.random_flm(L, 0, seed=0)
+    d = dev(flm)
+    f = api.s2_inverse(d, L, 0)
+    back = api.s2_forward(f, L, 0)
+    assert rel(f.cpu().numpy(), orc.s2_inverse(L, 0, orc.MW, flm)) < TOL
+    assert rel(back.cpu().numpy(), flm) < TOL
+    # Table 1 of the paper: 1.2e-15 at L=64 (norm unspecified): same order of magnitude or better
+    tab = {}
+    for line in open(os.path.join(HERE, "golden", "paper_tables_roundtrip.txt")):
+        if line.startswith("sht"):
+            _, l_, e_ = line.split(); tab[int(l_)] = float(e_)
+    sup = flm != 0
+    assert np.abs(back.cpu().numpy() - flm)[sup].mean() < 10 * tab[64]
+
+
+def test_forward_of_non_bandlimited_map_matches_oracle(api, orc):
+    """The forward transform is defined by the algorithm (upsampling + quadrature) for any input, not just
+    band-limited maps: check parity on white noise."""
+    L, spin = 40, 1
+    f = synth.random_map((L, 2 * L - 1), seed=9)
+    P = api.Plan(L, spin)
+    assert rel(P.forward(dev(f)).cpu().numpy(), orc.s2_forward(L, spin, orc.MW, f)) < TOL
+
+
+def test_theta_stage_entry_points(api, orc):
+    """Hot path alone: F_m(theta) of Eq. 33 against the oracle's columns; Eq. 30 on weighted rows."""
+    L, spin = 96, 2
+    flm = synth.random_flm(L, spin, seed=4)
+    P = api.Plan(L, spin)
+    F = P.theta_inverse(dev(flm)).cpu().numpy()
+    ms = np.arange(-(L - 1), L)
+    assert rel(F, orc.s2_theta_inverse_columns(L, spin, orc.MW, flm, ms)) < TOL
+    # forward theta step on the oracle's own upsampled + weighted rows would need oracle internals; instead use
+    # linearity: rows W = q_u * F_m(theta'_u) synthesised by the oracle's theta step on the MW(2L) rings is not
+    # exposed, so check adjoint consistency <theta_fwd(W), a> = <W, theta_inv-like(a)> via random probes:
+    nq = P.ntheta(True)
+    rng = np.random.default_rng(0)
+    W = (rng.standard_normal((2 * L - 1, nq)) + 1j * rng.standard_normal((2 * L - 1, nq)))
+    out = P.theta_forward(dev(W)).cpu().numpy()
+    # reference by the oracle's d-functions: out[l, m] = pref(l) * sum_u W[m, u] d^l_{m,-s}(theta'_u)
+    tab = orc.ring_table(orc.MW_QUAD, L)
+    el = np.arange(L)
+    pref = (-1.0) ** spin * np.sqrt((2 * el + 1) / (4 * np.pi))
+    for m in (-(L - 1), -5, 0, 2, 31, L - 1):
+        acc = np.zeros(L, complex)
+        for u in range(nq):
+            if u == nq - 1:
+                d = np.array([(-1.0) ** (l + m) if m == spin and l >= abs(spin) else 0.0 for l in range(L)])
+            else:
+                c2 = np.sqrt((1 + tab["cos_theta"][u]) / 2); s2 = np.sqrt((1 - tab["cos_theta"][u]) / 2)
+                d = np.asarray(orc.d_lrec(L, m, -spin, cos_half=c2, sin_half=s2), float)
+            acc += W[m + L - 1, u] * d
+        want = pref * acc
+        want[el < max(abs(m), abs(spin))] = 0
+        assert np.abs(out[:, m + L - 1] - want).max() < 1e-11 * np.abs(want).max(), m
+
+
+def test_real_signals(api, orc):
+    for L in (16, 65, 140):
+        flm = synth.random_flm(L, 0, seed=L, real=True)
+        P = api.Plan(L, 0, reality=True)
+        f = P.inverse(dev(flm)).cpu().numpy()
+        f_ref = orc.s2_inverse(L, 0, orc.MW, flm)
+        assert np.abs(f_ref.imag).max() < 1e-13
+        assert rel(f, f_ref.real) < TOL
+        back = P.forward(dev(f_ref.real.copy())).cpu().numpy()
+        assert rel(back, flm) < TOL
+        # input m<0 half is ignored
+        junk = flm.copy(); junk[:, :L - 1] = 99.0
+        assert np.array_equal(P.inverse(dev(junk)).cpu().numpy(), f)
+
+
+@pytest.mark.parametrize("L,N", [(4, 1), (8, 3), (16, 5), (33, 8), (40, 40)])
+def test_so3_vs_oracle(api, orc, L, N):
+    c = synth.random_flmn(L, N, seed=3 + L)
+    P = api.Plan(L, N=N)
+    f = P.inverse(dev(c)).cpu().numpy()
+    f_ref = orc.so3_inverse(L, N, c)
+    assert rel(f, f_ref) < TOL
+    back = P.forward(dev(f_ref)).cpu().numpy()
+    assert rel(back, c) < TOL
+    assert rel(back, orc.so3_forward(L, N, f_ref)) < TOL
+
+
+def test_host_buffer_calls_match_device_calls(api):
+    L, spin = 50, 1
+    flm = synth.random_flm(L, spin, seed=5)
+    f_dev = api.s2_inverse(dev(flm), L, spin).cpu().numpy()
+    f_host = api.s2_inverse_host(flm, L, spin)
+    assert np.abs(f_host - f_dev).max() < 1e-13 * np.abs(f_dev).max()      # atomics order may differ in the last bits
+    back = api.s2_forward_host(f_host, L, spin)
+    assert rel(back, flm) < TOL
+    c = synth.random_flmn(12, 3, seed=1)
+    assert rel(api.so3_forward_host(api.so3_inverse_host(c, 12, 3), 12, 3), c) < TOL
+
+
+def test_inputs_are_not_modified_and_errors_are_loud(api):
+    L = 20
+    flm = synth.random_flm(L, 0, seed=1)
+    d = dev(flm)
+    keep = d.clone()
+    f = api.s2_inverse(d, L, 0)
+    keepf = f.clone()
+    api.s2_forward(f, L, 0)
+    torch.cuda.synchronize()
+    assert torch.equal(d, keep) and torch.equal(f, keepf)
+    with pytest.raises(ValueError):
+        api.s2_inverse(d[:, :-1].contiguous(), L, 0)
+    with pytest.raises(Exception):
+        api.Plan(8, 9)
