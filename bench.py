@@ -138,7 +138,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sweep", action="store_true", help="also time the other configs (MW vs L, SO(3)) into the JSON line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--L", type=int, default=None, help="profiling only: override the band-limit of the workload")
+    ap.add_argument("--spin", type=int, default=None, help="profiling only: override the spin of the workload")
     args = ap.parse_args()
+    if args.L is not None:
+        WORKLOAD["L"] = args.L
+    if args.spin is not None:
+        WORKLOAD["spin"] = args.spin
     if args.impl == "reference":
         return run_reference(args)
 
@@ -247,7 +253,7 @@ def main():
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                "data": "synthetic",
-               "config": {"workload": f"BASELINE.json configs[1]: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
+               "config": {"workload": f"{'BASELINE.json configs[1]' if (L, spin) == (1024, 2) else 'override'}: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
                                       "flm ~ N(0, 1/(l(l+1))) l>=2, inverse + forward per step",
                           "l2": "flushed between timed iterations (256 MiB memset, untimed)", "parallelism": f"independent x{world}"},
                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

@@ -338,6 +338,9 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     a.kexp = P->kexp; a.kstride = P->kstride; a.kmin = P->kmin; a.rsq = P->rsq;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
+    a.all_n_zero = 1;
+    for (auto& ph : (fwd ? P->pfwd : P->pinv))
+        if ((ph.mode == 0) == pm && ph.p.n != 0) a.all_n_zero = 0;
     return a;
 }
 

@@ -7,15 +7,16 @@
 //       lambda'_m(theta) = lambda_m(theta) 2^{-k_m},     g'_m(l) = (l-m)(l+m+1) 2^{-2-k_m-k_{m+1}}.
 //   Both coefficients are separable (theta-only x l-only), so one d-step is 1 DMUL + 1 DFMA; the (l,m)-only factor
 //   c_m(l) is folded into the harmonic coefficients (inverse) or into the reduced sums (forward).
-//   Renormalisation (Sec. 3.4): the iterate pair carries a power-of-two scale 2^{-560 k}; while
-//   k > 0 the stored value stays below 2^-140, so its (wrong-scale) contribution is below fp64 resolution and no
-//   masking is needed; a check every 8 steps moves the window (k -> k-1) once the stored value exceeds 2^-300.
+//   Renormalisation (Sec. 3.4): the iterate pair carries a power-of-two scale 2^{-480 k}; while
+//   k > 0 the stored value stays below 2^-340 (it can grow by at most 2^20 per step between checks), so its
+//   (wrong-scale) contribution, even times c_m(l) <= 2^280, is below fp64 resolution and no masking is needed;
+//   a check every 8 steps moves the window (k -> k-1) once the stored value exceeds 2^-500.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define SHT_TWIN (-300)   // window top: stored start values with k > 0 are <= 2^TWIN
-#define SHT_SWIN 560      // window stride: true value = stored * 2^(-SWIN*k)
+#define SHT_TWIN (-500)   // window top: stored start values with k > 0 are <= 2^TWIN
+#define SHT_SWIN 480      // window stride: true value = stored * 2^(-SWIN*k)
 #define SHT_JCHK 8        // steps between window checks
 #define SHT_TQ 16         // quantum of the kappa tables: one row per l_top multiple of TQ
 
@@ -43,6 +44,7 @@ struct ThetaArgs {
     const double* rsq;     // [2*Lp+64] 1/sqrt(k)
     const ThetaPass* passes;
     int npass;
+    int all_n_zero;        // every pass of this launch has n == 0 (lets the kernel use lambda' = -m cot(theta) S_m)
 };
 
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)

@@ -51,7 +51,7 @@ __global__ void k_start_values(int L, int n, int nth, int ntp, const double* __r
         }
         long k = 0;
         if (e < SHT_TWIN) k = (SHT_TWIN - e) / SHT_SWIN;
-        if (k > 255) { st_val[(size_t)l * ntp + th] = 0.0; st_k[(size_t)l * ntp + th] = 0; continue; }   // < 2^-143000: never matters
+        if (k > 254) { st_val[(size_t)l * ntp + th] = 0.0; st_k[(size_t)l * ntp + th] = 0; continue; }   // < 2^-143000: never matters
         st_val[(size_t)l * ntp + th] = ldexp(v.hi + v.lo, (int)(e + k * SHT_SWIN));
         st_k[(size_t)l * ntp + th] = (uint8_t)k;
     }

@@ -2,13 +2,15 @@
 // contraction of Eq. 30 (forward, sum over rings) and Eq. 33 (inverse, sum over l) -- "interleaving recursion and
 // computation", Sec. 4.4.  d-values live only in registers; nothing O(L^3) touches memory.
 //
-// Thread mapping:
-//   inverse: lane <-> ring theta, registers <-> RL consecutive degrees l, warps <-> further l-chunks.
-//            sum_l is an in-thread FMA chain + a shared-memory reduction across warps + RED.ADD.F64 across l-tiles.
-//   forward: lane <-> degree l, registers <-> RT consecutive rings, warps <-> further ring chunks.
-//            sum_theta is an in-thread FMA chain + a shared-memory reduction across warps + RED.ADD.F64 across ring tiles.
-// Per-step operand tiles (harmonic coefficients / weighted F_m) arrive through 1-D TMA bulk copies
-// (cp.async.bulk + mbarrier) into a 4-stage shared-memory ring.
+// Thread mapping; every thread carries an RL x RT register tile of (l, ring) items:
+//   inverse: lane <-> ring (theta0 + lane + 32 i), registers <-> RL consecutive degrees, warps <-> further l-chunks.
+//            sum_l = in-thread FMA chain + shared-memory reduction over warps + RED.ADD.F64 over l-tiles.
+//   forward: lane <-> degree (l0 + lane + 32 r), registers <-> RT consecutive rings, warps <-> further ring chunks.
+//            sum_theta = in-thread FMA chain + shared-memory reduction over warps + RED.ADD.F64 over ring tiles.
+// One d-step is 1 DMUL + 1 DFMA (internal.h); the projection is 2 (one order) or 4 (both +-m) DFMA.  Operands that
+// are uniform across a warp (coefficients, weighted F_m, lambda', g') are read as shared-memory broadcasts, one
+// read serving RT (inverse) or RL (forward) items.  Per-step operand tiles arrive through 1-D TMA bulk copies
+// (cp.async.bulk + mbarrier) into a 4-stage ring; one __syncthreads per recursion step.
 #include "internal.h"
 
 #include <cuda_runtime.h>
@@ -43,38 +45,78 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ double pow2i(int e) { return __hiloint2double((1023 + e) << 20, 0); }
 __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7fffffff; }
 
-// window maintenance (Sec. 3.4 renormalisation; see internal.h): stored value above 2^TWIN with k > 0 -> shift window.
-// A stored value above 2^500 can only be an iterate that left its stable range (R5) on a ring that is
-// no longer served: it is zeroed so that it can never overflow.
 #define HI_TWIN ((1023 + SHT_TWIN) << 20)
 #define HI_DEAD ((1023 + 500) << 20)
-__device__ __forceinline__ void window_check(double& cur, double& prev, int& k) {
-    int h = hi_abs(cur);
-    if (k > 0 && h > HI_TWIN) {
-        const double s = pow2i(-SHT_SWIN);
-        cur *= s; prev *= s; k -= 1;
-    } else if (h > HI_DEAD) {
-        cur = 0.0; prev = 0.0;
-    }
-}
 
 constexpr int NST = 4;   // stages of the operand ring
+
+// Window counters k (internal.h) of the NI items of a thread, one byte each.
+template <int NI>
+struct KPack {
+    uint32_t w[(NI + 3) / 4];
+    __device__ __forceinline__ void fill(uint32_t v) {
+#pragma unroll
+        for (int i = 0; i < (NI + 3) / 4; ++i) w[i] = v;
+    }
+    __device__ __forceinline__ void set(int idx, uint32_t k) {
+        const int sh = (idx & 3) * 8;
+        w[idx >> 2] = (w[idx >> 2] & ~(0xffu << sh)) | (k << sh);
+    }
+    __device__ __forceinline__ uint32_t get(int idx) const { return (w[idx >> 2] >> ((idx & 3) * 8)) & 0xffu; }
+    __device__ __forceinline__ void dec(int idx) { w[idx >> 2] -= 1u << ((idx & 3) * 8); }
+    __device__ __forceinline__ bool any_nonzero() const {
+        uint32_t o = 0;
+#pragma unroll
+        for (int i = 0; i < (NI + 3) / 4; ++i) o |= w[i];
+        return o != 0;
+    }
+    __device__ __forceinline__ bool any_zero_byte() const {
+        bool z = false;
+#pragma unroll
+        for (int i = 0; i < (NI + 3) / 4; ++i) z = z || (((w[i] - 0x01010101u) & ~w[i] & 0x80808080u) != 0);
+        return z;
+    }
+};
+// Window maintenance (Sec. 3.4 renormalisation; internal.h): a stored value above 2^TWIN with k > 0 shifts its window.
+template <int NI>
+__device__ __forceinline__ void window_check(double (&cur)[NI], double (&prev)[NI], KPack<NI>& kp) {
+    const double s = pow2i(-SHT_SWIN);
+#pragma unroll
+    for (int q = 0; q < NI; ++q) {
+        if (hi_abs(cur[q]) > HI_TWIN && kp.get(q) != 0u && kp.get(q) != 0xffu) {
+            cur[q] *= s; prev[q] *= s; kp.dec(q);
+        }
+    }
+}
+// On rings a pass no longer serves (m < m_lo, R5) the iterate leaves its stable range; it is zeroed before it
+// can overflow.  Legitimate stored values never exceed ~2.
+template <int NI>
+__device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]) {
+#pragma unroll
+    for (int q = 0; q < NI; ++q)
+        if (hi_abs(cur[q]) > HI_DEAD) { cur[q] = 0.0; prev[q] = 0.0; }
+}
 
 // =============================================================================================================
 // inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * d^l_{m,n}(theta)
 // =============================================================================================================
 template <int RL, int RT, int NW, int NC>
-__global__ void __launch_bounds__(NW * 32) theta_inverse_kernel(const ThetaArgs A) {
-    constexpr int TL = NW * RL;      // degrees per block
-    constexpr int NTH = 32 * RT;     // rings per block
-    constexpr int SCW = (NC == 2) ? 6 : 4;
+struct InvSmem {
+    static constexpr int TL = NW * RL, NTH = 32 * RT, SCW = (NC == 2) ? 6 : 4;
+    double2 ctile[NST][TL * NC];        // raw coefficient tiles (TMA ring)
+    double sc[2][TL][SCW];              // per step: coefficients * c_m(l), then g'_m(l)
+    double red[2][NW][2 * NC][NTH];     // per-warp partial sums
+    double stv[TL][NTH];                // start values of the block's (l, ring) tile
+    uint8_t stk[TL][NTH];
+    uint64_t bar[NST + 1];
+};
+
+template <int RL, int RT, int NW, int NC, bool SPIN0>
+__global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kernel(const ThetaArgs A) {
+    using S = InvSmem<RL, RT, NW, NC>;
+    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2* ctile = reinterpret_cast<double2*>(smem_raw);                         // [NST][TL*NC]
-    double* sc = reinterpret_cast<double*>(ctile + NST * TL * NC);                 // [NW][RL][SCW]
-    double* red = sc + NW * RL * SCW;                                              // [2][NW][2*NC][NTH]
-    double* stv = red + 2 * NW * 2 * NC * NTH;                                     // [TL][NTH]
-    uint8_t* stk = reinterpret_cast<uint8_t*>(stv + TL * NTH);                     // [TL][NTH]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(stk + TL * NTH);                   // [NST + 1]
+    S& sm = *reinterpret_cast<S*>(smem_raw);
 
     const ThetaPass P = A.passes[blockIdx.y];
     const int ntt = A.ntp / NTH, nlt = A.Lp / TL;
@@ -85,172 +127,204 @@ __global__ void __launch_bounds__(NW * 32) theta_inverse_kernel(const ThetaArgs 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end;
     const int la = l0 + w * RL;                       // first degree of this warp
-    const uint32_t tile_bytes = TL * NC * sizeof(double2);
+    constexpr uint32_t tile_bytes = TL * NC * sizeof(double2);
 
-    // ---- prologue: barriers, start-value tile, first operand tiles
     if (tid == 0) {
-        for (int i = 0; i <= NST; ++i) mbar_init(&bar[i], 1);
+        for (int i = 0; i <= NST; ++i) mbar_init(&sm.bar[i], 1);
         mbar_fence_init();
     }
     __syncthreads();
     if (tid == 0) {
-        mbar_expect_tx(&bar[NST], TL * NTH * 9);
+        mbar_expect_tx(&sm.bar[NST], TL * NTH * 9);
         for (int r = 0; r < TL; ++r) {
-            bulk_g2s(stv + r * NTH, P.st_val + (size_t)(l0 + r) * A.ntp + th0, NTH * 8, &bar[NST]);
-            bulk_g2s(stk + r * NTH, P.st_k + (size_t)(l0 + r) * A.ntp + th0, NTH, &bar[NST]);
+            bulk_g2s(&sm.stv[r][0], P.st_val + (size_t)(l0 + r) * A.ntp + th0, NTH * 8, &sm.bar[NST]);
+            bulk_g2s(&sm.stk[r][0], P.st_k + (size_t)(l0 + r) * A.ntp + th0, NTH, &sm.bar[NST]);
         }
         for (int it = 0; it < NST; ++it) {
             int m = mtop - it;
             if (m >= m_end) {
-                mbar_expect_tx(&bar[it], tile_bytes);
-                bulk_g2s(ctile + it * TL * NC, P.in + ((size_t)(m - m_end) * A.Lp + l0) * NC, tile_bytes, &bar[it]);
+                mbar_expect_tx(&sm.bar[it], tile_bytes);
+                bulk_g2s(&sm.ctile[it][0], P.in + ((size_t)(m - m_end) * A.Lp + l0) * NC, tile_bytes, &sm.bar[it]);
             }
         }
     }
-    // per-ring constants of this thread's RT rings
-    double csc[RT], tau[RT], sg[RT];
+    // ---- ring constants: lambda'_m = S_m * ((n - sig m) csc + m tau)   [= S_m * m * (tau - sig csc) when n = 0]
+    double rc0[RT], rc1[RT];
+    bool north[RT];
 #pragma unroll
     for (int i = 0; i < RT; ++i) {
-        int th = th0 + lane + 32 * i;
-        csc[i] = A.csc[th]; tau[i] = A.tau[th]; sg[i] = A.sig[th];
+        const int th = th0 + lane + 32 * i;
+        const double csc = A.csc[th], tau = A.tau[th], sg = A.sig[th];
+        north[i] = sg > 0.0;
+        if (SPIN0) { rc0[i] = tau - sg * csc; rc1[i] = 0.0; }
+        else { rc0[i] = csc; rc1[i] = tau; }
     }
-    double cur[RL][RT], prev[RL][RT];
-    int kk[RL][RT];
+    double cur[NI], prev[NI];
+    KPack<NI> kp;
+    kp.fill(0xffffffffu);                             // 0xff = not started yet
 #pragma unroll
-    for (int j = 0; j < RL; ++j)
-#pragma unroll
-        for (int i = 0; i < RT; ++i) { cur[j][i] = 0.0; prev[j][i] = 0.0; kk[j][i] = 0; }
-    // helper-lane state: lane j < RL owns degree la + j
-    const int lj = la + lane;
-    double cfac = 1.0;
-    // kappa exponents of this warp's tile (l_top = la + RL rounded up to a multiple of TQ)
+    for (int q = 0; q < NI; ++q) { cur[q] = 0.0; prev[q] = 0.0; }
+    bool wact = false;                                // any item of this warp with k == 0 (contributes)
+    // kappa exponents of this warp's l-chunk (l_top = la + RL rounded up to a multiple of TQ)
     const int8_t* krow = A.kexp + (size_t)((la + RL + SHT_TQ - 1) / SHT_TQ - 1) * A.kstride - A.kmin;
     const double fn = (double)P.n;
-    mbar_wait(&bar[NST], 0);
 
-    for (int m = mtop; m >= m_end; --m) {
-        const int it = mtop - m, slot = it % NST;
+    // ---- helper threads: one per degree of the block, they prepare sc[] one step ahead
+    constexpr int HB = (NW * 32 >= 2 * TL) ? NW * 32 - TL : 0;      // last TL threads
+    const bool is_helper = tid >= HB && tid < HB + TL;
+    const int hl = tid - HB, lh = l0 + hl;
+    const int8_t* krow_h = A.kexp + (size_t)((l0 + (hl / RL) * RL + RL + SHT_TQ - 1) / SHT_TQ - 1) * A.kstride - A.kmin;
+    double cfac = 1.0;
+    auto helper = [&](int m, int it) {                // prepares sc[it & 1] for recursion step m
+        const int slot = it % NST;
+        mbar_wait(&sm.bar[slot], (it / NST) & 1);
+        if (lh > m && lh >= an) cfac *= pow2i(krow_h[m + 1] + 1) * A.rsq[lh - m] * A.rsq[lh + m + 1];   // c_{m} from c_{m+1}
+        const double2* raw = &sm.ctile[slot][hl * NC];
+        double* s = &sm.sc[it & 1][hl][0];
+        const double2 c0 = raw[0];
+        s[0] = c0.x * cfac; s[1] = c0.y * cfac;
+        if (NC == 2) { const double2 c1 = raw[1]; s[2] = c1.x * cfac; s[3] = c1.y * cfac; }
+        s[2 * NC] = (double)(lh - m) * (double)(lh + m + 1) * pow2i(-2 - krow_h[m] - krow_h[m + 1]);
+    };
+    if (is_helper) helper(mtop, 0);
+    mbar_wait(&sm.bar[NST], 0);
+    __syncthreads();
+
+    // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step,
+    // so the iterates never move between registers)
+    auto step = [&](const int m, double (&ca)[NI], double (&cb)[NI]) {
+        const int it = mtop - m;
         const bool warp_on = (m <= la + RL - 1) && (la < A.L);
         if (warp_on) {
-            // ---- activation of the degree l == m (warp-uniform)
-            if (m >= la) {
+            if (m >= la) {                            // ramp: the degree l == m starts (warp-uniform)
 #pragma unroll
                 for (int j = 0; j < RL; ++j) {
                     if (m == la + j) {
 #pragma unroll
                         for (int i = 0; i < RT; ++i) {
-                            cur[j][i] = stv[(w * RL + j) * NTH + lane + 32 * i];
-                            kk[j][i] = stk[(w * RL + j) * NTH + lane + 32 * i];
-                            prev[j][i] = 0.0;
+                            ca[j * RT + i] = sm.stv[w * RL + j][lane + 32 * i];
+                            cb[j * RT + i] = 0.0;
+                            kp.set(j * RT + i, sm.stk[w * RL + j][lane + 32 * i]);
                         }
                     }
                 }
+                wact = true;                          // re-evaluated at the next window check
             }
-            const int km = krow[m], km1 = krow[m + 1];
-            mbar_wait(&bar[slot], (it / NST) & 1);
-            // ---- helper lanes: scale this step's coefficients by c_m(l), form g'_m(l)
-            if (lane < RL) {
-                const double2* raw = ctile + slot * TL * NC + (w * RL + lane) * NC;
-                double* s = sc + (w * RL + lane) * SCW;
-                double2 c0 = raw[0];
-                s[0] = c0.x * cfac; s[1] = c0.y * cfac;
-                if (NC == 2) { double2 c1 = raw[1]; s[2] = c1.x * cfac; s[3] = c1.y * cfac; }
-                s[2 * NC] = (double)(lj - m) * (double)(lj + m + 1) * pow2i(-2 - km - km1);
-                if (lj >= m && lj >= an && m > m_end) cfac *= pow2i(km + 1) * A.rsq[lj - m + 1] * A.rsq[lj + m];
-            }
-            __syncwarp();
-            // ---- lambda'_m for this thread's rings
+            const int km = krow[m];
             double lam[RT];
-            const double sm = pow2i(-km), fm = (double)m;
+            {
+                const double smul = pow2i(-km), fm = (double)m;
+                if (SPIN0) {
+                    const double v = fm * smul;
 #pragma unroll
-            for (int i = 0; i < RT; ++i) lam[i] = sm * fma(fn - sg[i] * fm, csc[i], fm * tau[i]);
+                    for (int i = 0; i < RT; ++i) lam[i] = v * rc0[i];
+                } else {
+                    const double un = (fn - fm) * smul, us = (fn + fm) * smul, v = fm * smul;
+#pragma unroll
+                    for (int i = 0; i < RT; ++i) lam[i] = fma(north[i] ? un : us, rc0[i], v * rc1[i]);
+                }
+            }
             double acc[RT][2 * NC];
 #pragma unroll
             for (int i = 0; i < RT; ++i)
 #pragma unroll
                 for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
-            // ---- project (Eq. 33) and advance (Eq. 25) every (l, ring) item
+            const double* scw = &sm.sc[it & 1][w * RL][0];
+            if (wact) {
 #pragma unroll
-            for (int j = 0; j < RL; ++j) {
-                const double* s = sc + (w * RL + j) * SCW;
-                double cf[2 * NC];
-                {
-                    double2 t0 = *reinterpret_cast<const double2*>(s);
-                    cf[0] = t0.x; cf[1] = t0.y;
-                    if (NC == 2) { double2 t1 = *reinterpret_cast<const double2*>(s + 2); cf[2] = t1.x; cf[3] = t1.y; }
+                for (int j = 0; j < RL; ++j) {
+                    const double* s = scw + j * S::SCW;
+                    double cf[2 * NC];
+                    { const double2 t0 = *reinterpret_cast<const double2*>(s); cf[0] = t0.x; cf[1] = t0.y; }
+                    if (NC == 2) { const double2 t1 = *reinterpret_cast<const double2*>(s + 2); cf[2] = t1.x; cf[3] = t1.y; }
+                    const double g = s[2 * NC];
+#pragma unroll
+                    for (int i = 0; i < RT; ++i) {
+                        const double e = ca[j * RT + i];
+#pragma unroll
+                        for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fma(e, cf[c], acc[i][c]);
+                        cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
+                    }
                 }
-                const double g = s[2 * NC];
+            } else {                                  // every item of the warp is still below 2^-140: recursion only
 #pragma unroll
-                for (int i = 0; i < RT; ++i) {
-                    const double e = cur[j][i];
+                for (int j = 0; j < RL; ++j) {
+                    const double g = scw[j * S::SCW + 2 * NC];
 #pragma unroll
-                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fma(e, cf[c], acc[i][c]);
-                    const double t = g * prev[j][i];
-                    prev[j][i] = e;
-                    cur[j][i] = fma(lam[i], e, -t);
+                    for (int i = 0; i < RT; ++i) cb[j * RT + i] = fma(lam[i], ca[j * RT + i], -(g * cb[j * RT + i]));
                 }
             }
             if ((m & (SHT_JCHK - 1)) == 0) {
-#pragma unroll
-                for (int j = 0; j < RL; ++j)
-#pragma unroll
-                    for (int i = 0; i < RT; ++i) window_check(cur[j][i], prev[j][i], kk[j][i]);
+                if (kp.any_nonzero()) window_check<NI>(cb, ca, kp);
+                if (P.m_lo) dead_check<NI>(cb, ca);
+                if (m < la) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
             }
-            double* r = red + ((it & 1) * NW + w) * (2 * NC) * NTH;
+            double* r = &sm.red[it & 1][w][0][0];
 #pragma unroll
             for (int i = 0; i < RT; ++i)
 #pragma unroll
                 for (int c = 0; c < 2 * NC; ++c) r[c * NTH + lane + 32 * i] = acc[i][c];
-            __syncwarp();
         }
+        if (is_helper && m > m_end) helper(m - 1, it + 1);
         __syncthreads();
         if (tid == 0 && m - NST >= m_end) {
-            mbar_expect_tx(&bar[slot], tile_bytes);
-            bulk_g2s(ctile + slot * TL * NC, P.in + ((size_t)(m - NST - m_end) * A.Lp + l0) * NC, tile_bytes, &bar[slot]);
+            mbar_expect_tx(&sm.bar[it % NST], tile_bytes);
+            bulk_g2s(&sm.ctile[it % NST][0], P.in + ((size_t)(m - NST - m_end) * A.Lp + l0) * NC, tile_bytes, &sm.bar[it % NST]);
         }
         // ---- reduce over the warps that were active at this step, add into F
-        if (tid < 2 * NC * NTH) {
-            const int c = tid / NTH, tl = tid % NTH, th = th0 + tl;
+        for (int o = tid; o < 2 * NC * NTH; o += NW * 32) {
+            const int c = o / NTH, tl = o % NTH, th = th0 + tl;
             int wmin = (m - l0) / RL; if (wmin < 0) wmin = 0;
             int wmax = (A.L - 1 - l0) / RL; if (wmax > NW - 1) wmax = NW - 1;
             double v = 0.0;
-            const double* r = red + (it & 1) * NW * (2 * NC) * NTH + c * NTH + tl;
+            const double* r = &sm.red[it & 1][0][c][tl];
             for (int ww = wmin; ww <= wmax; ++ww) v += r[ww * (2 * NC) * NTH];
-            int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
+            const int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
             bool ok = th < A.nth && !(NC == 2 && (c >> 1) && m == 0);
             if (ok && P.m_lo) ok = m >= P.m_lo[th];
             if (ok) {
-                int row = m_out < 0 ? m_out + A.NB : m_out;
+                const int row = m_out < 0 ? m_out + A.NB : m_out;
                 atomicAdd(reinterpret_cast<double*>(P.out + (size_t)row * A.ntp + th) + (c & 1), v);
             }
         }
+    };
+    for (int m = mtop; m >= m_end; m -= 2) {
+        step(m, cur, prev);
+        if (m - 1 >= m_end) step(m - 1, prev, cur);
     }
 }
 
 // =============================================================================================================
 // forward theta step, Eq. 30:  H[m_out+L-1][l] += c_m(l) * sum_theta W[m][theta] * e^l_m(theta)
 // =============================================================================================================
-template <int RT, int NW, int NC>
-__global__ void __launch_bounds__(NW * 32) theta_forward_kernel(const ThetaArgs A) {
-    constexpr int NTB = NW * RT;     // rings per block
+template <int RL, int RT, int NW, int NC>
+struct FwdSmem {
+    static constexpr int TLB = 32 * RL, NTB = NW * RT;
+    double2 wtile[NST][NTB * NC];       // weighted F_m tiles (TMA ring)
+    double hdr[2][NTB + 2];             // per step: lambda'_m(theta) for the block's rings, then 2^{-2-k_m-k_{m+1}}
+    double red[2][NW][2 * NC][TLB];     // per-warp partial sums
+    uint64_t bar[NST];
+};
+
+template <int RL, int RT, int NW, int NC>
+__global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kernel(const ThetaArgs A) {
+    using S = FwdSmem<RL, RT, NW, NC>;
+    constexpr int TLB = S::TLB, NTB = S::NTB, NI = RL * RT;
+    static_assert(NW * 32 >= TLB + NTB + 1 || NW * 32 >= TLB, "block too small for reducer + producer roles");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2* wtile = reinterpret_cast<double2*>(smem_raw);                         // [NST][NTB*NC]
-    double* lamb = reinterpret_cast<double*>(wtile + NST * NTB * NC);              // [2][NTB]
-    double* red = lamb + 2 * NTB;                                                  // [2][NW][2*NC][32]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(red + 2 * NW * 2 * NC * 32);       // [NST]
+    S& sm = *reinterpret_cast<S*>(smem_raw);
 
     const ThetaPass P = A.passes[blockIdx.y];
-    const int ntt = A.ntp / NTB, nlt = A.Lp / 32;
+    const int ntt = A.ntp / NTB, nlt = A.Lp / TLB;
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
-    const int l0 = lt * 32, th0 = tt * NTB;
+    const int l0 = lt * TLB, th0 = tt * NTB;
     const int an = P.n < 0 ? -P.n : P.n;
-    if (l0 + 32 <= an || l0 >= A.L || th0 >= A.nth) return;
+    if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + 31, A.L - 1), m_end = P.m_end;
-    const int l = l0 + lane;
-    const uint32_t tile_bytes = NTB * NC * sizeof(double2);
+    const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end;
+    constexpr uint32_t tile_bytes = NTB * NC * sizeof(double2);
     if (tid == 0) {
-        for (int i = 0; i < NST; ++i) mbar_init(&bar[i], 1);
+        for (int i = 0; i < NST; ++i) mbar_init(&sm.bar[i], 1);
         mbar_fence_init();
     }
     __syncthreads();
@@ -258,86 +332,149 @@ __global__ void __launch_bounds__(NW * 32) theta_forward_kernel(const ThetaArgs 
         for (int it = 0; it < NST; ++it) {
             int m = mtop - it;
             if (m >= m_end) {
-                mbar_expect_tx(&bar[it], tile_bytes);
-                bulk_g2s(wtile + it * NTB * NC, P.in + ((size_t)(m - m_end) * A.ntp + th0) * NC, tile_bytes, &bar[it]);
+                mbar_expect_tx(&sm.bar[it], tile_bytes);
+                bulk_g2s(&sm.wtile[it][0], P.in + ((size_t)(m - m_end) * A.ntp + th0) * NC, tile_bytes, &sm.bar[it]);
             }
         }
     }
-    const int8_t* krow = A.kexp + (size_t)((l0 + 32) / SHT_TQ - 1) * A.kstride - A.kmin;
-    const double fn = (double)P.n;
-    // ring constants for the lambda' producer threads (tid < NTB)
+    const int8_t* krow = A.kexp + (size_t)((l0 + TLB) / SHT_TQ - 1) * A.kstride - A.kmin;
+    // ---- producers (the last NTB+1 threads): lambda' of one ring each, plus the g' scale
+    constexpr int PB = NW * 32 - (NTB + 1);
+    const bool is_prod = tid >= PB;
+    const int pt = tid - PB;
     double pcsc = 0, ptau = 0, psg = 1;
-    if (tid < NTB) { pcsc = A.csc[th0 + tid]; ptau = A.tau[th0 + tid]; psg = A.sig[th0 + tid]; }
-    auto lam_of = [&](int m) {
-        const double sm = pow2i(-(int)krow[m]), fm = (double)m;
-        return sm * fma(fn - psg * fm, pcsc, fm * ptau);
+    if (is_prod && pt < NTB) { pcsc = A.csc[th0 + pt]; ptau = A.tau[th0 + pt]; psg = A.sig[th0 + pt]; }
+    const double fn = (double)P.n;
+    auto produce = [&](int m, int buf) {
+        const int km = krow[m];
+        if (pt < NTB) {
+            const double fm = (double)m;
+            sm.hdr[buf][pt] = pow2i(-km) * fma(fn - psg * fm, pcsc, fm * ptau);
+        } else sm.hdr[buf][NTB] = pow2i(-2 - km - krow[m + 1]);
     };
-    if (tid < NTB) lamb[tid] = lam_of(mtop);
-    // state: start values are preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
-    double cur[RT], prev[RT];
-    int kk[RT];
-    const bool lane_ok = (l >= an) && (l < A.L);
+    if (is_prod) produce(mtop, 0);
+    // ---- state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
+    double cur[NI], prev[NI], x[RL];
+    KPack<NI> kp;
+    int lr[RL];
 #pragma unroll
-    for (int i = 0; i < RT; ++i) {
-        size_t o = (size_t)l * A.ntp + th0 + w * RT + i;
-        cur[i] = lane_ok ? P.st_val[o] : 0.0;
-        kk[i] = lane_ok ? (int)P.st_k[o] : 0;
-        prev[i] = 0.0;
+    for (int r = 0; r < RL; ++r) {
+        lr[r] = l0 + lane + 32 * r;
+        const bool ok = lr[r] >= an && lr[r] < A.L;
+        x[r] = (double)(lr[r] - mtop) * (double)(lr[r] + mtop + 1);
+#pragma unroll
+        for (int i = 0; i < RT; ++i) {
+            const size_t o = (size_t)lr[r] * A.ntp + th0 + w * RT + i;
+            cur[r * RT + i] = ok ? P.st_val[o] : 0.0;
+            prev[r * RT + i] = 0.0;
+            kp.set(r * RT + i, ok ? (uint32_t)P.st_k[o] : 0u);
+        }
     }
-    // reducer state (tid < 2*NC*32): degree l0 + (tid & 31), component tid >> 5
-    const int lr = l0 + (tid & 31);
+    double tm = 2.0 * (double)mtop;                    // x_{m-1} = x_m + 2m
+    bool wact = true;
+    // reducer state (tid < TLB): degree l0 + tid, all components
+    const int lred = l0 + tid;
     double cfac = 1.0;
     __syncthreads();
 
-    for (int m = mtop; m >= m_end; --m) {
+    // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
+    auto step = [&](const int m, double (&ca)[NI], double (&cb)[NI]) {
         const int it = mtop - m, slot = it % NST;
-        const int km = krow[m], km1 = krow[m + 1];
-        const bool on = m <= l;
-        const double g = on ? (double)(l - m) * (double)(l + m + 1) * pow2i(-2 - km - km1) : 0.0;
-        mbar_wait(&bar[slot], (it / NST) & 1);
-        const double2* T = wtile + slot * NTB * NC + w * RT * NC;
-        const double* LM = lamb + (it & 1) * NTB + w * RT;
-        double acc[2 * NC];
+        mbar_wait(&sm.bar[slot], (it / NST) & 1);
+        const double2* T = &sm.wtile[slot][w * RT * NC];
+        const double* LM = &sm.hdr[it & 1][w * RT];
+        const double G = sm.hdr[it & 1][NTB];
+        double acc[RL][2 * NC];
 #pragma unroll
-        for (int c = 0; c < 2 * NC; ++c) acc[c] = 0.0;
+        for (int r = 0; r < RL; ++r)
 #pragma unroll
-        for (int i = 0; i < RT; ++i) {
-            const double2 w0 = T[i * NC];
-            const double e = cur[i];
-            acc[0] = fma(e, w0.x, acc[0]); acc[1] = fma(e, w0.y, acc[1]);
-            if (NC == 2) { const double2 w1 = T[i * NC + 1]; acc[2] = fma(e, w1.x, acc[2]); acc[3] = fma(e, w1.y, acc[3]); }
-            const double lm = on ? LM[i] : 1.0;
-            const double t = g * prev[i];
-            prev[i] = on ? e : 0.0;
-            cur[i] = fma(lm, e, -t);
-        }
-        if ((m & (SHT_JCHK - 1)) == 0) {
+            for (int c = 0; c < 2 * NC; ++c) acc[r][c] = 0.0;
+        if (m >= l0) {
+            // ---- ramp: lanes whose degree is still above m hold still
+            double g[RL]; bool on[RL];
 #pragma unroll
-            for (int i = 0; i < RT; ++i) window_check(cur[i], prev[i], kk[i]);
-        }
-        double* r = red + ((it & 1) * NW + w) * (2 * NC) * 32;
+            for (int r = 0; r < RL; ++r) { on[r] = m <= lr[r]; g[r] = on[r] ? x[r] * G : 0.0; }
 #pragma unroll
-        for (int c = 0; c < 2 * NC; ++c) r[c * 32 + lane] = acc[c];
-        if (tid < NTB && m > m_end) lamb[((it + 1) & 1) * NTB + tid] = lam_of(m - 1);
-        __syncthreads();
-        if (tid == 0 && m - NST >= m_end) {
-            mbar_expect_tx(&bar[slot], tile_bytes);
-            bulk_g2s(wtile + slot * NTB * NC, P.in + ((size_t)(m - NST - m_end) * A.ntp + th0) * NC, tile_bytes, &bar[slot]);
-        }
-        if (tid < 2 * NC * 32) {
-            const int c = tid >> 5;
-            if (lr >= m && lr >= an && lr < A.L) {
-                double v = 0.0;
-                const double* rr = red + (it & 1) * NW * (2 * NC) * 32 + c * 32 + (tid & 31);
+            for (int i = 0; i < RT; ++i) {
+                const double2 w0 = T[i * NC];
+                double2 w1 = make_double2(0.0, 0.0);
+                if (NC == 2) w1 = T[i * NC + 1];
+                const double lm = LM[i];
 #pragma unroll
-                for (int ww = 0; ww < NW; ++ww) v += rr[ww * (2 * NC) * 32];
-                v *= cfac;
-                int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
-                if (!(NC == 2 && (c >> 1) && m == 0))
-                    atomicAdd(reinterpret_cast<double*>(P.out + (size_t)(m_out + A.L - 1) * A.Lp + lr) + (c & 1), v);
-                if (m > m_end) cfac *= pow2i(km + 1) * A.rsq[lr - m + 1] * A.rsq[lr + m];
+                for (int r = 0; r < RL; ++r) {
+                    const double e = ca[r * RT + i];
+                    acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
+                    if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
+                    cb[r * RT + i] = fma(on[r] ? lm : 1.0, e, -(g[r] * cb[r * RT + i]));     // off: copies the start value
+                    ca[r * RT + i] = on[r] ? e : 0.0;                                         //      and keeps e_{m+1} = 0
+                }
+            }
+        } else if (wact) {
+            double g[RL];
+#pragma unroll
+            for (int r = 0; r < RL; ++r) g[r] = x[r] * G;
+#pragma unroll
+            for (int i = 0; i < RT; ++i) {
+                const double2 w0 = T[i * NC];
+                double2 w1 = make_double2(0.0, 0.0);
+                if (NC == 2) w1 = T[i * NC + 1];
+                const double lm = LM[i];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) {
+                    const double e = ca[r * RT + i];
+                    acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
+                    if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
+                    cb[r * RT + i] = fma(lm, e, -(g[r] * cb[r * RT + i]));
+                }
+            }
+        } else {                                      // every item of the warp is still below 2^-140: recursion only
+            double g[RL];
+#pragma unroll
+            for (int r = 0; r < RL; ++r) g[r] = x[r] * G;
+#pragma unroll
+            for (int i = 0; i < RT; ++i) {
+                const double lm = LM[i];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) cb[r * RT + i] = fma(lm, ca[r * RT + i], -(g[r] * cb[r * RT + i]));
             }
         }
+#pragma unroll
+        for (int r = 0; r < RL; ++r) x[r] += tm;
+        tm -= 2.0;
+        if ((m & (SHT_JCHK - 1)) == 0) {
+            if (kp.any_nonzero()) window_check<NI>(cb, ca, kp);
+            if (P.m_lo) dead_check<NI>(cb, ca);
+            if (m < l0) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
+        }
+        double* rd = &sm.red[it & 1][w][0][0];
+#pragma unroll
+        for (int r = 0; r < RL; ++r)
+#pragma unroll
+            for (int c = 0; c < 2 * NC; ++c) rd[c * TLB + lane + 32 * r] = acc[r][c];
+        if (is_prod && m > m_end) produce(m - 1, (it + 1) & 1);
+        __syncthreads();
+        if (tid == 0 && m - NST >= m_end) {
+            mbar_expect_tx(&sm.bar[slot], tile_bytes);
+            bulk_g2s(&sm.wtile[slot][0], P.in + ((size_t)(m - NST - m_end) * A.ntp + th0) * NC, tile_bytes, &sm.bar[slot]);
+        }
+        if (tid < TLB && lred >= m && lred >= an && lred < A.L) {
+            const double* rr = &sm.red[it & 1][0][0][tid];
+#pragma unroll
+            for (int c = 0; c < 2 * NC; ++c) {
+                double v = 0.0;
+#pragma unroll
+                for (int ww = 0; ww < NW; ++ww) v += rr[(ww * 2 * NC + c) * TLB];
+                v *= cfac;
+                const int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
+                if (!(NC == 2 && (c >> 1) && m == 0))
+                    atomicAdd(reinterpret_cast<double*>(P.out + (size_t)(m_out + A.L - 1) * A.Lp + lred) + (c & 1), v);
+            }
+            if (m > m_end) cfac *= pow2i(krow[m] + 1) * A.rsq[lred - m + 1] * A.rsq[lred + m];
+        }
+    };
+    for (int m = mtop; m >= m_end; m -= 2) {
+        step(m, cur, prev);
+        if (m - 1 >= m_end) step(m - 1, prev, cur);
     }
 }
 
@@ -358,26 +495,33 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double* sink)
 }
 
 template <int RL, int RT, int NW, int NC>
-cudaError_t launch_inv(const ThetaArgs& a, cudaStream_t st) {
-    constexpr int TL = NW * RL, NTH = 32 * RT, SCW = (NC == 2) ? 6 : 4;
-    size_t smem = sizeof(double2) * NST * TL * NC + sizeof(double) * (NW * RL * SCW + 2 * NW * 2 * NC * NTH + TL * NTH) + TL * NTH +
-                  8 * (NST + 1) + 128;
-    auto k = theta_inverse_kernel<RL, RT, NW, NC>;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((a.Lp / TL) * (a.ntp / NTH), a.npass);
-    k<<<grid, NW * 32, smem, st>>>(a);
+cudaError_t launch_inv(const ThetaArgs& a, bool spin0, cudaStream_t st) {
+    using S = InvSmem<RL, RT, NW, NC>;
+    const size_t smem = sizeof(S) + 128;
+    dim3 grid((a.Lp / S::TL) * (a.ntp / S::NTH), a.npass);
+    cudaError_t e;
+    if (spin0) {
+        auto k = theta_inverse_kernel<RL, RT, NW, NC, true>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, NW * 32, smem, st>>>(a);
+    } else {
+        auto k = theta_inverse_kernel<RL, RT, NW, NC, false>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, NW * 32, smem, st>>>(a);
+    }
     count_launch();
     return cudaGetLastError();
 }
-template <int RT, int NW, int NC>
+template <int RL, int RT, int NW, int NC>
 cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
-    constexpr int NTB = NW * RT;
-    size_t smem = sizeof(double2) * NST * NTB * NC + sizeof(double) * (2 * NTB + 2 * NW * 2 * NC * 32) + 8 * NST + 128;
-    auto k = theta_forward_kernel<RT, NW, NC>;
+    using S = FwdSmem<RL, RT, NW, NC>;
+    const size_t smem = sizeof(S) + 128;
+    auto k = theta_forward_kernel<RL, RT, NW, NC>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid((a.Lp / 32) * (a.ntp / NTB), a.npass);
+    dim3 grid((a.Lp / S::TLB) * (a.ntp / S::NTB), a.npass);
     k<<<grid, NW * 32, smem, st>>>(a);
     count_launch();
     return cudaGetLastError();
@@ -385,15 +529,15 @@ cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
 
 }  // namespace
 
-// Tile shapes: inverse 128 degrees x 32 rings per block (8 warps x 16 degrees per thread);
-//              forward 32 degrees x 128 rings per block (8 warps x 16 rings per thread).
+// Tile shapes: inverse 64 degrees x 64 rings per block (8 warps, 8 degrees x 2 rings per thread);
+//              forward 64 degrees x 32 rings per block (4 warps, 2 degrees x 8 rings per thread).
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
-    return mode == 0 ? launch_inv<16, 1, 8, 2>(a, st) : launch_inv<16, 1, 8, 1>(a, st);
+    return mode == 0 ? launch_inv<8, 2, 8, 2>(a, true, st) : launch_inv<8, 2, 8, 1>(a, a.all_n_zero != 0, st);
 }
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
-    return mode == 0 ? launch_fwd<16, 8, 2>(a, st) : launch_fwd<16, 8, 1>(a, st);
+    return mode == 0 ? launch_fwd<2, 8, 4, 2>(a, st) : launch_fwd<2, 8, 4, 1>(a, st);
 }
 cudaError_t launch_fp64_peak(int iters, double* sink, cudaStream_t st, int* blocks, int* threads, int* fma_per_thread) {
     *blocks = 148 * 8; *threads = 256; *fma_per_thread = 16;
