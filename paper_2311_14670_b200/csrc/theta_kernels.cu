@@ -41,6 +41,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
             : "memory");
     } while (!ok);
 }
+// fire-and-forget fp64 add to GLOBAL memory (RED.E.ADD.F64); atomicAdd on a generic pointer compiles to an
+// address-space dispatch with CAS fallbacks
+__device__ __forceinline__ void red_add_f64(double* gptr, double v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gptr), "d"(v) : "memory");
+}
 // 2^e as a double, e in [-1022, 1023]
 __device__ __forceinline__ double pow2i(int e) { return __hiloint2double((1023 + e) << 20, 0); }
 __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7fffffff; }
@@ -105,7 +110,7 @@ struct InvSmem {
     static constexpr int TL = NW * RL, NTH = 32 * RT, SCW = (NC == 2) ? 6 : 4;
     double2 ctile[NST][TL * NC];        // raw coefficient tiles (TMA ring)
     double sc[2][TL][SCW];              // per step: coefficients * c_m(l), then g'_m(l)
-    double red[2][NW][2 * NC][NTH];     // per-warp partial sums
+    double red[2][NW][NTH][2 * NC];     // per-warp partial sums
     double stv[TL][NTH];                // start values of the block's (l, ring) tile
     uint8_t stk[TL][NTH];
     uint64_t bar[NST + 1];
@@ -175,8 +180,8 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kern
     const int hl = tid - HB, lh = l0 + hl;
     const int8_t* krow_h = A.kexp + (size_t)((l0 + (hl / RL) * RL + RL + SHT_TQ - 1) / SHT_TQ - 1) * A.kstride - A.kmin;
     double cfac = 1.0;
-    auto helper = [&](int m, int it) {                // prepares sc[it & 1] for recursion step m
-        const int slot = it % NST;
+    auto helper = [&](int m, unsigned it) {           // prepares sc[it & 1] for recursion step m
+        const unsigned slot = it & (NST - 1);
         mbar_wait(&sm.bar[slot], (it / NST) & 1);
         if (lh > m && lh >= an) cfac *= pow2i(krow_h[m + 1] + 1) * A.rsq[lh - m] * A.rsq[lh + m + 1];   // c_{m} from c_{m+1}
         const double2* raw = &sm.ctile[slot][hl * NC];
@@ -190,10 +195,20 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kern
     mbar_wait(&sm.bar[NST], 0);
     __syncthreads();
 
+    // reducer constants: output base as a global-space address, last warp holding real degrees, per-output m_lo
+    double* const out_g = reinterpret_cast<double*>(P.out);
+    int wmax_blk = (A.L - 1 - l0) / RL; if (wmax_blk > NW - 1) wmax_blk = NW - 1;
+    constexpr int NRED = (2 * NC * NTH + NW * 32 - 1) / (NW * 32);
+    int mlo_red[NRED];
+#pragma unroll
+    for (int q = 0; q < NRED; ++q) {
+        const int o = tid + q * NW * 32;
+        mlo_red[q] = (P.m_lo && o < 2 * NC * NTH) ? P.m_lo[th0 + o / (2 * NC)] : -(1 << 30);
+    }
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step,
     // so the iterates never move between registers)
     auto step = [&](const int m, double (&ca)[NI], double (&cb)[NI]) {
-        const int it = mtop - m;
+        const unsigned it = (unsigned)(mtop - m);
         const bool warp_on = (m <= la + RL - 1) && (la < A.L);
         if (warp_on) {
             if (m >= la) {                            // ramp: the degree l == m starts (warp-uniform)
@@ -259,32 +274,33 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kern
                 if (P.m_lo) dead_check<NI>(cb, ca);
                 if (m < la) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
             }
-            double* r = &sm.red[it & 1][w][0][0];
+            double2* r = reinterpret_cast<double2*>(&sm.red[it & 1][w][0][0]);
 #pragma unroll
             for (int i = 0; i < RT; ++i)
 #pragma unroll
-                for (int c = 0; c < 2 * NC; ++c) r[c * NTH + lane + 32 * i] = acc[i][c];
+                for (int c = 0; c < NC; ++c) r[(lane + 32 * i) * NC + c] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
         }
         if (is_helper && m > m_end) helper(m - 1, it + 1);
         __syncthreads();
         if (tid == 0 && m - NST >= m_end) {
-            mbar_expect_tx(&sm.bar[it % NST], tile_bytes);
-            bulk_g2s(&sm.ctile[it % NST][0], P.in + ((size_t)(m - NST - m_end) * A.Lp + l0) * NC, tile_bytes, &sm.bar[it % NST]);
+            mbar_expect_tx(&sm.bar[it & (NST - 1)], tile_bytes);
+            bulk_g2s(&sm.ctile[it & (NST - 1)][0], P.in + ((size_t)(m - NST - m_end) * A.Lp + l0) * NC, tile_bytes, &sm.bar[it & (NST - 1)]);
         }
-        // ---- reduce over the warps that were active at this step, add into F
-        for (int o = tid; o < 2 * NC * NTH; o += NW * 32) {
-            const int c = o / NTH, tl = o % NTH, th = th0 + tl;
+        // ---- reduce over the warps that were active at this step, add into F (thread <-> (ring, component))
+#pragma unroll
+        for (int q = 0; q < NRED; ++q) {
+            const int o = tid + q * NW * 32;
+            if (o >= 2 * NC * NTH) break;
+            const int c = o % (2 * NC), tl = o / (2 * NC), th = th0 + tl;
             int wmin = (m - l0) / RL; if (wmin < 0) wmin = 0;
-            int wmax = (A.L - 1 - l0) / RL; if (wmax > NW - 1) wmax = NW - 1;
             double v = 0.0;
-            const double* r = &sm.red[it & 1][0][c][tl];
-            for (int ww = wmin; ww <= wmax; ++ww) v += r[ww * (2 * NC) * NTH];
+            const double* r = &sm.red[it & 1][0][0][0] + o;
+            for (int ww = wmin; ww <= wmax_blk; ++ww) v += r[ww * (2 * NC) * NTH];
             const int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
-            bool ok = th < A.nth && !(NC == 2 && (c >> 1) && m == 0);
-            if (ok && P.m_lo) ok = m >= P.m_lo[th];
+            const bool ok = th < A.nth && !(NC == 2 && (c >> 1) && m == 0) && m >= mlo_red[q];
             if (ok) {
                 const int row = m_out < 0 ? m_out + A.NB : m_out;
-                atomicAdd(reinterpret_cast<double*>(P.out + (size_t)row * A.ntp + th) + (c & 1), v);
+                red_add_f64(out_g + ((size_t)row * A.ntp + th) * 2 + (c & 1), v);
             }
         }
     };
@@ -302,7 +318,7 @@ struct FwdSmem {
     static constexpr int TLB = 32 * RL, NTB = NW * RT;
     double2 wtile[NST][NTB * NC];       // weighted F_m tiles (TMA ring)
     double hdr[2][NTB + 2];             // per step: lambda'_m(theta) for the block's rings, then 2^{-2-k_m-k_{m+1}}
-    double red[2][NW][2 * NC][TLB];     // per-warp partial sums
+    double red[2][NW][TLB][2 * NC];     // per-warp partial sums
     uint64_t bar[NST];
 };
 
@@ -374,16 +390,21 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
     bool wact = true;
     // reducer state (tid < TLB): degree l0 + tid, all components
     const int lred = l0 + tid;
+    double* const out_g = reinterpret_cast<double*>(P.out);
     double cfac = 1.0;
     __syncthreads();
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
     auto step = [&](const int m, double (&ca)[NI], double (&cb)[NI]) {
-        const int it = mtop - m, slot = it % NST;
+        const unsigned it = (unsigned)(mtop - m), slot = it & (NST - 1);
         mbar_wait(&sm.bar[slot], (it / NST) & 1);
         const double2* T = &sm.wtile[slot][w * RT * NC];
         const double* LM = &sm.hdr[it & 1][w * RT];
         const double G = sm.hdr[it & 1][NTB];
+        double lmv[RT];
+        static_assert(RT % 2 == 0, "RT must be even (lambda' is read in pairs)");
+#pragma unroll
+        for (int i = 0; i < RT; i += 2) { const double2 t = *reinterpret_cast<const double2*>(LM + i); lmv[i] = t.x; lmv[i + 1] = t.y; }
         double acc[RL][2 * NC];
 #pragma unroll
         for (int r = 0; r < RL; ++r)
@@ -399,7 +420,7 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
                 const double2 w0 = T[i * NC];
                 double2 w1 = make_double2(0.0, 0.0);
                 if (NC == 2) w1 = T[i * NC + 1];
-                const double lm = LM[i];
+                const double lm = lmv[i];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
                     const double e = ca[r * RT + i];
@@ -418,7 +439,7 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
                 const double2 w0 = T[i * NC];
                 double2 w1 = make_double2(0.0, 0.0);
                 if (NC == 2) w1 = T[i * NC + 1];
-                const double lm = LM[i];
+                const double lm = lmv[i];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
                     const double e = ca[r * RT + i];
@@ -433,7 +454,7 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
             for (int r = 0; r < RL; ++r) g[r] = x[r] * G;
 #pragma unroll
             for (int i = 0; i < RT; ++i) {
-                const double lm = LM[i];
+                const double lm = lmv[i];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) cb[r * RT + i] = fma(lm, ca[r * RT + i], -(g[r] * cb[r * RT + i]));
             }
@@ -446,11 +467,11 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
             if (P.m_lo) dead_check<NI>(cb, ca);
             if (m < l0) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
         }
-        double* rd = &sm.red[it & 1][w][0][0];
+        double2* rd = reinterpret_cast<double2*>(&sm.red[it & 1][w][0][0]);
 #pragma unroll
         for (int r = 0; r < RL; ++r)
 #pragma unroll
-            for (int c = 0; c < 2 * NC; ++c) rd[c * TLB + lane + 32 * r] = acc[r][c];
+            for (int c = 0; c < NC; ++c) rd[(lane + 32 * r) * NC + c] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
         if (is_prod && m > m_end) produce(m - 1, (it + 1) & 1);
         __syncthreads();
         if (tid == 0 && m - NST >= m_end) {
@@ -458,16 +479,17 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
             bulk_g2s(&sm.wtile[slot][0], P.in + ((size_t)(m - NST - m_end) * A.ntp + th0) * NC, tile_bytes, &sm.bar[slot]);
         }
         if (tid < TLB && lred >= m && lred >= an && lred < A.L) {
-            const double* rr = &sm.red[it & 1][0][0][tid];
+            const double2* rr = reinterpret_cast<const double2*>(&sm.red[it & 1][0][tid][0]);
 #pragma unroll
-            for (int c = 0; c < 2 * NC; ++c) {
-                double v = 0.0;
+            for (int c = 0; c < NC; ++c) {
+                double2 v = make_double2(0.0, 0.0);
 #pragma unroll
-                for (int ww = 0; ww < NW; ++ww) v += rr[(ww * 2 * NC + c) * TLB];
-                v *= cfac;
-                const int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
-                if (!(NC == 2 && (c >> 1) && m == 0))
-                    atomicAdd(reinterpret_cast<double*>(P.out + (size_t)(m_out + A.L - 1) * A.Lp + lred) + (c & 1), v);
+                for (int ww = 0; ww < NW; ++ww) { const double2 t = rr[ww * TLB * NC + c]; v.x += t.x; v.y += t.y; }
+                const int m_out = (NC == 2) ? (c ? -m : m) : P.sgn_out * m;
+                if (!(NC == 2 && c && m == 0)) {
+                    double* o = out_g + ((size_t)(m_out + A.L - 1) * A.Lp + lred) * 2;
+                    red_add_f64(o, v.x * cfac); red_add_f64(o + 1, v.y * cfac);
+                }
             }
             if (m > m_end) cfac *= pow2i(krow[m] + 1) * A.rsq[lred - m + 1] * A.rsq[lred + m];
         }
