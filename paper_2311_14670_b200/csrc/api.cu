@@ -94,6 +94,11 @@ struct sht_plan {
     double* unit_wq = nullptr; // [fwd.ntp] ones (theta-stage entry point takes already weighted rows)
     size_t F_slab = 0, Fa_slab = 0, X_slab = 0, Z_slab = 0, H_slab = 0;
     int Ltp = 0;               // padded ring count of Fa rows
+    int fwd_ld = 0;            // row length of the forward ring-sample array U (MW: 4L-1, HEALPix: padded ring count)
+    // HEALPix ring-FFT staging (healpix.cu): Bluestein batch C[2(nside-1)][M], chirp spectra BF[nside-1][M], belt rows E
+    int hp_M = 0, hp_ncap = 0, hp_neq = 0; long long hp_off_eq = 0;
+    double2 *hp_C = nullptr, *hp_BF = nullptr, *hp_E = nullptr;
+    cufftHandle fft_hp_cap = 0, fft_hp_eq = 0;
     void* fft_work = nullptr; size_t fft_work_bytes = 0;
     cufftHandle fft_phi_inv = 0, fft_phi_fwd = 0, fft_th1 = 0, fft_th2 = 0, fft_gamma = 0;
     bool have_fft = false;
@@ -115,6 +120,21 @@ void rings_mw(RingSet& R, int Lt) {      // Eq. 37: theta_t = (2t
     for (int t = 0; t < R.nth; ++t) {
         ld th = PI_L * (ld)(2 * t + 1) / (ld)(2 * Lt - 1);
         R.ct[t] = cosl(th); R.c2[t] = cosl(th / 2); R.s2[t] = sinl(th / 2);
+    }
+    R.ntp = (int)rup((size_t)R.nth + 1, 128);
+}
+
+// HEALPix rings r = 1..4 nside-1 (public ring scheme, R11); half-angle trigonometry from z
+void rings_healpix(RingSet& R, int nside) {
+    R.nth = 4 * nside - 1; R.pole = false;
+    R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
+    const ld ns = (ld)nside;
+    for (int i = 0; i < R.nth; ++i) {
+        int r = i + 1, rr = r <= 2 * nside ? r : 4 * nside - r;
+        ld z = rr < nside ? 1.0L - (ld)rr * (ld)rr / (3.0L * ns * ns) : 4.0L / 3.0L - 2.0L * (ld)rr / (3.0L * ns);
+        if (r == 2 * nside) z = 0;
+        if (r > 2 * nside) z = -z;
+        R.ct[i] = z; R.c2[i] = sqrtl((1 + z) / 2); R.s2[i] = sqrtl((1 - z) / 2);
     }
     R.ntp = (int)rup((size_t)R.nth + 1, 128);
 }
@@ -168,15 +188,23 @@ void layout(sht_plan* P, char* base) {
     P->tmp = B.take<double>(2 * (size_t)Lp);
     P->unit_wq = B.take<double>(P->fwd.ntp);
     P->Ltp = P->inv.ntp;
-    P->Fa_slab = (size_t)NB * P->Ltp;
-    P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
-    P->X_slab = (size_t)NB * NB;
-    P->X = B.take<double2>(P->X_slab * P->nslab);
-    P->Z_slab = (size_t)NB * (4 * L - 1);
+    if (P->sampling == SHT_MW) {
+        P->fwd_ld = 4 * L - 1;
+        P->Fa_slab = (size_t)NB * P->Ltp;
+        P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
+        P->X_slab = (size_t)NB * NB;
+        P->X = B.take<double2>(P->X_slab * P->nslab);
+    } else {
+        P->fwd_ld = P->fwd.ntp;
+        P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
+        P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
+        P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
+    }
+    P->Z_slab = (size_t)NB * P->fwd_ld;
     P->Z = B.take<double2>(P->Z_slab * P->nslab);
     P->H_slab = (size_t)NB * Lp;
     P->H = B.take<double2>(P->H_slab * P->nslab);
-    if (P->reality) P->cplx = B.take<double2>((size_t)L * NB);
+    if (P->reality && P->sampling == SHT_MW) P->cplx = B.take<double2>((size_t)L * NB);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
     P->fft_work = B.take<char>(P->fft_work_bytes);
     // route every pass to its slab's output array
@@ -208,6 +236,23 @@ void add_passes(sht_plan* P, int slab, int n, bool real) {
 sht_status make_fft_plans(sht_plan* P) {
     const int L = P->L, NB = P->NB;
     size_t ws = 0, w;
+    if (P->sampling == SHT_HEALPIX) {
+        const int ns = P->nside;
+        P->hp_ncap = 2 * (ns - 1); P->hp_neq = 2 * ns + 1; P->hp_off_eq = 2LL * ns * (ns - 1);
+        P->hp_M = 1;
+        while (P->hp_M < 2 * 4 * (ns - 1) - 1) P->hp_M *= 2;
+        if (P->hp_ncap > 0) {
+            int nm[1] = {P->hp_M};
+            CF(cufftCreate(&P->fft_hp_cap)); CF(cufftSetAutoAllocation(P->fft_hp_cap, 0));
+            CF(cufftMakePlanMany(P->fft_hp_cap, 1, nm, nm, 1, P->hp_M, nm, 1, P->hp_M, CUFFT_Z2Z, P->hp_ncap, &w)); ws = w > ws ? w : ws;
+        }
+        int ne[1] = {4 * ns};
+        CF(cufftCreate(&P->fft_hp_eq)); CF(cufftSetAutoAllocation(P->fft_hp_eq, 0));
+        CF(cufftMakePlanMany(P->fft_hp_eq, 1, ne, ne, 1, 4 * ns, ne, 1, 4 * ns, CUFFT_Z2Z, P->hp_neq, &w)); ws = w > ws ? w : ws;
+        P->fft_work_bytes = ws + 256;
+        P->have_fft = true;
+        return SHT_OK;
+    }
     int n1[1] = {NB};
     CF(cufftCreate(&P->fft_phi_inv)); CF(cufftSetAutoAllocation(P->fft_phi_inv, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
@@ -408,6 +453,52 @@ sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
     return SHT_OK;
 }
 
+// HEALPix ring analysis: map -> U[bin(m)][ring] = e^{-i m phi0} DFT_ring[m mod nphi], in P->Z
+sht_status healpix_analysis(sht_plan* P, const void* f, cudaStream_t st) {
+    const int ns = P->nside, L = P->L, real = P->reality;
+    const size_t nbelt = (size_t)P->hp_neq * 4 * ns;
+    if (real) { stage(P, CAT_STAGE, st); CK(st_real_to_complex(nbelt, (const double*)f + P->hp_off_eq, P->hp_E, st)); }
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_hp_eq, st));
+    CF(cufftExecZ2Z(P->fft_hp_eq, real ? P->hp_E : const_cast<double2*>((const double2*)f + P->hp_off_eq), P->hp_E, CUFFT_FORWARD));
+    if (P->hp_ncap > 0) {
+        stage(P, CAT_STAGE, st);
+        CK(st_hp_pack_fwd(ns, P->hp_M, real, f, P->hp_C, st));
+        stage(P, CAT_FFT, st);
+        CF(cufftSetStream(P->fft_hp_cap, st)); CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD));
+        stage(P, CAT_STAGE, st);
+        CK(st_hp_mul(ns, P->hp_M, P->hp_BF, P->hp_C, st));
+        stage(P, CAT_FFT, st);
+        CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_INVERSE));
+    }
+    stage(P, CAT_STAGE, st);
+    CK(st_hp_unpack_fwd(ns, L, P->NB, real ? 0 : -(L - 1), P->fwd_ld, P->hp_M, P->hp_C, P->hp_E, P->Z, st));
+    return SHT_OK;
+}
+// HEALPix ring synthesis: F[bin][ring] -> fold onto m mod nphi with the ring phase -> per-ring synthesis
+sht_status healpix_synthesis(sht_plan* P, void* f, cudaStream_t st) {
+    const int ns = P->nside, L = P->L, real = P->reality;
+    const size_t nbelt = (size_t)P->hp_neq * 4 * ns;
+    stage(P, CAT_STAGE, st);
+    CK(st_hp_fold_inv(ns, L, P->NB, P->inv.ntp, P->hp_M, P->F, P->hp_C, P->hp_E, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_hp_eq, st));
+    CF(cufftExecZ2Z(P->fft_hp_eq, P->hp_E, real ? P->hp_E : (double2*)f + P->hp_off_eq, CUFFT_INVERSE));
+    if (real) { stage(P, CAT_STAGE, st); CK(st_hp_belt_real(nbelt, P->hp_E, (double*)f + P->hp_off_eq, st)); }
+    if (P->hp_ncap > 0) {
+        stage(P, CAT_FFT, st);
+        CF(cufftSetStream(P->fft_hp_cap, st)); CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD));
+        stage(P, CAT_STAGE, st);
+        CK(st_hp_mul(ns, P->hp_M, P->hp_BF, P->hp_C, st));
+        stage(P, CAT_FFT, st);
+        CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_INVERSE));
+        stage(P, CAT_STAGE, st);
+        CK(st_hp_unpack_inv(ns, P->hp_M, real, P->hp_C, f, st));
+    }
+    stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+
 }  // namespace
 
 void count_launch(int n) { g_launches += n; }
@@ -435,11 +526,12 @@ sht_status sht_plan_s2(sht_plan** out, int L, int spin, int sampling, int nside,
     if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || (sampling != SHT_MW && sampling != SHT_HEALPIX)) return SHT_EINVAL;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64) return SHT_EUNSUPPORTED;
-    if (sampling == SHT_HEALPIX) return SHT_EUNSUPPORTED;
+    if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
-    P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = nside; P->reality = reality ? 1 : 0;
+    P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->nslab = 1; P->slab_n = {-spin};        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
-    rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L);
+    if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L); }
+    else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
     sht_status s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
@@ -489,13 +581,32 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     }
     CS(up(si, P->scale_inv, st)); CS(up(sf, P->scale_fwd, st));
     CS(fill_ringset(P, P->inv, st)); CS(fill_ringset(P, P->fwd, st));
-    // forward quadrature weights on MW(2L): q_u = (2 pi/(2L-1)) v_u   (Eq. 41-44 at band-limit 2L)
     CK(cudaMemsetAsync(P->fwd.wq, 0, sizeof(double) * P->fwd.ntp, st));
-    CK(st_mw_weights(2 * L, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
+    if (P->sampling == SHT_MW) {
+        // forward quadrature weights on MW(2L): q_u = (2 pi/(2L-1)) v_u   (Eq. 41-44 at band-limit 2L)
+        CK(st_mw_weights(2 * L, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
+    } else {
+        // HEALPix: equal pixel weights 4 pi / Npix
+        std::vector<double> w(P->fwd.ntp, 0.0);
+        for (int t = 0; t < P->fwd.nth; ++t) w[t] = (double)(4 * PI_L / (12.0L * (ld)P->nside * (ld)P->nside));
+        CS(up(w, P->fwd.wq, st));
+    }
     { std::vector<double> ones(P->fwd.ntp, 1.0); CS(up(ones, P->unit_wq, st)); }
     CS(upload_passes(P, st));
-    for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));
-    if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
+    if (P->sampling == SHT_MW) {
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));
+        if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
+    } else {
+        CF(cufftSetWorkArea(P->fft_hp_eq, P->fft_work));
+        if (P->hp_ncap > 0) {
+            // chirp spectra: FFT of the wrapped chirps of the nside-1 distinct cap lengths (run through the cap batch plan)
+            CF(cufftSetWorkArea(P->fft_hp_cap, P->fft_work));
+            CK(cudaMemsetAsync(P->hp_C, 0, sizeof(double2) * (size_t)P->hp_ncap * P->hp_M, st));
+            CK(st_hp_chirp(P->nside, P->hp_M, P->hp_C, st));
+            CF(cufftSetStream(P->fft_hp_cap, st)); CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD));
+            CK(cudaMemcpyAsync(P->hp_BF, P->hp_C, sizeof(double2) * (size_t)(P->hp_ncap / 2) * P->hp_M, cudaMemcpyDeviceToDevice, st));
+        }
+    }
     CK(cudaStreamSynchronize(st));
     P->ready = true;
     return SHT_OK;
@@ -504,7 +615,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
 sht_status sht_plan_destroy(sht_plan* P) {
     if (!P) return SHT_OK;
     if (P->have_fft || P->fft_phi_inv) {
-        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma})
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_hp_cap, P->fft_hp_eq})
             if (h) cufftDestroy(h);
     }
     for (auto e : P->ev) cudaEventDestroy(e);
@@ -552,7 +663,7 @@ sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_str
     cudaStream_t st = (cudaStream_t)stream;
     P->ev_n = 0;
     // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
-    int nt = sht_plan_ntheta(P, 1), T2 = 4 * P->L - 1;
+    int nt = sht_plan_ntheta(P, 1), T2 = P->fwd_ld;
     CK(st_rows_reorder(P->L, P->NB, nt, nt, T2, 0, (const double2*)Wm, P->Z, st));
     double* saved = P->fwd.wq;
     P->fwd.wq = P->unit_wq;
@@ -574,6 +685,7 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     const int L = P->L, NB = P->NB;
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
+    if (P->sampling == SHT_HEALPIX) return healpix_synthesis(P, f, st);
     stage(P, CAT_FFT, st);
     CF(cufftSetStream(P->fft_phi_inv, st));
     double2* outc = P->reality ? P->cplx : (double2*)f;
@@ -588,6 +700,14 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB;
     P->ev_n = 0;
+    if (P->sampling == SHT_HEALPIX) {
+        CS(healpix_analysis(P, f, st));
+        CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
+        stage(P, CAT_STAGE, st);
+        CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H, (double2*)flm, st));
+        stage(P, CAT_STAGE, st);
+        return SHT_OK;
+    }
     const double2* fin = (const double2*)f;
     if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex((size_t)L * NB, (const double*)f, P->cplx, st)); fin = P->cplx; }
     stage(P, CAT_FFT, st);

@@ -22,3 +22,14 @@ cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole,
 cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st);
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st);
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st);
+
+// HEALPix ring Fourier staging (healpix.cu)
+void hp_ring_host(int nside, int i, int* nphi, int* shifted, long long* off);
+cudaError_t st_hp_chirp(int nside, int M, double2* BF, cudaStream_t st);
+cudaError_t st_hp_pack_fwd(int nside, int M, int real_in, const void* map, double2* C, cudaStream_t st);
+cudaError_t st_hp_mul(int nside, int M, const double2* BF, double2* C, cudaStream_t st);
+cudaError_t st_hp_unpack_fwd(int nside, int L, int NB, int mlo, int ldu, int M, const double2* C, const double2* E, double2* U,
+                             cudaStream_t st);
+cudaError_t st_hp_fold_inv(int nside, int L, int NB, int ldf, int M, const double2* F, double2* C, double2* E, cudaStream_t st);
+cudaError_t st_hp_unpack_inv(int nside, int M, int real_out, const double2* C, void* map, cudaStream_t st);
+cudaError_t st_hp_belt_real(size_t n, const double2* E, double* out, cudaStream_t st);

@@ -161,3 +161,36 @@ def test_inputs_are_not_modified_and_errors_are_loud(api):
         api.s2_inverse(d[:, :-1].contiguous(), L, 0)
     with pytest.raises(Exception):
         api.Plan(8, 9)
+
+
+# HEALPix: ring FFTs of variable length with phase shift, periodic extension / folding of F_m.
+# nside = 1 has no polar-cap rings; L > 4 nside - ... exercises aliasing (m >= nphi) on every ring; L = 2 nside is config 3's ratio.
+@pytest.mark.parametrize("nside,L,spin,real", [(1, 3, 0, False), (2, 4, 0, True), (2, 9, 0, False), (4, 8, 0, True), (4, 11, 2, False),
+                                               (8, 16, 0, True), (8, 16, -1, False), (16, 32, 0, True), (16, 40, 0, False), (32, 64, 0, True)])
+def test_healpix_vs_oracle(api, orc, nside, L, spin, real):
+    flm = synth.random_flm(L, spin, seed=nside + L, sigma=synth.SIGMA_RED, real=real)
+    P = api.Plan(L, spin, sampling=api.HEALPIX, nside=nside, reality=real)
+    f = P.inverse(dev(flm)).cpu().numpy()
+    f_ref = orc.s2_inverse(L, spin, orc.HEALPIX, flm, nside=nside)
+    assert f.shape == (12 * nside * nside,)
+    if real:
+        assert np.abs(f_ref.imag).max() < 1e-13 * np.abs(f_ref).max()
+        f_ref = f_ref.real.copy()
+    assert rel(f, f_ref) < TOL
+    # HEALPix has no sampling theorem: forward parity is against the oracle's forward of the same map
+    back = P.forward(dev(f_ref)).cpu().numpy()
+    want = orc.s2_forward(L, spin, orc.HEALPIX, f_ref.astype(np.complex128), nside=nside)
+    assert rel(back, want) < TOL
+    el = np.arange(L)[:, None]
+    m = np.arange(-(L - 1), L)[None, :]
+    assert np.all(back[(np.abs(m) > el) | (el < abs(spin))] == 0)
+
+
+def test_healpix_north_star_call_uses_nside_L_over_2(api, orc):
+    L = 16
+    flm = synth.random_flm(L, 0, seed=2, sigma=synth.SIGMA_RED, real=True)
+    f = api.s2_inverse(dev(flm), L, 0, sampling=api.HEALPIX, reality=True)
+    assert tuple(f.shape) == (12 * 8 * 8,)
+    assert rel(f.cpu().numpy(), orc.s2_inverse(L, 0, orc.HEALPIX, flm, nside=8).real) < TOL
+    back = api.s2_forward(f, L, 0, sampling=api.HEALPIX, reality=True).cpu().numpy()
+    assert rel(back, orc.s2_forward(L, 0, orc.HEALPIX, f.cpu().numpy().astype(np.complex128), nside=8)) < TOL
