@@ -1,0 +1,89 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times, on SAMPLED outputs the oracle
+can compute one by one (a few rings of the inverse, a few harmonic orders m of the forward), plus properties that hold
+at any size (exact MW round trip, zero pattern).  Forward inputs are white-noise maps from synth (the forward transform
+is defined by the algorithm for any input), never something the CUDA path produced."""
+import numpy as np
+import pytest
+
+from paper_2311_14670_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+TOL = 1e-11          # north_star: fp64 max|delta| / max|ref| <= 1e-11 up to L = 1024
+
+
+def rel(a, b, scale=None):
+    return float(np.abs(a - b).max() / (np.abs(b).max() if scale is None else scale))
+
+
+@pytest.fixture(scope="module")
+def api():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_14670_b200 import api as A
+    return A
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def test_config2_mw_L1024_spin2(api, orc):
+    """configs[1]: spin-2 complex SHT, MW L=1024, flm ~ N(0, 1/(l(l+1))), seed 1."""
+    L, spin = 1024, 2
+    flm = synth.random_flm(L, spin, seed=1, sigma=synth.SIGMA_CMB)
+    P = api.Plan(L, spin)
+    f = P.inverse(dev(flm))
+    back = P.forward(f).cpu().numpy()
+    f = f.cpu().numpy()
+    rings = np.array([0, 1, 37, 511, 700, 1022, 1023])              # incl. both near-pole rings and the theta = pi ring
+    rows = orc.s2_inverse_rings(L, spin, orc.MW, flm, rings)
+    scale = max(np.abs(r).max() for r in rows)
+    for r, row in zip(rings, rows):
+        assert rel(f[r], row, scale) < TOL, r
+    # sampling theorem (DESIGN.md pin 6): the round trip reproduces the generating coefficients
+    assert rel(back, flm) < TOL
+    # forward of a white-noise map against the oracle on sampled orders m
+    g = synth.random_map((L, 2 * L - 1), seed=11)
+    got = P.forward(dev(g)).cpu().numpy()
+    ms = np.array([-(L - 1), -700, -2, -1, 0, 1, 2, 3, 511, L - 1])
+    want = orc.s2_forward_columns(L, spin, orc.MW, g, ms)
+    sc = np.abs(want).max()
+    for m, col in zip(ms, want):
+        assert rel(got[:, m + L - 1], col, sc) < TOL, m
+
+
+def test_config3_healpix_nside1024_L2048_real(api, orc):
+    """configs[2]: spin-0 real SHT on HEALPix nside=1024, L=2048, sigma_l = 1/(l+1), seed 2."""
+    nside, L = 1024, 2048
+    flm = synth.random_flm(L, 0, seed=2, sigma=synth.SIGMA_RED, real=True)
+    P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=True)
+    f = P.inverse(dev(flm)).cpu().numpy()
+    tab = orc.ring_table(orc.HEALPIX, L, nside)
+    rings = np.array([0, 1, 2, 500, 1022, 1023, 1024, 2047, 2048, 3071, 3072, 4000, 4094])   # caps, belt edges, equator
+    rows = orc.s2_inverse_rings(L, 0, orc.HEALPIX, flm, rings, nside=nside)
+    scale = max(np.abs(r).max() for r in rows)
+    for r, row in zip(rings, rows):
+        o, n = int(tab["offset"][r]), int(tab["nphi"][r])
+        assert np.abs(row.imag).max() < 1e-12 * scale
+        assert rel(f[o:o + n], row.real, scale) < TOL, r
+    g = synth.random_map((12 * nside * nside,), seed=12, real=True)
+    got = P.forward(dev(g)).cpu().numpy()
+    ms = np.array([-2047, -3, 0, 1, 2, 1023, 2047])
+    want = orc.s2_forward_columns(L, 0, orc.HEALPIX, g.astype(np.complex128), ms, nside=nside)
+    sc = np.abs(want).max()
+    for m, col in zip(ms, want):
+        assert rel(got[:, m + L - 1], col, sc) < TOL, m
+
+
+def test_config4_so3_L256_N8(api, orc):
+    """configs[3]: Wigner transform, MW-SO3 sampling L=256, N=8, iid complex N(0,1), seed 3 -- full comparison."""
+    L, N = 256, 8
+    c = synth.random_flmn(L, N, seed=3)
+    P = api.Plan(L, N=N)
+    f = P.inverse(dev(c)).cpu().numpy()
+    f_ref = orc.so3_inverse(L, N, c)
+    assert rel(f, f_ref) < TOL
+    back = P.forward(dev(f_ref)).cpu().numpy()
+    assert rel(back, c) < TOL
+    g = synth.random_map((2 * N - 1, L, 2 * L - 1), seed=13)
+    assert rel(P.forward(dev(g)).cpu().numpy(), orc.so3_forward(L, N, g)) < TOL
