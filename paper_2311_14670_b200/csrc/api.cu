@@ -82,6 +82,9 @@ struct sht_plan {
     int kmin = 0, kstride = 0, krows = 0;
     int8_t* kexp = nullptr;
     double* rsq = nullptr;
+    int mmin = 0, sgstride = 0;    // lowest recursion step of any pass; columns of the (s, G) table
+    double* ctab = nullptr;        // [L - mmin][Lp] c_m(l)
+    double2* sgtab = nullptr;      // [Lp/TQ][sgstride]
     double *scale_inv = nullptr, *scale_fwd = nullptr;   // [Lp] l-dependent factors
     // pass lists (host copies + device arrays), split by kernel mode
     std::vector<PassHost> pinv, pfwd;
@@ -163,6 +166,8 @@ void layout(sht_plan* P, char* base) {
     const int L = P->L, Lp = P->Lp, NB = P->NB;
     P->rsq = B.take<double>(2 * (size_t)Lp + 64);
     P->kexp = B.take<int8_t>((size_t)P->krows * P->kstride);
+    P->ctab = B.take<double>((size_t)(L - P->mmin) * Lp);
+    P->sgtab = B.take<double2>((size_t)P->krows * P->sgstride);
     P->scale_inv = B.take<double>(Lp);
     P->scale_fwd = B.take<double>(Lp);
     for (RingSet* R : {&P->inv, &P->fwd}) {
@@ -178,9 +183,15 @@ void layout(sht_plan* P, char* base) {
     }
     P->d_inv_pm = B.take<ThetaPass>(P->pinv.size() + 1); P->d_inv_p = B.take<ThetaPass>(P->pinv.size() + 1);
     P->d_fwd_pm = B.take<ThetaPass>(P->pfwd.size() + 1); P->d_fwd_p = B.take<ThetaPass>(P->pfwd.size() + 1);
-    // per-pass operand buffers
-    for (auto& ph : P->pinv) ph.p.in = B.take<double2>((size_t)(L - ph.p.m_end) * Lp * (ph.mode == 0 ? 2 : 1));
-    for (auto& ph : P->pfwd) ph.p.in = B.take<double2>((size_t)(L - ph.p.m_end) * P->fwd.ntp * (ph.mode == 0 ? 2 : 1));
+    // per-pass operand buffers and lambda tables
+    for (auto& ph : P->pinv) {
+        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end) * Lp * theta_inverse_rowd(ph.mode));
+        ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end) * P->inv.ntp);
+    }
+    for (auto& ph : P->pfwd) {
+        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end) * P->fwd.ntp * (ph.mode == 0 ? 4 : 2));
+        ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end) * P->fwd.ntp);
+    }
     // scratch arrays
     P->F_slab = (size_t)NB * P->inv.ntp;
     P->F = B.take<double2>(P->F_slab * P->nslab);
@@ -285,7 +296,9 @@ sht_status plan_common(sht_plan* P) {
     for (int n : P->slab_n) nmax = (n < 0 ? -n : n) > nmax ? (n < 0 ? -n : n) : nmax;
     P->kmin = -(nmax + 2);
     P->kstride = (int)rup((size_t)P->Lp + SHT_TQ + (size_t)(-P->kmin) + 2, 16);
-    P->krows = P->Lp / SHT_TQ + 1;
+    P->krows = P->Lp / SHT_TQ;
+    P->mmin = -nmax;
+    P->sgstride = (int)rup((size_t)(L - P->mmin), 2);
     for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
     // d-step counts: rings * sum over l of the steps each pass runs
     for (int dir = 0; dir < 2; ++dir) {
@@ -363,6 +376,7 @@ sht_status upload_passes(sht_plan* P, cudaStream_t st) {
                 t.m_lo = R.mlo[2 * n_slab + (t.sgn_out > 0 ? 0 : 1)];
             } else t.m_lo = nullptr;
             ph.p = t;
+            CK(st_lamtab(t.n, R.nth, R.ntp, t.m_end, P->L - t.m_end, R.csc, R.tau, R.sig, const_cast<double*>(t.lam), st));
             (ph.mode == 0 ? pm : p).push_back(t);
         }
         ThetaPass* dpm = dir ? P->d_fwd_pm : P->d_inv_pm; ThetaPass* dp = dir ? P->d_fwd_p : P->d_inv_p;
@@ -379,13 +393,9 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     const RingSet& R = fwd ? P->fwd : P->inv;
     ThetaArgs a{};
     a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.NB = P->NB;
-    a.csc = R.csc; a.tau = R.tau; a.sig = R.sig;
-    a.kexp = P->kexp; a.kstride = P->kstride; a.kmin = P->kmin; a.rsq = P->rsq;
+    a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin; a.ctab = P->ctab;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
-    a.all_n_zero = 1;
-    for (auto& ph : (fwd ? P->pfwd : P->pinv))
-        if ((ph.mode == 0) == pm && ph.p.n != 0) a.all_n_zero = 0;
     return a;
 }
 
@@ -395,8 +405,8 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
     const int L = P->L;
     stage(P, CAT_STAGE, st);
     for (auto& ph : P->pinv)
-        CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, coef + (size_t)ph.p.slab * L * P->NB,
-                           P->scale_inv, const_cast<double2*>(ph.p.in), st));
+        CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->NB,
+                           P->scale_inv, P->ctab, P->sgtab, P->sgstride, const_cast<double*>(ph.p.in), st));
     CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
     CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
@@ -420,7 +430,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     for (auto& ph : P->pfwd) {
         int n_slab = P->slab_n[ph.p.slab];
         CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.m_lo,
-                           P->fwd.wq, U + U_slab * ph.p.slab, const_cast<double2*>(ph.p.in), st));
+                           P->fwd.wq, U + U_slab * ph.p.slab, reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)), st));
     }
     CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
@@ -569,6 +579,8 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     const int L = P->L, Lp = P->Lp;
     CK(st_rsq(2 * Lp + 64, P->rsq, st));
     CK(st_kexp(P->krows, P->kstride, P->kmin, P->kexp, st));
+    CK(st_ctab(L, Lp, P->mmin, P->kstride, P->kmin, P->kexp, P->rsq, P->ctab, st));
+    CK(st_sgtab(P->krows, P->sgstride, P->mmin, P->kstride, P->kmin, P->kexp, P->sgtab, st));
     std::vector<double> si(Lp, 0.0), sf(Lp, 0.0);
     for (int l = 0; l < L; ++l) {
         if (P->kind == 0) {

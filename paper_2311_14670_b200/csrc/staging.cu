@@ -82,6 +82,41 @@ __global__ void k_rsq(int n, double* __restrict__ rsq) {
     if (k < n) rsq[k] = k > 0 ? 1.0 / sqrt((double)k) : 0.0;
 }
 
+// c_m(l) table (internal.h): C[m - mmin][Lp]; c_l = 1, c_{m-1} = c_m a_{m-1}(l) 2^{k_m} = c_m 2^{k_m+1} / sqrt((l-m+1)(l+m)).
+// One thread per degree, sequential in m (an O(L^2) plan-time table, independent of the rings and of n).
+__global__ void k_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* __restrict__ kexp,
+                       const double* __restrict__ rsq, double* __restrict__ C) {
+    int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= Lp) return;
+    for (int m = L - 1; m > l || (l >= L && m >= mmin); --m) C[(size_t)(m - mmin) * Lp + l] = 0.0;
+    if (l >= L) return;
+    const int8_t* kr = kexp + (size_t)(l / SHT_TQ) * kstride - kmin;
+    double c = 1.0;
+    for (int m = l; m >= mmin; --m) {
+        C[(size_t)(m - mmin) * Lp + l] = c;
+        if (m > mmin) c = (l + m > 0) ? c * ldexp(1.0, kr[m] + 1) * rsq[l - m + 1] * rsq[l + m] : 0.0;
+    }
+}
+// (s_m, G_m) = (2^{-k_m}, 2^{-2-k_m-k_{m+1}}) per quantum row, column m - mmin
+__global__ void k_sgtab(int nrows, int ncol, int mmin, int kstride, int kmin, const int8_t* __restrict__ kexp, double2* __restrict__ SG) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
+    if (c >= ncol || row >= nrows) return;
+    const int m = mmin + c;
+    const int8_t* kr = kexp + (size_t)row * kstride - kmin;
+    SG[(size_t)row * ncol + c] = make_double2(ldexp(1.0, -kr[m]), ldexp(1.0, -2 - kr[m] - kr[m + 1]));
+}
+// lambda_m(theta) = (n - m cos theta)/sin theta, evaluated without cancellation (R8) as
+// (n - sigma m) csc + m tau;  table [m - m_end][ntp] for one second index n
+__global__ void k_lamtab(int n, int nth, int ntp, int m_end, const double* __restrict__ csc, const double* __restrict__ tau,
+                         const double* __restrict__ sig, double* __restrict__ lam) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = m_end + blockIdx.y;
+    if (th >= ntp) return;
+    double v = 0.0;
+    if (th < nth) v = fma((double)n - sig[th] * (double)m, csc[th], (double)m * tau[th]);
+    lam[(size_t)(m - m_end) * ntp + th] = v;
+}
+
 // MW theta-quadrature weights at band-limit Lq (closed form of Eq. 41-44 with reflection sign +1, R9):
 //   v_u = (zeta_u/(2Lq-1)) sum_{|2j|<=Lq-1} 4 cos(2j theta_u)/(1-4j^2),  theta_u = (2u+1)pi/(2Lq-1);  times qphi.
 __global__ void k_mw_weights(int Lq, double qphi, double* __restrict__ w) {
@@ -101,24 +136,39 @@ __global__ void k_mw_weights(int Lq, double qphi, double* __restrict__ w) {
 }
 
 // ---- per-transform staging ------------------------------------------------------------------------------------
-// inverse prep: coef[slab_in][L][NB] -> G[m-m_end][Lp][NC] of one pass, scaled by scale[l] and the pass sign.
-__global__ void k_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, const double2* __restrict__ coef,
-                               const double* __restrict__ scale, double2* __restrict__ G) {
-    int l = blockIdx.x * blockDim.x + threadIdx.x;
-    int m = m_end + blockIdx.y;
-    if (l >= Lp) return;
-    const int an = n < 0 ? -n : n, am = m < 0 ? -m : m, NB = 2 * L - 1;
-    for (int c = 0; c < NC; ++c) {
-        double2 v = {0.0, 0.0};
-        if (l < L && l >= an && l >= am && !(c == 1 && m == 0)) {
-            int m_out = (c == 1 || sgn_out < 0) ? -m : m;
-            double s = scale[l];
-            if (c == 1) s *= sgn_pow(m);
-            else if (sgn_out < 0) s *= sgn_pow(m + n);
-            double2 x = coef[(size_t)l * NB + m_out + L - 1];
-            v.x = s * x.x; v.y = s * x.y;
+// inverse prep: coef[l][NB] -> operand rows G[m-m_end][Lp][ROWD] of one pass: {c Re, c Im (x NC), g'_m(l), s_m} with
+// c = scale(l) * sign * c_m(l) (internal.h), through a 32x32 shared-memory transpose (coef is l-major, G is m-major).
+__global__ void k_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* __restrict__ coef,
+                               const double* __restrict__ scale, const double* __restrict__ C, const double2* __restrict__ SG,
+                               int sgstride, double* __restrict__ G) {
+    __shared__ double2 tile[2][32][33];
+    const int NB = 2 * L - 1, an = n < 0 ? -n : n, ROWD = 2 * NC + 2;
+    const int l0 = blockIdx.x * 32, m0 = m_end + blockIdx.y * 32;
+    for (int c = 0; c < NC; ++c)
+        for (int q = threadIdx.y; q < 32; q += blockDim.y) {          // read: rows l, columns m_out (contiguous)
+            const int l = l0 + q, m = m0 + threadIdx.x;
+            const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
+            double2 v = make_double2(0.0, 0.0);
+            const int am = m < 0 ? -m : m;
+            if (l < L && m < L && l >= an && l >= am && !(c == 1 && m == 0)) v = coef[(size_t)l * NB + m_out + L - 1];
+            tile[c][q][threadIdx.x] = v;
         }
-        G[((size_t)(m - m_end) * Lp + l) * NC + c] = v;
+    __syncthreads();
+    for (int q = threadIdx.y; q < 32; q += blockDim.y) {              // write: rows m, columns l (contiguous)
+        const int m = m0 + q, l = l0 + threadIdx.x;
+        if (m >= L || l >= Lp) continue;
+        double* g = G + ((size_t)(m - m_end) * Lp + l) * ROWD;
+        const double2 sg = SG[(size_t)(l / SHT_TQ) * sgstride + (m - mmin)];
+        const double cm = l < L ? scale[l] * C[(size_t)(m - mmin) * Lp + l] : 0.0;
+        for (int c = 0; c < NC; ++c) {
+            double sgn = 1.0;
+            if (c == 1) sgn = sgn_pow(m);
+            else if (sgn_out < 0) sgn = sgn_pow(m + n);
+            const double2 x = tile[c][threadIdx.x][q];
+            g[2 * c] = sgn * cm * x.x; g[2 * c + 1] = sgn * cm * x.y;
+        }
+        g[2 * NC] = l < L ? (double)(l - m) * (double)(l + m + 1) * sg.y : 0.0;
+        g[2 * NC + 1] = sg.x;
     }
 }
 // pole ring theta = pi, inverse (Eq. 29): F_{-n}(pi) = sum_l scale(l) f_{l,-n} (-1)^{l-n}.  One block per slab.
@@ -283,10 +333,23 @@ cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st) {
     k_mw_weights<<<cdiv(Lq, 128), 128, 0, st>>>(Lq, qphi, w);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, const double2* coef, const double* scale,
-                            double2* G, cudaStream_t st) {
-    dim3 grid(cdiv(Lp, 128), L - m_end);
-    k_prep_inverse<<<grid, 128, 0, st>>>(L, Lp, NC, n, sgn_out, m_end, coef, scale, G);
+cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* coef, const double* scale,
+                            const double* C, const double2* SG, int sgstride, double* G, cudaStream_t st) {
+    dim3 grid(cdiv(Lp, 32), cdiv(L - m_end, 32)), block(32, 8);
+    k_prep_inverse<<<grid, block, 0, st>>>(L, Lp, NC, n, sgn_out, m_end, mmin, coef, scale, C, SG, sgstride, G);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* kexp, const double* rsq, double* C, cudaStream_t st) {
+    k_ctab<<<cdiv(Lp, 64), 64, 0, st>>>(L, Lp, mmin, kstride, kmin, kexp, rsq, C);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_sgtab(int nrows, int ncol, int mmin, int kstride, int kmin, const int8_t* kexp, double2* SG, cudaStream_t st) {
+    k_sgtab<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(nrows, ncol, mmin, kstride, kmin, kexp, SG);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_lamtab(int n, int nth, int ntp, int m_end, int nrows, const double* csc, const double* tau, const double* sig, double* lam,
+                      cudaStream_t st) {
+    k_lamtab<<<dim3(cdiv(ntp, 128), nrows), 128, 0, st>>>(n, nth, ntp, m_end, csc, tau, sig, lam);
     LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_pole_inverse(int L, int n, const double2* coef, const double* scale, double2* out, cudaStream_t st) {

@@ -2,15 +2,19 @@
 // contraction of Eq. 30 (forward, sum over rings) and Eq. 33 (inverse, sum over l) -- "interleaving recursion and
 // computation", Sec. 4.4.  d-values live only in registers; nothing O(L^3) touches memory.
 //
-// Thread mapping; every thread carries an RL x RT register tile of (l, ring) items:
-//   inverse: lane <-> ring (theta0 + lane + 32 i), registers <-> RL consecutive degrees, warps <-> further l-chunks.
-//            sum_l = in-thread FMA chain + shared-memory reduction over warps + RED.ADD.F64 over l-tiles.
-//   forward: lane <-> degree (l0 + lane + 32 r), registers <-> RT consecutive rings, warps <-> further ring chunks.
-//            sum_theta = in-thread FMA chain + shared-memory reduction over warps + RED.ADD.F64 over ring tiles.
-// One d-step is 1 DMUL + 1 DFMA (internal.h); the projection is 2 (one order) or 4 (both +-m) DFMA.  Operands that
-// are uniform across a warp (coefficients, weighted F_m, lambda', g') are read as shared-memory broadcasts, one
-// read serving RT (inverse) or RL (forward) items.  Per-step operand tiles arrive through 1-D TMA bulk copies
-// (cp.async.bulk + mbarrier) into a 4-stage ring; one __syncthreads per recursion step.
+// Structure.  One CTA per SM: NW = 8 compute warps + 4 auxiliary warps (register budgets re-split
+// with setmaxnreg: 232 / 40 per thread), no block-wide barrier in the m-loop.
+//   compute warps: every thread carries an RL x RT register tile of (l, ring) items, 32 items, and per recursion
+//       step does 1 DMUL + 1 DFMA (recursion, internal.h) and 2 (one order) or 4 (+-m) DFMA (projection) per item.
+//       Operands that are uniform across the warp are shared-memory broadcasts.
+//       inverse: lane <-> ring, registers <-> RL degrees x RT rings;  sum_l = in-thread FMA chains over RL degrees
+//       forward: lane <-> degree, registers <-> RL degrees x RT rings; sum_theta = in-thread FMA chains over RT rings
+//   auxiliary warp: (1) streams the per-step operand rows into a 4-stage ring with 1-D TMA bulk copies
+//       (cp.async.bulk + mbarrier complete_tx), (2) forward only: scales the lambda row by the step's power of two,
+//       (3) adds the per-warp partial sums of every step and issues RED.ADD.F64 to the output rows.
+//   compute <-> auxiliary hand-off is a two-stage mbarrier pipeline (rfull / rempty); operand slots are recycled by the
+//       auxiliary warp right after the reduction of the step that used them.
+// All (l,m)-only and (theta,m)-only factors arrive as O(L^2) tables prepared by staging.cu.
 #include "internal.h"
 
 #include <cuda_runtime.h>
@@ -25,6 +29,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
 __device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
@@ -41,8 +48,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
             : "memory");
     } while (!ok);
 }
-// fire-and-forget fp64 add to GLOBAL memory (RED.E.ADD.F64); atomicAdd on a generic pointer compiles to an
-// address-space dispatch with CAS fallbacks
+// fire-and-forget fp64 add to GLOBAL memory (RED.E.ADD.F64)
 __device__ __forceinline__ void red_add_f64(double* gptr, double v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gptr), "d"(v) : "memory");
 }
@@ -54,8 +60,14 @@ __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7
 #define HI_DEAD ((1023 + 500) << 20)
 
 constexpr int NST = 4;   // stages of the operand ring
+constexpr int NRS = 2;   // stages of the partial-sum hand-off
+constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
+// The register file is split over the 4 SM sub-partitions (16 K registers each, 3 warps each here): compute warps take
+// 232 registers per thread, auxiliary warps 40 (2*32*232 + 32*40 = 16128); the kernel is launched at 168.
+__device__ __forceinline__ void reg_dealloc_aux() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
+__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
 
-// Window counters k (internal.h) of the NI items of a thread, one byte each.
+// Window counters k (internal.h) of the NI items of a thread, one byte each.  0xff = item not started yet.
 template <int NI>
 struct KPack {
     uint32_t w[(NI + 3) / 4];
@@ -94,7 +106,7 @@ __device__ __forceinline__ void window_check(double (&cur)[NI], double (&prev)[N
     }
 }
 // On rings a pass no longer serves (m < m_lo, R5) the iterate leaves its stable range; it is zeroed before it
-// can overflow.  Legitimate stored values never exceed ~2.
+// can overflow.  Legitimate stored values never exceed ~2^250.
 template <int NI>
 __device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]) {
 #pragma unroll
@@ -103,156 +115,157 @@ __device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]
 }
 
 // =============================================================================================================
-// inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * d^l_{m,n}(theta)
+// inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * e^l_m(theta)      (G carries c_m(l))
+// block tile: TL = NW*RL degrees x NTH = 32*RT rings
 // =============================================================================================================
 template <int RL, int RT, int NW, int NC>
 struct InvSmem {
-    static constexpr int TL = NW * RL, NTH = 32 * RT, SCW = (NC == 2) ? 6 : 4;
-    double2 ctile[NST][TL * NC];        // raw coefficient tiles (TMA ring)
-    double sc[2][TL][SCW];              // per step: coefficients * c_m(l), then g'_m(l)
-    double red[2][NW][NTH][2 * NC];     // per-warp partial sums
-    double stv[TL][NTH];                // start values of the block's (l, ring) tile
-    uint8_t stk[TL][NTH];
-    uint64_t bar[NST + 1];
+    static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2;
+    double op[NST][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
+    double lam[NST][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
+    double red[NRS][NW][NTH][2 * NC];   // per-warp partial sums
+    int act[NRS][NW];                   // warp wrote partial sums at this step
+    uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
-template <int RL, int RT, int NW, int NC, bool SPIN0>
-__global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kernel(const ThetaArgs A) {
+template <int RL, int RT, int NW, int NC>
+__global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(const ThetaArgs A) {
     using S = InvSmem<RL, RT, NW, NC>;
-    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT;
+    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD;
+    static_assert(TL == SHT_TQ, "the block's degrees must be one kappa quantum");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
     const ThetaPass P = A.passes[blockIdx.y];
     const int ntt = A.ntp / NTH, nlt = A.Lp / TL;
-    const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
+    const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;     // heavy (large-l) tiles first
     const int l0 = lt * TL, th0 = tt * NTH;
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TL <= an || l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end;
-    const int la = l0 + w * RL;                       // first degree of this warp
-    constexpr uint32_t tile_bytes = TL * NC * sizeof(double2);
+    const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end, nsteps = mtop - m_end + 1;
 
     if (tid == 0) {
-        for (int i = 0; i <= NST; ++i) mbar_init(&sm.bar[i], 1);
+        for (int i = 0; i < NST; ++i) mbar_init(&sm.full[i], 1);
+        for (int i = 0; i < NRS; ++i) { mbar_init(&sm.rfull[i], NW); mbar_init(&sm.rempty[i], NAUX); }
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == 0) {
-        mbar_expect_tx(&sm.bar[NST], TL * NTH * 9);
-        for (int r = 0; r < TL; ++r) {
-            bulk_g2s(&sm.stv[r][0], P.st_val + (size_t)(l0 + r) * A.ntp + th0, NTH * 8, &sm.bar[NST]);
-            bulk_g2s(&sm.stk[r][0], P.st_k + (size_t)(l0 + r) * A.ntp + th0, NTH, &sm.bar[NST]);
-        }
-        for (int it = 0; it < NST; ++it) {
-            int m = mtop - it;
-            if (m >= m_end) {
-                mbar_expect_tx(&sm.bar[it], tile_bytes);
-                bulk_g2s(&sm.ctile[it][0], P.in + ((size_t)(m - m_end) * A.Lp + l0) * NC, tile_bytes, &sm.bar[it]);
-            }
-        }
-    }
-    // ---- ring constants: lambda'_m = S_m * ((n - sig m) csc + m tau)   [= S_m * m * (tau - sig csc) when n = 0]
-    double rc0[RT], rc1[RT];
-    bool north[RT];
+
+    if (w >= NW) {
+        // ---------------------------------------------------------------- auxiliary warps: TMA producer + reducers
+        reg_dealloc_aux();
+        const int at = tid - NW * 32;                 // 0..127: owns outputs at, at+128, ... of the NOUT per step
+        constexpr int NOUT = NTH * 2 * NC, NQ = NOUT / (NAUX * 32);
+        constexpr uint32_t op_bytes = TL * ROWD * sizeof(double), lam_bytes = NTH * sizeof(double);
+        auto issue = [&](int it) {
+            const int m = mtop - it, slot = it & (NST - 1);
+            mbar_expect_tx(&sm.full[slot], op_bytes + lam_bytes);
+            bulk_g2s(&sm.op[slot][0], P.in + ((size_t)(m - m_end) * A.Lp + l0) * ROWD, op_bytes, &sm.full[slot]);
+            bulk_g2s(&sm.lam[slot][0], P.lam + (size_t)(m - m_end) * A.ntp + th0, lam_bytes, &sm.full[slot]);
+        };
+        if (at == 0)
+            for (int it = 0; it < NST && it < nsteps; ++it) issue(it);
+        int mlo[NQ], comp[NQ];
+        bool valid[NQ];
+        double* obase[NQ];
 #pragma unroll
-    for (int i = 0; i < RT; ++i) {
-        const int th = th0 + lane + 32 * i;
-        const double csc = A.csc[th], tau = A.tau[th], sg = A.sig[th];
-        north[i] = sg > 0.0;
-        if (SPIN0) { rc0[i] = tau - sg * csc; rc1[i] = 0.0; }
-        else { rc0[i] = csc; rc1[i] = tau; }
+        for (int q = 0; q < NQ; ++q) {
+            const int o = at + NAUX * 32 * q, th = th0 + o / (2 * NC);
+            comp[q] = o % (2 * NC);
+            valid[q] = th < A.nth;
+            mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
+            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2 + (comp[q] & 1);
+        }
+        for (int it = 0; it < nsteps; ++it) {
+            const int m = mtop - it, rs = it & (NRS - 1);
+            mbar_wait(&sm.rfull[rs], (it / NRS) & 1);
+            double v[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) v[q] = 0.0;
+            bool any = false;
+#pragma unroll
+            for (int ww = 0; ww < NW; ++ww) {
+                if (sm.act[rs][ww]) {
+                    any = true;
+                    const double* r = &sm.red[rs][ww][0][0] + at;
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) v[q] += r[NAUX * 32 * q];
+                }
+            }
+            if (any) {
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    const bool neg = NC == 2 && (comp[q] >> 1);
+                    if (valid[q] && m >= mlo[q] && !(neg && m == 0)) {
+                        const int m_out = (NC == 2) ? (neg ? -m : m) : P.sgn_out * m;
+                        const int row = m_out < 0 ? m_out + A.NB : m_out;
+                        red_add_f64(obase[q] + (size_t)row * A.ntp * 2, v[q]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.rempty[rs]);
+            if (at == 0 && it + NST < nsteps) issue(it + NST);   // every compute warp has finished step `it`: its slot is free
+        }
+        return;
     }
+    reg_alloc_compute();
+
+    // -------------------------------------------------------------------- compute warps
+    const int la = l0 + w * RL, l_hi = la + RL - 1;   // degrees of this warp
+    const bool warp_real = la < A.L;
     double cur[NI], prev[NI];
     KPack<NI> kp;
-    kp.fill(0xffffffffu);                             // 0xff = not started yet
+    kp.fill(0xffffffffu);
 #pragma unroll
     for (int q = 0; q < NI; ++q) { cur[q] = 0.0; prev[q] = 0.0; }
-    bool wact = false;                                // any item of this warp with k == 0 (contributes)
-    // kappa exponents of this warp's l-chunk (l_top = la + RL rounded up to a multiple of TQ)
-    const int8_t* krow = A.kexp + (size_t)((la + RL + SHT_TQ - 1) / SHT_TQ - 1) * A.kstride - A.kmin;
-    const double fn = (double)P.n;
+    bool wact = false;                                // some item of this warp has k == 0 (its contribution matters)
+    const double* stv = P.st_val + (size_t)la * A.ntp + th0 + lane;
+    const uint8_t* stk = P.st_k + (size_t)la * A.ntp + th0 + lane;
 
-    // ---- helper threads: one per degree of the block, they prepare sc[] one step ahead
-    constexpr int HB = (NW * 32 >= 2 * TL) ? NW * 32 - TL : 0;      // last TL threads
-    const bool is_helper = tid >= HB && tid < HB + TL;
-    const int hl = tid - HB, lh = l0 + hl;
-    const int8_t* krow_h = A.kexp + (size_t)((l0 + (hl / RL) * RL + RL + SHT_TQ - 1) / SHT_TQ - 1) * A.kstride - A.kmin;
-    double cfac = 1.0;
-    auto helper = [&](int m, unsigned it) {           // prepares sc[it & 1] for recursion step m
-        const unsigned slot = it & (NST - 1);
-        mbar_wait(&sm.bar[slot], (it / NST) & 1);
-        if (lh > m && lh >= an) cfac *= pow2i(krow_h[m + 1] + 1) * A.rsq[lh - m] * A.rsq[lh + m + 1];   // c_{m} from c_{m+1}
-        const double2* raw = &sm.ctile[slot][hl * NC];
-        double* s = &sm.sc[it & 1][hl][0];
-        const double2 c0 = raw[0];
-        s[0] = c0.x * cfac; s[1] = c0.y * cfac;
-        if (NC == 2) { const double2 c1 = raw[1]; s[2] = c1.x * cfac; s[3] = c1.y * cfac; }
-        s[2 * NC] = (double)(lh - m) * (double)(lh + m + 1) * pow2i(-2 - krow_h[m] - krow_h[m + 1]);
-    };
-    if (is_helper) helper(mtop, 0);
-    mbar_wait(&sm.bar[NST], 0);
-    __syncthreads();
-
-    // reducer constants: output base as a global-space address, last warp holding real degrees, per-output m_lo
-    double* const out_g = reinterpret_cast<double*>(P.out);
-    int wmax_blk = (A.L - 1 - l0) / RL; if (wmax_blk > NW - 1) wmax_blk = NW - 1;
-    constexpr int NRED = (2 * NC * NTH + NW * 32 - 1) / (NW * 32);
-    int mlo_red[NRED];
-#pragma unroll
-    for (int q = 0; q < NRED; ++q) {
-        const int o = tid + q * NW * 32;
-        mlo_red[q] = (P.m_lo && o < 2 * NC * NTH) ? P.m_lo[th0 + o / (2 * NC)] : -(1 << 30);
-    }
-    // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step,
-    // so the iterates never move between registers)
-    auto step = [&](const int m, double (&ca)[NI], double (&cb)[NI]) {
-        const unsigned it = (unsigned)(mtop - m);
-        const bool warp_on = (m <= la + RL - 1) && (la < A.L);
-        if (warp_on) {
-            if (m >= la) {                            // ramp: the degree l == m starts (warp-uniform)
+    // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step, so the
+    // iterates never move between registers)
+    auto step = [&](const int it, double (&ca)[NI], double (&cb)[NI]) {
+        const int m = mtop - it, slot = it & (NST - 1), rs = it & (NRS - 1);
+        mbar_wait(&sm.full[slot], (it / NST) & 1);
+        int flag = 0;
+        if (m <= l_hi && warp_real) {
+            if (m >= la) {                            // the degree l == m starts (warp-uniform): Eq. 27 start values
 #pragma unroll
                 for (int j = 0; j < RL; ++j) {
                     if (m == la + j) {
 #pragma unroll
                         for (int i = 0; i < RT; ++i) {
-                            ca[j * RT + i] = sm.stv[w * RL + j][lane + 32 * i];
+                            ca[j * RT + i] = stv[(size_t)j * A.ntp + 32 * i];
                             cb[j * RT + i] = 0.0;
-                            kp.set(j * RT + i, sm.stk[w * RL + j][lane + 32 * i]);
+                            kp.set(j * RT + i, stk[(size_t)j * A.ntp + 32 * i]);
                         }
                     }
                 }
                 wact = true;                          // re-evaluated at the next window check
             }
-            const int km = krow[m];
+            const double* row = &sm.op[slot][(w * RL) * ROWD];
+            const double s = row[ROWD - 1];
             double lam[RT];
-            {
-                const double smul = pow2i(-km), fm = (double)m;
-                if (SPIN0) {
-                    const double v = fm * smul;
 #pragma unroll
-                    for (int i = 0; i < RT; ++i) lam[i] = v * rc0[i];
-                } else {
-                    const double un = (fn - fm) * smul, us = (fn + fm) * smul, v = fm * smul;
-#pragma unroll
-                    for (int i = 0; i < RT; ++i) lam[i] = fma(north[i] ? un : us, rc0[i], v * rc1[i]);
-                }
-            }
-            double acc[RT][2 * NC];
-#pragma unroll
-            for (int i = 0; i < RT; ++i)
-#pragma unroll
-                for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
-            const double* scw = &sm.sc[it & 1][w * RL][0];
+            for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][lane + 32 * i] * s;
             if (wact) {
+                double acc[RT][2 * NC];
+#pragma unroll
+                for (int i = 0; i < RT; ++i)
+#pragma unroll
+                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
 #pragma unroll
                 for (int j = 0; j < RL; ++j) {
-                    const double* s = scw + j * S::SCW;
+                    const double* r = row + j * ROWD;
                     double cf[2 * NC];
-                    { const double2 t0 = *reinterpret_cast<const double2*>(s); cf[0] = t0.x; cf[1] = t0.y; }
-                    if (NC == 2) { const double2 t1 = *reinterpret_cast<const double2*>(s + 2); cf[2] = t1.x; cf[3] = t1.y; }
-                    const double g = s[2 * NC];
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) {
+                        const double2 t = *reinterpret_cast<const double2*>(r + 2 * c);
+                        cf[2 * c] = t.x; cf[2 * c + 1] = t.y;
+                    }
+                    const double g = r[2 * NC];
 #pragma unroll
                     for (int i = 0; i < RT; ++i) {
                         const double e = ca[j * RT + i];
@@ -261,10 +274,17 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kern
                         cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
                     }
                 }
-            } else {                                  // every item of the warp is still below 2^-140: recursion only
+                mbar_wait(&sm.rempty[rs], ((it / NRS) & 1) ^ 1);      // the reducer is done with this slot's previous use
+                double2* rd = reinterpret_cast<double2*>(&sm.red[rs][w][0][0]);
+#pragma unroll
+                for (int i = 0; i < RT; ++i)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) rd[(lane + 32 * i) * NC + c] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
+                flag = 1;
+            } else {                                  // every item of the warp is still below 2^-340: recursion only
 #pragma unroll
                 for (int j = 0; j < RL; ++j) {
-                    const double g = scw[j * S::SCW + 2 * NC];
+                    const double g = row[j * ROWD + 2 * NC];
 #pragma unroll
                     for (int i = 0; i < RT; ++i) cb[j * RT + i] = fma(lam[i], ca[j * RT + i], -(g * cb[j * RT + i]));
                 }
@@ -274,59 +294,44 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_inverse_kern
                 if (P.m_lo) dead_check<NI>(cb, ca);
                 if (m < la) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
             }
-            double2* r = reinterpret_cast<double2*>(&sm.red[it & 1][w][0][0]);
-#pragma unroll
-            for (int i = 0; i < RT; ++i)
-#pragma unroll
-                for (int c = 0; c < NC; ++c) r[(lane + 32 * i) * NC + c] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
         }
-        if (is_helper && m > m_end) helper(m - 1, it + 1);
-        __syncthreads();
-        if (tid == 0 && m - NST >= m_end) {
-            mbar_expect_tx(&sm.bar[it & (NST - 1)], tile_bytes);
-            bulk_g2s(&sm.ctile[it & (NST - 1)][0], P.in + ((size_t)(m - NST - m_end) * A.Lp + l0) * NC, tile_bytes, &sm.bar[it & (NST - 1)]);
-        }
-        // ---- reduce over the warps that were active at this step, add into F (thread <-> (ring, component))
-#pragma unroll
-        for (int q = 0; q < NRED; ++q) {
-            const int o = tid + q * NW * 32;
-            if (o >= 2 * NC * NTH) break;
-            const int c = o % (2 * NC), tl = o / (2 * NC), th = th0 + tl;
-            int wmin = (m - l0) / RL; if (wmin < 0) wmin = 0;
-            double v = 0.0;
-            const double* r = &sm.red[it & 1][0][0][0] + o;
-            for (int ww = wmin; ww <= wmax_blk; ++ww) v += r[ww * (2 * NC) * NTH];
-            const int m_out = (NC == 2) ? ((c >> 1) ? -m : m) : P.sgn_out * m;
-            const bool ok = th < A.nth && !(NC == 2 && (c >> 1) && m == 0) && m >= mlo_red[q];
-            if (ok) {
-                const int row = m_out < 0 ? m_out + A.NB : m_out;
-                red_add_f64(out_g + ((size_t)row * A.ntp + th) * 2 + (c & 1), v);
-            }
+        __syncwarp();
+        if (lane == 0) {
+            // never arrive on a phase before the previous use of the slot has been consumed (a warp that writes nothing
+            // must not run ahead either: its arrival would be counted in the wrong phase)
+            if (!flag) mbar_wait(&sm.rempty[rs], ((it / NRS) & 1) ^ 1);
+            sm.act[rs][w] = flag;
+            mbar_arrive(&sm.rfull[rs]);
         }
     };
-    for (int m = mtop; m >= m_end; m -= 2) {
-        step(m, cur, prev);
-        if (m - 1 >= m_end) step(m - 1, prev, cur);
+    for (int it = 0; it < nsteps; it += 2) {
+        step(it, cur, prev);
+        if (it + 1 < nsteps) step(it + 1, prev, cur);
     }
 }
 
 // =============================================================================================================
 // forward theta step, Eq. 30:  H[m_out+L-1][l] += c_m(l) * sum_theta W[m][theta] * e^l_m(theta)
+// block tile: TLB = 32*RL degrees x NTB = NW*RT rings
 // =============================================================================================================
 template <int RL, int RT, int NW, int NC>
 struct FwdSmem {
     static constexpr int TLB = 32 * RL, NTB = NW * RT;
-    double2 wtile[NST][NTB * NC];       // weighted F_m tiles (TMA ring)
-    double hdr[2][NTB + 2];             // per step: lambda'_m(theta) for the block's rings, then 2^{-2-k_m-k_{m+1}}
-    double red[2][NW][TLB][2 * NC];     // per-warp partial sums
-    uint64_t bar[NST];
+    double2 wt[NST][NTB * NC];          // weighted F_m samples of the block's rings (TMA ring)
+    double lamraw[NST][NTB];            // lambda_m(theta) (TMA ring)
+    double2 sg[NST];                    // (s_m, G_m) of the block's quantum (TMA ring)
+    double hdr[NST][NTB];               // lambda'_m = lambda_m s_m (written by the auxiliary warp)
+    double red[NRS][NW][TLB][2 * NC];   // per-warp partial sums
+    int act[NRS][NW];
+    uint64_t full[NST], ready[NST], rfull[NRS], rempty[NRS];
 };
 
 template <int RL, int RT, int NW, int NC>
-__global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kernel(const ThetaArgs A) {
+__global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(const ThetaArgs A) {
     using S = FwdSmem<RL, RT, NW, NC>;
     constexpr int TLB = S::TLB, NTB = S::NTB, NI = RL * RT;
-    static_assert(NW * 32 >= TLB + NTB + 1 || NW * 32 >= TLB, "block too small for reducer + producer roles");
+    static_assert(TLB == SHT_TQ, "the block's degrees must be one kappa quantum");
+    static_assert(RT % 2 == 0, "RT must be even (lambda' is read in pairs)");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
@@ -337,39 +342,101 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end;
-    constexpr uint32_t tile_bytes = NTB * NC * sizeof(double2);
+    const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end, nsteps = mtop - m_end + 1;
+
     if (tid == 0) {
-        for (int i = 0; i < NST; ++i) mbar_init(&sm.bar[i], 1);
+        for (int i = 0; i < NST; ++i) { mbar_init(&sm.full[i], 1); mbar_init(&sm.ready[i], 1); }
+        for (int i = 0; i < NRS; ++i) { mbar_init(&sm.rfull[i], NW); mbar_init(&sm.rempty[i], NAUX); }
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == 0) {
-        for (int it = 0; it < NST; ++it) {
-            int m = mtop - it;
-            if (m >= m_end) {
-                mbar_expect_tx(&sm.bar[it], tile_bytes);
-                bulk_g2s(&sm.wtile[it][0], P.in + ((size_t)(m - m_end) * A.ntp + th0) * NC, tile_bytes, &sm.bar[it]);
-            }
+
+    if (w >= NW) {
+        // ---------------------------------------------------------------- auxiliary warps
+        reg_dealloc_aux();
+        const int at = tid - NW * 32, aw = w - NW;
+        constexpr int NOUT = TLB * 2 * NC, NQ = NOUT / (NAUX * 32);
+        constexpr uint32_t wt_bytes = NTB * NC * sizeof(double2), lam_bytes = NTB * sizeof(double);
+        const double2* sgrow = A.sg + (size_t)lt * A.sgstride - A.mmin;
+        auto issue = [&](int it) {
+            const int m = mtop - it, slot = it & (NST - 1);
+            mbar_expect_tx(&sm.full[slot], wt_bytes + lam_bytes + (uint32_t)sizeof(double2));
+            bulk_g2s(&sm.wt[slot][0], P.in + ((size_t)(m - m_end) * A.ntp + th0) * 2 * NC, wt_bytes, &sm.full[slot]);
+            bulk_g2s(&sm.lamraw[slot][0], P.lam + (size_t)(m - m_end) * A.ntp + th0, lam_bytes, &sm.full[slot]);
+            bulk_g2s(&sm.sg[slot], sgrow + m, (uint32_t)sizeof(double2), &sm.full[slot]);
+        };
+        auto produce = [&](int it) {                  // lambda' row of step `it` (auxiliary warp 0)
+            const int slot = it & (NST - 1);
+            mbar_wait(&sm.full[slot], (it / NST) & 1);
+            const double s = sm.sg[slot].x;
+            for (int i = lane; i < NTB; i += 32) sm.hdr[slot][i] = sm.lamraw[slot][i] * s;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.ready[slot]);
+        };
+        if (at == 0)
+            for (int it = 0; it < NST && it < nsteps; ++it) issue(it);
+        if (aw == 0) { produce(0); if (nsteps > 1) produce(1); }
+        int lq[NQ], comp[NQ];
+        bool valid[NQ];
+        double* obase[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            const int o = at + NAUX * 32 * q;
+            lq[q] = l0 + o / (2 * NC);
+            comp[q] = o % (2 * NC);
+            valid[q] = lq[q] >= an && lq[q] < A.L;
+            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)lq[q] * 2 + (comp[q] & 1);
         }
+        // c_m(l) of the owned degrees, fetched one step ahead (coalesced rows of the plan-time table)
+        const double* crow = A.ctab + (size_t)(mtop - A.mmin) * A.Lp;
+        double cn[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) cn[q] = crow[lq[q]];
+        for (int it = 0; it < nsteps; ++it) {
+            const int m = mtop - it, rs = it & (NRS - 1);
+            double cm[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) cm[q] = cn[q];
+            if (it + 1 < nsteps) {
+                crow -= A.Lp;
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) cn[q] = crow[lq[q]];
+            }
+            if (aw == 0 && it + 2 < nsteps) produce(it + 2);
+            mbar_wait(&sm.rfull[rs], (it / NRS) & 1);
+            double v[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) v[q] = 0.0;
+            bool any = false;
+#pragma unroll
+            for (int ww = 0; ww < NW; ++ww) {
+                if (sm.act[rs][ww]) {
+                    any = true;
+                    const double* r = &sm.red[rs][ww][0][0] + at;
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) v[q] += r[NAUX * 32 * q];
+                }
+            }
+            if (any) {
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    const bool neg = NC == 2 && (comp[q] >> 1);
+                    if (valid[q] && lq[q] >= m && !(neg && m == 0)) {
+                        const int m_out = (NC == 2) ? (neg ? -m : m) : P.sgn_out * m;
+                        red_add_f64(obase[q] + (size_t)(m_out + A.L - 1) * A.Lp * 2, v[q] * cm[q]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.rempty[rs]);
+            if (at == 0 && it + NST < nsteps) issue(it + NST);
+        }
+        return;
     }
-    const int8_t* krow = A.kexp + (size_t)((l0 + TLB) / SHT_TQ - 1) * A.kstride - A.kmin;
-    // ---- producers (the last NTB+1 threads): lambda' of one ring each, plus the g' scale
-    constexpr int PB = NW * 32 - (NTB + 1);
-    const bool is_prod = tid >= PB;
-    const int pt = tid - PB;
-    double pcsc = 0, ptau = 0, psg = 1;
-    if (is_prod && pt < NTB) { pcsc = A.csc[th0 + pt]; ptau = A.tau[th0 + pt]; psg = A.sig[th0 + pt]; }
-    const double fn = (double)P.n;
-    auto produce = [&](int m, int buf) {
-        const int km = krow[m];
-        if (pt < NTB) {
-            const double fm = (double)m;
-            sm.hdr[buf][pt] = pow2i(-km) * fma(fn - psg * fm, pcsc, fm * ptau);
-        } else sm.hdr[buf][NTB] = pow2i(-2 - km - krow[m + 1]);
-    };
-    if (is_prod) produce(mtop, 0);
-    // ---- state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
+    reg_alloc_compute();
+
+    // -------------------------------------------------------------------- compute warps
+    // state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
     double cur[NI], prev[NI], x[RL];
     KPack<NI> kp;
     int lr[RL];
@@ -388,23 +455,16 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
     }
     double tm = 2.0 * (double)mtop;                    // x_{m-1} = x_m + 2m
     bool wact = true;
-    // reducer state (tid < TLB): degree l0 + tid, all components
-    const int lred = l0 + tid;
-    double* const out_g = reinterpret_cast<double*>(P.out);
-    double cfac = 1.0;
-    __syncthreads();
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
-    auto step = [&](const int m, double (&ca)[NI], double (&cb)[NI]) {
-        const unsigned it = (unsigned)(mtop - m), slot = it & (NST - 1);
-        mbar_wait(&sm.bar[slot], (it / NST) & 1);
-        const double2* T = &sm.wtile[slot][w * RT * NC];
-        const double* LM = &sm.hdr[it & 1][w * RT];
-        const double G = sm.hdr[it & 1][NTB];
-        double lmv[RT];
-        static_assert(RT % 2 == 0, "RT must be even (lambda' is read in pairs)");
-#pragma unroll
-        for (int i = 0; i < RT; i += 2) { const double2 t = *reinterpret_cast<const double2*>(LM + i); lmv[i] = t.x; lmv[i + 1] = t.y; }
+    auto step = [&](const int it, double (&ca)[NI], double (&cb)[NI]) {
+        const int m = mtop - it, slot = it & (NST - 1), rs = it & (NRS - 1);
+        mbar_wait(&sm.ready[slot], (it / NST) & 1);
+        mbar_wait(&sm.full[slot], (it / NST) & 1);
+        const double2* T = &sm.wt[slot][w * RT * NC];
+        const double* LM = &sm.hdr[slot][w * RT];
+        const double G = sm.sg[slot].y;
+        int flag = 0;
         double acc[RL][2 * NC];
 #pragma unroll
         for (int r = 0; r < RL; ++r)
@@ -420,7 +480,7 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
                 const double2 w0 = T[i * NC];
                 double2 w1 = make_double2(0.0, 0.0);
                 if (NC == 2) w1 = T[i * NC + 1];
-                const double lm = lmv[i];
+                const double lm = LM[i];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
                     const double e = ca[r * RT + i];
@@ -430,31 +490,37 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
                     ca[r * RT + i] = on[r] ? e : 0.0;                                         //      and keeps e_{m+1} = 0
                 }
             }
+            flag = 1;
         } else if (wact) {
             double g[RL];
 #pragma unroll
             for (int r = 0; r < RL; ++r) g[r] = x[r] * G;
 #pragma unroll
-            for (int i = 0; i < RT; ++i) {
-                const double2 w0 = T[i * NC];
-                double2 w1 = make_double2(0.0, 0.0);
-                if (NC == 2) w1 = T[i * NC + 1];
-                const double lm = lmv[i];
+            for (int i = 0; i < RT; i += 2) {
+                const double2 lm2 = *reinterpret_cast<const double2*>(LM + i);
 #pragma unroll
-                for (int r = 0; r < RL; ++r) {
-                    const double e = ca[r * RT + i];
-                    acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
-                    if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
-                    cb[r * RT + i] = fma(lm, e, -(g[r] * cb[r * RT + i]));
+                for (int ii = 0; ii < 2; ++ii) {
+                    const double2 w0 = T[(i + ii) * NC];
+                    double2 w1 = make_double2(0.0, 0.0);
+                    if (NC == 2) w1 = T[(i + ii) * NC + 1];
+                    const double lm = ii ? lm2.y : lm2.x;
+#pragma unroll
+                    for (int r = 0; r < RL; ++r) {
+                        const double e = ca[r * RT + i + ii];
+                        acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
+                        if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
+                        cb[r * RT + i + ii] = fma(lm, e, -(g[r] * cb[r * RT + i + ii]));
+                    }
                 }
             }
-        } else {                                      // every item of the warp is still below 2^-140: recursion only
+            flag = 1;
+        } else {                                      // every item of the warp is still below 2^-340: recursion only
             double g[RL];
 #pragma unroll
             for (int r = 0; r < RL; ++r) g[r] = x[r] * G;
 #pragma unroll
             for (int i = 0; i < RT; ++i) {
-                const double lm = lmv[i];
+                const double lm = LM[i];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) cb[r * RT + i] = fma(lm, ca[r * RT + i], -(g[r] * cb[r * RT + i]));
             }
@@ -467,36 +533,20 @@ __global__ void __launch_bounds__(NW * 32, (NW <= 4 ? 4 : 2)) theta_forward_kern
             if (P.m_lo) dead_check<NI>(cb, ca);
             if (m < l0) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
         }
-        double2* rd = reinterpret_cast<double2*>(&sm.red[it & 1][w][0][0]);
+        mbar_wait(&sm.rempty[rs], ((it / NRS) & 1) ^ 1);          // also keeps a non-writing warp from running ahead
+        if (flag) {
+            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][w][0][0]);
 #pragma unroll
-        for (int r = 0; r < RL; ++r)
+            for (int r = 0; r < RL; ++r)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) rd[(lane + 32 * r) * NC + c] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
-        if (is_prod && m > m_end) produce(m - 1, (it + 1) & 1);
-        __syncthreads();
-        if (tid == 0 && m - NST >= m_end) {
-            mbar_expect_tx(&sm.bar[slot], tile_bytes);
-            bulk_g2s(&sm.wtile[slot][0], P.in + ((size_t)(m - NST - m_end) * A.ntp + th0) * NC, tile_bytes, &sm.bar[slot]);
+                for (int c = 0; c < NC; ++c) rd[(lane + 32 * r) * NC + c] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
         }
-        if (tid < TLB && lred >= m && lred >= an && lred < A.L) {
-            const double2* rr = reinterpret_cast<const double2*>(&sm.red[it & 1][0][tid][0]);
-#pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                double2 v = make_double2(0.0, 0.0);
-#pragma unroll
-                for (int ww = 0; ww < NW; ++ww) { const double2 t = rr[ww * TLB * NC + c]; v.x += t.x; v.y += t.y; }
-                const int m_out = (NC == 2) ? (c ? -m : m) : P.sgn_out * m;
-                if (!(NC == 2 && c && m == 0)) {
-                    double* o = out_g + ((size_t)(m_out + A.L - 1) * A.Lp + lred) * 2;
-                    red_add_f64(o, v.x * cfac); red_add_f64(o + 1, v.y * cfac);
-                }
-            }
-            if (m > m_end) cfac *= pow2i(krow[m] + 1) * A.rsq[lred - m + 1] * A.rsq[lred + m];
-        }
+        __syncwarp();
+        if (lane == 0) { sm.act[rs][w] = flag; mbar_arrive(&sm.rfull[rs]); }
     };
-    for (int m = mtop; m >= m_end; m -= 2) {
-        step(m, cur, prev);
-        if (m - 1 >= m_end) step(m - 1, prev, cur);
+    for (int it = 0; it < nsteps; it += 2) {
+        step(it, cur, prev);
+        if (it + 1 < nsteps) step(it + 1, prev, cur);
     }
 }
 
@@ -517,22 +567,14 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double* sink)
 }
 
 template <int RL, int RT, int NW, int NC>
-cudaError_t launch_inv(const ThetaArgs& a, bool spin0, cudaStream_t st) {
+cudaError_t launch_inv(const ThetaArgs& a, cudaStream_t st) {
     using S = InvSmem<RL, RT, NW, NC>;
     const size_t smem = sizeof(S) + 128;
     dim3 grid((a.Lp / S::TL) * (a.ntp / S::NTH), a.npass);
-    cudaError_t e;
-    if (spin0) {
-        auto k = theta_inverse_kernel<RL, RT, NW, NC, true>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k<<<grid, NW * 32, smem, st>>>(a);
-    } else {
-        auto k = theta_inverse_kernel<RL, RT, NW, NC, false>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k<<<grid, NW * 32, smem, st>>>(a);
-    }
+    auto k = theta_inverse_kernel<RL, RT, NW, NC>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k<<<grid, (NW + NAUX) * 32, smem, st>>>(a);
     count_launch();
     return cudaGetLastError();
 }
@@ -544,22 +586,23 @@ cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((a.Lp / S::TLB) * (a.ntp / S::NTB), a.npass);
-    k<<<grid, NW * 32, smem, st>>>(a);
+    k<<<grid, (NW + NAUX) * 32, smem, st>>>(a);
     count_launch();
     return cudaGetLastError();
 }
 
 }  // namespace
 
-// Tile shapes: inverse 64 degrees x 64 rings per block (8 warps, 8 degrees x 2 rings per thread);
-//              forward 64 degrees x 32 rings per block (4 warps, 2 degrees x 8 rings per thread).
+// Tile shapes: inverse 64 degrees x 128 rings per block (8 compute warps, 8 degrees x 4 rings per thread);
+//              forward 64 degrees x 128 rings per block (8 compute warps, 2 degrees x 16 rings per thread).
+int theta_inverse_rowd(int mode) { return mode == 0 ? 6 : 4; }
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
-    return mode == 0 ? launch_inv<8, 2, 8, 2>(a, true, st) : launch_inv<8, 2, 8, 1>(a, a.all_n_zero != 0, st);
+    return mode == 0 ? launch_inv<8, 4, 8, 2>(a, st) : launch_inv<8, 4, 8, 1>(a, st);
 }
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
-    return mode == 0 ? launch_fwd<2, 8, 4, 2>(a, st) : launch_fwd<2, 8, 4, 1>(a, st);
+    return mode == 0 ? launch_fwd<2, 16, 8, 2>(a, st) : launch_fwd<2, 16, 8, 1>(a, st);
 }
 cudaError_t launch_fp64_peak(int iters, double* sink, cudaStream_t st, int* blocks, int* threads, int* fma_per_thread) {
     *blocks = 148 * 8; *threads = 256; *fma_per_thread = 16;
