@@ -184,13 +184,14 @@ void layout(sht_plan* P, char* base) {
     P->d_inv_pm = B.take<ThetaPass>(P->pinv.size() + 1); P->d_inv_p = B.take<ThetaPass>(P->pinv.size() + 1);
     P->d_fwd_pm = B.take<ThetaPass>(P->pfwd.size() + 1); P->d_fwd_p = B.take<ThetaPass>(P->pfwd.size() + 1);
     // per-pass operand buffers and lambda tables
+    // (rows m = m_end-1 .. L-1; row m_end-1 is all zero: the dummy second step of a final odd pair reads it)
     for (auto& ph : P->pinv) {
-        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end) * Lp * theta_inverse_rowd(ph.mode));
-        ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end) * P->inv.ntp);
+        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end + 1) * Lp * theta_inverse_rowd(ph.mode));
+        ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->inv.ntp);
     }
     for (auto& ph : P->pfwd) {
-        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end) * P->fwd.ntp * (ph.mode == 0 ? 4 : 2));
-        ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end) * P->fwd.ntp);
+        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->fwd.ntp * (ph.mode == 0 ? 4 : 2));
+        ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->fwd.ntp);
     }
     // scratch arrays
     P->F_slab = (size_t)NB * P->inv.ntp;
@@ -294,10 +295,10 @@ sht_status plan_common(sht_plan* P) {
     P->Lp = (int)rup(L, 128); P->NB = 2 * L - 1;
     int nmax = 0;
     for (int n : P->slab_n) nmax = (n < 0 ? -n : n) > nmax ? (n < 0 ? -n : n) : nmax;
-    P->kmin = -(nmax + 2);
+    P->kmin = -(nmax + 3);
     P->kstride = (int)rup((size_t)P->Lp + SHT_TQ + (size_t)(-P->kmin) + 2, 16);
     P->krows = P->Lp / SHT_TQ;
-    P->mmin = -nmax;
+    P->mmin = -nmax - 1;           // one row below the lowest recursion step (dummy step of an odd final pair)
     P->sgstride = (int)rup((size_t)(L - P->mmin), 2);
     for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
     // d-step counts: rings * sum over l of the steps each pass runs
@@ -376,7 +377,13 @@ sht_status upload_passes(sht_plan* P, cudaStream_t st) {
                 t.m_lo = R.mlo[2 * n_slab + (t.sgn_out > 0 ? 0 : 1)];
             } else t.m_lo = nullptr;
             ph.p = t;
-            CK(st_lamtab(t.n, R.nth, R.ntp, t.m_end, P->L - t.m_end, R.csc, R.tau, R.sig, const_cast<double*>(t.lam), st));
+            {   // zero the operand / lambda buffers once (their first row stays zero for good), then fill the lambda table
+                const size_t rows = (size_t)(P->L - t.m_end + 1);
+                const size_t in_doubles = dir ? rows * R.ntp * (ph.mode == 0 ? 4 : 2) : rows * P->Lp * theta_inverse_rowd(ph.mode);
+                CK(cudaMemsetAsync(const_cast<double*>(t.in), 0, in_doubles * sizeof(double), st));
+                CK(cudaMemsetAsync(const_cast<double*>(t.lam), 0, rows * R.ntp * sizeof(double), st));
+                CK(st_lamtab(t.n, R.nth, R.ntp, t.m_end, P->L - t.m_end, R.csc, R.tau, R.sig, const_cast<double*>(t.lam) + R.ntp, st));
+            }
             (ph.mode == 0 ? pm : p).push_back(t);
         }
         ThetaPass* dpm = dir ? P->d_fwd_pm : P->d_inv_pm; ThetaPass* dp = dir ? P->d_fwd_p : P->d_inv_p;
@@ -406,7 +413,8 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
     stage(P, CAT_STAGE, st);
     for (auto& ph : P->pinv)
         CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->NB,
-                           P->scale_inv, P->ctab, P->sgtab, P->sgstride, const_cast<double*>(ph.p.in), st));
+                           P->scale_inv, P->ctab, P->sgtab, P->sgstride,
+                           const_cast<double*>(ph.p.in) + (size_t)P->Lp * theta_inverse_rowd(ph.mode), st));
     CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
     CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
@@ -430,7 +438,8 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     for (auto& ph : P->pfwd) {
         int n_slab = P->slab_n[ph.p.slab];
         CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.m_lo,
-                           P->fwd.wq, U + U_slab * ph.p.slab, reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)), st));
+                           P->fwd.wq, U + U_slab * ph.p.slab,
+                           reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), st));
     }
     CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);

@@ -61,6 +61,7 @@ __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7
 
 constexpr int NST = 4;   // stages of the operand ring
 constexpr int NRS = 2;   // stages of the partial-sum hand-off
+constexpr int KS = 2;    // recursion steps per pipeline stage (one TMA barrier, one hand-off per KS steps)
 constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
 // The register file is split over the 4 SM sub-partitions (16 K registers each, 3 warps each here): compute warps take
 // 232 registers per thread, auxiliary warps 40 (2*32*232 + 32*40 = 16128); the kernel is launched at 168.
@@ -116,15 +117,15 @@ __device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]
 
 // =============================================================================================================
 // inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * e^l_m(theta)      (G carries c_m(l))
-// block tile: TL = NW*RL degrees x NTH = 32*RT rings
+// block tile: TL = NW*RL degrees x NTH = 32*RT rings; KS = 2 recursion steps per pipeline stage
 // =============================================================================================================
 template <int RL, int RT, int NW, int NC>
 struct InvSmem {
     static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2;
-    double op[NST][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
-    double lam[NST][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
-    double red[NRS][NW][NTH][2 * NC];   // per-warp partial sums
-    int act[NRS][NW];                   // warp wrote partial sums at this step
+    double op[NST][KS][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
+    double lam[NST][KS][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
+    double red[NRS][KS][NW][NTH][2 * NC];   // per-warp partial sums
+    int act[NRS][NW];                       // bit h: the warp wrote partial sums for step h of the pair
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
@@ -143,7 +144,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TL <= an || l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end, nsteps = mtop - m_end + 1;
+    const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end;
+    const int npairs = (mtop - m_end + 2) / KS;       // an odd step count ends with a dummy step m_end-1 (all-zero table row)
 
     if (tid == 0) {
         for (int i = 0; i < NST; ++i) mbar_init(&sm.full[i], 1);
@@ -155,58 +157,70 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     if (w >= NW) {
         // ---------------------------------------------------------------- auxiliary warps: TMA producer + reducers
         reg_dealloc_aux();
-        const int at = tid - NW * 32;                 // 0..127: owns outputs at, at+128, ... of the NOUT per step
-        constexpr int NOUT = NTH * 2 * NC, NQ = NOUT / (NAUX * 32);
+        const int at = tid - NW * 32;                 // 0..127: owns output pairs (re, im) at, at+128, ... of the NOUT per step
+        constexpr int NOUT = NTH * NC, NQ = NOUT / (NAUX * 32);
         constexpr uint32_t op_bytes = TL * ROWD * sizeof(double), lam_bytes = NTH * sizeof(double);
-        auto issue = [&](int it) {
-            const int m = mtop - it, slot = it & (NST - 1);
-            mbar_expect_tx(&sm.full[slot], op_bytes + lam_bytes);
-            bulk_g2s(&sm.op[slot][0], P.in + ((size_t)(m - m_end) * A.Lp + l0) * ROWD, op_bytes, &sm.full[slot]);
-            bulk_g2s(&sm.lam[slot][0], P.lam + (size_t)(m - m_end) * A.ntp + th0, lam_bytes, &sm.full[slot]);
+        auto issue = [&](int p) {
+            const int m = mtop - KS * p, slot = p & (NST - 1);
+            mbar_expect_tx(&sm.full[slot], KS * (op_bytes + lam_bytes));
+#pragma unroll
+            for (int h = 0; h < KS; ++h) {
+                const size_t row = (size_t)(m - h - m_end + 1);      // table rows start at m_end-1
+                bulk_g2s(&sm.op[slot][h][0], P.in + (row * A.Lp + l0) * ROWD, op_bytes, &sm.full[slot]);
+                bulk_g2s(&sm.lam[slot][h][0], P.lam + row * A.ntp + th0, lam_bytes, &sm.full[slot]);
+            }
         };
         if (at == 0)
-            for (int it = 0; it < NST && it < nsteps; ++it) issue(it);
-        int mlo[NQ], comp[NQ];
-        bool valid[NQ];
+            for (int p = 0; p < NST && p < npairs; ++p) issue(p);
+        int mlo[NQ];
+        bool valid[NQ], neg[NQ];
         double* obase[NQ];
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
-            const int o = at + NAUX * 32 * q, th = th0 + o / (2 * NC);
-            comp[q] = o % (2 * NC);
+            const int o = at + NAUX * 32 * q, th = th0 + o / NC;
+            neg[q] = NC == 2 && (o % NC);
             valid[q] = th < A.nth;
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
-            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2 + (comp[q] & 1);
+            if (mlo[q] < m_end) mlo[q] = m_end;
+            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2;
         }
-        for (int it = 0; it < nsteps; ++it) {
-            const int m = mtop - it, rs = it & (NRS - 1);
-            mbar_wait(&sm.rfull[rs], (it / NRS) & 1);
-            double v[NQ];
+        for (int p = 0; p < npairs; ++p) {
+            const int rs = p & (NRS - 1);
+            mbar_wait(&sm.rfull[rs], (p / NRS) & 1);
+            int actb[NW];
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) v[q] = 0.0;
-            bool any = false;
+            for (int ww = 0; ww < NW; ++ww) actb[ww] = sm.act[rs][ww];
 #pragma unroll
-            for (int ww = 0; ww < NW; ++ww) {
-                if (sm.act[rs][ww]) {
-                    any = true;
-                    const double* r = &sm.red[rs][ww][0][0] + at;
+            for (int h = 0; h < KS; ++h) {
+                const int m = mtop - KS * p - h;
+                double2 v[NQ];
 #pragma unroll
-                    for (int q = 0; q < NQ; ++q) v[q] += r[NAUX * 32 * q];
+                for (int q = 0; q < NQ; ++q) v[q] = make_double2(0.0, 0.0);
+                bool any = false;
+#pragma unroll
+                for (int ww = 0; ww < NW; ++ww) {
+                    if ((actb[ww] >> h) & 1) {
+                        any = true;
+                        const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]) + at;
+#pragma unroll
+                        for (int q = 0; q < NQ; ++q) { const double2 t = r[NAUX * 32 * q]; v[q].x += t.x; v[q].y += t.y; }
+                    }
                 }
-            }
-            if (any) {
+                if (any) {
 #pragma unroll
-                for (int q = 0; q < NQ; ++q) {
-                    const bool neg = NC == 2 && (comp[q] >> 1);
-                    if (valid[q] && m >= mlo[q] && !(neg && m == 0)) {
-                        const int m_out = (NC == 2) ? (neg ? -m : m) : P.sgn_out * m;
-                        const int row = m_out < 0 ? m_out + A.NB : m_out;
-                        red_add_f64(obase[q] + (size_t)row * A.ntp * 2, v[q]);
+                    for (int q = 0; q < NQ; ++q) {
+                        if (valid[q] && m >= mlo[q] && !(neg[q] && m == 0)) {
+                            const int m_out = (NC == 2) ? (neg[q] ? -m : m) : P.sgn_out * m;
+                            const int row = m_out < 0 ? m_out + A.NB : m_out;
+                            double* o = obase[q] + (size_t)row * A.ntp * 2;
+                            red_add_f64(o, v[q].x); red_add_f64(o + 1, v[q].y);
+                        }
                     }
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm.rempty[rs]);
-            if (at == 0 && it + NST < nsteps) issue(it + NST);   // every compute warp has finished step `it`: its slot is free
+            if (at == 0 && p + NST < npairs) issue(p + NST);   // every compute warp has finished pair p: its slot is free
         }
         return;
     }
@@ -225,105 +239,109 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     const uint8_t* stk = P.st_k + (size_t)la * A.ntp + th0 + lane;
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step, so the
-    // iterates never move between registers)
-    auto step = [&](const int it, double (&ca)[NI], double (&cb)[NI]) {
-        const int m = mtop - it, slot = it & (NST - 1), rs = it & (NRS - 1);
-        mbar_wait(&sm.full[slot], (it / NST) & 1);
-        int flag = 0;
-        if (m <= l_hi && warp_real) {
-            if (m >= la) {                            // the degree l == m starts (warp-uniform): Eq. 27 start values
+    // iterates never move between registers).  Returns true if partial sums were written.
+    auto step = [&](const int m, const int slot, const int rs, const int h, const uint32_t rparity, bool& waited, double (&ca)[NI],
+                    double (&cb)[NI]) -> bool {
+        if (!(m <= l_hi && warp_real)) return false;
+        bool wrote = false;
+        if (m >= la) {                                // the degree l == m starts (warp-uniform): Eq. 27 start values
 #pragma unroll
-                for (int j = 0; j < RL; ++j) {
-                    if (m == la + j) {
-#pragma unroll
-                        for (int i = 0; i < RT; ++i) {
-                            ca[j * RT + i] = stv[(size_t)j * A.ntp + 32 * i];
-                            cb[j * RT + i] = 0.0;
-                            kp.set(j * RT + i, stk[(size_t)j * A.ntp + 32 * i]);
-                        }
-                    }
-                }
-                wact = true;                          // re-evaluated at the next window check
-            }
-            const double* row = &sm.op[slot][(w * RL) * ROWD];
-            const double s = row[ROWD - 1];
-            double lam[RT];
-#pragma unroll
-            for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][lane + 32 * i] * s;
-            if (wact) {
-                double acc[RT][2 * NC];
-#pragma unroll
-                for (int i = 0; i < RT; ++i)
-#pragma unroll
-                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
-#pragma unroll
-                for (int j = 0; j < RL; ++j) {
-                    const double* r = row + j * ROWD;
-                    double cf[2 * NC];
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) {
-                        const double2 t = *reinterpret_cast<const double2*>(r + 2 * c);
-                        cf[2 * c] = t.x; cf[2 * c + 1] = t.y;
-                    }
-                    const double g = r[2 * NC];
+            for (int j = 0; j < RL; ++j) {
+                if (m == la + j) {
 #pragma unroll
                     for (int i = 0; i < RT; ++i) {
-                        const double e = ca[j * RT + i];
-#pragma unroll
-                        for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fma(e, cf[c], acc[i][c]);
-                        cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
+                        ca[j * RT + i] = stv[(size_t)j * A.ntp + 32 * i];
+                        cb[j * RT + i] = 0.0;
+                        kp.set(j * RT + i, stk[(size_t)j * A.ntp + 32 * i]);
                     }
                 }
-                mbar_wait(&sm.rempty[rs], ((it / NRS) & 1) ^ 1);      // the reducer is done with this slot's previous use
-                double2* rd = reinterpret_cast<double2*>(&sm.red[rs][w][0][0]);
+            }
+            wact = true;                              // re-evaluated at the next window check
+        }
+        const double* row = &sm.op[slot][h][(w * RL) * ROWD];
+        const double s = row[ROWD - 1];
+        double lam[RT];
 #pragma unroll
-                for (int i = 0; i < RT; ++i)
+        for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][h][lane + 32 * i] * s;
+        if (wact) {
+            double acc[RT][2 * NC];
 #pragma unroll
-                    for (int c = 0; c < NC; ++c) rd[(lane + 32 * i) * NC + c] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
-                flag = 1;
-            } else {                                  // every item of the warp is still below 2^-340: recursion only
+            for (int i = 0; i < RT; ++i)
 #pragma unroll
-                for (int j = 0; j < RL; ++j) {
-                    const double g = row[j * ROWD + 2 * NC];
+                for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
 #pragma unroll
-                    for (int i = 0; i < RT; ++i) cb[j * RT + i] = fma(lam[i], ca[j * RT + i], -(g * cb[j * RT + i]));
+            for (int j = 0; j < RL; ++j) {
+                const double* r = row + j * ROWD;
+                double cf[2 * NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const double2 t = *reinterpret_cast<const double2*>(r + 2 * c);
+                    cf[2 * c] = t.x; cf[2 * c + 1] = t.y;
+                }
+                const double g = r[2 * NC];
+#pragma unroll
+                for (int i = 0; i < RT; ++i) {
+                    const double e = ca[j * RT + i];
+#pragma unroll
+                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fma(e, cf[c], acc[i][c]);
+                    cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
                 }
             }
-            if ((m & (SHT_JCHK - 1)) == 0) {
-                if (kp.any_nonzero()) window_check<NI>(cb, ca, kp);
-                if (P.m_lo) dead_check<NI>(cb, ca);
-                if (m < la) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
+            if (!waited) { mbar_wait(&sm.rempty[rs], rparity); waited = true; }   // the reducers are done with this slot
+            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
+#pragma unroll
+            for (int i = 0; i < RT; ++i)
+#pragma unroll
+                for (int c = 0; c < NC; ++c) rd[(lane + 32 * i) * NC + c] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
+            wrote = true;
+        } else {                                      // every item of the warp is still below 2^-340: recursion only
+#pragma unroll
+            for (int j = 0; j < RL; ++j) {
+                const double g = row[j * ROWD + 2 * NC];
+#pragma unroll
+                for (int i = 0; i < RT; ++i) cb[j * RT + i] = fma(lam[i], ca[j * RT + i], -(g * cb[j * RT + i]));
             }
         }
+        if ((m & (SHT_JCHK - 1)) == 0) {
+            if (kp.any_nonzero()) window_check<NI>(cb, ca, kp);
+            if (P.m_lo) dead_check<NI>(cb, ca);
+            if (m < la) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
+        }
+        return wrote;
+    };
+    for (int p = 0; p < npairs; ++p) {
+        const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
+        const uint32_t rparity = ((p / NRS) & 1) ^ 1;
+        mbar_wait(&sm.full[slot], (p / NST) & 1);
+        bool waited = false;
+        int flags = 0;
+        if (step(m, slot, rs, 0, rparity, waited, cur, prev)) flags |= 1;
+        if (step(m - 1, slot, rs, 1, rparity, waited, prev, cur)) flags |= 2;
         __syncwarp();
         if (lane == 0) {
             // never arrive on a phase before the previous use of the slot has been consumed (a warp that writes nothing
             // must not run ahead either: its arrival would be counted in the wrong phase)
-            if (!flag) mbar_wait(&sm.rempty[rs], ((it / NRS) & 1) ^ 1);
-            sm.act[rs][w] = flag;
+            if (!waited) mbar_wait(&sm.rempty[rs], rparity);
+            sm.act[rs][w] = flags;
             mbar_arrive(&sm.rfull[rs]);
         }
-    };
-    for (int it = 0; it < nsteps; it += 2) {
-        step(it, cur, prev);
-        if (it + 1 < nsteps) step(it + 1, prev, cur);
     }
 }
 
 // =============================================================================================================
 // forward theta step, Eq. 30:  H[m_out+L-1][l] += c_m(l) * sum_theta W[m][theta] * e^l_m(theta)
-// block tile: TLB = 32*RL degrees x NTB = NW*RT rings
+// block tile: TLB = 32*RL degrees x NTB = NW*RT rings; KS = 2 recursion steps per pipeline stage
 // =============================================================================================================
 template <int RL, int RT, int NW, int NC>
 struct FwdSmem {
     static constexpr int TLB = 32 * RL, NTB = NW * RT;
-    double2 wt[NST][NTB * NC];          // weighted F_m samples of the block's rings (TMA ring)
-    double lamraw[NST][NTB];            // lambda_m(theta) (TMA ring)
-    double2 sg[NST];                    // (s_m, G_m) of the block's quantum (TMA ring)
-    double hdr[NST][NTB];               // lambda'_m = lambda_m s_m (written by the auxiliary warp)
-    double red[NRS][NW][TLB][2 * NC];   // per-warp partial sums
+    double2 wt[NST][KS][NTB * NC];          // weighted F_m samples of the block's rings (TMA ring)
+    double lamraw[NST][KS][NTB];            // lambda_m(theta) (TMA ring)
+    double2 sg[NST][KS];                    // (s, G) of the block's quantum: [KS-1-h] belongs to step h of the pair
+    double hdr[NW][KS][RT];                 // lambda'_m = lambda_m s_m of each warp's own rings
+    double red[NRS][KS][NW][TLB][2 * NC];   // per-warp partial sums
     int act[NRS][NW];
-    uint64_t full[NST], ready[NST], rfull[NRS], rempty[NRS];
+    uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
 template <int RL, int RT, int NW, int NC>
@@ -331,7 +349,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     using S = FwdSmem<RL, RT, NW, NC>;
     constexpr int TLB = S::TLB, NTB = S::NTB, NI = RL * RT;
     static_assert(TLB == SHT_TQ, "the block's degrees must be one kappa quantum");
-    static_assert(RT % 2 == 0, "RT must be even (lambda' is read in pairs)");
+    static_assert(KS * RT <= 32, "one lane per lambda' value of a pair");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
@@ -342,10 +360,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end, nsteps = mtop - m_end + 1;
+    const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end;
+    const int npairs = (mtop - m_end + 2) / KS;
 
     if (tid == 0) {
-        for (int i = 0; i < NST; ++i) { mbar_init(&sm.full[i], 1); mbar_init(&sm.ready[i], 1); }
+        for (int i = 0; i < NST; ++i) mbar_init(&sm.full[i], 1);
         for (int i = 0; i < NRS; ++i) { mbar_init(&sm.rfull[i], NW); mbar_init(&sm.rempty[i], NAUX); }
         mbar_fence_init();
     }
@@ -354,82 +373,93 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     if (w >= NW) {
         // ---------------------------------------------------------------- auxiliary warps
         reg_dealloc_aux();
-        const int at = tid - NW * 32, aw = w - NW;
-        constexpr int NOUT = TLB * 2 * NC, NQ = NOUT / (NAUX * 32);
+        const int at = tid - NW * 32;
+        constexpr int NOUT = TLB * NC, NQ = (NOUT + NAUX * 32 - 1) / (NAUX * 32);
         constexpr uint32_t wt_bytes = NTB * NC * sizeof(double2), lam_bytes = NTB * sizeof(double);
         const double2* sgrow = A.sg + (size_t)lt * A.sgstride - A.mmin;
-        auto issue = [&](int it) {
-            const int m = mtop - it, slot = it & (NST - 1);
-            mbar_expect_tx(&sm.full[slot], wt_bytes + lam_bytes + (uint32_t)sizeof(double2));
-            bulk_g2s(&sm.wt[slot][0], P.in + ((size_t)(m - m_end) * A.ntp + th0) * 2 * NC, wt_bytes, &sm.full[slot]);
-            bulk_g2s(&sm.lamraw[slot][0], P.lam + (size_t)(m - m_end) * A.ntp + th0, lam_bytes, &sm.full[slot]);
-            bulk_g2s(&sm.sg[slot], sgrow + m, (uint32_t)sizeof(double2), &sm.full[slot]);
-        };
-        auto produce = [&](int it) {                  // lambda' row of step `it` (auxiliary warp 0)
-            const int slot = it & (NST - 1);
-            mbar_wait(&sm.full[slot], (it / NST) & 1);
-            const double s = sm.sg[slot].x;
-            for (int i = lane; i < NTB; i += 32) sm.hdr[slot][i] = sm.lamraw[slot][i] * s;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&sm.ready[slot]);
+        auto issue = [&](int p) {
+            const int m = mtop - KS * p, slot = p & (NST - 1);
+            mbar_expect_tx(&sm.full[slot], KS * (wt_bytes + lam_bytes + (uint32_t)sizeof(double2)));
+#pragma unroll
+            for (int h = 0; h < KS; ++h) {
+                const size_t row = (size_t)(m - h - m_end + 1);
+                bulk_g2s(&sm.wt[slot][h][0], P.in + (row * A.ntp + th0) * 2 * NC, wt_bytes, &sm.full[slot]);
+                bulk_g2s(&sm.lamraw[slot][h][0], P.lam + row * A.ntp + th0, lam_bytes, &sm.full[slot]);
+            }
+            bulk_g2s(&sm.sg[slot][0], sgrow + (m - KS + 1), KS * (uint32_t)sizeof(double2), &sm.full[slot]);
         };
         if (at == 0)
-            for (int it = 0; it < NST && it < nsteps; ++it) issue(it);
-        if (aw == 0) { produce(0); if (nsteps > 1) produce(1); }
-        int lq[NQ], comp[NQ];
-        bool valid[NQ];
+            for (int p = 0; p < NST && p < npairs; ++p) issue(p);
+        int lq[NQ];
+        bool valid[NQ], neg[NQ];
         double* obase[NQ];
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             const int o = at + NAUX * 32 * q;
-            lq[q] = l0 + o / (2 * NC);
-            comp[q] = o % (2 * NC);
-            valid[q] = lq[q] >= an && lq[q] < A.L;
-            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)lq[q] * 2 + (comp[q] & 1);
+            lq[q] = l0 + o / NC;
+            neg[q] = NC == 2 && (o % NC);
+            valid[q] = o < NOUT && lq[q] >= an && lq[q] < A.L;
+            if (o >= NOUT) lq[q] = l0;
+            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)lq[q] * 2;
         }
-        // c_m(l) of the owned degrees, fetched one step ahead (coalesced rows of the plan-time table)
+        // c_m(l) of the owned degrees, fetched one pair ahead (coalesced rows of the plan-time table)
         const double* crow = A.ctab + (size_t)(mtop - A.mmin) * A.Lp;
-        double cn[NQ];
+        double cn[KS][NQ];
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) cn[q] = crow[lq[q]];
-        for (int it = 0; it < nsteps; ++it) {
-            const int m = mtop - it, rs = it & (NRS - 1);
-            double cm[NQ];
+        for (int h = 0; h < KS; ++h)
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) cm[q] = cn[q];
-            if (it + 1 < nsteps) {
-                crow -= A.Lp;
+            for (int q = 0; q < NQ; ++q) cn[h][q] = crow[-(ptrdiff_t)h * A.Lp + lq[q]];
+        for (int p = 0; p < npairs; ++p) {
+            const int rs = p & (NRS - 1);
+            double cm[KS][NQ];
 #pragma unroll
-                for (int q = 0; q < NQ; ++q) cn[q] = crow[lq[q]];
+            for (int h = 0; h < KS; ++h)
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) cm[h][q] = cn[h][q];
+            if (p + 1 < npairs) {
+                crow -= (size_t)KS * A.Lp;
+#pragma unroll
+                for (int h = 0; h < KS; ++h)
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) cn[h][q] = crow[-(ptrdiff_t)h * A.Lp + lq[q]];
             }
-            if (aw == 0 && it + 2 < nsteps) produce(it + 2);
-            mbar_wait(&sm.rfull[rs], (it / NRS) & 1);
-            double v[NQ];
+            mbar_wait(&sm.rfull[rs], (p / NRS) & 1);
+            int actb[NW];
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) v[q] = 0.0;
-            bool any = false;
+            for (int ww = 0; ww < NW; ++ww) actb[ww] = sm.act[rs][ww];
 #pragma unroll
-            for (int ww = 0; ww < NW; ++ww) {
-                if (sm.act[rs][ww]) {
-                    any = true;
-                    const double* r = &sm.red[rs][ww][0][0] + at;
+            for (int h = 0; h < KS; ++h) {
+                const int m = mtop - KS * p - h;
+                double2 v[NQ];
 #pragma unroll
-                    for (int q = 0; q < NQ; ++q) v[q] += r[NAUX * 32 * q];
+                for (int q = 0; q < NQ; ++q) v[q] = make_double2(0.0, 0.0);
+                bool any = false;
+#pragma unroll
+                for (int ww = 0; ww < NW; ++ww) {
+                    if ((actb[ww] >> h) & 1) {
+                        any = true;
+                        const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]);
+#pragma unroll
+                        for (int q = 0; q < NQ; ++q) {
+                            const int o = at + NAUX * 32 * q;
+                            if (o < NOUT) { const double2 t = r[o]; v[q].x += t.x; v[q].y += t.y; }
+                        }
+                    }
                 }
-            }
-            if (any) {
+                if (any && m >= m_end) {
 #pragma unroll
-                for (int q = 0; q < NQ; ++q) {
-                    const bool neg = NC == 2 && (comp[q] >> 1);
-                    if (valid[q] && lq[q] >= m && !(neg && m == 0)) {
-                        const int m_out = (NC == 2) ? (neg ? -m : m) : P.sgn_out * m;
-                        red_add_f64(obase[q] + (size_t)(m_out + A.L - 1) * A.Lp * 2, v[q] * cm[q]);
+                    for (int q = 0; q < NQ; ++q) {
+                        if (valid[q] && lq[q] >= m && !(neg[q] && m == 0)) {
+                            const int m_out = (NC == 2) ? (neg[q] ? -m : m) : P.sgn_out * m;
+                            double* o = obase[q] + (size_t)(m_out + A.L - 1) * A.Lp * 2;
+                            red_add_f64(o, v[q].x * cm[h][q]); red_add_f64(o + 1, v[q].y * cm[h][q]);
+                        }
                     }
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm.rempty[rs]);
-            if (at == 0 && it + NST < nsteps) issue(it + NST);
+            if (at == 0 && p + NST < npairs) issue(p + NST);
         }
         return;
     }
@@ -457,14 +487,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     bool wact = true;
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
-    auto step = [&](const int it, double (&ca)[NI], double (&cb)[NI]) {
-        const int m = mtop - it, slot = it & (NST - 1), rs = it & (NRS - 1);
-        mbar_wait(&sm.ready[slot], (it / NST) & 1);
-        mbar_wait(&sm.full[slot], (it / NST) & 1);
-        const double2* T = &sm.wt[slot][w * RT * NC];
-        const double* LM = &sm.hdr[slot][w * RT];
-        const double G = sm.sg[slot].y;
-        int flag = 0;
+    auto step = [&](const int m, const int slot, const int rs, const int h, const uint32_t rparity, bool& waited, double (&ca)[NI],
+                    double (&cb)[NI]) -> bool {
+        const double2* T = &sm.wt[slot][h][w * RT * NC];
+        const double* LM = &sm.hdr[w][h][0];
+        const double G = sm.sg[slot][KS - 1 - h].y;
+        bool wrote = false;
         double acc[RL][2 * NC];
 #pragma unroll
         for (int r = 0; r < RL; ++r)
@@ -490,7 +518,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
                     ca[r * RT + i] = on[r] ? e : 0.0;                                         //      and keeps e_{m+1} = 0
                 }
             }
-            flag = 1;
+            wrote = true;
         } else if (wact) {
             double g[RL];
 #pragma unroll
@@ -513,7 +541,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
                     }
                 }
             }
-            flag = 1;
+            wrote = true;
         } else {                                      // every item of the warp is still below 2^-340: recursion only
             double g[RL];
 #pragma unroll
@@ -533,20 +561,36 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             if (P.m_lo) dead_check<NI>(cb, ca);
             if (m < l0) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
         }
-        mbar_wait(&sm.rempty[rs], ((it / NRS) & 1) ^ 1);          // also keeps a non-writing warp from running ahead
-        if (flag) {
-            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][w][0][0]);
+        if (wrote) {
+            if (!waited) { mbar_wait(&sm.rempty[rs], rparity); waited = true; }
+            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
 #pragma unroll
             for (int r = 0; r < RL; ++r)
 #pragma unroll
                 for (int c = 0; c < NC; ++c) rd[(lane + 32 * r) * NC + c] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
         }
-        __syncwarp();
-        if (lane == 0) { sm.act[rs][w] = flag; mbar_arrive(&sm.rfull[rs]); }
+        return wrote;
     };
-    for (int it = 0; it < nsteps; it += 2) {
-        step(it, cur, prev);
-        if (it + 1 < nsteps) step(it + 1, prev, cur);
+    for (int p = 0; p < npairs; ++p) {
+        const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
+        const uint32_t rparity = ((p / NRS) & 1) ^ 1;
+        mbar_wait(&sm.full[slot], (p / NST) & 1);
+        // lambda' of this warp's rings for both steps of the pair: lane -> (step h, ring i)
+        if (lane < KS * RT) {
+            const int h = lane / RT, i = lane % RT;
+            sm.hdr[w][h][i] = sm.lamraw[slot][h][w * RT + i] * sm.sg[slot][KS - 1 - h].x;
+        }
+        __syncwarp();
+        bool waited = false;
+        int flags = 0;
+        if (step(m, slot, rs, 0, rparity, waited, cur, prev)) flags |= 1;
+        if (step(m - 1, slot, rs, 1, rparity, waited, prev, cur)) flags |= 2;
+        __syncwarp();
+        if (lane == 0) {
+            if (!waited) mbar_wait(&sm.rempty[rs], rparity);
+            sm.act[rs][w] = flags;
+            mbar_arrive(&sm.rfull[rs]);
+        }
     }
 }
 

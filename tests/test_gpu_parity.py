@@ -120,7 +120,8 @@ def test_real_signals(api, orc):
         assert rel(back, flm) < TOL
         # input m<0 half is ignored
         junk = flm.copy(); junk[:, :L - 1] = 99.0
-        assert np.array_equal(P.inverse(dev(junk)).cpu().numpy(), f)
+        # (not bit-equal: several l-tiles add into F_m(theta) with RED.ADD, whose order is not fixed)
+        assert rel(P.inverse(dev(junk)).cpu().numpy(), f) < 1e-13
 
 
 @pytest.mark.parametrize("L,N", [(4, 1), (8, 3), (16, 5), (33, 8), (40, 40)])
