@@ -59,7 +59,20 @@ __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7
 #define HI_TWIN ((1023 + SHT_TWIN) << 20)
 #define HI_DEAD ((1023 + 500) << 20)
 
-constexpr int NST = 4;   // stages of the operand ring
+#ifdef SHT_PROF
+__device__ unsigned long long g_prof[16];
+#define PROF_T0() long long t0__ = clock64()
+#define PROF_ADD(slot) do { pf__[(slot) & 1] += (unsigned long long)(clock64() - t0__); } while (0)
+#define PROF_DECL() unsigned long long pf__[2] = {0, 0}, pc__[3] = {0, 0, 0}
+#else
+#define PROF_T0() do {} while (0)
+#define PROF_ADD(slot) do {} while (0)
+#define PROF_DECL() do {} while (0)
+#endif
+#ifndef SHT_NST
+#define SHT_NST 4
+#endif
+constexpr int NST = SHT_NST;   // stages of the operand ring
 constexpr int NRS = 2;   // stages of the partial-sum hand-off
 constexpr int KS = 2;    // recursion steps per pipeline stage (one TMA barrier, one hand-off per KS steps)
 constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
@@ -177,8 +190,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         double* obase[NQ];
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
-            const int o = at + NAUX * 32 * q, th = th0 + o / NC;
-            neg[q] = NC == 2 && (o % NC);
+            const int o = at + NAUX * 32 * q;
+            const int th = th0 + o % NTH;             // partial sums are stored [column][ring]
+            neg[q] = NC == 2 && (o / NTH);
             valid[q] = th < A.nth;
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
             if (mlo[q] < m_end) mlo[q] = m_end;
@@ -225,6 +239,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         return;
     }
     reg_alloc_compute();
+    PROF_DECL();
 
     // -------------------------------------------------------------------- compute warps
     const int la = l0 + w * RL, l_hi = la + RL - 1;   // degrees of this warp
@@ -240,7 +255,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step, so the
     // iterates never move between registers).  Returns true if partial sums were written.
-    auto step = [&](const int m, const int slot, const int rs, const int h, const uint32_t rparity, bool& waited, double (&ca)[NI],
+    auto step = [&](const int m, const int slot, const int rs, const int h, double (&ca)[NI],
                     double (&cb)[NI]) -> bool {
         if (!(m <= l_hi && warp_real)) return false;
         bool wrote = false;
@@ -287,12 +302,13 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                     cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
                 }
             }
-            if (!waited) { mbar_wait(&sm.rempty[rs], rparity); waited = true; }   // the reducers are done with this slot
             double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
 #pragma unroll
             for (int i = 0; i < RT; ++i)
 #pragma unroll
-                for (int c = 0; c < NC; ++c) rd[(lane + 32 * i) * NC + c] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
+                for (int c = 0; c < NC; ++c) {
+                    rd[c * NTH + lane + 32 * i] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
+                }
             wrote = true;
         } else {                                      // every item of the warp is still below 2^-340: recursion only
 #pragma unroll
@@ -309,23 +325,36 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         }
         return wrote;
     };
+    constexpr int PB = 0;
+#ifdef SHT_PROF
+    const long long tloop__ = clock64();
+#endif
     for (int p = 0; p < npairs; ++p) {
         const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
         const uint32_t rparity = ((p / NRS) & 1) ^ 1;
-        mbar_wait(&sm.full[slot], (p / NST) & 1);
-        bool waited = false;
+        { PROF_T0(); mbar_wait(&sm.full[slot], (p / NST) & 1); PROF_ADD(PB + 0); }
+        // the reducers are done with this hand-off slot (waiting here, not in front of the first partial-sum store, keeps
+        // the compute section free of barriers so that operand loads of both steps can be hoisted above the FMAs)
+        { PROF_T0(); mbar_wait(&sm.rempty[rs], rparity); PROF_ADD(PB + 1); }
         int flags = 0;
-        if (step(m, slot, rs, 0, rparity, waited, cur, prev)) flags |= 1;
-        if (step(m - 1, slot, rs, 1, rparity, waited, prev, cur)) flags |= 2;
+        if (step(m, slot, rs, 0, cur, prev)) flags |= 1;
+        if (step(m - 1, slot, rs, 1, prev, cur)) flags |= 2;
         __syncwarp();
         if (lane == 0) {
-            // never arrive on a phase before the previous use of the slot has been consumed (a warp that writes nothing
-            // must not run ahead either: its arrival would be counted in the wrong phase)
-            if (!waited) mbar_wait(&sm.rempty[rs], rparity);
             sm.act[rs][w] = flags;
             mbar_arrive(&sm.rfull[rs]);
         }
+#ifdef SHT_PROF
+        pc__[0]++; if (flags == 3) pc__[1]++; if (flags == 0) pc__[2]++;
+#endif
     }
+#ifdef SHT_PROF
+    if (lane == 0) {
+        atomicAdd(&g_prof[PB + 2], (unsigned long long)(clock64() - tloop__));
+        atomicAdd(&g_prof[PB + 0], pf__[0]); atomicAdd(&g_prof[PB + 1], pf__[1]);
+        atomicAdd(&g_prof[PB + 3], pc__[0]); atomicAdd(&g_prof[PB + 4], pc__[1]); atomicAdd(&g_prof[PB + 5], pc__[2]);
+    }
+#endif
 }
 
 // =============================================================================================================
@@ -396,8 +425,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             const int o = at + NAUX * 32 * q;
-            lq[q] = l0 + o / NC;
-            neg[q] = NC == 2 && (o % NC);
+            lq[q] = l0 + o % TLB;                     // partial sums are stored [column][degree]
+            neg[q] = NC == 2 && (o / TLB);
             valid[q] = o < NOUT && lq[q] >= an && lq[q] < A.L;
             if (o >= NOUT) lq[q] = l0;
             obase[q] = reinterpret_cast<double*>(P.out) + (size_t)lq[q] * 2;
@@ -464,6 +493,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         return;
     }
     reg_alloc_compute();
+    PROF_DECL();
 
     // -------------------------------------------------------------------- compute warps
     // state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
@@ -487,7 +517,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     bool wact = true;
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
-    auto step = [&](const int m, const int slot, const int rs, const int h, const uint32_t rparity, bool& waited, double (&ca)[NI],
+    auto step = [&](const int m, const int slot, const int rs, const int h, double (&ca)[NI],
                     double (&cb)[NI]) -> bool {
         const double2* T = &sm.wt[slot][h][w * RT * NC];
         const double* LM = &sm.hdr[w][h][0];
@@ -562,36 +592,50 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             if (m < l0) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
         }
         if (wrote) {
-            if (!waited) { mbar_wait(&sm.rempty[rs], rparity); waited = true; }
             double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
 #pragma unroll
             for (int r = 0; r < RL; ++r)
 #pragma unroll
-                for (int c = 0; c < NC; ++c) rd[(lane + 32 * r) * NC + c] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
+                for (int c = 0; c < NC; ++c) {
+                    rd[c * TLB + lane + 32 * r] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
+                }
         }
         return wrote;
     };
+    constexpr int PB = 8;
+#ifdef SHT_PROF
+    const long long tloop__ = clock64();
+#endif
     for (int p = 0; p < npairs; ++p) {
         const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
         const uint32_t rparity = ((p / NRS) & 1) ^ 1;
-        mbar_wait(&sm.full[slot], (p / NST) & 1);
+        { PROF_T0(); mbar_wait(&sm.full[slot], (p / NST) & 1); PROF_ADD(PB + 0); }
+        { PROF_T0(); mbar_wait(&sm.rempty[rs], rparity); PROF_ADD(PB + 1); }
         // lambda' of this warp's rings for both steps of the pair: lane -> (step h, ring i)
         if (lane < KS * RT) {
             const int h = lane / RT, i = lane % RT;
             sm.hdr[w][h][i] = sm.lamraw[slot][h][w * RT + i] * sm.sg[slot][KS - 1 - h].x;
         }
         __syncwarp();
-        bool waited = false;
         int flags = 0;
-        if (step(m, slot, rs, 0, rparity, waited, cur, prev)) flags |= 1;
-        if (step(m - 1, slot, rs, 1, rparity, waited, prev, cur)) flags |= 2;
+        if (step(m, slot, rs, 0, cur, prev)) flags |= 1;
+        if (step(m - 1, slot, rs, 1, prev, cur)) flags |= 2;
         __syncwarp();
         if (lane == 0) {
-            if (!waited) mbar_wait(&sm.rempty[rs], rparity);
             sm.act[rs][w] = flags;
             mbar_arrive(&sm.rfull[rs]);
         }
+#ifdef SHT_PROF
+        pc__[0]++; if (flags == 3) pc__[1]++; if (flags == 0) pc__[2]++;
+#endif
     }
+#ifdef SHT_PROF
+    if (lane == 0) {
+        atomicAdd(&g_prof[PB + 2], (unsigned long long)(clock64() - tloop__));
+        atomicAdd(&g_prof[PB + 0], pf__[0]); atomicAdd(&g_prof[PB + 1], pf__[1]);
+        atomicAdd(&g_prof[PB + 3], pc__[0]); atomicAdd(&g_prof[PB + 4], pc__[1]); atomicAdd(&g_prof[PB + 5], pc__[2]);
+    }
+#endif
 }
 
 // register-only DFMA chains: the FP64 roofline denominator is measured, not assumed
@@ -639,6 +683,12 @@ cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
 
 // Tile shapes: inverse 64 degrees x 128 rings per block (8 compute warps, 8 degrees x 4 rings per thread);
 //              forward 64 degrees x 128 rings per block (8 compute warps, 2 degrees x 16 rings per thread).
+#ifdef SHT_PROF
+extern "C" void sht_prof_read(unsigned long long* out, int reset) {
+    cudaMemcpyFromSymbol(out, g_prof, sizeof(g_prof));
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_prof, z, sizeof(z)); }
+}
+#endif
 int theta_inverse_rowd(int mode) { return mode == 0 ? 6 : 4; }
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
