@@ -60,6 +60,14 @@ const char* sht_last_error(void);       /* text of the last CUDA / cuFFT failure
  */
 sht_status sht_plan_s2(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype);
 sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);
+/* A batch of `batch` S^2 problems with identical (L, spin, sampling, reality) transformed together (BASELINE config 5b):
+ * the Wigner-d recursion is run once and shared by all maps, which turns the theta / l contraction of Eq. 30 / 33
+ * into a dense GEMM per harmonic order m (the einsum of Sec. 4.3, without storing the d-functions); it
+ * runs on the FP64 tensor cores.  Arrays gain a leading [batch] axis: f[batch][L][2L-1], flm[batch][L][2L-1].
+ * batch = 1 is sht_plan_s2().  MW sampling only (HEALPix with batch > 1: SHT_EUNSUPPORTED).  The theta-stage entry
+ * points below are single-map only. */
+sht_status sht_plan_s2_batch(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype, int batch);
+int        sht_plan_batch(const sht_plan* plan);
 size_t     sht_plan_workspace_bytes(const sht_plan* plan);
 sht_status sht_plan_set_workspace(sht_plan* plan, void* work, size_t work_bytes, sht_stream stream);
 sht_status sht_plan_destroy(sht_plan* plan);

@@ -16,6 +16,8 @@ SIGNATURES = {
     "sht_last_error": (C.c_char_p, []),
     "sht_plan_s2": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i]),
     "sht_plan_so3": (_i, [C.POINTER(_vp), _i, _i, _i]),
+    "sht_plan_s2_batch": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i, _i]),
+    "sht_plan_batch": (_i, [_vp]),
     "sht_plan_workspace_bytes": (_sz, [_vp]),
     "sht_plan_set_workspace": (_i, [_vp, _vp, _sz, _vp]),
     "sht_plan_destroy": (_i, [_vp]),

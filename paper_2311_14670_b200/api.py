@@ -34,14 +34,15 @@ def map_shape(L, sampling=MW, nside=0):
 class Plan:
     """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
 
-    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0"):
+    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1):
         self._h = C.c_void_p()
         self.L, self.spin, self.sampling, self.nside, self.reality, self.N = L, spin, sampling, nside, bool(reality), N
+        self.batch = int(batch)
         self.device = torch.device(device)
         L_ = lib()
         with torch.cuda.device(self.device):
             if N is None:
-                check(L_.sht_plan_s2(C.byref(self._h), L, spin, sampling, nside, int(self.reality), SHT_F64))
+                check(L_.sht_plan_s2_batch(C.byref(self._h), L, spin, sampling, nside, int(self.reality), SHT_F64, self.batch))
             else:
                 check(L_.sht_plan_so3(C.byref(self._h), L, N, SHT_F64))
             nbytes = L_.sht_plan_workspace_bytes(self._h)
@@ -50,6 +51,9 @@ class Plan:
         self.map_dtype = torch.float64 if self.reality else torch.complex128
         self.coef_shape = (L, 2 * L - 1) if N is None else (2 * N - 1, L, 2 * L - 1)
         self.map_shape = map_shape(L, sampling, nside) if N is None else (2 * N - 1, L, 2 * L - 1)
+        if self.batch > 1:            # a batch of maps transformed together: leading [batch] axis on both sides
+            self.coef_shape = (self.batch,) + self.coef_shape
+            self.map_shape = (self.batch,) + self.map_shape
 
     def __del__(self):
         try:

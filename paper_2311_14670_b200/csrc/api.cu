@@ -77,6 +77,10 @@ struct sht_plan {
     int L = 0, spin = 0, sampling = 0, nside = 0, reality = 0, N = 1;
     int Lp = 0, NB = 0;        // padded L; 2L-1
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
+    int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
+    int ncg = 0;               // batched path: column groups of 16 complex columns
+    double* Ob = nullptr;      // batched path: result scratch of all passes
+    std::vector<size_t> ob_off_inv, ob_off_fwd;   // per-pass offsets (doubles) into Ob
     std::vector<int> slab_n;   // second index n of d^l_{m,n} per slab
     RingSet inv, fwd;          // rings of the inverse theta step / of the forward quadrature
     int kmin = 0, kstride = 0, krows = 0;
@@ -152,6 +156,14 @@ struct Bump {
     }
 };
 
+// doubles of one pass's operand buffer (single-map kernels: rows m_end-1..L-1; batched: rows m_end..L-1 per column group)
+size_t pass_in_doubles(const sht_plan* P, const PassHost& ph, bool fwd) {
+    const size_t K = fwd ? P->fwd.ntp : P->Lp;
+    if (P->batch > 1) return (size_t)P->ncg * (P->L - ph.p.m_end) * K * SHT_MMA_ROW;
+    const size_t rows = (size_t)(P->L - ph.p.m_end + 1);
+    return fwd ? rows * K * (ph.mode == 0 ? 4 : 2) : rows * K * theta_inverse_rowd(ph.mode);
+}
+
 void stage(sht_plan* P, int cat, cudaStream_t st) {
     if (!P->timing) return;
     if (P->ev_n >= (int)P->ev.size()) return;
@@ -186,12 +198,19 @@ void layout(sht_plan* P, char* base) {
     // per-pass operand buffers and lambda tables
     // (rows m = m_end-1 .. L-1; row m_end-1 is all zero: the dummy second step of a final odd pair reads it)
     for (auto& ph : P->pinv) {
-        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end + 1) * Lp * theta_inverse_rowd(ph.mode));
+        ph.p.in = B.take<double>(pass_in_doubles(P, ph, false));
         ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->inv.ntp);
     }
     for (auto& ph : P->pfwd) {
-        ph.p.in = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->fwd.ntp * (ph.mode == 0 ? 4 : 2));
+        ph.p.in = B.take<double>(pass_in_doubles(P, ph, true));
         ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->fwd.ntp);
+    }
+    if (P->batch > 1) {
+        size_t oi = 0, of = 0;
+        P->ob_off_inv.clear(); P->ob_off_fwd.clear();
+        for (auto& ph : P->pinv) { P->ob_off_inv.push_back(oi); oi += (size_t)P->ncg * (L - ph.p.m_end) * P->inv.ntp * SHT_MMA_NCOL; }
+        for (auto& ph : P->pfwd) { P->ob_off_fwd.push_back(of); of += (size_t)P->ncg * (L - ph.p.m_end) * Lp * SHT_MMA_NCOL; }
+        P->Ob = B.take<double>(oi > of ? oi : of);
     }
     // scratch arrays
     P->F_slab = (size_t)NB * P->inv.ntp;
@@ -216,12 +235,16 @@ void layout(sht_plan* P, char* base) {
     P->Z = B.take<double2>(P->Z_slab * P->nslab);
     P->H_slab = (size_t)NB * Lp;
     P->H = B.take<double2>(P->H_slab * P->nslab);
-    if (P->reality && P->sampling == SHT_MW) P->cplx = B.take<double2>((size_t)L * NB);
+    if (P->reality && P->sampling == SHT_MW) P->cplx = B.take<double2>((size_t)L * NB * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
     P->fft_work = B.take<char>(P->fft_work_bytes);
     // route every pass to its slab's output array
     for (auto& ph : P->pinv) ph.p.out = P->F ? P->F + P->F_slab * ph.p.slab : nullptr;
     for (auto& ph : P->pfwd) ph.p.out = P->H ? P->H + P->H_slab * ph.p.slab : nullptr;
+    if (P->batch > 1 && P->Ob) {
+        for (size_t i = 0; i < P->pinv.size(); ++i) P->pinv[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_inv[i]);
+        for (size_t i = 0; i < P->pfwd.size(); ++i) P->pfwd[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_fwd[i]);
+    }
     P->need_bytes = rup(B.off, 256);
 }
 
@@ -300,7 +323,11 @@ sht_status plan_common(sht_plan* P) {
     P->krows = P->Lp / SHT_TQ;
     P->mmin = -nmax - 1;           // one row below the lowest recursion step (dummy step of an odd final pair)
     P->sgstride = (int)rup((size_t)(L - P->mmin), 2);
-    for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
+    if (P->batch > 1) {            // one pass list serves every map of the batch
+        add_passes(P, 0, P->slab_n[0], P->reality != 0);
+        P->ncg = (P->batch * (P->pinv[0].mode == 0 ? 2 : 1) + 15) / 16;
+    } else
+        for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
     // d-step counts: rings * sum over l of the steps each pass runs
     for (int dir = 0; dir < 2; ++dir) {
         double tot = 0; const RingSet& R = dir ? P->fwd : P->inv;
@@ -379,12 +406,12 @@ sht_status upload_passes(sht_plan* P, cudaStream_t st) {
             ph.p = t;
             {   // zero the operand / lambda buffers once (their first row stays zero for good), then fill the lambda table
                 const size_t rows = (size_t)(P->L - t.m_end + 1);
-                const size_t in_doubles = dir ? rows * R.ntp * (ph.mode == 0 ? 4 : 2) : rows * P->Lp * theta_inverse_rowd(ph.mode);
+                const size_t in_doubles = pass_in_doubles(P, ph, dir != 0);
                 CK(cudaMemsetAsync(const_cast<double*>(t.in), 0, in_doubles * sizeof(double), st));
                 CK(cudaMemsetAsync(const_cast<double*>(t.lam), 0, rows * R.ntp * sizeof(double), st));
                 CK(st_lamtab(t.n, R.nth, R.ntp, t.m_end, P->L - t.m_end, R.csc, R.tau, R.sig, const_cast<double*>(t.lam) + R.ntp, st));
             }
-            (ph.mode == 0 ? pm : p).push_back(t);
+            (ph.mode == 0 && P->batch == 1 ? pm : p).push_back(t);
         }
         ThetaPass* dpm = dir ? P->d_fwd_pm : P->d_inv_pm; ThetaPass* dp = dir ? P->d_fwd_p : P->d_inv_p;
         if (!pm.empty()) CK(cudaMemcpyAsync(dpm, pm.data(), pm.size() * sizeof(ThetaPass), cudaMemcpyHostToDevice, st));
@@ -406,11 +433,61 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     return a;
 }
 
+MmaArgs mma_args(const sht_plan* P, bool fwd) {
+    const RingSet& R = fwd ? P->fwd : P->inv;
+    MmaArgs a{};
+    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.ncg = P->ncg;
+    a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin;
+    a.passes = fwd ? P->d_fwd_p : P->d_inv_p;
+    a.npass = fwd ? P->n_fwd_p : P->n_inv_p;
+    return a;
+}
+
 // ---- the stages --------------------------------------------------------------------------------------------------
 // coef: nslab slabs of [L][NB] in *slab order*.  Leaves F[slab][row][ring] complete (all rows, incl. the pole ring).
 sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) {
     const int L = P->L;
     stage(P, CAT_STAGE, st);
+    if (P->batch > 1) {
+        // batched path: one recursion for all maps, contraction on FP64 tensor-core MMAs (theta_mma.cu).  All passes of a
+        // plan have the same m_end up to 1, but their operand / result buffers are separate; the kernel takes the
+        // column-group strides of the FIRST pass, so passes are launched one by one when their row counts differ.
+        CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab * P->nslab, st));
+        for (size_t i = 0; i < P->pinv.size(); ++i) {
+            auto& ph = P->pinv[i];
+            const int NC = ph.mode == 0 ? 2 : 1;
+            const size_t rows = (size_t)(L - ph.p.m_end);
+            CK(st_prep_inverse_batch(L, P->Lp, NC, P->batch, P->ncg, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef, P->scale_inv,
+                                     P->ctab, P->sgtab, P->sgstride, const_cast<double*>(ph.p.in), rows * P->Lp * SHT_MMA_ROW, st));
+            CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg * rows * P->inv.ntp * SHT_MMA_NCOL, st));
+        }
+        stage(P, CAT_HOT, st);
+        for (size_t i = 0; i < P->pinv.size(); ++i) {
+            MmaArgs a = mma_args(P, false);
+            const size_t rows = (size_t)(L - P->pinv[i].p.m_end);
+            a.passes += i; a.npass = 1;
+            a.in_cg_stride = rows * P->Lp * SHT_MMA_ROW; a.out_cg_stride = rows * P->inv.ntp * SHT_MMA_NCOL;
+            CK(launch_theta_mma(a, false, st));
+        }
+        stage(P, CAT_STAGE, st);
+        for (size_t i = 0; i < P->pinv.size(); ++i) {
+            auto& ph = P->pinv[i];
+            const size_t rows = (size_t)(L - ph.p.m_end);
+            CK(st_unpack_batch(L, P->Lp, P->inv.ntp, P->inv.nth, ph.mode == 0 ? 2 : 1, P->batch, P->ncg, ph.p.n, ph.p.sgn_out, ph.p.m_end,
+                               P->mmin, 0, P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->inv.ntp * SHT_MMA_NCOL, P->F,
+                               P->F_slab, P->inv.ntp, st));
+        }
+        if (P->inv.pole) {
+            for (int s = 0; s < P->nslab; ++s) {
+                int n = P->slab_n[s];
+                int row = (-n) < 0 ? -n + P->NB : -n;
+                CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->inv.ntp + P->inv.nth, st));
+            }
+        }
+        if (P->reality)
+            for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->inv.ntp, P->inv.nth + (P->inv.pole ? 1 : 0), P->F + P->F_slab * s, st));
+        return SHT_OK;
+    }
     for (auto& ph : P->pinv)
         CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->NB,
                            P->scale_inv, P->ctab, P->sgtab, P->sgstride,
@@ -435,6 +512,37 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
 sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int ldu, cudaStream_t st) {
     const int L = P->L;
     stage(P, CAT_STAGE, st);
+    if (P->batch > 1) {
+        CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
+        for (size_t i = 0; i < P->pfwd.size(); ++i) {
+            auto& ph = P->pfwd[i];
+            const size_t rows = (size_t)(L - ph.p.m_end);
+            CK(st_weight_split_batch(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg, P->slab_n[0],
+                                     ph.p.sgn_out, ph.p.m_end, ph.p.m_lo, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
+                                     rows * P->fwd.ntp * SHT_MMA_ROW, st));
+            CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg * rows * P->Lp * SHT_MMA_NCOL, st));
+        }
+        stage(P, CAT_HOT, st);
+        for (size_t i = 0; i < P->pfwd.size(); ++i) {
+            MmaArgs a = mma_args(P, true);
+            const size_t rows = (size_t)(L - P->pfwd[i].p.m_end);
+            a.passes += i; a.npass = 1;
+            a.in_cg_stride = rows * P->fwd.ntp * SHT_MMA_ROW; a.out_cg_stride = rows * P->Lp * SHT_MMA_NCOL;
+            CK(launch_theta_mma(a, true, st));
+        }
+        stage(P, CAT_STAGE, st);
+        for (size_t i = 0; i < P->pfwd.size(); ++i) {
+            auto& ph = P->pfwd[i];
+            const size_t rows = (size_t)(L - ph.p.m_end);
+            CK(st_unpack_batch(L, P->Lp, P->Lp, L, ph.mode == 0 ? 2 : 1, P->batch, P->ncg, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, 1,
+                               P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->Lp * SHT_MMA_NCOL, P->H, P->H_slab, P->Lp, st));
+        }
+        if (P->fwd.pole) {
+            for (int s = 0; s < P->nslab; ++s)
+                CK(st_pole_forward(L, P->Lp, P->slab_n[s], P->NB, ldu, P->fwd.nth, P->fwd.wq, U + U_slab * s, P->H + P->H_slab * s, st));
+        }
+        return SHT_OK;
+    }
     for (auto& ph : P->pfwd) {
         int n_slab = P->slab_n[ph.p.slab];
         CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.m_lo,
@@ -540,15 +648,20 @@ const char* sht_version(void) { return "b200sht 0.1 (sm_100a)"; }
 long sht_launch_count(int reset) { long v = g_launches; if (reset) g_launches = 0; return v; }
 
 sht_status sht_plan_s2(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype) {
+    return sht_plan_s2_batch(out, L, spin, sampling, nside, reality, dtype, 1);
+}
+sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch) {
     if (!out) return SHT_EINVAL;
     *out = nullptr;
+    if (batch < 1 || batch > 1024) return SHT_EINVAL;
+    if (batch > 1 && sampling != SHT_MW) return SHT_EUNSUPPORTED;
     if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || (sampling != SHT_MW && sampling != SHT_HEALPIX)) return SHT_EINVAL;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
-    P->nslab = 1; P->slab_n = {-spin};        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
+    P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L); }
     else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
     sht_status s = plan_common(P);
@@ -572,6 +685,7 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     return SHT_OK;
 }
 size_t sht_plan_workspace_bytes(const sht_plan* P) { return P ? P->need_bytes : 0; }
+int sht_plan_batch(const sht_plan* P) { return P ? P->batch : 0; }
 int sht_plan_ntheta(const sht_plan* P, int forward) {
     if (!P) return 0;
     const RingSet& R = forward ? P->fwd : P->inv;
@@ -670,6 +784,7 @@ sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
 sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
+    if (P->batch > 1) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
@@ -681,6 +796,7 @@ sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_str
 sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_stream stream) {
     CS(check_ready(P));
     if (!Wm || !flm || P->kind != 0) return SHT_EINVAL;
+    if (P->batch > 1) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     P->ev_n = 0;
     // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
@@ -710,8 +826,9 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     stage(P, CAT_FFT, st);
     CF(cufftSetStream(P->fft_phi_inv, st));
     double2* outc = P->reality ? P->cplx : (double2*)f;
-    CF(cufftExecZ2Z(P->fft_phi_inv, P->F, outc, CUFFT_INVERSE));                      // Eq. 32
-    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_complex_to_real((size_t)L * NB, P->cplx, (double*)f, st)); }
+    for (int b = 0; b < P->batch; ++b)
+        CF(cufftExecZ2Z(P->fft_phi_inv, P->F + P->F_slab * b, outc + (size_t)L * NB * b, CUFFT_INVERSE));   // Eq. 32
+    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_complex_to_real((size_t)L * NB * P->batch, P->cplx, (double*)f, st)); }
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
@@ -730,14 +847,16 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
         return SHT_OK;
     }
     const double2* fin = (const double2*)f;
-    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex((size_t)L * NB, (const double*)f, P->cplx, st)); fin = P->cplx; }
+    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex((size_t)L * NB * P->batch, (const double*)f, P->cplx, st)); fin = P->cplx; }
     stage(P, CAT_FFT, st);
     CF(cufftSetStream(P->fft_phi_fwd, st));
-    CF(cufftExecZ2Z(P->fft_phi_fwd, const_cast<double2*>(fin), P->Fa, CUFFT_FORWARD)); // Eq. 31 (weight folded into q_u)
+    for (int b = 0; b < P->batch; ++b)                                                 // Eq. 31 (weight folded into q_u)
+        CF(cufftExecZ2Z(P->fft_phi_fwd, const_cast<double2*>(fin) + (size_t)L * NB * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD));
     CS(mw_upsample(P, st));
     CS(run_theta_forward(P, P->Z, P->Z_slab, 4 * L - 1, st));
     stage(P, CAT_STAGE, st);
-    CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H, (double2*)flm, st));
+    for (int b = 0; b < P->batch; ++b)
+        CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + (size_t)L * NB * b, st));
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }

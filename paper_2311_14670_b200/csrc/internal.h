@@ -47,6 +47,24 @@ struct ThetaArgs {
     int npass;
 };
 
+// ---- batched path (theta_mma.cu): the contraction of a batch of maps runs on FP64 tensor-core MMAs -----------------
+#define SHT_MMA_NCOL 32   // real columns per column group = 16 complex columns (map, +-m)
+#define SHT_MMA_ROW 36    // doubles per operand row: 32 columns + 2 side columns + 2 pad (conflict-free LDS.64)
+// Operand rows, one per (column group, m - m_end, K index), SHT_MMA_ROW doubles:
+//   inverse  Gb[cg][m-m_end][Lp][36]:  32 columns c_m(l) scale(l) f_lm (re, im per complex column), [32] g'_m(l), [33] s_m
+//   forward  Wb[cg][m-m_end][ntp][36]: 32 columns q(theta) F_m(theta),                                [32] lambda_m(theta)
+// Results:   Ob[cg][m-m_end][Mp][32]   (Mp = ntp rings on the inverse, Lp degrees on the forward), accumulated by bulk reduce.
+struct MmaArgs {
+    int L, Lp, nth, ntp;
+    int ncg;                   // column groups (gridDim.z)
+    const double2* sg;         // (s_m, G_m) per quantum, as in ThetaArgs
+    int sgstride, mmin;
+    size_t in_cg_stride, out_cg_stride;   // doubles between column groups of ThetaPass::in / ::out
+    const ThetaPass* passes;   // in = Gb / Wb of the pass, out = Ob of the pass, lam / st_val / st_k / m_lo as in the single-map kernels
+    int npass;
+};
+cudaError_t launch_theta_mma(const MmaArgs& a, bool forward, cudaStream_t st);
+
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st);
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st);

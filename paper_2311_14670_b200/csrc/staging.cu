@@ -309,6 +309,111 @@ __global__ void k_scale_copy(size_t n, double s, const double2* __restrict__ in,
     if (i < n) out[i] = make_double2(s * in[i].x, s * in[i].y);
 }
 
+// ---- batched path (theta_mma.cu; operand layouts in internal.h) ----------------------------------------------------
+// Complex column j = cg*16 + jc of a pass belongs to map b = j / NC and, with NC = 2 (spin 0 complex), to order +m
+// (c = 0) or -m (c = 1); columns j >= B*NC are zero padding.
+// inverse prep: coef[b][l][NB] -> Gb[cg][m-m_end][Lp][36].  Block = 16 degrees x 8 orders x one column group.
+__global__ void k_prep_inverse_batch(int L, int Lp, int NC, int B, int n, int sgn_out, int m_end, int mmin,
+                                     const double2* __restrict__ coef, const double* __restrict__ scale, const double* __restrict__ C,
+                                     const double2* __restrict__ SG, int sgstride, double* __restrict__ Gb, size_t cg_stride) {
+    __shared__ double2 tile[16][16][9];
+    const int NB = 2 * L - 1, an = n < 0 ? -n : n, cg = blockIdx.z;
+    const int l0 = blockIdx.x * 16, m0 = m_end + blockIdx.y * 8;
+    const int tx = threadIdx.x & 7, ty = threadIdx.x >> 3;
+    for (int jc = 0; jc < 16; ++jc) {
+        const int j = cg * 16 + jc, b = j / NC, c = j % NC;
+        const int l = l0 + ty, m = m0 + tx, am = m < 0 ? -m : m;
+        const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
+        double2 v = make_double2(0.0, 0.0);
+        if (b < B && l < L && m < L && l >= an && l >= am && !(c == 1 && m == 0)) {
+            v = coef[((size_t)b * L + l) * NB + m_out + L - 1];
+            double sgn = 1.0;
+            if (c == 1) sgn = sgn_pow(m);
+            else if (sgn_out < 0) sgn = sgn_pow(m + n);
+            const double cm = sgn * scale[l] * C[(size_t)(m - mmin) * Lp + l];
+            v.x *= cm; v.y *= cm;
+        }
+        tile[ty][jc][tx] = v;
+    }
+    __syncthreads();
+    for (int mi = 0; mi < 8; ++mi) {
+        const int m = m0 + mi;
+        if (m >= L) break;
+        double* g = Gb + (size_t)cg * cg_stride + ((size_t)(m - m_end) * Lp + l0) * SHT_MMA_ROW;
+        for (int idx = threadIdx.x; idx < 16 * SHT_MMA_ROW; idx += blockDim.x) {
+            const int li = idx / SHT_MMA_ROW, col = idx % SHT_MMA_ROW, l = l0 + li;
+            double v = 0.0;
+            if (col < SHT_MMA_NCOL) { const double2 t = tile[li][col >> 1][mi]; v = (col & 1) ? t.y : t.x; }
+            else if (col == SHT_MMA_NCOL) v = l < L ? (double)(l - m) * (double)(l + m + 1) * SG[(size_t)(l / SHT_TQ) * sgstride + (m - mmin)].y : 0.0;
+            else if (col == SHT_MMA_NCOL + 1) v = SG[(size_t)(l / SHT_TQ) * sgstride + (m - mmin)].x;
+            g[idx] = v;
+        }
+    }
+}
+// forward split: U[b][bin][ldu] -> Wb[cg][m-m_end][ntp][36] (weighted, masked by the peak split; [32] = lambda_m(theta)).
+// Block = 32 rings x one order x one column group.
+__global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int n, int sgn_out,
+                                     int m_end, const int* __restrict__ m_lo, const double* __restrict__ wq,
+                                     const double* __restrict__ lam, const double2* __restrict__ U, double* __restrict__ Wb,
+                                     size_t cg_stride) {
+    __shared__ double2 tile[32][17];
+    const int cg = blockIdx.z, m = m_end + blockIdx.y, t0 = blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, th = t0 + tx;
+    for (int jc = ty; jc < 16; jc += 4) {
+        const int j = cg * 16 + jc, b = j / NC, c = j % NC;
+        double2 v = make_double2(0.0, 0.0);
+        bool ok = b < B && th < nth && !(c == 1 && m == 0) && m < L && m > -L;
+        if (ok && m_lo) ok = m >= m_lo[th];
+        if (ok) {
+            const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
+            double s = wq[th];
+            if (c == 1) s *= sgn_pow(m);
+            else if (sgn_out < 0) s *= sgn_pow(m + n);
+            const double2 x = U[(size_t)b * U_slab + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + th];
+            v.x = s * x.x; v.y = s * x.y;
+        }
+        tile[tx][jc] = v;
+    }
+    __syncthreads();
+    double* g = Wb + (size_t)cg * cg_stride + ((size_t)(m - m_end) * ntp + t0) * SHT_MMA_ROW;
+    for (int idx = threadIdx.x; idx < 32 * SHT_MMA_ROW; idx += blockDim.x) {
+        const int ti = idx / SHT_MMA_ROW, col = idx % SHT_MMA_ROW;
+        double v = 0.0;
+        if (col < SHT_MMA_NCOL) { const double2 t = tile[ti][col >> 1]; v = (col & 1) ? t.y : t.x; }
+        else if (col == SHT_MMA_NCOL) v = lam[(size_t)(m - m_end + 1) * ntp + t0 + ti];
+        g[idx] = v;
+    }
+}
+// results: Ob[cg][m-m_end][Mp][32] -> out[b][row(m_out)][ld] += factor * value, complex.  fwd = 0: rows are phi-FFT bins
+// (m_out mod NB) of F, columns rings; fwd = 1: rows m_out+L-1 of H, columns degrees, factor c_m(l) (internal.h).
+__global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int n, int sgn_out, int m_end, int mmin, int fwd,
+                               const double* __restrict__ C, const double* __restrict__ Ob, size_t cg_stride,
+                               double2* __restrict__ out, size_t out_slab, int ld) {
+    __shared__ double tile[32][33];
+    const int NB = 2 * L - 1, an = n < 0 ? -n : n;
+    const int cg = blockIdx.z, m = m_end + blockIdx.y, i0 = blockIdx.x * 32;
+    const double* src = Ob + (size_t)cg * cg_stride + ((size_t)(m - m_end) * Mp + i0) * SHT_MMA_NCOL;
+    for (int idx = threadIdx.x; idx < 32 * SHT_MMA_NCOL; idx += blockDim.x) tile[idx / SHT_MMA_NCOL][idx % SHT_MMA_NCOL] = src[idx];
+    __syncthreads();
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, mi = i0 + tx, am = m < 0 ? -m : m;
+    if (mi >= mlim || m >= L || m <= -L) return;
+    double fac = 1.0;
+    if (fwd) {
+        if (mi < an || mi < am) return;
+        fac = C[(size_t)(m - mmin) * Lp + mi];
+    }
+    for (int jc = ty; jc < 16; jc += 4) {
+        const int j = cg * 16 + jc, b = j / NC, c = j % NC;
+        if (b >= B || (c == 1 && m == 0)) continue;
+        const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
+        const int row = fwd ? m_out + L - 1 : (m_out < 0 ? m_out + NB : m_out);
+        double2* o = out + (size_t)b * out_slab + (size_t)row * ld + mi;
+        double2 v = *o;
+        v.x += fac * tile[tx][2 * jc]; v.y += fac * tile[tx][2 * jc + 1];
+        *o = v;
+    }
+}
+
 inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 }  // namespace
@@ -403,5 +508,25 @@ cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int t
 }
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st) {
     k_scale_copy<<<cdiv(n, 256), 256, 0, st>>>(n, s, in, out);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, const double2* coef,
+                                  const double* scale, const double* C, const double2* SG, int sgstride, double* Gb, size_t cg_stride,
+                                  cudaStream_t st) {
+    dim3 grid(cdiv(Lp, 16), cdiv(L - m_end, 8), ncg);
+    k_prep_inverse_batch<<<grid, 128, 0, st>>>(L, Lp, NC, B, n, sgn_out, m_end, mmin, coef, scale, C, SG, sgstride, Gb, cg_stride);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
+                                  int m_end, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
+                                  size_t cg_stride, cudaStream_t st) {
+    dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
+    k_weight_split_batch<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, NC, B, n, sgn_out, m_end, m_lo, wq, lam, U, Wb, cg_stride);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd,
+                            const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st) {
+    dim3 grid(cdiv(Mp, 32), L - m_end, ncg);
+    k_unpack_batch<<<grid, 128, 0, st>>>(L, Lp, Mp, mlim, NC, B, n, sgn_out, m_end, mmin, fwd, C, Ob, cg_stride, out, out_slab, ld);
     LAUNCHED(); return cudaSuccess;
 }

@@ -27,6 +27,16 @@ cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* sc
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st);
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st);
 
+// batched path (operand / result layouts of theta_mma.cu, internal.h)
+cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, const double2* coef,
+                                  const double* scale, const double* C, const double2* SG, int sgstride, double* Gb, size_t cg_stride,
+                                  cudaStream_t st);
+cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
+                                  int m_end, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
+                                  size_t cg_stride, cudaStream_t st);
+cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd,
+                            const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st);
+
 // HEALPix ring Fourier staging (healpix.cu)
 void hp_ring_host(int nside, int i, int* nphi, int* shifted, long long* off);
 cudaError_t st_hp_chirp(int nside, int M, double2* BF, cudaStream_t st);

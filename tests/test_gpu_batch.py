@@ -1,0 +1,93 @@
+"""GPU parity of the batched path (BASELINE.json configs[4] second half): a batch of S^2 maps sharing
+one recursion, contraction on FP64 tensor-core MMAs (csrc/theta_mma.cu).  Every map of the batch is compared with the
+CPU oracle element by element at small sizes (several 64 x 128 tiles plus ragged tails in L, rings and batch), and at
+the full size of the config (16 maps, L = 2048) on sampled rings / harmonic orders plus the exact MW round trip."""
+import numpy as np
+import pytest
+
+from paper_2311_14670_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+
+def rel(a, b, scale=None):
+    return float(np.abs(a - b).max() / (np.abs(b).max() if scale is None else scale))
+
+
+@pytest.fixture(scope="module")
+def api():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_14670_b200 import api as A
+    return A
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# batch sizes: 16 complex columns per group -> spin 0 complex (2 columns per map): 8 maps fill one group, 3 leave
+# padding, 9 straddle two groups; spin != 0 (1 column per map and pass, two passes); real (1 column per map)
+@pytest.mark.parametrize("L,spin,batch,real", [(8, 0, 2, False), (33, 0, 3, False), (64, 0, 8, False), (130, 0, 9, False),
+                                               (200, 0, 16, False), (48, 2, 5, False), (131, -2, 17, False), (65, 1, 16, False),
+                                               (96, 0, 4, True), (257, 0, 2, False)])
+def test_batched_s2_vs_oracle(api, orc, L, spin, batch, real):
+    flm = np.stack([synth.random_flm(L, spin, seed=100 * L + b, real=real) for b in range(batch)])
+    P = api.Plan(L, spin, reality=real, batch=batch)
+    f = P.inverse(dev(flm)).cpu().numpy()
+    f_ref = np.stack([orc.s2_inverse(L, spin, orc.MW, flm[b]) for b in range(batch)])
+    if real:
+        assert np.abs(f_ref.imag).max() < 1e-12 * np.abs(f_ref).max()
+        f_ref = np.ascontiguousarray(f_ref.real)
+    assert rel(f, f_ref) < TOL
+    back = P.forward(dev(f_ref)).cpu().numpy()
+    assert rel(back, flm) < TOL                                   # sampling theorem: exact round trip (pin 6)
+    for b in (0, batch - 1):
+        assert rel(back[b], orc.s2_forward(L, spin, orc.MW, f_ref[b].astype(np.complex128))) < TOL
+    # coefficients outside the support are exact zeros
+    el = np.arange(L)[:, None]
+    m = np.arange(-(L - 1), L)[None, :]
+    assert np.all(back[:, (np.abs(m) > el) | (el < abs(spin))] == 0)
+
+
+def test_batched_equals_single_map_plans(api):
+    """The batched kernels and the single-map kernels run the same recursion: results agree to rounding."""
+    L, spin, batch = 192, 0, 6
+    flm = np.stack([synth.random_flm(L, spin, seed=b) for b in range(batch)])
+    Pb, P1 = api.Plan(L, spin, batch=batch), api.Plan(L, spin)
+    fb = Pb.inverse(dev(flm))
+    f1 = torch.stack([P1.inverse(dev(flm[b])) for b in range(batch)])
+    assert float((fb - f1).abs().max() / f1.abs().max()) < 1e-13
+    g = synth.random_map((batch, L, 2 * L - 1), seed=5)
+    cb = Pb.forward(dev(g))
+    c1 = torch.stack([P1.forward(dev(g[b])) for b in range(batch)])
+    assert float((cb - c1).abs().max() / c1.abs().max()) < 1e-13
+
+
+def test_config5b_batch16_L2048(api, orc):
+    """configs[4], second half: 16 maps at L = 2048, spin 0, MW, sigma_l = 1/(l+1), seeds 4+b."""
+    L, batch = 2048, 16
+    flm = np.stack([synth.random_flm(L, 0, seed=4 + b, sigma=synth.SIGMA_RED) for b in range(batch)])
+    P = api.Plan(L, 0, batch=batch)
+    d = dev(flm)
+    f = P.inverse(d)
+    back = P.forward(f)
+    assert float((back - d).abs().max() / d.abs().max()) < TOL       # exact round trip for every map
+    rings = np.array([0, 3, 1000, 2046, 2047])
+    for b in (0, 7, 15):
+        rows = orc.s2_inverse_rings(L, 0, orc.MW, flm[b], rings)
+        scale = max(np.abs(r).max() for r in rows)
+        fb = f[b].cpu().numpy()
+        for r, row in zip(rings, rows):
+            assert rel(fb[r], row, scale) < TOL, (b, r)
+    # forward of white-noise maps against the oracle on sampled orders m
+    g = synth.random_map((batch, L, 2 * L - 1), seed=21)
+    got = P.forward(dev(g))
+    ms = np.array([-(L - 1), -1000, -1, 0, 1, 2, 777, L - 1])
+    for b in (0, 15):
+        want = orc.s2_forward_columns(L, 0, orc.MW, g[b], ms)
+        sc = np.abs(want).max()
+        gb = got[b].cpu().numpy()
+        for m, col in zip(ms, want):
+            assert rel(gb[:, m + L - 1], col, sc) < TOL, (b, m)
