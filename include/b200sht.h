@@ -73,9 +73,10 @@ sht_status sht_plan_set_workspace(sht_plan* plan, void* work, size_t work_bytes,
 sht_status sht_plan_destroy(sht_plan* plan);
 
 /* ---- transforms through a plan (device pointers) -----------------------------------------------------------
- * s2_forward : map f -> flm.  MW: FFT in phi (Eq. 31), extension to the torus and 2x upsampling in theta
- *              (PAPER.md:379-381), quadrature weights Eq. 41-44 at band-limit 2L, then the fused recursion +
- *              theta contraction of Eq. 30.  HEALPix: ring FFTs with phase shift and periodic extension
+ * s2_forward : map f -> flm.  MW: FFT in phi (Eq. 31), extension to the torus and upsampling in theta to 2L
+ *              rings (the rings are theta'_u = (2u+1) pi/(4L), u = 0..2L-1, on which the
+ *              quadrature of Eq. 41-44 is exact for the band-limit-(2L-2) integrand), then the fused recursion
+ *              + theta contraction of Eq. 30.  HEALPix: ring FFTs with phase shift and periodic extension
  *              (PAPER.md:403-407), weights 4 pi/Npix, Eq. 30.
  * s2_inverse : flm -> map f.  Fused recursion + l contraction of Eq. 33, then ring synthesis Eq. 32 (HEALPix:
  *              aliasing fold of F_m onto m mod nphi).
@@ -91,7 +92,7 @@ sht_status so3_inverse_plan(sht_plan* plan, const void* flmn, void* f, sht_strea
  * for sampled parity at sizes where the full map is too large for the oracle:
  *   s2_theta_inverse_plan: flm -> Fm[2L-1][ntheta] (row m+L-1; ntheta = sht_plan_ntheta(plan, 0)); Eq. 33.
  *   s2_theta_forward_plan: Wm[2L-1][ntheta_q] (row m+L-1; already weighted; ntheta_q = sht_plan_ntheta(plan, 1),
- *                          2L on MW) -> flm; Eq. 30.
+ *                          2L on MW: the rings theta'_u = (2u+1) pi/(4L)) -> flm; Eq. 30.
  */
 int        sht_plan_ntheta(const sht_plan* plan, int forward);
 sht_status s2_theta_inverse_plan(sht_plan* plan, const void* flm, void* Fm, sht_stream stream);

@@ -101,7 +101,7 @@ struct sht_plan {
     double* unit_wq = nullptr; // [fwd.ntp] ones (theta-stage entry point takes already weighted rows)
     size_t F_slab = 0, Fa_slab = 0, X_slab = 0, Z_slab = 0, H_slab = 0;
     int Ltp = 0;               // padded ring count of Fa rows
-    int fwd_ld = 0;            // row length of the forward ring-sample array U (MW: 4L-1, HEALPix: padded ring count)
+    int fwd_ld = 0;            // row length of the forward ring-sample array U (MW: 4L, HEALPix: padded ring count)
     // HEALPix ring-FFT staging (healpix.cu): Bluestein batch C[2(nside-1)][M], chirp spectra BF[nside-1][M], belt rows E
     int hp_M = 0, hp_ncap = 0, hp_neq = 0; long long hp_off_eq = 0;
     double2 *hp_C = nullptr, *hp_BF = nullptr, *hp_E = nullptr;
@@ -129,6 +129,20 @@ void rings_mw(RingSet& R, int Lt) {      // Eq. 37: theta_t = (2t
         R.ct[t] = cosl(th); R.c2[t] = cosl(th / 2); R.s2[t] = sinl(th / 2);
     }
     R.ntp = (int)rup((size_t)R.nth + 1, 128);
+}
+
+// Forward quadrature rings of the MW transform (R9): theta'_u = (2u+1)pi/(4L), u = 0..2L-1 -- the midpoints of
+// 4L equispaced samples of the theta circle.  The paper upsamples F_m(theta) to "2L" rings; any ring set
+// on which the quadrature of the band-limit-(2L-2) integrand is exact gives the same result, and this one has a
+// power-of-two FFT length 4L (the MW(2L) set needs 4L-1, often prime) and no pole ring.
+void rings_mid(RingSet& R, int L) {
+    R.nth = 2 * L; R.pole = false;
+    R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
+    for (int u = 0; u < R.nth; ++u) {
+        ld th = PI_L * (ld)(2 * u + 1) / (ld)(4 * L);
+        R.ct[u] = cosl(th); R.c2[u] = cosl(th / 2); R.s2[u] = sinl(th / 2);
+    }
+    R.ntp = (int)rup((size_t)R.nth, 128);
 }
 
 // HEALPix rings r = 1..4 nside-1 (public ring scheme, R11); half-angle trigonometry from z
@@ -220,7 +234,7 @@ void layout(sht_plan* P, char* base) {
     P->unit_wq = B.take<double>(P->fwd.ntp);
     P->Ltp = P->inv.ntp;
     if (P->sampling == SHT_MW) {
-        P->fwd_ld = 4 * L - 1;
+        P->fwd_ld = 4 * L;
         P->Fa_slab = (size_t)NB * P->Ltp;
         P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
         P->X_slab = (size_t)NB * NB;
@@ -298,10 +312,10 @@ sht_status make_fft_plans(sht_plan* P) {
     CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
     { int inembed[1] = {NB};
       CF(cufftMakePlanMany(P->fft_th1, 1, n1, inembed, 1, NB, inembed, 1, NB, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
-    int n2[1] = {4 * L - 1};
+    int n2[1] = {4 * L};
     CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
-    { int inembed[1] = {4 * L - 1};
-      CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L - 1, inembed, 1, 4 * L - 1, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
+    { int inembed[1] = {4 * L};
+      CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L, inembed, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
     if (P->kind == 1) {
         int n3[1] = {2 * P->N - 1};
         CF(cufftCreate(&P->fft_gamma)); CF(cufftSetAutoAllocation(P->fft_gamma, 0));
@@ -566,9 +580,9 @@ sht_status check_ready(const sht_plan* P) {
     return SHT_OK;
 }
 
-// MW: F_m(theta_t) on L rings (Fa, [bin][Ltp]) -> U[bin][4L-1] on the MW(2L) rings (in Z)
+// MW: F_m(theta_t) on L rings (Fa, [bin][Ltp]) -> U[bin][4L] on the rings theta'_u = (2u+1)pi/(4L) (in Z; u < 2L used)
 sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
-    const int L = P->L, NB = P->NB, T2 = 4 * L - 1;
+    const int L = P->L, NB = P->NB, T2 = 4 * L;
     stage(P, CAT_STAGE, st);
     for (int s = 0; s < P->nslab; ++s) CK(st_mw_extend(L, P->slab_n[s], P->Ltp, NB, P->Fa + P->Fa_slab * s, P->X + P->X_slab * s, st));
     stage(P, CAT_FFT, st);
@@ -662,7 +676,7 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
     sht_plan* P = new sht_plan();
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
-    if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L); }
+    if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, L); }
     else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
     sht_status s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
@@ -678,7 +692,7 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     P->kind = 1; P->L = L; P->N = N; P->sampling = SHT_MW;
     P->nslab = 2 * N - 1;
     for (int b = 0; b < P->nslab; ++b) P->slab_n.push_back(b < N ? b : b - (2 * N - 1));   // gamma-FFT bin order
-    rings_mw(P->inv, L); rings_mw(P->fwd, 2 * L);
+    rings_mw(P->inv, L); rings_mid(P->fwd, L);
     sht_status s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
@@ -718,8 +732,8 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     CS(fill_ringset(P, P->inv, st)); CS(fill_ringset(P, P->fwd, st));
     CK(cudaMemsetAsync(P->fwd.wq, 0, sizeof(double) * P->fwd.ntp, st));
     if (P->sampling == SHT_MW) {
-        // forward quadrature weights on MW(2L): q_u = (2 pi/(2L-1)) v_u   (Eq. 41-44 at band-limit 2L)
-        CK(st_mw_weights(2 * L, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
+        // forward quadrature weights q_u = (2 pi/(2L-1)) v_u on the 2L midpoint rings (Eq. 41-44 restated for that ring set)
+        CK(st_mid_weights(L, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
     } else {
         // HEALPix: equal pixel weights 4 pi / Npix
         std::vector<double> w(P->fwd.ntp, 0.0);
@@ -853,7 +867,7 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     for (int b = 0; b < P->batch; ++b)                                                 // Eq. 31 (weight folded into q_u)
         CF(cufftExecZ2Z(P->fft_phi_fwd, const_cast<double2*>(fin) + (size_t)L * NB * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD));
     CS(mw_upsample(P, st));
-    CS(run_theta_forward(P, P->Z, P->Z_slab, 4 * L - 1, st));
+    CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
     stage(P, CAT_STAGE, st);
     for (int b = 0; b < P->batch; ++b)
         CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + (size_t)L * NB * b, st));
@@ -895,7 +909,7 @@ sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream s
     CF(cufftSetStream(P->fft_phi_fwd, st));
     for (int b = 0; b < P->nslab; ++b) CF(cufftExecZ2Z(P->fft_phi_fwd, P->fn + slab * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD));
     CS(mw_upsample(P, st));
-    CS(run_theta_forward(P, P->Z, P->Z_slab, 4 * L - 1, st));
+    CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
     stage(P, CAT_STAGE, st);
     for (int b = 0; b < P->nslab; ++b)
         CK(st_finalize_forward(L, P->Lp, P->slab_n[b], 0, P->scale_fwd, P->H + P->H_slab * b, (double2*)flmn + slab * (P->slab_n[b] + N - 1), st));

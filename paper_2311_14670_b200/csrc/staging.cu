@@ -117,6 +117,23 @@ __global__ void k_lamtab(int n, int nth, int ntp, int m_end, const double* __res
     lam[(size_t)(m - m_end) * ntp + th] = v;
 }
 
+// Theta-quadrature weights of the MW forward transform on the midpoint rings theta'_u = (2u+1)pi/N, N = 4L, u < 2L.
+// The integrand G(theta) = F_m(theta) d^l_{m,-s}(theta) is a trigonometric polynomial of degree <= 2L-2, even about 0, so
+//   int_0^pi G sin = (1/2) int_0^2pi G |sin| = pi sum_k G^_k c_k,  |sin| = sum_k c_k e^{ik theta}, c_k = (2/pi)/(1-k^2) (k even),
+// which is Eq. 41-44 with the reflection sign +1 (R9); G^_k from N samples is exact (N > 4L-4).
+// Folding theta <-> 2pi - theta:  v_u = (1/N) (4 + 8 sum_{j=1}^{L-1} cos(2j theta'_u)/(1-4j^2)).   Output: v_u * qphi.
+__global__ void k_mid_weights(int L, double qphi, double* __restrict__ w) {
+    int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= 2 * L) return;
+    const long N = 4L * L;
+    double acc = 0.0;
+    for (int j = L - 1; j >= 1; --j) {              // small terms first
+        long r = ((long)2 * j * (2 * u + 1)) % (2 * N);
+        acc += 1.0 / (1.0 - 4.0 * (double)j * (double)j) * cospi((double)r / (double)N);
+    }
+    w[u] = (4.0 + 8.0 * acc) / (double)N * qphi;
+}
+
 // MW theta-quadrature weights at band-limit Lq (closed form of Eq. 41-44 with reflection sign +1, R9):
 //   v_u = (zeta_u/(2Lq-1)) sum_{|2j|<=Lq-1} 4 cos(2j theta_u)/(1-4j^2),  theta_u = (2u+1)pi/(2Lq-1);  times qphi.
 __global__ void k_mw_weights(int Lq, double qphi, double* __restrict__ w) {
@@ -219,7 +236,7 @@ __global__ void k_mw_extend(int L, int n, int ldin, int ldout, const double2* __
 // MW forward (iii)->(iv): F_{mm'} = (1/T) e^{-i m' pi/T} Y[m' mod T]; Z[m' mod T2] = F_{mm'} e^{+i m' pi/T2}; zero elsewhere.
 __global__ void k_mw_pad_phase(int L, int ldin, int ldout, const double2* __restrict__ Y, double2* __restrict__ Z) {
     int k2 = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
-    const int T = 2 * L - 1, T2 = 4 * L - 1;
+    const int T = 2 * L - 1, T2 = ldout;
     if (k2 >= T2) return;
     int mp = k2 < L ? k2 : (k2 > T2 - L ? k2 - T2 : T2);      // |m'| <= L-1, else none
     double2 v = {0.0, 0.0};
@@ -434,6 +451,10 @@ cudaError_t st_rsq(int n, double* rsq, cudaStream_t st) {
     k_rsq<<<cdiv(n, 256), 256, 0, st>>>(n, rsq);
     LAUNCHED(); return cudaSuccess;
 }
+cudaError_t st_mid_weights(int L, double qphi, double* w, cudaStream_t st) {
+    k_mid_weights<<<cdiv(2 * L, 128), 128, 0, st>>>(L, qphi, w);
+    LAUNCHED(); return cudaSuccess;
+}
 cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st) {
     k_mw_weights<<<cdiv(Lq, 128), 128, 0, st>>>(Lq, qphi, w);
     LAUNCHED(); return cudaSuccess;
@@ -481,7 +502,7 @@ cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, d
     LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st) {
-    dim3 grid(cdiv(4 * L - 1, 128), 2 * L - 1);
+    dim3 grid(cdiv(ldout, 128), 2 * L - 1);
     k_mw_pad_phase<<<grid, 128, 0, st>>>(L, ldin, ldout, Y, Z);
     LAUNCHED(); return cudaSuccess;
 }

@@ -7,6 +7,7 @@ cudaError_t st_start_values(int L, int n, int nth, int ntp, const double* c2hi, 
 cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t st);
 cudaError_t st_rsq(int n, double* rsq, cudaStream_t st);
 cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st);
+cudaError_t st_mid_weights(int L, double qphi, double* w, cudaStream_t st);
 cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* coef, const double* scale,
                             const double* C, const double2* SG, int sgstride, double* G, cudaStream_t st);
 cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* kexp, const double* rsq, double* C, cudaStream_t st);

@@ -1,7 +1,7 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times, on SAMPLED outputs the oracle
 can compute one by one (a few rings of the inverse, a few harmonic orders m of the forward), plus properties that hold
-at any size (exact MW round trip, zero pattern).  Forward inputs are white-noise maps from synth (the forward transform
-is defined by the algorithm for any input), never something the CUDA path produced."""
+at any size (exact MW round trip, zero pattern).  Forward inputs are white-noise maps from synth (not band-limited; only
+the theta = pi ring is that of a function, R21), never something the CUDA path produced."""
 import numpy as np
 import pytest
 
@@ -43,7 +43,7 @@ def test_config2_mw_L1024_spin2(api, orc):
     # sampling theorem (DESIGN.md pin 6): the round trip reproduces the generating coefficients
     assert rel(back, flm) < TOL
     # forward of a white-noise map against the oracle on sampled orders m
-    g = synth.random_map((L, 2 * L - 1), seed=11)
+    g = synth.random_map((L, 2 * L - 1), seed=11, mw_pole_spin=spin)
     got = P.forward(dev(g)).cpu().numpy()
     ms = np.array([-(L - 1), -700, -2, -1, 0, 1, 2, 3, 511, L - 1])
     want = orc.s2_forward_columns(L, spin, orc.MW, g, ms)
@@ -86,4 +86,5 @@ def test_config4_so3_L256_N8(api, orc):
     back = P.forward(dev(f_ref)).cpu().numpy()
     assert rel(back, c) < TOL
     g = synth.random_map((2 * N - 1, L, 2 * L - 1), seed=13)
+    g[:, L - 1, :] = f_ref[:, L - 1, :]      # a function on SO(3) has one value per (alpha - gamma) at beta = pi (R21)
     assert rel(P.forward(dev(g)).cpu().numpy(), orc.so3_forward(L, N, g)) < TOL

@@ -67,10 +67,10 @@ def test_config1_L64_spin0_round_trip_and_forward(api, orc):
 
 
 def test_forward_of_non_bandlimited_map_matches_oracle(api, orc):
-    """The forward transform is defined by the algorithm (upsampling + quadrature) for any input, not just
-    band-limited maps: check parity on white noise."""
+    """The forward transform is defined by the algorithm (upsampling + quadrature) for any sampled function, not just
+    band-limited ones: check parity on white noise (single-valued at the pole ring, R21)."""
     L, spin = 40, 1
-    f = synth.random_map((L, 2 * L - 1), seed=9)
+    f = synth.random_map((L, 2 * L - 1), seed=9, mw_pole_spin=spin)
     P = api.Plan(L, spin)
     assert rel(P.forward(dev(f)).cpu().numpy(), orc.s2_forward(L, spin, orc.MW, f)) < TOL
 
@@ -83,25 +83,21 @@ def test_theta_stage_entry_points(api, orc):
     F = P.theta_inverse(dev(flm)).cpu().numpy()
     ms = np.arange(-(L - 1), L)
     assert rel(F, orc.s2_theta_inverse_columns(L, spin, orc.MW, flm, ms)) < TOL
-    # forward theta step on the oracle's own upsampled + weighted rows would need oracle internals; instead use
-    # linearity: rows W = q_u * F_m(theta'_u) synthesised by the oracle's theta step on the MW(2L) rings is not
-    # exposed, so check adjoint consistency <theta_fwd(W), a> = <W, theta_inv-like(a)> via random probes:
+    # forward theta step (Eq. 30) on arbitrary weighted rows W[m][u], u indexing the library's quadrature rings
+    # theta'_u = (2u+1) pi / (4L) (include/b200sht.h), against a direct sum with the oracle's d-functions
     nq = P.ntheta(True)
+    assert nq == 2 * L
     rng = np.random.default_rng(0)
     W = (rng.standard_normal((2 * L - 1, nq)) + 1j * rng.standard_normal((2 * L - 1, nq)))
     out = P.theta_forward(dev(W)).cpu().numpy()
-    # reference by the oracle's d-functions: out[l, m] = pref(l) * sum_u W[m, u] d^l_{m,-s}(theta'_u)
-    tab = orc.ring_table(orc.MW_QUAD, L)
+    # out[l, m] = pref(l) * sum_u W[m, u] d^l_{m,-s}(theta'_u)
     el = np.arange(L)
     pref = (-1.0) ** spin * np.sqrt((2 * el + 1) / (4 * np.pi))
+    half = np.pi * (2 * np.arange(nq) + 1) / (8 * L)
     for m in (-(L - 1), -5, 0, 2, 31, L - 1):
         acc = np.zeros(L, complex)
         for u in range(nq):
-            if u == nq - 1:
-                d = np.array([(-1.0) ** (l + m) if m == spin and l >= abs(spin) else 0.0 for l in range(L)])
-            else:
-                c2 = np.sqrt((1 + tab["cos_theta"][u]) / 2); s2 = np.sqrt((1 - tab["cos_theta"][u]) / 2)
-                d = np.asarray(orc.d_lrec(L, m, -spin, cos_half=c2, sin_half=s2), float)
+            d = np.asarray(orc.d_lrec(L, m, -spin, cos_half=np.cos(half[u]), sin_half=np.sin(half[u])), float)
             acc += W[m + L - 1, u] * d
         want = pref * acc
         want[el < max(abs(m), abs(spin))] = 0
