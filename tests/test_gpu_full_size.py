@@ -88,3 +88,33 @@ def test_config4_so3_L256_N8(api, orc):
     g = synth.random_map((2 * N - 1, L, 2 * L - 1), seed=13)
     g[:, L - 1, :] = f_ref[:, L - 1, :]      # a function on SO(3) has one value per (alpha - gamma) at beta = pi (R21)
     assert rel(P.forward(dev(g)).cpu().numpy(), orc.so3_forward(L, N, g)) < TOL
+
+
+def test_config5a_mw_L8192_spin0(api, orc):
+    """configs[4], first half: spin-0 complex SHT, MW L = 8192 (8192 x 16383 map, 2.1 GB), sigma_l = 1/(l+1), seed 4, fp64.
+    The oracle cannot synthesise the full map: inverse parity on sampled rings, forward parity of a white-noise map on
+    sampled orders m, and the sampling-theorem round trip against the generating coefficients (a property at any size).
+    north_star states 1e-11 up to L = 1024 and asks for the growth with L: the bound used here is 1e-11 * L/1024."""
+    L, spin = 8192, 0
+    tol = TOL * L / 1024
+    flm = synth.random_flm(L, spin, seed=4, sigma=synth.SIGMA_RED)
+    P = api.Plan(L, spin)
+    d = dev(flm)
+    f = P.inverse(d)
+    rings = np.array([0, 1, 4097, 8190, 8191])
+    rows = orc.s2_inverse_rings(L, spin, orc.MW, flm, rings)
+    scale = max(np.abs(r).max() for r in rows)
+    for r, row in zip(rings, rows):
+        assert rel(f[int(r)].cpu().numpy(), row, scale) < tol, r
+    back = P.forward(f)
+    err = float((back - d).abs().max() / d.abs().max())
+    print(f"L=8192 round trip max rel err {err:.3e}")
+    assert err < tol
+    del f, back, d
+    g = synth.random_map((L, 2 * L - 1), seed=14, mw_pole_spin=spin)
+    got = P.forward(dev(g)).cpu().numpy()
+    ms = np.array([-(L - 1), -1, 0, 1, 4096, L - 1])
+    want = orc.s2_forward_columns(L, spin, orc.MW, g, ms)
+    sc = np.abs(want).max()
+    for m, col in zip(ms, want):
+        assert rel(got[:, m + L - 1], col, sc) < tol, m
