@@ -140,6 +140,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--L", type=int, default=None, help="profiling only: override the band-limit of the workload")
     ap.add_argument("--spin", type=int, default=None, help="profiling only: override the spin of the workload")
+    ap.add_argument("--batch", type=int, default=1, help="profiling only: transform a batch of maps together (configs[4]: --L 2048 --spin 0 --batch 16)")
     args = ap.parse_args()
     if args.L is not None:
         WORKLOAD["L"] = args.L
@@ -162,12 +163,15 @@ def main():
     torch.cuda.set_device(local_rank)
     dev = torch.device(f"cuda:{local_rank}")
 
-    L, spin = WORKLOAD["L"], WORKLOAD["spin"]
+    L, spin, B = WORKLOAD["L"], WORKLOAD["spin"], args.batch
     # weak scaling: every rank transforms its own seeded field (independent problems, no data-path collective)
-    flm_h = synth.random_flm(L, spin, seed=WORKLOAD["seed"] + rank, sigma=synth.SIGMA_CMB)
+    if B == 1:
+        flm_h = synth.random_flm(L, spin, seed=WORKLOAD["seed"] + rank, sigma=synth.SIGMA_CMB)
+    else:
+        flm_h = np.stack([synth.random_flm(L, spin, seed=4 + i + 1000 * rank, sigma=synth.SIGMA_RED) for i in range(B)])
     flm = torch.from_numpy(flm_h).to(dev)
-    plan = api.Plan(L, spin, device=dev)
-    f = torch.empty((L, 2 * L - 1), dtype=torch.complex128, device=dev)
+    plan = api.Plan(L, spin, device=dev, batch=B)
+    f = torch.empty(plan.map_shape, dtype=torch.complex128, device=dev)
     back = torch.empty_like(flm)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
@@ -200,7 +204,7 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
     ms_per_step = total_ms / args.steps
-    value = world * args.steps / (total_ms * 1e-3)
+    value = world * B * args.steps / (total_ms * 1e-3)
     err = float((back - flm).abs().max() / flm.abs().max())
 
     # per-stage device times (CUDA events recorded inside the library on the launching stream)
@@ -219,10 +223,12 @@ def main():
         pk, pk_kind = peaks()
         fp64_tf, _ = api.fp64_peak(20000)
         fl = FLOP_PER_DSTEP[spin == 0]
+        if B > 1:                # shared recursion (6 flop) + 4 flop per order served per map
+            fl = 6.0 + (8.0 if spin == 0 else 4.0) * B
         flops_fwd = plan.dsteps(True) * fl
         flops_inv = plan.dsteps(False) * fl
         ach = flops_fwd / (stages["forward_ms"]["hot"] * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": "theta_forward_kernel (fused m-recursion + theta contraction, Eq. 25+30)",
+        roof = {"bound": "alu", "kernel": ("theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>") + " (fused m-recursion + theta contraction, Eq. 25+30)",
                 "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf, "traffic": None,
                 "peak_kind": "measured in this run by a register-only DFMA chain (sht_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
@@ -230,30 +236,40 @@ def main():
                                    "frac": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12 / fp64_tf},
                 "hbm_peak_gbs": pk.get("hbm_gbs"), "hbm_peak_kind": pk_kind}
         # end to end through host buffers (pinned), H2D + D2H inside the timed region
-        fh = torch.empty((L, 2 * L - 1), dtype=torch.complex128).pin_memory().numpy()
-        ch = torch.from_numpy(flm_h).pin_memory().numpy()
-        bh = torch.empty((L, 2 * L - 1), dtype=torch.complex128).pin_memory().numpy()
+        fh = torch.empty(plan.map_shape, dtype=torch.complex128).pin_memory()
+        ch = torch.from_numpy(flm_h).pin_memory()
+        bh = torch.empty(plan.coef_shape, dtype=torch.complex128).pin_memory()
+
+        def pair_host():
+            if B == 1:          # the C-ABI host-buffer calls copy in and out themselves
+                api.s2_inverse_host(ch.numpy(), L, spin, out=fh.numpy()); api.s2_forward_host(fh.numpy(), L, spin, out=bh.numpy())
+            else:               # batched plans take device pointers: pinned copies around them, same bytes
+                flm.copy_(ch, non_blocking=True); plan.inverse(flm, out=f); fh.copy_(f, non_blocking=True)
+                f.copy_(fh, non_blocking=True); plan.forward(f, out=back); bh.copy_(back, non_blocking=True)
+                torch.cuda.synchronize()
         for _ in range(2):
-            api.s2_inverse_host(ch, L, spin, out=fh); api.s2_forward_host(fh, L, spin, out=bh)
+            pair_host()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         ne = max(3, min(args.steps, 10))
         for _ in range(ne):
-            api.s2_inverse_host(ch, L, spin, out=fh); api.s2_forward_host(fh, L, spin, out=bh)
+            pair_host()
         torch.cuda.synchronize()
         te = (time.perf_counter() - t0) / ne
-        nbytes = L * (2 * L - 1) * 16
-        e2e = {"value": world / te, "unit": UNIT, "h2d_bytes_per_step": 2 * nbytes, "d2h_bytes_per_step": 2 * nbytes,
+        fh, ch, bh = fh.numpy(), ch.numpy(), bh.numpy()
+        nbytes = B * L * (2 * L - 1) * 16
+        e2e = {"value": world * B / te, "unit": UNIT, "h2d_bytes_per_step": 2 * nbytes, "d2h_bytes_per_step": 2 * nbytes,
                "ms_per_step": te * 1e3, "roundtrip_err": float(np.abs(bh - flm_h).max() / np.abs(flm_h).max())}
         cpu = None
         if not args.no_cpu:
-            t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm_h)
+            t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm_h if B == 1 else flm_h[0])
             cpu = {"value": 1.0 / (t_inv + t_fwd), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                    "inverse_s": t_inv, "forward_s": t_fwd}
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                "data": "synthetic",
-               "config": {"workload": f"{'BASELINE.json configs[1]' if (L, spin) == (1024, 2) else 'override'}: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
+               "config": {"workload": f"{'BASELINE.json configs[1]' if (L, spin, B) == (1024, 2, 1) else 'override'}: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
+                                      + (f"batch of {B} maps transformed together, " if B > 1 else "") +
                                       "flm ~ N(0, 1/(l(l+1))) l>=2, inverse + forward per step",
                           "l2": "flushed between timed iterations (256 MiB memset, untimed)", "parallelism": f"independent x{world}"},
                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
@@ -270,7 +286,7 @@ def main():
 def sweep(api, synth, torch, dev, flush, fp64_tf):
     """ms (hot / fft / staging) and fraction of FP64 peak vs L for MW spin 0, plus the SO(3) config."""
     rows = []
-    for L in (64, 256, 512, 1024, 2048, 4096):
+    for L in (64, 256, 512, 1024, 2048, 4096, 8192):
         flm = torch.from_numpy(synth.random_flm(L, 0, seed=4, sigma=synth.SIGMA_RED)).to(dev)
         P = api.Plan(L, 0, device=dev)
         P.enable_timing(True)
@@ -285,7 +301,29 @@ def sweep(api, synth, torch, dev, flush, fp64_tf):
                      "inverse_frac_fp64": P.dsteps(False) * 14 / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
                      "forward_frac_fp64": P.dsteps(True) * 14 / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
                      "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
-        del P
+        del P, f, b, flm
+        torch.cuda.empty_cache()
+    # BASELINE.json configs[4], second half: 16 maps at L = 2048 transformed together (shared recursion, DMMA contraction)
+    L, B = 2048, 16
+    import numpy as _np
+    flm = torch.from_numpy(_np.stack([synth.random_flm(L, 0, seed=4 + i, sigma=synth.SIGMA_RED) for i in range(B)])).to(dev)
+    P = api.Plan(L, 0, device=dev, batch=B)
+    P.enable_timing(True)
+    f = P.inverse(flm); b = P.forward(f)
+    ti, tf = [], []
+    for _ in range(3):
+        flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
+        flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
+    mi = {k: min(t[k] for t in ti) for k in ti[0]}
+    mf = {k: min(t[k] for t in tf) for k in tf[0]}
+    fl = 6.0 + 8.0 * B            # per d-step: recursion 6 flop + 2 orders x 4 flop per map
+    rows.append({"config": f"MW spin-0 L={L}, batch of {B} maps (theta_mma_kernel, FP64 DMMA)", "inverse_ms": mi, "forward_ms": mf,
+                 "inverse_frac_fp64": P.dsteps(False) * fl / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
+                 "forward_frac_fp64": P.dsteps(True) * fl / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
+                 "ms_per_map": {"inverse": mi["total"] / B, "forward": mf["total"] / B},
+                 "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
+    del P, f, b, flm
+    torch.cuda.empty_cache()
     L, N = 256, 8
     c = torch.from_numpy(synth.random_flmn(L, N, seed=3)).to(dev)
     P = api.Plan(L, N=N, device=dev)
