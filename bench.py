@@ -28,7 +28,9 @@ WORKLOAD = dict(L=1024, spin=2, seed=1)
 METRIC = "SHT fwd+inv transform pairs per second (MW L=1024 spin-2 fp64, 1 B200)"
 UNIT = "transform_pairs/s"
 # algorithmic flop per d-step: recursion 6 + projection 4 per order served
-FLOP_PER_DSTEP = {True: 14.0, False: 10.0}     # key: spin == 0 (complex, +-m from one step)
+# dram__bytes_read.sum + dram__bytes_write.sum of the forward theta kernel, per launch, from the ncu --set full captures in
+# profiles/r1_v6_theta_kernels.md; key (L, spin, batch).  Not measurable inside this process: null for other workloads.
+NCU_TRAFFIC_BYTES = {(1024, 2, 1): 164.536e6 + 14.288e6, (2048, 0, 1): 1.588936e9 + 82.18e6, (2048, 0, 16): 51.356830e9 + 13.395911e9}
 
 
 def peaks():
@@ -222,14 +224,14 @@ def main():
     if rank == 0:
         pk, pk_kind = peaks()
         fp64_tf, _ = api.fp64_peak(20000)
-        fl = FLOP_PER_DSTEP[spin == 0]
-        if B > 1:                # shared recursion (6 flop) + 4 flop per order served per map
-            fl = 6.0 + (8.0 if spin == 0 else 4.0) * B
-        flops_fwd = plan.dsteps(True) * fl
-        flops_inv = plan.dsteps(False) * fl
+        # algorithmic flop: per d-step 6 (recursion) + 4 per order and map served
+        flops_fwd = plan.flops(True)
+        flops_inv = plan.flops(False)
+        fl = flops_fwd / plan.dsteps(True)
         ach = flops_fwd / (stages["forward_ms"]["hot"] * 1e-3) / 1e12
         roof = {"bound": "alu", "kernel": ("theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>") + " (fused m-recursion + theta contraction, Eq. 25+30)",
-                "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf, "traffic": None,
+                "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf, "traffic": NCU_TRAFFIC_BYTES.get((L, spin, B)),
+                "traffic_source": "profiles/r1_v6_theta_kernels.md (ncu --set full, bytes per launch)",
                 "peak_kind": "measured in this run by a register-only DFMA chain (sht_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
                 "inverse_kernel": {"achieved": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12,
@@ -298,8 +300,8 @@ def sweep(api, synth, torch, dev, flush, fp64_tf):
         mi = {k: min(t[k] for t in ti) for k in ti[0]}
         mf = {k: min(t[k] for t in tf) for k in tf[0]}
         rows.append({"config": f"MW spin-0 L={L}", "inverse_ms": mi, "forward_ms": mf,
-                     "inverse_frac_fp64": P.dsteps(False) * 14 / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
-                     "forward_frac_fp64": P.dsteps(True) * 14 / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
+                     "inverse_frac_fp64": P.flops(False) / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
+                     "forward_frac_fp64": P.flops(True) / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
                      "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
         del P, f, b, flm
         torch.cuda.empty_cache()
@@ -316,10 +318,9 @@ def sweep(api, synth, torch, dev, flush, fp64_tf):
         flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
     mi = {k: min(t[k] for t in ti) for k in ti[0]}
     mf = {k: min(t[k] for t in tf) for k in tf[0]}
-    fl = 6.0 + 8.0 * B            # per d-step: recursion 6 flop + 2 orders x 4 flop per map
     rows.append({"config": f"MW spin-0 L={L}, batch of {B} maps (theta_mma_kernel, FP64 DMMA)", "inverse_ms": mi, "forward_ms": mf,
-                 "inverse_frac_fp64": P.dsteps(False) * fl / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
-                 "forward_frac_fp64": P.dsteps(True) * fl / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
+                 "inverse_frac_fp64": P.flops(False) / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
+                 "forward_frac_fp64": P.flops(True) / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
                  "ms_per_map": {"inverse": mi["total"] / B, "forward": mf["total"] / B},
                  "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
     del P, f, b, flm

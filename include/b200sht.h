@@ -135,6 +135,9 @@ sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream
 long       sht_launch_count(int reset);
 /* number of d-steps (one Eq. 25 evaluation for one (l, theta, pass)) one transform of this plan performs */
 double     sht_plan_dsteps(const sht_plan* plan, int forward);
+/* algorithmic flop of the hot kernels of one transform of this plan: per d-step 6 (Eq. 25 as the paper states it:
+ * 1 FMA + 2 MUL + 1 FMA) + 4 per (harmonic order, map) served (Eq. 30 / 33: complex x real multiply-add) */
+double     sht_plan_flops(const sht_plan* plan, int forward);
 const char* sht_version(void);
 
 #ifdef __cplusplus

@@ -42,6 +42,7 @@ SIGNATURES = {
     "sht_fp64_peak": (_i, [_i, C.POINTER(C.c_double), C.POINTER(C.c_float), _vp]),
     "sht_launch_count": (C.c_long, [_i]),
     "sht_plan_dsteps": (C.c_double, [_vp, _i]),
+    "sht_plan_flops": (C.c_double, [_vp, _i]),
     "sht_version": (C.c_char_p, []),
 }
 

@@ -104,6 +104,10 @@ class Plan:
     def dsteps(self, forward):
         return float(lib().sht_plan_dsteps(self._h, int(forward)))
 
+    def flops(self, forward):
+        """Algorithmic flop of the hot kernels of one transform (6 per d-step + 4 per order and map served)."""
+        return float(lib().sht_plan_flops(self._h, int(forward)))
+
 
 # -- the north-star calls (library-side plan cache; device tensors) --
 def s2_forward(f, L, spin=0, sampling=MW, reality=False):

@@ -55,6 +55,7 @@ inline size_t rup(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct RingSet {
     int nth = 0, ntp = 0;      // regular rings, padded count (multiple of 128; > nth so a pole ring fits)
     bool pole = false;         // a theta = pi ring at index nth (MW, Eq. 29)
+    bool symmetric = false;    // ring nth-1-t is the mirror image pi - theta_t of ring t
     std::vector<ld> ct, c2, s2;  // host: cos(theta), cos(theta/2), sin(theta/2) of the regular rings
     double *csc = nullptr, *tau = nullptr, *sig = nullptr, *c2hi = nullptr, *c2lo = nullptr, *s2hi = nullptr, *s2lo = nullptr;
     double* wq = nullptr;      // [ntp] forward quadrature weight per ring (incl. the pole ring at index nth)
@@ -78,7 +79,7 @@ struct sht_plan {
     int Lp = 0, NB = 0;        // padded L; 2L-1
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
     int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
-    int ncg = 0;               // batched path: column groups of 16 complex columns
+    int ncg = 0, ncg_fwd = 0;  // batched path: column groups of 16 complex columns (inverse / forward passes)
     double* Ob = nullptr;      // batched path: result scratch of all passes
     std::vector<size_t> ob_off_inv, ob_off_fwd;   // per-pass offsets (doubles) into Ob
     std::vector<int> slab_n;   // second index n of d^l_{m,n} per slab
@@ -115,7 +116,7 @@ struct sht_plan {
     // timing
     bool timing = false;
     std::vector<cudaEvent_t> ev; std::vector<int> ev_cat; int ev_n = 0;
-    double dsteps_inv = 0, dsteps_fwd = 0;
+    double dsteps_inv = 0, dsteps_fwd = 0, flops_inv = 0, flops_fwd = 0;
 };
 
 namespace {
@@ -136,7 +137,7 @@ void rings_mw(RingSet& R, int Lt) {      // Eq. 37: theta_t = (2t
 // on which the quadrature of the band-limit-(2L-2) integrand is exact gives the same result, and this one has a
 // power-of-two FFT length 4L (the MW(2L) set needs 4L-1, often prime) and no pole ring.
 void rings_mid(RingSet& R, int L) {
-    R.nth = 2 * L; R.pole = false;
+    R.nth = 2 * L; R.pole = false; R.symmetric = true;
     R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
     for (int u = 0; u < R.nth; ++u) {
         ld th = PI_L * (ld)(2 * u + 1) / (ld)(4 * L);
@@ -147,7 +148,7 @@ void rings_mid(RingSet& R, int L) {
 
 // HEALPix rings r = 1..4 nside-1 (public ring scheme, R11); half-angle trigonometry from z
 void rings_healpix(RingSet& R, int nside) {
-    R.nth = 4 * nside - 1; R.pole = false;
+    R.nth = 4 * nside - 1; R.pole = false; R.symmetric = true;
     R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
     const ld ns = (ld)nside;
     for (int i = 0; i < R.nth; ++i) {
@@ -173,7 +174,7 @@ struct Bump {
 // doubles of one pass's operand buffer (single-map kernels: rows m_end-1..L-1; batched: rows m_end..L-1 per column group)
 size_t pass_in_doubles(const sht_plan* P, const PassHost& ph, bool fwd) {
     const size_t K = fwd ? P->fwd.ntp : P->Lp;
-    if (P->batch > 1) return (size_t)P->ncg * (P->L - ph.p.m_end) * K * SHT_MMA_ROW;
+    if (P->batch > 1) return (size_t)(fwd ? P->ncg_fwd : P->ncg) * (P->L - ph.p.m_end) * K * SHT_MMA_ROW;
     const size_t rows = (size_t)(P->L - ph.p.m_end + 1);
     return fwd ? rows * K * (ph.mode == 0 ? 4 : 2) : rows * K * theta_inverse_rowd(ph.mode);
 }
@@ -223,7 +224,7 @@ void layout(sht_plan* P, char* base) {
         size_t oi = 0, of = 0;
         P->ob_off_inv.clear(); P->ob_off_fwd.clear();
         for (auto& ph : P->pinv) { P->ob_off_inv.push_back(oi); oi += (size_t)P->ncg * (L - ph.p.m_end) * P->inv.ntp * SHT_MMA_NCOL; }
-        for (auto& ph : P->pfwd) { P->ob_off_fwd.push_back(of); of += (size_t)P->ncg * (L - ph.p.m_end) * Lp * SHT_MMA_NCOL; }
+        for (auto& ph : P->pfwd) { P->ob_off_fwd.push_back(of); of += (size_t)P->ncg_fwd * (L - ph.p.m_end) * Lp * SHT_MMA_NCOL; }
         P->Ob = B.take<double>(oi > of ? oi : of);
     }
     // scratch arrays
@@ -277,8 +278,13 @@ void add_passes(sht_plan* P, int slab, int n, bool real) {
         int an = n < 0 ? -n : n;
         PassHost a = mk(n, +1, -an, 1, 2 * n), b = mk(-n, -1, 1 - an, 1, 2 * n + 1);
         P->pinv.push_back(a); P->pinv.push_back(b);
-        P->pfwd.push_back(a); P->pfwd.push_back(b);
-        for (RingSet* R : {&P->inv, &P->fwd}) { R->start[n]; R->start[-n]; R->mlo[2 * n]; R->mlo[2 * n + 1]; }
+        // forward: the quadrature rings are symmetric about the equator, so ONE pass serves order +m from its own ring and order
+        // -m from the mirrored ring (d^l_{-m,n}(pi - theta) = (-1)^{l-n} d^l_{m,n}(theta)): two orders per d-step
+        PassHost c = mk(n, +1, -an, 0, 2 * n);
+        c.p.fold = 1;
+        P->pfwd.push_back(c);
+        P->inv.start[n]; P->inv.start[-n]; P->inv.mlo[2 * n]; P->inv.mlo[2 * n + 1];
+        P->fwd.start[n]; P->fwd.mlo[2 * n];
     }
 }
 
@@ -340,16 +346,21 @@ sht_status plan_common(sht_plan* P) {
     if (P->batch > 1) {            // one pass list serves every map of the batch
         add_passes(P, 0, P->slab_n[0], P->reality != 0);
         P->ncg = (P->batch * (P->pinv[0].mode == 0 ? 2 : 1) + 15) / 16;
+        P->ncg_fwd = (P->batch * (P->pfwd[0].mode == 0 ? 2 : 1) + 15) / 16;
     } else
         for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
     // d-step counts: rings * sum over l of the steps each pass runs
     for (int dir = 0; dir < 2; ++dir) {
-        double tot = 0; const RingSet& R = dir ? P->fwd : P->inv;
+        // algorithmic flop per d-step: 6 (recursion, as the paper states it) + 4 per order served and map
+        double tot = 0, fl = 0; const RingSet& R = dir ? P->fwd : P->inv;
         for (auto& ph : (dir ? P->pfwd : P->pinv)) {
             int an = ph.p.n < 0 ? -ph.p.n : ph.p.n;
-            for (int l = an; l < L; ++l) tot += (double)(l - ph.p.m_end + 1);
+            double t = 0;
+            for (int l = an; l < L; ++l) t += (double)(l - ph.p.m_end + 1);
+            tot += t; fl += t * (6.0 + 4.0 * (ph.mode == 0 ? 2 : 1) * P->batch);
         }
         (dir ? P->dsteps_fwd : P->dsteps_inv) = tot * R.nth;
+        (dir ? P->flops_fwd : P->flops_inv) = fl * R.nth;
     }
     CS(make_fft_plans(P));
     layout(P, nullptr);
@@ -397,7 +408,11 @@ sht_status fill_ringset(sht_plan* P, RingSet& R, cudaStream_t st) {
         int key = kv.first, n = (key - (key & 1)) / 2, passB = key & 1;
         std::vector<int> h(R.ntp, 1 << 30);
         for (int t = 0; t < R.nth; ++t) {
-            int ms = (int)llroundl((ld)n * R.ct[t]);
+            // m_s(pi - theta) = -m_s(theta) exactly (the fold passes rely on it): evaluate on the northern ring of a mirror pair
+            const int tm = R.nth - 1 - t;
+            const bool mirrored = R.symmetric && tm < t;
+            int ms = (int)llroundl((ld)n * R.ct[mirrored ? tm : t]);
+            if (mirrored) ms = -ms;
             h[t] = passB ? 1 - ms : ms;
         }
         CK(cudaMemcpyAsync(kv.second, h.data(), sizeof(int) * R.ntp, cudaMemcpyHostToDevice, st));
@@ -450,7 +465,7 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
 MmaArgs mma_args(const sht_plan* P, bool fwd) {
     const RingSet& R = fwd ? P->fwd : P->inv;
     MmaArgs a{};
-    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.ncg = P->ncg;
+    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.ncg = fwd ? P->ncg_fwd : P->ncg;
     a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin;
     a.passes = fwd ? P->d_fwd_p : P->d_inv_p;
     a.npass = fwd ? P->n_fwd_p : P->n_inv_p;
@@ -488,7 +503,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
             auto& ph = P->pinv[i];
             const size_t rows = (size_t)(L - ph.p.m_end);
             CK(st_unpack_batch(L, P->Lp, P->inv.ntp, P->inv.nth, ph.mode == 0 ? 2 : 1, P->batch, P->ncg, ph.p.n, ph.p.sgn_out, ph.p.m_end,
-                               P->mmin, 0, P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->inv.ntp * SHT_MMA_NCOL, P->F,
+                               P->mmin, 0, 0, P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->inv.ntp * SHT_MMA_NCOL, P->F,
                                P->F_slab, P->inv.ntp, st));
         }
         if (P->inv.pole) {
@@ -531,10 +546,10 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         for (size_t i = 0; i < P->pfwd.size(); ++i) {
             auto& ph = P->pfwd[i];
             const size_t rows = (size_t)(L - ph.p.m_end);
-            CK(st_weight_split_batch(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg, P->slab_n[0],
-                                     ph.p.sgn_out, ph.p.m_end, ph.p.m_lo, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
+            CK(st_weight_split_batch(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, P->slab_n[0],
+                                     ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
                                      rows * P->fwd.ntp * SHT_MMA_ROW, st));
-            CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg * rows * P->Lp * SHT_MMA_NCOL, st));
+            CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
         }
         stage(P, CAT_HOT, st);
         for (size_t i = 0; i < P->pfwd.size(); ++i) {
@@ -548,7 +563,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         for (size_t i = 0; i < P->pfwd.size(); ++i) {
             auto& ph = P->pfwd[i];
             const size_t rows = (size_t)(L - ph.p.m_end);
-            CK(st_unpack_batch(L, P->Lp, P->Lp, L, ph.mode == 0 ? 2 : 1, P->batch, P->ncg, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, 1,
+            CK(st_unpack_batch(L, P->Lp, P->Lp, L, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, 1, ph.p.fold,
                                P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->Lp * SHT_MMA_NCOL, P->H, P->H_slab, P->Lp, st));
         }
         if (P->fwd.pole) {
@@ -559,7 +574,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     }
     for (auto& ph : P->pfwd) {
         int n_slab = P->slab_n[ph.p.slab];
-        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.m_lo,
+        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo,
                            P->fwd.wq, U + U_slab * ph.p.slab,
                            reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), st));
     }
@@ -706,6 +721,7 @@ int sht_plan_ntheta(const sht_plan* P, int forward) {
     return R.nth + (R.pole ? 1 : 0);
 }
 double sht_plan_dsteps(const sht_plan* P, int forward) { return P ? (forward ? P->dsteps_fwd : P->dsteps_inv) : 0.0; }
+double sht_plan_flops(const sht_plan* P, int forward) { return P ? (forward ? P->flops_fwd : P->flops_inv) : 0.0; }
 
 sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sht_stream stream) {
     if (!P || !work) return SHT_EINVAL;

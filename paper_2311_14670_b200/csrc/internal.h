@@ -27,6 +27,8 @@ struct ThetaPass {
     int sgn_out;           // harmonic order served at recursion step m is m_out = sgn_out * m  (P mode)
     int m_end;             // last recursion step (inclusive), <= 0
     int slab;              // which (n-)slab of the in/out arrays this pass belongs to
+    int fold;              // forward, n != 0: one pass serves +m from its own ring and -m from the mirrored ring pi - theta via
+                           // d^l_{-m,n}(pi - theta) = (-1)^{l-n} d^l_{m,n}(theta); the sign is applied to the -m column
     const double* st_val;  // [Lp][ntp] windowed start values of d^l_{l,n}
     const uint8_t* st_k;   // [Lp][ntp] window counters
     const int* m_lo;       // [ntp] ring theta is served at step m iff m >= m_lo[theta] (nullptr: always)

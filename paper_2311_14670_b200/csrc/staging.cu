@@ -253,7 +253,9 @@ __global__ void k_mw_pad_phase(int L, int ldin, int ldout, const double2* __rest
 }
 // forward split: U[bin][u] (upsampled F_m(theta'_u), or the ring-FFT output on other samplings) -> weighted operand
 // tiles W[m-m_end][ntp][NC] of one pass; rings not served by the pass at step m get 0 (peak split, R5).
-__global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end,
+// fold != 0 (n != 0, symmetric ring set): column 0 = order +m at the ring itself (m >= m_s), column 1 = order -m at the MIRRORED
+// ring pi - theta (index nth-1-th), served by the same d-value up to (-1)^{l-n} (applied at the output), for m > m_s.
+__global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold,
                                const int* __restrict__ m_lo, const double* __restrict__ wq, const double2* __restrict__ U,
                                double2* __restrict__ W) {
     int th = blockIdx.x * blockDim.x + threadIdx.x;
@@ -261,14 +263,21 @@ __global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int 
     if (th >= ntp) return;
     for (int c = 0; c < NC; ++c) {
         double2 v = {0.0, 0.0};
-        bool ok = th < nth && !(c == 1 && m == 0) && (m < L) && (m > -L);
-        if (ok && m_lo) ok = m >= m_lo[th];
+        bool ok = th < nth && (m < L) && (m > -L);
+        if (fold) { if (ok) ok = c == 0 ? m >= m_lo[th] : m > m_lo[th]; }
+        else {
+            ok = ok && !(c == 1 && m == 0);
+            if (ok && m_lo) ok = m >= m_lo[th];
+        }
         if (ok) {
             int m_out = (c == 1 || sgn_out < 0) ? -m : m;
-            double s = wq[th];
-            if (c == 1) s *= sgn_pow(m);
-            else if (sgn_out < 0) s *= sgn_pow(m + n);
-            double2 x = U[(size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + th];
+            const int ts = (fold && c == 1) ? nth - 1 - th : th;
+            double s = wq[ts];
+            if (!fold) {
+                if (c == 1) s *= sgn_pow(m);
+                else if (sgn_out < 0) s *= sgn_pow(m + n);
+            }
+            double2 x = U[(size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + ts];
             v.x = s * x.x; v.y = s * x.y;
         }
         W[((size_t)(m - m_end) * ntp + th) * NC + c] = v;
@@ -370,7 +379,7 @@ __global__ void k_prep_inverse_batch(int L, int Lp, int NC, int B, int n, int sg
 // forward split: U[b][bin][ldu] -> Wb[cg][m-m_end][ntp][36] (weighted, masked by the peak split; [32] = lambda_m(theta)).
 // Block = 32 rings x one order x one column group.
 __global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int n, int sgn_out,
-                                     int m_end, const int* __restrict__ m_lo, const double* __restrict__ wq,
+                                     int m_end, int fold, const int* __restrict__ m_lo, const double* __restrict__ wq,
                                      const double* __restrict__ lam, const double2* __restrict__ U, double* __restrict__ Wb,
                                      size_t cg_stride) {
     __shared__ double2 tile[32][17];
@@ -379,14 +388,21 @@ __global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, i
     for (int jc = ty; jc < 16; jc += 4) {
         const int j = cg * 16 + jc, b = j / NC, c = j % NC;
         double2 v = make_double2(0.0, 0.0);
-        bool ok = b < B && th < nth && !(c == 1 && m == 0) && m < L && m > -L;
-        if (ok && m_lo) ok = m >= m_lo[th];
+        bool ok = b < B && th < nth && m < L && m > -L;
+        if (fold) { if (ok) ok = c == 0 ? m >= m_lo[th] : m > m_lo[th]; }
+        else {
+            ok = ok && !(c == 1 && m == 0);
+            if (ok && m_lo) ok = m >= m_lo[th];
+        }
         if (ok) {
             const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
-            double s = wq[th];
-            if (c == 1) s *= sgn_pow(m);
-            else if (sgn_out < 0) s *= sgn_pow(m + n);
-            const double2 x = U[(size_t)b * U_slab + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + th];
+            const int ts = (fold && c == 1) ? nth - 1 - th : th;
+            double s = wq[ts];
+            if (!fold) {
+                if (c == 1) s *= sgn_pow(m);
+                else if (sgn_out < 0) s *= sgn_pow(m + n);
+            }
+            const double2 x = U[(size_t)b * U_slab + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + ts];
             v.x = s * x.x; v.y = s * x.y;
         }
         tile[tx][jc] = v;
@@ -403,7 +419,7 @@ __global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, i
 }
 // results: Ob[cg][m-m_end][Mp][32] -> out[b][row(m_out)][ld] += factor * value, complex.  fwd = 0: rows are phi-FFT bins
 // (m_out mod NB) of F, columns rings; fwd = 1: rows m_out+L-1 of H, columns degrees, factor c_m(l) (internal.h).
-__global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int n, int sgn_out, int m_end, int mmin, int fwd,
+__global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
                                const double* __restrict__ C, const double* __restrict__ Ob, size_t cg_stride,
                                double2* __restrict__ out, size_t out_slab, int ld) {
     __shared__ double tile[32][33];
@@ -421,12 +437,17 @@ __global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, i
     }
     for (int jc = ty; jc < 16; jc += 4) {
         const int j = cg * 16 + jc, b = j / NC, c = j % NC;
-        if (b >= B || (c == 1 && m == 0)) continue;
+        if (b >= B || (c == 1 && m == 0 && !fold)) continue;
         const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
         const int row = fwd ? m_out + L - 1 : (m_out < 0 ? m_out + NB : m_out);
         double2* o = out + (size_t)b * out_slab + (size_t)row * ld + mi;
+        const double f2 = (fold && c == 1 && ((mi - n) & 1)) ? -fac : fac;       // (-1)^{l-n} on the mirrored-ring column
+        if (fold && am <= an) {      // rows |m_out| <= |n| receive step m (own ring) and step -m (mirrored ring) of the same launch
+            atomicAdd(&o->x, f2 * tile[tx][2 * jc]); atomicAdd(&o->y, f2 * tile[tx][2 * jc + 1]);
+            continue;
+        }
         double2 v = *o;
-        v.x += fac * tile[tx][2 * jc]; v.y += fac * tile[tx][2 * jc + 1];
+        v.x += f2 * tile[tx][2 * jc]; v.y += f2 * tile[tx][2 * jc + 1];
         *o = v;
     }
 }
@@ -506,10 +527,10 @@ cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double
     k_mw_pad_phase<<<grid, 128, 0, st>>>(L, ldin, ldout, Y, Z);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, const int* m_lo,
+cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
                             const double* wq, const double2* U, double2* W, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
-    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, m_lo, wq, U, W);
+    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, fold, m_lo, wq, U, W);
     LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
@@ -539,15 +560,15 @@ cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, 
     LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
-                                  int m_end, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
+                                  int m_end, int fold, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
                                   size_t cg_stride, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
-    k_weight_split_batch<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, NC, B, n, sgn_out, m_end, m_lo, wq, lam, U, Wb, cg_stride);
+    k_weight_split_batch<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, NC, B, n, sgn_out, m_end, fold, m_lo, wq, lam, U, Wb, cg_stride);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd,
+cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st) {
     dim3 grid(cdiv(Mp, 32), L - m_end, ncg);
-    k_unpack_batch<<<grid, 128, 0, st>>>(L, Lp, Mp, mlim, NC, B, n, sgn_out, m_end, mmin, fwd, C, Ob, cg_stride, out, out_slab, ld);
+    k_unpack_batch<<<grid, 128, 0, st>>>(L, Lp, Mp, mlim, NC, B, n, sgn_out, m_end, mmin, fwd, fold, C, Ob, cg_stride, out, out_slab, ld);
     LAUNCHED(); return cudaSuccess;
 }

@@ -20,7 +20,7 @@ cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStr
 cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st);
 cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st);
 cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
-cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, const int* m_lo,
+cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
                             const double* wq, const double2* U, double2* W, cudaStream_t st);
 cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
                             cudaStream_t st);
@@ -33,9 +33,9 @@ cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, 
                                   const double* scale, const double* C, const double2* SG, int sgstride, double* Gb, size_t cg_stride,
                                   cudaStream_t st);
 cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
-                                  int m_end, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
+                                  int m_end, int fold, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
                                   size_t cg_stride, cudaStream_t st);
-cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd,
+cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st);
 
 // HEALPix ring Fourier staging (healpix.cu)

@@ -422,6 +422,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         int lq[NQ];
         bool valid[NQ], neg[NQ];
         double* obase[NQ];
+        double osgn[NQ];                              // fold passes: (-1)^{l-n} on the -m column (internal.h)
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             const int o = at + NAUX * 32 * q;
@@ -430,6 +431,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             valid[q] = o < NOUT && lq[q] >= an && lq[q] < A.L;
             if (o >= NOUT) lq[q] = l0;
             obase[q] = reinterpret_cast<double*>(P.out) + (size_t)lq[q] * 2;
+            osgn[q] = (P.fold && neg[q] && ((lq[q] - P.n) & 1)) ? -1.0 : 1.0;
         }
         // c_m(l) of the owned degrees, fetched one pair ahead (coalesced rows of the plan-time table)
         const double* crow = A.ctab + (size_t)(mtop - A.mmin) * A.Lp;
@@ -478,10 +480,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
                 if (any && m >= m_end) {
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
-                        if (valid[q] && lq[q] >= m && !(neg[q] && m == 0)) {
+                        // (the -m column of a plain PM pass is all zero at m = 0: its operand is zeroed by the weight split)
+                        if (valid[q] && lq[q] >= m && lq[q] >= -m) {
                             const int m_out = (NC == 2) ? (neg[q] ? -m : m) : P.sgn_out * m;
                             double* o = obase[q] + (size_t)(m_out + A.L - 1) * A.Lp * 2;
-                            red_add_f64(o, v[q].x * cm[h][q]); red_add_f64(o + 1, v[q].y * cm[h][q]);
+                            const double cmq = cm[h][q] * osgn[q];
+                            red_add_f64(o, v[q].x * cmq); red_add_f64(o + 1, v[q].y * cmq);
                         }
                     }
                 }
