@@ -57,6 +57,8 @@ const char* sht_last_error(void);       /* text of the last CUDA / cuFFT failure
  * additional internal terms ... O(L^2)"; Eq. 27 start values in mantissa/exponent form).
  * The workspace must stay valid and untouched while the plan is used.  One plan = one stream at a time.
  * nside is used for HEALPix only (the band-limit L is independent of it).
+ * Environment: SHT_FOLD0=0/1 forces the north-south fold of spin-0 forward transforms off / on at plan creation
+ * (default: on when the northern rings alone fill the GPU, L >= 2048 on MW); results agree to rounding either way.
  */
 sht_status sht_plan_s2(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype);
 sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);

@@ -11,6 +11,7 @@
 #include <cufft.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <map>
@@ -56,6 +57,7 @@ struct RingSet {
     int nth = 0, ntp = 0;      // regular rings, padded count (multiple of 128; > nth so a pole ring fits)
     bool pole = false;         // a theta = pi ring at index nth (MW, Eq. 29)
     bool symmetric = false;    // ring nth-1-t is the mirror image pi - theta_t of ring t
+    int nfull = 0;             // > 0: this set is the northern half (incl. an equator ring) of a symmetric set of nfull rings
     std::vector<ld> ct, c2, s2;  // host: cos(theta), cos(theta/2), sin(theta/2) of the regular rings
     double *csc = nullptr, *tau = nullptr, *sig = nullptr, *c2hi = nullptr, *c2lo = nullptr, *s2hi = nullptr, *s2lo = nullptr;
     double* wq = nullptr;      // [ntp] forward quadrature weight per ring (incl. the pole ring at index nth)
@@ -78,6 +80,7 @@ struct sht_plan {
     int L = 0, spin = 0, sampling = 0, nside = 0, reality = 0, N = 1;
     int Lp = 0, NB = 0;        // padded L; 2L-1
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
+    int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
     int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
     int ncg = 0, ncg_fwd = 0;  // batched path: column groups of 16 complex columns (inverse / forward passes)
     double* Ob = nullptr;      // batched path: result scratch of all passes
@@ -161,6 +164,13 @@ void rings_healpix(RingSet& R, int nside) {
     R.ntp = (int)rup((size_t)R.nth + 1, 128);
 }
 
+// keep the northern half of a symmetric ring set (n = 0 forward fold, theta_kernels.cu FOLD); ring t mirrors ring nfull-1-t
+void north_only(RingSet& R) {
+    R.nfull = R.nth; R.nth = (R.nth + 1) / 2; R.symmetric = false;
+    R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
+    R.ntp = (int)rup((size_t)R.nth, 128);
+}
+
 struct Bump {
     size_t off = 0; char* base = nullptr;
     template <class T> T* take(size_t n) {
@@ -176,7 +186,7 @@ size_t pass_in_doubles(const sht_plan* P, const PassHost& ph, bool fwd) {
     const size_t K = fwd ? P->fwd.ntp : P->Lp;
     if (P->batch > 1) return (size_t)(fwd ? P->ncg_fwd : P->ncg) * (P->L - ph.p.m_end) * K * SHT_MMA_ROW;
     const size_t rows = (size_t)(P->L - ph.p.m_end + 1);
-    return fwd ? rows * K * (ph.mode == 0 ? 4 : 2) : rows * K * theta_inverse_rowd(ph.mode);
+    return fwd ? rows * K * (ph.mode == 0 ? 4 : 2) * (P->fold0 ? 2 : 1) : rows * K * theta_inverse_rowd(ph.mode);
 }
 
 void stage(sht_plan* P, int cat, cudaStream_t st) {
@@ -241,7 +251,7 @@ void layout(sht_plan* P, char* base) {
         P->X_slab = (size_t)NB * NB;
         P->X = B.take<double2>(P->X_slab * P->nslab);
     } else {
-        P->fwd_ld = P->fwd.ntp;
+        P->fwd_ld = (int)rup((size_t)(P->fwd.nfull ? P->fwd.nfull : P->fwd.nth) + 1, 128);
         P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
         P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
         P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
@@ -457,6 +467,7 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     ThetaArgs a{};
     a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.NB = P->NB;
     a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin; a.ctab = P->ctab;
+    a.fold0 = fwd ? P->fold0 : 0;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
     return a;
@@ -574,6 +585,12 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     }
     for (auto& ph : P->pfwd) {
         int n_slab = P->slab_n[ph.p.slab];
+        if (P->fold0) {
+            const int NC = ph.mode == 0 ? 2 : 1;
+            CK(st_weight_split_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, ph.p.m_end, P->fwd.wq, U + U_slab * ph.p.slab,
+                                     reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * 2 * NC, st));
+            continue;
+        }
         CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo,
                            P->fwd.wq, U + U_slab * ph.p.slab,
                            reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), st));
@@ -693,6 +710,14 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, L); }
     else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
+    if (spin == 0 && batch == 1) {
+        // n = 0 fold (theta_kernels.cu FOLD): worth it once the northern half alone fills the GPU with >= 2 waves of 64 x 128 tiles
+        // (L >= 2048 on MW); SHT_FOLD0=0/1 in the environment overrides the choice (used by the tests to cover both paths at small L)
+        const long tiles = (long)(rup(L, 128) / SHT_TQ) * (long)(rup((size_t)(P->fwd.nth + 1) / 2, 128) / 128);
+        bool on = tiles >= 2 * 148;
+        if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
+        if (on) { P->fold0 = 1; north_only(P->fwd); }
+    }
     sht_status s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
@@ -718,7 +743,7 @@ int sht_plan_batch(const sht_plan* P) { return P ? P->batch : 0; }
 int sht_plan_ntheta(const sht_plan* P, int forward) {
     if (!P) return 0;
     const RingSet& R = forward ? P->fwd : P->inv;
-    return R.nth + (R.pole ? 1 : 0);
+    return (R.nfull ? R.nfull : R.nth) + (R.pole ? 1 : 0);
 }
 double sht_plan_dsteps(const sht_plan* P, int forward) { return P ? (forward ? P->dsteps_fwd : P->dsteps_inv) : 0.0; }
 double sht_plan_flops(const sht_plan* P, int forward) { return P ? (forward ? P->flops_fwd : P->flops_inv) : 0.0; }
@@ -749,7 +774,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     CK(cudaMemsetAsync(P->fwd.wq, 0, sizeof(double) * P->fwd.ntp, st));
     if (P->sampling == SHT_MW) {
         // forward quadrature weights q_u = (2 pi/(2L-1)) v_u on the 2L midpoint rings (Eq. 41-44 restated for that ring set)
-        CK(st_mid_weights(L, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
+        CK(st_mid_weights(L, P->fwd.nth, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
     } else {
         // HEALPix: equal pixel weights 4 pi / Npix
         std::vector<double> w(P->fwd.ntp, 0.0);

@@ -47,6 +47,7 @@ struct ThetaArgs {
     const double* ctab;    // [m - mmin][Lp] c_m(l) (forward: applied to the reduced sums of each pass)
     const ThetaPass* passes;
     int npass;
+    int fold0;             // forward, n = 0, northern rings only: operand rows hold the E / O sets (theta_kernels.cu FOLD)
 };
 
 // ---- batched path (theta_mma.cu): the contraction of a batch of maps runs on FP64 tensor-core MMAs -----------------

@@ -122,9 +122,9 @@ __global__ void k_lamtab(int n, int nth, int ntp, int m_end, const double* __res
 //   int_0^pi G sin = (1/2) int_0^2pi G |sin| = pi sum_k G^_k c_k,  |sin| = sum_k c_k e^{ik theta}, c_k = (2/pi)/(1-k^2) (k even),
 // which is Eq. 41-44 with the reflection sign +1 (R9); G^_k from N samples is exact (N > 4L-4).
 // Folding theta <-> 2pi - theta:  v_u = (1/N) (4 + 8 sum_{j=1}^{L-1} cos(2j theta'_u)/(1-4j^2)).   Output: v_u * qphi.
-__global__ void k_mid_weights(int L, double qphi, double* __restrict__ w) {
+__global__ void k_mid_weights(int L, int count, double qphi, double* __restrict__ w) {
     int u = blockIdx.x * blockDim.x + threadIdx.x;
-    if (u >= 2 * L) return;
+    if (u >= count) return;
     const long N = 4L * L;
     double acc = 0.0;
     for (int j = L - 1; j >= 1; --j) {              // small terms first
@@ -281,6 +281,31 @@ __global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int 
             v.x = s * x.x; v.y = s * x.y;
         }
         W[((size_t)(m - m_end) * ntp + th) * NC + c] = v;
+    }
+}
+// forward split for n = 0 on a ring set symmetric about the equator (theta_kernels.cu FOLD): only the nth northern rings are
+// recursed.  W[m][ntp][2][NC]: set 0 = E = q (F_m(theta) + F_m(pi - theta)), set 1 = O = q (F_m(theta) - F_m(pi - theta)); the mirror of
+// ring th is nfull-1-th (the equator ring of HEALPix is its own mirror: E = q F_m, O = 0).  Column c = 1 is order -m with (-1)^m.
+__global__ void k_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end,
+                                     const double* __restrict__ wq, const double2* __restrict__ U, double2* __restrict__ W) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x;
+    int m = m_end + blockIdx.y;
+    if (th >= ntp) return;
+    for (int c = 0; c < NC; ++c) {
+        double2 e = {0.0, 0.0}, o = {0.0, 0.0};
+        if (th < nth && !(c == 1 && m == 0) && m < L && m > -L) {
+            const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
+            const double2* row = U + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
+            double s = wq[th];
+            if (c == 1) s *= sgn_pow(m);
+            const double2 a = row[th];
+            double2 b = {0.0, 0.0};
+            if (tm != th) b = row[tm];
+            e.x = s * (a.x + b.x); e.y = s * (a.y + b.y);
+            if (tm != th) { o.x = s * (a.x - b.x); o.y = s * (a.y - b.y); }
+        }
+        double2* w = W + ((size_t)(m - m_end) * ntp + th) * 2 * NC;
+        w[c] = e; w[NC + c] = o;
     }
 }
 // pole ring theta = pi, forward (Eq. 29): H[-n+L-1][l] += (-1)^{l-n} * wq_pole * U_{-n}(pi)
@@ -472,8 +497,8 @@ cudaError_t st_rsq(int n, double* rsq, cudaStream_t st) {
     k_rsq<<<cdiv(n, 256), 256, 0, st>>>(n, rsq);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mid_weights(int L, double qphi, double* w, cudaStream_t st) {
-    k_mid_weights<<<cdiv(2 * L, 128), 128, 0, st>>>(L, qphi, w);
+cudaError_t st_mid_weights(int L, int count, double qphi, double* w, cudaStream_t st) {
+    k_mid_weights<<<cdiv(count, 128), 128, 0, st>>>(L, count, qphi, w);
     LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st) {
@@ -570,5 +595,11 @@ cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int 
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st) {
     dim3 grid(cdiv(Mp, 32), L - m_end, ncg);
     k_unpack_batch<<<grid, 128, 0, st>>>(L, Lp, Mp, mlim, NC, B, n, sgn_out, m_end, mmin, fwd, fold, C, Ob, cg_stride, out, out_slab, ld);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
+                                  const double2* U, double2* W, cudaStream_t st) {
+    dim3 grid(cdiv(ntp, 128), L - m_end);
+    k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, m_end, wq, U, W);
     LAUNCHED(); return cudaSuccess;
 }

@@ -7,7 +7,7 @@ cudaError_t st_start_values(int L, int n, int nth, int ntp, const double* c2hi, 
 cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t st);
 cudaError_t st_rsq(int n, double* rsq, cudaStream_t st);
 cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st);
-cudaError_t st_mid_weights(int L, double qphi, double* w, cudaStream_t st);
+cudaError_t st_mid_weights(int L, int count, double qphi, double* w, cudaStream_t st);
 cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* coef, const double* scale,
                             const double* C, const double2* SG, int sgstride, double* G, cudaStream_t st);
 cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* kexp, const double* rsq, double* C, cudaStream_t st);
@@ -22,6 +22,8 @@ cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, d
 cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
 cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
                             const double* wq, const double2* U, double2* W, cudaStream_t st);
+cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
+                                  const double2* U, double2* W, cudaStream_t st);
 cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
                             cudaStream_t st);
 cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st);

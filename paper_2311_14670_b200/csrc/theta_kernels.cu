@@ -361,10 +361,14 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 // forward theta step, Eq. 30:  H[m_out+L-1][l] += c_m(l) * sum_theta W[m][theta] * e^l_m(theta)
 // block tile: TLB = 32*RL degrees x NTB = NW*RT rings; KS = 2 recursion steps per pipeline stage
 // =============================================================================================================
-template <int RL, int RT, int NW, int NC>
+// FOLD (n = 0 on a ring set symmetric about the equator): only the northern rings are recursed; d^l_{m,0}(pi - theta) =
+// (-1)^{l+m} d^l_{m,0}(theta), so a degree with l+m even contracts with E = W(theta) + W(pi-theta) and one with
+// l+m odd with O = W(theta) - W(pi-theta).  Operand rows then hold both sets: [ring][E, O][NC]; a thread's two degrees
+// l0 + 2 lane + {0, 1} have opposite, warp-uniform parities.
+template <int RL, int RT, int NW, int NC, bool FOLD>
 struct FwdSmem {
-    static constexpr int TLB = 32 * RL, NTB = NW * RT;
-    double2 wt[NST][KS][NTB * NC];          // weighted F_m samples of the block's rings (TMA ring)
+    static constexpr int TLB = 32 * RL, NTB = NW * RT, NCW = FOLD ? 2 * NC : NC;
+    double2 wt[NST][KS][NTB * NCW];         // weighted F_m samples of the block's rings (TMA ring)
     double lamraw[NST][KS][NTB];            // lambda_m(theta) (TMA ring)
     double2 sg[NST][KS];                    // (s, G) of the block's quantum: [KS-1-h] belongs to step h of the pair
     double hdr[NW][KS][RT];                 // lambda'_m = lambda_m s_m of each warp's own rings
@@ -373,10 +377,11 @@ struct FwdSmem {
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
-template <int RL, int RT, int NW, int NC>
+template <int RL, int RT, int NW, int NC, bool FOLD>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(const ThetaArgs A) {
-    using S = FwdSmem<RL, RT, NW, NC>;
-    constexpr int TLB = S::TLB, NTB = S::NTB, NI = RL * RT;
+    using S = FwdSmem<RL, RT, NW, NC, FOLD>;
+    constexpr int TLB = S::TLB, NTB = S::NTB, NI = RL * RT, NCW = S::NCW;
+    static_assert(RL == 2, "two degrees of opposite parity per thread");
     static_assert(TLB == SHT_TQ, "the block's degrees must be one kappa quantum");
     static_assert(KS * RT <= 32, "one lane per lambda' value of a pair");
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -404,7 +409,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         reg_dealloc_aux();
         const int at = tid - NW * 32;
         constexpr int NOUT = TLB * NC, NQ = (NOUT + NAUX * 32 - 1) / (NAUX * 32);
-        constexpr uint32_t wt_bytes = NTB * NC * sizeof(double2), lam_bytes = NTB * sizeof(double);
+        constexpr uint32_t wt_bytes = NTB * NCW * sizeof(double2), lam_bytes = NTB * sizeof(double);
         const double2* sgrow = A.sg + (size_t)lt * A.sgstride - A.mmin;
         auto issue = [&](int p) {
             const int m = mtop - KS * p, slot = p & (NST - 1);
@@ -412,7 +417,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
 #pragma unroll
             for (int h = 0; h < KS; ++h) {
                 const size_t row = (size_t)(m - h - m_end + 1);
-                bulk_g2s(&sm.wt[slot][h][0], P.in + (row * A.ntp + th0) * 2 * NC, wt_bytes, &sm.full[slot]);
+                bulk_g2s(&sm.wt[slot][h][0], P.in + (row * A.ntp + th0) * 2 * NCW, wt_bytes, &sm.full[slot]);
                 bulk_g2s(&sm.lamraw[slot][h][0], P.lam + row * A.ntp + th0, lam_bytes, &sm.full[slot]);
             }
             bulk_g2s(&sm.sg[slot][0], sgrow + (m - KS + 1), KS * (uint32_t)sizeof(double2), &sm.full[slot]);
@@ -506,7 +511,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     int lr[RL];
 #pragma unroll
     for (int r = 0; r < RL; ++r) {
-        lr[r] = l0 + lane + 32 * r;
+        lr[r] = l0 + RL * lane + r;                    // the thread's degrees are neighbours: opposite parities
         const bool ok = lr[r] >= an && lr[r] < A.L;
         x[r] = (double)(lr[r] - mtop) * (double)(lr[r] + mtop + 1);
 #pragma unroll
@@ -523,7 +528,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
     auto step = [&](const int m, const int slot, const int rs, const int h, double (&ca)[NI],
                     double (&cb)[NI]) -> bool {
-        const double2* T = &sm.wt[slot][h][w * RT * NC];
+        // operand set of degree r: FOLD picks E (l+m even) or O (l+m odd); the parity is warp-uniform
+        const double2* T = &sm.wt[slot][h][w * RT * NCW];
+        const int par = FOLD ? ((l0 + m) & 1) : 0;
+        const double2* Tr[RL];
+#pragma unroll
+        for (int r = 0; r < RL; ++r) Tr[r] = T + (FOLD ? ((par ^ r) & 1) * NC : 0);
         const double* LM = &sm.hdr[w][h][0];
         const double G = sm.sg[slot][KS - 1 - h].y;
         bool wrote = false;
@@ -539,12 +549,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             for (int r = 0; r < RL; ++r) { on[r] = m <= lr[r]; g[r] = on[r] ? x[r] * G : 0.0; }
 #pragma unroll
             for (int i = 0; i < RT; ++i) {
-                const double2 w0 = T[i * NC];
-                double2 w1 = make_double2(0.0, 0.0);
-                if (NC == 2) w1 = T[i * NC + 1];
                 const double lm = LM[i];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
+                    const double2 w0 = Tr[r][i * NCW];
+                    double2 w1 = make_double2(0.0, 0.0);
+                    if (NC == 2) w1 = Tr[r][i * NCW + 1];
                     const double e = ca[r * RT + i];
                     acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
                     if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
@@ -562,12 +572,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
                 const double2 lm2 = *reinterpret_cast<const double2*>(LM + i);
 #pragma unroll
                 for (int ii = 0; ii < 2; ++ii) {
-                    const double2 w0 = T[(i + ii) * NC];
-                    double2 w1 = make_double2(0.0, 0.0);
-                    if (NC == 2) w1 = T[(i + ii) * NC + 1];
                     const double lm = ii ? lm2.y : lm2.x;
 #pragma unroll
                     for (int r = 0; r < RL; ++r) {
+                        const double2 w0 = Tr[r][(i + ii) * NCW];
+                        double2 w1 = make_double2(0.0, 0.0);
+                        if (NC == 2) w1 = Tr[r][(i + ii) * NCW + 1];
                         const double e = ca[r * RT + i + ii];
                         acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
                         if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
@@ -601,7 +611,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             for (int r = 0; r < RL; ++r)
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
-                    rd[c * TLB + lane + 32 * r] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
+                    rd[c * TLB + RL * lane + r] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
                 }
         }
         return wrote;
@@ -670,11 +680,11 @@ cudaError_t launch_inv(const ThetaArgs& a, cudaStream_t st) {
     count_launch();
     return cudaGetLastError();
 }
-template <int RL, int RT, int NW, int NC>
+template <int RL, int RT, int NW, int NC, bool FOLD>
 cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
-    using S = FwdSmem<RL, RT, NW, NC>;
+    using S = FwdSmem<RL, RT, NW, NC, FOLD>;
     const size_t smem = sizeof(S) + 128;
-    auto k = theta_forward_kernel<RL, RT, NW, NC>;
+    auto k = theta_forward_kernel<RL, RT, NW, NC, FOLD>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((a.Lp / S::TLB) * (a.ntp / S::NTB), a.npass);
@@ -700,7 +710,8 @@ cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) 
 }
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
-    return mode == 0 ? launch_fwd<2, 16, 8, 2>(a, st) : launch_fwd<2, 16, 8, 1>(a, st);
+    if (a.fold0) return mode == 0 ? launch_fwd<2, 16, 8, 2, true>(a, st) : launch_fwd<2, 16, 8, 1, true>(a, st);
+    return mode == 0 ? launch_fwd<2, 16, 8, 2, false>(a, st) : launch_fwd<2, 16, 8, 1, false>(a, st);
 }
 cudaError_t launch_fp64_peak(int iters, double* sink, cudaStream_t st, int* blocks, int* threads, int* fma_per_thread) {
     *blocks = 148 * 8; *threads = 256; *fma_per_thread = 16;

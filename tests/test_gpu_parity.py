@@ -191,3 +191,21 @@ def test_healpix_north_star_call_uses_nside_L_over_2(api, orc):
     assert rel(f.cpu().numpy(), orc.s2_inverse(L, 0, orc.HEALPIX, flm, nside=8).real) < TOL
     back = api.s2_forward(f, L, 0, sampling=api.HEALPIX, reality=True).cpu().numpy()
     assert rel(back, orc.s2_forward(L, 0, orc.HEALPIX, f.cpu().numpy().astype(np.complex128), nside=8)) < TOL
+
+
+@pytest.mark.parametrize("fold", ["0", "1"])
+@pytest.mark.parametrize("sampling,L,nside,real", [("mw", 8, 0, False), ("mw", 33, 0, False), ("mw", 130, 0, False), ("mw", 200, 0, True),
+                                                   ("hp", 9, 2, False), ("hp", 24, 8, True), ("hp", 64, 32, False)])
+def test_spin0_forward_with_and_without_north_south_fold(api, orc, monkeypatch, fold, sampling, L, nside, real):
+    """The spin-0 forward runs the recursion on the northern rings only when the plan enables the fold (default at large L):
+    d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta).  Both paths against the oracle, element by element."""
+    monkeypatch.setenv("SHT_FOLD0", fold)
+    if sampling == "mw":
+        f = synth.random_map((L, 2 * L - 1), seed=L, real=real, mw_pole_spin=0)
+        P = api.Plan(L, 0, reality=real)
+        want = orc.s2_forward(L, 0, orc.MW, f.astype(np.complex128))
+    else:
+        f = synth.random_map((12 * nside * nside,), seed=L, real=real)
+        P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=real)
+        want = orc.s2_forward(L, 0, orc.HEALPIX, f.astype(np.complex128), nside=nside)
+    assert rel(P.forward(dev(f)).cpu().numpy(), want) < TOL
