@@ -325,6 +325,24 @@ def sweep(api, synth, torch, dev, flush, fp64_tf):
                  "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
     del P, f, b, flm
     torch.cuda.empty_cache()
+    # BASELINE.json configs[2]: real spin-0 SHT on HEALPix nside = 1024, L = 2048 (forward of the synthesised map: inexact by design)
+    nside, L = 1024, 2048
+    flm = torch.from_numpy(synth.random_flm(L, 0, seed=2, sigma=synth.SIGMA_RED, real=True)).to(dev)
+    P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=True, device=dev)
+    P.enable_timing(True)
+    f = P.inverse(flm); b = P.forward(f)
+    ti, tf = [], []
+    for _ in range(3):
+        flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
+        flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
+    mi = {k: min(t[k] for t in ti) for k in ti[0]}
+    mf = {k: min(t[k] for t in tf) for k in tf[0]}
+    rows.append({"config": f"HEALPix nside={nside} L={L} spin-0 real", "inverse_ms": mi, "forward_ms": mf,
+                 "inverse_frac_fp64": P.flops(False) / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
+                 "forward_frac_fp64": P.flops(True) / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
+                 "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
+    del P, f, b, flm
+    torch.cuda.empty_cache()
     L, N = 256, 8
     c = torch.from_numpy(synth.random_flmn(L, N, seed=3)).to(dev)
     P = api.Plan(L, N=N, device=dev)

@@ -19,6 +19,7 @@
 
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 namespace {
 
@@ -171,7 +172,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         // ---------------------------------------------------------------- auxiliary warps: TMA producer + reducers
         reg_dealloc_aux();
         const int at = tid - NW * 32;                 // 0..127: owns output pairs (re, im) at, at+128, ... of the NOUT per step
-        constexpr int NOUT = NTH * NC, NQ = NOUT / (NAUX * 32);
+        constexpr int NOUT = NTH * NC, NQ = (NOUT + NAUX * 32 - 1) / (NAUX * 32);
         constexpr uint32_t op_bytes = TL * ROWD * sizeof(double), lam_bytes = NTH * sizeof(double);
         auto issue = [&](int p) {
             const int m = mtop - KS * p, slot = p & (NST - 1);
@@ -193,7 +194,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             const int o = at + NAUX * 32 * q;
             const int th = th0 + o % NTH;             // partial sums are stored [column][ring]
             neg[q] = NC == 2 && (o / NTH);
-            valid[q] = th < A.nth;
+            valid[q] = th < A.nth && o < NOUT;
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
             if (mlo[q] < m_end) mlo[q] = m_end;
             obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2;
@@ -217,7 +218,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                         any = true;
                         const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]) + at;
 #pragma unroll
-                        for (int q = 0; q < NQ; ++q) { const double2 t = r[NAUX * 32 * q]; v[q].x += t.x; v[q].y += t.y; }
+                        for (int q = 0; q < NQ; ++q)
+                            if (at + NAUX * 32 * q < NOUT) { const double2 t = r[NAUX * 32 * q]; v[q].x += t.x; v[q].y += t.y; }
                     }
                 }
                 if (any) {
@@ -704,12 +706,28 @@ extern "C" void sht_prof_read(unsigned long long* out, int reset) {
 }
 #endif
 int theta_inverse_rowd(int mode) { return mode == 0 ? 6 : 4; }
+// Tile choice.  A launch has (Lp/64) x (ntp/rings_per_block) x npass blocks whose step counts grow linearly with the degree
+// tile, and the longest block alone runs ~L steps.  When 64 x 128 tiles do not even give one block per SM the launch is bound by
+// that longest block while the other SMs idle; 64 x 64 tiles then halve the work per step of every block (measured: L = 512
+// spin 0 inverse 0.456 -> 0.275 ms, L = 1024 spin 0 inverse 0.906 -> 0.548 ms; with more blocks than SMs the big tile wins).
+// SHT_TILE=64/128 overrides.
+static bool small_tiles(const ThetaArgs& a, int big) {
+    static const char* env = getenv("SHT_TILE");
+    if (env) return atoi(env) == 64;
+    const long blocks = (long)(a.Lp / SHT_TQ) * (a.ntp / big) * a.npass;
+    return blocks <= 148;
+}
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
+    if (small_tiles(a, 128)) return mode == 0 ? launch_inv<8, 2, 8, 2>(a, st) : launch_inv<8, 2, 8, 1>(a, st);
     return mode == 0 ? launch_inv<8, 4, 8, 2>(a, st) : launch_inv<8, 4, 8, 1>(a, st);
 }
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
+    if (small_tiles(a, 128)) {
+        if (a.fold0) return mode == 0 ? launch_fwd<2, 8, 8, 2, true>(a, st) : launch_fwd<2, 8, 8, 1, true>(a, st);
+        return mode == 0 ? launch_fwd<2, 8, 8, 2, false>(a, st) : launch_fwd<2, 8, 8, 1, false>(a, st);
+    }
     if (a.fold0) return mode == 0 ? launch_fwd<2, 16, 8, 2, true>(a, st) : launch_fwd<2, 16, 8, 1, true>(a, st);
     return mode == 0 ? launch_fwd<2, 16, 8, 2, false>(a, st) : launch_fwd<2, 16, 8, 1, false>(a, st);
 }
