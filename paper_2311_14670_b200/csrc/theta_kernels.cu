@@ -136,6 +136,7 @@ __device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]
 template <int RL, int RT, int NW, int NC>
 struct InvSmem {
     static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2;
+    static constexpr int NRS = NC == 1 ? 4 : 2;   // the one-column partial sums are half the size: a deeper hand-off fits
     double op[NST][KS][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
     double lam[NST][KS][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
     double red[NRS][KS][NW][NTH][2 * NC];   // per-warp partial sums
@@ -146,7 +147,7 @@ struct InvSmem {
 template <int RL, int RT, int NW, int NC>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(const ThetaArgs A) {
     using S = InvSmem<RL, RT, NW, NC>;
-    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD;
+    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS;
     static_assert(TL == SHT_TQ, "the block's degrees must be one kappa quantum");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
