@@ -184,7 +184,7 @@ struct Bump {
 // doubles of one pass's operand buffer (single-map kernels: rows m_end-1..L-1; batched: rows m_end..L-1 per column group)
 size_t pass_in_doubles(const sht_plan* P, const PassHost& ph, bool fwd) {
     const size_t K = fwd ? P->fwd.ntp : P->Lp;
-    if (P->batch > 1) return (size_t)(fwd ? P->ncg_fwd : P->ncg) * (P->L - ph.p.m_end) * K * SHT_MMA_ROW;
+    if (P->batch > 1) return (size_t)(fwd ? P->ncg_fwd : P->ncg) * (P->L - ph.p.m_end) * K * (fwd && P->fold0 ? SHT_MMA_ROWF : SHT_MMA_ROW);
     const size_t rows = (size_t)(P->L - ph.p.m_end + 1);
     return fwd ? rows * K * (ph.mode == 0 ? 4 : 2) * (P->fold0 ? 2 : 1) : rows * K * theta_inverse_rowd(ph.mode);
 }
@@ -476,7 +476,7 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
 MmaArgs mma_args(const sht_plan* P, bool fwd) {
     const RingSet& R = fwd ? P->fwd : P->inv;
     MmaArgs a{};
-    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.ncg = fwd ? P->ncg_fwd : P->ncg;
+    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.ncg = fwd ? P->ncg_fwd : P->ncg; a.fold0 = fwd ? P->fold0 : 0;
     a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin;
     a.passes = fwd ? P->d_fwd_p : P->d_inv_p;
     a.npass = fwd ? P->n_fwd_p : P->n_inv_p;
@@ -557,6 +557,13 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         for (size_t i = 0; i < P->pfwd.size(); ++i) {
             auto& ph = P->pfwd[i];
             const size_t rows = (size_t)(L - ph.p.m_end);
+            if (P->fold0) {
+                CK(st_weight_split_batch_fold0(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, ph.mode == 0 ? 2 : 1, P->batch,
+                                               P->ncg_fwd, ph.p.m_end, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
+                                               rows * P->fwd.ntp * SHT_MMA_ROWF, st));
+                CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
+                continue;
+            }
             CK(st_weight_split_batch(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, P->slab_n[0],
                                      ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
                                      rows * P->fwd.ntp * SHT_MMA_ROW, st));
@@ -567,7 +574,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
             MmaArgs a = mma_args(P, true);
             const size_t rows = (size_t)(L - P->pfwd[i].p.m_end);
             a.passes += i; a.npass = 1;
-            a.in_cg_stride = rows * P->fwd.ntp * SHT_MMA_ROW; a.out_cg_stride = rows * P->Lp * SHT_MMA_NCOL;
+            a.in_cg_stride = rows * P->fwd.ntp * (P->fold0 ? SHT_MMA_ROWF : SHT_MMA_ROW); a.out_cg_stride = rows * P->Lp * SHT_MMA_NCOL;
             CK(launch_theta_mma(a, true, st));
         }
         stage(P, CAT_STAGE, st);
@@ -710,10 +717,10 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, L); }
     else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
-    if (spin == 0 && batch == 1) {
+    if (spin == 0) {
         // n = 0 fold (theta_kernels.cu FOLD): worth it once the northern half alone fills the GPU with >= 2 waves of 64 x 128 tiles
         // (L >= 2048 on MW); SHT_FOLD0=0/1 in the environment overrides the choice (used by the tests to cover both paths at small L)
-        const long tiles = (long)(rup(L, 128) / SHT_TQ) * (long)(rup((size_t)(P->fwd.nth + 1) / 2, 128) / 128);
+        const long tiles = (long)(rup(L, 128) / SHT_TQ) * (long)(rup((size_t)(P->fwd.nth + 1) / 2, 128) / 128) * (batch > 1 ? 4 : 1);
         bool on = tiles >= 2 * 148;
         if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
         if (on) { P->fold0 = 1; north_only(P->fwd); }

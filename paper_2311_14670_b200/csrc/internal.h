@@ -53,6 +53,7 @@ struct ThetaArgs {
 // ---- batched path (theta_mma.cu): the contraction of a batch of maps runs on FP64 tensor-core MMAs -----------------
 #define SHT_MMA_NCOL 32   // real columns per column group = 16 complex columns (map, +-m)
 #define SHT_MMA_ROW 36    // doubles per operand row: 32 columns + 2 side columns + 2 pad (conflict-free LDS.64)
+#define SHT_MMA_ROWF 68   // forward rows of the n = 0 fold: 32 columns E + 32 columns O + lambda + 3 pad
 // Operand rows, one per (column group, m - m_end, K index), SHT_MMA_ROW doubles:
 //   inverse  Gb[cg][m-m_end][Lp][36]:  32 columns c_m(l) scale(l) f_lm (re, im per complex column), [32] g'_m(l), [33] s_m
 //   forward  Wb[cg][m-m_end][ntp][36]: 32 columns q(theta) F_m(theta),                                [32] lambda_m(theta)
@@ -63,6 +64,7 @@ struct MmaArgs {
     const double2* sg;         // (s_m, G_m) per quantum, as in ThetaArgs
     int sgstride, mmin;
     size_t in_cg_stride, out_cg_stride;   // doubles between column groups of ThetaPass::in / ::out
+    int fold0;                 // forward, n = 0: northern rings only, operand rows of SHT_MMA_ROWF doubles (E and O column sets)
     const ThetaPass* passes;   // in = Gb / Wb of the pass, out = Ob of the pass, lam / st_val / st_k / m_lo as in the single-map kernels
     int npass;
 };

@@ -442,6 +442,40 @@ __global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, i
         g[idx] = v;
     }
 }
+// forward split of the n = 0 fold (theta_mma.cu FOLD): Wb[cg][m-m_end][ntp north][68] = {32 columns E, 32 columns O, lambda, pad};
+// E = q (F_m(theta) + F_m(pi - theta)), O = q (F_m(theta) - F_m(pi - theta)), mirror ring index nfull-1-th.
+__global__ void k_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int m_end,
+                                           const double* __restrict__ wq, const double* __restrict__ lam,
+                                           const double2* __restrict__ U, double* __restrict__ Wb, size_t cg_stride) {
+    __shared__ double2 tile[2][32][17];
+    const int cg = blockIdx.z, m = m_end + blockIdx.y, t0 = blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, th = t0 + tx;
+    for (int jc = ty; jc < 16; jc += 4) {
+        const int j = cg * 16 + jc, b = j / NC, c = j % NC;
+        double2 e = make_double2(0.0, 0.0), o = make_double2(0.0, 0.0);
+        if (b < B && th < nth && !(c == 1 && m == 0) && m < L && m > -L) {
+            const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
+            const double2* row = U + (size_t)b * U_slab + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
+            double s = wq[th];
+            if (c == 1) s *= sgn_pow(m);
+            const double2 a = row[th];
+            double2 v = make_double2(0.0, 0.0);
+            if (tm != th) v = row[tm];
+            e.x = s * (a.x + v.x); e.y = s * (a.y + v.y);
+            if (tm != th) { o.x = s * (a.x - v.x); o.y = s * (a.y - v.y); }
+        }
+        tile[0][tx][jc] = e; tile[1][tx][jc] = o;
+    }
+    __syncthreads();
+    double* g = Wb + (size_t)cg * cg_stride + ((size_t)(m - m_end) * ntp + t0) * SHT_MMA_ROWF;
+    for (int idx = threadIdx.x; idx < 32 * SHT_MMA_ROWF; idx += blockDim.x) {
+        const int ti = idx / SHT_MMA_ROWF, col = idx % SHT_MMA_ROWF;
+        double v = 0.0;
+        if (col < 2 * SHT_MMA_NCOL) { const int cc = col % SHT_MMA_NCOL; const double2 t = tile[col / SHT_MMA_NCOL][ti][cc >> 1]; v = (cc & 1) ? t.y : t.x; }
+        else if (col == 2 * SHT_MMA_NCOL) v = lam[(size_t)(m - m_end + 1) * ntp + t0 + ti];
+        g[idx] = v;
+    }
+}
 // results: Ob[cg][m-m_end][Mp][32] -> out[b][row(m_out)][ld] += factor * value, complex.  fwd = 0: rows are phi-FFT bins
 // (m_out mod NB) of F, columns rings; fwd = 1: rows m_out+L-1 of H, columns degrees, factor c_m(l) (internal.h).
 __global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
@@ -601,5 +635,12 @@ cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, i
                                   const double2* U, double2* W, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
     k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, m_end, wq, U, W);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
+                                        int m_end, const double* wq, const double* lam, const double2* U, double* Wb, size_t cg_stride,
+                                        cudaStream_t st) {
+    dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
+    k_weight_split_batch_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, nfull, NC, B, m_end, wq, lam, U, Wb, cg_stride);
     LAUNCHED(); return cudaSuccess;
 }

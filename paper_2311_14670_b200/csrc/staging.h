@@ -37,6 +37,9 @@ cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, 
 cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
                                   int m_end, int fold, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
                                   size_t cg_stride, cudaStream_t st);
+cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
+                                        int m_end, const double* wq, const double* lam, const double2* U, double* Wb, size_t cg_stride,
+                                        cudaStream_t st);
 cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st);
 

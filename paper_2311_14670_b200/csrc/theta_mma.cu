@@ -110,18 +110,25 @@ struct KPack32 {
     }
 };
 
+// FOLD (forward, n = 0, northern rings only): an operand row holds two column sets, E = q (F_m(theta) + F_m(pi - theta)) and
+// O = q (F_m(theta) - F_m(pi - theta)); a degree with l+m even contracts with E, one with l+m odd with O (PAPER.md:236,
+// d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta)).  The M rows of one DMMA are then the 8 degrees mw0 + 2 gid + ib of equal parity.
+template <int ROW_>
 struct MmaSmem {
-    double op[NSTG][TK * ROW];      // operand rows of the CTA's 64 K-values: 32 columns + side columns (TMA ring)
+    double op[NSTG][TK * ROW_];     // operand rows of the CTA's 64 K-values: 32 columns + side columns (TMA ring)
     double side[NSTG][TM];          // inverse: lambda_m(theta) of the CTA's 128 rings; forward: (s, G) of its 2 quanta
     double stg[NW][2][16 * SHT_MMA_NCOL];   // per-warp result tiles (double-buffered source of the bulk reduce)
     uint64_t full[NSTG], empty[NSTG];
 };
 
 // FWD = false: inverse (K = degrees, M = rings).  FWD = true: forward (K = rings, M = degrees).
-template <bool FWD>
+template <bool FWD, bool FOLD>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const MmaArgs A) {
+    static_assert(FWD || !FOLD, "the fold is a forward variant");
+    constexpr int ROW = FOLD ? SHT_MMA_ROWF : SHT_MMA_ROW;       // shadows the namespace constant
+    constexpr int SIDE = FOLD ? 2 * SHT_MMA_NCOL : SHT_MMA_NCOL;  // index of the first side column of an operand row
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    MmaSmem& sm = *reinterpret_cast<MmaSmem*>(smem_raw);
+    MmaSmem<ROW>& sm = *reinterpret_cast<MmaSmem<ROW>*>(smem_raw);
 
     const ThetaPass P = A.passes[blockIdx.y];
     const int cg = blockIdx.z;
@@ -173,6 +180,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
     // ----------------------------------------------------------------------------- compute warps
     const int gid = lane >> 2, tig = lane & 3;
     const int mw0 = m0 + w * 8 * NIB;                   // first M row of this warp
+    auto mrow = [&](int ib) { return FOLD ? 2 * gid + ib : 8 * ib + gid; };   // M row (within the warp's 16) of the thread's block ib
     // forward: this warp's degrees are mw0 .. mw0+15 (inside one quantum); inverse: the CTA's 64 degrees are shared
     const int l_hi = FWD ? mw0 + 8 * NIB - 1 : l0 + TK - 1;       // highest degree this warp touches
     const int l_lo = FWD ? mw0 : l0;
@@ -187,7 +195,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
     double lr[NIB];                                     // forward: degree of the thread's M rows (as double)
 #pragma unroll
     for (int ib = 0; ib < NIB; ++ib) {
-        const int mi = mw0 + 8 * ib + gid;
+        const int mi = mw0 + mrow(ib);
         mlo[ib] = -(1 << 30);
         if (!FWD) {
             if (P.m_lo) mlo[ib] = P.m_lo[mi];
@@ -204,8 +212,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
         // ---- Eq. 27 start values of the degree l == m (items of that degree were all-zero so far)
         if (m >= l_lo) {
             if (FWD) {
-                const int d = m - mw0, ibs = d >> 3;
-                if (gid == (d & 7)) {
+                const int d = m - mw0, ibs = FOLD ? (d & 1) : (d >> 3);
+                if (gid == (FOLD ? (d >> 1) : (d & 7))) {
                     const double* sv = P.st_val + (size_t)m * A.ntp + th0 + tig;
                     const uint8_t* sk = P.st_k + (size_t)m * A.ntp + th0 + tig;
 #pragma unroll
@@ -252,6 +260,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
             for (int ib = 0; ib < NIB; ++ib) cM[ib] = sm.side[slot][w * 8 * NIB + 8 * ib + gid] * s;
         }
         const double* kr = op + tig * ROW;              // row of K = 4 jb + tig is kr + 4 jb ROW
+        const int par0 = (mw0 + m) & 1;                 // FOLD: parity of l + m of block ib = 0 (block 1 has the other one)
         if (wact) {
             double acc[NIB][NT8][2];
 #pragma unroll
@@ -261,15 +270,17 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
 #pragma unroll
             for (int jb = 0; jb < NJ; ++jb) {
                 const double* r = kr + 4 * jb * ROW;
-                double b[NT8];
+                double b[FOLD ? NIB : 1][NT8];            // FOLD: block ib contracts with the column set of its parity
 #pragma unroll
-                for (int nt = 0; nt < NT8; ++nt) b[nt] = r[8 * nt + gid];
-                const double cK = r[SHT_MMA_NCOL] * sK;   // inverse: g'_m(l); forward: lambda_m(theta) s_m
+                for (int s2 = 0; s2 < (FOLD ? NIB : 1); ++s2)
+#pragma unroll
+                    for (int nt = 0; nt < NT8; ++nt) b[s2][nt] = r[(FOLD ? ((par0 ^ s2) & 1) * SHT_MMA_NCOL : 0) + 8 * nt + gid];
+                const double cK = r[SIDE] * sK;           // inverse: g'_m(l); forward: lambda_m(theta) s_m
 #pragma unroll
                 for (int ib = 0; ib < NIB; ++ib) {
                     const double e = ca[jb * NIB + ib];
 #pragma unroll
-                    for (int nt = 0; nt < NT8; ++nt) dmma(acc[ib][nt], e, b[nt]);
+                    for (int nt = 0; nt < NT8; ++nt) dmma(acc[ib][nt], e, b[FOLD ? ib : 0][nt]);
                     if (FWD) cb[jb * NIB + ib] = fma(cK, e, -(cM[ib] * cb[jb * NIB + ib]));
                     else cb[jb * NIB + ib] = fma(cM[ib], e, -(cK * cb[jb * NIB + ib]));
                 }
@@ -283,7 +294,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
                 const bool keep = m >= mlo[ib];
 #pragma unroll
                 for (int nt = 0; nt < NT8; ++nt)
-                    *reinterpret_cast<double2*>(sb + (8 * ib + gid) * SHT_MMA_NCOL + 8 * nt + 2 * tig) =
+                    *reinterpret_cast<double2*>(sb + mrow(ib) * SHT_MMA_NCOL + 8 * nt + 2 * tig) =
                         keep ? make_double2(acc[ib][nt][0], acc[ib][nt][1]) : make_double2(0.0, 0.0);
             }
             fence_async_smem();
@@ -296,7 +307,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
         } else {                                        // every item of the warp is still below 2^-340: recursion only
 #pragma unroll
             for (int jb = 0; jb < NJ; ++jb) {
-                const double cK = kr[4 * jb * ROW + SHT_MMA_NCOL] * sK;
+                const double cK = kr[4 * jb * ROW + SIDE] * sK;
 #pragma unroll
                 for (int ib = 0; ib < NIB; ++ib) {
                     if (FWD) cb[jb * NIB + ib] = fma(cK, ca[jb * NIB + ib], -(cM[ib] * cb[jb * NIB + ib]));
@@ -343,21 +354,19 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
 
 }  // namespace
 
-cudaError_t launch_theta_mma(const MmaArgs& a, bool forward, cudaStream_t st) {
-    if (a.npass == 0) return cudaSuccess;
-    const size_t smem = sizeof(MmaSmem) + 128;
-    cudaError_t e;
-    if (forward) {
-        e = cudaFuncSetAttribute(theta_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        dim3 grid((a.Lp / TM) * (a.ntp / TK), a.npass, a.ncg);
-        theta_mma_kernel<true><<<grid, (NW + NAUX) * 32, smem, st>>>(a);
-    } else {
-        e = cudaFuncSetAttribute(theta_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        dim3 grid((a.Lp / TK) * (a.ntp / TM), a.npass, a.ncg);
-        theta_mma_kernel<false><<<grid, (NW + NAUX) * 32, smem, st>>>(a);
-    }
+template <bool FWD, bool FOLD>
+static cudaError_t launch_mma(const MmaArgs& a, cudaStream_t st) {
+    const size_t smem = sizeof(MmaSmem<FOLD ? SHT_MMA_ROWF : SHT_MMA_ROW>) + 128;
+    cudaError_t e = cudaFuncSetAttribute(theta_mma_kernel<FWD, FOLD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(FWD ? (a.Lp / TM) * (a.ntp / TK) : (a.Lp / TK) * (a.ntp / TM), a.npass, a.ncg);
+    theta_mma_kernel<FWD, FOLD><<<grid, (NW + NAUX) * 32, smem, st>>>(a);
     count_launch();
     return cudaGetLastError();
+}
+
+cudaError_t launch_theta_mma(const MmaArgs& a, bool forward, cudaStream_t st) {
+    if (a.npass == 0) return cudaSuccess;
+    if (!forward) return launch_mma<false, false>(a, st);
+    return a.fold0 ? launch_mma<true, true>(a, st) : launch_mma<true, false>(a, st);
 }

@@ -91,3 +91,16 @@ def test_config5b_batch16_L2048(api, orc):
         gb = got[b].cpu().numpy()
         for m, col in zip(ms, want):
             assert rel(gb[:, m + L - 1], col, sc) < TOL, (b, m)
+
+
+@pytest.mark.parametrize("fold", ["0", "1"])
+@pytest.mark.parametrize("L,batch,real", [(8, 2, False), (33, 3, False), (130, 9, False), (200, 16, False), (96, 4, True)])
+def test_batched_spin0_forward_with_and_without_fold(api, orc, monkeypatch, fold, L, batch, real):
+    """Batched spin-0 forward with the north-south fold forced on / off (default: on at large L): recursion on the northern rings,
+    even / odd l+m rows contract with the E / O column sets (theta_mma.cu FOLD).  White-noise maps, every map against the oracle."""
+    monkeypatch.setenv("SHT_FOLD0", fold)
+    g = synth.random_map((batch, L, 2 * L - 1), seed=7 * L, real=real, mw_pole_spin=0)
+    P = api.Plan(L, 0, reality=real, batch=batch)
+    got = P.forward(dev(g)).cpu().numpy()
+    for b in range(batch):
+        assert rel(got[b], orc.s2_forward(L, 0, orc.MW, g[b].astype(np.complex128))) < TOL, b
