@@ -80,6 +80,8 @@ struct sht_plan {
     int L = 0, spin = 0, sampling = 0, nside = 0, reality = 0, N = 1;
     int Lp = 0, NB = 0;        // padded L; 2L-1
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
+    int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
+    int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
     int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
     int ncg = 0, ncg_fwd = 0;  // batched path: column groups of 16 complex columns (inverse / forward passes)
@@ -238,12 +240,14 @@ void layout(sht_plan* P, char* base) {
         P->Ob = B.take<double>(oi > of ? oi : of);
     }
     // scratch arrays
-    P->F_slab = (size_t)NB * P->inv.ntp;
+    P->F_nrings = (P->inv.nfull ? P->inv.nfull : P->inv.nth) + (P->inv.pole ? 1 : 0);
+    P->F_ld = P->inv.nfull ? (int)rup((size_t)P->inv.nfull + 1, 128) : P->inv.ntp;
+    P->F_slab = (size_t)NB * P->F_ld;
     P->F = B.take<double2>(P->F_slab * P->nslab);
     P->polev = B.take<double2>(P->nslab);
     P->tmp = B.take<double>(2 * (size_t)Lp);
     P->unit_wq = B.take<double>(P->fwd.ntp);
-    P->Ltp = P->inv.ntp;
+    P->Ltp = P->F_ld;
     if (P->sampling == SHT_MW) {
         P->fwd_ld = 4 * L;
         P->Fa_slab = (size_t)NB * P->Ltp;
@@ -321,10 +325,10 @@ sht_status make_fft_plans(sht_plan* P) {
     int n1[1] = {NB};
     CF(cufftCreate(&P->fft_phi_inv)); CF(cufftSetAutoAllocation(P->fft_phi_inv, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, P->inv.ntp, 1, onembed, 1, NB, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, (int)rup((size_t)L, 128), 1, onembed, 1, NB, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
     CF(cufftCreate(&P->fft_phi_fwd)); CF(cufftSetAutoAllocation(P->fft_phi_fwd, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, P->inv.ntp, 1, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, (int)rup((size_t)L, 128), 1, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
     CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
     { int inembed[1] = {NB};
       CF(cufftMakePlanMany(P->fft_th1, 1, n1, inembed, 1, NB, inembed, 1, NB, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
@@ -467,7 +471,8 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     ThetaArgs a{};
     a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.NB = P->NB;
     a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin; a.ctab = P->ctab;
-    a.fold0 = fwd ? P->fold0 : 0;
+    a.fold0 = fwd ? P->fold0 : P->fold0i;
+    a.ldout = P->F_ld; a.nfull = R.nfull;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
     return a;
@@ -521,11 +526,11 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
             for (int s = 0; s < P->nslab; ++s) {
                 int n = P->slab_n[s];
                 int row = (-n) < 0 ? -n + P->NB : -n;
-                CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->inv.ntp + P->inv.nth, st));
+                CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->F_ld + P->inv.nth, st));
             }
         }
         if (P->reality)
-            for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->inv.ntp, P->inv.nth + (P->inv.pole ? 1 : 0), P->F + P->F_slab * s, st));
+            for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F + P->F_slab * s, st));
         return SHT_OK;
     }
     for (auto& ph : P->pinv)
@@ -540,12 +545,12 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         for (int s = 0; s < P->nslab; ++s) {
             int n = P->slab_n[s];
             int row = (-n) < 0 ? -n + P->NB : -n;
-            CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->inv.ntp + P->inv.nth, st));
+            CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->F_ld + P->inv.nth, st));
         }
     }
     stage(P, CAT_STAGE, st);
     if (P->reality)
-        for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->inv.ntp, P->inv.nth + (P->inv.pole ? 1 : 0), P->F + P->F_slab * s, st));
+        for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F + P->F_slab * s, st));
     return SHT_OK;
 }
 // U: [slab][bin][ldu] samples of F_m on the forward ring set (weights not yet applied).  Leaves H complete.
@@ -660,7 +665,7 @@ sht_status healpix_synthesis(sht_plan* P, void* f, cudaStream_t st) {
     const int ns = P->nside, L = P->L, real = P->reality;
     const size_t nbelt = (size_t)P->hp_neq * 4 * ns;
     stage(P, CAT_STAGE, st);
-    CK(st_hp_fold_inv(ns, L, P->NB, P->inv.ntp, P->hp_M, P->F, P->hp_C, P->hp_E, st));
+    CK(st_hp_fold_inv(ns, L, P->NB, P->F_ld, P->hp_M, P->F, P->hp_C, P->hp_E, st));
     stage(P, CAT_FFT, st);
     CF(cufftSetStream(P->fft_hp_eq, st));
     CF(cufftExecZ2Z(P->fft_hp_eq, P->hp_E, real ? P->hp_E : (double2*)f + P->hp_off_eq, CUFFT_INVERSE));
@@ -724,6 +729,8 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
         bool on = tiles >= 2 * 148;
         if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
         if (on) { P->fold0 = 1; north_only(P->fwd); }
+        // the inverse rings of HEALPix are symmetric too (the MW rings (2t+1)pi/(2L-1) are not)
+        if (on && sampling == SHT_HEALPIX && batch == 1) { P->fold0i = 1; north_only(P->inv); }
     }
     sht_status s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
@@ -851,7 +858,7 @@ sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_str
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
     int nt = sht_plan_ntheta(P, 0);
-    CK(st_rows_reorder(P->L, P->NB, nt, P->inv.ntp, nt, 1, P->F, (double2*)Fm, st));
+    CK(st_rows_reorder(P->L, P->NB, nt, P->F_ld, nt, 1, P->F, (double2*)Fm, st));
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }

@@ -42,12 +42,15 @@ struct ThetaArgs {
     int L, Lp;             // band-limit, padded (multiple of 128)
     int nth, ntp;          // regular rings, padded (multiple of 128)
     int NB;                // rows of the inverse output (FFT length in phi, 2L-1)
+    int ldout;             // inverse: row length of the output F[row][ldout] (= ntp unless the ring set is a folded half)
+    int nfull;             // folded ring sets: ring th of the northern half mirrors ring nfull-1-th of the full set
     const double2* sg;     // [Lp/TQ][sgstride] (s_m, G_m) per quantum, column m - mmin
     int sgstride, mmin;
     const double* ctab;    // [m - mmin][Lp] c_m(l) (forward: applied to the reduced sums of each pass)
     const ThetaPass* passes;
     int npass;
-    int fold0;             // forward, n = 0, northern rings only: operand rows hold the E / O sets (theta_kernels.cu FOLD)
+    int fold0;             // n = 0, northern rings only (theta_kernels.cu FOLD): forward operand rows hold the E / O sets,
+                           // the inverse keeps even-l / odd-l partial sums and writes both rings of a mirror pair
 };
 
 // ---- batched path (theta_mma.cu): the contraction of a batch of maps runs on FP64 tensor-core MMAs -----------------

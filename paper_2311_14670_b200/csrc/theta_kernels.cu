@@ -133,21 +133,26 @@ __device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]
 // inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * e^l_m(theta)      (G carries c_m(l))
 // block tile: TL = NW*RL degrees x NTH = 32*RT rings; KS = 2 recursion steps per pipeline stage
 // =============================================================================================================
-template <int RL, int RT, int NW, int NC>
+// FOLD (n = 0 on a ring set symmetric about the equator): only the northern rings are recursed.  d^l_{m0}(pi - theta) =
+// (-1)^{l+m} d^l_{m0}(theta), so with E = sum over l+m even and O = sum over l+m odd of G d:
+// F_m(theta) = E + O and F_m(pi - theta) = E - O.  A thread's degrees la + j alternate in parity with j (la is even), so two
+// accumulator sets (j even / j odd) are kept and the reducers emit both rings.
+template <int RL, int RT, int NW, int NC, bool FOLD>
 struct InvSmem {
-    static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2;
-    static constexpr int NRS = NC == 1 ? 4 : 2;   // the one-column partial sums are half the size: a deeper hand-off fits
+    static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2, NSET = FOLD ? 2 : 1;
+    static constexpr int NRS = (NC == 1 && !FOLD) ? 4 : 2;   // the one-column partial sums are half the size: a deeper hand-off fits
     double op[NST][KS][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
     double lam[NST][KS][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
-    double red[NRS][KS][NW][NTH][2 * NC];   // per-warp partial sums
+    double red[NRS][KS][NW][NSET][NTH][2 * NC];   // per-warp partial sums
     int act[NRS][NW];                       // bit h: the warp wrote partial sums for step h of the pair
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
-template <int RL, int RT, int NW, int NC>
+template <int RL, int RT, int NW, int NC, bool FOLD>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(const ThetaArgs A) {
-    using S = InvSmem<RL, RT, NW, NC>;
-    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS;
+    using S = InvSmem<RL, RT, NW, NC, FOLD>;
+    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS, NSET = S::NSET;
+    static_assert(!FOLD || (RL % 2 == 0), "degrees of a thread alternate in parity");
     static_assert(TL == SHT_TQ, "the block's degrees must be one kappa quantum");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
@@ -188,8 +193,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         if (at == 0)
             for (int p = 0; p < NST && p < npairs; ++p) issue(p);
         int mlo[NQ];
-        bool valid[NQ], neg[NQ];
+        bool valid[NQ], neg[NQ], south[NQ];
         double* obase[NQ];
+        ptrdiff_t osouth[NQ];                         // FOLD: offset (doubles) from the ring's entry to its mirror ring's
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             const int o = at + NAUX * 32 * q;
@@ -199,6 +205,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
             if (mlo[q] < m_end) mlo[q] = m_end;
             obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2;
+            const int tm = A.nfull - 1 - th;
+            south[q] = FOLD && tm != th;              // the equator ring of an odd ring count mirrors itself
+            osouth[q] = ((ptrdiff_t)tm - th) * 2;
         }
         for (int p = 0; p < npairs; ++p) {
             const int rs = p & (NRS - 1);
@@ -209,18 +218,23 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 #pragma unroll
             for (int h = 0; h < KS; ++h) {
                 const int m = mtop - KS * p - h;
-                double2 v[NQ];
+                double2 v[NSET][NQ];
 #pragma unroll
-                for (int q = 0; q < NQ; ++q) v[q] = make_double2(0.0, 0.0);
+                for (int e = 0; e < NSET; ++e)
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) v[e][q] = make_double2(0.0, 0.0);
                 bool any = false;
 #pragma unroll
                 for (int ww = 0; ww < NW; ++ww) {
                     if ((actb[ww] >> h) & 1) {
                         any = true;
-                        const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]) + at;
 #pragma unroll
-                        for (int q = 0; q < NQ; ++q)
-                            if (at + NAUX * 32 * q < NOUT) { const double2 t = r[NAUX * 32 * q]; v[q].x += t.x; v[q].y += t.y; }
+                        for (int e = 0; e < NSET; ++e) {
+                            const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][e][0][0]) + at;
+#pragma unroll
+                            for (int q = 0; q < NQ; ++q)
+                                if (at + NAUX * 32 * q < NOUT) { const double2 t = r[NAUX * 32 * q]; v[e][q].x += t.x; v[e][q].y += t.y; }
+                        }
                     }
                 }
                 if (any) {
@@ -229,8 +243,18 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                         if (valid[q] && m >= mlo[q] && !(neg[q] && m == 0)) {
                             const int m_out = (NC == 2) ? (neg[q] ? -m : m) : P.sgn_out * m;
                             const int row = m_out < 0 ? m_out + A.NB : m_out;
-                            double* o = obase[q] + (size_t)row * A.ntp * 2;
-                            red_add_f64(o, v[q].x); red_add_f64(o + 1, v[q].y);
+                            double* o = obase[q] + (size_t)row * A.ldout * 2;
+                            if (FOLD) {
+                                // set 0 = degrees of even l (la is even): E if m is even, O if m is odd
+                                const double2 a = v[0][q], b = v[NSET - 1][q];
+                                red_add_f64(o, a.x + b.x); red_add_f64(o + 1, a.y + b.y);                    // F_m(theta) = E + O
+                                if (south[q]) {
+                                    const double sg = (m & 1) ? -1.0 : 1.0;                                     // F_m(pi - theta) = E - O
+                                    red_add_f64(o + osouth[q], sg * (a.x - b.x)); red_add_f64(o + osouth[q] + 1, sg * (a.y - b.y));
+                                }
+                            } else {
+                                red_add_f64(o, v[0][q].x); red_add_f64(o + 1, v[0][q].y);
+                            }
                         }
                     }
                 }
@@ -282,11 +306,13 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 #pragma unroll
         for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][h][lane + 32 * i] * s;
         if (wact) {
-            double acc[RT][2 * NC];
+            double acc[NSET][RT][2 * NC];
 #pragma unroll
-            for (int i = 0; i < RT; ++i)
+            for (int e = 0; e < NSET; ++e)
 #pragma unroll
-                for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
+                for (int i = 0; i < RT; ++i)
+#pragma unroll
+                    for (int c = 0; c < 2 * NC; ++c) acc[e][i][c] = 0.0;
 #pragma unroll
             for (int j = 0; j < RL; ++j) {
                 const double* r = row + j * ROWD;
@@ -301,17 +327,20 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                 for (int i = 0; i < RT; ++i) {
                     const double e = ca[j * RT + i];
 #pragma unroll
-                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fma(e, cf[c], acc[i][c]);
+                    for (int c = 0; c < 2 * NC; ++c) acc[FOLD ? (j & 1) : 0][i][c] = fma(e, cf[c], acc[FOLD ? (j & 1) : 0][i][c]);
                     cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
                 }
             }
-            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
 #pragma unroll
-            for (int i = 0; i < RT; ++i)
+            for (int e = 0; e < NSET; ++e) {
+                double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][e][0][0]);
 #pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    rd[c * NTH + lane + 32 * i] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
-                }
+                for (int i = 0; i < RT; ++i)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) {
+                        rd[c * NTH + lane + 32 * i] = make_double2(acc[e][i][2 * c], acc[e][i][2 * c + 1]);
+                    }
+            }
             wrote = true;
         } else {                                      // every item of the warp is still below 2^-340: recursion only
 #pragma unroll
@@ -671,12 +700,12 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double* sink)
     if (s == 123.456) sink[0] = s;
 }
 
-template <int RL, int RT, int NW, int NC>
+template <int RL, int RT, int NW, int NC, bool FOLD = false>
 cudaError_t launch_inv(const ThetaArgs& a, cudaStream_t st) {
-    using S = InvSmem<RL, RT, NW, NC>;
+    using S = InvSmem<RL, RT, NW, NC, FOLD>;
     const size_t smem = sizeof(S) + 128;
     dim3 grid((a.Lp / S::TL) * (a.ntp / S::NTH), a.npass);
-    auto k = theta_inverse_kernel<RL, RT, NW, NC>;
+    auto k = theta_inverse_kernel<RL, RT, NW, NC, FOLD>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid, (NW + NAUX) * 32, smem, st>>>(a);
@@ -720,6 +749,8 @@ static bool small_tiles(const ThetaArgs& a, int big) {
 }
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
+    // folded inverse: two partial-sum sets; the two-column (PM) variant fits shared memory with 64 rings per block only
+    if (a.fold0) return mode == 0 ? launch_inv<8, 2, 8, 2, true>(a, st) : launch_inv<8, 4, 8, 1, true>(a, st);
     if (small_tiles(a, 128)) return mode == 0 ? launch_inv<8, 2, 8, 2>(a, st) : launch_inv<8, 2, 8, 1>(a, st);
     return mode == 0 ? launch_inv<8, 4, 8, 2>(a, st) : launch_inv<8, 4, 8, 1>(a, st);
 }

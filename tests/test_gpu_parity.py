@@ -209,3 +209,8 @@ def test_spin0_forward_with_and_without_north_south_fold(api, orc, monkeypatch, 
         P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=real)
         want = orc.s2_forward(L, 0, orc.HEALPIX, f.astype(np.complex128), nside=nside)
     assert rel(P.forward(dev(f)).cpu().numpy(), want) < TOL
+    if sampling == "hp":      # HEALPix rings are symmetric on the inverse side too: F_m(theta) = E + O, F_m(pi - theta) = E - O
+        flm = synth.random_flm(L, 0, seed=3 * L, sigma=synth.SIGMA_RED, real=real)
+        ref = orc.s2_inverse(L, 0, orc.HEALPIX, flm, nside=nside)
+        got = P.inverse(dev(flm)).cpu().numpy()
+        assert rel(got, ref.real if real else ref) < TOL
