@@ -29,8 +29,8 @@ METRIC = "SHT fwd+inv transform pairs per second (MW L=1024 spin-2 fp64, 1 B200)
 UNIT = "transform_pairs/s"
 # algorithmic flop per d-step: recursion 6 + projection 4 per order served
 # dram__bytes_read.sum + dram__bytes_write.sum of the forward theta kernel, per launch, from the ncu --set full captures in
-# profiles/r1_v6_theta_kernels.md; key (L, spin, batch).  Not measurable inside this process: null for other workloads.
-NCU_TRAFFIC_BYTES = {(1024, 2, 1): 164.536e6 + 14.288e6, (2048, 0, 1): 1.588936e9 + 82.18e6, (2048, 0, 16): 51.356830e9 + 13.395911e9}
+# profiles/r1_v7_theta_kernels.md; key (L, spin, batch).  Not measurable inside this process: null for other workloads.
+NCU_TRAFFIC_BYTES = {(1024, 2, 1): 128.008e6 + 11.222e6, (2048, 0, 1): 1.516876e9 + 155.507e6, (2048, 0, 16): 46.314083e9 + 11.453921e9}
 
 
 def peaks():
@@ -231,7 +231,7 @@ def main():
         ach = flops_fwd / (stages["forward_ms"]["hot"] * 1e-3) / 1e12
         roof = {"bound": "alu", "kernel": ("theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>") + " (fused m-recursion + theta contraction, Eq. 25+30)",
                 "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf, "traffic": NCU_TRAFFIC_BYTES.get((L, spin, B)),
-                "traffic_source": "profiles/r1_v6_theta_kernels.md (ncu --set full, bytes per launch)",
+                "traffic_source": "profiles/r1_v7_theta_kernels.md (ncu --set full, bytes per launch)",
                 "peak_kind": "measured in this run by a register-only DFMA chain (sht_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
                 "inverse_kernel": {"achieved": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12,
