@@ -21,7 +21,10 @@
  *       flmn [2N-1][L][2L-1]      (n+N-1, l, m+L-1)
  *     With reality = 1 (spin 0 only) maps are arrays of real doubles of the same shape, and the m < 0 half of
  *     flm is ignored on input / filled with (-1)^m conj(f_{l,-m}) on output.
- *   - dtype: SHT_F64 only in this version (SHT_F32 returns SHT_EUNSUPPORTED).
+ *   - dtype: SHT_F64, or SHT_F32 for spin-0 MW plans of one map (BASELINE config 5; other SHT_F32 requests return
+ *     SHT_EUNSUPPORTED).  With SHT_F32 every public array is interleaved floats (complex64 / float32) and the fused
+ *     recursion + contraction kernels compute in fp32 (Eq. 25 in the paper's own form, windows of 2^48); FFTs and staging
+ *     run in fp64 on internal copies.  Accuracy: max|delta| / max|ref| <= 1e-4 (north_star).
  */
 #ifndef B200SHT_H
 #define B200SHT_H

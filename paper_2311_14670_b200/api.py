@@ -10,7 +10,7 @@ import ctypes as C
 import numpy as np
 import torch
 
-from ._lib import SHT_F64, SHT_HEALPIX, SHT_MW, check, lib
+from ._lib import SHT_F32, SHT_F64, SHT_HEALPIX, SHT_MW, check, lib
 
 MW, HEALPIX = SHT_MW, SHT_HEALPIX
 
@@ -34,21 +34,29 @@ def map_shape(L, sampling=MW, nside=0):
 class Plan:
     """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
 
-    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1):
+    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1, dtype="f64"):
         self._h = C.c_void_p()
         self.L, self.spin, self.sampling, self.nside, self.reality, self.N = L, spin, sampling, nside, bool(reality), N
         self.batch = int(batch)
+        if dtype not in ("f64", "f32"):
+            raise ValueError("dtype must be 'f64' or 'f32'")
+        self.dtype = dtype          # 'f32': fp32 hot kernels and complex64 / float32 arrays (spin 0, MW, batch 1)
+        code = SHT_F32 if dtype == "f32" else SHT_F64
         self.device = torch.device(device)
         L_ = lib()
         with torch.cuda.device(self.device):
             if N is None:
-                check(L_.sht_plan_s2_batch(C.byref(self._h), L, spin, sampling, nside, int(self.reality), SHT_F64, self.batch))
+                check(L_.sht_plan_s2_batch(C.byref(self._h), L, spin, sampling, nside, int(self.reality), code, self.batch))
             else:
-                check(L_.sht_plan_so3(C.byref(self._h), L, N, SHT_F64))
+                check(L_.sht_plan_so3(C.byref(self._h), L, N, code))
             nbytes = L_.sht_plan_workspace_bytes(self._h)
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             check(L_.sht_plan_set_workspace(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes, _stream()))
-        self.map_dtype = torch.float64 if self.reality else torch.complex128
+        self.coef_dtype = torch.complex64 if dtype == "f32" else torch.complex128
+        if dtype == "f32":
+            self.map_dtype = torch.float32 if self.reality else torch.complex64
+        else:
+            self.map_dtype = torch.float64 if self.reality else torch.complex128
         self.coef_shape = (L, 2 * L - 1) if N is None else (2 * N - 1, L, 2 * L - 1)
         self.map_shape = map_shape(L, sampling, nside) if N is None else (2 * N - 1, L, 2 * L - 1)
         if self.batch > 1:            # a batch of maps transformed together: leading [batch] axis on both sides
@@ -65,15 +73,15 @@ class Plan:
 
     # -- transforms (device tensors in, device tensors out) --
     def forward(self, f, out=None):
-        out = torch.empty(self.coef_shape, dtype=torch.complex128, device=self.device) if out is None else out
+        out = torch.empty(self.coef_shape, dtype=self.coef_dtype, device=self.device) if out is None else out
         fn = lib().s2_forward_plan if self.N is None else lib().so3_forward_plan
-        check(fn(self._h, _dev(f, self.map_dtype, self.map_shape, "f"), _dev(out, torch.complex128, self.coef_shape, "flm"), _stream()))
+        check(fn(self._h, _dev(f, self.map_dtype, self.map_shape, "f"), _dev(out, self.coef_dtype, self.coef_shape, "flm"), _stream()))
         return out
 
     def inverse(self, flm, out=None):
         out = torch.empty(self.map_shape, dtype=self.map_dtype, device=self.device) if out is None else out
         fn = lib().s2_inverse_plan if self.N is None else lib().so3_inverse_plan
-        check(fn(self._h, _dev(flm, torch.complex128, self.coef_shape, "flm"), _dev(out, self.map_dtype, self.map_shape, "f"), _stream()))
+        check(fn(self._h, _dev(flm, self.coef_dtype, self.coef_shape, "flm"), _dev(out, self.map_dtype, self.map_shape, "f"), _stream()))
         return out
 
     def ntheta(self, forward):

@@ -80,6 +80,11 @@ struct sht_plan {
     int L = 0, spin = 0, sampling = 0, nside = 0, reality = 0, N = 1;
     int Lp = 0, NB = 0;        // padded L; 2L-1
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
+    bool f32_inner = false;    // set while an fp32 transform runs its fp64-array core
+    int dtype = SHT_F64;       // SHT_F32: fp32 hot kernels (theta_f32.cu) and fp32 public arrays; staging and FFTs stay fp64
+    float2* ab32 = nullptr;    // fp32: [L][Lp] recursion coefficients
+    float *st32_inv = nullptr, *st32_fwd = nullptr; uint16_t *k16_inv = nullptr, *k16_fwd = nullptr;   // fp32 start values
+    double2 *io_a = nullptr, *io_b = nullptr;   // fp32: fp64 copies of the public arrays
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
@@ -266,6 +271,12 @@ void layout(sht_plan* P, char* base) {
     P->H = B.take<double2>(P->H_slab * P->nslab);
     if (P->reality && P->sampling == SHT_MW) P->cplx = B.take<double2>((size_t)L * NB * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
+    if (P->dtype == SHT_F32) {
+        P->ab32 = B.take<float2>((size_t)L * Lp);
+        P->st32_inv = B.take<float>((size_t)Lp * P->inv.ntp); P->k16_inv = B.take<uint16_t>((size_t)Lp * P->inv.ntp);
+        P->st32_fwd = B.take<float>((size_t)Lp * P->fwd.ntp); P->k16_fwd = B.take<uint16_t>((size_t)Lp * P->fwd.ntp);
+        P->io_a = B.take<double2>((size_t)L * NB); P->io_b = B.take<double2>((size_t)L * NB);
+    }
     P->fft_work = B.take<char>(P->fft_work_bytes);
     // route every pass to its slab's output array
     for (auto& ph : P->pinv) ph.p.out = P->F ? P->F + P->F_slab * ph.p.slab : nullptr;
@@ -533,6 +544,22 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
             for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F + P->F_slab * s, st));
         return SHT_OK;
     }
+    if (P->dtype == SHT_F32) {
+        auto& ph = P->pinv[0];
+        const int NC = ph.mode == 0 ? 2 : 1;
+        CK(st_prep_inverse_f32(L, P->Lp, NC, coef, P->scale_inv, reinterpret_cast<float2*>(const_cast<double*>(ph.p.in)), st));
+        CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab, st));
+        stage(P, CAT_HOT, st);
+        F32Args a{};
+        a.L = L; a.Lp = P->Lp; a.nth = P->inv.nth; a.ntp = P->inv.ntp; a.NB = P->NB; a.ldout = P->F_ld;
+        a.ab = P->ab32; a.lam = ph.p.lam; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
+        a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F;
+        CK(launch_theta_f32(a, false, NC, st));
+        CK(st_pole_inverse(L, 0, coef, P->scale_inv, P->F + P->inv.nth, st));
+        stage(P, CAT_STAGE, st);
+        if (P->reality) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F, st));
+        return SHT_OK;
+    }
     for (auto& ph : P->pinv)
         CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->NB,
                            P->scale_inv, P->ctab, P->sgtab, P->sgstride,
@@ -593,6 +620,19 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
             for (int s = 0; s < P->nslab; ++s)
                 CK(st_pole_forward(L, P->Lp, P->slab_n[s], P->NB, ldu, P->fwd.nth, P->fwd.wq, U + U_slab * s, P->H + P->H_slab * s, st));
         }
+        return SHT_OK;
+    }
+    if (P->dtype == SHT_F32) {
+        auto& ph = P->pfwd[0];
+        const int NC = ph.mode == 0 ? 2 : 1;
+        CK(st_weight_split_f32(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, reinterpret_cast<float2*>(const_cast<double*>(ph.p.in)), st));
+        CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab, st));
+        stage(P, CAT_HOT, st);
+        F32Args a{};
+        a.L = L; a.Lp = P->Lp; a.nth = P->fwd.nth; a.ntp = P->fwd.ntp; a.NB = P->NB; a.ldout = 0;
+        a.ab = P->ab32; a.lam = ph.p.lam; a.st_val = P->st32_fwd; a.st_k = P->k16_fwd;
+        a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->H;
+        CK(launch_theta_f32(a, true, NC, st));
         return SHT_OK;
     }
     for (auto& ph : P->pfwd) {
@@ -715,9 +755,12 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
     if (batch > 1 && sampling != SHT_MW) return SHT_EUNSUPPORTED;
     if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || (sampling != SHT_MW && sampling != SHT_HEALPIX)) return SHT_EINVAL;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
-    if (dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
+    // fp32 variant (BASELINE config 5): spin 0, MW sampling, one map
+    if (dtype == SHT_F32 && (spin != 0 || sampling != SHT_MW || batch != 1)) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
+    P->dtype = dtype;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, L); }
@@ -728,6 +771,7 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
         const long tiles = (long)(rup(L, 128) / SHT_TQ) * (long)(rup((size_t)(P->fwd.nth + 1) / 2, 128) / 128) * (batch > 1 ? 4 : 1);
         bool on = tiles >= 2 * 148;
         if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
+        if (dtype == SHT_F32) on = false;          // the fp32 kernels recurse every ring
         if (on) { P->fold0 = 1; north_only(P->fwd); }
         // the inverse rings of HEALPix are symmetric too (the MW rings (2t+1)pi/(2L-1) are not)
         if (on && sampling == SHT_HEALPIX && batch == 1) { P->fold0i = 1; north_only(P->inv); }
@@ -797,6 +841,11 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     }
     { std::vector<double> ones(P->fwd.ntp, 1.0); CS(up(ones, P->unit_wq, st)); }
     CS(upload_passes(P, st));
+    if (P->dtype == SHT_F32) {
+        CK(st_ab32(L, Lp, P->ab32, st));
+        CK(st_start32((size_t)Lp * P->inv.ntp, P->inv.start[0].val, P->inv.start[0].k, P->st32_inv, P->k16_inv, st));
+        CK(st_start32((size_t)Lp * P->fwd.ntp, P->fwd.start[0].val, P->fwd.start[0].k, P->st32_fwd, P->k16_fwd, st));
+    }
     if (P->sampling == SHT_MW) {
         for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));
         if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
@@ -853,7 +902,7 @@ sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
 sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
-    if (P->batch > 1) return SHT_EUNSUPPORTED;
+    if (P->batch > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
@@ -865,7 +914,7 @@ sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_str
 sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_stream stream) {
     CS(check_ready(P));
     if (!Wm || !flm || P->kind != 0) return SHT_EINVAL;
-    if (P->batch > 1) return SHT_EUNSUPPORTED;
+    if (P->batch > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     P->ev_n = 0;
     // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
@@ -889,6 +938,17 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB;
+    if (P->dtype == SHT_F32 && !P->f32_inner) {      // fp32 public arrays: fp64 copies around the core (staging and FFTs are fp64)
+        const size_t nc = (size_t)L * NB;
+        CK(st_f32_to_f64(2 * nc, (const float*)flm, (double*)P->io_a, st));
+        P->f32_inner = true;
+        sht_status s = s2_inverse_plan(P, P->io_a, P->io_b, stream);
+        P->f32_inner = false;
+        if (s != SHT_OK) return s;
+        CK(st_f64_to_f32(P->reality ? nc : 2 * nc, (const double*)P->io_b, (float*)f, st));
+        stage(P, CAT_STAGE, st);
+        return SHT_OK;
+    }
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
     if (P->sampling == SHT_HEALPIX) return healpix_synthesis(P, f, st);
@@ -906,6 +966,17 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB;
+    if (P->dtype == SHT_F32 && !P->f32_inner) {
+        const size_t nc = (size_t)L * NB;
+        CK(st_f32_to_f64(P->reality ? nc : 2 * nc, (const float*)f, (double*)P->io_a, st));
+        P->f32_inner = true;
+        sht_status s = s2_forward_plan(P, P->io_a, P->io_b, stream);
+        P->f32_inner = false;
+        if (s != SHT_OK) return s;
+        CK(st_f64_to_f32(2 * nc, (const double*)P->io_b, (float*)flm, st));
+        stage(P, CAT_STAGE, st);
+        return SHT_OK;
+    }
     P->ev_n = 0;
     if (P->sampling == SHT_HEALPIX) {
         CS(healpix_analysis(P, f, st));

@@ -73,6 +73,18 @@ struct MmaArgs {
 };
 cudaError_t launch_theta_mma(const MmaArgs& a, bool forward, cudaStream_t st);
 
+// ---- fp32 variant (theta_f32.cu): n = 0, MW sampling, one map ------------------------------------------------------------
+struct F32Args {
+    int L, Lp, nth, ntp, NB, ldout;
+    const float2* ab;         // [m][Lp] {A_m(l) = a_{m-1}(l), B_m(l) = a_{m-1}(l)/a_m(l)} (Eq. 25-26), rows m = 0..L-1 (row 0 unused: zeros)
+    const double* lam;        // lambda table of the n = 0 pass, row m + 1 (internal layout of ThetaPass::lam with m_end = 0)
+    const float* st_val;      // [Lp][ntp] Eq. 27 start values, windowed: true value = st_val * 2^(-48 st_k)
+    const uint16_t* st_k;
+    const float2* in;         // inverse: G32[m][Lp][NC] = scale(l) f_lm; forward: W32[m][ntp][NC] = q(theta) F_m(theta)
+    double2* out;             // inverse: F[row][ldout]; forward: H[m + L - 1][Lp]   (fp64 accumulators shared with the fp64 staging)
+};
+cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st);
+
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st);
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st);

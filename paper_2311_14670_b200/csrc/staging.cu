@@ -511,6 +511,84 @@ __global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, i
     }
 }
 
+// ---- fp32 variant (theta_f32.cu) ----------------------------------------------------------------------------------------
+// recursion coefficients of Eq. 25-26 in the paper's own form, fp32: AB[m][l] = {a_{m-1}(l), a_{m-1}(l)/a_m(l)}, a_m = 2/sqrt((l-m)(l+m+1))
+__global__ void k_ab32(int L, int Lp, float2* __restrict__ AB) {
+    int l = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (l >= Lp) return;
+    float2 v = make_float2(0.f, 0.f);
+    if (l < L && m >= 1 && l >= m) {
+        const double p = (double)(l - m + 1) * (double)(l + m);
+        v.x = (float)(2.0 / sqrt(p));
+        v.y = (float)sqrt((double)(l - m) * (double)(l + m + 1) / p);
+    }
+    AB[(size_t)m * Lp + l] = v;
+}
+// fp64 windowed start values (stride 2^480, internal.h) -> fp32 windowed ones (stride 2^48, top 2^-64)
+__global__ void k_start32(size_t n, const double* __restrict__ v64, const uint8_t* __restrict__ k64, float* __restrict__ v32,
+                          uint16_t* __restrict__ k16) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v = v64[i];
+    float o = 0.f; int k = 0;
+    if (v != 0.0) {
+        int ex; (void)frexp(v, &ex);                       // |v| = f 2^ex, f in [0.5, 1)
+        const long e = (long)ex - (long)SHT_SWIN * k64[i];  // true value = f 2^e
+        if (e > -64) k = 0; else k = (int)((-64 - e) / 48 + 1);
+        if (k <= 65535) o = (float)ldexp(v, (int)(48L * k - (long)SHT_SWIN * k64[i]));
+        else k = 0;
+    }
+    v32[i] = o; k16[i] = (uint16_t)k;
+}
+// inverse operands: G32[m][Lp][NC] = scale(l) f_{l,+m} and, for NC = 2, (-1)^m scale(l) f_{l,-m} (32 x 32 transpose, coef is l-major)
+__global__ void k_prep_inverse_f32(int L, int Lp, int NC, const double2* __restrict__ coef, const double* __restrict__ scale,
+                                   float2* __restrict__ G) {
+    __shared__ double2 tile[2][32][33];
+    const int NB = 2 * L - 1, l0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    for (int c = 0; c < NC; ++c)
+        for (int q = threadIdx.y; q < 32; q += blockDim.y) {
+            const int l = l0 + q, m = m0 + threadIdx.x;
+            double2 v = make_double2(0.0, 0.0);
+            if (l < L && m < L && l >= m && !(c == 1 && m == 0)) v = coef[(size_t)l * NB + (c == 1 ? -m : m) + L - 1];
+            tile[c][q][threadIdx.x] = v;
+        }
+    __syncthreads();
+    for (int q = threadIdx.y; q < 32; q += blockDim.y) {
+        const int m = m0 + q, l = l0 + threadIdx.x;
+        if (m >= L || l >= Lp) continue;
+        const double sc = l < L ? scale[l] : 0.0;
+        for (int c = 0; c < NC; ++c) {
+            const double sg = (c == 1 && (m & 1)) ? -sc : sc;
+            const double2 x = tile[c][threadIdx.x][q];
+            G[((size_t)m * Lp + l) * NC + c] = make_float2((float)(sg * x.x), (float)(sg * x.y));
+        }
+    }
+}
+// forward operands: W32[m][ntp][NC] = q(theta) F_{+m}(theta) and, for NC = 2, (-1)^m q(theta) F_{-m}(theta)
+__global__ void k_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* __restrict__ wq,
+                                   const double2* __restrict__ U, float2* __restrict__ W) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (th >= ntp) return;
+    for (int c = 0; c < NC; ++c) {
+        float2 v = make_float2(0.f, 0.f);
+        if (th < nth && !(c == 1 && m == 0)) {
+            const int m_out = c == 1 ? -m : m;
+            const double s = (c == 1 && (m & 1)) ? -wq[th] : wq[th];
+            const double2 x = U[(size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + th];
+            v = make_float2((float)(s * x.x), (float)(s * x.y));
+        }
+        W[((size_t)m * ntp + th) * NC + c] = v;
+    }
+}
+__global__ void k_c64_to_c128(size_t n, const float* __restrict__ in, double* __restrict__ out) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (double)in[i];
+}
+__global__ void k_c128_to_c64(size_t n, const double* __restrict__ in, float* __restrict__ out) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (float)in[i];
+}
+
 inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 }  // namespace
@@ -642,5 +720,31 @@ cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab
                                         cudaStream_t st) {
     dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
     k_weight_split_batch_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, nfull, NC, B, m_end, wq, lam, U, Wb, cg_stride);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st) {
+    k_ab32<<<dim3(cdiv(Lp, 128), L), 128, 0, st>>>(L, Lp, AB);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v32, uint16_t* k16, cudaStream_t st) {
+    k_start32<<<cdiv(n, 256), 256, 0, st>>>(n, v64, k64, v32, k16);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st) {
+    dim3 grid(cdiv(Lp, 32), cdiv(L, 32)), block(32, 8);
+    k_prep_inverse_f32<<<grid, block, 0, st>>>(L, Lp, NC, coef, scale, G);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
+                                cudaStream_t st) {
+    k_weight_split_f32<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, wq, U, W);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st) {
+    k_c64_to_c128<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t st) {
+    k_c128_to_c64<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
     LAUNCHED(); return cudaSuccess;
 }

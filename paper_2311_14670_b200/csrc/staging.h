@@ -43,6 +43,15 @@ cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab
 cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st);
 
+// fp32 variant (theta_f32.cu): tables, operand preparation, precision conversion of the public arrays
+cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st);
+cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v32, uint16_t* k16, cudaStream_t st);
+cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st);
+cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
+                                cudaStream_t st);
+cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st);
+cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t st);
+
 // HEALPix ring Fourier staging (healpix.cu)
 void hp_ring_host(int nside, int i, int* nphi, int* shifted, long long* off);
 cudaError_t st_hp_chirp(int nside, int M, double2* BF, cudaStream_t st);

@@ -1,0 +1,262 @@
+// theta_f32.cu -- the fp32 variant of the hot path (BASELINE config 5: "fp64 and fp32"): Wigner-d recursion in m (Eq. 25-27,
+// PAPER.md:225-234) fused with the contractions of Eq. 30 / Eq. 33, with iterates, coefficients and partial sums in fp32.
+//
+// The fp64 kernels run the recursion in the "e-form" (internal.h), whose factor c_m(l) spans up to 2^250 inside a 64-degree
+// quantum -- outside the fp32 exponent range.  Here the recursion is the paper's own form on the true d-values,
+//     d_{m-1} = (lambda_m A_m(l)) d_m - B_m(l) d_{m+1},   A_m = a_{m-1} = 2/sqrt((l-m+1)(l+m)),   B_m = a_{m-1}/a_m,
+// (3 FP32 instructions per step) with fp32 tables A, B (plan time) and the renormalisation of Sec. 3.4 as
+// power-of-two windows sized for fp32: true value = stored * 2^(-48 k); a stored value with k > 0 stays below 2^-43 (it grows by
+// less than 2^21 per step and is checked every step against 2^-64), which is below fp32 resolution of the sums, so no masking.
+// Scope: second index n = 0 (spin-0 plans), MW sampling, one map.  Everything around the two kernels (FFTs, staging, the pole
+// ring) is the fp64 code; the kernels read fp32 operand tables and add their block sums into the fp64 F / H arrays.
+#include "internal.h"
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace {
+
+constexpr int FW = 48;                 // window stride (bits)
+constexpr int FTOP = -64;              // a stored value with k > 0 is rescaled once it exceeds 2^FTOP
+constexpr int TLF = 64, NTF = 128;     // block tile: degrees x rings
+constexpr int NWF = 8;                 // warps per block
+
+__device__ __forceinline__ float pow2f(int e) { return __int_as_float((127 + e) << 23); }
+__device__ __forceinline__ void red_add_f64(double* gptr, double v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gptr), "d"(v) : "memory");
+}
+
+// window counters of 32 items, 16 bits each
+struct KPackF {
+    uint32_t w[16];
+    __device__ __forceinline__ void fill(uint32_t v) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) w[i] = v;
+    }
+    __device__ __forceinline__ void set(int idx, uint32_t k) {
+        const int sh = (idx & 1) * 16;
+        w[idx >> 1] = (w[idx >> 1] & ~(0xffffu << sh)) | (k << sh);
+    }
+    __device__ __forceinline__ uint32_t get(int idx) const { return (w[idx >> 1] >> ((idx & 1) * 16)) & 0xffffu; }
+    __device__ __forceinline__ void dec(int idx) { w[idx >> 1] -= 1u << ((idx & 1) * 16); }
+    __device__ __forceinline__ bool any_nonzero() const {
+        uint32_t o = 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) o |= w[i];
+        return o != 0;
+    }
+};
+template <int NI>
+__device__ __forceinline__ void window_check_f(float (&cur)[NI], float (&prev)[NI], KPackF& kp) {
+    const float s = pow2f(-FW), top = pow2f(FTOP);
+#pragma unroll
+    for (int q = 0; q < NI; ++q) {
+        if (fabsf(cur[q]) > top && kp.get(q) != 0u) { cur[q] *= s; prev[q] *= s; kp.dec(q); }
+    }
+}
+
+// =============================================================================================================
+// inverse, Eq. 33:  F[row(+-m)][theta] += sum_l G[m][l][c] d^l_{m,0}(theta)
+// warp w: degrees l0 + 8 w + j (j < 8); lane: rings th0 + lane + 32 i (i < 4)
+// =============================================================================================================
+template <int NC>
+__global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
+    constexpr int RL = 8, RT = 4, NI = RL * RT;
+    __shared__ float2 s_ab[2][TLF];
+    __shared__ float2 s_g[2][TLF * NC];
+    __shared__ float s_lam[2][NTF];
+    __shared__ float2 s_part[NWF][NC][NTF];
+    const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
+    const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;      // heavy tiles first
+    const int l0 = lt * TLF, th0 = tt * NTF;
+    if (l0 >= A.L || th0 >= A.nth) return;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int mtop = min(l0 + TLF - 1, A.L - 1);
+    const int la = l0 + w * RL;
+
+    auto load_ops = [&](int m, int buf) {           // operand rows of step m: one element per thread
+        if (tid < TLF) s_ab[buf][tid] = A.ab[(size_t)m * A.Lp + l0 + tid];
+        if (tid < TLF * NC) s_g[buf][tid] = A.in[((size_t)m * A.Lp + l0) * NC + tid];
+        if (tid >= 128 && tid < 128 + NTF) s_lam[buf][tid - 128] = (float)A.lam[(size_t)(m + 1) * A.ntp + th0 + tid - 128];
+    };
+    float cur[NI], prev[NI];
+    KPackF kp;
+    kp.fill(0u);
+#pragma unroll
+    for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
+    load_ops(mtop, 0);
+    __syncthreads();
+
+    // one step: project d_m, then advance to d_{m-1}.  `ca` holds d_m, `cb` holds d_{m+1} on entry and d_{m-1} on exit.
+    auto step = [&](const int m, const int buf, float (&ca)[NI], float (&cb)[NI]) {
+        if (m > 0) load_ops(m - 1, buf ^ 1);
+        bool mine = m <= la + RL - 1 && la < A.L;   // this warp has started degrees
+        if (mine && m >= la) {                      // the degree l == m starts (warp-uniform)
+#pragma unroll
+            for (int j = 0; j < RL; ++j)
+                if (m == la + j) {
+#pragma unroll
+                    for (int i = 0; i < RT; ++i) {
+                        const size_t o = (size_t)m * A.ntp + th0 + lane + 32 * i;
+                        ca[j * RT + i] = A.st_val[o]; cb[j * RT + i] = 0.f;
+                        kp.set(j * RT + i, A.st_k[o]);
+                    }
+                }
+        }
+        float acc[RT][2 * NC];
+#pragma unroll
+        for (int i = 0; i < RT; ++i)
+#pragma unroll
+            for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.f;
+        if (mine) {
+            float lam[RT];
+#pragma unroll
+            for (int i = 0; i < RT; ++i) lam[i] = s_lam[buf][lane + 32 * i];
+#pragma unroll
+            for (int j = 0; j < RL; ++j) {
+                const float2 ab = s_ab[buf][w * RL + j];
+                float cf[2 * NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) { const float2 t = s_g[buf][(w * RL + j) * NC + c]; cf[2 * c] = t.x; cf[2 * c + 1] = t.y; }
+#pragma unroll
+                for (int i = 0; i < RT; ++i) {
+                    const float e = ca[j * RT + i];
+#pragma unroll
+                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fmaf(e, cf[c], acc[i][c]);
+                    cb[j * RT + i] = fmaf(lam[i] * ab.x, e, -(ab.y * cb[j * RT + i]));
+                }
+            }
+            if (kp.any_nonzero()) window_check_f<NI>(cb, ca, kp);
+        }
+#pragma unroll
+        for (int i = 0; i < RT; ++i)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) s_part[w][c][lane + 32 * i] = make_float2(acc[i][2 * c], acc[i][2 * c + 1]);
+        __syncthreads();
+        for (int o = tid; o < NC * NTF; o += NWF * 32) {
+            const int c = o / NTF, t = o % NTF, th = th0 + t;
+            double sx = 0.0, sy = 0.0;
+#pragma unroll
+            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += (double)v.x; sy += (double)v.y; }
+            if (th < A.nth && !(c == 1 && m == 0)) {
+                const int m_out = c == 1 ? -m : m;
+                const int row = m_out < 0 ? m_out + A.NB : m_out;
+                double* op = reinterpret_cast<double*>(A.out) + ((size_t)row * A.ldout + th) * 2;
+                red_add_f64(op, sx); red_add_f64(op + 1, sy);
+            }
+        }
+        __syncthreads();
+    };
+    for (int m = mtop; m >= 0; m -= 2) {
+        step(m, (mtop - m) & 1, cur, prev);
+        if (m - 1 >= 0) step(m - 1, (mtop - m + 1) & 1, prev, cur);
+    }
+}
+
+// =============================================================================================================
+// forward, Eq. 30:  H[+-m + L-1][l] += sum_theta W[m][theta][c] d^l_{m,0}(theta)
+// warp w: rings th0 + 16 w + i (i < 16); lane: degrees l0 + lane + 32 r (r < 2)
+// =============================================================================================================
+template <int NC>
+__global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
+    constexpr int RL = 2, RT = 16, NI = RL * RT;
+    __shared__ float2 s_ab[2][TLF];
+    __shared__ float2 s_w[2][NTF * NC];
+    __shared__ float s_lam[2][NTF];
+    __shared__ float2 s_part[NWF][NC][TLF];
+    const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
+    const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
+    const int l0 = lt * TLF, th0 = tt * NTF;
+    if (l0 >= A.L || th0 >= A.nth) return;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int mtop = min(l0 + TLF - 1, A.L - 1);
+
+    auto load_ops = [&](int m, int buf) {
+        if (tid < TLF) s_ab[buf][tid] = A.ab[(size_t)m * A.Lp + l0 + tid];
+        for (int o = tid; o < NTF * NC; o += NWF * 32) s_w[buf][o] = A.in[((size_t)m * A.ntp + th0) * NC + o];
+        if (tid >= 128 && tid < 128 + NTF) s_lam[buf][tid - 128] = (float)A.lam[(size_t)(m + 1) * A.ntp + th0 + tid - 128];
+    };
+    float cur[NI], prev[NI];
+    KPackF kp;
+    kp.fill(0u);
+#pragma unroll
+    for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
+    int lr[RL];
+#pragma unroll
+    for (int r = 0; r < RL; ++r) lr[r] = l0 + lane + 32 * r;
+    load_ops(mtop, 0);
+    __syncthreads();
+
+    auto step = [&](const int m, const int buf, float (&ca)[NI], float (&cb)[NI]) {
+        if (m > 0) load_ops(m - 1, buf ^ 1);
+#pragma unroll
+        for (int r = 0; r < RL; ++r)
+            if (m == lr[r] && lr[r] < A.L) {        // this lane's degree starts
+#pragma unroll
+                for (int i = 0; i < RT; ++i) {
+                    const size_t o = (size_t)m * A.ntp + th0 + w * RT + i;
+                    ca[r * RT + i] = A.st_val[o]; cb[r * RT + i] = 0.f;
+                    kp.set(r * RT + i, A.st_k[o]);
+                }
+            }
+        float acc[RL][2 * NC];
+#pragma unroll
+        for (int r = 0; r < RL; ++r)
+#pragma unroll
+            for (int c = 0; c < 2 * NC; ++c) acc[r][c] = 0.f;
+        float2 ab[RL];
+#pragma unroll
+        for (int r = 0; r < RL; ++r) ab[r] = s_ab[buf][lane + 32 * r];
+#pragma unroll
+        for (int i = 0; i < RT; ++i) {
+            const float lam = s_lam[buf][w * RT + i];
+            float wv[2 * NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) { const float2 t = s_w[buf][(w * RT + i) * NC + c]; wv[2 * c] = t.x; wv[2 * c + 1] = t.y; }
+#pragma unroll
+            for (int r = 0; r < RL; ++r) {
+                const float e = ca[r * RT + i];
+#pragma unroll
+                for (int c = 0; c < 2 * NC; ++c) acc[r][c] = fmaf(e, wv[c], acc[r][c]);
+                cb[r * RT + i] = fmaf(lam * ab[r].x, e, -(ab[r].y * cb[r * RT + i]));
+            }
+        }
+        if (kp.any_nonzero()) window_check_f<NI>(cb, ca, kp);
+#pragma unroll
+        for (int r = 0; r < RL; ++r)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) s_part[w][c][lane + 32 * r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
+        __syncthreads();
+        for (int o = tid; o < NC * TLF; o += NWF * 32) {
+            const int c = o / TLF, t = o % TLF, l = l0 + t;
+            double sx = 0.0, sy = 0.0;
+#pragma unroll
+            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += (double)v.x; sy += (double)v.y; }
+            if (l < A.L && l >= m && !(c == 1 && m == 0)) {
+                const int m_out = c == 1 ? -m : m;
+                double* op = reinterpret_cast<double*>(A.out) + ((size_t)(m_out + A.L - 1) * A.Lp + l) * 2;
+                red_add_f64(op, sx); red_add_f64(op + 1, sy);
+            }
+        }
+        __syncthreads();
+    };
+    for (int m = mtop; m >= 0; m -= 2) {
+        step(m, (mtop - m) & 1, cur, prev);
+        if (m - 1 >= 0) step(m - 1, (mtop - m + 1) & 1, prev, cur);
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st) {
+    dim3 grid((a.Lp / TLF) * (a.ntp / NTF));
+    if (forward) {
+        if (NC == 2) theta_forward_f32<2><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_forward_f32<1><<<grid, NWF * 32, 0, st>>>(a);
+    } else {
+        if (NC == 2) theta_inverse_f32<2><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_inverse_f32<1><<<grid, NWF * 32, 0, st>>>(a);
+    }
+    count_launch();
+    return cudaGetLastError();
+}

@@ -1,0 +1,75 @@
+"""GPU parity of the fp32 variant (BASELINE.json configs[4]: "fp64 and fp32"): spin-0 MW plans whose fused recursion +
+contraction kernels compute in fp32 (csrc/theta_f32.cu).  Tolerance from north_star: max|delta| / max|ref| <= 1e-4, both sides
+deciding nothing in floating point (linear maps), against the fp64/long-double CPU oracle on the same seeded inputs."""
+import numpy as np
+import pytest
+
+from paper_2311_14670_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+TOL32 = 1e-4
+
+
+def rel(a, b, scale=None):
+    return float(np.abs(a - b).max() / (np.abs(b).max() if scale is None else scale))
+
+
+@pytest.fixture(scope="module")
+def api():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_14670_b200 import api as A
+    return A
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.parametrize("L,real", [(1, False), (2, False), (8, False), (33, False), (64, False), (130, False), (200, True), (257, False), (512, False)])
+def test_f32_inverse_forward_vs_oracle(api, orc, L, real):
+    flm = synth.random_flm(L, 0, seed=11 * L, sigma=synth.SIGMA_RED, real=real)
+    P = api.Plan(L, 0, reality=real, dtype="f32")
+    f = P.inverse(dev(flm.astype(np.complex64))).cpu().numpy()
+    assert f.dtype == (np.float32 if real else np.complex64)
+    f_ref = orc.s2_inverse(L, 0, orc.MW, flm)
+    f_ref = f_ref.real if real else f_ref
+    assert rel(f, f_ref) < TOL32
+    back = P.forward(dev(f_ref.astype(f.dtype))).cpu().numpy()
+    assert back.dtype == np.complex64
+    assert rel(back, flm) < TOL32                                 # sampling theorem (pin 6), at fp32 accuracy
+    g = synth.random_map((L, 2 * L - 1), seed=L, real=real, mw_pole_spin=0)
+    got = P.forward(dev(g.astype(f.dtype))).cpu().numpy()
+    assert rel(got, orc.s2_forward(L, 0, orc.MW, g.astype(np.complex128))) < TOL32
+    el = np.arange(L)[:, None]
+    m = np.arange(-(L - 1), L)[None, :]
+    assert np.all(back[np.abs(m) > el] == 0)
+
+
+def test_f32_unsupported_requests_are_refused(api):
+    from paper_2311_14670_b200._lib import ShtError
+    for kw in (dict(spin=2), dict(sampling=api.HEALPIX, nside=4), dict(batch=4), dict(N=3)):
+        with pytest.raises(ShtError):
+            api.Plan(16, dtype="f32", **kw)
+
+
+def test_f32_config5a_scale_L2048_sampled(api, orc):
+    """fp32 at a size with deep underflow of the start values (2^-9000 at the first rings): sampled rings / orders vs the oracle."""
+    L = 2048
+    flm = synth.random_flm(L, 0, seed=4, sigma=synth.SIGMA_RED)
+    P = api.Plan(L, 0, dtype="f32")
+    f = P.inverse(dev(flm.astype(np.complex64))).cpu().numpy()
+    rings = np.array([0, 1, 2, 1000, 2046, 2047])
+    rows = orc.s2_inverse_rings(L, 0, orc.MW, flm, rings)
+    scale = max(np.abs(r).max() for r in rows)
+    for r, row in zip(rings, rows):
+        assert rel(f[r], row, scale) < TOL32, r
+    back = P.forward(dev(f)).cpu().numpy()
+    assert rel(back, flm) < 2 * TOL32                             # two fp32 transforms in a row
+    g = synth.random_map((L, 2 * L - 1), seed=15, mw_pole_spin=0)
+    got = P.forward(dev(g.astype(np.complex64))).cpu().numpy()
+    ms = np.array([-(L - 1), -1, 0, 1, 2, 1024, L - 1])
+    want = orc.s2_forward_columns(L, 0, orc.MW, g, ms)
+    sc = np.abs(want).max()
+    for m, col in zip(ms, want):
+        assert rel(got[:, m + L - 1], col, sc) < TOL32, m
