@@ -625,11 +625,13 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     if (P->dtype == SHT_F32) {
         auto& ph = P->pfwd[0];
         const int NC = ph.mode == 0 ? 2 : 1;
-        CK(st_weight_split_f32(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, reinterpret_cast<float2*>(const_cast<double*>(ph.p.in)), st));
+        float2* W32 = reinterpret_cast<float2*>(const_cast<double*>(ph.p.in));
+        if (P->fold0) CK(st_weight_split_f32_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, P->fwd.wq, U, W32, st));
+        else CK(st_weight_split_f32(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, W32, st));
         CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab, st));
         stage(P, CAT_HOT, st);
         F32Args a{};
-        a.L = L; a.Lp = P->Lp; a.nth = P->fwd.nth; a.ntp = P->fwd.ntp; a.NB = P->NB; a.ldout = 0;
+        a.L = L; a.Lp = P->Lp; a.nth = P->fwd.nth; a.ntp = P->fwd.ntp; a.NB = P->NB; a.ldout = 0; a.fold0 = P->fold0;
         a.ab = P->ab32; a.lam = ph.p.lam; a.st_val = P->st32_fwd; a.st_k = P->k16_fwd;
         a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->H;
         CK(launch_theta_f32(a, true, NC, st));
@@ -771,7 +773,6 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
         const long tiles = (long)(rup(L, 128) / SHT_TQ) * (long)(rup((size_t)(P->fwd.nth + 1) / 2, 128) / 128) * (batch > 1 ? 4 : 1);
         bool on = tiles >= 2 * 148;
         if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
-        if (dtype == SHT_F32) on = false;          // the fp32 kernels recurse every ring
         if (on) { P->fold0 = 1; north_only(P->fwd); }
         // the inverse rings of HEALPix are symmetric too (the MW rings (2t+1)pi/(2L-1) are not)
         if (on && sampling == SHT_HEALPIX && batch == 1) { P->fold0i = 1; north_only(P->inv); }

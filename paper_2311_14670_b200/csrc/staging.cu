@@ -580,6 +580,27 @@ __global__ void k_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, 
         W[((size_t)m * ntp + th) * NC + c] = v;
     }
 }
+// the same for the north-south fold: W32[m][ntp north][2][NC], set 0 = E = q (F(theta) + F(pi - theta)), set 1 = O = q (F(theta) - F(pi - theta))
+__global__ void k_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* __restrict__ wq,
+                                         const double2* __restrict__ U, float2* __restrict__ W) {
+    int th = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (th >= ntp) return;
+    for (int c = 0; c < NC; ++c) {
+        float2 e = make_float2(0.f, 0.f), o = make_float2(0.f, 0.f);
+        if (th < nth && !(c == 1 && m == 0)) {
+            const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
+            const double s = (c == 1 && (m & 1)) ? -wq[th] : wq[th];
+            const double2* row = U + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
+            const double2 a = row[th];
+            double2 b = make_double2(0.0, 0.0);
+            if (tm != th) b = row[tm];
+            e = make_float2((float)(s * (a.x + b.x)), (float)(s * (a.y + b.y)));
+            if (tm != th) o = make_float2((float)(s * (a.x - b.x)), (float)(s * (a.y - b.y)));
+        }
+        float2* w = W + ((size_t)m * ntp + th) * 2 * NC;
+        w[c] = e; w[NC + c] = o;
+    }
+}
 __global__ void k_c64_to_c128(size_t n, const float* __restrict__ in, double* __restrict__ out) {
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) out[i] = (double)in[i];
@@ -746,5 +767,10 @@ cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t s
 }
 cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t st) {
     k_c128_to_c64<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
+                                      float2* W, cudaStream_t st) {
+    k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, wq, U, W);
     LAUNCHED(); return cudaSuccess;
 }

@@ -49,6 +49,8 @@ cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v
 cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st);
 cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
                                 cudaStream_t st);
+cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
+                                      float2* W, cudaStream_t st);
 cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st);
 cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t st);
 

@@ -135,14 +135,14 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
         __syncthreads();
         for (int o = tid; o < NC * NTF; o += NWF * 32) {
             const int c = o / NTF, t = o % NTF, th = th0 + t;
-            double sx = 0.0, sy = 0.0;
+            float sx = 0.f, sy = 0.f;
 #pragma unroll
-            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += (double)v.x; sy += (double)v.y; }
+            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += v.x; sy += v.y; }
             if (th < A.nth && !(c == 1 && m == 0)) {
                 const int m_out = c == 1 ? -m : m;
                 const int row = m_out < 0 ? m_out + A.NB : m_out;
                 double* op = reinterpret_cast<double*>(A.out) + ((size_t)row * A.ldout + th) * 2;
-                red_add_f64(op, sx); red_add_f64(op + 1, sy);
+                red_add_f64(op, (double)sx); red_add_f64(op + 1, (double)sy);
             }
         }
         __syncthreads();
@@ -155,13 +155,15 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
 
 // =============================================================================================================
 // forward, Eq. 30:  H[+-m + L-1][l] += sum_theta W[m][theta][c] d^l_{m,0}(theta)
-// warp w: rings th0 + 16 w + i (i < 16); lane: degrees l0 + lane + 32 r (r < 2)
+// warp w: rings th0 + 16 w + i (i < 16); lane: degrees l0 + 2 lane + r (r < 2)
+// FOLD: northern rings only; W32 rows hold E = q (F_m(theta) + F_m(pi - theta)) and O = q (F_m(theta) - F_m(pi - theta)); the degree
+// with l+m even contracts with E, the other one with O (d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta)).
 // =============================================================================================================
-template <int NC>
+template <int NC, bool FOLD>
 __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
-    constexpr int RL = 2, RT = 16, NI = RL * RT;
+    constexpr int RL = 2, RT = 16, NI = RL * RT, NCW = FOLD ? 2 * NC : NC;
     __shared__ float2 s_ab[2][TLF];
-    __shared__ float2 s_w[2][NTF * NC];
+    __shared__ float2 s_w[2][NTF * NCW];
     __shared__ float s_lam[2][NTF];
     __shared__ float2 s_part[NWF][NC][TLF];
     const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
 
     auto load_ops = [&](int m, int buf) {
         if (tid < TLF) s_ab[buf][tid] = A.ab[(size_t)m * A.Lp + l0 + tid];
-        for (int o = tid; o < NTF * NC; o += NWF * 32) s_w[buf][o] = A.in[((size_t)m * A.ntp + th0) * NC + o];
+        for (int o = tid; o < NTF * NCW; o += NWF * 32) s_w[buf][o] = A.in[((size_t)m * A.ntp + th0) * NCW + o];
         if (tid >= 128 && tid < 128 + NTF) s_lam[buf][tid - 128] = (float)A.lam[(size_t)(m + 1) * A.ntp + th0 + tid - 128];
     };
     float cur[NI], prev[NI];
@@ -183,7 +185,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
     for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
     int lr[RL];
 #pragma unroll
-    for (int r = 0; r < RL; ++r) lr[r] = l0 + lane + 32 * r;
+    for (int r = 0; r < RL; ++r) lr[r] = l0 + RL * lane + r;
     load_ops(mtop, 0);
     __syncthreads();
 
@@ -206,15 +208,19 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
             for (int c = 0; c < 2 * NC; ++c) acc[r][c] = 0.f;
         float2 ab[RL];
 #pragma unroll
-        for (int r = 0; r < RL; ++r) ab[r] = s_ab[buf][lane + 32 * r];
+        for (int r = 0; r < RL; ++r) ab[r] = s_ab[buf][RL * lane + r];
+        const int par = (l0 + m) & 1;                 // FOLD: degree r uses set (par ^ r): 0 = E, 1 = O (warp-uniform)
 #pragma unroll
         for (int i = 0; i < RT; ++i) {
             const float lam = s_lam[buf][w * RT + i];
-            float wv[2 * NC];
-#pragma unroll
-            for (int c = 0; c < NC; ++c) { const float2 t = s_w[buf][(w * RT + i) * NC + c]; wv[2 * c] = t.x; wv[2 * c + 1] = t.y; }
 #pragma unroll
             for (int r = 0; r < RL; ++r) {
+                float wv[2 * NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const float2 t = s_w[buf][(w * RT + i) * NCW + (FOLD ? ((par ^ r) & 1) * NC : 0) + c];
+                    wv[2 * c] = t.x; wv[2 * c + 1] = t.y;
+                }
                 const float e = ca[r * RT + i];
 #pragma unroll
                 for (int c = 0; c < 2 * NC; ++c) acc[r][c] = fmaf(e, wv[c], acc[r][c]);
@@ -225,17 +231,17 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
 #pragma unroll
         for (int r = 0; r < RL; ++r)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) s_part[w][c][lane + 32 * r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
+            for (int c = 0; c < NC; ++c) s_part[w][c][RL * lane + r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
         __syncthreads();
         for (int o = tid; o < NC * TLF; o += NWF * 32) {
             const int c = o / TLF, t = o % TLF, l = l0 + t;
-            double sx = 0.0, sy = 0.0;
+            float sx = 0.f, sy = 0.f;
 #pragma unroll
-            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += (double)v.x; sy += (double)v.y; }
+            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += v.x; sy += v.y; }
             if (l < A.L && l >= m && !(c == 1 && m == 0)) {
                 const int m_out = c == 1 ? -m : m;
                 double* op = reinterpret_cast<double*>(A.out) + ((size_t)(m_out + A.L - 1) * A.Lp + l) * 2;
-                red_add_f64(op, sx); red_add_f64(op + 1, sy);
+                red_add_f64(op, (double)sx); red_add_f64(op + 1, (double)sy);
             }
         }
         __syncthreads();
@@ -250,9 +256,12 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
 
 cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st) {
     dim3 grid((a.Lp / TLF) * (a.ntp / NTF));
-    if (forward) {
-        if (NC == 2) theta_forward_f32<2><<<grid, NWF * 32, 0, st>>>(a);
-        else theta_forward_f32<1><<<grid, NWF * 32, 0, st>>>(a);
+    if (forward && a.fold0) {
+        if (NC == 2) theta_forward_f32<2, true><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_forward_f32<1, true><<<grid, NWF * 32, 0, st>>>(a);
+    } else if (forward) {
+        if (NC == 2) theta_forward_f32<2, false><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_forward_f32<1, false><<<grid, NWF * 32, 0, st>>>(a);
     } else {
         if (NC == 2) theta_inverse_f32<2><<<grid, NWF * 32, 0, st>>>(a);
         else theta_inverse_f32<1><<<grid, NWF * 32, 0, st>>>(a);

@@ -73,3 +73,13 @@ def test_f32_config5a_scale_L2048_sampled(api, orc):
     sc = np.abs(want).max()
     for m, col in zip(ms, want):
         assert rel(got[:, m + L - 1], col, sc) < TOL32, m
+
+
+@pytest.mark.parametrize("L,real", [(8, False), (33, False), (130, False), (200, True)])
+def test_f32_forward_with_north_south_fold(api, orc, monkeypatch, L, real):
+    """fp32 forward with the north-south fold forced on (default at L >= 2048): northern rings only, E / O operand sets."""
+    monkeypatch.setenv("SHT_FOLD0", "1")
+    g = synth.random_map((L, 2 * L - 1), seed=3 * L, real=real, mw_pole_spin=0)
+    P = api.Plan(L, 0, reality=real, dtype="f32")
+    got = P.forward(dev(g.astype(np.float32 if real else np.complex64))).cpu().numpy()
+    assert rel(got, orc.s2_forward(L, 0, orc.MW, g.astype(np.complex128))) < TOL32
