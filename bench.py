@@ -305,6 +305,25 @@ def sweep(api, synth, torch, dev, flush, fp64_tf):
                      "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
         del P, f, b, flm
         torch.cuda.empty_cache()
+    # BASELINE.json configs[4], fp32 variant (theta_f32.cu): complex64 arrays, fp32 recursion + contraction
+    for L in (2048, 8192):
+        flm64 = synth.random_flm(L, 0, seed=4, sigma=synth.SIGMA_RED)
+        flm = torch.from_numpy(flm64.astype("complex64")).to(dev)
+        P = api.Plan(L, 0, device=dev, dtype="f32")
+        P.enable_timing(True)
+        f = P.inverse(flm); b = P.forward(f)
+        ti, tf = [], []
+        for _ in range(3):
+            flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
+            flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
+        mi = {k: min(t[k] for t in ti) for k in ti[0]}
+        mf = {k: min(t[k] for t in tf) for k in tf[0]}
+        rows.append({"config": f"MW spin-0 L={L} fp32", "inverse_ms": mi, "forward_ms": mf,
+                     "inverse_tflops_fp32": P.flops(False) / (mi["hot"] * 1e-3) / 1e12, "forward_tflops_fp32": P.flops(True) / (mf["hot"] * 1e-3) / 1e12,
+                     "fp32_peak_nominal_tflops": 148 * 128 * 2 * 1.965e-3,
+                     "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
+        del P, f, b, flm
+        torch.cuda.empty_cache()
     # BASELINE.json configs[4], second half: 16 maps at L = 2048 transformed together (shared recursion, DMMA contraction)
     L, B = 2048, 16
     import numpy as _np

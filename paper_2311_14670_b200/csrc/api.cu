@@ -83,6 +83,7 @@ struct sht_plan {
     bool f32_inner = false;    // set while an fp32 transform runs its fp64-array core
     int dtype = SHT_F64;       // SHT_F32: fp32 hot kernels (theta_f32.cu) and fp32 public arrays; staging and FFTs stay fp64
     float2* ab32 = nullptr;    // fp32: [L][Lp] recursion coefficients
+    float *lam32_inv = nullptr, *lam32_fwd = nullptr;
     float *st32_inv = nullptr, *st32_fwd = nullptr; uint16_t *k16_inv = nullptr, *k16_fwd = nullptr;   // fp32 start values
     double2 *io_a = nullptr, *io_b = nullptr;   // fp32: fp64 copies of the public arrays
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
@@ -276,6 +277,7 @@ void layout(sht_plan* P, char* base) {
         P->st32_inv = B.take<float>((size_t)Lp * P->inv.ntp); P->k16_inv = B.take<uint16_t>((size_t)Lp * P->inv.ntp);
         P->st32_fwd = B.take<float>((size_t)Lp * P->fwd.ntp); P->k16_fwd = B.take<uint16_t>((size_t)Lp * P->fwd.ntp);
         P->io_a = B.take<double2>((size_t)L * NB); P->io_b = B.take<double2>((size_t)L * NB);
+        P->lam32_inv = B.take<float>((size_t)(L + 1) * P->inv.ntp); P->lam32_fwd = B.take<float>((size_t)(L + 1) * P->fwd.ntp);
     }
     P->fft_work = B.take<char>(P->fft_work_bytes);
     // route every pass to its slab's output array
@@ -552,7 +554,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         stage(P, CAT_HOT, st);
         F32Args a{};
         a.L = L; a.Lp = P->Lp; a.nth = P->inv.nth; a.ntp = P->inv.ntp; a.NB = P->NB; a.ldout = P->F_ld;
-        a.ab = P->ab32; a.lam = ph.p.lam; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
+        a.ab = P->ab32; a.lam32 = P->lam32_inv; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
         a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F;
         CK(launch_theta_f32(a, false, NC, st));
         CK(st_pole_inverse(L, 0, coef, P->scale_inv, P->F + P->inv.nth, st));
@@ -632,7 +634,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         stage(P, CAT_HOT, st);
         F32Args a{};
         a.L = L; a.Lp = P->Lp; a.nth = P->fwd.nth; a.ntp = P->fwd.ntp; a.NB = P->NB; a.ldout = 0; a.fold0 = P->fold0;
-        a.ab = P->ab32; a.lam = ph.p.lam; a.st_val = P->st32_fwd; a.st_k = P->k16_fwd;
+        a.ab = P->ab32; a.lam32 = P->lam32_fwd; a.st_val = P->st32_fwd; a.st_k = P->k16_fwd;
         a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->H;
         CK(launch_theta_f32(a, true, NC, st));
         return SHT_OK;
@@ -846,6 +848,8 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         CK(st_ab32(L, Lp, P->ab32, st));
         CK(st_start32((size_t)Lp * P->inv.ntp, P->inv.start[0].val, P->inv.start[0].k, P->st32_inv, P->k16_inv, st));
         CK(st_start32((size_t)Lp * P->fwd.ntp, P->fwd.start[0].val, P->fwd.start[0].k, P->st32_fwd, P->k16_fwd, st));
+        CK(st_f64_to_f32((size_t)(L + 1) * P->inv.ntp, P->pinv[0].p.lam, P->lam32_inv, st));
+        CK(st_f64_to_f32((size_t)(L + 1) * P->fwd.ntp, P->pfwd[0].p.lam, P->lam32_fwd, st));
     }
     if (P->sampling == SHT_MW) {
         for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));

@@ -78,7 +78,7 @@ struct F32Args {
     int L, Lp, nth, ntp, NB, ldout;
     int fold0;                // forward: northern rings only, W32 rows hold the E / O sets (as theta_kernels.cu FOLD)
     const float2* ab;         // [m][Lp] {A_m(l) = a_{m-1}(l), B_m(l) = a_{m-1}(l)/a_m(l)} (Eq. 25-26), rows m = 0..L-1 (row 0 unused: zeros)
-    const double* lam;        // lambda table of the n = 0 pass, row m + 1 (internal layout of ThetaPass::lam with m_end = 0)
+    const float* lam32;       // fp32 copy of the lambda table of the n = 0 pass, row m + 1 (layout of ThetaPass::lam with m_end = 0)
     const float* st_val;      // [Lp][ntp] Eq. 27 start values, windowed: true value = st_val * 2^(-48 st_k)
     const uint16_t* st_k;
     const float2* in;         // inverse: G32[m][Lp][NC] = scale(l) f_lm; forward: W32[m][ntp][NC] = q(theta) F_m(theta)

@@ -11,6 +11,7 @@
 // ring) is the fp64 code; the kernels read fp32 operand tables and add their block sums into the fp64 F / H arrays.
 #include "internal.h"
 
+#include <cuda_pipeline.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -74,10 +75,14 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
     const int mtop = min(l0 + TLF - 1, A.L - 1);
     const int la = l0 + w * RL;
 
-    auto load_ops = [&](int m, int buf) {           // operand rows of step m: one element per thread
-        if (tid < TLF) s_ab[buf][tid] = A.ab[(size_t)m * A.Lp + l0 + tid];
-        if (tid < TLF * NC) s_g[buf][tid] = A.in[((size_t)m * A.Lp + l0) * NC + tid];
-        if (tid >= 128 && tid < 128 + NTF) s_lam[buf][tid - 128] = (float)A.lam[(size_t)(m + 1) * A.ntp + th0 + tid - 128];
+    // operand rows of step m, one element per thread, copied global -> shared asynchronously (cp.async): the copy of step m-1
+    // is in flight while step m is computed and is awaited just before the block barrier
+    auto load_ops = [&](int m, int buf) {
+        if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float2));
+        if (tid < TLF * NC) __pipeline_memcpy_async(&s_g[buf][tid], &A.in[((size_t)m * A.Lp + l0) * NC + tid], sizeof(float2));
+        if (tid >= 128 && tid < 128 + NTF)
+            __pipeline_memcpy_async(&s_lam[buf][tid - 128], &A.lam32[(size_t)(m + 1) * A.ntp + th0 + tid - 128], sizeof(float));
+        __pipeline_commit();
     };
     float cur[NI], prev[NI];
     KPackF kp;
@@ -85,6 +90,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
 #pragma unroll
     for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
     load_ops(mtop, 0);
+    __pipeline_wait_prior(0);
     __syncthreads();
 
     // one step: project d_m, then advance to d_{m-1}.  `ca` holds d_m, `cb` holds d_{m+1} on entry and d_{m-1} on exit.
@@ -132,6 +138,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
         for (int i = 0; i < RT; ++i)
 #pragma unroll
             for (int c = 0; c < NC; ++c) s_part[w][c][lane + 32 * i] = make_float2(acc[i][2 * c], acc[i][2 * c + 1]);
+        __pipeline_wait_prior(0);
         __syncthreads();
         for (int o = tid; o < NC * NTF; o += NWF * 32) {
             const int c = o / NTF, t = o % NTF, th = th0 + t;
@@ -174,9 +181,12 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
     const int mtop = min(l0 + TLF - 1, A.L - 1);
 
     auto load_ops = [&](int m, int buf) {
-        if (tid < TLF) s_ab[buf][tid] = A.ab[(size_t)m * A.Lp + l0 + tid];
-        for (int o = tid; o < NTF * NCW; o += NWF * 32) s_w[buf][o] = A.in[((size_t)m * A.ntp + th0) * NCW + o];
-        if (tid >= 128 && tid < 128 + NTF) s_lam[buf][tid - 128] = (float)A.lam[(size_t)(m + 1) * A.ntp + th0 + tid - 128];
+        if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float2));
+        for (int o = tid; o < NTF * NCW; o += NWF * 32)
+            __pipeline_memcpy_async(&s_w[buf][o], &A.in[((size_t)m * A.ntp + th0) * NCW + o], sizeof(float2));
+        if (tid >= 128 && tid < 128 + NTF)
+            __pipeline_memcpy_async(&s_lam[buf][tid - 128], &A.lam32[(size_t)(m + 1) * A.ntp + th0 + tid - 128], sizeof(float));
+        __pipeline_commit();
     };
     float cur[NI], prev[NI];
     KPackF kp;
@@ -187,6 +197,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
 #pragma unroll
     for (int r = 0; r < RL; ++r) lr[r] = l0 + RL * lane + r;
     load_ops(mtop, 0);
+    __pipeline_wait_prior(0);
     __syncthreads();
 
     auto step = [&](const int m, const int buf, float (&ca)[NI], float (&cb)[NI]) {
@@ -232,6 +243,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
         for (int r = 0; r < RL; ++r)
 #pragma unroll
             for (int c = 0; c < NC; ++c) s_part[w][c][RL * lane + r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
+        __pipeline_wait_prior(0);
         __syncthreads();
         for (int o = tid; o < NC * TLF; o += NWF * 32) {
             const int c = o / TLF, t = o % TLF, l = l0 + t;

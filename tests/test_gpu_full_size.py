@@ -91,7 +91,7 @@ def test_config4_so3_L256_N8(api, orc):
 
 
 def test_config5a_mw_L8192_spin0(api, orc):
-    """configs[4], first half: spin-0 complex SHT, MW L = 8192 (8192 x 16383 map, 2.1 GB), sigma_l = 1/(l+1), seed 4, fp64.
+    """configs[4], first half: spin-0 complex SHT, MW L = 8192 (8192 x 16383 map, 2.1 GB), sigma_l = 1/(l+1), seed 4, fp64 and fp32.
     The oracle cannot synthesise the full map: inverse parity on sampled rings, forward parity of a white-noise map on
     sampled orders m, and the sampling-theorem round trip against the generating coefficients (a property at any size).
     north_star states 1e-11 up to L = 1024 and asks for the growth with L: the bound used here is 1e-11 * L/1024."""
@@ -118,3 +118,18 @@ def test_config5a_mw_L8192_spin0(api, orc):
     sc = np.abs(want).max()
     for m, col in zip(ms, want):
         assert rel(got[:, m + L - 1], col, sc) < tol, m
+    # the fp32 variant of the same config (csrc/theta_f32.cu): north_star tolerance 1e-4
+    del P, got
+    torch.cuda.empty_cache()
+    P32 = api.Plan(L, spin, dtype="f32")
+    d32 = dev(flm.astype(np.complex64))
+    f32 = P32.inverse(d32)
+    for r, row in zip(rings, rows):
+        assert rel(f32[int(r)].cpu().numpy(), row, scale) < 1e-4, r
+    back32 = P32.forward(f32)
+    err32 = float((back32 - d32).abs().max() / d32.abs().max())
+    print(f"L=8192 fp32 round trip max rel err {err32:.3e}")
+    assert err32 < 2e-4
+    got32 = P32.forward(dev(g.astype(np.complex64))).cpu().numpy()
+    for m, col in zip(ms, want):
+        assert rel(got32[:, m + L - 1], col, sc) < 1e-4, m
