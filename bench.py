@@ -142,6 +142,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--L", type=int, default=None, help="profiling only: override the band-limit of the workload")
     ap.add_argument("--spin", type=int, default=None, help="profiling only: override the spin of the workload")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="profiling only: fp32 variant (needs --spin 0)")
     ap.add_argument("--batch", type=int, default=1, help="profiling only: transform a batch of maps together (configs[4]: --L 2048 --spin 0 --batch 16)")
     args = ap.parse_args()
     if args.L is not None:
@@ -171,9 +172,11 @@ def main():
         flm_h = synth.random_flm(L, spin, seed=WORKLOAD["seed"] + rank, sigma=synth.SIGMA_CMB)
     else:
         flm_h = np.stack([synth.random_flm(L, spin, seed=4 + i + 1000 * rank, sigma=synth.SIGMA_RED) for i in range(B)])
+    if args.dtype == "f32":
+        flm_h = flm_h.astype(np.complex64)
     flm = torch.from_numpy(flm_h).to(dev)
-    plan = api.Plan(L, spin, device=dev, batch=B)
-    f = torch.empty(plan.map_shape, dtype=torch.complex128, device=dev)
+    plan = api.Plan(L, spin, device=dev, batch=B, dtype=args.dtype)
+    f = torch.empty(plan.map_shape, dtype=plan.map_dtype, device=dev)
     back = torch.empty_like(flm)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
@@ -224,26 +227,30 @@ def main():
     if rank == 0:
         pk, pk_kind = peaks()
         fp64_tf, _ = api.fp64_peak(20000)
+        peak_tf = fp64_tf
+        if args.dtype == "f32":       # FP32 FMA pipe: 148 SM x 128 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts; not in MEASURED_PEAKS.json)
+            peak_tf = 148 * 128 * 2 * 1.965e-3
         # algorithmic flop: per d-step 6 (recursion) + 4 per order and map served
         flops_fwd = plan.flops(True)
         flops_inv = plan.flops(False)
         fl = flops_fwd / plan.dsteps(True)
         ach = flops_fwd / (stages["forward_ms"]["hot"] * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": ("theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>") + " (fused m-recursion + theta contraction, Eq. 25+30)",
-                "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf, "traffic": NCU_TRAFFIC_BYTES.get((L, spin, B)),
+        roof = {"bound": "alu", "kernel": ("theta_forward_f32" if args.dtype == "f32" else "theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>") + " (fused m-recursion + theta contraction, Eq. 25+30)",
+                "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
+                "traffic": NCU_TRAFFIC_BYTES.get((L, spin, B)) if args.dtype == "f64" else None,
                 "traffic_source": "profiles/r1_v7_theta_kernels.md (ncu --set full, bytes per launch)",
                 "peak_kind": "measured in this run by a register-only DFMA chain (sht_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
                 "inverse_kernel": {"achieved": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12,
-                                   "frac": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12 / fp64_tf},
+                                   "frac": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12 / peak_tf},
                 "hbm_peak_gbs": pk.get("hbm_gbs"), "hbm_peak_kind": pk_kind}
         # end to end through host buffers (pinned), H2D + D2H inside the timed region
-        fh = torch.empty(plan.map_shape, dtype=torch.complex128).pin_memory()
+        fh = torch.empty(plan.map_shape, dtype=plan.map_dtype).pin_memory()
         ch = torch.from_numpy(flm_h).pin_memory()
-        bh = torch.empty(plan.coef_shape, dtype=torch.complex128).pin_memory()
+        bh = torch.empty(plan.coef_shape, dtype=plan.coef_dtype).pin_memory()
 
         def pair_host():
-            if B == 1:          # the C-ABI host-buffer calls copy in and out themselves
+            if B == 1 and args.dtype == "f64":          # the C-ABI host-buffer calls copy in and out themselves
                 api.s2_inverse_host(ch.numpy(), L, spin, out=fh.numpy()); api.s2_forward_host(fh.numpy(), L, spin, out=bh.numpy())
             else:               # batched plans take device pointers: pinned copies around them, same bytes
                 flm.copy_(ch, non_blocking=True); plan.inverse(flm, out=f); fh.copy_(f, non_blocking=True)
@@ -259,16 +266,16 @@ def main():
         torch.cuda.synchronize()
         te = (time.perf_counter() - t0) / ne
         fh, ch, bh = fh.numpy(), ch.numpy(), bh.numpy()
-        nbytes = B * L * (2 * L - 1) * 16
+        nbytes = B * L * (2 * L - 1) * (8 if args.dtype == "f32" else 16)
         e2e = {"value": world * B / te, "unit": UNIT, "h2d_bytes_per_step": 2 * nbytes, "d2h_bytes_per_step": 2 * nbytes,
                "ms_per_step": te * 1e3, "roundtrip_err": float(np.abs(bh - flm_h).max() / np.abs(flm_h).max())}
         cpu = None
         if not args.no_cpu:
-            t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm_h if B == 1 else flm_h[0])
+            t_inv, t_fwd, cores, sample = oracle_sample(L, spin, (flm_h if B == 1 else flm_h[0]).astype(np.complex128))
             cpu = {"value": 1.0 / (t_inv + t_fwd), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                    "inverse_s": t_inv, "forward_s": t_fwd}
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-               "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+               "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
                "data": "synthetic",
                "config": {"workload": f"{'BASELINE.json configs[1]' if (L, spin, B) == (1024, 2, 1) else 'override'}: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
                                       + (f"batch of {B} maps transformed together, " if B > 1 else "") +
