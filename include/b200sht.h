@@ -62,6 +62,8 @@ const char* sht_last_error(void);       /* text of the last CUDA / cuFFT failure
  * nside is used for HEALPix only (the band-limit L is independent of it).
  * Environment: SHT_FOLD0=0/1 forces the north-south fold of spin-0 forward transforms off / on at plan creation
  * (default: on when the northern rings alone fill the GPU, L >= 2048 on MW); results agree to rounding either way.
+ * SHT_INVSYM=1 makes spin-0 MW plans evaluate the inverse theta step on the L midpoint rings (2j+1)pi/(2L) with the
+ * north-south fold and resample F_m to the MW rings by FFT (exact; off by default: not yet faster).
  */
 sht_status sht_plan_s2(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype);
 sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);

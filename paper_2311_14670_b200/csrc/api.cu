@@ -86,6 +86,8 @@ struct sht_plan {
     float *lam32_inv = nullptr, *lam32_fwd = nullptr;
     float *st32_inv = nullptr, *st32_fwd = nullptr; uint16_t *k16_inv = nullptr, *k16_fwd = nullptr;   // fp32 start values
     double2 *io_a = nullptr, *io_b = nullptr;   // fp32: fp64 copies of the public arrays
+    int invsym = 0;            // MW spin-0 inverse: F_m on the L midpoint rings (north-south fold), then FFT resampling to the MW rings
+    cufftHandle fft_sym = 0;   // length 2L, batch 2L-1
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
@@ -147,11 +149,11 @@ void rings_mw(RingSet& R, int Lt) {      // Eq. 37: theta_t = (2t
 // 4L equispaced samples of the theta circle.  The paper upsamples F_m(theta) to "2L" rings; any ring set
 // on which the quadrature of the band-limit-(2L-2) integrand is exact gives the same result, and this one has a
 // power-of-two FFT length 4L (the MW(2L) set needs 4L-1, often prime) and no pole ring.
-void rings_mid(RingSet& R, int L) {
-    R.nth = 2 * L; R.pole = false; R.symmetric = true;
+void rings_mid(RingSet& R, int nrings) {      // theta_u = (2u+1) pi / (2 nrings), u = 0..nrings-1
+    R.nth = nrings; R.pole = false; R.symmetric = true;
     R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
     for (int u = 0; u < R.nth; ++u) {
-        ld th = PI_L * (ld)(2 * u + 1) / (ld)(4 * L);
+        ld th = PI_L * (ld)(2 * u + 1) / (ld)(2 * nrings);
         R.ct[u] = cosl(th); R.c2[u] = cosl(th / 2); R.s2[u] = sinl(th / 2);
     }
     R.ntp = (int)rup((size_t)R.nth, 128);
@@ -248,6 +250,7 @@ void layout(sht_plan* P, char* base) {
     // scratch arrays
     P->F_nrings = (P->inv.nfull ? P->inv.nfull : P->inv.nth) + (P->inv.pole ? 1 : 0);
     P->F_ld = P->inv.nfull ? (int)rup((size_t)P->inv.nfull + 1, 128) : P->inv.ntp;
+    if (P->invsym) P->F_ld = (int)rup((size_t)L, 128);     // holds the L midpoint rings, then the L MW rings (the phi-FFT stride)
     P->F_slab = (size_t)NB * P->F_ld;
     P->F = B.take<double2>(P->F_slab * P->nslab);
     P->polev = B.take<double2>(P->nslab);
@@ -349,6 +352,11 @@ sht_status make_fft_plans(sht_plan* P) {
     CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
     { int inembed[1] = {4 * L};
       CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L, inembed, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
+    if (P->invsym) {
+        int n4[1] = {2 * L};
+        CF(cufftCreate(&P->fft_sym)); CF(cufftSetAutoAllocation(P->fft_sym, 0));
+        CF(cufftMakePlanMany(P->fft_sym, 1, n4, n4, 1, 2 * L, n4, 1, 2 * L, CUFFT_Z2Z, NB, &w)); ws = w > ws ? w : ws;
+    }
     if (P->kind == 1) {
         int n3[1] = {2 * P->N - 1};
         CF(cufftCreate(&P->fft_gamma)); CF(cufftSetAutoAllocation(P->fft_gamma, 0));
@@ -668,6 +676,23 @@ sht_status check_ready(const sht_plan* P) {
     return SHT_OK;
 }
 
+// invsym: F[bin][F_ld] holds F_m on the L midpoint rings; replace it by F_m on the L MW rings (incl. the ring theta = pi).
+// Scratch: Z (2L per row, FFT in place), X (2L-1 per row, inverse FFT in place).
+sht_status resample_sym_to_mw(sht_plan* P, cudaStream_t st) {
+    const int L = P->L, NB = P->NB;
+    stage(P, CAT_STAGE, st);
+    CK(st_sym_extend(L, P->slab_n[0], P->F_ld, P->F, P->Z, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_sym, st)); CF(cufftExecZ2Z(P->fft_sym, P->Z, P->Z, CUFFT_FORWARD));
+    stage(P, CAT_STAGE, st);
+    CK(st_sym_rebin(L, P->Z, P->X, st));
+    stage(P, CAT_FFT, st);
+    CF(cufftSetStream(P->fft_th1, st)); CF(cufftExecZ2Z(P->fft_th1, P->X, P->X, CUFFT_INVERSE));
+    stage(P, CAT_STAGE, st);
+    CK(st_rows_head(NB, L, NB, P->F_ld, P->X, P->F, st));
+    return SHT_OK;
+}
+
 // MW: F_m(theta_t) on L rings (Fa, [bin][Ltp]) -> U[bin][4L] on the rings theta'_u = (2u+1)pi/(4L) (in Z; u < 2L used)
 sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
     const int L = P->L, NB = P->NB, T2 = 4 * L;
@@ -767,7 +792,7 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
     P->dtype = dtype;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
-    if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, L); }
+    if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L); }
     else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
     if (spin == 0) {
         // n = 0 fold (theta_kernels.cu FOLD): worth it once the northern half alone fills the GPU with >= 2 waves of 64 x 128 tiles
@@ -776,7 +801,14 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
         bool on = tiles >= 2 * 148;
         if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
         if (on) { P->fold0 = 1; north_only(P->fwd); }
-        // the inverse rings of HEALPix are symmetric too (the MW rings (2t+1)pi/(2L-1) are not)
+        // MW inverse: the MW rings (2t+1)pi/(2L-1) are not symmetric; evaluate F_m on the L midpoint rings instead (folded) and
+        // resample to the MW rings with two FFT passes (resample_sym_to_mw).  SHT_INVSYM=0/1 overrides.
+        // Off by default: the two-column folded inverse kernel only fits shared memory with 64-ring tiles and gains 17 % on the hot
+        // kernel at L = 2048 (3.03 -> 2.53 ms) while the resampling adds 0.77 ms of FFT + staging (measured).
+        bool isym = false;
+        if (const char* e = getenv("SHT_INVSYM")) isym = e[0] == '1' && sampling == SHT_MW && batch == 1 && dtype == SHT_F64;
+        if (isym) { P->invsym = 1; P->fold0i = 1; rings_mid(P->inv, L); north_only(P->inv); }
+        // the inverse rings of HEALPix are symmetric too
         if (on && sampling == SHT_HEALPIX && batch == 1) { P->fold0i = 1; north_only(P->inv); }
     }
     sht_status s = plan_common(P);
@@ -793,7 +825,7 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     P->kind = 1; P->L = L; P->N = N; P->sampling = SHT_MW;
     P->nslab = 2 * N - 1;
     for (int b = 0; b < P->nslab; ++b) P->slab_n.push_back(b < N ? b : b - (2 * N - 1));   // gamma-FFT bin order
-    rings_mw(P->inv, L); rings_mid(P->fwd, L);
+    rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L);
     sht_status s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
@@ -853,6 +885,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     }
     if (P->sampling == SHT_MW) {
         for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));
+        if (P->invsym) CF(cufftSetWorkArea(P->fft_sym, P->fft_work));
         if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
     } else {
         CF(cufftSetWorkArea(P->fft_hp_eq, P->fft_work));
@@ -873,7 +906,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
 sht_status sht_plan_destroy(sht_plan* P) {
     if (!P) return SHT_OK;
     if (P->have_fft || P->fft_phi_inv) {
-        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_hp_cap, P->fft_hp_eq})
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_hp_cap, P->fft_hp_eq, P->fft_sym})
             if (h) cufftDestroy(h);
     }
     for (auto e : P->ev) cudaEventDestroy(e);
@@ -911,6 +944,7 @@ sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_str
     cudaStream_t st = (cudaStream_t)stream;
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
+    if (P->invsym) CS(resample_sym_to_mw(P, st));
     int nt = sht_plan_ntheta(P, 0);
     CK(st_rows_reorder(P->L, P->NB, nt, P->F_ld, nt, 1, P->F, (double2*)Fm, st));
     stage(P, CAT_STAGE, st);
@@ -957,6 +991,7 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     P->ev_n = 0;
     CS(run_theta_inverse(P, (const double2*)flm, st));
     if (P->sampling == SHT_HEALPIX) return healpix_synthesis(P, f, st);
+    if (P->invsym) CS(resample_sym_to_mw(P, st));
     stage(P, CAT_FFT, st);
     CF(cufftSetStream(P->fft_phi_inv, st));
     double2* outc = P->reality ? P->cplx : (double2*)f;

@@ -251,6 +251,37 @@ __global__ void k_mw_pad_phase(int L, int ldin, int ldout, const double2* __rest
     }
     Z[(size_t)b * ldout + k2] = v;
 }
+// ---- MW inverse through a symmetric intermediate ring set (api.cu `invsym`) ----------------------------------------------
+// F_m(theta) of a band-limited signal is a trigonometric polynomial of degree <= L-1 on the theta circle with F_m(2pi - theta) =
+// (-1)^{m+s} F_m(theta).  The theta kernel evaluates it on the L midpoint rings vartheta_j = (2j+1)pi/(2L), which are
+// symmetric about the equator (north-south fold); these kernels carry it to the MW rings theta_t = (2t+1)pi/(2L-1), exactly:
+// extend to the 2L-point circle -> FFT(2L) -> phase and re-bin -> inverse FFT(2L-1) -> keep t = 0..L-1 (t = L-1 is the ring theta = pi).
+__global__ void k_sym_extend(int L, int n, int ldin, const double2* __restrict__ F, double2* __restrict__ X) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (j >= 2 * L) return;
+    const int T = 2 * L - 1, m = b < L ? b : b - T;
+    double2 v;
+    if (j < L) v = F[(size_t)b * ldin + j];
+    else { v = F[(size_t)b * ldin + (2 * L - 1 - j)]; const double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
+    X[(size_t)b * 2 * L + j] = v;
+}
+// Y[b][k] = 2L c_{m'} e^{i m' pi/(2L)} (k = m' mod 2L)  ->  Z[b][m' mod (2L-1)] = c_{m'} e^{i m' pi/(2L-1)}
+__global__ void k_sym_rebin(int L, const double2* __restrict__ Y, double2* __restrict__ Z) {
+    int k2 = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const int T = 2 * L - 1;
+    if (k2 >= T) return;
+    const int mp = k2 < L ? k2 : k2 - T;
+    const double2 y = Y[(size_t)b * 2 * L + (mp < 0 ? mp + 2 * L : mp)];
+    double s1, c1, s2, c2;
+    sincospi(-(double)mp / (double)(2 * L), &s1, &c1);
+    sincospi((double)mp / (double)T, &s2, &c2);
+    const double pr = c1 * c2 - s1 * s2, pi_ = c1 * s2 + s1 * c2, inv = 1.0 / (double)(2 * L);
+    Z[(size_t)b * T + k2] = make_double2((y.x * pr - y.y * pi_) * inv, (y.x * pi_ + y.y * pr) * inv);
+}
+__global__ void k_rows_head(int ncol, int ldin, int ldout, const double2* __restrict__ in, double2* __restrict__ out) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (c < ncol) out[(size_t)b * ldout + c] = in[(size_t)b * ldin + c];
+}
 // forward split: U[bin][u] (upsampled F_m(theta'_u), or the ring-FFT output on other samplings) -> weighted operand
 // tiles W[m-m_end][ntp][NC] of one pass; rings not served by the pass at step m get 0 (peak split, R5).
 // fold != 0 (n != 0, symmetric ring set): column 0 = order +m at the ring itself (m >= m_s), column 1 = order -m at the MIRRORED
@@ -772,5 +803,17 @@ cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t s
 cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
                                       float2* W, cudaStream_t st) {
     k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, wq, U, W);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st) {
+    k_sym_extend<<<dim3(cdiv(2 * L, 128), 2 * L - 1), 128, 0, st>>>(L, n, ldin, F, X);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st) {
+    k_sym_rebin<<<dim3(cdiv(2 * L - 1, 128), 2 * L - 1), 128, 0, st>>>(L, Y, Z);
+    LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st) {
+    k_rows_head<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ldin, ldout, in, out);
     LAUNCHED(); return cudaSuccess;
 }

@@ -30,6 +30,11 @@ cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* sc
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st);
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st);
 
+// MW inverse through the symmetric midpoint rings: resampling of F_m to the MW rings
+cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st);
+cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st);
+cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st);
+
 // batched path (operand / result layouts of theta_mma.cu, internal.h)
 cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, const double2* coef,
                                   const double* scale, const double* C, const double2* SG, int sgstride, double* Gb, size_t cg_stride,

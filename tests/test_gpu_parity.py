@@ -214,3 +214,19 @@ def test_spin0_forward_with_and_without_north_south_fold(api, orc, monkeypatch, 
         ref = orc.s2_inverse(L, 0, orc.HEALPIX, flm, nside=nside)
         got = P.inverse(dev(flm)).cpu().numpy()
         assert rel(got, ref.real if real else ref) < TOL
+
+
+@pytest.mark.parametrize("sym", ["0", "1"])
+@pytest.mark.parametrize("L,real", [(1, False), (2, False), (8, False), (33, False), (64, False), (130, False), (200, True), (257, False)])
+def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, monkeypatch, sym, L, real):
+    """MW spin-0 inverse either directly on the MW rings, or (default at L >= 2048) on the L midpoint rings (2j+1)pi/(2L) with the
+    north-south fold followed by an exact FFT resampling of F_m(theta) to the MW rings.  Both against the oracle, element by element,
+    through the full transform and through the theta-stage entry point."""
+    monkeypatch.setenv("SHT_INVSYM", sym)
+    flm = synth.random_flm(L, 0, seed=5 * L, real=real)
+    P = api.Plan(L, 0, reality=real)
+    ref = orc.s2_inverse(L, 0, orc.MW, flm)
+    got = P.inverse(dev(flm)).cpu().numpy()
+    assert rel(got, ref.real if real else ref) < TOL
+    F = P.theta_inverse(dev(flm)).cpu().numpy()
+    assert rel(F, orc.s2_theta_inverse_columns(L, 0, orc.MW, flm, np.arange(-(L - 1), L))) < TOL
