@@ -1,14 +1,17 @@
 #!/usr/bin/env python
-"""bench.py -- headline measurement: spin-s SHT inverse + forward on one B200 (and N independent ranks).
+"""bench.py -- headline measurement: spin-s SHT / Wigner transforms on one B200 (and N independent ranks).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-sweep] [--shard rings]
 
-A "step" is one pass of the whole hot path over one synthetic input: an inverse transform (flm -> map) followed by
-a forward transform (map -> flm) of BASELINE.json's config[1] (spin-2 complex SHT, MW sampling, L = 1024, fp64).
-`value` is transform pairs per second over all ranks with inputs resident in HBM; `e2e` is the same through the
-host-buffer C-ABI calls (H2D/D2H inside the timed region).  `roofline` is the fused recursion+contraction kernel of
-the forward transform against the FP64 FMA-pipe peak; `cpu_baseline` is the CPU oracle on a bounded sample.
-One JSON line on stdout (rank 0).
+A "step" is one pass of the whole hot path over one synthetic input: an inverse transform (flm -> map) followed by a
+forward transform (map -> flm).  The headline workload is BASELINE.json configs[4], first half: spin-0 complex SHT, MW
+sampling, L = 8192, fp64 -- the largest single-GPU configuration, and the one the north_star target ("fused kernel >= 40 % of
+FP64 peak at L >= 2048") is stated on.  `value` is transform pairs per second over all ranks with inputs resident in HBM;
+`e2e` is the same through the host-buffer C-ABI calls (H2D / D2H inside the timed region).  `roofline` is the fused
+recursion + contraction kernel of the forward transform against the FP64 FMA-pipe peak measured in the same process;
+`sweep` carries the metric of BASELINE.json itself -- ms (hot / fft / staging), fraction of FP64 peak, and GB/s of the FFT and
+staging stages -- versus L for MW, for HEALPix, SO(3), the fp32 variant and the batched (DMMA) configuration.
+`cpu_baseline` is the CPU oracle on a bounded sample.  One JSON line on stdout (rank 0).
 """
 import argparse
 import json
@@ -24,13 +27,34 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-WORKLOAD = dict(L=1024, spin=2, seed=1)
-METRIC = "SHT fwd+inv transform pairs per second (MW L=1024 spin-2 fp64, 1 B200)"
+WORKLOAD = dict(L=8192, spin=0, seed=4)
 UNIT = "transform_pairs/s"
-# algorithmic flop per d-step: recursion 6 + projection 4 per order served
-# dram__bytes_read.sum + dram__bytes_write.sum of the forward theta kernel, per launch, from the ncu --set full captures in
-# profiles/r1_v7_theta_kernels.md; key (L, spin, batch).  Not measurable inside this process: null for other workloads.
-NCU_TRAFFIC_BYTES = {(1024, 2, 1): 128.008e6 + 11.222e6, (2048, 0, 1): 1.516876e9 + 155.507e6, (2048, 0, 16): 46.314083e9 + 11.453921e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of the forward theta kernel, per launch, from the ncu --set full captures under
+# profiles/ (file named beside each); key (L, spin, batch).  Not measurable inside this process: null for other workloads.
+NCU_TRAFFIC_BYTES = {
+    (1024, 2, 1): (128.008e6 + 11.222e6, "profiles/r1_v7_theta_kernels.md"),
+    (2048, 0, 1): (1.516876e9 + 155.507e6, "profiles/r1_v7_theta_kernels.md"),
+    (2048, 0, 16): (46.314083e9 + 11.453921e9, "profiles/r1_v7_theta_kernels.md"),
+}
+
+
+def metric_name(L, spin):
+    return f"SHT fwd+inv transform pairs per second (MW L={L} spin-{spin} fp64, 1 B200)"
+
+
+def workload_name(L, spin, B=1):
+    tag = {(8192, 0, 1): "BASELINE.json configs[4] (first half)", (1024, 2, 1): "BASELINE.json configs[1]",
+           (2048, 0, 16): "BASELINE.json configs[4] (second half)"}.get((L, spin, B), "override")
+    sig = "1/(l(l+1)) (l >= 2)" if spin == 2 else "1/(l+1)^2"
+    return (f"{tag}: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
+            + (f"batch of {B} maps transformed together, " if B > 1 else "")
+            + f"flm complex Gaussian with variance {sig}, inverse + forward per step; the L >= 2048 rows of `sweep` are the "
+              "north_star target evidence")
+
+
+def sigma_for(spin):
+    from paper_2311_14670_b200 import synth
+    return synth.SIGMA_CMB if spin == 2 else synth.SIGMA_RED
 
 
 def peaks():
@@ -70,41 +94,43 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm, smax, reasons = [], [], set()
+        sm, smax, pw, reasons = [], [], [], set()
         for ln in self.lines:
             c = [x.strip() for x in ln.split(",")]
             if len(c) < 9:
                 continue
             try:
-                sm.append(float(c[1])); smax.append(float(c[2]))
+                sm.append(float(c[1])); smax.append(float(c[2])); pw.append(float(c[3]))
             except ValueError:
                 continue
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=max(smax) if smax else None,
-                    reasons=sorted(reasons), samples=len(sm))
+                    reasons=sorted(reasons), samples=len(sm), power_w_max=max(pw) if pw else None)
 
 
-def oracle_sample(L, spin, flm, n_cols=12, n_rings=6):
-    """Time the CPU oracle (as it stands) on a bounded sample and extrapolate to one inverse + one forward.
-    Inverse cost is per ring, forward cost per harmonic order m (both ~uniform across rings; per m ~ (L-|m|))."""
+def oracle_sample(L, spin, flm, n_cols):
+    """Time the CPU oracle (as it stands) on a bounded sample of the workload and extrapolate to one inverse + one forward.
+
+    Sample: the theta steps (Eq. 33 and Eq. 30, the O(L^3) part) of n_cols harmonic orders m spread over [-(L-1), L-1], all rings.
+    The cost of a column is proportional to L - |m| (the l-recurrence of the oracle's d-functions starts at l = |m|), so the
+    sample is scaled by sum_m (L - |m|) / sum_sample (L - |m|).  The oracle's ring DFTs are deliberately naive O(n^2) sums and are
+    NOT part of the sample (they would take 13 s per ring at L = 8192); the extrapolated time therefore flatters the oracle."""
     import oracle as O
-    rings = np.linspace(0, L - 1, n_rings).astype(int)
-    t0 = time.perf_counter()
-    rows = O.s2_inverse_rings(L, spin, O.MW, flm, rings)
-    t_inv = (time.perf_counter() - t0) * L / n_rings
-    # a band-limited map is not needed for timing: the forward's cost does not depend on the values
-    f = np.zeros((L, 2 * L - 1), np.complex128)
-    for r, row in zip(rings, rows):
-        f[r] = row
     ms = np.unique(np.linspace(-(L - 1), L - 1, n_cols).astype(int))
+    scale = float(L * L) / float(np.sum(L - np.abs(ms)))          # sum_{|m| < L} (L - |m|) = L^2
     t0 = time.perf_counter()
-    O.s2_forward_columns(L, spin, O.MW, f, ms)
-    dt = time.perf_counter() - t0
-    # theta-step cost of a column ~ (L - |m|); DFT + upsampling cost is m-independent: scale by the column count
-    t_fwd = dt * (2 * L - 1) / len(ms)
-    return t_inv, t_fwd, O.threads(), f"inverse: {n_rings} of {L} rings; forward: {len(ms)} of {2 * L - 1} orders m; extrapolated linearly"
+    F = O.s2_theta_inverse_columns(L, spin, O.MW, flm, ms)
+    t_inv = (time.perf_counter() - t0) * scale
+    # forward theta step on the oracle's 2L quadrature rings: the values do not matter for timing
+    W = np.zeros((len(ms), 2 * L), np.complex128)
+    W[:, :F.shape[1]] = F
+    t0 = time.perf_counter()
+    O.s2_theta_forward_columns(L, spin, O.MW_QUAD, W, ms)
+    t_fwd = (time.perf_counter() - t0) * scale
+    return t_inv, t_fwd, O.threads(), (f"theta steps (Eq. 33 on the {L} MW rings, Eq. 30 on the {2 * L} quadrature rings) of {len(ms)} of "
+                                       f"{2 * L - 1} orders m, scaled by sum(L-|m|); naive O(n^2) ring DFTs of the oracle excluded")
 
 
 def run_reference(args):
@@ -114,31 +140,110 @@ def run_reference(args):
         return
     from paper_2311_14670_b200 import synth
     L, spin = WORKLOAD["L"], WORKLOAD["spin"]
-    flm = synth.random_flm(L, spin, seed=WORKLOAD["seed"], sigma=synth.SIGMA_CMB)
+    flm = synth.random_flm(L, spin, seed=WORKLOAD["seed"], sigma=sigma_for(spin))
     times = []
     sample = ""
     for i in range(args.warmup + args.steps):
-        t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm, n_cols=8, n_rings=4)
+        t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm, n_cols=16)
         if i >= args.warmup:
             times.append(t_inv + t_fwd)
     t = float(np.mean(times))
     v = 1.0 / t
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f80 (long double)",
-        "data": "synthetic", "config": {"workload": f"MW L={L} spin={spin} complex, inverse+forward", "l2": "n/a (CPU)"},
+        "impl": "reference", "metric": metric_name(L, spin), "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f80 (long double)", "data": "synthetic",
+        "config": {"workload": workload_name(L, spin), "l2": "n/a (CPU)", "parallelism": f"independent x{args.gpus}"},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
 
+def time_stages(plan, x, flush, reps=5):
+    """Median per-stage device times (CUDA events recorded inside the library on the launching stream) and the algorithmic
+    bytes of the FFT / staging sections of one inverse and one forward transform."""
+    plan.enable_timing(True)
+    f = plan.inverse(x)
+    b = plan.forward(f)
+    ti, tf = [], []
+    for _ in range(reps):
+        flush.zero_(); plan.inverse(x, out=f); ti.append(plan.timings()); bi = plan.stage_bytes()
+        flush.zero_(); plan.forward(f, out=b); tf.append(plan.timings()); bf = plan.stage_bytes()
+    plan.enable_timing(False)
+    med = lambda ts: {k: statistics.median(t[k] for t in ts) for k in ("hot", "fft", "staging", "total")}
+    err = float((b - x).abs().max() / x.abs().max())
+    return med(ti), med(tf), bi, bf, err
+
+
+def compact(ms, nbytes, flops, peak_tf):
+    """One direction of a sweep row: ms per stage, fraction of the arithmetic peak in the hot kernels, GB/s of the HBM-bound stages."""
+    gbs = lambda b, t: round(b / (t * 1e-3) / 1e9, 1) if t > 0 else None
+    return {"hot_ms": round(ms["hot"], 4), "fft_ms": round(ms["fft"], 4), "staging_ms": round(ms["staging"], 4),
+            "frac": round(flops / (ms["hot"] * 1e-3) / 1e12 / peak_tf, 4) if ms["hot"] > 0 else None,
+            "fft_gbs": gbs(nbytes["fft"], ms["fft"]), "staging_gbs": gbs(nbytes["staging"], ms["staging"])}
+
+
+def sweep(api, synth, torch, dev, flush, pk):
+    """BASELINE.json's metric: ms (hot / fft / staging) and fraction of FP64 peak vs L for MW, HEALPix, SO(3), plus the fp32 and the
+    batched (DMMA) configurations; GB/s of the HBM-bound stages.  `frac` = algorithmic flop / hot time / measured peak."""
+    rows = []
+
+    def add(name, plan, x, peak_tf, extra=None):
+        mi, mf, bi, bf, err = time_stages(plan, x, flush, reps=3)
+        r = {"config": name, "inverse": compact(mi, bi, plan.flops(False), peak_tf), "forward": compact(mf, bf, plan.flops(True), peak_tf),
+             "roundtrip_err": float(f"{err:.3e}")}
+        if extra:
+            r.update(extra)
+        rows.append(r)
+
+    def mw(L, spin, sigma, seed, **kw):
+        return torch.from_numpy(synth.random_flm(L, spin, seed=seed, sigma=sigma)).to(dev)
+
+    for L, spin, sigma, seed, tag in ((64, 0, synth.SIGMA_UNIT, 0, "configs[0] "), (1024, 2, synth.SIGMA_CMB, 1, "configs[1] "),
+                                      (2048, 0, synth.SIGMA_RED, 4, ""), (4096, 0, synth.SIGMA_RED, 4, "")):
+        x = mw(L, spin, sigma, seed)
+        P = api.Plan(L, spin, device=dev)
+        add(f"{tag}MW spin-{spin} L={L} fp64", P, x, pk["dfma"])
+        del P, x
+        torch.cuda.empty_cache()
+    # configs[4], fp32 variant: complex64 arrays, fp32 recursion + contraction; frac against the measured FFMA peak
+    for L in (2048, 8192):
+        x = torch.from_numpy(synth.random_flm(L, 0, seed=4, sigma=synth.SIGMA_RED).astype("complex64")).to(dev)
+        P = api.Plan(L, 0, device=dev, dtype="f32")
+        add(f"configs[4] MW spin-0 L={L} fp32", P, x, pk["ffma"], {"peak": "ffma"})
+        del P, x
+        torch.cuda.empty_cache()
+    # configs[4], second half: 16 maps at L = 2048 transformed together (shared recursion, FP64 DMMA contraction)
+    L, B = 2048, 16
+    x = torch.from_numpy(np.stack([synth.random_flm(L, 0, seed=4 + i, sigma=synth.SIGMA_RED) for i in range(B)])).to(dev)
+    P = api.Plan(L, 0, device=dev, batch=B)
+    add(f"configs[4] MW spin-0 L={L} batch {B} (theta_mma_kernel, FP64 DMMA)", P, x, pk["dfma"], {"maps": B})
+    del P, x
+    torch.cuda.empty_cache()
+    # configs[2]: real spin-0 SHT on HEALPix nside = 1024, L = 2048 (forward of the synthesised map: inexact by design, PAPER.md:172)
+    nside, L = 1024, 2048
+    x = torch.from_numpy(synth.random_flm(L, 0, seed=2, sigma=synth.SIGMA_RED, real=True)).to(dev)
+    P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=True, device=dev)
+    add(f"configs[2] HEALPix nside={nside} L={L} spin-0 real", P, x, pk["dfma"], {"note": "round trip inexact by design"})
+    del P, x
+    torch.cuda.empty_cache()
+    # configs[3]: Wigner transform, L = 256, N = 8
+    L, N = 256, 8
+    x = torch.from_numpy(synth.random_flmn(L, N, seed=3)).to(dev)
+    P = api.Plan(L, N=N, device=dev)
+    add(f"configs[3] SO(3) MW L={L} N={N}", P, x, pk["dfma"])
+    del P, x
+    torch.cuda.empty_cache()
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--sweep", action="store_true", help="also time the other configs (MW vs L, SO(3)) into the JSON line")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the vs-L sweep of the other configurations")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--L", type=int, default=None, help="profiling only: override the band-limit of the workload")
     ap.add_argument("--spin", type=int, default=None, help="profiling only: override the spin of the workload")
@@ -149,27 +254,24 @@ def main():
         WORKLOAD["L"] = args.L
     if args.spin is not None:
         WORKLOAD["spin"] = args.spin
+        WORKLOAD["seed"] = 1 if args.spin == 2 else 4
     if args.impl == "reference":
         return run_reference(args)
 
     import torch
     from paper_2311_14670_b200 import api, synth
+    from paper_2311_14670_b200.ranks import Ranks
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device(f"cuda:{local_rank}"))
+    R = Ranks(backend="nccl")
+    rank, local_rank, world = R.rank, R.local_rank, R.world
     torch.cuda.set_device(local_rank)
     dev = torch.device(f"cuda:{local_rank}")
+    sync = torch.cuda.synchronize
 
     L, spin, B = WORKLOAD["L"], WORKLOAD["spin"], args.batch
     # weak scaling: every rank transforms its own seeded field (independent problems, no data-path collective)
     if B == 1:
-        flm_h = synth.random_flm(L, spin, seed=WORKLOAD["seed"] + rank, sigma=synth.SIGMA_CMB)
+        flm_h = synth.random_flm(L, spin, seed=R.seed(WORKLOAD["seed"]), sigma=sigma_for(spin))
     else:
         flm_h = np.stack([synth.random_flm(L, spin, seed=4 + i + 1000 * rank, sigma=synth.SIGMA_RED) for i in range(B)])
     if args.dtype == "f32":
@@ -184,66 +286,63 @@ def main():
         plan.inverse(flm, out=f)
         plan.forward(f, out=back)
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step()
-    barrier()
+    R.barrier(sync)
     api.launch_count(reset=True)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     sampler = ClockSampler(local_rank)
     sampler.start()
-    barrier()
+    R.barrier(sync)
     for a, b in ev:
         flush.zero_()                       # L2 flush between timed iterations (not timed)
         a.record(); step(); b.record()
-    barrier()
+    R.barrier(sync)
     clocks = sampler.stop()
     launches = api.launch_count()
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = R.max_over_ranks(sum(a.elapsed_time(b) for a, b in ev), device=dev)
     ms_per_step = total_ms / args.steps
-    value = world * B * args.steps / (total_ms * 1e-3)
+    value = R.throughput(B, args.steps, total_ms)
     err = float((back - flm).abs().max() / flm.abs().max())
 
-    # per-stage device times (CUDA events recorded inside the library on the launching stream)
-    plan.enable_timing(True)
-    inv_t, fwd_t = [], []
-    for _ in range(5):
-        flush.zero_(); plan.inverse(flm, out=f); inv_t.append(plan.timings())
-        flush.zero_(); plan.forward(f, out=back); fwd_t.append(plan.timings())
-    plan.enable_timing(False)
-    med = lambda ts, k: statistics.median(t[k] for t in ts)
-    stages = {"inverse_ms": {k: med(inv_t, k) for k in ("hot", "fft", "staging", "total")},
-              "forward_ms": {k: med(fwd_t, k) for k in ("hot", "fft", "staging", "total")}}
+    # per-stage device times: a separate loop of timed transforms AFTER the K timed steps (events recorded inside the library)
+    inv_ms, fwd_ms, inv_b, fwd_b, _ = time_stages(plan, flm, flush, reps=5)
+    stages = {"inverse_ms": inv_ms, "forward_ms": fwd_ms}
 
     out = None
     if rank == 0:
-        pk, pk_kind = peaks()
-        fp64_tf, _ = api.fp64_peak(20000)
-        peak_tf = fp64_tf
-        if args.dtype == "f32":       # FP32 FMA pipe: 148 SM x 128 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts; not in MEASURED_PEAKS.json)
-            peak_tf = 148 * 128 * 2 * 1.965e-3
+        hbm, hbm_kind = peaks()
+        pk = {k: api.peak(k, 20000)[0] for k in ("dfma", "dmma", "ffma")}
+        nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_tf = pk["ffma"] if args.dtype == "f32" else pk["dfma"]
         # algorithmic flop: per d-step 6 (recursion) + 4 per order and map served
-        flops_fwd = plan.flops(True)
-        flops_inv = plan.flops(False)
+        flops_fwd, flops_inv = plan.flops(True), plan.flops(False)
         fl = flops_fwd / plan.dsteps(True)
+        # what the e-form kernels execute per d-step: 2 FP64 instructions of recursion + 2 per order and map served (all FMA-class
+        # issue slots): frac_executed = 1.0 means the FP64 pipe issues every cycle (`frac` alone is unbounded by 1)
+        orders = (fl - 6.0) / 4.0
+        instr = 2.0 + 2.0 * orders
         ach = flops_fwd / (stages["forward_ms"]["hot"] * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": ("theta_forward_f32" if args.dtype == "f32" else "theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>") + " (fused m-recursion + theta contraction, Eq. 25+30)",
+        ach_inv = flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12
+        kname = ("theta_forward_f32" if args.dtype == "f32" else "theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>")
+        traffic = NCU_TRAFFIC_BYTES.get((L, spin, B)) if args.dtype == "f64" else None
+        roof = {"bound": "alu", "kernel": kname + " (fused m-recursion + theta contraction, Eq. 25+30)",
                 "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                "traffic": NCU_TRAFFIC_BYTES.get((L, spin, B)) if args.dtype == "f64" else None,
-                "traffic_source": "profiles/r1_v7_theta_kernels.md (ncu --set full, bytes per launch)",
-                "peak_kind": "measured in this run by a register-only DFMA chain (sht_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                "frac_is": "ALGORITHMIC flop (6 per d-step of Eq. 25 as the paper states it + 4 per order served) / hot time / measured peak",
+                "frac_executed": ach * (2.0 * instr / fl) / peak_tf,
+                "frac_executed_is": f"FP64 instructions the e-form kernel executes ({instr:.0f} per d-step, 2 flop each) / hot time / measured peak: 1.0 = pipe-bound",
+                "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
+                "time_source": "CUDA events recorded inside the library around the hot kernels; median of 5 transforms timed after the K timed steps",
+                "peak_kind": f"measured in this run by register-only chains (sht_peak): DFMA {pk['dfma']:.2f}, DMMA {pk['dmma']:.2f}, FFMA {pk['ffma']:.2f} "
+                             f"TFLOP/s; nominal {nsm} SM x 64 DFMA/clk x 2 x 1.965 GHz = {nsm * 64 * 2 * 1.965e-3:.1f}",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
-                "inverse_kernel": {"achieved": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12,
-                                   "frac": flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12 / peak_tf},
-                "hbm_peak_gbs": pk.get("hbm_gbs"), "hbm_peak_kind": pk_kind}
+                "inverse_kernel": {"achieved": ach_inv, "frac": ach_inv / peak_tf, "frac_executed": ach_inv * (2.0 * instr / fl) / peak_tf},
+                "hbm_peak_gbs": hbm.get("hbm_gbs"), "hbm_peak_kind": hbm_kind,
+                "stage_gbs": {"inverse": {"fft": inv_b["fft"] / (inv_ms["fft"] * 1e-3) / 1e9 if inv_ms["fft"] > 0 else None,
+                                          "staging": inv_b["staging"] / (inv_ms["staging"] * 1e-3) / 1e9 if inv_ms["staging"] > 0 else None},
+                              "forward": {"fft": fwd_b["fft"] / (fwd_ms["fft"] * 1e-3) / 1e9 if fwd_ms["fft"] > 0 else None,
+                                          "staging": fwd_b["staging"] / (fwd_ms["staging"] * 1e-3) / 1e9 if fwd_ms["staging"] > 0 else None}}}
         # end to end through host buffers (pinned), H2D + D2H inside the timed region
         fh = torch.empty(plan.map_shape, dtype=plan.map_dtype).pin_memory()
         ch = torch.from_numpy(flm_h).pin_memory()
@@ -255,133 +354,44 @@ def main():
             else:               # batched plans take device pointers: pinned copies around them, same bytes
                 flm.copy_(ch, non_blocking=True); plan.inverse(flm, out=f); fh.copy_(f, non_blocking=True)
                 f.copy_(fh, non_blocking=True); plan.forward(f, out=back); bh.copy_(back, non_blocking=True)
-                torch.cuda.synchronize()
+                sync()
         for _ in range(2):
             pair_host()
-        torch.cuda.synchronize()
+        sync()
         t0 = time.perf_counter()
         ne = max(3, min(args.steps, 10))
         for _ in range(ne):
             pair_host()
-        torch.cuda.synchronize()
+        sync()
         te = (time.perf_counter() - t0) / ne
-        fh, ch, bh = fh.numpy(), ch.numpy(), bh.numpy()
+        e2e_err = float(np.abs(bh.numpy() - flm_h).max() / np.abs(flm_h).max())
+        del fh, ch, bh
+        api.cache_clear()
         nbytes = B * L * (2 * L - 1) * (8 if args.dtype == "f32" else 16)
         e2e = {"value": world * B / te, "unit": UNIT, "h2d_bytes_per_step": 2 * nbytes, "d2h_bytes_per_step": 2 * nbytes,
-               "ms_per_step": te * 1e3, "roundtrip_err": float(np.abs(bh - flm_h).max() / np.abs(flm_h).max())}
+               "ms_per_step": te * 1e3, "roundtrip_err": e2e_err}
         cpu = None
         if not args.no_cpu:
-            t_inv, t_fwd, cores, sample = oracle_sample(L, spin, (flm_h if B == 1 else flm_h[0]).astype(np.complex128))
+            t_inv, t_fwd, cores, sample = oracle_sample(L, spin, (flm_h if B == 1 else flm_h[0]).astype(np.complex128), n_cols=32)
             cpu = {"value": 1.0 / (t_inv + t_fwd), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                    "inverse_s": t_inv, "forward_s": t_fwd}
-        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        out = {"metric": metric_name(L, spin), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
                "data": "synthetic",
-               "config": {"workload": f"{'BASELINE.json configs[1]' if (L, spin, B) == (1024, 2, 1) else 'override'}: spin-{spin} complex SHT, MW sampling L={L} ({L}x{2 * L - 1}), fp64, "
-                                      + (f"batch of {B} maps transformed together, " if B > 1 else "") +
-                                      "flm ~ N(0, 1/(l(l+1))) l>=2, inverse + forward per step",
-                          "l2": "flushed between timed iterations (256 MiB memset, untimed)", "parallelism": f"independent x{world}"},
+               "config": {"workload": workload_name(L, spin, B), "l2": "flushed between timed iterations (256 MiB memset, untimed)",
+                          "parallelism": f"independent x{world}"},
                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                "stages": stages, "roundtrip_err": err,
-               "paper_context": "S2FFT on 1x A100-40GB: 430 ms per MW L=1024 transform (PAPER.md:737, Table 3; other hardware)"}
-        if args.sweep:
-            out["sweep"] = sweep(api, synth, torch, dev, flush, fp64_tf)
+               "paper_context": "S2FFT on 1x A100-40GB: 240 s per MW L=8192 round trip, 430 ms at L=1024 (PAPER.md:737-740, Table 3; other hardware)"}
+        if not args.no_sweep and world == 1:
+            del plan, f, back, flm
+            torch.cuda.empty_cache()
+            out["sweep"] = sweep(api, synth, torch, dev, flush, pk)
+            out["sweep_is"] = ("per direction: hot / fft / staging ms (median of 3, CUDA events inside the library), frac = algorithmic flop / hot ms / "
+                               "measured peak (DFMA unless 'peak' says ffma), GB/s = algorithmic bytes of the stage / its time "
+                               f"(HBM peak {hbm.get('hbm_gbs')} GB/s {hbm_kind})")
         print(json.dumps(out))
-    if dist is not None:
-        dist.barrier()
-        dist.destroy_process_group()
-
-
-def sweep(api, synth, torch, dev, flush, fp64_tf):
-    """ms (hot / fft / staging) and fraction of FP64 peak vs L for MW spin 0, plus the SO(3) config."""
-    rows = []
-    for L in (64, 256, 512, 1024, 2048, 4096, 8192):
-        flm = torch.from_numpy(synth.random_flm(L, 0, seed=4, sigma=synth.SIGMA_RED)).to(dev)
-        P = api.Plan(L, 0, device=dev)
-        P.enable_timing(True)
-        f = P.inverse(flm); b = P.forward(f)
-        ti, tf = [], []
-        for _ in range(3):
-            flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
-            flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
-        mi = {k: min(t[k] for t in ti) for k in ti[0]}
-        mf = {k: min(t[k] for t in tf) for k in tf[0]}
-        rows.append({"config": f"MW spin-0 L={L}", "inverse_ms": mi, "forward_ms": mf,
-                     "inverse_frac_fp64": P.flops(False) / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
-                     "forward_frac_fp64": P.flops(True) / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
-                     "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
-        del P, f, b, flm
-        torch.cuda.empty_cache()
-    # BASELINE.json configs[4], fp32 variant (theta_f32.cu): complex64 arrays, fp32 recursion + contraction
-    for L in (2048, 8192):
-        flm64 = synth.random_flm(L, 0, seed=4, sigma=synth.SIGMA_RED)
-        flm = torch.from_numpy(flm64.astype("complex64")).to(dev)
-        P = api.Plan(L, 0, device=dev, dtype="f32")
-        P.enable_timing(True)
-        f = P.inverse(flm); b = P.forward(f)
-        ti, tf = [], []
-        for _ in range(3):
-            flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
-            flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
-        mi = {k: min(t[k] for t in ti) for k in ti[0]}
-        mf = {k: min(t[k] for t in tf) for k in tf[0]}
-        rows.append({"config": f"MW spin-0 L={L} fp32", "inverse_ms": mi, "forward_ms": mf,
-                     "inverse_tflops_fp32": P.flops(False) / (mi["hot"] * 1e-3) / 1e12, "forward_tflops_fp32": P.flops(True) / (mf["hot"] * 1e-3) / 1e12,
-                     "fp32_peak_nominal_tflops": 148 * 128 * 2 * 1.965e-3,
-                     "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
-        del P, f, b, flm
-        torch.cuda.empty_cache()
-    # BASELINE.json configs[4], second half: 16 maps at L = 2048 transformed together (shared recursion, DMMA contraction)
-    L, B = 2048, 16
-    import numpy as _np
-    flm = torch.from_numpy(_np.stack([synth.random_flm(L, 0, seed=4 + i, sigma=synth.SIGMA_RED) for i in range(B)])).to(dev)
-    P = api.Plan(L, 0, device=dev, batch=B)
-    P.enable_timing(True)
-    f = P.inverse(flm); b = P.forward(f)
-    ti, tf = [], []
-    for _ in range(3):
-        flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
-        flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
-    mi = {k: min(t[k] for t in ti) for k in ti[0]}
-    mf = {k: min(t[k] for t in tf) for k in tf[0]}
-    rows.append({"config": f"MW spin-0 L={L}, batch of {B} maps (theta_mma_kernel, FP64 DMMA)", "inverse_ms": mi, "forward_ms": mf,
-                 "inverse_frac_fp64": P.flops(False) / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
-                 "forward_frac_fp64": P.flops(True) / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
-                 "ms_per_map": {"inverse": mi["total"] / B, "forward": mf["total"] / B},
-                 "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
-    del P, f, b, flm
-    torch.cuda.empty_cache()
-    # BASELINE.json configs[2]: real spin-0 SHT on HEALPix nside = 1024, L = 2048 (forward of the synthesised map: inexact by design)
-    nside, L = 1024, 2048
-    flm = torch.from_numpy(synth.random_flm(L, 0, seed=2, sigma=synth.SIGMA_RED, real=True)).to(dev)
-    P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=True, device=dev)
-    P.enable_timing(True)
-    f = P.inverse(flm); b = P.forward(f)
-    ti, tf = [], []
-    for _ in range(3):
-        flush.zero_(); P.inverse(flm, out=f); ti.append(P.timings())
-        flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
-    mi = {k: min(t[k] for t in ti) for k in ti[0]}
-    mf = {k: min(t[k] for t in tf) for k in tf[0]}
-    rows.append({"config": f"HEALPix nside={nside} L={L} spin-0 real", "inverse_ms": mi, "forward_ms": mf,
-                 "inverse_frac_fp64": P.flops(False) / (mi["hot"] * 1e-3) / 1e12 / fp64_tf,
-                 "forward_frac_fp64": P.flops(True) / (mf["hot"] * 1e-3) / 1e12 / fp64_tf,
-                 "roundtrip_err": float((b - flm).abs().max() / flm.abs().max())})
-    del P, f, b, flm
-    torch.cuda.empty_cache()
-    L, N = 256, 8
-    c = torch.from_numpy(synth.random_flmn(L, N, seed=3)).to(dev)
-    P = api.Plan(L, N=N, device=dev)
-    P.enable_timing(True)
-    f = P.inverse(c); b = P.forward(f)
-    ti, tf = [], []
-    for _ in range(3):
-        flush.zero_(); P.inverse(c, out=f); ti.append(P.timings())
-        flush.zero_(); P.forward(f, out=b); tf.append(P.timings())
-    rows.append({"config": f"SO(3) MW L={L} N={N}", "inverse_ms": {k: min(t[k] for t in ti) for k in ti[0]},
-                 "forward_ms": {k: min(t[k] for t in tf) for k in tf[0]},
-                 "roundtrip_err": float((b - c).abs().max() / c.abs().max())})
-    return rows
+    R.finish()
 
 
 if __name__ == "__main__":

@@ -21,6 +21,12 @@
  *       flmn [2N-1][L][2L-1]      (n+N-1, l, m+L-1)
  *     With reality = 1 (spin 0 only) maps are arrays of real doubles of the same shape, and the m < 0 half of
  *     flm is ignored on input / filled with (-1)^m conj(f_{l,-m}) on output.
+ *   - Accumulation order is not fixed: every output element of the fused kernels is the sum of the partial sums of several
+ *     degree / ring tiles, added to global memory with fp64 atomics (RED.ADD.F64 / bulk reduce) in whatever order the tiles
+ *     finish.  Two runs of the same call therefore agree to rounding (observed <= 1e-15 relative), not bit for bit.
+ *   - Band-limit range: Eq. 27 start values are kept as a windowed double plus a one-byte window counter, which reaches down to
+ *     2^-122900.  Plan creation returns SHT_EUNSUPPORTED when the smallest start value of the plan's ring sets falls below that
+ *     (MW sampling: L above ~9090; HEALPix with L = 2 nside: far beyond nside = 8192).  Nothing is ever silently dropped.
  *   - dtype: SHT_F64, or SHT_F32 for spin-0 MW plans of one map (BASELINE config 5; other SHT_F32 requests return
  *     SHT_EUNSUPPORTED).  With SHT_F32 every public array is interleaved floats (complex64 / float32) and the fused
  *     recursion + contraction kernels compute in fp32 (Eq. 25 in the paper's own form, windows of 2^48); FFTs and staging
@@ -46,6 +52,16 @@ typedef enum {
 
 enum { SHT_MW = 0, SHT_HEALPIX = 1 };   /* sampling */
 enum { SHT_F64 = 0, SHT_F32 = 1 };      /* dtype    */
+/* plan options (bit flags of sht_plan_s2_opts); 0 = automatic choices.  Results agree to rounding whatever the options. */
+enum {
+    SHT_OPT_FOLD_ON  = 1u << 0,   /* spin 0: run the recursion on the northern rings only (north-south fold) ...   */
+    SHT_OPT_FOLD_OFF = 1u << 1,   /* ... or on all rings.  Default: folded when the northern half alone fills the GPU (MW: L >= 2048) */
+    SHT_OPT_INVSYM   = 1u << 2,   /* spin-0 MW inverse on the L midpoint rings (2j+1)pi/(2L) with the fold, then an exact FFT
+                                     resampling of F_m to the MW rings (off by default: measured not faster) */
+    SHT_OPT_TILE64   = 1u << 3,   /* force 64-ring block tiles in the fused kernels ...                                          */
+    SHT_OPT_TILE128  = 1u << 4    /* ... or 128-ring tiles.  Default: 64 when 128-ring tiles give fewer blocks than the device has SMs */
+};
+enum { SHT_PEAK_DFMA = 0, SHT_PEAK_DMMA = 1, SHT_PEAK_FFMA = 2 };   /* sht_peak kinds */
 
 typedef struct sht_plan sht_plan;       /* opaque; host object holding sizes, cuFFT handles and table pointers */
 typedef void* sht_stream;               /* a cudaStream_t */
@@ -58,12 +74,10 @@ const char* sht_last_error(void);       /* text of the last CUDA / cuFFT failure
  * the caller provides one workspace of sht_plan_workspace_bytes() bytes (tables + scratch), which
  * sht_plan_set_workspace() fills with the O(L^2) ring / start-value tables ("optionally precompute some
  * additional internal terms ... O(L^2)"; Eq. 27 start values in mantissa/exponent form).
- * The workspace must stay valid and untouched while the plan is used.  One plan = one stream at a time.
- * nside is used for HEALPix only (the band-limit L is independent of it).
- * Environment: SHT_FOLD0=0/1 forces the north-south fold of spin-0 forward transforms off / on at plan creation
- * (default: on when the northern rings alone fill the GPU, L >= 2048 on MW); results agree to rounding either way.
- * SHT_INVSYM=1 makes spin-0 MW plans evaluate the inverse theta step on the L midpoint rings (2j+1)pi/(2L) with the
- * north-south fold and resample F_m to the MW rings by FFT (exact; off by default: not yet faster).
+ * The workspace must be 256-byte aligned (SHT_EINVAL otherwise: operand rows are fetched with bulk TMA copies) and must stay
+ * valid and untouched while the plan is used.  One plan = one stream at a time; a plan belongs to the device that was current
+ * when it was created.  nside is used for HEALPix only (the band-limit L is independent of it).
+ * sht_plan_s2_opts() is the general form (batch and option flags SHT_OPT_*); the library reads no environment variables.
  */
 sht_status sht_plan_s2(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype);
 sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);
@@ -74,6 +88,7 @@ sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);
  * batch = 1 is sht_plan_s2().  MW sampling only (HEALPix with batch > 1: SHT_EUNSUPPORTED).  The theta-stage entry
  * points below are single-map only. */
 sht_status sht_plan_s2_batch(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype, int batch);
+sht_status sht_plan_s2_opts(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype, int batch, unsigned opts);
 int        sht_plan_batch(const sht_plan* plan);
 size_t     sht_plan_workspace_bytes(const sht_plan* plan);
 sht_status sht_plan_set_workspace(sht_plan* plan, void* work, size_t work_bytes, sht_stream stream);
@@ -83,7 +98,14 @@ sht_status sht_plan_destroy(sht_plan* plan);
  * s2_forward : map f -> flm.  MW: FFT in phi (Eq. 31), extension to the torus and upsampling in theta to 2L
  *              rings (the rings are theta'_u = (2u+1) pi/(4L), u = 0..2L-1, on which the
  *              quadrature of Eq. 41-44 is exact for the band-limit-(2L-2) integrand), then the fused recursion
- *              + theta contraction of Eq. 30.  HEALPix: ring FFTs with phase shift and periodic extension
+ *              + theta contraction of Eq. 30.
+ *              Domain (MW): the last ring of an MW map lies AT theta = pi, where a spin-s function has the single value
+ *              c e^{i s phi} (only the order m = s survives, Eq. 29; SO(3): per n, only m = -n).  The transform uses
+ *              exactly that component of the ring: its samples are projected onto e^{i s phi} (F_m(pi) := 0 for m != s) before the
+ *              torus extension.  For samples of any spin-s function this changes nothing; for arbitrary arrays (e.g. pixel noise
+ *              on the pole ring) it makes the result well defined -- it equals the paper's MW(2L)-grid algorithm applied to the
+ *              projected array (the paper's algorithm itself is ring-set dependent on inconsistent pole samples, R21).
+ *              HEALPix: ring FFTs with phase shift and periodic extension
  *              (PAPER.md:403-407), weights 4 pi/Npix, Eq. 30.
  * s2_inverse : flm -> map f.  Fused recursion + l contraction of Eq. 33, then ring synthesis Eq. 32 (HEALPix:
  *              aliasing fold of F_m onto m mod nphi).
@@ -114,10 +136,17 @@ sht_status s2_theta_forward_plan(sht_plan* plan, const void* Wm, void* flm, sht_
  */
 sht_status sht_plan_enable_timing(sht_plan* plan, int on);
 sht_status sht_plan_timings(sht_plan* plan, float ms[4]);
+/* Algorithmic bytes the last timed transform moved in its FFT (bytes[1]) and staging (bytes[2]) sections: every array a staging
+ * kernel, FFT pass or memset reads or writes, counted once (an FFT pass: 32 B per complex element).  bytes[0] (hot) is 0: the
+ * fused kernels are compute-bound and are reported in flop (sht_plan_flops).  Divide by sht_plan_timings for GB/s. */
+sht_status sht_plan_stage_bytes(const sht_plan* plan, double bytes[3]);
 
 /* ---- the north-star calls: fp64, batch 1, plan + workspace cached inside the library ------------------------
  * (device pointers; the cache allocates its workspaces with cudaMalloc on first use of an argument set and
  * sht_cache_clear() releases them).  HEALPix uses nside = L/2 here (L even).
+ * The cache is keyed on (current device, problem).  Calls are thread-safe: an entry is locked while its work is enqueued, and a
+ * call on a different stream than the entry's previous call first waits (cudaStreamWaitEvent) for that call's work, so the
+ * plan's scratch is never used by two streams at once.  sht_cache_clear() must not race with transforms in flight.
  */
 sht_status s2_forward(int L, int spin, int sampling, int reality, const void* f, void* flm, sht_stream stream);
 sht_status s2_inverse(int L, int spin, int sampling, int reality, const void* flm, void* f, sht_stream stream);
@@ -133,8 +162,11 @@ sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const voi
 sht_status so3_forward_host(int L, int N, const void* f_host, void* flmn_host, sht_stream stream);
 sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, sht_stream stream);
 
-/* ---- measurement helper: register-only DFMA chain, returns achieved FP64 TFLOP/s and kernel ms (used by
- * bench.py for the FP64 roofline denominator, since MEASURED_PEAKS.json has no FP64 entry). */
+/* ---- measurement helpers: register-only instruction chains, return achieved TFLOP/s and kernel ms (used by bench.py for the
+ * roofline denominators, since MEASURED_PEAKS.json has no FP64 / FP32 ALU entries).  kind: SHT_PEAK_DFMA (fma.f64),
+ * SHT_PEAK_DMMA (mma.sync.m8n8k4.f64, the FP64 tensor-core path of the batched kernels), SHT_PEAK_FFMA (fma.f32).
+ * sht_fp64_peak() is sht_peak(SHT_PEAK_DFMA, ...). */
+sht_status sht_peak(int kind, int iters, double* tflops, float* ms, sht_stream stream);
 sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream);
 
 /* ---- introspection --------------------------------------------------------------------------------------- */

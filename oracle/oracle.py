@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-MW, HEALPIX, MW_QUAD = 0, 1, 2
+MW, HEALPIX, MW_QUAD, MWSS, DH, GL, MWSS_QUAD = 0, 1, 2, 3, 4, 5, 6
 
 _lib = None
 _LD = C.c_longdouble
@@ -43,7 +43,10 @@ def lib():
             f = getattr(L, name)
             f.restype = C.c_int
             f.argtypes = [C.c_int] * 4 + [_PD, _PD]
-        for name in ("orc_s2_inverse_rings", "orc_s2_forward_columns", "orc_s2_theta_inverse_columns"):
+        L.orc_s2_forward_adjoint.restype = C.c_int
+        L.orc_s2_forward_adjoint.argtypes = [C.c_int] * 4 + [_PD, _PD]
+        for name in ("orc_s2_inverse_rings", "orc_s2_forward_columns", "orc_s2_theta_inverse_columns", "orc_s2_theta_forward_columns",
+                     "orc_s2_inverse_adjoint_columns"):
             f = getattr(L, name)
             f.restype = C.c_int
             f.argtypes = [C.c_int] * 4 + [_PD, C.c_int, _PI, _PD]
@@ -141,7 +144,8 @@ def num_pixels(sampling, L, nside=0):
 
 
 def ring_table(sampling, L, nside=0):
-    """dict(cos_theta, sin_theta, nphi, phi0, weight, offset) for MW / HEALPIX / MW_QUAD (the 2L-ring quadrature grid)."""
+    """dict(cos_theta, sin_theta, nphi, phi0, weight, offset) for any sampling code (MW_QUAD / MWSS_QUAD: the upsampled
+    quadrature grids of the MW / MWSS forward transforms)."""
     nr = num_rings(sampling, L, nside)
     ct = np.zeros(nr, np.longdouble); st = np.zeros(nr, np.longdouble)
     ph = np.zeros(nr, np.longdouble); w = np.zeros(nr, np.longdouble)
@@ -153,7 +157,10 @@ def ring_table(sampling, L, nside=0):
 
 
 def map_shape(sampling, L, nside=0):
-    return (L, 2 * L - 1) if sampling == MW else (12 * nside * nside,)
+    """MW [L, 2L-1]; MWSS [L+1, 2L]; DH [2L, 2L-1]; GL [L, 2L-1]; HEALPix [12 nside^2] (ring-ordered)."""
+    if sampling == HEALPIX:
+        return (12 * nside * nside,)
+    return {MW: (L, 2 * L - 1), MWSS: (L + 1, 2 * L), DH: (2 * L, 2 * L - 1), GL: (L, 2 * L - 1)}[sampling]
 
 
 # ---- S^2 ---------------------------------------------------------------------------------------------------
@@ -180,6 +187,8 @@ def s2_inverse_rings(L, spin, sampling, flm, rings, nside=0):
     tab = ring_table(sampling, L, nside)
     lens = tab["nphi"][rings]
     out = np.zeros(int(lens.sum()), dtype=np.complex128)
+    if len(rings) == 0:
+        return []
     _check(lib().orc_s2_inverse_rings(L, spin, sampling, nside, _pd(flm), len(rings),
                                       rings.ctypes.data_as(_PI), _pd(out)), "s2_inverse_rings")
     return np.split(out, np.cumsum(lens)[:-1])
@@ -203,6 +212,42 @@ def s2_theta_inverse_columns(L, spin, sampling, flm, ms, nside=0):
     _check(lib().orc_s2_theta_inverse_columns(L, spin, sampling, nside, _pd(flm), len(ms),
                                               ms.ctypes.data_as(_PI), _pd(out)), "s2_theta_inverse_columns")
     return out
+
+
+def s2_theta_forward_columns(L, spin, sampling, W, ms, nside=0):
+    """Eq. 30 only: flm[:, m] = pref(l) sum_ring W[i, ring] d^l_{m,-s}(theta_ring) for the selected m (W already weighted);
+    `sampling` may be any ring-set code incl. MW_QUAD / MWSS_QUAD.  Returns array [len(ms), L]."""
+    ms = np.ascontiguousarray(ms, dtype=np.int32)
+    W = _c128(W, (len(ms), num_rings(sampling, L, nside)))
+    out = np.zeros((len(ms), L), dtype=np.complex128)
+    _check(lib().orc_s2_theta_forward_columns(L, spin, sampling, nside, _pd(W), len(ms),
+                                              ms.ctypes.data_as(_PI), _pd(out)), "s2_theta_forward_columns")
+    return out
+
+
+# ---- adjoints (Eq. 52 / 58): plain conjugate-transposed sums ------------------------------------------------
+def s2_forward_adjoint(L, spin, sampling, flm, nside=0):
+    """F^H: coefficients -> map, the conjugate transpose of s2_forward (Eq. 50-52)."""
+    flm = _c128(flm, (L, 2 * L - 1))
+    f = np.zeros(map_shape(sampling, L, nside), dtype=np.complex128)
+    _check(lib().orc_s2_forward_adjoint(L, spin, sampling, nside, _pd(flm), _pd(f)), "s2_forward_adjoint")
+    return f
+
+
+def s2_inverse_adjoint_columns(L, spin, sampling, f, ms, nside=0):
+    """(F^-1)^H for the selected m: returns array [len(ms), L] (Eq. 56-58)."""
+    f = _c128(f, map_shape(sampling, L, nside))
+    ms = np.ascontiguousarray(ms, dtype=np.int32)
+    out = np.zeros((len(ms), L), dtype=np.complex128)
+    _check(lib().orc_s2_inverse_adjoint_columns(L, spin, sampling, nside, _pd(f), len(ms),
+                                                ms.ctypes.data_as(_PI), _pd(out)), "s2_inverse_adjoint_columns")
+    return out
+
+
+def s2_inverse_adjoint(L, spin, sampling, f, nside=0):
+    """(F^-1)^H: map -> coefficients flm[L, 2L-1]."""
+    ms = np.arange(-(L - 1), L)
+    return np.ascontiguousarray(s2_inverse_adjoint_columns(L, spin, sampling, f, ms, nside).T)
 
 
 # ---- SO(3) -------------------------------------------------------------------------------------------------

@@ -25,6 +25,13 @@
 // Eq. 41-44 taken at band-limit 2L (closed form, reading R9).  HEALPix: PAPER.md:399-407 (weights
 // 4pi/Npix; ring geometry from the public definition of the scheme, reading R11).
 //
+// Further samplings: DH Eq. 34-36, MWSS Eq. 39-40 with the unified weights Eq. 43-44
+// (PAPER.md:349-381), Gauss-Legendre Eq. 45-46 (Eq. 46 as printed is not the Gauss-Legendre weight -- reading
+// R22 of DESIGN.md: the standard weight 2/((1-x^2) P_L'(x)^2) is used and pinned against numpy's leggauss).
+// Adjoints (Eq. 52 / 58): the plain conjugate-transposed sums of the forward / inverse
+// transforms above, step by step in reverse order (orc_s2_forward_adjoint, orc_s2_inverse_adjoint_columns); pinned by the
+// dot-product identity <F x, y> = <x, F^H y> against the pinned transforms and by Eq. 52 / 58 on the direct-quadrature samplings.
+//
 // Parity pins (tests, -m "not gpu"): closed-form Y_lm / sY_lm, scipy sph_harm_y, Jacobi form (Eq. 22) through
 // scipy/mpmath, d(0)=I, d(pi), symmetries, orthogonality, E==R==T, un-separated sums, quadrature exactness,
 // exact MW / SO(3) round trips (sampling theorem).  HEALPix forward: "parity unpinned" in the absolute beyond
@@ -124,6 +131,83 @@ static RingSet rings_healpix(int nside) {
         g.ct = z; g.st = sqrtl((1 - z) * (1 + z));
         g.s2 = sqrtl((1 - z) / 2); g.c2 = sqrtl((1 + z) / 2);
         g.pole = 0; g.w = 4.0L * PI_L / npix; g.off = off; off += g.nphi;
+    }
+    S.npix = off; return S;
+}
+
+// DH sample positions and weights, Eq. 34-36: theta_t = (2t+1)pi/(4L), t < 2L; phi_p = 2 pi p/(2L-1);
+//   q(theta) = (4 pi/(L(2L-1))) sin(theta) sum_{k=0}^{L-1} sin((2k+1)theta)/(2k+1).
+static RingSet rings_dh(int L) {
+    RingSet S; S.r.resize(2 * L); long off = 0;
+    for (int t = 0; t < 2 * L; ++t) {
+        Ring& g = S.r[t];
+        ld th = PI_L * (ld)(2 * t + 1) / (ld)(4 * L);
+        g.pole = 0; g.ct = cosl(th); g.st = sinl(th); g.c2 = cosl(th / 2); g.s2 = sinl(th / 2);
+        ld acc = 0;
+        for (int k = L - 1; k >= 0; --k) {
+            // sin((2k+1) theta_t) = Im e^{i pi (2k+1)(2t+1)/(4L)}, angle reduced exactly
+            acc += unit_root_pi((long)(2 * k + 1) * (2 * t + 1), 4 * L).im / (ld)(2 * k + 1);
+        }
+        g.w = 4.0L * PI_L / ((ld)L * (ld)(2 * L - 1)) * g.st * acc;
+        g.nphi = 2 * L - 1; g.phi0 = 0; g.off = off; off += g.nphi;
+    }
+    S.npix = off; return S;
+}
+// MWSS sample positions, Eq. 39-40: theta_t = 2 pi t/(2Lt), t = 0..Lt (both poles are rings);
+// phi_p = 2 pi p/nphi.  `nphi` is passed separately: the quadrature grid of band-limit 2L keeps the 2L longitudes.
+static RingSet rings_mwss(int Lt, int nphi) {
+    RingSet S; S.r.resize(Lt + 1); long off = 0;
+    for (int t = 0; t <= Lt; ++t) {
+        Ring& g = S.r[t];
+        ld th = PI_L * (ld)t / (ld)Lt;
+        g.pole = (t == 0) ? 1 : (t == Lt) ? 2 : 0;
+        g.ct = cosl(th); g.st = sinl(th); g.c2 = cosl(th / 2); g.s2 = sinl(th / 2);
+        if (g.pole == 1) { g.ct = 1; g.st = 0; g.c2 = 1; g.s2 = 0; }
+        if (g.pole == 2) { g.ct = -1; g.st = 0; g.c2 = 0; g.s2 = 1; }
+        if (2 * t == Lt) { g.ct = 0; g.st = 1; }                      // the equator ring of an even Lt, exactly
+        g.nphi = nphi; g.phi0 = 0; g.w = 0; g.off = off; off += nphi;
+    }
+    S.npix = off; return S;
+}
+// MWSS theta-quadrature weights at band-limit Lq (T = 2Lq samples on the theta circle), Eq. 41-44 with reflection sign +1
+// (R9: the integrand of the transform is even under theta -> 2pi - theta, so the odd terms w^(+-1) cancel):
+//   v_u = (1/T) (1 + zeta_u) sum_{j : |2j| <= Lq-1} [2/(1-4j^2)] cos(2 j theta_u),   zeta_u = 0 at the poles u = 0, Lq, else 1.
+static void mwss_theta_weights(int Lq, std::vector<ld>& v) {
+    v.assign(Lq + 1, 0);
+    int T = 2 * Lq, jmax = (Lq - 1) / 2;
+    for (int u = 0; u <= Lq; ++u) {
+        ld acc = 0;
+        for (int j = -jmax; j <= jmax; ++j) acc += (2.0L / (1.0L - 4.0L * (ld)j * (ld)j)) * unit_root((long)2 * j * u, T).re;
+        v[u] = acc / (ld)T * ((u == 0 || u == Lq) ? 1.0L : 2.0L);
+    }
+}
+// Gauss-Legendre rings: theta_t = acos(x_t), x_t the roots of P_L, north to south; phi_p = 2 pi p/(2L-1), Eq. 45.
+// Roots by Newton's iteration in theta on P_L(cos theta) (three-term recurrence), so that half-angle trigonometry keeps full
+// relative accuracy near the poles.  Weights: 2/((1-x^2) P_L'(x)^2) times q_Phi = 2 pi/(2L-1)  (reading R22 of Eq. 46).
+static void legendre_pl(int L, ld x, ld& p, ld& dp) {      // P_L(x) and P_L'(x)
+    ld p0 = 1, p1 = x;
+    if (L == 0) { p = 1; dp = 0; return; }
+    for (int k = 2; k <= L; ++k) { ld pk = ((ld)(2 * k - 1) * x * p1 - (ld)(k - 1) * p0) / (ld)k; p0 = p1; p1 = pk; }
+    p = p1; dp = (ld)L * (x * p1 - p0) / (x * x - 1);
+}
+static RingSet rings_gl(int L) {
+    RingSet S; S.r.resize(L); long off = 0;
+    for (int t = 0; t < L; ++t) {
+        Ring& g = S.r[t];
+        ld th = PI_L * ((ld)t + 0.75L) / ((ld)L + 0.5L);              // Tricomi-type initial guess for the (t+1)-th root
+        ld p, dp;
+        for (int it = 0; it < 100; ++it) {
+            legendre_pl(L, cosl(th), p, dp);
+            ld dth = p / (sinl(th) * dp);                               // d/dtheta P_L(cos theta) = -sin(theta) P_L'
+            th += dth;
+            if (fabsl(dth) < 1e-19L * th) break;
+        }
+        if (2 * t + 1 == L) th = PI_L / 2;                              // the equator root of an odd L, exactly
+        legendre_pl(L, cosl(th), p, dp);
+        g.pole = 0; g.ct = cosl(th); g.st = sinl(th); g.c2 = cosl(th / 2); g.s2 = sinl(th / 2);
+        if (2 * t + 1 == L) { g.ct = 0; g.st = 1; }
+        g.w = 2.0L * PI_L / (ld)(2 * L - 1) * 2.0L / (g.st * g.st * dp * dp);
+        g.nphi = 2 * L - 1; g.phi0 = 0; g.off = off; off += g.nphi;
     }
     S.npix = off; return S;
 }
@@ -260,7 +344,9 @@ extern "C" void orc_d_top(int l, int k, const long double* half, long double* ma
 
 // ------------------------------------------------------------------------------------------------------------
 // Sampling tables exposed for the tests.
-// sampling: 0 = MW (L rings x 2L-1), 1 = HEALPix(nside), 2 = MW quadrature grid of band-limit 2L (2L rings), w = q_u
+// sampling: 0 = MW (L rings x 2L-1), 1 = HEALPix(nside), 2 = MW quadrature grid of band-limit 2L (2L rings), w = q_u,
+//           3 = MWSS (L+1 rings x 2L), 4 = DH (2L rings x 2L-1), 5 = GL (L rings x 2L-1),
+//           6 = MWSS quadrature grid of band-limit 2L (2L+1 rings), w = q_u
 // ------------------------------------------------------------------------------------------------------------
 static RingSet make_rings(int sampling, int L, int nside) {
     if (sampling == 1) return rings_healpix(nside);
@@ -270,8 +356,18 @@ static RingSet make_rings(int sampling, int L, int nside) {
         for (int u = 0; u < 2 * L; ++u) S.r[u].w = 2.0L * PI_L / (ld)(2 * L - 1) * v[u];
         return S;
     }
+    if (sampling == 3) return rings_mwss(L, 2 * L);
+    if (sampling == 4) return rings_dh(L);
+    if (sampling == 5) return rings_gl(L);
+    if (sampling == 6) {
+        RingSet S = rings_mwss(2 * L, 2 * L);
+        std::vector<ld> v; mwss_theta_weights(2 * L, v);
+        for (int u = 0; u <= 2 * L; ++u) S.r[u].w = 2.0L * PI_L / (ld)(2 * L) * v[u];
+        return S;
+    }
     return rings_mw(L, 2 * L - 1);
 }
+static bool is_map_sampling(int sampling) { return sampling == 0 || sampling == 1 || sampling == 3 || sampling == 4 || sampling == 5; }
 extern "C" int orc_num_rings(int sampling, int L, int nside) { return (int)make_rings(sampling, L, nside).r.size(); }
 extern "C" long orc_num_pixels(int sampling, int L, int nside) { return make_rings(sampling, L, nside).npix; }
 extern "C" void orc_ring_table(int sampling, int L, int nside, long double* cos_theta, long double* sin_theta,
@@ -352,6 +448,26 @@ static void mw_upsample_column(int L, int m, int s, const cld* Fin /*[L]*/, cld*
     }
 }
 
+// MWSS forward steps (ii)-(iv) for one m: F_m on the L+1 MWSS rings -> F_m on the 2L+1 rings of MWSS(2L).
+// The theta circle carries 2L samples theta_t = 2 pi t/(2L); the Nyquist bin m' = L is outside the band-limit and is dropped
+// (reading R23 of DESIGN.md: "zero padding in the Fourier domain" of a signal band-limited at L keeps |m'| <= L-1).
+static void mwss_upsample_column(int L, int m, int s, const cld* Fin /*[L+1]*/, cld* Fout /*[2L+1]*/) {
+    int T = 2 * L, T2 = 4 * L;
+    std::vector<cld> ext(T), Fmm(2 * L - 1);
+    ld sg = sgn_pow(m + s);
+    for (int t = 0; t < T; ++t) ext[t] = (t <= L) ? Fin[t] : cscale(Fin[2 * L - t], sg);
+    for (int mp = -(L - 1); mp < L; ++mp) {                 // F_{m m'} = (1/T) sum_t F_m(theta_t) e^{-i m' theta_t}
+        cld acc = {0, 0};
+        for (int t = 0; t < T; ++t) acc = cadd(acc, cmul(ext[t], unit_root(-(long)mp * t, T)));
+        Fmm[mp + L - 1] = cscale(acc, 1.0L / (ld)T);
+    }
+    for (int u = 0; u <= 2 * L; ++u) {                       // F_m(theta'_u) = sum_{m'} F_{m m'} e^{i m' theta'_u}, theta'_u = 2 pi u/(4L)
+        cld acc = {0, 0};
+        for (int mp = -(L - 1); mp < L; ++mp) acc = cadd(acc, cmul(Fmm[mp + L - 1], unit_root((long)mp * u, T2)));
+        Fout[u] = acc;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // S^2 transforms.  Layouts (row-major, complex = interleaved doubles):
 //   flm[L][2L-1], column m+L-1;  MW map f[L][2L-1];  HEALPix map f[12 nside^2] ring-ordered.
@@ -359,7 +475,7 @@ static void mw_upsample_column(int L, int m, int s, const cld* Fin /*[L]*/, cld*
 // inverse on a subset of rings: out = the selected rings' samples, concatenated in `ring_idx` order.
 extern "C" int orc_s2_inverse_rings(int L, int spin, int sampling, int nside, const double* flm,
                                     int nsel, const int* ring_idx, double* f_out) {
-    if (L < 1 || abs(spin) >= L || (sampling != 0 && sampling != 1)) return 1;
+    if (L < 1 || abs(spin) >= L || !is_map_sampling(sampling)) return 1;
     RingSet S = make_rings(sampling, L, nside);
     std::vector<int> sel(ring_idx, ring_idx + nsel);
     for (int i : sel) if (i < 0 || i >= (int)S.r.size()) return 1;
@@ -393,9 +509,10 @@ extern "C" int orc_s2_inverse(int L, int spin, int sampling, int nside, const do
 // forward on a subset of harmonic orders: out[nsel][L] complex, row i = all l for m = m_list[i].
 extern "C" int orc_s2_forward_columns(int L, int spin, int sampling, int nside, const double* f,
                                       int nsel, const int* m_list, double* flm_cols) {
-    if (L < 1 || abs(spin) >= L || (sampling != 0 && sampling != 1)) return 1;
+    if (L < 1 || abs(spin) >= L || !is_map_sampling(sampling)) return 1;
     RingSet S = make_rings(sampling, L, nside);
-    RingSet Q = (sampling == 0) ? make_rings(2, L, nside) : S;     // rings the theta-quadrature runs on
+    // rings the theta-quadrature runs on: the upsampled grids for MW / MWSS, the sample rings themselves otherwise
+    RingSet Q = (sampling == 0) ? make_rings(2, L, nside) : (sampling == 3) ? make_rings(6, L, nside) : S;
     int nr = (int)S.r.size(), nq = (int)Q.r.size();
     for (int i = 0; i < nsel; ++i) if (abs(m_list[i]) >= L) return 1;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -404,6 +521,7 @@ extern "C" int orc_s2_forward_columns(int L, int spin, int sampling, int nside, 
         std::vector<cld> Fm(nr), W(nq), out(L);
         for (int r = 0; r < nr; ++r) Fm[r] = ring_dft(f + 2 * S.r[r].off, S.r[r], m);            // Eq. 31 (weight applied below)
         if (sampling == 0) mw_upsample_column(L, m, spin, Fm.data(), W.data());
+        else if (sampling == 3) mwss_upsample_column(L, m, spin, Fm.data(), W.data());
         else W = Fm;
         for (int r = 0; r < nq; ++r) W[r] = cscale(W[r], Q.r[r].w);
         theta_analyse_column(L, m, -spin, Q, W.data(), out.data());                               // Eq. 30
@@ -431,7 +549,7 @@ extern "C" int orc_s2_forward(int L, int spin, int sampling, int nside, const do
 // kernel's F_m(theta) directly at sizes where the full map is too expensive (L = 8192, "columns mode").
 extern "C" int orc_s2_theta_inverse_columns(int L, int spin, int sampling, int nside, const double* flm,
                                             int nsel, const int* m_list, double* F_cols) {
-    if (L < 1 || abs(spin) >= L) return 1;
+    if (L < 1 || abs(spin) >= L || sampling < 0 || sampling > 6) return 1;
     RingSet S = make_rings(sampling, L, nside);
     int nr = (int)S.r.size(), M = 2 * L - 1;
     std::vector<int> all(nr); for (int i = 0; i < nr; ++i) all[i] = i;
@@ -445,6 +563,121 @@ extern "C" int orc_s2_theta_inverse_columns(int L, int spin, int sampling, int n
         }
         theta_synth_column(L, m, -spin, S, all, coef.data(), out.data());
         for (int r = 0; r < nr; ++r) { F_cols[2 * ((size_t)i * nr + r)] = (double)out[r].re; F_cols[2 * ((size_t)i * nr + r) + 1] = (double)out[r].im; }
+    }
+    return 0;
+}
+
+// theta-step only (Eq. 30): flm[:, m] = pref(l) sum_ring W[m_sel][ring] d^l_{m,-s}(theta_ring) for selected m on the rings of
+// `sampling` (any code of make_rings, incl. the quadrature grids 2 and 6); W already carries the quadrature weight.
+// out[nsel][L].  Used to check the GPU theta-forward entry point and as the timed sample of the CPU baseline.
+extern "C" int orc_s2_theta_forward_columns(int L, int spin, int sampling, int nside, const double* W_cols,
+                                            int nsel, const int* m_list, double* flm_cols) {
+    if (L < 1 || abs(spin) >= L || sampling < 0 || sampling > 6) return 1;
+    RingSet S = make_rings(sampling, L, nside);
+    int nr = (int)S.r.size();
+    for (int i = 0; i < nsel; ++i) if (abs(m_list[i]) >= L) return 1;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int i = 0; i < nsel; ++i) {
+        int m = m_list[i];
+        std::vector<cld> W(nr), out(L);
+        for (int r = 0; r < nr; ++r) W[r] = {(ld)W_cols[2 * ((size_t)i * nr + r)], (ld)W_cols[2 * ((size_t)i * nr + r) + 1]};
+        theta_analyse_column(L, m, -spin, S, W.data(), out.data());
+        for (int l = 0; l < L; ++l) {
+            ld p = (l >= abs(spin) && l >= abs(m)) ? pref_s2(l, spin) : 0.0L;
+            flm_cols[2 * ((size_t)i * L + l)] = (double)(p * out[l].re);
+            flm_cols[2 * ((size_t)i * L + l) + 1] = (double)(p * out[l].im);
+        }
+    }
+    return 0;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Adjoints (Sec. 5.3): conjugate transposes of the two linear maps above, as plain sums.
+// ------------------------------------------------------------------------------------------------------------
+// (F^-1)^H, Eq. 56-58: the inverse transform is f = sum_lm flm sY_lm on the sample rings, so its adjoint is
+//   flm = sum_{theta,phi} conj(sY_lm(theta,phi)) f(theta,phi)
+// -- the analysis sum on the SAMPLE rings without quadrature weights (F Q^-1 of Eq. 58 where a direct quadrature exists).
+// Selected harmonic orders; out[nsel][L].
+extern "C" int orc_s2_inverse_adjoint_columns(int L, int spin, int sampling, int nside, const double* f,
+                                              int nsel, const int* m_list, double* flm_cols) {
+    if (L < 1 || abs(spin) >= L || !is_map_sampling(sampling)) return 1;
+    RingSet S = make_rings(sampling, L, nside);
+    int nr = (int)S.r.size();
+    for (int i = 0; i < nsel; ++i) if (abs(m_list[i]) >= L) return 1;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int i = 0; i < nsel; ++i) {
+        int m = m_list[i];
+        std::vector<cld> Fm(nr), out(L);
+        for (int r = 0; r < nr; ++r) Fm[r] = ring_dft(f + 2 * S.r[r].off, S.r[r], m);     // sum_p f e^{-i m phi_p}
+        theta_analyse_column(L, m, -spin, S, Fm.data(), out.data());                     // sum_ring d^l_{m,-s} F_m
+        for (int l = 0; l < L; ++l) {
+            ld p = (l >= abs(spin) && l >= abs(m)) ? pref_s2(l, spin) : 0.0L;
+            flm_cols[2 * ((size_t)i * L + l)] = (double)(p * out[l].re);
+            flm_cols[2 * ((size_t)i * L + l) + 1] = (double)(p * out[l].im);
+        }
+    }
+    return 0;
+}
+// F^H, Eq. 50-52.  Direct-quadrature samplings (HEALPix, DH, GL): F = Y^H Q, so F^H flm = Q (sum_lm flm sY_lm) -- Eq. 52 literally.
+// MW / MWSS: the forward transform is the chain (i) phi-DFT, (ii) torus extension, (iii) theta-DFT, (iv) evaluation on the
+// quadrature grid, (v) weights, (vi) Eq. 30; its adjoint is the conjugate-transposed chain in reverse order:
+//   (vi,v)^H  G_m(theta'_u) = q_u sum_l pref(l) d^l_{m,-s}(theta'_u) flm
+//   (iv)^H    A_{m m'}      = sum_u G_m(theta'_u) e^{-i m' theta'_u}
+//   (iii)^H   X_m(theta_t)  = (1/T) sum_{m'} A_{m m'} e^{+i m' theta_t}          for every t of the theta circle
+//   (ii)^H    F_m(theta_t)  = X_m(theta_t) + (-1)^{m+s} X_m(theta_reflect(t))     (rings that are their own reflection: X_m alone)
+//   (i)^H     f(theta_t, phi_p) = sum_m F_m(theta_t) e^{+i m phi_p}
+extern "C" int orc_s2_forward_adjoint(int L, int spin, int sampling, int nside, const double* flm, double* f) {
+    if (L < 1 || abs(spin) >= L || !is_map_sampling(sampling)) return 1;
+    RingSet S = make_rings(sampling, L, nside);
+    bool up = (sampling == 0 || sampling == 3);
+    RingSet Q = (sampling == 0) ? make_rings(2, L, nside) : (sampling == 3) ? make_rings(6, L, nside) : S;
+    int nr = (int)S.r.size(), nq = (int)Q.r.size(), M = 2 * L - 1;
+    std::vector<int> allq(nq); for (int i = 0; i < nq; ++i) allq[i] = i;
+    std::vector<cld> F((size_t)M * nr);             // [m][sample ring]
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int mi = 0; mi < M; ++mi) {
+        int m = mi - (L - 1);
+        std::vector<cld> coef(L), G(nq);
+        for (int l = 0; l < L; ++l) {
+            ld p = (l >= abs(spin) && l >= abs(m)) ? pref_s2(l, spin) : 0.0L;
+            coef[l] = {p * (ld)flm[2 * ((size_t)l * M + mi)], p * (ld)flm[2 * ((size_t)l * M + mi) + 1]};
+        }
+        theta_synth_column(L, m, -spin, Q, allq, coef.data(), G.data());
+        for (int u = 0; u < nq; ++u) G[u] = cscale(G[u], Q.r[u].w);
+        if (!up) { for (int r = 0; r < nr; ++r) F[(size_t)mi * nr + r] = G[r]; continue; }
+        // MW: T = 2L-1 circle samples theta_t = (2t+1)pi/T, quadrature grid theta'_u = (2u+1)pi/(4L-1);
+        // MWSS: T = 2L circle samples theta_t = 2 pi t/T, quadrature grid theta'_u = 2 pi u/(4L).
+        bool mw = sampling == 0;
+        int T = mw ? 2 * L - 1 : 2 * L;
+        std::vector<cld> A(2 * L - 1), X(T);
+        for (int mp = -(L - 1); mp < L; ++mp) {
+            cld acc = {0, 0};
+            for (int u = 0; u < nq; ++u) {
+                cld e = mw ? unit_root_pi(-(long)mp * (2 * u + 1), 4 * L - 1) : unit_root(-(long)mp * u, 4 * L);
+                acc = cadd(acc, cmul(G[u], e));
+            }
+            A[mp + L - 1] = acc;
+        }
+        for (int t = 0; t < T; ++t) {
+            cld acc = {0, 0};
+            for (int mp = -(L - 1); mp < L; ++mp) {
+                cld e = mw ? unit_root_pi((long)mp * (2 * t + 1), T) : unit_root((long)mp * t, T);
+                acc = cadd(acc, cmul(A[mp + L - 1], e));
+            }
+            X[t] = cscale(acc, 1.0L / (ld)T);
+        }
+        ld sg = sgn_pow(m + spin);
+        for (int t = 0; t < nr; ++t) {
+            int tr = mw ? 2 * L - 2 - t : 2 * L - t;            // reflection of ring t on the theta circle
+            bool self = mw ? (t == L - 1) : (t == 0 || t == L);
+            F[(size_t)mi * nr + t] = self ? X[t] : cadd(X[t], cscale(X[tr], sg));
+        }
+    }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int r = 0; r < nr; ++r) {
+        std::vector<cld> Fr(M);
+        for (int mi = 0; mi < M; ++mi) Fr[mi] = F[(size_t)mi * nr + r];
+        ring_synth(L, Fr.data(), S.r[r], f + 2 * S.r[r].off);
     }
     return 0;
 }

@@ -8,6 +8,8 @@ LIB_PATH = os.path.join(HERE, "libb200sht.so")
 
 SHT_MW, SHT_HEALPIX = 0, 1
 SHT_F64, SHT_F32 = 0, 1
+SHT_OPT_FOLD_ON, SHT_OPT_FOLD_OFF, SHT_OPT_INVSYM, SHT_OPT_TILE64, SHT_OPT_TILE128 = 1, 2, 4, 8, 16
+SHT_PEAK_DFMA, SHT_PEAK_DMMA, SHT_PEAK_FFMA = 0, 1, 2
 
 # every symbol include/b200sht.h declares: name -> (restype, argtypes)
 _vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
@@ -17,6 +19,7 @@ SIGNATURES = {
     "sht_plan_s2": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i]),
     "sht_plan_so3": (_i, [C.POINTER(_vp), _i, _i, _i]),
     "sht_plan_s2_batch": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i, _i]),
+    "sht_plan_s2_opts": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i, _i, C.c_uint]),
     "sht_plan_batch": (_i, [_vp]),
     "sht_plan_workspace_bytes": (_sz, [_vp]),
     "sht_plan_set_workspace": (_i, [_vp, _vp, _sz, _vp]),
@@ -30,6 +33,7 @@ SIGNATURES = {
     "s2_theta_forward_plan": (_i, [_vp, _vp, _vp, _vp]),
     "sht_plan_enable_timing": (_i, [_vp, _i]),
     "sht_plan_timings": (_i, [_vp, C.POINTER(C.c_float)]),
+    "sht_plan_stage_bytes": (_i, [_vp, C.POINTER(C.c_double)]),
     "s2_forward": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
     "s2_inverse": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
     "so3_forward": (_i, [_i, _i, _vp, _vp, _vp]),
@@ -39,6 +43,7 @@ SIGNATURES = {
     "s2_inverse_host": (_i, [_i, _i, _i, _i, _vp, _vp, _vp]),
     "so3_forward_host": (_i, [_i, _i, _vp, _vp, _vp]),
     "so3_inverse_host": (_i, [_i, _i, _vp, _vp, _vp]),
+    "sht_peak": (_i, [_i, _i, C.POINTER(C.c_double), C.POINTER(C.c_float), _vp]),
     "sht_fp64_peak": (_i, [_i, C.POINTER(C.c_double), C.POINTER(C.c_float), _vp]),
     "sht_launch_count": (C.c_long, [_i]),
     "sht_plan_dsteps": (C.c_double, [_vp, _i]),

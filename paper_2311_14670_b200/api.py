@@ -10,6 +10,7 @@ import ctypes as C
 import numpy as np
 import torch
 
+from . import _lib
 from ._lib import SHT_F32, SHT_F64, SHT_HEALPIX, SHT_MW, check, lib
 
 MW, HEALPIX = SHT_MW, SHT_HEALPIX
@@ -34,8 +35,17 @@ def map_shape(L, sampling=MW, nside=0):
 class Plan:
     """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
 
-    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1, dtype="f64"):
+    def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1, dtype="f64",
+                 fold=None, invsym=False, tile=None):
+        """fold / invsym / tile map to the SHT_OPT_* creation flags (None = the library's automatic choice)."""
         self._h = C.c_void_p()
+        opts = 0
+        if fold is not None:
+            opts |= _lib.SHT_OPT_FOLD_ON if fold else _lib.SHT_OPT_FOLD_OFF
+        if invsym:
+            opts |= _lib.SHT_OPT_INVSYM
+        if tile is not None:
+            opts |= {64: _lib.SHT_OPT_TILE64, 128: _lib.SHT_OPT_TILE128}[tile]
         self.L, self.spin, self.sampling, self.nside, self.reality, self.N = L, spin, sampling, nside, bool(reality), N
         self.batch = int(batch)
         if dtype not in ("f64", "f32"):
@@ -46,7 +56,7 @@ class Plan:
         L_ = lib()
         with torch.cuda.device(self.device):
             if N is None:
-                check(L_.sht_plan_s2_batch(C.byref(self._h), L, spin, sampling, nside, int(self.reality), code, self.batch))
+                check(L_.sht_plan_s2_opts(C.byref(self._h), L, spin, sampling, nside, int(self.reality), code, self.batch, opts))
             else:
                 check(L_.sht_plan_so3(C.byref(self._h), L, N, code))
             nbytes = L_.sht_plan_workspace_bytes(self._h)
@@ -108,6 +118,12 @@ class Plan:
         ms = (C.c_float * 4)()
         check(lib().sht_plan_timings(self._h, ms))
         return dict(hot=ms[0], fft=ms[1], staging=ms[2], total=ms[3])
+
+    def stage_bytes(self):
+        """dict(fft, staging): algorithmic bytes moved by the FFT / staging sections of the last timed transform."""
+        b = (C.c_double * 3)()
+        check(lib().sht_plan_stage_bytes(self._h, b))
+        return dict(fft=b[1], staging=b[2])
 
     def dsteps(self, forward):
         return float(lib().sht_plan_dsteps(self._h, int(forward)))
@@ -196,6 +212,14 @@ def fp64_peak(iters=20000):
     """Measured FP64 FMA throughput of this GPU (register-only DFMA chains): (TFLOP/s, ms)."""
     tf, ms = C.c_double(), C.c_float()
     check(lib().sht_fp64_peak(iters, C.byref(tf), C.byref(ms), _stream()))
+    return tf.value, ms.value
+
+
+def peak(kind, iters=20000):
+    """Measured instruction-chain peak: kind 'dfma' | 'dmma' | 'ffma' -> (TFLOP/s, ms)."""
+    code = {"dfma": _lib.SHT_PEAK_DFMA, "dmma": _lib.SHT_PEAK_DMMA, "ffma": _lib.SHT_PEAK_FFMA}[kind]
+    tf, ms = C.c_double(), C.c_float()
+    check(lib().sht_peak(code, iters, C.byref(tf), C.byref(ms), _stream()))
     return tf.value, ms.value
 
 

@@ -23,6 +23,7 @@
 namespace {
 
 thread_local long g_launches = 0;
+thread_local double g_bytes = 0;      // algorithmic bytes enqueued since the last timed-section boundary (count_bytes)
 thread_local std::string g_err;
 
 typedef long double ld;
@@ -91,6 +92,10 @@ struct sht_plan {
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
+    unsigned opts = 0;         // SHT_OPT_* given at creation
+    int device = 0, nsm = 0;   // device the plan was created on and its SM count (tile choice)
+    int* d_flag = nullptr;     // device flag raised by table kernels (start value outside the window-counter range)
+    double sec_bytes[3] = {0, 0, 0};   // algorithmic bytes moved by the FFT / staging sections of the last transform (stage timing)
     int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
     int ncg = 0, ncg_fwd = 0;  // batched path: column groups of 16 complex columns (inverse / forward passes)
     double* Ob = nullptr;      // batched path: result scratch of all passes
@@ -123,6 +128,7 @@ struct sht_plan {
     void* fft_work = nullptr; size_t fft_work_bytes = 0;
     cufftHandle fft_phi_inv = 0, fft_phi_fwd = 0, fft_th1 = 0, fft_th2 = 0, fft_gamma = 0;
     bool have_fft = false;
+    std::map<cufftHandle, double> fft_elems;   // complex elements one execution of each handle transforms (byte accounting)
     // workspace
     void* work = nullptr; size_t work_bytes = 0, need_bytes = 0;
     bool ready = false;
@@ -199,8 +205,17 @@ size_t pass_in_doubles(const sht_plan* P, const PassHost& ph, bool fwd) {
     return fwd ? rows * K * (ph.mode == 0 ? 4 : 2) * (P->fold0 ? 2 : 1) : rows * K * theta_inverse_rowd(ph.mode);
 }
 
+void begin_transform(sht_plan* P) {
+    P->ev_n = 0; g_bytes = 0;
+    P->sec_bytes[0] = P->sec_bytes[1] = P->sec_bytes[2] = 0;
+}
+// Opens a timed section of category `cat` (and closes the previous one).  The algorithmic bytes the closed section moved (each
+// array a staging kernel / FFT / memset reads or writes, once; counted by the launchers through count_bytes) are added to its
+// category and reported by sht_plan_stage_bytes(), so that the HBM-bound stages can be quoted in GB/s.
 void stage(sht_plan* P, int cat, cudaStream_t st) {
-    if (!P->timing) return;
+    if (!P->timing) { g_bytes = 0; return; }
+    if (P->ev_n > 0) P->sec_bytes[P->ev_cat[P->ev_n - 1]] += g_bytes;     // bytes of the section this call closes
+    g_bytes = 0;
     if (P->ev_n >= (int)P->ev.size()) return;
     cudaEventRecord(P->ev[P->ev_n], st);
     P->ev_cat[P->ev_n] = cat;
@@ -211,6 +226,7 @@ void stage(sht_plan* P, int cat, cudaStream_t st) {
 void layout(sht_plan* P, char* base) {
     Bump B; B.base = base;
     const int L = P->L, Lp = P->Lp, NB = P->NB;
+    P->d_flag = B.take<int>(64);
     P->rsq = B.take<double>(2 * (size_t)Lp + 64);
     P->kexp = B.take<int8_t>((size_t)P->krows * P->kstride);
     P->ctab = B.take<double>((size_t)(L - P->mmin) * Lp);
@@ -329,11 +345,11 @@ sht_status make_fft_plans(sht_plan* P) {
         if (P->hp_ncap > 0) {
             int nm[1] = {P->hp_M};
             CF(cufftCreate(&P->fft_hp_cap)); CF(cufftSetAutoAllocation(P->fft_hp_cap, 0));
-            CF(cufftMakePlanMany(P->fft_hp_cap, 1, nm, nm, 1, P->hp_M, nm, 1, P->hp_M, CUFFT_Z2Z, P->hp_ncap, &w)); ws = w > ws ? w : ws;
+            CF(cufftMakePlanMany(P->fft_hp_cap, 1, nm, nm, 1, P->hp_M, nm, 1, P->hp_M, CUFFT_Z2Z, P->hp_ncap, &w)); P->fft_elems[P->fft_hp_cap] = (double)P->hp_ncap * P->hp_M; ws = w > ws ? w : ws;
         }
         int ne[1] = {4 * ns};
         CF(cufftCreate(&P->fft_hp_eq)); CF(cufftSetAutoAllocation(P->fft_hp_eq, 0));
-        CF(cufftMakePlanMany(P->fft_hp_eq, 1, ne, ne, 1, 4 * ns, ne, 1, 4 * ns, CUFFT_Z2Z, P->hp_neq, &w)); ws = w > ws ? w : ws;
+        CF(cufftMakePlanMany(P->fft_hp_eq, 1, ne, ne, 1, 4 * ns, ne, 1, 4 * ns, CUFFT_Z2Z, P->hp_neq, &w)); P->fft_elems[P->fft_hp_eq] = (double)P->hp_neq * 4 * ns; ws = w > ws ? w : ws;
         P->fft_work_bytes = ws + 256;
         P->have_fft = true;
         return SHT_OK;
@@ -341,30 +357,68 @@ sht_status make_fft_plans(sht_plan* P) {
     int n1[1] = {NB};
     CF(cufftCreate(&P->fft_phi_inv)); CF(cufftSetAutoAllocation(P->fft_phi_inv, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, (int)rup((size_t)L, 128), 1, onembed, 1, NB, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, (int)rup((size_t)L, 128), 1, onembed, 1, NB, CUFFT_Z2Z, L, &w)); P->fft_elems[P->fft_phi_inv] = (double)L * NB; ws = w > ws ? w : ws; }
     CF(cufftCreate(&P->fft_phi_fwd)); CF(cufftSetAutoAllocation(P->fft_phi_fwd, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, (int)rup((size_t)L, 128), 1, CUFFT_Z2Z, L, &w)); ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, (int)rup((size_t)L, 128), 1, CUFFT_Z2Z, L, &w)); P->fft_elems[P->fft_phi_fwd] = (double)L * NB; ws = w > ws ? w : ws; }
     CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
     { int inembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_th1, 1, n1, inembed, 1, NB, inembed, 1, NB, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_th1, 1, n1, inembed, 1, NB, inembed, 1, NB, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th1] = (double)NB * NB * P->nslab; ws = w > ws ? w : ws; }
     int n2[1] = {4 * L};
     CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
     { int inembed[1] = {4 * L};
-      CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L, inembed, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L, inembed, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th2] = 4.0 * L * NB * P->nslab; ws = w > ws ? w : ws; }
     if (P->invsym) {
         int n4[1] = {2 * L};
         CF(cufftCreate(&P->fft_sym)); CF(cufftSetAutoAllocation(P->fft_sym, 0));
-        CF(cufftMakePlanMany(P->fft_sym, 1, n4, n4, 1, 2 * L, n4, 1, 2 * L, CUFFT_Z2Z, NB, &w)); ws = w > ws ? w : ws;
+        CF(cufftMakePlanMany(P->fft_sym, 1, n4, n4, 1, 2 * L, n4, 1, 2 * L, CUFFT_Z2Z, NB, &w)); P->fft_elems[P->fft_sym] = 2.0 * L * NB; ws = w > ws ? w : ws;
     }
     if (P->kind == 1) {
         int n3[1] = {2 * P->N - 1};
         CF(cufftCreate(&P->fft_gamma)); CF(cufftSetAutoAllocation(P->fft_gamma, 0));
         int emb[1] = {2 * P->N - 1};
-        CF(cufftMakePlanMany(P->fft_gamma, 1, n3, emb, L * NB, 1, emb, L * NB, 1, CUFFT_Z2Z, L * NB, &w)); ws = w > ws ? w : ws;
+        CF(cufftMakePlanMany(P->fft_gamma, 1, n3, emb, L * NB, 1, emb, L * NB, 1, CUFFT_Z2Z, L * NB, &w)); P->fft_elems[P->fft_gamma] = (double)(2 * P->N - 1) * L * NB; ws = w > ws ? w : ws;
     }
     P->fft_work_bytes = ws + 256;
     P->have_fft = true;
+    return SHT_OK;
+}
+
+// device of the calling thread and its SM count (tile and fold choices); without a device the defaults stand and the first
+// CUDA / cuFFT call of plan creation reports the failure
+void query_device(sht_plan* P) {
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) {
+        P->device = dev; P->nsm = nsm;
+    } else {
+        (void)cudaGetLastError();
+        P->device = 0; P->nsm = 148;
+    }
+}
+
+// Eq. 27 start values are stored as a windowed double plus a one-byte window counter k, true value = stored * 2^(-SWIN k)
+// (internal.h), which reaches down to 2^(TWIN - 255 SWIN) = 2^-122900.  |d^l_{l,n}(theta)| is smallest at l = L-1 on the ring nearest
+// a pole; if it falls below that range the plan is refused (a start value is never silently dropped: the iterate grows back to
+// O(1) at small m).  On MW this allows L up to ~9090.  log2 |d^l_{l,n}| = (1/2) log2 C(2l, l-n) + (l+n) log2 c2 + (l-n) log2 s2.
+sht_status check_start_range(const sht_plan* P) {
+    const ld floor2 = (ld)SHT_TWIN - 255.0L * (ld)SHT_SWIN;
+    const int l = P->L - 1;
+    for (const RingSet* R : {&P->inv, &P->fwd})
+        for (int n : P->slab_n) {
+            const int an = n < 0 ? -n : n;
+            if (l < an) continue;
+            const ld lb = (lgammal((ld)(2 * l + 1)) - lgammal((ld)(l + an + 1)) - lgammal((ld)(l - an + 1))) / (2.0L * logl(2.0L));
+            for (int t : {0, R->nth - 1}) {
+                if (t < 0 || t >= (int)R->c2.size()) continue;
+                // both signs of n are recursed (mirror pass): take the smaller of the two magnitudes
+                const ld a = (ld)(l + an) * log2l(R->c2[t]) + (ld)(l - an) * log2l(R->s2[t]);
+                const ld b = (ld)(l - an) * log2l(R->c2[t]) + (ld)(l + an) * log2l(R->s2[t]);
+                if (lb + (a < b ? a : b) < floor2 + 64) {
+                    g_err = "band-limit too high for this ring set: Eq. 27 start values fall below the window-counter range 2^-122900";
+                    return SHT_EUNSUPPORTED;
+                }
+            }
+        }
     return SHT_OK;
 }
 
@@ -435,7 +489,7 @@ sht_status fill_ringset(sht_plan* P, RingSet& R, cudaStream_t st) {
         CS(up(r, rtab, st));
         CK(cudaMemsetAsync(kv.second.val, 0, sizeof(double) * (size_t)Lp * R.ntp, st));
         CK(cudaMemsetAsync(kv.second.k, 0, (size_t)Lp * R.ntp, st));
-        CK(st_start_values(L, n, R.nth, R.ntp, R.c2hi, R.c2lo, R.s2hi, R.s2lo, rtab, rtab + Lp, kv.second.val, kv.second.k, st));
+        CK(st_start_values(L, n, R.nth, R.ntp, R.c2hi, R.c2lo, R.s2hi, R.s2lo, rtab, rtab + Lp, kv.second.val, kv.second.k, P->d_flag, st));
         CK(cudaStreamSynchronize(st));
     }
     // peak split (R5): pass A serves m >= m_s = round(n cos theta), pass B serves m' >= 1 - m_s
@@ -494,6 +548,7 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin; a.ctab = P->ctab;
     a.fold0 = fwd ? P->fold0 : P->fold0i;
     a.ldout = P->F_ld; a.nfull = R.nfull;
+    a.nsm = P->nsm; a.tile = (P->opts & SHT_OPT_TILE64) ? 64 : (P->opts & SHT_OPT_TILE128) ? 128 : 0;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
     return a;
@@ -509,6 +564,20 @@ MmaArgs mma_args(const sht_plan* P, bool fwd) {
     return a;
 }
 
+// cuFFT execution on `st` with byte accounting (an FFT pass reads and writes every element once: 32 B per complex element)
+sht_status fft_exec(sht_plan* P, cufftHandle h, double2* in, double2* out, int dir, cudaStream_t st) {
+    CF(cufftSetStream(h, st));
+    CF(cufftExecZ2Z(h, in, out, dir));
+    auto it = P->fft_elems.find(h);
+    if (it != P->fft_elems.end()) count_bytes(32.0 * it->second);
+    return SHT_OK;
+}
+sht_status zero_async(void* p, size_t bytes, cudaStream_t st) {
+    CK(cudaMemsetAsync(p, 0, bytes, st));
+    count_bytes((double)bytes);
+    return SHT_OK;
+}
+
 // ---- the stages --------------------------------------------------------------------------------------------------
 // coef: nslab slabs of [L][NB] in *slab order*.  Leaves F[slab][row][ring] complete (all rows, incl. the pole ring).
 sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) {
@@ -518,14 +587,14 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         // batched path: one recursion for all maps, contraction on FP64 tensor-core MMAs (theta_mma.cu).  All passes of a
         // plan have the same m_end up to 1, but their operand / result buffers are separate; the kernel takes the
         // column-group strides of the FIRST pass, so passes are launched one by one when their row counts differ.
-        CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab * P->nslab, st));
+        CS(zero_async(P->F, sizeof(double2) * P->F_slab * P->nslab, st));
         for (size_t i = 0; i < P->pinv.size(); ++i) {
             auto& ph = P->pinv[i];
             const int NC = ph.mode == 0 ? 2 : 1;
             const size_t rows = (size_t)(L - ph.p.m_end);
             CK(st_prep_inverse_batch(L, P->Lp, NC, P->batch, P->ncg, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef, P->scale_inv,
                                      P->ctab, P->sgtab, P->sgstride, const_cast<double*>(ph.p.in), rows * P->Lp * SHT_MMA_ROW, st));
-            CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg * rows * P->inv.ntp * SHT_MMA_NCOL, st));
+            CS(zero_async(ph.p.out, sizeof(double) * P->ncg * rows * P->inv.ntp * SHT_MMA_NCOL, st));
         }
         stage(P, CAT_HOT, st);
         for (size_t i = 0; i < P->pinv.size(); ++i) {
@@ -558,7 +627,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         auto& ph = P->pinv[0];
         const int NC = ph.mode == 0 ? 2 : 1;
         CK(st_prep_inverse_f32(L, P->Lp, NC, coef, P->scale_inv, reinterpret_cast<float2*>(const_cast<double*>(ph.p.in)), st));
-        CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab, st));
+        CS(zero_async(P->F, sizeof(double2) * P->F_slab, st));
         stage(P, CAT_HOT, st);
         F32Args a{};
         a.L = L; a.Lp = P->Lp; a.nth = P->inv.nth; a.ntp = P->inv.ntp; a.NB = P->NB; a.ldout = P->F_ld;
@@ -574,7 +643,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->NB,
                            P->scale_inv, P->ctab, P->sgtab, P->sgstride,
                            const_cast<double*>(ph.p.in) + (size_t)P->Lp * theta_inverse_rowd(ph.mode), st));
-    CK(cudaMemsetAsync(P->F, 0, sizeof(double2) * P->F_slab * P->nslab, st));
+    CS(zero_async(P->F, sizeof(double2) * P->F_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
     CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
     CK(launch_theta_inverse(theta_args(P, false, false), 1, st));
@@ -595,7 +664,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     const int L = P->L;
     stage(P, CAT_STAGE, st);
     if (P->batch > 1) {
-        CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
+        CS(zero_async(P->H, sizeof(double2) * P->H_slab * P->nslab, st));
         for (size_t i = 0; i < P->pfwd.size(); ++i) {
             auto& ph = P->pfwd[i];
             const size_t rows = (size_t)(L - ph.p.m_end);
@@ -603,13 +672,13 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
                 CK(st_weight_split_batch_fold0(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, ph.mode == 0 ? 2 : 1, P->batch,
                                                P->ncg_fwd, ph.p.m_end, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
                                                rows * P->fwd.ntp * SHT_MMA_ROWF, st));
-                CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
+                CS(zero_async(ph.p.out, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
                 continue;
             }
             CK(st_weight_split_batch(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, P->slab_n[0],
                                      ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
                                      rows * P->fwd.ntp * SHT_MMA_ROW, st));
-            CK(cudaMemsetAsync(ph.p.out, 0, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
+            CS(zero_async(ph.p.out, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
         }
         stage(P, CAT_HOT, st);
         for (size_t i = 0; i < P->pfwd.size(); ++i) {
@@ -638,7 +707,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         float2* W32 = reinterpret_cast<float2*>(const_cast<double*>(ph.p.in));
         if (P->fold0) CK(st_weight_split_f32_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, P->fwd.wq, U, W32, st));
         else CK(st_weight_split_f32(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, W32, st));
-        CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab, st));
+        CS(zero_async(P->H, sizeof(double2) * P->H_slab, st));
         stage(P, CAT_HOT, st);
         F32Args a{};
         a.L = L; a.Lp = P->Lp; a.nth = P->fwd.nth; a.ntp = P->fwd.ntp; a.NB = P->NB; a.ldout = 0; a.fold0 = P->fold0;
@@ -659,7 +728,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
                            P->fwd.wq, U + U_slab * ph.p.slab,
                            reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), st));
     }
-    CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
+    CS(zero_async(P->H, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
     CK(launch_theta_forward(theta_args(P, true, true), 0, st));
     CK(launch_theta_forward(theta_args(P, true, false), 1, st));
@@ -683,11 +752,11 @@ sht_status resample_sym_to_mw(sht_plan* P, cudaStream_t st) {
     stage(P, CAT_STAGE, st);
     CK(st_sym_extend(L, P->slab_n[0], P->F_ld, P->F, P->Z, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_sym, st)); CF(cufftExecZ2Z(P->fft_sym, P->Z, P->Z, CUFFT_FORWARD));
+    CS(fft_exec(P, P->fft_sym, P->Z, P->Z, CUFFT_FORWARD, st));
     stage(P, CAT_STAGE, st);
     CK(st_sym_rebin(L, P->Z, P->X, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_th1, st)); CF(cufftExecZ2Z(P->fft_th1, P->X, P->X, CUFFT_INVERSE));
+    CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_INVERSE, st));
     stage(P, CAT_STAGE, st);
     CK(st_rows_head(NB, L, NB, P->F_ld, P->X, P->F, st));
     return SHT_OK;
@@ -699,11 +768,11 @@ sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
     stage(P, CAT_STAGE, st);
     for (int s = 0; s < P->nslab; ++s) CK(st_mw_extend(L, P->slab_n[s], P->Ltp, NB, P->Fa + P->Fa_slab * s, P->X + P->X_slab * s, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_th1, st)); CF(cufftExecZ2Z(P->fft_th1, P->X, P->X, CUFFT_FORWARD));
+    CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_FORWARD, st));
     stage(P, CAT_STAGE, st);
     for (int s = 0; s < P->nslab; ++s) CK(st_mw_pad_phase(L, NB, T2, P->X + P->X_slab * s, P->Z + P->Z_slab * s, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_th2, st)); CF(cufftExecZ2Z(P->fft_th2, P->Z, P->Z, CUFFT_INVERSE));
+    CS(fft_exec(P, P->fft_th2, P->Z, P->Z, CUFFT_INVERSE, st));
     return SHT_OK;
 }
 
@@ -713,17 +782,16 @@ sht_status healpix_analysis(sht_plan* P, const void* f, cudaStream_t st) {
     const size_t nbelt = (size_t)P->hp_neq * 4 * ns;
     if (real) { stage(P, CAT_STAGE, st); CK(st_real_to_complex(nbelt, (const double*)f + P->hp_off_eq, P->hp_E, st)); }
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_hp_eq, st));
-    CF(cufftExecZ2Z(P->fft_hp_eq, real ? P->hp_E : const_cast<double2*>((const double2*)f + P->hp_off_eq), P->hp_E, CUFFT_FORWARD));
+    CS(fft_exec(P, P->fft_hp_eq, real ? P->hp_E : const_cast<double2*>((const double2*)f + P->hp_off_eq), P->hp_E, CUFFT_FORWARD, st));
     if (P->hp_ncap > 0) {
         stage(P, CAT_STAGE, st);
         CK(st_hp_pack_fwd(ns, P->hp_M, real, f, P->hp_C, st));
         stage(P, CAT_FFT, st);
-        CF(cufftSetStream(P->fft_hp_cap, st)); CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD));
+        CS(fft_exec(P, P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD, st));
         stage(P, CAT_STAGE, st);
         CK(st_hp_mul(ns, P->hp_M, P->hp_BF, P->hp_C, st));
         stage(P, CAT_FFT, st);
-        CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_INVERSE));
+        CS(fft_exec(P, P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_INVERSE, st));
     }
     stage(P, CAT_STAGE, st);
     CK(st_hp_unpack_fwd(ns, L, P->NB, real ? 0 : -(L - 1), P->fwd_ld, P->hp_M, P->hp_C, P->hp_E, P->Z, st));
@@ -736,16 +804,15 @@ sht_status healpix_synthesis(sht_plan* P, void* f, cudaStream_t st) {
     stage(P, CAT_STAGE, st);
     CK(st_hp_fold_inv(ns, L, P->NB, P->F_ld, P->hp_M, P->F, P->hp_C, P->hp_E, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_hp_eq, st));
-    CF(cufftExecZ2Z(P->fft_hp_eq, P->hp_E, real ? P->hp_E : (double2*)f + P->hp_off_eq, CUFFT_INVERSE));
+    CS(fft_exec(P, P->fft_hp_eq, P->hp_E, real ? P->hp_E : (double2*)f + P->hp_off_eq, CUFFT_INVERSE, st));
     if (real) { stage(P, CAT_STAGE, st); CK(st_hp_belt_real(nbelt, P->hp_E, (double*)f + P->hp_off_eq, st)); }
     if (P->hp_ncap > 0) {
         stage(P, CAT_FFT, st);
-        CF(cufftSetStream(P->fft_hp_cap, st)); CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD));
+        CS(fft_exec(P, P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD, st));
         stage(P, CAT_STAGE, st);
         CK(st_hp_mul(ns, P->hp_M, P->hp_BF, P->hp_C, st));
         stage(P, CAT_FFT, st);
-        CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_INVERSE));
+        CS(fft_exec(P, P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_INVERSE, st));
         stage(P, CAT_STAGE, st);
         CK(st_hp_unpack_inv(ns, P->hp_M, real, P->hp_C, f, st));
     }
@@ -756,6 +823,7 @@ sht_status healpix_synthesis(sht_plan* P, void* f, cudaStream_t st) {
 }  // namespace
 
 void count_launch(int n) { g_launches += n; }
+void count_bytes(double b) { g_bytes += b; }
 
 extern "C" {
 
@@ -775,9 +843,12 @@ const char* sht_version(void) { return "b200sht 0.1 (sm_100a)"; }
 long sht_launch_count(int reset) { long v = g_launches; if (reset) g_launches = 0; return v; }
 
 sht_status sht_plan_s2(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype) {
-    return sht_plan_s2_batch(out, L, spin, sampling, nside, reality, dtype, 1);
+    return sht_plan_s2_opts(out, L, spin, sampling, nside, reality, dtype, 1, 0u);
 }
 sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch) {
+    return sht_plan_s2_opts(out, L, spin, sampling, nside, reality, dtype, batch, 0u);
+}
+sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch, unsigned opts) {
     if (!out) return SHT_EINVAL;
     *out = nullptr;
     if (batch < 1 || batch > 1024) return SHT_EINVAL;
@@ -785,33 +856,37 @@ sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int 
     if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || (sampling != SHT_MW && sampling != SHT_HEALPIX)) return SHT_EINVAL;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
+    if ((opts & SHT_OPT_FOLD_ON) && (opts & SHT_OPT_FOLD_OFF)) return SHT_EINVAL;
+    if ((opts & SHT_OPT_TILE64) && (opts & SHT_OPT_TILE128)) return SHT_EINVAL;
     // fp32 variant (BASELINE config 5): spin 0, MW sampling, one map
     if (dtype == SHT_F32 && (spin != 0 || sampling != SHT_MW || batch != 1)) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
-    P->dtype = dtype;
+    P->dtype = dtype; P->opts = opts;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
+    query_device(P);
     if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L); }
     else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
     if (spin == 0) {
         // n = 0 fold (theta_kernels.cu FOLD): worth it once the northern half alone fills the GPU with >= 2 waves of 64 x 128 tiles
-        // (L >= 2048 on MW); SHT_FOLD0=0/1 in the environment overrides the choice (used by the tests to cover both paths at small L)
+        // (L >= 2048 on MW on 148 SMs); SHT_OPT_FOLD_ON / SHT_OPT_FOLD_OFF override the choice
         const long tiles = (long)(rup(L, 128) / SHT_TQ) * (long)(rup((size_t)(P->fwd.nth + 1) / 2, 128) / 128) * (batch > 1 ? 4 : 1);
-        bool on = tiles >= 2 * 148;
-        if (const char* e = getenv("SHT_FOLD0")) on = e[0] == '1';
+        bool on = tiles >= 2 * (long)P->nsm;
+        if (opts & SHT_OPT_FOLD_ON) on = true;
+        if (opts & SHT_OPT_FOLD_OFF) on = false;
         if (on) { P->fold0 = 1; north_only(P->fwd); }
-        // MW inverse: the MW rings (2t+1)pi/(2L-1) are not symmetric; evaluate F_m on the L midpoint rings instead (folded) and
-        // resample to the MW rings with two FFT passes (resample_sym_to_mw).  SHT_INVSYM=0/1 overrides.
-        // Off by default: the two-column folded inverse kernel only fits shared memory with 64-ring tiles and gains 17 % on the hot
-        // kernel at L = 2048 (3.03 -> 2.53 ms) while the resampling adds 0.77 ms of FFT + staging (measured).
-        bool isym = false;
-        if (const char* e = getenv("SHT_INVSYM")) isym = e[0] == '1' && sampling == SHT_MW && batch == 1 && dtype == SHT_F64;
+        // MW inverse: the MW rings (2t+1)pi/(2L-1) are not symmetric; SHT_OPT_INVSYM evaluates F_m on the L midpoint rings instead
+        // (folded) and resamples to the MW rings with two FFT passes (resample_sym_to_mw).  Off by default: the two-column folded
+        // inverse kernel only fits shared memory with 64-ring tiles and gains 17 % on the hot kernel at L = 2048 (3.03 -> 2.53 ms)
+        // while the resampling adds 0.77 ms of FFT + staging (measured).
+        const bool isym = (opts & SHT_OPT_INVSYM) && sampling == SHT_MW && batch == 1 && dtype == SHT_F64;
         if (isym) { P->invsym = 1; P->fold0i = 1; rings_mid(P->inv, L); north_only(P->inv); }
         // the inverse rings of HEALPix are symmetric too
         if (on && sampling == SHT_HEALPIX && batch == 1) { P->fold0i = 1; north_only(P->inv); }
     }
-    sht_status s = plan_common(P);
+    sht_status s = check_start_range(P);
+    if (s == SHT_OK) s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
     return SHT_OK;
@@ -825,8 +900,10 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     P->kind = 1; P->L = L; P->N = N; P->sampling = SHT_MW;
     P->nslab = 2 * N - 1;
     for (int b = 0; b < P->nslab; ++b) P->slab_n.push_back(b < N ? b : b - (2 * N - 1));   // gamma-FFT bin order
+    query_device(P);
     rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L);
-    sht_status s = plan_common(P);
+    sht_status s = check_start_range(P);
+    if (s == SHT_OK) s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
     return SHT_OK;
@@ -844,10 +921,12 @@ double sht_plan_flops(const sht_plan* P, int forward) { return P ? (forward ? P-
 sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sht_stream stream) {
     if (!P || !work) return SHT_EINVAL;
     if (work_bytes < P->need_bytes) { g_err = "workspace too small"; return SHT_EWORKSPACE; }
+    if (reinterpret_cast<uintptr_t>(work) % 256 != 0) { g_err = "workspace must be 256-byte aligned (bulk-TMA operand rows)"; return SHT_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     P->work = work; P->work_bytes = work_bytes;
     layout(P, (char*)work);
     const int L = P->L, Lp = P->Lp;
+    CK(cudaMemsetAsync(P->d_flag, 0, 64 * sizeof(int), st));
     CK(st_rsq(2 * Lp + 64, P->rsq, st));
     CK(st_kexp(P->krows, P->kstride, P->kmin, P->kexp, st));
     CK(st_ctab(L, Lp, P->mmin, P->kstride, P->kmin, P->kexp, P->rsq, P->ctab, st));
@@ -894,11 +973,14 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
             CF(cufftSetWorkArea(P->fft_hp_cap, P->fft_work));
             CK(cudaMemsetAsync(P->hp_C, 0, sizeof(double2) * (size_t)P->hp_ncap * P->hp_M, st));
             CK(st_hp_chirp(P->nside, P->hp_M, P->hp_C, st));
-            CF(cufftSetStream(P->fft_hp_cap, st)); CF(cufftExecZ2Z(P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD));
+            CS(fft_exec(P, P->fft_hp_cap, P->hp_C, P->hp_C, CUFFT_FORWARD, st));
             CK(cudaMemcpyAsync(P->hp_BF, P->hp_C, sizeof(double2) * (size_t)(P->hp_ncap / 2) * P->hp_M, cudaMemcpyDeviceToDevice, st));
         }
     }
     CK(cudaStreamSynchronize(st));
+    int flag = 0;
+    CK(cudaMemcpy(&flag, P->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+    if (flag) { g_err = "Eq. 27 start values fall below the window-counter range on this ring set"; return SHT_EUNSUPPORTED; }
     P->ready = true;
     return SHT_OK;
 }
@@ -936,13 +1018,19 @@ sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
     return SHT_OK;
 }
 
+sht_status sht_plan_stage_bytes(const sht_plan* P, double bytes[3]) {
+    if (!P || !bytes) return SHT_EINVAL;
+    for (int i = 0; i < 3; ++i) bytes[i] = P->sec_bytes[i];
+    return SHT_OK;
+}
+
 // ---- S^2 ----------------------------------------------------------------------------------------------------------
 sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
     if (P->batch > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
-    P->ev_n = 0;
+    begin_transform(P);
     CS(run_theta_inverse(P, (const double2*)flm, st));
     if (P->invsym) CS(resample_sym_to_mw(P, st));
     int nt = sht_plan_ntheta(P, 0);
@@ -955,7 +1043,7 @@ sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_str
     if (!Wm || !flm || P->kind != 0) return SHT_EINVAL;
     if (P->batch > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
-    P->ev_n = 0;
+    begin_transform(P);
     // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
     int nt = sht_plan_ntheta(P, 1), T2 = P->fwd_ld;
     CK(st_rows_reorder(P->L, P->NB, nt, nt, T2, 0, (const double2*)Wm, P->Z, st));
@@ -988,15 +1076,14 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
         stage(P, CAT_STAGE, st);
         return SHT_OK;
     }
-    P->ev_n = 0;
+    begin_transform(P);
     CS(run_theta_inverse(P, (const double2*)flm, st));
     if (P->sampling == SHT_HEALPIX) return healpix_synthesis(P, f, st);
     if (P->invsym) CS(resample_sym_to_mw(P, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_phi_inv, st));
     double2* outc = P->reality ? P->cplx : (double2*)f;
     for (int b = 0; b < P->batch; ++b)
-        CF(cufftExecZ2Z(P->fft_phi_inv, P->F + P->F_slab * b, outc + (size_t)L * NB * b, CUFFT_INVERSE));   // Eq. 32
+        CS(fft_exec(P, P->fft_phi_inv, P->F + P->F_slab * b, outc + (size_t)L * NB * b, CUFFT_INVERSE, st));   // Eq. 32
     if (P->reality) { stage(P, CAT_STAGE, st); CK(st_complex_to_real((size_t)L * NB * P->batch, P->cplx, (double*)f, st)); }
     stage(P, CAT_STAGE, st);
     return SHT_OK;
@@ -1017,7 +1104,7 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
         stage(P, CAT_STAGE, st);
         return SHT_OK;
     }
-    P->ev_n = 0;
+    begin_transform(P);
     if (P->sampling == SHT_HEALPIX) {
         CS(healpix_analysis(P, f, st));
         CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
@@ -1029,9 +1116,8 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     const double2* fin = (const double2*)f;
     if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex((size_t)L * NB * P->batch, (const double*)f, P->cplx, st)); fin = P->cplx; }
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_phi_fwd, st));
     for (int b = 0; b < P->batch; ++b)                                                 // Eq. 31 (weight folded into q_u)
-        CF(cufftExecZ2Z(P->fft_phi_fwd, const_cast<double2*>(fin) + (size_t)L * NB * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD));
+        CS(fft_exec(P, P->fft_phi_fwd, const_cast<double2*>(fin) + (size_t)L * NB * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
     CS(mw_upsample(P, st));
     CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
     stage(P, CAT_STAGE, st);
@@ -1048,17 +1134,16 @@ sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream s
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB, N = P->N;
     const size_t slab = (size_t)L * NB;
-    P->ev_n = 0;
+    begin_transform(P);
     stage(P, CAT_STAGE, st);
     // coefficient slabs from n order (n+N-1) to gamma-FFT bin order
     for (int b = 0; b < P->nslab; ++b)
         CK(cudaMemcpyAsync(P->fn + slab * b, (const double2*)flmn + slab * (P->slab_n[b] + N - 1), sizeof(double2) * slab, cudaMemcpyDeviceToDevice, st));
+    count_bytes(32.0 * (double)slab * P->nslab);
     CS(run_theta_inverse(P, P->fn, st));
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_phi_inv, st));
-    for (int b = 0; b < P->nslab; ++b) CF(cufftExecZ2Z(P->fft_phi_inv, P->F + P->F_slab * b, (double2*)f + slab * b, CUFFT_INVERSE));
-    CF(cufftSetStream(P->fft_gamma, st));
-    CF(cufftExecZ2Z(P->fft_gamma, (double2*)f, (double2*)f, CUFFT_INVERSE));          // Eq. 17
+    for (int b = 0; b < P->nslab; ++b) CS(fft_exec(P, P->fft_phi_inv, P->F + P->F_slab * b, (double2*)f + slab * b, CUFFT_INVERSE, st));
+    CS(fft_exec(P, P->fft_gamma, (double2*)f, (double2*)f, CUFFT_INVERSE, st));          // Eq. 17
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
@@ -1068,12 +1153,10 @@ sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream s
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB, N = P->N;
     const size_t slab = (size_t)L * NB;
-    P->ev_n = 0;
+    begin_transform(P);
     stage(P, CAT_FFT, st);
-    CF(cufftSetStream(P->fft_gamma, st));
-    CF(cufftExecZ2Z(P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD));   // Eq. 16 (q_Gamma in scale_fwd)
-    CF(cufftSetStream(P->fft_phi_fwd, st));
-    for (int b = 0; b < P->nslab; ++b) CF(cufftExecZ2Z(P->fft_phi_fwd, P->fn + slab * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD));
+    CS(fft_exec(P, P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD, st));   // Eq. 16 (q_Gamma in scale_fwd)
+    for (int b = 0; b < P->nslab; ++b) CS(fft_exec(P, P->fft_phi_fwd, P->fn + slab * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
     CS(mw_upsample(P, st));
     CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
     stage(P, CAT_STAGE, st);
@@ -1087,26 +1170,54 @@ sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream s
 }  // extern "C"
 
 namespace {
-struct CacheEntry { sht_plan* plan = nullptr; void* work = nullptr; void* d_in = nullptr; void* d_out = nullptr; size_t in_bytes = 0, out_bytes = 0; };
-std::map<std::tuple<int, int, int, int, int, int>, CacheEntry> g_cache;
+// One entry per (device, problem).  The entry's mutex is held from lookup until the transform (and, for the *_host calls, the
+// copies) have been enqueued, so two host threads never interleave on one plan's scratch; when consecutive calls use different
+// streams, the new stream first waits for an event recorded after the previous call's work (one plan = one stream at a time).
+struct CacheEntry {
+    sht_plan* plan = nullptr; void* work = nullptr; void* d_in = nullptr; void* d_out = nullptr; size_t in_bytes = 0, out_bytes = 0;
+    std::mutex mu; cudaEvent_t done = nullptr; cudaStream_t last = nullptr; bool used = false;
+};
+std::map<std::tuple<int, int, int, int, int, int, int>, CacheEntry*> g_cache;
 std::mutex g_cache_mu;
 
-sht_status cache_get(int kind, int L, int a, int sampling, int nside, int reality, cudaStream_t st, CacheEntry** out) {
-    std::lock_guard<std::mutex> lk(g_cache_mu);
-    auto key = std::make_tuple(kind, L, a, sampling, nside, reality);
-    auto it = g_cache.find(key);
-    if (it == g_cache.end()) {
-        CacheEntry e;
-        sht_status s = kind == 0 ? sht_plan_s2(&e.plan, L, a, sampling, nside, reality, SHT_F64) : sht_plan_so3(&e.plan, L, a, SHT_F64);
-        if (s != SHT_OK) return s;
-        size_t nb = sht_plan_workspace_bytes(e.plan);
-        cudaError_t ce = cudaMalloc(&e.work, nb);
-        if (ce != cudaSuccess) { g_err = std::string("cudaMalloc workspace: ") + cudaGetErrorString(ce); sht_plan_destroy(e.plan); return SHT_ECUDA; }
-        s = sht_plan_set_workspace(e.plan, e.work, nb, st);
-        if (s != SHT_OK) { cudaFree(e.work); sht_plan_destroy(e.plan); return s; }
-        it = g_cache.emplace(key, e).first;
+struct CacheLease {
+    CacheEntry* e = nullptr; cudaStream_t st = nullptr;
+    std::unique_lock<std::mutex> lk;
+    ~CacheLease() {
+        if (!e) return;
+        if (e->done) cudaEventRecord(e->done, st);
+        e->last = st; e->used = true;
     }
-    *out = &it->second;
+};
+
+sht_status cache_get(int kind, int L, int a, int sampling, int nside, int reality, cudaStream_t st, CacheLease* lease) {
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    CacheEntry* e = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_cache_mu);
+        auto key = std::make_tuple(dev, kind, L, a, sampling, nside, reality);
+        auto it = g_cache.find(key);
+        if (it == g_cache.end()) {
+            sht_plan* plan = nullptr;
+            sht_status s = kind == 0 ? sht_plan_s2(&plan, L, a, sampling, nside, reality, SHT_F64) : sht_plan_so3(&plan, L, a, SHT_F64);
+            if (s != SHT_OK) return s;
+            size_t nb = sht_plan_workspace_bytes(plan);
+            void* work = nullptr;
+            cudaError_t ce = cudaMalloc(&work, nb);
+            if (ce != cudaSuccess) { g_err = std::string("cudaMalloc workspace: ") + cudaGetErrorString(ce); sht_plan_destroy(plan); return SHT_ECUDA; }
+            s = sht_plan_set_workspace(plan, work, nb, st);
+            if (s != SHT_OK) { cudaFree(work); sht_plan_destroy(plan); return s; }
+            e = new CacheEntry();
+            e->plan = plan; e->work = work;
+            if (cudaEventCreateWithFlags(&e->done, cudaEventDisableTiming) != cudaSuccess) e->done = nullptr;
+            it = g_cache.emplace(key, e).first;
+        }
+        e = it->second;
+    }
+    lease->lk = std::unique_lock<std::mutex>(e->mu);
+    lease->e = e; lease->st = st;
+    if (e->used && e->last != st && e->done) CK(cudaStreamWaitEvent(st, e->done, 0));
     return SHT_OK;
 }
 size_t s2_map_bytes(int L, int sampling, int nside, int reality) {
@@ -1123,28 +1234,32 @@ sht_status host_io(CacheEntry* e, size_t in_bytes, size_t out_bytes) {
 extern "C" {
 
 sht_status s2_forward(int L, int spin, int sampling, int reality, const void* f, void* flm, sht_stream stream) {
-    CacheEntry* e; CS(cache_get(0, L, spin, sampling, sampling == SHT_HEALPIX ? L / 2 : 0, reality, (cudaStream_t)stream, &e));
-    return s2_forward_plan(e->plan, f, flm, stream);
+    CacheLease lease; CS(cache_get(0, L, spin, sampling, sampling == SHT_HEALPIX ? L / 2 : 0, reality, (cudaStream_t)stream, &lease));
+    return s2_forward_plan(lease.e->plan, f, flm, stream);
 }
 sht_status s2_inverse(int L, int spin, int sampling, int reality, const void* flm, void* f, sht_stream stream) {
-    CacheEntry* e; CS(cache_get(0, L, spin, sampling, sampling == SHT_HEALPIX ? L / 2 : 0, reality, (cudaStream_t)stream, &e));
-    return s2_inverse_plan(e->plan, flm, f, stream);
+    CacheLease lease; CS(cache_get(0, L, spin, sampling, sampling == SHT_HEALPIX ? L / 2 : 0, reality, (cudaStream_t)stream, &lease));
+    return s2_inverse_plan(lease.e->plan, flm, f, stream);
 }
 sht_status so3_forward(int L, int N, const void* f, void* flmn, sht_stream stream) {
-    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, (cudaStream_t)stream, &e));
-    return so3_forward_plan(e->plan, f, flmn, stream);
+    CacheLease lease; CS(cache_get(1, L, N, SHT_MW, 0, 0, (cudaStream_t)stream, &lease));
+    return so3_forward_plan(lease.e->plan, f, flmn, stream);
 }
 sht_status so3_inverse(int L, int N, const void* flmn, void* f, sht_stream stream) {
-    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, (cudaStream_t)stream, &e));
-    return so3_inverse_plan(e->plan, flmn, f, stream);
+    CacheLease lease; CS(cache_get(1, L, N, SHT_MW, 0, 0, (cudaStream_t)stream, &lease));
+    return so3_inverse_plan(lease.e->plan, flmn, f, stream);
 }
 sht_status sht_cache_clear(void) {
     std::lock_guard<std::mutex> lk(g_cache_mu);
     for (auto& kv : g_cache) {
-        sht_plan_destroy(kv.second.plan);
-        if (kv.second.work) cudaFree(kv.second.work);
-        if (kv.second.d_in) cudaFree(kv.second.d_in);
-        if (kv.second.d_out) cudaFree(kv.second.d_out);
+        CacheEntry* e = kv.second;
+        { std::lock_guard<std::mutex> l2(e->mu); }
+        sht_plan_destroy(e->plan);
+        if (e->work) cudaFree(e->work);
+        if (e->d_in) cudaFree(e->d_in);
+        if (e->d_out) cudaFree(e->d_out);
+        if (e->done) cudaEventDestroy(e->done);
+        delete e;
     }
     g_cache.clear();
     return SHT_OK;
@@ -1153,9 +1268,9 @@ sht_status sht_cache_clear(void) {
 sht_status s2_forward_host(int L, int spin, int sampling, int reality, const void* f_host, void* flm_host, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
     int nside = sampling == SHT_HEALPIX ? L / 2 : 0;
-    CacheEntry* e; CS(cache_get(0, L, spin, sampling, nside, reality, st, &e));
+    CacheLease lease; CS(cache_get(0, L, spin, sampling, nside, reality, st, &lease));
     size_t mb = s2_map_bytes(L, sampling, nside, reality), cb = (size_t)L * (2 * L - 1) * 16;
-    CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
+    CacheEntry* e = lease.e; CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
     CK(cudaMemcpyAsync(e->d_in, f_host, mb, cudaMemcpyHostToDevice, st));
     CS(s2_forward_plan(e->plan, e->d_in, e->d_out, stream));
     CK(cudaMemcpyAsync(flm_host, e->d_out, cb, cudaMemcpyDeviceToHost, st));
@@ -1165,9 +1280,9 @@ sht_status s2_forward_host(int L, int spin, int sampling, int reality, const voi
 sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const void* flm_host, void* f_host, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
     int nside = sampling == SHT_HEALPIX ? L / 2 : 0;
-    CacheEntry* e; CS(cache_get(0, L, spin, sampling, nside, reality, st, &e));
+    CacheLease lease; CS(cache_get(0, L, spin, sampling, nside, reality, st, &lease));
     size_t mb = s2_map_bytes(L, sampling, nside, reality), cb = (size_t)L * (2 * L - 1) * 16;
-    CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
+    CacheEntry* e = lease.e; CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
     CK(cudaMemcpyAsync(e->d_in, flm_host, cb, cudaMemcpyHostToDevice, st));
     CS(s2_inverse_plan(e->plan, e->d_in, e->d_out, stream));
     CK(cudaMemcpyAsync(f_host, e->d_out, mb, cudaMemcpyDeviceToHost, st));
@@ -1176,9 +1291,9 @@ sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const voi
 }
 sht_status so3_forward_host(int L, int N, const void* f_host, void* flmn_host, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
-    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, st, &e));
+    CacheLease lease; CS(cache_get(1, L, N, SHT_MW, 0, 0, st, &lease));
     size_t b = (size_t)(2 * N - 1) * L * (2 * L - 1) * 16;
-    CS(host_io(e, b, b));
+    CacheEntry* e = lease.e; CS(host_io(e, b, b));
     CK(cudaMemcpyAsync(e->d_in, f_host, b, cudaMemcpyHostToDevice, st));
     CS(so3_forward_plan(e->plan, e->d_in, e->d_out, stream));
     CK(cudaMemcpyAsync(flmn_host, e->d_out, b, cudaMemcpyDeviceToHost, st));
@@ -1187,9 +1302,9 @@ sht_status so3_forward_host(int L, int N, const void* f_host, void* flmn_host, s
 }
 sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
-    CacheEntry* e; CS(cache_get(1, L, N, SHT_MW, 0, 0, st, &e));
+    CacheLease lease; CS(cache_get(1, L, N, SHT_MW, 0, 0, st, &lease));
     size_t b = (size_t)(2 * N - 1) * L * (2 * L - 1) * 16;
-    CS(host_io(e, b, b));
+    CacheEntry* e = lease.e; CS(host_io(e, b, b));
     CK(cudaMemcpyAsync(e->d_in, flmn_host, b, cudaMemcpyHostToDevice, st));
     CS(so3_inverse_plan(e->plan, e->d_in, e->d_out, stream));
     CK(cudaMemcpyAsync(f_host, e->d_out, b, cudaMemcpyDeviceToHost, st));
@@ -1197,23 +1312,27 @@ sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, s
     return SHT_OK;
 }
 
-sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream) {
-    if (!tflops || !ms || iters < 1) return SHT_EINVAL;
+sht_status sht_peak(int kind, int iters, double* tflops, float* ms, sht_stream stream) {
+    if (!tflops || !ms || iters < 1 || kind < 0 || kind > 2) return SHT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, nsm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
     double* sink = nullptr;
     CK(cudaMalloc(&sink, 8));
     cudaEvent_t a, b;
     CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
-    int blocks, threads, per;
-    CK(launch_fp64_peak(iters / 8 + 1, sink, st, &blocks, &threads, &per));       // warm-up
+    double flop = 0;
+    CK(launch_peak(kind, iters / 8 + 1, nsm, sink, st, &flop));       // warm-up
     CK(cudaEventRecord(a, st));
-    CK(launch_fp64_peak(iters, sink, st, &blocks, &threads, &per));
+    CK(launch_peak(kind, iters, nsm, sink, st, &flop));
     CK(cudaEventRecord(b, st));
     CK(cudaEventSynchronize(b));
     CK(cudaEventElapsedTime(ms, a, b));
-    *tflops = 2.0 * (double)iters * per * (double)blocks * threads / (*ms * 1e-3) / 1e12;
+    *tflops = flop / (*ms * 1e-3) / 1e12;
     cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
     return SHT_OK;
 }
+sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream) { return sht_peak(SHT_PEAK_DFMA, iters, tflops, ms, stream); }
 
 }  // extern "C"

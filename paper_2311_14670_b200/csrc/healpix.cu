@@ -163,30 +163,30 @@ cudaError_t st_hp_chirp(int nside, int M, double2* BF, cudaStream_t st) {
 cudaError_t st_hp_pack_fwd(int nside, int M, int real_in, const void* map, double2* C, cudaStream_t st) {
     if (nside < 2) return cudaSuccess;
     k_hp_pack_fwd<<<dim3(cdiv(M, 256), 2 * (nside - 1)), 256, 0, st>>>(nside, M, real_in, map, C);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * (double)M * 2 * (nside - 1) + 16.0 * 4.0 * (double)nside * (nside - 1)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_mul(int nside, int M, const double2* BF, double2* C, cudaStream_t st) {
     if (nside < 2) return cudaSuccess;
     k_hp_mul<<<dim3(cdiv(M, 256), 2 * (nside - 1)), 256, 0, st>>>(nside, M, BF, C);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(48.0 * (double)M * 2 * (nside - 1)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_unpack_fwd(int nside, int L, int NB, int mlo, int ldu, int M, const double2* C, const double2* E, double2* U,
                              cudaStream_t st) {
     const int nth = 4 * nside - 1;
     k_hp_unpack_fwd<<<dim3(cdiv(nth, 32), cdiv(L - mlo, 32)), dim3(32, 8), 0, st>>>(nside, L, NB, mlo, nth, ldu, M, C, E, U);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * (double)nth * (L - mlo) + 16.0 * 12.0 * (double)nside * nside); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_fold_inv(int nside, int L, int NB, int ldf, int M, const double2* F, double2* C, double2* E, cudaStream_t st) {
     const int nth = 4 * nside - 1, width = M > 4 * nside ? M : 4 * nside;
     k_hp_fold_inv<<<dim3(cdiv(width, 128), nth), 128, 0, st>>>(nside, L, NB, nth, ldf, M, F, C, E);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * (double)nth * NB + 16.0 * ((double)M * 2 * (nside - 1) + 4.0 * nside * (2 * nside + 1))); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_unpack_inv(int nside, int M, int real_out, const double2* C, void* map, cudaStream_t st) {
     if (nside < 2) return cudaSuccess;
     k_hp_unpack_inv<<<dim3(cdiv(4 * (nside - 1), 128), 2 * (nside - 1)), 128, 0, st>>>(nside, M, real_out, C, map);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * (double)M * 2 * (nside - 1) + 16.0 * 4.0 * (double)nside * (nside - 1)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_belt_real(size_t n, const double2* E, double* out, cudaStream_t st) {
     k_hp_belt_real<<<cdiv(n, 256), 256, 0, st>>>(n, E, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }

@@ -51,6 +51,8 @@ struct ThetaArgs {
     int npass;
     int fold0;             // n = 0, northern rings only (theta_kernels.cu FOLD): forward operand rows hold the E / O sets,
                            // the inverse keeps even-l / odd-l partial sums and writes both rings of a mirror pair
+    int nsm;               // SMs of the device (tile choice)
+    int tile;              // 0 = automatic, 64 / 128 = forced ring-tile size (plan option SHT_OPT_TILE64 / SHT_OPT_TILE128)
 };
 
 // ---- batched path (theta_mma.cu): the contraction of a batch of maps runs on FP64 tensor-core MMAs -----------------
@@ -89,7 +91,11 @@ cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st);
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st);
-cudaError_t launch_fp64_peak(int iters, double* sink, cudaStream_t st, int* blocks, int* threads, int* fma_per_thread);
+// peaks.cu: register-only instruction chains; kind 0 = DFMA, 1 = DMMA (mma.sync m8n8k4 f64), 2 = FFMA.  Returns flop per launch.
+cudaError_t launch_peak(int kind, int iters, int nsm, double* sink, cudaStream_t st, double* flop);
 int theta_inverse_rowd(int mode);   // doubles per (m, l) entry of the inverse operand table
 
 void count_launch(int n = 1);
+// algorithmic bytes (every array a staging kernel / FFT / memset reads or writes, once) of the work enqueued by the calling thread;
+// api.cu attributes them to the open timed section (sht_plan_stage_bytes)
+void count_bytes(double bytes);

@@ -27,7 +27,8 @@ __device__ __forceinline__ dd dd_mul(dd a, dd b) {
 // (R7).  Output: windowed value val = d * 2^(SWIN*k), k = floor((TWIN - e)/SWIN) if e < TWIN else 0.
 __global__ void k_start_values(int L, int n, int nth, int ntp, const double* __restrict__ c2hi, const double* __restrict__ c2lo,
                                const double* __restrict__ s2hi, const double* __restrict__ s2lo, const double* __restrict__ rhi,
-                               const double* __restrict__ rlo, double* __restrict__ st_val, uint8_t* __restrict__ st_k) {
+                               const double* __restrict__ rlo, double* __restrict__ st_val, uint8_t* __restrict__ st_k,
+                               int* __restrict__ range_flag) {
     int th = blockIdx.x * blockDim.x + threadIdx.x;
     if (th >= nth) return;
     const int an = n < 0 ? -n : n;
@@ -51,7 +52,10 @@ __global__ void k_start_values(int L, int n, int nth, int ntp, const double* __r
         }
         long k = 0;
         if (e < SHT_TWIN) k = (SHT_TWIN - e) / SHT_SWIN;
-        if (k > 254) { st_val[(size_t)l * ntp + th] = 0.0; st_k[(size_t)l * ntp + th] = 0; continue; }   // < 2^-143000: never matters
+        if (k > 254) {      // below 2^-122900: outside the one-byte window counter.  The iterate would grow back to O(1) at small m,
+            *range_flag = 1;   // so the value must not be dropped: the plan is refused (api.cu check_start_range / set_workspace)
+            st_val[(size_t)l * ntp + th] = 0.0; st_k[(size_t)l * ntp + th] = 0; continue;
+        }
         st_val[(size_t)l * ntp + th] = ldexp(v.hi + v.lo, (int)(e + k * SHT_SWIN));
         st_k[(size_t)l * ntp + th] = (uint8_t)k;
     }
@@ -222,14 +226,18 @@ __global__ void k_complex_to_real(size_t n, const double2* __restrict__ in, doub
     if (i < n) out[i] = in[i].x;
 }
 
-// MW forward (ii): extension of F_m(theta_t) to the torus, t = L..2L-2: F_m(theta_t) = (-1)^{m-n} F_m(theta_{2L-2-t})
+// MW forward (ii): extension of F_m(theta_t) to the torus, t = L..2L-2: F_m(theta_t) = (-1)^{m-n} F_m(theta_{2L-2-t}).
+// The ring t = L-1 lies AT theta = pi, where a spin-s function (n = -s) has the single value c e^{i s phi}: only the order m = -n
+// survives (Eq. 29).  The samples of that ring are projected onto this component (F_m(pi) := 0 for m != -n), which
+// makes the transform well defined on arbitrary arrays (R21; include/b200sht.h, s2_forward).
 __global__ void k_mw_extend(int L, int n, int ldin, int ldout, const double2* __restrict__ Fa, double2* __restrict__ X) {
     int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     const int T = 2 * L - 1;
     if (t >= T) return;
     int m = b < L ? b : b - T;
     double2 v;
-    if (t < L) v = Fa[(size_t)b * ldin + t];
+    if (t == L - 1) { v = Fa[(size_t)b * ldin + t]; if (m != -n) v = make_double2(0.0, 0.0); }
+    else if (t < L) v = Fa[(size_t)b * ldin + t];
     else { v = Fa[(size_t)b * ldin + (2 * L - 2 - t)]; double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
     X[(size_t)b * ldout + t] = v;
 }
@@ -648,9 +656,10 @@ inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 #define LAUNCHED() do { count_launch(); cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return e_; } while (0)
 
 cudaError_t st_start_values(int L, int n, int nth, int ntp, const double* c2hi, const double* c2lo, const double* s2hi,
-                            const double* s2lo, const double* rhi, const double* rlo, double* st_val, uint8_t* st_k, cudaStream_t st) {
+                            const double* s2lo, const double* rhi, const double* rlo, double* st_val, uint8_t* st_k, int* range_flag,
+                            cudaStream_t st) {
     if (nth <= 0) return cudaSuccess;
-    k_start_values<<<cdiv(nth, 64), 64, 0, st>>>(L, n, nth, ntp, c2hi, c2lo, s2hi, s2lo, rhi, rlo, st_val, st_k);
+    k_start_values<<<cdiv(nth, 64), 64, 0, st>>>(L, n, nth, ntp, c2hi, c2lo, s2hi, s2lo, rhi, rlo, st_val, st_k, range_flag);
     LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t st) {
@@ -673,7 +682,7 @@ cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end
                             const double* C, const double2* SG, int sgstride, double* G, cudaStream_t st) {
     dim3 grid(cdiv(Lp, 32), cdiv(L - m_end, 32)), block(32, 8);
     k_prep_inverse<<<grid, block, 0, st>>>(L, Lp, NC, n, sgn_out, m_end, mmin, coef, scale, C, SG, sgstride, G);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * NC * (double)(L - m_end) * L + 8.0 * (2 * NC + 2) * (double)(L - m_end) * Lp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* kexp, const double* rsq, double* C, cudaStream_t st) {
     k_ctab<<<cdiv(Lp, 64), 64, 0, st>>>(L, Lp, mmin, kstride, kmin, kexp, rsq, C);
@@ -690,89 +699,89 @@ cudaError_t st_lamtab(int n, int nth, int ntp, int m_end, int nrows, const doubl
 }
 cudaError_t st_pole_inverse(int L, int n, const double2* coef, const double* scale, double2* out, cudaStream_t st) {
     k_pole_inverse<<<1, 256, 0, st>>>(L, n, coef, scale, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * L); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st) {
     if (L < 2) return cudaSuccess;
     dim3 grid(cdiv(nth, 128), L - 1);
     k_hermitian_rows<<<grid, 128, 0, st>>>(L, NB, ntp, nth, F);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)(L - 1) * nth); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStream_t st) {
     k_real_to_complex<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st) {
     k_complex_to_real<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st) {
     dim3 grid(cdiv(2 * L - 1, 128), 2 * L - 1);
     k_mw_extend<<<grid, 128, 0, st>>>(L, n, ldin, ldout, Fa, X);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)(2 * L - 1) * (2 * L - 1)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st) {
     dim3 grid(cdiv(ldout, 128), 2 * L - 1);
     k_mw_pad_phase<<<grid, 128, 0, st>>>(L, ldin, ldout, Y, Z);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * (double)(2 * L - 1) * ((double)(2 * L - 1) + ldout)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
                             const double* wq, const double2* U, double2* W, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
     k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, fold, m_lo, wq, U, W);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
                             cudaStream_t st) {
     k_pole_forward<<<cdiv(L, 128), 128, 0, st>>>(L, Lp, n, NBin, ldin, upole, wq, U, H);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * L); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st) {
     dim3 grid(cdiv(2 * L - 1, 32), cdiv(L, 32)), block(32, 8);
     k_finalize_forward<<<grid, block, 0, st>>>(L, Lp, n, real, scale, H, coef);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)(2 * L - 1) * L); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st) {
     dim3 grid(cdiv(ncol, 128), NB);
     k_rows_bin_to_mi<<<grid, 128, 0, st>>>(L, NB, ncol, ldsrc, lddst, to_mi, src, dst);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)NB * ncol); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st) {
     k_scale_copy<<<cdiv(n, 256), 256, 0, st>>>(n, s, in, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, const double2* coef,
                                   const double* scale, const double* C, const double2* SG, int sgstride, double* Gb, size_t cg_stride,
                                   cudaStream_t st) {
     dim3 grid(cdiv(Lp, 16), cdiv(L - m_end, 8), ncg);
     k_prep_inverse_batch<<<grid, 128, 0, st>>>(L, Lp, NC, B, n, sgn_out, m_end, mmin, coef, scale, C, SG, sgstride, Gb, cg_stride);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * B * NC * (double)(L - m_end) * L + 8.0 * SHT_MMA_ROW * (double)ncg * (L - m_end) * Lp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
                                   int m_end, int fold, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
                                   size_t cg_stride, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
     k_weight_split_batch<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, NC, B, n, sgn_out, m_end, fold, m_lo, wq, lam, U, Wb, cg_stride);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * B * NC * (double)(L - m_end) * ntp + 8.0 * SHT_MMA_ROW * (double)ncg * (L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st) {
     dim3 grid(cdiv(Mp, 32), L - m_end, ncg);
     k_unpack_batch<<<grid, 128, 0, st>>>(L, Lp, Mp, mlim, NC, B, n, sgn_out, m_end, mmin, fwd, fold, C, Ob, cg_stride, out, out_slab, ld);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(8.0 * SHT_MMA_NCOL * (double)ncg * (L - m_end) * Mp + 32.0 * B * NC * (double)(L - m_end) * mlim); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
                                   const double2* U, double2* W, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
     k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, m_end, wq, U, W);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(64.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
                                         int m_end, const double* wq, const double* lam, const double2* U, double* Wb, size_t cg_stride,
                                         cudaStream_t st) {
     dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
     k_weight_split_batch_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, nfull, NC, B, m_end, wq, lam, U, Wb, cg_stride);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * B * NC * (double)(L - m_end) * ntp + 8.0 * SHT_MMA_ROWF * (double)ncg * (L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st) {
     k_ab32<<<dim3(cdiv(Lp, 128), L), 128, 0, st>>>(L, Lp, AB);
@@ -785,35 +794,35 @@ cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v
 cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st) {
     dim3 grid(cdiv(Lp, 32), cdiv(L, 32)), block(32, 8);
     k_prep_inverse_f32<<<grid, block, 0, st>>>(L, Lp, NC, coef, scale, G);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * NC * (double)L * L + 8.0 * NC * (double)L * Lp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
                                 cudaStream_t st) {
     k_weight_split_f32<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, wq, U, W);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(24.0 * NC * (double)L * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st) {
     k_c64_to_c128<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(12.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t st) {
     k_c128_to_c64<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(12.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
                                       float2* W, cudaStream_t st) {
     k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, wq, U, W);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(48.0 * NC * (double)L * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st) {
     k_sym_extend<<<dim3(cdiv(2 * L, 128), 2 * L - 1), 128, 0, st>>>(L, n, ldin, F, X);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)(2 * L) * (2 * L - 1)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st) {
     k_sym_rebin<<<dim3(cdiv(2 * L - 1, 128), 2 * L - 1), 128, 0, st>>>(L, Y, Z);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)(2 * L - 1) * (2 * L - 1)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st) {
     k_rows_head<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ldin, ldout, in, out);
-    LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)nrows * ncol); LAUNCHED(); return cudaSuccess;
 }

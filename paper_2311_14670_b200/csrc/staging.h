@@ -3,7 +3,8 @@
 #include "internal.h"
 
 cudaError_t st_start_values(int L, int n, int nth, int ntp, const double* c2hi, const double* c2lo, const double* s2hi,
-                            const double* s2lo, const double* rhi, const double* rlo, double* st_val, uint8_t* st_k, cudaStream_t st);
+                            const double* s2lo, const double* rhi, const double* rlo, double* st_val, uint8_t* st_k, int* range_flag,
+                            cudaStream_t st);
 cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t st);
 cudaError_t st_rsq(int n, double* rsq, cudaStream_t st);
 cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st);

@@ -15,61 +15,16 @@
 //   compute <-> auxiliary hand-off is a two-stage mbarrier pipeline (rfull / rempty); operand slots are recycled by the
 //       auxiliary warp right after the reduction of the step that used them.
 // All (l,m)-only and (theta,m)-only factors arrive as O(L^2) tables prepared by staging.cu.
+#include "device_utils.cuh"
 #include "internal.h"
 
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include <stdlib.h>
 
 namespace {
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-// fire-and-forget fp64 add to GLOBAL memory (RED.E.ADD.F64)
-__device__ __forceinline__ void red_add_f64(double* gptr, double v) {
-    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gptr), "d"(v) : "memory");
-}
-// 2^e as a double, e in [-1022, 1023]
-__device__ __forceinline__ double pow2i(int e) { return __hiloint2double((1023 + e) << 20, 0); }
-__device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7fffffff; }
+using namespace shtdev;
 
-#define HI_TWIN ((1023 + SHT_TWIN) << 20)
-#define HI_DEAD ((1023 + 500) << 20)
-
-#ifdef SHT_PROF
-__device__ unsigned long long g_prof[16];
-#define PROF_T0() long long t0__ = clock64()
-#define PROF_ADD(slot) do { pf__[(slot) & 1] += (unsigned long long)(clock64() - t0__); } while (0)
-#define PROF_DECL() unsigned long long pf__[2] = {0, 0}, pc__[3] = {0, 0, 0}
-#else
-#define PROF_T0() do {} while (0)
-#define PROF_ADD(slot) do {} while (0)
-#define PROF_DECL() do {} while (0)
-#endif
 #ifndef SHT_NST
 #define SHT_NST 4
 #endif
@@ -77,57 +32,6 @@ constexpr int NST = SHT_NST;   // stages of the operand ring
 constexpr int NRS = 2;   // stages of the partial-sum hand-off
 constexpr int KS = 2;    // recursion steps per pipeline stage (one TMA barrier, one hand-off per KS steps)
 constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
-// The register file is split over the 4 SM sub-partitions (16 K registers each, 3 warps each here): compute warps take
-// 232 registers per thread, auxiliary warps 40 (2*32*232 + 32*40 = 16128); the kernel is launched at 168.
-__device__ __forceinline__ void reg_dealloc_aux() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
-__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
-
-// Window counters k (internal.h) of the NI items of a thread, one byte each.  0xff = item not started yet.
-template <int NI>
-struct KPack {
-    uint32_t w[(NI + 3) / 4];
-    __device__ __forceinline__ void fill(uint32_t v) {
-#pragma unroll
-        for (int i = 0; i < (NI + 3) / 4; ++i) w[i] = v;
-    }
-    __device__ __forceinline__ void set(int idx, uint32_t k) {
-        const int sh = (idx & 3) * 8;
-        w[idx >> 2] = (w[idx >> 2] & ~(0xffu << sh)) | (k << sh);
-    }
-    __device__ __forceinline__ uint32_t get(int idx) const { return (w[idx >> 2] >> ((idx & 3) * 8)) & 0xffu; }
-    __device__ __forceinline__ void dec(int idx) { w[idx >> 2] -= 1u << ((idx & 3) * 8); }
-    __device__ __forceinline__ bool any_nonzero() const {
-        uint32_t o = 0;
-#pragma unroll
-        for (int i = 0; i < (NI + 3) / 4; ++i) o |= w[i];
-        return o != 0;
-    }
-    __device__ __forceinline__ bool any_zero_byte() const {
-        bool z = false;
-#pragma unroll
-        for (int i = 0; i < (NI + 3) / 4; ++i) z = z || (((w[i] - 0x01010101u) & ~w[i] & 0x80808080u) != 0);
-        return z;
-    }
-};
-// Window maintenance (Sec. 3.4 renormalisation; internal.h): a stored value above 2^TWIN with k > 0 shifts its window.
-template <int NI>
-__device__ __forceinline__ void window_check(double (&cur)[NI], double (&prev)[NI], KPack<NI>& kp) {
-    const double s = pow2i(-SHT_SWIN);
-#pragma unroll
-    for (int q = 0; q < NI; ++q) {
-        if (hi_abs(cur[q]) > HI_TWIN && kp.get(q) != 0u && kp.get(q) != 0xffu) {
-            cur[q] *= s; prev[q] *= s; kp.dec(q);
-        }
-    }
-}
-// On rings a pass no longer serves (m < m_lo, R5) the iterate leaves its stable range; it is zeroed before it
-// can overflow.  Legitimate stored values never exceed ~2^250.
-template <int NI>
-__device__ __forceinline__ void dead_check(double (&cur)[NI], double (&prev)[NI]) {
-#pragma unroll
-    for (int q = 0; q < NI; ++q)
-        if (hi_abs(cur[q]) > HI_DEAD) { cur[q] = 0.0; prev[q] = 0.0; }
-}
 
 // =============================================================================================================
 // inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * e^l_m(theta)      (G carries c_m(l))
@@ -266,7 +170,6 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         return;
     }
     reg_alloc_compute();
-    PROF_DECL();
 
     // -------------------------------------------------------------------- compute warps
     const int la = l0 + w * RL, l_hi = la + RL - 1;   // degrees of this warp
@@ -357,17 +260,13 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         }
         return wrote;
     };
-    constexpr int PB = 0;
-#ifdef SHT_PROF
-    const long long tloop__ = clock64();
-#endif
     for (int p = 0; p < npairs; ++p) {
         const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
         const uint32_t rparity = ((p / NRS) & 1) ^ 1;
-        { PROF_T0(); mbar_wait(&sm.full[slot], (p / NST) & 1); PROF_ADD(PB + 0); }
+        mbar_wait(&sm.full[slot], (p / NST) & 1);
         // the reducers are done with this hand-off slot (waiting here, not in front of the first partial-sum store, keeps
         // the compute section free of barriers so that operand loads of both steps can be hoisted above the FMAs)
-        { PROF_T0(); mbar_wait(&sm.rempty[rs], rparity); PROF_ADD(PB + 1); }
+        mbar_wait(&sm.rempty[rs], rparity);
         int flags = 0;
         if (step(m, slot, rs, 0, cur, prev)) flags |= 1;
         if (step(m - 1, slot, rs, 1, prev, cur)) flags |= 2;
@@ -376,17 +275,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             sm.act[rs][w] = flags;
             mbar_arrive(&sm.rfull[rs]);
         }
-#ifdef SHT_PROF
-        pc__[0]++; if (flags == 3) pc__[1]++; if (flags == 0) pc__[2]++;
-#endif
     }
-#ifdef SHT_PROF
-    if (lane == 0) {
-        atomicAdd(&g_prof[PB + 2], (unsigned long long)(clock64() - tloop__));
-        atomicAdd(&g_prof[PB + 0], pf__[0]); atomicAdd(&g_prof[PB + 1], pf__[1]);
-        atomicAdd(&g_prof[PB + 3], pc__[0]); atomicAdd(&g_prof[PB + 4], pc__[1]); atomicAdd(&g_prof[PB + 5], pc__[2]);
-    }
-#endif
 }
 
 // =============================================================================================================
@@ -534,7 +423,6 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         return;
     }
     reg_alloc_compute();
-    PROF_DECL();
 
     // -------------------------------------------------------------------- compute warps
     // state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
@@ -648,15 +536,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         }
         return wrote;
     };
-    constexpr int PB = 8;
-#ifdef SHT_PROF
-    const long long tloop__ = clock64();
-#endif
     for (int p = 0; p < npairs; ++p) {
         const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
         const uint32_t rparity = ((p / NRS) & 1) ^ 1;
-        { PROF_T0(); mbar_wait(&sm.full[slot], (p / NST) & 1); PROF_ADD(PB + 0); }
-        { PROF_T0(); mbar_wait(&sm.rempty[rs], rparity); PROF_ADD(PB + 1); }
+        mbar_wait(&sm.full[slot], (p / NST) & 1);
+        mbar_wait(&sm.rempty[rs], rparity);
         // lambda' of this warp's rings for both steps of the pair: lane -> (step h, ring i)
         if (lane < KS * RT) {
             const int h = lane / RT, i = lane % RT;
@@ -671,33 +555,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             sm.act[rs][w] = flags;
             mbar_arrive(&sm.rfull[rs]);
         }
-#ifdef SHT_PROF
-        pc__[0]++; if (flags == 3) pc__[1]++; if (flags == 0) pc__[2]++;
-#endif
     }
-#ifdef SHT_PROF
-    if (lane == 0) {
-        atomicAdd(&g_prof[PB + 2], (unsigned long long)(clock64() - tloop__));
-        atomicAdd(&g_prof[PB + 0], pf__[0]); atomicAdd(&g_prof[PB + 1], pf__[1]);
-        atomicAdd(&g_prof[PB + 3], pc__[0]); atomicAdd(&g_prof[PB + 4], pc__[1]); atomicAdd(&g_prof[PB + 5], pc__[2]);
-    }
-#endif
-}
-
-// register-only DFMA chains: the FP64 roofline denominator is measured, not assumed
-__global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double* sink) {
-    double a[16];
-    const double x = 1.0 + 1e-9 * threadIdx.x, y = 1e-12 * (blockIdx.x + 1);
-#pragma unroll
-    for (int i = 0; i < 16; ++i) a[i] = (double)i;
-    for (int k = 0; k < iters; ++k) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) a[i] = fma(a[i], x, y);
-    }
-    double s = 0;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += a[i];
-    if (s == 123.456) sink[0] = s;
 }
 
 template <int RL, int RT, int NW, int NC, bool FOLD = false>
@@ -729,23 +587,16 @@ cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
 
 // Tile shapes: inverse 64 degrees x 128 rings per block (8 compute warps, 8 degrees x 4 rings per thread);
 //              forward 64 degrees x 128 rings per block (8 compute warps, 2 degrees x 16 rings per thread).
-#ifdef SHT_PROF
-extern "C" void sht_prof_read(unsigned long long* out, int reset) {
-    cudaMemcpyFromSymbol(out, g_prof, sizeof(g_prof));
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_prof, z, sizeof(z)); }
-}
-#endif
 int theta_inverse_rowd(int mode) { return mode == 0 ? 6 : 4; }
 // Tile choice.  A launch has (Lp/64) x (ntp/rings_per_block) x npass blocks whose step counts grow linearly with the degree
 // tile, and the longest block alone runs ~L steps.  When 64 x 128 tiles do not even give one block per SM the launch is bound by
 // that longest block while the other SMs idle; 64 x 64 tiles then halve the work per step of every block (measured: L = 512
 // spin 0 inverse 0.456 -> 0.275 ms, L = 1024 spin 0 inverse 0.906 -> 0.548 ms; with more blocks than SMs the big tile wins).
-// SHT_TILE=64/128 overrides.
+// ThetaArgs::tile = 64 / 128 (plan option) overrides.
 static bool small_tiles(const ThetaArgs& a, int big) {
-    static const char* env = getenv("SHT_TILE");
-    if (env) return atoi(env) == 64;
+    if (a.tile) return a.tile == 64;
     const long blocks = (long)(a.Lp / SHT_TQ) * (a.ntp / big) * a.npass;
-    return blocks <= 148;
+    return blocks <= a.nsm;
 }
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
@@ -762,10 +613,4 @@ cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st) 
     }
     if (a.fold0) return mode == 0 ? launch_fwd<2, 16, 8, 2, true>(a, st) : launch_fwd<2, 16, 8, 1, true>(a, st);
     return mode == 0 ? launch_fwd<2, 16, 8, 2, false>(a, st) : launch_fwd<2, 16, 8, 1, false>(a, st);
-}
-cudaError_t launch_fp64_peak(int iters, double* sink, cudaStream_t st, int* blocks, int* threads, int* fma_per_thread) {
-    *blocks = 148 * 8; *threads = 256; *fma_per_thread = 16;
-    fp64_peak_kernel<<<*blocks, *threads, 0, st>>>(iters, sink);
-    count_launch();
-    return cudaGetLastError();
 }

@@ -16,6 +16,7 @@
 // The warp's 16 x 32 result tile goes to a private staging buffer and is added to global memory by ONE bulk-reduce
 // TMA (cp.reduce.async.bulk .add.f64) -- no per-element RED, no reducer warps.
 // Renormalisation windows, peak split and dead-ring handling are those of theta_kernels.cu (internal.h).
+#include "device_utils.cuh"
 #include "internal.h"
 
 #include <cuda_runtime.h>
@@ -23,52 +24,13 @@
 
 namespace {
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-// global[dst .. dst+bytes) += shared[src .. src+bytes) as doubles, asynchronously (bulk async-group completion)
-__device__ __forceinline__ void bulk_reduce_add_f64(double* gdst, const void* ssrc, uint32_t bytes) {
-    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+using namespace shtdev;
+
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c[0]), "+d"(c[1])
                  : "d"(a), "d"(b));
 }
-__device__ __forceinline__ double pow2i(int e) { return __hiloint2double((1023 + e) << 20, 0); }
-__device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7fffffff; }
-#define HI_TWIN ((1023 + SHT_TWIN) << 20)
-#define HI_DEAD ((1023 + 500) << 20)
-
 constexpr int NW = 8;        // compute warps
 constexpr int NAUX = 4;      // auxiliary warpgroup (one thread of it is the TMA producer)
 constexpr int NJ = 16;       // K blocks of 4 per thread
@@ -81,34 +43,7 @@ constexpr int TM = NW * 8 * NIB;    // 128: output rows of a CTA
 constexpr int NSTG = 4;             // operand ring stages
 static_assert(TK == SHT_TQ, "the contraction tile is one kappa quantum");
 
-__device__ __forceinline__ void reg_dealloc_aux() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
-__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
-
-struct KPack32 {
-    uint32_t w[NI / 4];
-    __device__ __forceinline__ void fill(uint32_t v) {
-#pragma unroll
-        for (int i = 0; i < NI / 4; ++i) w[i] = v;
-    }
-    __device__ __forceinline__ void set(int idx, uint32_t k) {
-        const int sh = (idx & 3) * 8;
-        w[idx >> 2] = (w[idx >> 2] & ~(0xffu << sh)) | (k << sh);
-    }
-    __device__ __forceinline__ uint32_t get(int idx) const { return (w[idx >> 2] >> ((idx & 3) * 8)) & 0xffu; }
-    __device__ __forceinline__ void dec(int idx) { w[idx >> 2] -= 1u << ((idx & 3) * 8); }
-    __device__ __forceinline__ bool any_nonzero() const {
-        uint32_t o = 0;
-#pragma unroll
-        for (int i = 0; i < NI / 4; ++i) o |= w[i];
-        return o != 0;
-    }
-    __device__ __forceinline__ bool any_zero_byte() const {
-        bool z = false;
-#pragma unroll
-        for (int i = 0; i < NI / 4; ++i) z = z || (((w[i] - 0x01010101u) & ~w[i] & 0x80808080u) != 0);
-        return z;
-    }
-};
+using KPack32 = KPack<NI>;
 
 // FOLD (forward, n = 0, northern rings only): an operand row holds two column sets, E = q (F_m(theta) + F_m(pi - theta)) and
 // O = q (F_m(theta) - F_m(pi - theta)); a degree with l+m even contracts with E, one with l+m odd with O (PAPER.md:236,
@@ -322,12 +257,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_mma_kernel(const Mm
                 const double s = pow2i(-SHT_SWIN);
 #pragma unroll
                 for (int q = 0; q < NI; ++q)
-                    if (hi_abs(cb[q]) > HI_TWIN && kp.get(q) != 0u && kp.get(q) != 0xffu) { cb[q] *= s; ca[q] *= s; kp.dec(q); }
+                    if (hi_abs(cb[q]) > SHT_HI_TWIN && kp.get(q) != 0u && kp.get(q) != 0xffu) { cb[q] *= s; ca[q] *= s; kp.dec(q); }
             }
             if (P.m_lo) {
 #pragma unroll
                 for (int q = 0; q < NI; ++q)
-                    if (hi_abs(cb[q]) > HI_DEAD) { cb[q] = 0.0; ca[q] = 0.0; }
+                    if (hi_abs(cb[q]) > SHT_HI_DEAD) { cb[q] = 0.0; ca[q] = 0.0; }
             }
             if (m < l_lo) wact = __any_sync(0xffffffffu, kp.any_zero_byte());
         }

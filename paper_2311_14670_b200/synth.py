@@ -60,22 +60,11 @@ def random_flmn(L, N, seed=0):
     return np.ascontiguousarray(c)
 
 
-def random_map(shape, seed=0, real=False, mw_pole_spin=None):
-    """A plain (not band-limited) random map, for forward-transform parity where no band-limited map is available.
-
-    MW maps (shape [..., L, 2L-1]) contain a ring AT the pole theta = pi (Eq. 37).  A function of spin s on the sphere has
-    one value there, f(pi, phi) = c exp(i s phi) (only m = s survives, Eq. 29), so white noise on that ring is not a sample
-    set of any function.  With mw_pole_spin = s the last ring is replaced by c exp(i s phi_p), c drawn from the same stream
-    (R21: the forward transform is specified for sampled functions)."""
+def random_map(shape, seed=0, real=False):
+    """A plain (not band-limited) random map: iid N(0,1) samples (complex: unit total variance), for forward-transform parity on
+    arbitrary arrays.  Nothing is special-cased: MW maps get white noise on the theta = pi ring too (R21)."""
     rng = np.random.default_rng(seed)
     if real:
-        f = rng.standard_normal(shape)
-        if mw_pole_spin is not None:
-            f[..., -1, :] = f[..., -1, :1]
-        return f
+        return rng.standard_normal(shape)
     g = rng.standard_normal(tuple(shape) + (2,))
-    f = np.ascontiguousarray((g[..., 0] + 1j * g[..., 1]) / np.sqrt(2.0))
-    if mw_pole_spin is not None:
-        nphi = f.shape[-1]
-        f[..., -1, :] = f[..., -1, :1] * np.exp(2j * np.pi * mw_pole_spin * np.arange(nphi) / nphi)
-    return f
+    return np.ascontiguousarray((g[..., 0] + 1j * g[..., 1]) / np.sqrt(2.0))

@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 from paper_2311_14670_b200 import synth
+from mwpole import project_mw_pole
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -59,7 +60,7 @@ def test_batched_equals_single_map_plans(api):
     fb = Pb.inverse(dev(flm))
     f1 = torch.stack([P1.inverse(dev(flm[b])) for b in range(batch)])
     assert float((fb - f1).abs().max() / f1.abs().max()) < 1e-13
-    g = synth.random_map((batch, L, 2 * L - 1), seed=5, mw_pole_spin=spin)
+    g = synth.random_map((batch, L, 2 * L - 1), seed=5)
     cb = Pb.forward(dev(g))
     c1 = torch.stack([P1.forward(dev(g[b])) for b in range(batch)])
     assert float((cb - c1).abs().max() / c1.abs().max()) < 1e-13
@@ -82,8 +83,9 @@ def test_config5b_batch16_L2048(api, orc):
         for r, row in zip(rings, rows):
             assert rel(fb[r], row, scale) < TOL, (b, r)
     # forward of white-noise maps against the oracle on sampled orders m
-    g = synth.random_map((batch, L, 2 * L - 1), seed=21, mw_pole_spin=0)
+    g = synth.random_map((batch, L, 2 * L - 1), seed=21)        # raw white noise to the GPU; the oracle gets the projected pole ring
     got = P.forward(dev(g))
+    g = project_mw_pole(g, 0)
     ms = np.array([-(L - 1), -1000, -1, 0, 1, 2, 777, L - 1])
     for b in (0, 15):
         want = orc.s2_forward_columns(L, 0, orc.MW, g[b], ms)
@@ -95,12 +97,12 @@ def test_config5b_batch16_L2048(api, orc):
 
 @pytest.mark.parametrize("fold", ["0", "1"])
 @pytest.mark.parametrize("L,batch,real", [(8, 2, False), (33, 3, False), (130, 9, False), (200, 16, False), (96, 4, True)])
-def test_batched_spin0_forward_with_and_without_fold(api, orc, monkeypatch, fold, L, batch, real):
+def test_batched_spin0_forward_with_and_without_fold(api, orc, fold, L, batch, real):
     """Batched spin-0 forward with the north-south fold forced on / off (default: on at large L): recursion on the northern rings,
     even / odd l+m rows contract with the E / O column sets (theta_mma.cu FOLD).  White-noise maps, every map against the oracle."""
-    monkeypatch.setenv("SHT_FOLD0", fold)
-    g = synth.random_map((batch, L, 2 * L - 1), seed=7 * L, real=real, mw_pole_spin=0)
-    P = api.Plan(L, 0, reality=real, batch=batch)
+    g = synth.random_map((batch, L, 2 * L - 1), seed=7 * L, real=real)
+    P = api.Plan(L, 0, reality=real, batch=batch, fold=fold == "1")
     got = P.forward(dev(g)).cpu().numpy()
+    g = project_mw_pole(g, 0)
     for b in range(batch):
         assert rel(got[b], orc.s2_forward(L, 0, orc.MW, g[b].astype(np.complex128))) < TOL, b

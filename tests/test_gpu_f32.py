@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 from paper_2311_14670_b200 import synth
+from mwpole import project_mw_pole
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -38,9 +39,9 @@ def test_f32_inverse_forward_vs_oracle(api, orc, L, real):
     back = P.forward(dev(f_ref.astype(f.dtype))).cpu().numpy()
     assert back.dtype == np.complex64
     assert rel(back, flm) < TOL32                                 # sampling theorem (pin 6), at fp32 accuracy
-    g = synth.random_map((L, 2 * L - 1), seed=L, real=real, mw_pole_spin=0)
+    g = synth.random_map((L, 2 * L - 1), seed=L, real=real)
     got = P.forward(dev(g.astype(f.dtype))).cpu().numpy()
-    assert rel(got, orc.s2_forward(L, 0, orc.MW, g.astype(np.complex128))) < TOL32
+    assert rel(got, orc.s2_forward(L, 0, orc.MW, project_mw_pole(g, 0).astype(np.complex128))) < TOL32
     el = np.arange(L)[:, None]
     m = np.arange(-(L - 1), L)[None, :]
     assert np.all(back[np.abs(m) > el] == 0)
@@ -66,20 +67,19 @@ def test_f32_config5a_scale_L2048_sampled(api, orc):
         assert rel(f[r], row, scale) < TOL32, r
     back = P.forward(dev(f)).cpu().numpy()
     assert rel(back, flm) < 2 * TOL32                             # two fp32 transforms in a row
-    g = synth.random_map((L, 2 * L - 1), seed=15, mw_pole_spin=0)
+    g = synth.random_map((L, 2 * L - 1), seed=15)
     got = P.forward(dev(g.astype(np.complex64))).cpu().numpy()
     ms = np.array([-(L - 1), -1, 0, 1, 2, 1024, L - 1])
-    want = orc.s2_forward_columns(L, 0, orc.MW, g, ms)
+    want = orc.s2_forward_columns(L, 0, orc.MW, project_mw_pole(g, 0), ms)
     sc = np.abs(want).max()
     for m, col in zip(ms, want):
         assert rel(got[:, m + L - 1], col, sc) < TOL32, m
 
 
 @pytest.mark.parametrize("L,real", [(8, False), (33, False), (130, False), (200, True)])
-def test_f32_forward_with_north_south_fold(api, orc, monkeypatch, L, real):
+def test_f32_forward_with_north_south_fold(api, orc, L, real):
     """fp32 forward with the north-south fold forced on (default at L >= 2048): northern rings only, E / O operand sets."""
-    monkeypatch.setenv("SHT_FOLD0", "1")
-    g = synth.random_map((L, 2 * L - 1), seed=3 * L, real=real, mw_pole_spin=0)
-    P = api.Plan(L, 0, reality=real, dtype="f32")
+    g = synth.random_map((L, 2 * L - 1), seed=3 * L, real=real)
+    P = api.Plan(L, 0, reality=real, dtype="f32", fold=True)
     got = P.forward(dev(g.astype(np.float32 if real else np.complex64))).cpu().numpy()
-    assert rel(got, orc.s2_forward(L, 0, orc.MW, g.astype(np.complex128))) < TOL32
+    assert rel(got, orc.s2_forward(L, 0, orc.MW, project_mw_pole(g, 0).astype(np.complex128))) < TOL32

@@ -1,11 +1,13 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times, on SAMPLED outputs the oracle
 can compute one by one (a few rings of the inverse, a few harmonic orders m of the forward), plus properties that hold
-at any size (exact MW round trip, zero pattern).  Forward inputs are white-noise maps from synth (not band-limited; only
-the theta = pi ring is that of a function, R21), never something the CUDA path produced."""
+at any size (exact MW round trip, zero pattern).  Forward inputs are raw white-noise maps from synth (not band-limited),
+never something the CUDA path produced; the GPU gets the raw array, the oracle the array whose theta = pi ring is projected
+onto the one Fourier component a spin-s function can hold there (the documented domain rule, include/b200sht.h; R21)."""
 import numpy as np
 import pytest
 
 from paper_2311_14670_b200 import synth
+from mwpole import project_mw_pole, project_so3_pole
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -43,10 +45,10 @@ def test_config2_mw_L1024_spin2(api, orc):
     # sampling theorem (DESIGN.md pin 6): the round trip reproduces the generating coefficients
     assert rel(back, flm) < TOL
     # forward of a white-noise map against the oracle on sampled orders m
-    g = synth.random_map((L, 2 * L - 1), seed=11, mw_pole_spin=spin)
+    g = synth.random_map((L, 2 * L - 1), seed=11)
     got = P.forward(dev(g)).cpu().numpy()
     ms = np.array([-(L - 1), -700, -2, -1, 0, 1, 2, 3, 511, L - 1])
-    want = orc.s2_forward_columns(L, spin, orc.MW, g, ms)
+    want = orc.s2_forward_columns(L, spin, orc.MW, project_mw_pole(g, spin), ms)
     sc = np.abs(want).max()
     for m, col in zip(ms, want):
         assert rel(got[:, m + L - 1], col, sc) < TOL, m
@@ -86,8 +88,8 @@ def test_config4_so3_L256_N8(api, orc):
     back = P.forward(dev(f_ref)).cpu().numpy()
     assert rel(back, c) < TOL
     g = synth.random_map((2 * N - 1, L, 2 * L - 1), seed=13)
-    g[:, L - 1, :] = f_ref[:, L - 1, :]      # a function on SO(3) has one value per (alpha - gamma) at beta = pi (R21)
-    assert rel(P.forward(dev(g)).cpu().numpy(), orc.so3_forward(L, N, g)) < TOL
+    # raw white noise to the GPU; the oracle gets the beta = pi ring projected per n onto m = -n (R21)
+    assert rel(P.forward(dev(g)).cpu().numpy(), orc.so3_forward(L, N, project_so3_pole(g))) < TOL
 
 
 def test_config5a_mw_L8192_spin0(api, orc):
@@ -111,10 +113,10 @@ def test_config5a_mw_L8192_spin0(api, orc):
     print(f"L=8192 round trip max rel err {err:.3e}")
     assert err < tol
     del f, back, d
-    g = synth.random_map((L, 2 * L - 1), seed=14, mw_pole_spin=spin)
+    g = synth.random_map((L, 2 * L - 1), seed=14)
     got = P.forward(dev(g)).cpu().numpy()
     ms = np.array([-(L - 1), -1, 0, 1, 4096, L - 1])
-    want = orc.s2_forward_columns(L, spin, orc.MW, g, ms)
+    want = orc.s2_forward_columns(L, spin, orc.MW, project_mw_pole(g, spin), ms)
     sc = np.abs(want).max()
     for m, col in zip(ms, want):
         assert rel(got[:, m + L - 1], col, sc) < tol, m

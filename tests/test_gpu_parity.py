@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 from paper_2311_14670_b200 import synth
+from mwpole import project_mw_pole, project_so3_pole
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -66,13 +67,33 @@ def test_config1_L64_spin0_round_trip_and_forward(api, orc):
     assert np.abs(back.cpu().numpy() - flm)[sup].mean() < 10 * tab[64]
 
 
-def test_forward_of_non_bandlimited_map_matches_oracle(api, orc):
-    """The forward transform is defined by the algorithm (upsampling + quadrature) for any sampled function, not just
-    band-limited ones: check parity on white noise (single-valued at the pole ring, R21)."""
-    L, spin = 40, 1
-    f = synth.random_map((L, 2 * L - 1), seed=9, mw_pole_spin=spin)
+@pytest.mark.parametrize("L,spin", [(40, 1), (33, 0), (64, -2), (130, 2)])
+def test_forward_of_raw_white_noise_matches_oracle_on_projected_pole_ring(api, orc, L, spin):
+    """The forward transform is defined by the algorithm (upsampling + quadrature) for any array, not just band-limited maps.
+    The GPU gets RAW white noise; the library projects the theta = pi ring onto exp(i s phi) (include/b200sht.h, R21), so
+    the oracle is called on the array with that projection applied by the test.  The size of the departure from the paper's
+    MW(2L)-grid algorithm on the raw array (which is ring-set dependent there) is measured and printed, not hidden."""
+    f = synth.random_map((L, 2 * L - 1), seed=9 + L)
     P = api.Plan(L, spin)
-    assert rel(P.forward(dev(f)).cpu().numpy(), orc.s2_forward(L, spin, orc.MW, f)) < TOL
+    got = P.forward(dev(f)).cpu().numpy()
+    fp = project_mw_pole(f, spin)
+    assert rel(got, orc.s2_forward(L, spin, orc.MW, fp)) < TOL
+    assert rel(P.forward(dev(fp)).cpu().numpy(), got) < 1e-14          # the projection is idempotent inside the library
+    raw = orc.s2_forward(L, spin, orc.MW, f)
+    dep = rel(got, raw)
+    print(f"L={L} spin={spin}: max|GPU(raw) - oracle(raw)| / max|oracle(raw)| = {dep:.3e} (white noise on the pole ring; "
+          f"pole-ring rms {np.abs(f[-1]).std():.2f})")
+    # the departure is confined to the odd-symmetry component of the single pole ring: one ring of L, weight ~ 1/L^2
+    assert dep < 0.5
+
+
+def test_so3_forward_of_raw_white_noise(api, orc):
+    L, N = 24, 4
+    g = synth.random_map((2 * N - 1, L, 2 * L - 1), seed=77)
+    P = api.Plan(L, N=N)
+    got = P.forward(dev(g)).cpu().numpy()
+    assert rel(got, orc.so3_forward(L, N, project_so3_pole(g))) < TOL
+    print(f"SO(3) L={L} N={N}: departure from the oracle on the raw array {rel(got, orc.so3_forward(L, N, g)):.3e}")
 
 
 def test_theta_stage_entry_points(api, orc):
@@ -196,17 +217,17 @@ def test_healpix_north_star_call_uses_nside_L_over_2(api, orc):
 @pytest.mark.parametrize("fold", ["0", "1"])
 @pytest.mark.parametrize("sampling,L,nside,real", [("mw", 8, 0, False), ("mw", 33, 0, False), ("mw", 130, 0, False), ("mw", 200, 0, True),
                                                    ("hp", 9, 2, False), ("hp", 24, 8, True), ("hp", 64, 32, False)])
-def test_spin0_forward_with_and_without_north_south_fold(api, orc, monkeypatch, fold, sampling, L, nside, real):
+def test_spin0_forward_with_and_without_north_south_fold(api, orc, fold, sampling, L, nside, real):
     """The spin-0 forward runs the recursion on the northern rings only when the plan enables the fold (default at large L):
     d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta).  Both paths against the oracle, element by element."""
-    monkeypatch.setenv("SHT_FOLD0", fold)
+    fold = fold == "1"
     if sampling == "mw":
-        f = synth.random_map((L, 2 * L - 1), seed=L, real=real, mw_pole_spin=0)
-        P = api.Plan(L, 0, reality=real)
-        want = orc.s2_forward(L, 0, orc.MW, f.astype(np.complex128))
+        f = synth.random_map((L, 2 * L - 1), seed=L, real=real)
+        P = api.Plan(L, 0, reality=real, fold=fold)
+        want = orc.s2_forward(L, 0, orc.MW, project_mw_pole(f, 0).astype(np.complex128))
     else:
         f = synth.random_map((12 * nside * nside,), seed=L, real=real)
-        P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=real)
+        P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=real, fold=fold)
         want = orc.s2_forward(L, 0, orc.HEALPIX, f.astype(np.complex128), nside=nside)
     assert rel(P.forward(dev(f)).cpu().numpy(), want) < TOL
     if sampling == "hp":      # HEALPix rings are symmetric on the inverse side too: F_m(theta) = E + O, F_m(pi - theta) = E - O
@@ -218,13 +239,12 @@ def test_spin0_forward_with_and_without_north_south_fold(api, orc, monkeypatch, 
 
 @pytest.mark.parametrize("sym", ["0", "1"])
 @pytest.mark.parametrize("L,real", [(1, False), (2, False), (8, False), (33, False), (64, False), (130, False), (200, True), (257, False)])
-def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, monkeypatch, sym, L, real):
-    """MW spin-0 inverse either directly on the MW rings, or (default at L >= 2048) on the L midpoint rings (2j+1)pi/(2L) with the
+def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, sym, L, real):
+    """MW spin-0 inverse either directly on the MW rings (default), or (plan option SHT_OPT_INVSYM) on the L midpoint rings (2j+1)pi/(2L) with the
     north-south fold followed by an exact FFT resampling of F_m(theta) to the MW rings.  Both against the oracle, element by element,
     through the full transform and through the theta-stage entry point."""
-    monkeypatch.setenv("SHT_INVSYM", sym)
     flm = synth.random_flm(L, 0, seed=5 * L, real=real)
-    P = api.Plan(L, 0, reality=real)
+    P = api.Plan(L, 0, reality=real, invsym=sym == "1")
     ref = orc.s2_inverse(L, 0, orc.MW, flm)
     got = P.inverse(dev(flm)).cpu().numpy()
     assert rel(got, ref.real if real else ref) < TOL
