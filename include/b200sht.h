@@ -16,6 +16,9 @@
  *   - Layouts are row-major, last index fastest; complex = interleaved (re, im) doubles.
  *       flm  [L][2L-1]            (l, m+L-1)                              embeds C^{L^2}
  *       MW map   f[L][2L-1]       (theta_t, phi_p), theta_t=(2t+1)pi/(2L-1), phi_p=2 pi p/(2L-1)   (Eq. 37-38)
+ *       MWSS map f[L+1][2L]       theta_t = 2 pi t/(2L) (t = 0 and t = L are the poles), phi_p = 2 pi p/(2L)              (Eq. 39-40)
+ *       DH map   f[2L][2L-1]      theta_t = (2t+1)pi/(4L), phi_p = 2 pi p/(2L-1)                                          (Eq. 34-35)
+ *       GL map   f[L][2L-1]       theta_t = acos(x_t), x_t the roots of the Legendre polynomial P_L (north to south)      (Eq. 45)
  *       HEALPix  f[12 nside^2]    ring-ordered: rings north to south, phi increasing within a ring
  *       SO(3)    f[2N-1][L][2L-1] (gamma_g, beta_b, alpha_a), MW in (beta, alpha), gamma_g = 2 pi g/(2N-1)
  *       flmn [2N-1][L][2L-1]      (n+N-1, l, m+L-1)
@@ -50,7 +53,7 @@ typedef enum {
     SHT_ECUFFT = 5         /* a cuFFT call failed */
 } sht_status;
 
-enum { SHT_MW = 0, SHT_HEALPIX = 1 };   /* sampling */
+enum { SHT_MW = 0, SHT_HEALPIX = 1, SHT_MWSS = 2, SHT_DH = 3, SHT_GL = 4 };   /* sampling */
 enum { SHT_F64 = 0, SHT_F32 = 1 };      /* dtype    */
 /* plan options (bit flags of sht_plan_s2_opts); 0 = automatic choices.  Results agree to rounding whatever the options. */
 enum {
@@ -105,6 +108,9 @@ sht_status sht_plan_destroy(sht_plan* plan);
  *              torus extension.  For samples of any spin-s function this changes nothing; for arbitrary arrays (e.g. pixel noise
  *              on the pole ring) it makes the result well defined -- it equals the paper's MW(2L)-grid algorithm applied to the
  *              projected array (the paper's algorithm itself is ring-set dependent on inconsistent pole samples, R21).
+ *              MWSS: as MW on the theta circle of 2L samples (both pole rings are projected: theta = 0 keeps m = -s, theta = pi keeps
+ *              m = s).  DH / GL: explicit quadrature on the rings of the map, weights Eq. 36 / the Gauss-Legendre weights Eq. 46 stands
+ *              for (2/((1-x^2) P_L'(x)^2) times 2 pi/(2L-1); Eq. 46 as printed is not that weight, R22).
  *              HEALPix: ring FFTs with phase shift and periodic extension
  *              (PAPER.md:403-407), weights 4 pi/Npix, Eq. 30.
  * s2_inverse : flm -> map f.  Fused recursion + l contraction of Eq. 33, then ring synthesis Eq. 32 (HEALPix:

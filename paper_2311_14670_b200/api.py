@@ -1,7 +1,8 @@
 """Python binding of include/b200sht.h -- argument marshalling only; every step of the transforms runs in the CUDA
 library.  PyTorch supplies device memory and the current CUDA stream, nothing else.
 
-Layouts (see include/b200sht.h): flm[L, 2L-1] complex128 (column m+L-1); MW maps f[L, 2L-1]; HEALPix maps
+Layouts (see include/b200sht.h): flm[L, 2L-1] complex128 (column m+L-1); MW maps f[L, 2L-1] (MWSS [L+1, 2L], DH [2L, 2L-1],
+GL [L, 2L-1]); HEALPix maps
 f[12 nside^2] ring-ordered; SO(3) f[2N-1, L, 2L-1] = (gamma, beta, alpha); flmn[2N-1, L, 2L-1] = (n+N-1, l, m+L-1).
 With reality=True maps are float64.
 """
@@ -11,9 +12,9 @@ import numpy as np
 import torch
 
 from . import _lib
-from ._lib import SHT_F32, SHT_F64, SHT_HEALPIX, SHT_MW, check, lib
+from ._lib import SHT_DH, SHT_F32, SHT_F64, SHT_GL, SHT_HEALPIX, SHT_MW, SHT_MWSS, check, lib
 
-MW, HEALPIX = SHT_MW, SHT_HEALPIX
+MW, HEALPIX, MWSS, DH, GL = SHT_MW, SHT_HEALPIX, SHT_MWSS, SHT_DH, SHT_GL
 
 
 def _stream():
@@ -29,7 +30,10 @@ def _dev(t, dtype, shape, what):
 
 
 def map_shape(L, sampling=MW, nside=0):
-    return (L, 2 * L - 1) if sampling == MW else (12 * nside * nside,)
+    """MW [L, 2L-1]; MWSS [L+1, 2L]; DH [2L, 2L-1]; GL [L, 2L-1]; HEALPix [12 nside^2] (ring-ordered)."""
+    if sampling == HEALPIX:
+        return (12 * nside * nside,)
+    return {MW: (L, 2 * L - 1), MWSS: (L + 1, 2 * L), DH: (2 * L, 2 * L - 1), GL: (L, 2 * L - 1)}[sampling]
 
 
 class Plan:

@@ -56,7 +56,8 @@ inline size_t rup(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // ---- one set of iso-latitude rings the theta kernels run on -----------------------------------------------------
 struct RingSet {
     int nth = 0, ntp = 0;      // regular rings, padded count (multiple of 128; > nth so a pole ring fits)
-    bool pole = false;         // a theta = pi ring at index nth (MW, Eq. 29)
+    bool pole = false;         // a theta = pi ring right after the regular rings (MW, MWSS; Eq. 29)
+    bool pole_n = false;       // a theta = 0 ring in front of the regular rings (MWSS; Eq. 28)
     bool symmetric = false;    // ring nth-1-t is the mirror image pi - theta_t of ring t
     int nfull = 0;             // > 0: this set is the northern half (incl. an equator ring) of a symmetric set of nfull rings
     std::vector<ld> ct, c2, s2;  // host: cos(theta), cos(theta/2), sin(theta/2) of the regular rings
@@ -79,7 +80,13 @@ enum { CAT_HOT = 0, CAT_FFT = 1, CAT_STAGE = 2 };
 struct sht_plan {
     int kind = 0;              // 0 S^2, 1 SO(3)
     int L = 0, spin = 0, sampling = 0, nside = 0, reality = 0, N = 1;
-    int Lp = 0, NB = 0;        // padded L; 2L-1
+    int Lp = 0, NB = 0;        // padded L; number of phi bins = rows of F / Fa / Z = length of the phi FFT (2L-1; MWSS: 2L)
+    int M = 0;                 // 2L-1: row length of the coefficient arrays flm[L][M]
+    int nrmap = 0;             // rings of the map (equiangular samplings): L (MW, GL), L+1 (MWSS), 2L (DH)
+    size_t map_elems = 0;      // samples of one map
+    int Tcirc = 0;             // MW / MWSS: samples of the theta circle the forward extension works on (= NB)
+    int col0 = 0;              // column of F (= ring of the map) of the first regular ring of the inverse ring set (MWSS: 1)
+    std::vector<ld> gl_w;      // GL: Gauss weights of the rings
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
     bool f32_inner = false;    // set while an fp32 transform runs its fp64-array core
     int dtype = SHT_F64;       // SHT_F32: fp32 hot kernels (theta_f32.cu) and fp32 public arrays; staging and FFTs stay fp64
@@ -91,6 +98,7 @@ struct sht_plan {
     cufftHandle fft_sym = 0;   // length 2L, batch 2L-1
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
+    bool upsampled = false;    // MW / MWSS: the forward transform extends F_m to the theta circle and upsamples to the quadrature rings
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
     unsigned opts = 0;         // SHT_OPT_* given at creation
     int device = 0, nsm = 0;   // device the plan was created on and its SM count (tile choice)
@@ -165,6 +173,54 @@ void rings_mid(RingSet& R, int nrings) {      // theta_u = (2u+1) pi / (2 nrings
     R.ntp = (int)rup((size_t)R.nth, 128);
 }
 
+// MWSS, Eq. 39: theta_t = 2 pi t/(2L), t = 0..L.  Rings t = 0 and t = L are the poles (Eq. 28 / 29, handled apart);
+// the regular rings t = 1..L-1 are symmetric about the equator.
+void rings_mwss(RingSet& R, int L) {
+    R.nth = L - 1; R.pole = true; R.pole_n = true; R.symmetric = true;
+    R.ct.resize(R.nth); R.c2.resize(R.nth); R.s2.resize(R.nth);
+    for (int i = 0; i < R.nth; ++i) {
+        // mirror pairs get exactly mirrored trigonometry: evaluate on the northern ring
+        const int t = i + 1, tn = t <= L - t ? t : L - t;
+        ld th = PI_L * (ld)tn / (ld)L;
+        ld c = cosl(th), c2 = cosl(th / 2), s2 = sinl(th / 2);
+        if (2 * t == L) c = 0;
+        const bool south = t > L - t;
+        R.ct[i] = south ? -c : c; R.c2[i] = south ? s2 : c2; R.s2[i] = south ? c2 : s2;
+    }
+    R.ntp = (int)rup((size_t)R.nth + 2, 128);
+}
+// Gauss-Legendre rings: theta_t = acos(x_t), x_t the roots of P_L, north to south.  Newton's iteration in theta on
+// P_L(cos theta) (three-term recurrence in long double), so the half angles keep full relative accuracy near the poles.  Also
+// returns the Gauss weights 2/((1-x^2) P_L'(x)^2) (the weight Eq. 46 stands for, R22).
+void rings_gl(RingSet& R, int L, std::vector<ld>* wts) {
+    R.nth = L; R.pole = false; R.symmetric = true;
+    R.ct.resize(L); R.c2.resize(L); R.s2.resize(L);
+    if (wts) wts->assign(L, 0);
+    auto pl = [L](ld x, ld& p, ld& dp) {
+        ld p0 = 1, p1 = x;
+        for (int k = 2; k <= L; ++k) { ld pk = ((ld)(2 * k - 1) * x * p1 - (ld)(k - 1) * p0) / (ld)k; p0 = p1; p1 = pk; }
+        p = p1; dp = (ld)L * (x * p1 - p0) / (x * x - 1);
+    };
+    for (int t = 0; t < (L + 1) / 2; ++t) {
+        ld th = PI_L * ((ld)t + 0.75L) / ((ld)L + 0.5L), p, dp;
+        for (int it = 0; it < 100; ++it) {
+            pl(cosl(th), p, dp);
+            ld dth = p / (sinl(th) * dp);
+            th += dth;
+            if (fabsl(dth) < 1e-19L * th) break;
+        }
+        const bool eq = 2 * t + 1 == L;
+        if (eq) th = PI_L / 2;
+        pl(cosl(th), p, dp);
+        const ld c = eq ? 0.0L : cosl(th), sn = eq ? 1.0L : sinl(th), c2 = cosl(th / 2), s2 = sinl(th / 2);
+        const ld w = 2.0L / (sn * sn * dp * dp);
+        R.ct[t] = c; R.c2[t] = c2; R.s2[t] = s2;
+        R.ct[L - 1 - t] = -c; R.c2[L - 1 - t] = s2; R.s2[L - 1 - t] = c2;       // the mirror ring, exactly mirrored
+        if (wts) { (*wts)[t] = w; (*wts)[L - 1 - t] = w; }
+    }
+    R.ntp = (int)rup((size_t)R.nth + 1, 128);
+}
+
 // HEALPix rings r = 1..4 nside-1 (public ring scheme, R11); half-angle trigonometry from z
 void rings_healpix(RingSet& R, int nside) {
     R.nth = 4 * nside - 1; R.pole = false; R.symmetric = true;
@@ -222,6 +278,41 @@ void stage(sht_plan* P, int cat, cudaStream_t st) {
     P->ev_n++;
 }
 
+// Array dimensions that depend on the sampling (called once the ring sets and folds are fixed).
+//   F  [slab][NB bins][F_ld]   F_m on the rings of the map (columns in map-ring order, poles included); Fa likewise (forward side)
+//   X  [slab][NB bins][Tcirc]  MW / MWSS: F_m extended to the theta circle          Z [slab][NB][fwd_ld]: F_m on the quadrature rings
+//   H  [slab][NB rows >= M][Lp]
+void plan_dims(sht_plan* P) {
+    const int L = P->L;
+    P->M = 2 * L - 1;
+    P->upsampled = P->sampling == SHT_MW || P->sampling == SHT_MWSS;
+    switch (P->sampling) {
+        case SHT_MWSS: P->NB = 2 * L; P->nrmap = L + 1; break;
+        case SHT_DH: P->NB = 2 * L - 1; P->nrmap = 2 * L; break;
+        default: P->NB = 2 * L - 1; P->nrmap = L; break;         // MW, GL; HEALPix keeps 2L-1 "bins" as its F-row convention
+    }
+    P->Tcirc = P->NB;
+    P->col0 = P->inv.pole_n ? 1 : 0;
+    if (P->sampling == SHT_HEALPIX) {
+        P->nrmap = 4 * P->nside - 1;
+        P->map_elems = (size_t)12 * P->nside * P->nside;
+    } else
+        P->map_elems = (size_t)P->nrmap * P->NB;
+    P->F_nrings = P->invsym ? L : P->nrmap;
+    P->F_ld = (int)rup((size_t)P->F_nrings, 128);
+    if (!P->inv.nfull && P->inv.ntp > P->F_ld) P->F_ld = P->inv.ntp;
+    P->F_slab = (size_t)P->NB * P->F_ld;
+    P->Ltp = P->F_ld;
+    P->Fa_slab = (size_t)P->NB * P->Ltp;
+    P->X_slab = (size_t)P->NB * P->Tcirc;
+    const int nq = P->fwd.nfull ? P->fwd.nfull : P->fwd.nth;
+    if (P->upsampled) P->fwd_ld = 4 * L;
+    else if (P->sampling == SHT_HEALPIX) P->fwd_ld = (int)rup((size_t)nq + 1, 128);
+    else P->fwd_ld = P->Ltp;                                       // DH / GL: the quadrature runs on the map's own rings (U = Fa)
+    P->Z_slab = (size_t)P->NB * P->fwd_ld;
+    P->H_slab = (size_t)P->NB * P->Lp;
+}
+
 // Walks the workspace layout.  With base == nullptr it only measures; otherwise it assigns every pointer.
 void layout(sht_plan* P, char* base) {
     Bump B; B.base = base;
@@ -263,33 +354,22 @@ void layout(sht_plan* P, char* base) {
         for (auto& ph : P->pfwd) { P->ob_off_fwd.push_back(of); of += (size_t)P->ncg_fwd * (L - ph.p.m_end) * Lp * SHT_MMA_NCOL; }
         P->Ob = B.take<double>(oi > of ? oi : of);
     }
-    // scratch arrays
-    P->F_nrings = (P->inv.nfull ? P->inv.nfull : P->inv.nth) + (P->inv.pole ? 1 : 0);
-    P->F_ld = P->inv.nfull ? (int)rup((size_t)P->inv.nfull + 1, 128) : P->inv.ntp;
-    if (P->invsym) P->F_ld = (int)rup((size_t)L, 128);     // holds the L midpoint rings, then the L MW rings (the phi-FFT stride)
-    P->F_slab = (size_t)NB * P->F_ld;
+    // scratch arrays (dimensions fixed by plan_dims)
     P->F = B.take<double2>(P->F_slab * P->nslab);
     P->polev = B.take<double2>(P->nslab);
     P->tmp = B.take<double>(2 * (size_t)Lp);
     P->unit_wq = B.take<double>(P->fwd.ntp);
-    P->Ltp = P->F_ld;
-    if (P->sampling == SHT_MW) {
-        P->fwd_ld = 4 * L;
-        P->Fa_slab = (size_t)NB * P->Ltp;
+    if (P->sampling != SHT_HEALPIX) {
         P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
-        P->X_slab = (size_t)NB * NB;
-        P->X = B.take<double2>(P->X_slab * P->nslab);
+        if (P->upsampled) P->X = B.take<double2>(P->X_slab * P->nslab);
     } else {
-        P->fwd_ld = (int)rup((size_t)(P->fwd.nfull ? P->fwd.nfull : P->fwd.nth) + 1, 128);
         P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
         P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
         P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
     }
-    P->Z_slab = (size_t)NB * P->fwd_ld;
     P->Z = B.take<double2>(P->Z_slab * P->nslab);
-    P->H_slab = (size_t)NB * Lp;
     P->H = B.take<double2>(P->H_slab * P->nslab);
-    if (P->reality && P->sampling == SHT_MW) P->cplx = B.take<double2>((size_t)L * NB * P->batch);
+    if (P->reality && P->sampling != SHT_HEALPIX) P->cplx = B.take<double2>(P->map_elems * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
     if (P->dtype == SHT_F32) {
         P->ab32 = B.take<float2>((size_t)L * Lp);
@@ -300,7 +380,7 @@ void layout(sht_plan* P, char* base) {
     }
     P->fft_work = B.take<char>(P->fft_work_bytes);
     // route every pass to its slab's output array
-    for (auto& ph : P->pinv) ph.p.out = P->F ? P->F + P->F_slab * ph.p.slab : nullptr;
+    for (auto& ph : P->pinv) ph.p.out = P->F ? P->F + P->F_slab * ph.p.slab + P->col0 : nullptr;   // regular ring th -> map ring col0 + th
     for (auto& ph : P->pfwd) ph.p.out = P->H ? P->H + P->H_slab * ph.p.slab : nullptr;
     if (P->batch > 1 && P->Ob) {
         for (size_t i = 0; i < P->pinv.size(); ++i) P->pinv[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_inv[i]);
@@ -354,20 +434,24 @@ sht_status make_fft_plans(sht_plan* P) {
         P->have_fft = true;
         return SHT_OK;
     }
+    // phi FFTs (Eq. 31 / 32): one ring per batch entry; F / Fa hold bin-major rows [bin][ring], the map is [ring][phi]
+    const int nr = P->nrmap;
     int n1[1] = {NB};
     CF(cufftCreate(&P->fft_phi_inv)); CF(cufftSetAutoAllocation(P->fft_phi_inv, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, (int)rup((size_t)L, 128), 1, onembed, 1, NB, CUFFT_Z2Z, L, &w)); P->fft_elems[P->fft_phi_inv] = (double)L * NB; ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_phi_inv, 1, n1, inembed, P->F_ld, 1, onembed, 1, NB, CUFFT_Z2Z, nr, &w)); P->fft_elems[P->fft_phi_inv] = (double)nr * NB; ws = w > ws ? w : ws; }
     CF(cufftCreate(&P->fft_phi_fwd)); CF(cufftSetAutoAllocation(P->fft_phi_fwd, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, (int)rup((size_t)L, 128), 1, CUFFT_Z2Z, L, &w)); P->fft_elems[P->fft_phi_fwd] = (double)L * NB; ws = w > ws ? w : ws; }
-    CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
-    { int inembed[1] = {NB};
-      CF(cufftMakePlanMany(P->fft_th1, 1, n1, inembed, 1, NB, inembed, 1, NB, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th1] = (double)NB * NB * P->nslab; ws = w > ws ? w : ws; }
-    int n2[1] = {4 * L};
-    CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
-    { int inembed[1] = {4 * L};
-      CF(cufftMakePlanMany(P->fft_th2, 1, n2, inembed, 1, 4 * L, inembed, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th2] = 4.0 * L * NB * P->nslab; ws = w > ws ? w : ws; }
+      CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, P->Ltp, 1, CUFFT_Z2Z, nr, &w)); P->fft_elems[P->fft_phi_fwd] = (double)nr * NB; ws = w > ws ? w : ws; }
+    if (P->upsampled) {
+        // theta FFTs of the forward upsampling: length Tcirc on the extended samples, length 4L onto the quadrature rings
+        int nt[1] = {P->Tcirc};
+        CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
+        CF(cufftMakePlanMany(P->fft_th1, 1, nt, nt, 1, P->Tcirc, nt, 1, P->Tcirc, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th1] = (double)P->Tcirc * NB * P->nslab; ws = w > ws ? w : ws;
+        int n2[1] = {4 * L};
+        CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
+        CF(cufftMakePlanMany(P->fft_th2, 1, n2, n2, 1, 4 * L, n2, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th2] = 4.0 * L * NB * P->nslab; ws = w > ws ? w : ws;
+    }
     if (P->invsym) {
         int n4[1] = {2 * L};
         CF(cufftCreate(&P->fft_sym)); CF(cufftSetAutoAllocation(P->fft_sym, 0));
@@ -424,7 +508,8 @@ sht_status check_start_range(const sht_plan* P) {
 
 sht_status plan_common(sht_plan* P) {
     const int L = P->L;
-    P->Lp = (int)rup(L, 128); P->NB = 2 * L - 1;
+    P->Lp = (int)rup(L, 128);
+    plan_dims(P);
     int nmax = 0;
     for (int n : P->slab_n) nmax = (n < 0 ? -n : n) > nmax ? (n < 0 ? -n : n) : nmax;
     P->kmin = -(nmax + 3);
@@ -578,6 +663,26 @@ sht_status zero_async(void* p, size_t bytes, cudaStream_t st) {
     return SHT_OK;
 }
 
+// pole rings of the inverse ring set (the kernels skip them): theta = pi holds only the order m = -n (Eq. 29), theta = 0 only m = n
+// (Eq. 28); F has been zeroed, so only those two entries are written.  Columns of F are in map-ring order.
+sht_status inverse_poles(sht_plan* P, const double2* coef, cudaStream_t st) {
+    const int L = P->L;
+    const int nreg = P->inv.nfull ? P->inv.nfull : P->inv.nth;
+    for (int s = 0; s < P->nslab; ++s) {
+        const int n = P->slab_n[s];
+        double2* Fs = P->F + P->F_slab * s;
+        if (P->inv.pole) {
+            const int row = (-n) < 0 ? -n + P->NB : -n;
+            CK(st_pole_inverse(L, n, 0, coef + (size_t)s * L * P->M, P->scale_inv, Fs + (size_t)row * P->F_ld + P->col0 + nreg, st));
+        }
+        if (P->inv.pole_n) {
+            const int row = n < 0 ? n + P->NB : n;
+            CK(st_pole_inverse(L, n, 1, coef + (size_t)s * L * P->M, P->scale_inv, Fs + (size_t)row * P->F_ld, st));
+        }
+    }
+    return SHT_OK;
+}
+
 // ---- the stages --------------------------------------------------------------------------------------------------
 // coef: nslab slabs of [L][NB] in *slab order*.  Leaves F[slab][row][ring] complete (all rows, incl. the pole ring).
 sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) {
@@ -612,13 +717,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
                                P->mmin, 0, 0, P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->inv.ntp * SHT_MMA_NCOL, P->F,
                                P->F_slab, P->inv.ntp, st));
         }
-        if (P->inv.pole) {
-            for (int s = 0; s < P->nslab; ++s) {
-                int n = P->slab_n[s];
-                int row = (-n) < 0 ? -n + P->NB : -n;
-                CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->F_ld + P->inv.nth, st));
-            }
-        }
+        CS(inverse_poles(P, coef, st));
         if (P->reality)
             for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F + P->F_slab * s, st));
         return SHT_OK;
@@ -634,26 +733,20 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         a.ab = P->ab32; a.lam32 = P->lam32_inv; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
         a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F;
         CK(launch_theta_f32(a, false, NC, st));
-        CK(st_pole_inverse(L, 0, coef, P->scale_inv, P->F + P->inv.nth, st));
+        CS(inverse_poles(P, coef, st));
         stage(P, CAT_STAGE, st);
         if (P->reality) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F, st));
         return SHT_OK;
     }
     for (auto& ph : P->pinv)
-        CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->NB,
+        CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->M,
                            P->scale_inv, P->ctab, P->sgtab, P->sgstride,
                            const_cast<double*>(ph.p.in) + (size_t)P->Lp * theta_inverse_rowd(ph.mode), st));
     CS(zero_async(P->F, sizeof(double2) * P->F_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
     CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
     CK(launch_theta_inverse(theta_args(P, false, false), 1, st));
-    if (P->inv.pole) {
-        for (int s = 0; s < P->nslab; ++s) {
-            int n = P->slab_n[s];
-            int row = (-n) < 0 ? -n + P->NB : -n;
-            CK(st_pole_inverse(L, n, coef + (size_t)s * L * P->NB, P->scale_inv, P->F + P->F_slab * s + (size_t)row * P->F_ld + P->inv.nth, st));
-        }
-    }
+    CS(inverse_poles(P, coef, st));
     stage(P, CAT_STAGE, st);
     if (P->reality)
         for (int s = 0; s < P->nslab; ++s) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F + P->F_slab * s, st));
@@ -762,15 +855,15 @@ sht_status resample_sym_to_mw(sht_plan* P, cudaStream_t st) {
     return SHT_OK;
 }
 
-// MW: F_m(theta_t) on L rings (Fa, [bin][Ltp]) -> U[bin][4L] on the rings theta'_u = (2u+1)pi/(4L) (in Z; u < 2L used)
+// MW / MWSS: F_m on the rings of the map (Fa, [bin][Ltp]) -> U[bin][4L] on the rings theta'_u = (2u+1)pi/(4L) (in Z; u < 2L used)
 sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
-    const int L = P->L, NB = P->NB, T2 = 4 * L;
+    const int L = P->L, T2 = 4 * L, mwss = P->sampling == SHT_MWSS;
     stage(P, CAT_STAGE, st);
-    for (int s = 0; s < P->nslab; ++s) CK(st_mw_extend(L, P->slab_n[s], P->Ltp, NB, P->Fa + P->Fa_slab * s, P->X + P->X_slab * s, st));
+    for (int s = 0; s < P->nslab; ++s) CK(st_mw_extend(L, P->slab_n[s], mwss, P->Ltp, P->Tcirc, P->Fa + P->Fa_slab * s, P->X + P->X_slab * s, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_FORWARD, st));
     stage(P, CAT_STAGE, st);
-    for (int s = 0; s < P->nslab; ++s) CK(st_mw_pad_phase(L, NB, T2, P->X + P->X_slab * s, P->Z + P->Z_slab * s, st));
+    for (int s = 0; s < P->nslab; ++s) CK(st_mw_pad_phase(L, mwss, P->Tcirc, T2, P->X + P->X_slab * s, P->Z + P->Z_slab * s, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th2, P->Z, P->Z, CUFFT_INVERSE, st));
     return SHT_OK;
@@ -852,8 +945,8 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
     if (!out) return SHT_EINVAL;
     *out = nullptr;
     if (batch < 1 || batch > 1024) return SHT_EINVAL;
+    if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || sampling < SHT_MW || sampling > SHT_GL) return SHT_EINVAL;
     if (batch > 1 && sampling != SHT_MW) return SHT_EUNSUPPORTED;
-    if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || (sampling != SHT_MW && sampling != SHT_HEALPIX)) return SHT_EINVAL;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
     if ((opts & SHT_OPT_FOLD_ON) && (opts & SHT_OPT_FOLD_OFF)) return SHT_EINVAL;
@@ -866,8 +959,14 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     query_device(P);
-    if (sampling == SHT_MW) { rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L); }
-    else { rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); }
+    // ring sets: `inv` = the rings of the map (inverse theta step), `fwd` = the rings the forward quadrature runs on
+    switch (sampling) {
+        case SHT_MW: rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L); break;           // Eq. 37; upsampled to the 2L midpoint rings (R9)
+        case SHT_MWSS: rings_mwss(P->inv, L); rings_mid(P->fwd, 2 * L); break;       // Eq. 39; same quadrature rings
+        case SHT_DH: rings_mid(P->inv, 2 * L); rings_mid(P->fwd, 2 * L); break;      // Eq. 34: theta_t = (2t+1)pi/(4L) -- the midpoint rings themselves
+        case SHT_GL: rings_gl(P->inv, L, nullptr); rings_gl(P->fwd, L, &P->gl_w); break;   // roots of P_L
+        default: rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); break;
+    }
     if (spin == 0) {
         // n = 0 fold (theta_kernels.cu FOLD): worth it once the northern half alone fills the GPU with >= 2 waves of 64 x 128 tiles
         // (L >= 2048 on MW on 148 SMs); SHT_OPT_FOLD_ON / SHT_OPT_FOLD_OFF override the choice
@@ -882,8 +981,11 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
         // while the resampling adds 0.77 ms of FFT + staging (measured).
         const bool isym = (opts & SHT_OPT_INVSYM) && sampling == SHT_MW && batch == 1 && dtype == SHT_F64;
         if (isym) { P->invsym = 1; P->fold0i = 1; rings_mid(P->inv, L); north_only(P->inv); }
-        // the inverse rings of HEALPix are symmetric too
-        if (on && sampling == SHT_HEALPIX && batch == 1) { P->fold0i = 1; north_only(P->inv); }
+        // the rings of the map are symmetric about the equator on every sampling but MW: fold the inverse too.  DH has 2L rings, so
+        // its folded inverse does the work of an MW inverse; it is folded whatever the size.
+        if ((on || sampling == SHT_DH) && !(opts & SHT_OPT_FOLD_OFF) && sampling != SHT_MW && batch == 1 && P->inv.symmetric) {
+            P->fold0i = 1; north_only(P->inv);
+        }
     }
     sht_status s = check_start_range(P);
     if (s == SHT_OK) s = plan_common(P);
@@ -912,7 +1014,8 @@ size_t sht_plan_workspace_bytes(const sht_plan* P) { return P ? P->need_bytes : 
 int sht_plan_batch(const sht_plan* P) { return P ? P->batch : 0; }
 int sht_plan_ntheta(const sht_plan* P, int forward) {
     if (!P) return 0;
-    const RingSet& R = forward ? P->fwd : P->inv;
+    if (!forward) return P->F_nrings;
+    const RingSet& R = P->fwd;
     return (R.nfull ? R.nfull : R.nth) + (R.pole ? 1 : 0);
 }
 double sht_plan_dsteps(const sht_plan* P, int forward) { return P ? (forward ? P->dsteps_fwd : P->dsteps_inv) : 0.0; }
@@ -944,9 +1047,16 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     CS(up(si, P->scale_inv, st)); CS(up(sf, P->scale_fwd, st));
     CS(fill_ringset(P, P->inv, st)); CS(fill_ringset(P, P->fwd, st));
     CK(cudaMemsetAsync(P->fwd.wq, 0, sizeof(double) * P->fwd.ntp, st));
-    if (P->sampling == SHT_MW) {
-        // forward quadrature weights q_u = (2 pi/(2L-1)) v_u on the 2L midpoint rings (Eq. 41-44 restated for that ring set)
-        CK(st_mid_weights(L, P->fwd.nth, (double)(2 * PI_L / (ld)(2 * L - 1)), P->fwd.wq, st));
+    if (P->sampling == SHT_MW || P->sampling == SHT_MWSS || P->sampling == SHT_DH) {
+        // forward quadrature weights q_u = q_Phi v_u on the 2L midpoint rings, q_Phi = 2 pi / (phi samples per ring).  MW / MWSS: Eq. 41-44
+        // restated for that ring set (R9).  DH: the rings ARE the DH rings and v_u equals the DH weight of Eq. 36 (Fejer's first
+        // rule: (2/L) sin(theta) sum_k sin((2k+1)theta)/(2k+1) = (1/L)(1 + 2 sum_j cos(2j theta)/(1-4j^2)); the oracle uses Eq. 36 as printed).
+        CK(st_mid_weights(L, P->fwd.nth, (double)(2 * PI_L / (ld)P->NB), P->fwd.wq, st));
+    } else if (P->sampling == SHT_GL) {
+        // Gauss-Legendre weights 2/((1-x^2) P_L'(x)^2) times q_Phi = 2 pi/(2L-1)  (Eq. 45-46, reading R22)
+        std::vector<double> w(P->fwd.ntp, 0.0);
+        for (int t = 0; t < P->fwd.nth; ++t) w[t] = (double)(2 * PI_L / (ld)(2 * L - 1) * P->gl_w[t]);
+        CS(up(w, P->fwd.wq, st));
     } else {
         // HEALPix: equal pixel weights 4 pi / Npix
         std::vector<double> w(P->fwd.ntp, 0.0);
@@ -962,8 +1072,9 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         CK(st_f64_to_f32((size_t)(L + 1) * P->inv.ntp, P->pinv[0].p.lam, P->lam32_inv, st));
         CK(st_f64_to_f32((size_t)(L + 1) * P->fwd.ntp, P->pfwd[0].p.lam, P->lam32_fwd, st));
     }
-    if (P->sampling == SHT_MW) {
-        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2}) CF(cufftSetWorkArea(h, P->fft_work));
+    if (P->sampling != SHT_HEALPIX) {
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2})
+            if (h) CF(cufftSetWorkArea(h, P->fft_work));
         if (P->invsym) CF(cufftSetWorkArea(P->fft_sym, P->fft_work));
         if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
     } else {
@@ -1064,15 +1175,15 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     CS(check_ready(P));
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    const int L = P->L, NB = P->NB;
+    const int L = P->L;
+    const size_t ncoef = (size_t)L * P->M, nmap = P->map_elems;
     if (P->dtype == SHT_F32 && !P->f32_inner) {      // fp32 public arrays: fp64 copies around the core (staging and FFTs are fp64)
-        const size_t nc = (size_t)L * NB;
-        CK(st_f32_to_f64(2 * nc, (const float*)flm, (double*)P->io_a, st));
+        CK(st_f32_to_f64(2 * ncoef, (const float*)flm, (double*)P->io_a, st));
         P->f32_inner = true;
         sht_status s = s2_inverse_plan(P, P->io_a, P->io_b, stream);
         P->f32_inner = false;
         if (s != SHT_OK) return s;
-        CK(st_f64_to_f32(P->reality ? nc : 2 * nc, (const double*)P->io_b, (float*)f, st));
+        CK(st_f64_to_f32(P->reality ? nmap : 2 * nmap, (const double*)P->io_b, (float*)f, st));
         stage(P, CAT_STAGE, st);
         return SHT_OK;
     }
@@ -1083,8 +1194,8 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     stage(P, CAT_FFT, st);
     double2* outc = P->reality ? P->cplx : (double2*)f;
     for (int b = 0; b < P->batch; ++b)
-        CS(fft_exec(P, P->fft_phi_inv, P->F + P->F_slab * b, outc + (size_t)L * NB * b, CUFFT_INVERSE, st));   // Eq. 32
-    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_complex_to_real((size_t)L * NB * P->batch, P->cplx, (double*)f, st)); }
+        CS(fft_exec(P, P->fft_phi_inv, P->F + P->F_slab * b, outc + nmap * b, CUFFT_INVERSE, st));   // Eq. 32
+    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_complex_to_real(nmap * P->batch, P->cplx, (double*)f, st)); }
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
@@ -1092,15 +1203,15 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     CS(check_ready(P));
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    const int L = P->L, NB = P->NB;
+    const int L = P->L;
+    const size_t ncoef = (size_t)L * P->M, nmap = P->map_elems;
     if (P->dtype == SHT_F32 && !P->f32_inner) {
-        const size_t nc = (size_t)L * NB;
-        CK(st_f32_to_f64(P->reality ? nc : 2 * nc, (const float*)f, (double*)P->io_a, st));
+        CK(st_f32_to_f64(P->reality ? nmap : 2 * nmap, (const float*)f, (double*)P->io_a, st));
         P->f32_inner = true;
         sht_status s = s2_forward_plan(P, P->io_a, P->io_b, stream);
         P->f32_inner = false;
         if (s != SHT_OK) return s;
-        CK(st_f64_to_f32(2 * nc, (const double*)P->io_b, (float*)flm, st));
+        CK(st_f64_to_f32(2 * ncoef, (const double*)P->io_b, (float*)flm, st));
         stage(P, CAT_STAGE, st);
         return SHT_OK;
     }
@@ -1114,15 +1225,18 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
         return SHT_OK;
     }
     const double2* fin = (const double2*)f;
-    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex((size_t)L * NB * P->batch, (const double*)f, P->cplx, st)); fin = P->cplx; }
+    if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex(nmap * P->batch, (const double*)f, P->cplx, st)); fin = P->cplx; }
     stage(P, CAT_FFT, st);
     for (int b = 0; b < P->batch; ++b)                                                 // Eq. 31 (weight folded into q_u)
-        CS(fft_exec(P, P->fft_phi_fwd, const_cast<double2*>(fin) + (size_t)L * NB * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
-    CS(mw_upsample(P, st));
-    CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
+        CS(fft_exec(P, P->fft_phi_fwd, const_cast<double2*>(fin) + nmap * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
+    if (P->upsampled) {         // MW / MWSS: extension to the theta circle + upsampling to the quadrature rings
+        CS(mw_upsample(P, st));
+        CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
+    } else                      // DH / GL: explicit quadrature on the rings of the map (Eq. 36 / 46)
+        CS(run_theta_forward(P, P->Fa, P->Fa_slab, P->Ltp, st));
     stage(P, CAT_STAGE, st);
     for (int b = 0; b < P->batch; ++b)
-        CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + (size_t)L * NB * b, st));
+        CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + ncoef * b, st));
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
@@ -1221,7 +1335,13 @@ sht_status cache_get(int kind, int L, int a, int sampling, int nside, int realit
     return SHT_OK;
 }
 size_t s2_map_bytes(int L, int sampling, int nside, int reality) {
-    size_t n = sampling == SHT_MW ? (size_t)L * (2 * L - 1) : (size_t)12 * nside * nside;
+    size_t n;
+    switch (sampling) {
+        case SHT_HEALPIX: n = (size_t)12 * nside * nside; break;
+        case SHT_MWSS: n = (size_t)(L + 1) * (2 * L); break;
+        case SHT_DH: n = (size_t)(2 * L) * (2 * L - 1); break;
+        default: n = (size_t)L * (2 * L - 1); break;
+    }
     return n * (reality ? 8 : 16);
 }
 sht_status host_io(CacheEntry* e, size_t in_bytes, size_t out_bytes) {

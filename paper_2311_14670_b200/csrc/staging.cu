@@ -192,14 +192,15 @@ __global__ void k_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_
         g[2 * NC + 1] = sg.x;
     }
 }
-// pole ring theta = pi, inverse (Eq. 29): F_{-n}(pi) = sum_l scale(l) f_{l,-n} (-1)^{l-n}.  One block per slab.
-__global__ void k_pole_inverse(int L, int n, const double2* __restrict__ coef, const double* __restrict__ scale, double2* __restrict__ out) {
+// pole rings, inverse.  South (theta = pi, Eq. 29): F_{-n}(pi) = sum_l scale(l) f_{l,-n} (-1)^{l-n};  north (theta = 0, Eq. 28,
+// MWSS only): F_n(0) = sum_l scale(l) f_{l,n}  (d^l_{mn}(0) = delta_mn, d^l_{mn}(pi) = (-1)^{l+m} delta_{m,-n}).  One block per slab.
+__global__ void k_pole_inverse(int L, int n, int north, const double2* __restrict__ coef, const double* __restrict__ scale, double2* __restrict__ out) {
     __shared__ double sre[256], sim[256];
-    const int an = n < 0 ? -n : n, NB = 2 * L - 1;
+    const int an = n < 0 ? -n : n, NB = 2 * L - 1, m = north ? n : -n;
     double re = 0, im = 0;
     for (int l = an + threadIdx.x; l < L; l += blockDim.x) {
-        double2 x = coef[(size_t)l * NB + (-n) + L - 1];
-        double s = scale[l] * sgn_pow(l - n);
+        double2 x = coef[(size_t)l * NB + m + L - 1];
+        double s = north ? scale[l] : scale[l] * sgn_pow(l - n);
         re += s * x.x; im += s * x.y;
     }
     sre[threadIdx.x] = re; sim[threadIdx.x] = im;
@@ -226,32 +227,38 @@ __global__ void k_complex_to_real(size_t n, const double2* __restrict__ in, doub
     if (i < n) out[i] = in[i].x;
 }
 
-// MW forward (ii): extension of F_m(theta_t) to the torus, t = L..2L-2: F_m(theta_t) = (-1)^{m-n} F_m(theta_{2L-2-t}).
-// The ring t = L-1 lies AT theta = pi, where a spin-s function (n = -s) has the single value c e^{i s phi}: only the order m = -n
-// survives (Eq. 29).  The samples of that ring are projected onto this component (F_m(pi) := 0 for m != -n), which
+// MW / MWSS forward (ii): extension of F_m(theta_t) to the theta circle of T samples:
+//   MW   (mwss = 0): T = 2L-1, theta_t = (2t+1)pi/T, rings t = 0..L-1 given, t = L..2L-2: F_m(theta_t) = (-1)^{m-n} F_m(theta_{2L-2-t})
+//   MWSS (mwss = 1): T = 2L,   theta_t = 2 pi t/T,   rings t = 0..L   given, t = L+1..2L-1: F_m(theta_t) = (-1)^{m-n} F_m(theta_{2L-t})
+// Rings AT a pole hold one value of a spin-s function (n = -s): at theta = pi only the order m = -n survives (Eq. 29),
+// at theta = 0 only m = n (Eq. 28).  The samples of those rings are projected onto that component (F_m := 0 for the other m), which
 // makes the transform well defined on arbitrary arrays (R21; include/b200sht.h, s2_forward).
-__global__ void k_mw_extend(int L, int n, int ldin, int ldout, const double2* __restrict__ Fa, double2* __restrict__ X) {
+__global__ void k_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* __restrict__ Fa, double2* __restrict__ X) {
     int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
-    const int T = 2 * L - 1;
+    const int T = mwss ? 2 * L : 2 * L - 1, tpole = mwss ? L : L - 1;
     if (t >= T) return;
     int m = b < L ? b : b - T;
     double2 v;
-    if (t == L - 1) { v = Fa[(size_t)b * ldin + t]; if (m != -n) v = make_double2(0.0, 0.0); }
-    else if (t < L) v = Fa[(size_t)b * ldin + t];
-    else { v = Fa[(size_t)b * ldin + (2 * L - 2 - t)]; double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
+    if (mwss && b == L) v = make_double2(0.0, 0.0);                  // phi-Nyquist bin of the 2L-point ring FFT: outside the band-limit
+    else if (t == tpole) { v = Fa[(size_t)b * ldin + t]; if (m != -n) v = make_double2(0.0, 0.0); }
+    else if (mwss && t == 0) { v = Fa[(size_t)b * ldin]; if (m != n) v = make_double2(0.0, 0.0); }
+    else if (t < tpole) v = Fa[(size_t)b * ldin + t];
+    else { v = Fa[(size_t)b * ldin + (2 * tpole - t)]; double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
     X[(size_t)b * ldout + t] = v;
 }
-// MW forward (iii)->(iv): F_{mm'} = (1/T) e^{-i m' pi/T} Y[m' mod T]; Z[m' mod T2] = F_{mm'} e^{+i m' pi/T2}; zero elsewhere.
-__global__ void k_mw_pad_phase(int L, int ldin, int ldout, const double2* __restrict__ Y, double2* __restrict__ Z) {
+// MW / MWSS forward (iii)->(iv): with Y = FFT_T of the extended samples, F_{mm'} = (1/T) e^{-i m' theta_0} Y[m' mod T] (theta_0 = pi/T
+// on MW, 0 on MWSS); Z[m' mod T2] = F_{mm'} e^{+i m' pi/T2} for |m'| <= L-1, zero elsewhere, so that the inverse FFT of length T2 = 4L
+// evaluates F_m on the midpoint rings theta'_u = (2u+1) pi/T2 (T2 samples of the circle; u < 2L are the rings in (0, pi)).
+__global__ void k_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* __restrict__ Y, double2* __restrict__ Z) {
     int k2 = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
-    const int T = 2 * L - 1, T2 = ldout;
+    const int T = mwss ? 2 * L : 2 * L - 1, T2 = ldout;
     if (k2 >= T2) return;
     int mp = k2 < L ? k2 : (k2 > T2 - L ? k2 - T2 : T2);      // |m'| <= L-1, else none
     double2 v = {0.0, 0.0};
     if (mp != T2) {
         double2 y = Y[(size_t)b * ldin + (mp < 0 ? mp + T : mp)];
-        double s1, c1, s2, c2;
-        sincospi(-(double)mp / (double)T, &s1, &c1);
+        double s1 = 0.0, c1 = 1.0, s2, c2;
+        if (!mwss) sincospi(-(double)mp / (double)T, &s1, &c1);
         sincospi((double)mp / (double)T2, &s2, &c2);
         double pr = c1 * c2 - s1 * s2, pi_ = c1 * s2 + s1 * c2;
         double inv = 1.0 / (double)T;
@@ -697,8 +704,8 @@ cudaError_t st_lamtab(int n, int nth, int ntp, int m_end, int nrows, const doubl
     k_lamtab<<<dim3(cdiv(ntp, 128), nrows), 128, 0, st>>>(n, nth, ntp, m_end, csc, tau, sig, lam);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_pole_inverse(int L, int n, const double2* coef, const double* scale, double2* out, cudaStream_t st) {
-    k_pole_inverse<<<1, 256, 0, st>>>(L, n, coef, scale, out);
+cudaError_t st_pole_inverse(int L, int n, int north, const double2* coef, const double* scale, double2* out, cudaStream_t st) {
+    k_pole_inverse<<<1, 256, 0, st>>>(L, n, north, coef, scale, out);
     count_bytes(16.0 * L); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st) {
@@ -715,15 +722,17 @@ cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStr
     k_complex_to_real<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
     count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st) {
-    dim3 grid(cdiv(2 * L - 1, 128), 2 * L - 1);
-    k_mw_extend<<<grid, 128, 0, st>>>(L, n, ldin, ldout, Fa, X);
-    count_bytes(32.0 * (double)(2 * L - 1) * (2 * L - 1)); LAUNCHED(); return cudaSuccess;
+cudaError_t st_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st) {
+    const int T = mwss ? 2 * L : 2 * L - 1;
+    dim3 grid(cdiv(T, 128), T);
+    k_mw_extend<<<grid, 128, 0, st>>>(L, n, mwss, ldin, ldout, Fa, X);
+    count_bytes(32.0 * (double)T * T); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st) {
-    dim3 grid(cdiv(ldout, 128), 2 * L - 1);
-    k_mw_pad_phase<<<grid, 128, 0, st>>>(L, ldin, ldout, Y, Z);
-    count_bytes(16.0 * (double)(2 * L - 1) * ((double)(2 * L - 1) + ldout)); LAUNCHED(); return cudaSuccess;
+cudaError_t st_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st) {
+    const int T = mwss ? 2 * L : 2 * L - 1;
+    dim3 grid(cdiv(ldout, 128), T);
+    k_mw_pad_phase<<<grid, 128, 0, st>>>(L, mwss, ldin, ldout, Y, Z);
+    count_bytes(16.0 * (double)T * ((double)T + ldout)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
                             const double* wq, const double2* U, double2* W, cudaStream_t st) {
@@ -742,9 +751,9 @@ cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* sc
     count_bytes(32.0 * (double)(2 * L - 1) * L); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st) {
-    dim3 grid(cdiv(ncol, 128), NB);
+    dim3 grid(cdiv(ncol, 128), 2 * L - 1);      // rows r = m + L - 1 of the m-ordered array; NB = number of phi bins of the other one
     k_rows_bin_to_mi<<<grid, 128, 0, st>>>(L, NB, ncol, ldsrc, lddst, to_mi, src, dst);
-    count_bytes(32.0 * (double)NB * ncol); LAUNCHED(); return cudaSuccess;
+    count_bytes(32.0 * (double)(2 * L - 1) * ncol); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st) {
     k_scale_copy<<<cdiv(n, 256), 256, 0, st>>>(n, s, in, out);

@@ -15,12 +15,12 @@ cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t
 cudaError_t st_sgtab(int nrows, int ncol, int mmin, int kstride, int kmin, const int8_t* kexp, double2* SG, cudaStream_t st);
 cudaError_t st_lamtab(int n, int nth, int ntp, int m_end, int nrows, const double* csc, const double* tau, const double* sig, double* lam,
                       cudaStream_t st);
-cudaError_t st_pole_inverse(int L, int n, const double2* coef, const double* scale, double2* out, cudaStream_t st);
+cudaError_t st_pole_inverse(int L, int n, int north, const double2* coef, const double* scale, double2* out, cudaStream_t st);
 cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st);
 cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStream_t st);
 cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st);
-cudaError_t st_mw_extend(int L, int n, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st);
-cudaError_t st_mw_pad_phase(int L, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
+cudaError_t st_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st);
+cudaError_t st_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
 cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
                             const double* wq, const double2* U, double2* W, cudaStream_t st);
 cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,

@@ -31,3 +31,17 @@ def project_so3_pole(f):
         fn[b] = ((fn[b] * np.conj(e)).sum() / na) * e
     f[:, -1, :] = np.fft.ifft(fn, axis=0)
     return f
+
+
+def project_mwss_poles(f, spin):
+    """MWSS maps f[..., L+1, 2L] hold BOTH poles as rings: theta = 0 keeps only the order m = -s (Eq. 28), theta = pi only m = +s
+    (Eq. 29)."""
+    f = np.array(f, copy=True)
+    n = f.shape[-1]
+    p = np.arange(n)
+    for ring, m in ((0, -spin), (-1, spin)):
+        e = np.exp(2j * np.pi * m * p / n)
+        c = (f[..., ring, :] * np.conj(e)).sum(-1, keepdims=True) / n
+        out = c * e
+        f[..., ring, :] = out.real if np.isrealobj(f) else out
+    return f
