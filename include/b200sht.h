@@ -62,7 +62,9 @@ enum {
     SHT_OPT_INVSYM   = 1u << 2,   /* spin-0 MW inverse on the L midpoint rings (2j+1)pi/(2L) with the fold, then an exact FFT
                                      resampling of F_m to the MW rings (off by default: measured not faster) */
     SHT_OPT_TILE64   = 1u << 3,   /* force 64-ring block tiles in the fused kernels ...                                          */
-    SHT_OPT_TILE128  = 1u << 4    /* ... or 128-ring tiles.  Default: 64 when 128-ring tiles give fewer blocks than the device has SMs */
+    SHT_OPT_TILE128  = 1u << 4,   /* ... or 128-ring tiles.  Default: 64 when 128-ring tiles give fewer blocks than the device has SMs */
+    SHT_OPT_ADJOINT  = 1u << 5    /* also build what the adjoint entry points need (complex fp64 single-map plans; MW / MWSS plans then
+                                     carry the tables of two more ring sets: about twice the workspace) */
 };
 enum { SHT_PEAK_DFMA = 0, SHT_PEAK_DMMA = 1, SHT_PEAK_FFMA = 2 };   /* sht_peak kinds */
 
@@ -132,6 +134,25 @@ sht_status so3_inverse_plan(sht_plan* plan, const void* flmn, void* f, sht_strea
 int        sht_plan_ntheta(const sht_plan* plan, int forward);
 sht_status s2_theta_inverse_plan(sht_plan* plan, const void* flm, void* Fm, sht_stream stream);
 sht_status s2_theta_forward_plan(sht_plan* plan, const void* Wm, void* flm, sht_stream stream);
+
+/* ---- adjoints (Sec. 5.3-5.4): the conjugate transposes of the four maps above, for plans created with
+ * SHT_OPT_ADJOINT (SHT_EUNSUPPORTED otherwise).  They are what a vector-Jacobian product of the (linear) transforms needs
+ * (VJP = conj(adjoint(conj v)), Eq. 51 / 57).  Same layouts as the transforms; the fused recursion kernels are the existing ones.
+ *   s2_forward_adjoint_plan : flm -> map,  F^H.  DH / GL / HEALPix: F^H = Q F^-1 (Eq. 52) -- the inverse transform with every ring
+ *                             multiplied by its quadrature weight.  MW / MWSS: the forward transform upsamples, so F^H is the inverse
+ *                             theta step ON THE 2L QUADRATURE RINGS, the weights, and the conjugate transposes of the upsampling, the
+ *                             torus extension (with the pole-ring projection) and the ring DFT.
+ *   s2_inverse_adjoint_plan : map -> flm,  (F^-1)^H = the analysis sum on the rings of the map WITHOUT quadrature weights (Eq. 56;
+ *                             F Q^-1 of Eq. 58 where a direct quadrature exists).
+ *   s2_theta_forward_adjoint_plan : flm -> Wm[2L-1][ntheta_q], the conjugate transpose of s2_theta_forward_plan (Eq. 62-63 without
+ *                             the factor Q_Theta, which that entry point does not apply either).
+ *   s2_theta_inverse_adjoint_plan : Fm[2L-1][ntheta] -> flm, the conjugate transpose of s2_theta_inverse_plan (Eq. 67-68).
+ * Identities (tests): <F x, y> = <x, F^H y> and <F^-1 c, g> = <c, (F^-1)^H g> to rounding, for arbitrary x, y, c, g.
+ */
+sht_status s2_forward_adjoint_plan(sht_plan* plan, const void* flm, void* f, sht_stream stream);
+sht_status s2_inverse_adjoint_plan(sht_plan* plan, const void* f, void* flm, sht_stream stream);
+sht_status s2_theta_forward_adjoint_plan(sht_plan* plan, const void* flm, void* Wm, sht_stream stream);
+sht_status s2_theta_inverse_adjoint_plan(sht_plan* plan, const void* Fm, void* flm, sht_stream stream);
 
 /* Stage timing.  After sht_plan_enable_timing(plan, 1) every transform records CUDA events between its stages;
  * sht_plan_timings() synchronises on the last transform's final event and returns milliseconds:

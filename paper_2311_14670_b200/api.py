@@ -40,7 +40,7 @@ class Plan:
     """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
 
     def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1, dtype="f64",
-                 fold=None, invsym=False, tile=None):
+                 fold=None, invsym=False, tile=None, adjoint=False):
         """fold / invsym / tile map to the SHT_OPT_* creation flags (None = the library's automatic choice)."""
         self._h = C.c_void_p()
         opts = 0
@@ -50,6 +50,8 @@ class Plan:
             opts |= _lib.SHT_OPT_INVSYM
         if tile is not None:
             opts |= {64: _lib.SHT_OPT_TILE64, 128: _lib.SHT_OPT_TILE128}[tile]
+        if adjoint:
+            opts |= _lib.SHT_OPT_ADJOINT
         self.L, self.spin, self.sampling, self.nside, self.reality, self.N = L, spin, sampling, nside, bool(reality), N
         self.batch = int(batch)
         if dtype not in ("f64", "f32"):
@@ -96,6 +98,34 @@ class Plan:
         out = torch.empty(self.map_shape, dtype=self.map_dtype, device=self.device) if out is None else out
         fn = lib().s2_inverse_plan if self.N is None else lib().so3_inverse_plan
         check(fn(self._h, _dev(flm, self.coef_dtype, self.coef_shape, "flm"), _dev(out, self.map_dtype, self.map_shape, "f"), _stream()))
+        return out
+
+    # -- adjoints (plans created with adjoint=True; Eq. 52 / 58) --
+    def forward_adjoint(self, flm, out=None):
+        """F^H: coefficients -> map (the conjugate transpose of forward)."""
+        out = torch.empty(self.map_shape, dtype=self.map_dtype, device=self.device) if out is None else out
+        check(lib().s2_forward_adjoint_plan(self._h, _dev(flm, self.coef_dtype, self.coef_shape, "flm"),
+                                            _dev(out, self.map_dtype, self.map_shape, "f"), _stream()))
+        return out
+
+    def inverse_adjoint(self, f, out=None):
+        """(F^-1)^H: map -> coefficients (the conjugate transpose of inverse)."""
+        out = torch.empty(self.coef_shape, dtype=self.coef_dtype, device=self.device) if out is None else out
+        check(lib().s2_inverse_adjoint_plan(self._h, _dev(f, self.map_dtype, self.map_shape, "f"),
+                                            _dev(out, self.coef_dtype, self.coef_shape, "flm"), _stream()))
+        return out
+
+    def theta_forward_adjoint(self, flm):
+        """Conjugate transpose of theta_forward: flm -> W[2L-1, ntheta_q] (Eq. 62-63 without Q_Theta)."""
+        out = torch.empty((2 * self.L - 1, self.ntheta(True)), dtype=torch.complex128, device=self.device)
+        check(lib().s2_theta_forward_adjoint_plan(self._h, _dev(flm, torch.complex128, self.coef_shape, "flm"), C.c_void_p(out.data_ptr()), _stream()))
+        return out
+
+    def theta_inverse_adjoint(self, F):
+        """Conjugate transpose of theta_inverse: F[2L-1, ntheta] -> flm (Eq. 67-68)."""
+        shape = (2 * self.L - 1, self.ntheta(False))
+        out = torch.empty(self.coef_shape, dtype=torch.complex128, device=self.device)
+        check(lib().s2_theta_inverse_adjoint_plan(self._h, _dev(F, torch.complex128, shape, "F"), C.c_void_p(out.data_ptr()), _stream()))
         return out
 
     def ntheta(self, forward):

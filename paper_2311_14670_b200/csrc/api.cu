@@ -74,6 +74,8 @@ struct PassHost {
 };
 
 enum { CAT_HOT = 0, CAT_FFT = 1, CAT_STAGE = 2 };
+// internal samplings of the adjoint helper plans: the rings of an MW / MWSS map with a direct, unit-weight "quadrature"
+enum { SHT_INT_MWRINGS = 100, SHT_INT_MWSSRINGS = 101 };
 
 }  // namespace
 
@@ -101,6 +103,14 @@ struct sht_plan {
     bool upsampled = false;    // MW / MWSS: the forward transform extends F_m to the theta circle and upsamples to the quadrature rings
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
     unsigned opts = 0;         // SHT_OPT_* given at creation
+    // Helper plans of the adjoint entry points (SHT_OPT_ADJOINT; MW / MWSS only, where the forward quadrature does not run on the
+    // rings of the map): adj_inv runs the FORWARD-type kernel on the rings of the map ((F^-1)^H, Eq. 58), adj_fwd runs the
+    // INVERSE-type kernel on the 2L quadrature rings (F^H, Eq. 52).  A helper owns only the tables / buffers of its one direction.
+    sht_plan *adj_inv = nullptr, *adj_fwd = nullptr;
+    bool helper = false;
+    int only_dir = 0;          // helper plans: 1 = inverse-type kernel only, 2 = forward-type kernel only
+    double* wq_map = nullptr;  // [F_ld] quadrature weight of every ring of the map (direct-quadrature samplings; adjoints)
+    double* wq_quad = nullptr; // [4L] MW / MWSS: weight of every one of the 2L quadrature rings (not folded; adjoints)
     int device = 0, nsm = 0;   // device the plan was created on and its SM count (tile choice)
     int* d_flag = nullptr;     // device flag raised by table kernels (start value outside the window-counter range)
     double sec_bytes[3] = {0, 0, 0};   // algorithmic bytes moved by the FFT / staging sections of the last transform (stage timing)
@@ -287,7 +297,7 @@ void plan_dims(sht_plan* P) {
     P->M = 2 * L - 1;
     P->upsampled = P->sampling == SHT_MW || P->sampling == SHT_MWSS;
     switch (P->sampling) {
-        case SHT_MWSS: P->NB = 2 * L; P->nrmap = L + 1; break;
+        case SHT_MWSS: case SHT_INT_MWSSRINGS: P->NB = 2 * L; P->nrmap = L + 1; break;
         case SHT_DH: P->NB = 2 * L - 1; P->nrmap = 2 * L; break;
         default: P->NB = 2 * L - 1; P->nrmap = L; break;         // MW, GL; HEALPix keeps 2L-1 "bins" as its F-row convention
     }
@@ -325,6 +335,7 @@ void layout(sht_plan* P, char* base) {
     P->scale_inv = B.take<double>(Lp);
     P->scale_fwd = B.take<double>(Lp);
     for (RingSet* R : {&P->inv, &P->fwd}) {
+        if ((R == &P->inv && P->only_dir == 2) || (R == &P->fwd && P->only_dir == 1)) continue;
         R->csc = B.take<double>(R->ntp); R->tau = B.take<double>(R->ntp); R->sig = B.take<double>(R->ntp);
         R->c2hi = B.take<double>(R->ntp); R->c2lo = B.take<double>(R->ntp);
         R->s2hi = B.take<double>(R->ntp); R->s2lo = B.take<double>(R->ntp);
@@ -339,7 +350,7 @@ void layout(sht_plan* P, char* base) {
     P->d_fwd_pm = B.take<ThetaPass>(P->pfwd.size() + 1); P->d_fwd_p = B.take<ThetaPass>(P->pfwd.size() + 1);
     // per-pass operand buffers and lambda tables
     // (rows m = m_end-1 .. L-1; row m_end-1 is all zero: the dummy second step of a final odd pair reads it)
-    for (auto& ph : P->pinv) {
+    for (auto& ph : P->pinv) {      // (empty for forward-only helpers, and vice versa)
         ph.p.in = B.take<double>(pass_in_doubles(P, ph, false));
         ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->inv.ntp);
     }
@@ -355,20 +366,24 @@ void layout(sht_plan* P, char* base) {
         P->Ob = B.take<double>(oi > of ? oi : of);
     }
     // scratch arrays (dimensions fixed by plan_dims)
-    P->F = B.take<double2>(P->F_slab * P->nslab);
+    if (P->only_dir != 2) P->F = B.take<double2>(P->F_slab * P->nslab);
     P->polev = B.take<double2>(P->nslab);
     P->tmp = B.take<double>(2 * (size_t)Lp);
     P->unit_wq = B.take<double>(P->fwd.ntp);
-    if (P->sampling != SHT_HEALPIX) {
-        P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
-        if (P->upsampled) P->X = B.take<double2>(P->X_slab * P->nslab);
-    } else {
-        P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
-        P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
-        P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
+    P->wq_map = B.take<double>(P->F_ld);
+    P->wq_quad = B.take<double>(4 * (size_t)L);
+    if (!P->helper) {
+        if (P->sampling != SHT_HEALPIX) {
+            P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
+            if (P->upsampled) P->X = B.take<double2>(P->X_slab * P->nslab);
+        } else {
+            P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
+            P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
+            P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
+        }
+        P->Z = B.take<double2>(P->Z_slab * P->nslab);
     }
-    P->Z = B.take<double2>(P->Z_slab * P->nslab);
-    P->H = B.take<double2>(P->H_slab * P->nslab);
+    if (P->only_dir != 1) P->H = B.take<double2>(P->H_slab * P->nslab);
     if (P->reality && P->sampling != SHT_HEALPIX) P->cplx = B.take<double2>(P->map_elems * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
     if (P->dtype == SHT_F32) {
@@ -386,6 +401,9 @@ void layout(sht_plan* P, char* base) {
         for (size_t i = 0; i < P->pinv.size(); ++i) P->pinv[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_inv[i]);
         for (size_t i = 0; i < P->pfwd.size(); ++i) P->pfwd[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_fwd[i]);
     }
+    // the helper plans of the adjoints live at the end of the same workspace
+    for (sht_plan* Q : {P->adj_inv, P->adj_fwd})
+        if (Q) { B.off = rup(B.off, 256); Q->work = base ? base + B.off : nullptr; B.off += Q->need_bytes; }
     P->need_bytes = rup(B.off, 256);
 }
 
@@ -406,11 +424,16 @@ void add_passes(sht_plan* P, int slab, int n, bool real) {
         P->pinv.push_back(a); P->pinv.push_back(b);
         // forward: the quadrature rings are symmetric about the equator, so ONE pass serves order +m from its own ring and order
         // -m from the mirrored ring (d^l_{-m,n}(pi - theta) = (-1)^{l-n} d^l_{m,n}(theta)): two orders per d-step
-        PassHost c = mk(n, +1, -an, 0, 2 * n);
-        c.p.fold = 1;
-        P->pfwd.push_back(c);
+        if (P->fwd.symmetric) {
+            PassHost c = mk(n, +1, -an, 0, 2 * n);
+            c.p.fold = 1;
+            P->pfwd.push_back(c);
+            P->fwd.start[n]; P->fwd.mlo[2 * n];
+        } else {        // (the MW rings, adjoint helper): no mirror ring to serve -m from: two passes, as on the inverse side
+            P->pfwd.push_back(a); P->pfwd.push_back(b);
+            P->fwd.start[n]; P->fwd.start[-n]; P->fwd.mlo[2 * n]; P->fwd.mlo[2 * n + 1];
+        }
         P->inv.start[n]; P->inv.start[-n]; P->inv.mlo[2 * n]; P->inv.mlo[2 * n + 1];
-        P->fwd.start[n]; P->fwd.mlo[2 * n];
     }
 }
 
@@ -523,6 +546,8 @@ sht_status plan_common(sht_plan* P) {
         P->ncg_fwd = (P->batch * (P->pfwd[0].mode == 0 ? 2 : 1) + 15) / 16;
     } else
         for (int s = 0; s < P->nslab; ++s) add_passes(P, s, P->slab_n[s], P->reality != 0);
+    if (P->only_dir == 1) { P->pfwd.clear(); P->fwd.start.clear(); P->fwd.mlo.clear(); }
+    if (P->only_dir == 2) { P->pinv.clear(); P->inv.start.clear(); P->inv.mlo.clear(); }
     // d-step counts: rings * sum over l of the steps each pass runs
     for (int dir = 0; dir < 2; ++dir) {
         // algorithmic flop per d-step: 6 (recursion, as the paper states it) + 4 per order served and map
@@ -536,7 +561,7 @@ sht_status plan_common(sht_plan* P) {
         (dir ? P->dsteps_fwd : P->dsteps_inv) = tot * R.nth;
         (dir ? P->flops_fwd : P->flops_inv) = fl * R.nth;
     }
-    CS(make_fft_plans(P));
+    if (!P->helper) CS(make_fft_plans(P));
     layout(P, nullptr);
     return SHT_OK;
 }
@@ -788,10 +813,6 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
             CK(st_unpack_batch(L, P->Lp, P->Lp, L, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, 1, ph.p.fold,
                                P->ctab, reinterpret_cast<const double*>(ph.p.out), rows * P->Lp * SHT_MMA_NCOL, P->H, P->H_slab, P->Lp, st));
         }
-        if (P->fwd.pole) {
-            for (int s = 0; s < P->nslab; ++s)
-                CK(st_pole_forward(L, P->Lp, P->slab_n[s], P->NB, ldu, P->fwd.nth, P->fwd.wq, U + U_slab * s, P->H + P->H_slab * s, st));
-        }
         return SHT_OK;
     }
     if (P->dtype == SHT_F32) {
@@ -825,9 +846,12 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     stage(P, CAT_HOT, st);
     CK(launch_theta_forward(theta_args(P, true, true), 0, st));
     CK(launch_theta_forward(theta_args(P, true, false), 1, st));
-    if (P->fwd.pole) {
-        for (int s = 0; s < P->nslab; ++s)
-            CK(st_pole_forward(L, P->Lp, P->slab_n[s], P->NB, ldu, P->fwd.nth, P->fwd.wq, U + U_slab * s, P->H + P->H_slab * s, st));
+    // pole rings of the ring set (only the adjoint helpers on the rings of an MW / MWSS map have any; unit weight): U points at
+    // the first regular ring, the south pole follows the regular rings, the north pole precedes them
+    const int nreg = P->fwd.nfull ? P->fwd.nfull : P->fwd.nth;
+    for (int s = 0; s < P->nslab; ++s) {
+        if (P->fwd.pole) CK(st_pole_forward(L, P->Lp, P->slab_n[s], 0, P->NB, ldu, nreg, 1.0, U + U_slab * s, P->H + P->H_slab * s, st));
+        if (P->fwd.pole_n) CK(st_pole_forward(L, P->Lp, P->slab_n[s], 1, P->NB, ldu, -1, 1.0, U + U_slab * s, P->H + P->H_slab * s, st));
     }
     return SHT_OK;
 }
@@ -941,11 +965,13 @@ sht_status sht_plan_s2(sht_plan** out, int L, int spin, int sampling, int nside,
 sht_status sht_plan_s2_batch(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch) {
     return sht_plan_s2_opts(out, L, spin, sampling, nside, reality, dtype, batch, 0u);
 }
-sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch, unsigned opts) {
+static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch, unsigned opts,
+                               int only_dir, bool helper) {
     if (!out) return SHT_EINVAL;
     *out = nullptr;
     if (batch < 1 || batch > 1024) return SHT_EINVAL;
-    if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || sampling < SHT_MW || sampling > SHT_GL) return SHT_EINVAL;
+    const bool internal = helper && (sampling == SHT_INT_MWRINGS || sampling == SHT_INT_MWSSRINGS);
+    if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || ((sampling < SHT_MW || sampling > SHT_GL) && !internal)) return SHT_EINVAL;
     if (batch > 1 && sampling != SHT_MW) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
@@ -955,7 +981,7 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
     if (dtype == SHT_F32 && (spin != 0 || sampling != SHT_MW || batch != 1)) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
-    P->dtype = dtype; P->opts = opts;
+    P->dtype = dtype; P->opts = opts; P->helper = helper; P->only_dir = only_dir;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     query_device(P);
@@ -965,6 +991,8 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
         case SHT_MWSS: rings_mwss(P->inv, L); rings_mid(P->fwd, 2 * L); break;       // Eq. 39; same quadrature rings
         case SHT_DH: rings_mid(P->inv, 2 * L); rings_mid(P->fwd, 2 * L); break;      // Eq. 34: theta_t = (2t+1)pi/(4L) -- the midpoint rings themselves
         case SHT_GL: rings_gl(P->inv, L, nullptr); rings_gl(P->fwd, L, &P->gl_w); break;   // roots of P_L
+        case SHT_INT_MWRINGS: rings_mw(P->inv, L); rings_mw(P->fwd, L); break;        // adjoint helper: the rings of an MW map
+        case SHT_INT_MWSSRINGS: rings_mwss(P->inv, L); rings_mwss(P->fwd, L); break;  // adjoint helper: the rings of an MWSS map
         default: rings_healpix(P->inv, nside); rings_healpix(P->fwd, nside); break;
     }
     if (spin == 0) {
@@ -974,7 +1002,7 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
         bool on = tiles >= 2 * (long)P->nsm;
         if (opts & SHT_OPT_FOLD_ON) on = true;
         if (opts & SHT_OPT_FOLD_OFF) on = false;
-        if (on) { P->fold0 = 1; north_only(P->fwd); }
+        if (on && P->fwd.symmetric && only_dir != 1) { P->fold0 = 1; north_only(P->fwd); }
         // MW inverse: the MW rings (2t+1)pi/(2L-1) are not symmetric; SHT_OPT_INVSYM evaluates F_m on the L midpoint rings instead
         // (folded) and resamples to the MW rings with two FFT passes (resample_sym_to_mw).  Off by default: the two-column folded
         // inverse kernel only fits shared memory with 64-ring tiles and gains 17 % on the hot kernel at L = 2048 (3.03 -> 2.53 ms)
@@ -983,16 +1011,29 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
         if (isym) { P->invsym = 1; P->fold0i = 1; rings_mid(P->inv, L); north_only(P->inv); }
         // the rings of the map are symmetric about the equator on every sampling but MW: fold the inverse too.  DH has 2L rings, so
         // its folded inverse does the work of an MW inverse; it is folded whatever the size.
-        if ((on || sampling == SHT_DH) && !(opts & SHT_OPT_FOLD_OFF) && sampling != SHT_MW && batch == 1 && P->inv.symmetric) {
+        if ((on || sampling == SHT_DH) && !(opts & SHT_OPT_FOLD_OFF) && sampling != SHT_MW && batch == 1 && P->inv.symmetric && only_dir != 2) {
             P->fold0i = 1; north_only(P->inv);
         }
     }
     sht_status s = check_start_range(P);
+    if (s == SHT_OK && (opts & SHT_OPT_ADJOINT) && !helper) {
+        // adjoint entry points (Eq. 52 / 58): complex fp64 single-map plans
+        if (batch != 1 || dtype != SHT_F64 || reality) { g_err = "SHT_OPT_ADJOINT needs a complex fp64 single-map plan"; s = SHT_EUNSUPPORTED; }
+        else if (sampling == SHT_MW || sampling == SHT_MWSS) {
+            const unsigned hopts = opts & ~(unsigned)(SHT_OPT_ADJOINT | SHT_OPT_INVSYM);
+            s = make_s2_plan(&P->adj_inv, L, spin, sampling == SHT_MW ? SHT_INT_MWRINGS : SHT_INT_MWSSRINGS, 0, 0, dtype, 1, hopts, 2, true);
+            if (s == SHT_OK) s = make_s2_plan(&P->adj_fwd, L, spin, SHT_DH, 0, 0, dtype, 1, hopts, 1, true);
+        }
+    }
     if (s == SHT_OK) s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
     return SHT_OK;
 }
+sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int nside, int reality, int dtype, int batch, unsigned opts) {
+    return make_s2_plan(out, L, spin, sampling, nside, reality, dtype, batch, opts, 0, false);
+}
+
 sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     if (!out) return SHT_EINVAL;
     *out = nullptr;
@@ -1045,8 +1086,31 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         }
     }
     CS(up(si, P->scale_inv, st)); CS(up(sf, P->scale_fwd, st));
-    CS(fill_ringset(P, P->inv, st)); CS(fill_ringset(P, P->fwd, st));
+    if (P->only_dir != 2) CS(fill_ringset(P, P->inv, st));
+    if (P->only_dir != 1) CS(fill_ringset(P, P->fwd, st));
+    { std::vector<double> ones(P->fwd.ntp, 1.0); CS(up(ones, P->unit_wq, st)); }
+    CK(cudaMemsetAsync(P->wq_map, 0, sizeof(double) * P->F_ld, st));
+    CK(cudaMemsetAsync(P->wq_quad, 0, sizeof(double) * 4 * (size_t)L, st));
+    if (P->helper) {
+        // helper plans of the adjoints: only tables and pass lists; the forward-type helper sums with unit weights (Eq. 56)
+        if (P->only_dir != 1) CK(cudaMemcpyAsync(P->fwd.wq, P->unit_wq, sizeof(double) * P->fwd.ntp, cudaMemcpyDeviceToDevice, st));
+        CS(upload_passes(P, st));
+        CK(cudaStreamSynchronize(st));
+        int hflag = 0;
+        CK(cudaMemcpy(&hflag, P->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+        if (hflag) { g_err = "Eq. 27 start values fall below the window-counter range on this ring set"; return SHT_EUNSUPPORTED; }
+        P->ready = true;
+        return SHT_OK;
+    }
     CK(cudaMemsetAsync(P->fwd.wq, 0, sizeof(double) * P->fwd.ntp, st));
+    if (P->upsampled) CK(st_mid_weights(L, 2 * L, (double)(2 * PI_L / (ld)P->NB), P->wq_quad, st));      // all 2L quadrature rings
+    if (P->sampling == SHT_DH) CK(st_mid_weights(L, 2 * L, (double)(2 * PI_L / (ld)P->NB), P->wq_map, st));
+    if (P->sampling == SHT_GL || P->sampling == SHT_HEALPIX) {
+        std::vector<double> w(P->F_ld, 0.0);
+        for (int t = 0; t < P->nrmap; ++t)
+            w[t] = P->sampling == SHT_GL ? (double)(2 * PI_L / (ld)(2 * L - 1) * P->gl_w[t]) : (double)(4 * PI_L / (12.0L * (ld)P->nside * (ld)P->nside));
+        CS(up(w, P->wq_map, st));
+    }
     if (P->sampling == SHT_MW || P->sampling == SHT_MWSS || P->sampling == SHT_DH) {
         // forward quadrature weights q_u = q_Phi v_u on the 2L midpoint rings, q_Phi = 2 pi / (phi samples per ring).  MW / MWSS: Eq. 41-44
         // restated for that ring set (R9).  DH: the rings ARE the DH rings and v_u equals the DH weight of Eq. 36 (Fejer's first
@@ -1063,8 +1127,9 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         for (int t = 0; t < P->fwd.nth; ++t) w[t] = (double)(4 * PI_L / (12.0L * (ld)P->nside * (ld)P->nside));
         CS(up(w, P->fwd.wq, st));
     }
-    { std::vector<double> ones(P->fwd.ntp, 1.0); CS(up(ones, P->unit_wq, st)); }
     CS(upload_passes(P, st));
+    for (sht_plan* Q : {P->adj_inv, P->adj_fwd})
+        if (Q) CS(sht_plan_set_workspace(Q, Q->work, Q->need_bytes, stream));
     if (P->dtype == SHT_F32) {
         CK(st_ab32(L, Lp, P->ab32, st));
         CK(st_start32((size_t)Lp * P->inv.ntp, P->inv.start[0].val, P->inv.start[0].k, P->st32_inv, P->k16_inv, st));
@@ -1103,6 +1168,7 @@ sht_status sht_plan_destroy(sht_plan* P) {
             if (h) cufftDestroy(h);
     }
     for (auto e : P->ev) cudaEventDestroy(e);
+    sht_plan_destroy(P->adj_inv); sht_plan_destroy(P->adj_fwd);
     delete P;
     return SHT_OK;
 }
@@ -1239,6 +1305,99 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
         CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + ncoef * b, st));
     stage(P, CAT_STAGE, st);
     return SHT_OK;
+}
+
+// ---- adjoints (Sec. 5.3-5.4) -----------------------------------------------------------------------------------
+namespace {
+sht_status check_adjoint(const sht_plan* P) {
+    if (!(P->opts & SHT_OPT_ADJOINT)) { g_err = "plan was not created with SHT_OPT_ADJOINT"; return SHT_EUNSUPPORTED; }
+    return SHT_OK;
+}
+// forward-type kernel with unit weights on the rings of the map: U = F_m on those rings ([bin][ld], columns in map-ring order)
+sht_status adjoint_analysis(sht_plan* P, const double2* U, size_t U_slab, int ldu, double2* flm, cudaStream_t st) {
+    if (P->adj_inv) {           // MW / MWSS: helper plan on the rings of the map; U points at its first regular ring
+        sht_plan* Q = P->adj_inv;
+        CS(run_theta_forward(Q, U + P->col0, U_slab, ldu, st));
+        CK(st_finalize_forward(P->L, Q->Lp, Q->slab_n[0], 0, Q->scale_fwd, Q->H, flm, st));
+        return SHT_OK;
+    }
+    double* saved = P->fwd.wq;
+    P->fwd.wq = P->unit_wq;
+    sht_status s = run_theta_forward(P, U, U_slab, ldu, st);
+    P->fwd.wq = saved;
+    CS(s);
+    CK(st_finalize_forward(P->L, P->Lp, P->slab_n[0], 0, P->scale_fwd, P->H, flm, st));
+    return SHT_OK;
+}
+// inverse-type kernel on the quadrature rings: returns the array [bins][ld] holding F_m on ALL quadrature rings (unweighted)
+sht_status adjoint_synthesis(sht_plan* P, const double2* flm, const double2** Fq, int* NBq, int* ldq, cudaStream_t st) {
+    sht_plan* Q = P->adj_fwd ? P->adj_fwd : P;      // MW / MWSS: helper plan on the 2L midpoint rings
+    CS(run_theta_inverse(Q, flm, st));
+    *Fq = Q->F; *NBq = Q->NB; *ldq = Q->F_ld;
+    return SHT_OK;
+}
+}  // namespace
+
+sht_status s2_inverse_adjoint_plan(sht_plan* P, const void* f, void* flm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+    CS(check_adjoint(P));
+    cudaStream_t st = (cudaStream_t)stream;
+    begin_transform(P);
+    if (P->sampling == SHT_HEALPIX) {
+        CS(healpix_analysis(P, f, st));                                          // ring DFTs with the ring phases: conj. transpose of Eq. 32
+        return adjoint_analysis(P, P->Z, P->Z_slab, P->fwd_ld, (double2*)flm, st);
+    }
+    CS(fft_exec(P, P->fft_phi_fwd, (double2*)const_cast<void*>(f), P->Fa, CUFFT_FORWARD, st));
+    return adjoint_analysis(P, P->Fa, P->Fa_slab, P->Ltp, (double2*)flm, st);
+}
+sht_status s2_theta_inverse_adjoint_plan(sht_plan* P, const void* Fm, void* flm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
+    CS(check_adjoint(P));
+    cudaStream_t st = (cudaStream_t)stream;
+    begin_transform(P);
+    const int nt = sht_plan_ntheta(P, 0);
+    double2* U = P->sampling == SHT_HEALPIX ? P->Z : P->Fa;
+    const int ldu = P->sampling == SHT_HEALPIX ? P->fwd_ld : P->Ltp;
+    CK(st_rows_reorder(P->L, P->NB, nt, nt, ldu, 0, (const double2*)Fm, U, st));
+    return adjoint_analysis(P, U, P->sampling == SHT_HEALPIX ? P->Z_slab : P->Fa_slab, ldu, (double2*)flm, st);
+}
+sht_status s2_theta_forward_adjoint_plan(sht_plan* P, const void* flm, void* Wm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !Wm || P->kind != 0) return SHT_EINVAL;
+    CS(check_adjoint(P));
+    cudaStream_t st = (cudaStream_t)stream;
+    begin_transform(P);
+    const double2* Fq; int NBq, ldq;
+    CS(adjoint_synthesis(P, (const double2*)flm, &Fq, &NBq, &ldq, st));
+    const int nq = sht_plan_ntheta(P, 1);
+    CK(st_rows_reorder(P->L, NBq, nq, ldq, nq, 1, Fq, (double2*)Wm, st));
+    return SHT_OK;
+}
+sht_status s2_forward_adjoint_plan(sht_plan* P, const void* flm, void* f, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+    CS(check_adjoint(P));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int L = P->L;
+    begin_transform(P);
+    const double2* Fq; int NBq, ldq;
+    CS(adjoint_synthesis(P, (const double2*)flm, &Fq, &NBq, &ldq, st));
+    if (!P->upsampled) {
+        // direct quadrature (DH, GL, HEALPix): F = Y^H Q, so F^H = Q Y -- Eq. 52 literally: weight the rings, then the ring synthesis
+        CK(st_scale_cols(P->NB, P->nrmap, P->F_ld, P->wq_map, P->F, st));
+        if (P->sampling == SHT_HEALPIX) return healpix_synthesis(P, f, st);
+        return fft_exec(P, P->fft_phi_inv, P->F, (double2*)f, CUFFT_INVERSE, st);
+    }
+    // MW / MWSS: conjugate transpose of weights + upsampling + extension (mw_upsample), then of the ring DFT
+    const int mwss = P->sampling == SHT_MWSS, T2 = 4 * L;
+    CK(st_adj_weight_pad(L, NBq, ldq, Fq, P->wq_quad, P->NB, T2, P->Z, st));
+    CS(fft_exec(P, P->fft_th2, P->Z, P->Z, CUFFT_FORWARD, st));
+    CK(st_adj_trunc_phase(L, mwss, P->NB, T2, P->Z, P->X, st));
+    CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_INVERSE, st));
+    CK(st_adj_fold(L, P->slab_n[0], mwss, P->NB, P->nrmap, P->F_ld, P->X, P->F, st));
+    return fft_exec(P, P->fft_phi_inv, P->F, (double2*)f, CUFFT_INVERSE, st);
 }
 
 // ---- SO(3) (Eq. 15-18) ----------------------------------------------------------------------------

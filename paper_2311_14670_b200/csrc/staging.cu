@@ -354,15 +354,16 @@ __global__ void k_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp
         w[c] = e; w[NC + c] = o;
     }
 }
-// pole ring theta = pi, forward (Eq. 29): H[-n+L-1][l] += (-1)^{l-n} * wq_pole * U_{-n}(pi)
-__global__ void k_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* __restrict__ wq,
-                               const double2* __restrict__ U, double2* __restrict__ H) {
+// pole rings, forward.  South (theta = pi, Eq. 29): H[-n+L-1][l] += (-1)^{l-n} w U_{-n}(pi);  north (theta = 0, Eq. 28): H[n+L-1][l] += w U_n(0).
+// `col` is the ring's column of U (may be -1 when U points at the first regular ring and the north pole precedes it).
+__global__ void k_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* __restrict__ U,
+                               double2* __restrict__ H) {
     int l = blockIdx.x * blockDim.x + threadIdx.x;
     const int an = n < 0 ? -n : n;
     if (l >= L || l < an) return;
-    int mo = -n;
-    double2 x = U[(size_t)(mo < 0 ? mo + NBin : mo) * ldin + upole];
-    double s = wq[upole] * sgn_pow(l - n);
+    int mo = north ? n : -n;
+    double2 x = U[(ptrdiff_t)(mo < 0 ? mo + NBin : mo) * ldin + col];
+    double s = north ? w : w * sgn_pow(l - n);
     double2* h = H + (size_t)(mo + L - 1) * Lp + l;
     h->x += s * x.x; h->y += s * x.y;
 }
@@ -404,6 +405,62 @@ __global__ void k_rows_bin_to_mi(int L, int NB, int ncol, int ldsrc, int lddst, 
 __global__ void k_scale_copy(size_t n, double s, const double2* __restrict__ in, double2* __restrict__ out) {
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) out[i] = make_double2(s * in[i].x, s * in[i].y);
+}
+
+// ---- adjoint transforms (Sec. 5.3): conjugate transposes of the staging steps above -------------------------------
+// F[row][c] *= w[c]: the diagonal operator Q of Eq. 52 on the rings of the map (direct-quadrature samplings)
+__global__ void k_scale_cols(int ncol, int ld, const double* __restrict__ w, double2* __restrict__ F) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y;
+    if (c >= ncol) return;
+    double2 v = F[(size_t)r * ld + c];
+    const double s = w[c];
+    F[(size_t)r * ld + c] = make_double2(s * v.x, s * v.y);
+}
+// Adjoint of "weights, restriction to u < 2L": Z[bin(m)][u] = q_u Fq[binq(m)][u] for u < 2L, 0 for 2L <= u < T2 = 4L.  Fq has NBq = 2L-1
+// bins (the helper plan's rows), Z has NB bins; on MWSS the phi-Nyquist bin b = L carries nothing.
+__global__ void k_adj_weight_pad(int L, int NBq, int ldq, const double2* __restrict__ Fq, const double* __restrict__ wq, int NB, int T2,
+                                 double2* __restrict__ Z) {
+    int u = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (u >= T2) return;
+    double2 v = make_double2(0.0, 0.0);
+    const int m = b < L ? b : b - NB;
+    if (u < 2 * L && m > -L) {
+        const double2 x = Fq[(size_t)(m < 0 ? m + NBq : m) * ldq + u];
+        v = make_double2(wq[u] * x.x, wq[u] * x.y);
+    }
+    Z[(size_t)b * T2 + u] = v;
+}
+// Adjoint of k_mw_pad_phase: X[b][m' mod T] = (1/T) e^{+i m' theta_0} e^{-i m' pi/T2} Zf[b][m' mod T2] for |m'| <= L-1, 0 elsewhere
+__global__ void k_adj_trunc_phase(int L, int mwss, int T2, const double2* __restrict__ Zf, double2* __restrict__ X) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const int T = mwss ? 2 * L : 2 * L - 1;
+    if (k >= T) return;
+    const int mp = k < L ? k : k - T;
+    double2 v = make_double2(0.0, 0.0);
+    if (mp > -L) {
+        const double2 y = Zf[(size_t)b * T2 + (mp < 0 ? mp + T2 : mp)];
+        double s1 = 0.0, c1 = 1.0, s2, c2;
+        if (!mwss) sincospi((double)mp / (double)T, &s1, &c1);
+        sincospi(-(double)mp / (double)T2, &s2, &c2);
+        const double pr = c1 * c2 - s1 * s2, pi_ = c1 * s2 + s1 * c2, inv = 1.0 / (double)T;
+        v = make_double2((y.x * pr - y.y * pi_) * inv, (y.x * pi_ + y.y * pr) * inv);
+    }
+    X[(size_t)b * T + k] = v;
+}
+// Adjoint of k_mw_extend: F[b][t] = X[b][t] + (-1)^{m-n} X[b][2 t_pole - t] on the regular rings; the pole rings keep X only for the one
+// order a spin function can hold there (the projection is diagonal, hence self-adjoint); the MWSS phi-Nyquist bin is zero.
+__global__ void k_adj_fold(int L, int n, int mwss, int nrmap, int ldf, const double2* __restrict__ X, double2* __restrict__ F) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const int T = mwss ? 2 * L : 2 * L - 1, tpole = mwss ? L : L - 1;
+    if (t >= nrmap) return;
+    const int m = b < L ? b : b - T;
+    const double2* x = X + (size_t)b * T;
+    double2 v = make_double2(0.0, 0.0);
+    if (mwss && b == L) { }
+    else if (t == tpole) { if (m == -n) v = x[t]; }
+    else if (mwss && t == 0) { if (m == n) v = x[0]; }
+    else { const double2 r = x[2 * tpole - t]; const double s = sgn_pow(m - n); v = make_double2(x[t].x + s * r.x, x[t].y + s * r.y); }
+    F[(size_t)b * ldf + t] = v;
 }
 
 // ---- batched path (theta_mma.cu; operand layouts in internal.h) ----------------------------------------------------
@@ -740,9 +797,9 @@ cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC,
     k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, fold, m_lo, wq, U, W);
     count_bytes(32.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
+cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
                             cudaStream_t st) {
-    k_pole_forward<<<cdiv(L, 128), 128, 0, st>>>(L, Lp, n, NBin, ldin, upole, wq, U, H);
+    k_pole_forward<<<cdiv(L, 128), 128, 0, st>>>(L, Lp, n, north, NBin, ldin, col, w, U, H);
     count_bytes(32.0 * L); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st) {
@@ -834,4 +891,21 @@ cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st) {
 cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st) {
     k_rows_head<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ldin, ldout, in, out);
     count_bytes(32.0 * (double)nrows * ncol); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_scale_cols(int nrows, int ncol, int ld, const double* w, double2* F, cudaStream_t st) {
+    k_scale_cols<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ld, w, F);
+    count_bytes(32.0 * (double)nrows * ncol); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_adj_weight_pad(int L, int NBq, int ldq, const double2* Fq, const double* wq, int NB, int T2, double2* Z, cudaStream_t st) {
+    k_adj_weight_pad<<<dim3(cdiv(T2, 128), NB), 128, 0, st>>>(L, NBq, ldq, Fq, wq, NB, T2, Z);
+    count_bytes(16.0 * (double)NB * (2.0 * L + T2)); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_adj_trunc_phase(int L, int mwss, int NB, int T2, const double2* Zf, double2* X, cudaStream_t st) {
+    const int T = mwss ? 2 * L : 2 * L - 1;
+    k_adj_trunc_phase<<<dim3(cdiv(T, 128), NB), 128, 0, st>>>(L, mwss, T2, Zf, X);
+    count_bytes(32.0 * (double)NB * T); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_adj_fold(int L, int n, int mwss, int NB, int nrmap, int ldf, const double2* X, double2* F, cudaStream_t st) {
+    k_adj_fold<<<dim3(cdiv(nrmap, 128), NB), 128, 0, st>>>(L, n, mwss, nrmap, ldf, X, F);
+    count_bytes(16.0 * (double)NB * (3.0 * nrmap)); LAUNCHED(); return cudaSuccess;
 }

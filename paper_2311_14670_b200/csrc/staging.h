@@ -25,11 +25,17 @@ cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC,
                             const double* wq, const double2* U, double2* W, cudaStream_t st);
 cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
                                   const double2* U, double2* W, cudaStream_t st);
-cudaError_t st_pole_forward(int L, int Lp, int n, int NBin, int ldin, int upole, const double* wq, const double2* U, double2* H,
+cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
                             cudaStream_t st);
 cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st);
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st);
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st);
+
+// adjoint transforms: conjugate transposes of the staging steps (Sec. 5.3)
+cudaError_t st_scale_cols(int nrows, int ncol, int ld, const double* w, double2* F, cudaStream_t st);
+cudaError_t st_adj_weight_pad(int L, int NBq, int ldq, const double2* Fq, const double* wq, int NB, int T2, double2* Z, cudaStream_t st);
+cudaError_t st_adj_trunc_phase(int L, int mwss, int NB, int T2, const double2* Zf, double2* X, cudaStream_t st);
+cudaError_t st_adj_fold(int L, int n, int mwss, int NB, int nrmap, int ldf, const double2* X, double2* F, cudaStream_t st);
 
 // MW inverse through the symmetric midpoint rings: resampling of F_m to the MW rings
 cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st);
