@@ -135,6 +135,21 @@ int        sht_plan_ntheta(const sht_plan* plan, int forward);
 sht_status s2_theta_inverse_plan(sht_plan* plan, const void* flm, void* Fm, sht_stream stream);
 sht_status s2_theta_forward_plan(sht_plan* plan, const void* Wm, void* flm, sht_stream stream);
 
+/* ---- ring shards: one transform spread over several GPUs ("distributes expensive operations evenly across
+ * available devices").  Every ring costs the same number of recursion steps, so the O(L^3) theta step is split by
+ * rings: sht_plan_set_shard(plan, rank, nranks) makes the plan serve share `rank` of `nranks` of the rings its fused kernels run
+ * on (contiguous shares differing by at most one ring; with the north-south fold a kernel ring stands for a mirror pair).  Arrays
+ * keep their full shapes:
+ *   forward : the full map in (MW / MWSS: the upsampling mixes rings, so the O(L^2 log L) staging runs in full on every rank; other
+ *             samplings read only the shard's rings) -> the PARTIAL flm of the shard's quadrature rings.  The sum over ranks is
+ *             the transform: one all-reduce (NCCL, fp64 sum) of L (2L-1) complex numbers.
+ *   inverse : the full flm in (replicated) -> a map in which only the shard's rings are filled, all others are zero.  No
+ *             collective is needed (each GPU owns its rings); the sum over ranks is the full map.
+ * (0, 1) restores the whole transform.  SO(3) plans shard the same way.  SHT_EUNSUPPORTED for batched / fp32 / INVSYM / ADJOINT plans.
+ * sht_plan_shard_range() reports the share: first kernel ring and count, for the forward or the inverse ring set. */
+sht_status sht_plan_set_shard(sht_plan* plan, int rank, int nranks);
+sht_status sht_plan_shard_range(const sht_plan* plan, int forward, int* first, int* count);
+
 /* ---- adjoints (Sec. 5.3-5.4): the conjugate transposes of the four maps above, for plans created with
  * SHT_OPT_ADJOINT (SHT_EUNSUPPORTED otherwise).  They are what a vector-Jacobian product of the (linear) transforms needs
  * (VJP = conj(adjoint(conj v)), Eq. 51 / 57).  Same layouts as the transforms; the fused recursion kernels are the existing ones.

@@ -32,6 +32,8 @@ SIGNATURES = {
     "s2_inverse_adjoint_plan": (_i, [_vp, _vp, _vp, _vp]),
     "s2_theta_forward_adjoint_plan": (_i, [_vp, _vp, _vp, _vp]),
     "s2_theta_inverse_adjoint_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "sht_plan_set_shard": (_i, [_vp, _i, _i]),
+    "sht_plan_shard_range": (_i, [_vp, _i, C.POINTER(_i), C.POINTER(_i)]),
     "sht_plan_ntheta": (_i, [_vp, _i]),
     "s2_theta_inverse_plan": (_i, [_vp, _vp, _vp, _vp]),
     "s2_theta_forward_plan": (_i, [_vp, _vp, _vp, _vp]),

@@ -128,6 +128,17 @@ class Plan:
         check(lib().s2_theta_inverse_adjoint_plan(self._h, _dev(F, torch.complex128, shape, "F"), C.c_void_p(out.data_ptr()), _stream()))
         return out
 
+    # -- ring shards (one transform over several GPUs) --
+    def set_shard(self, rank, nranks):
+        """Serve share `rank` of `nranks` of the kernel rings: forward returns a partial flm (sum over ranks = transform), inverse
+        a map with only this shard's rings filled."""
+        check(lib().sht_plan_set_shard(self._h, int(rank), int(nranks)))
+
+    def shard_range(self, forward):
+        a, n = C.c_int(), C.c_int()
+        check(lib().sht_plan_shard_range(self._h, int(forward), C.byref(a), C.byref(n)))
+        return a.value, a.value + n.value
+
     def ntheta(self, forward):
         return int(lib().sht_plan_ntheta(self._h, int(forward)))
 

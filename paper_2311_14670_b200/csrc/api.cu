@@ -102,6 +102,7 @@ struct sht_plan {
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     bool upsampled = false;    // MW / MWSS: the forward transform extends F_m to the theta circle and upsamples to the quadrature rings
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
+    int shard_rank = 0, shard_n = 1;   // ring shard (sht_plan_set_shard): this plan serves share shard_rank of shard_n of the kernel rings
     unsigned opts = 0;         // SHT_OPT_* given at creation
     // Helper plans of the adjoint entry points (SHT_OPT_ADJOINT; MW / MWSS only, where the forward quadrature does not run on the
     // rings of the map): adj_inv runs the FORWARD-type kernel on the rings of the map ((F^-1)^H, Eq. 58), adj_fwd runs the
@@ -651,6 +652,15 @@ sht_status upload_passes(sht_plan* P, cudaStream_t st) {
     return SHT_OK;
 }
 
+// contiguous, balanced share of the kernel rings of one direction (every ring costs the same number of d-steps);
+// shares differ by at most one ring: the first (nth mod n) shares get one more
+void shard_range(const sht_plan* P, bool fwd, int* lo, int* hi) {
+    const int nth = (fwd ? P->fwd : P->inv).nth, n = P->shard_n, i = P->shard_rank;
+    const int q = nth / n, r = nth % n;
+    *lo = i * q + (i < r ? i : r);
+    *hi = *lo + q + (i < r ? 1 : 0);
+}
+
 ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     const RingSet& R = fwd ? P->fwd : P->inv;
     ThetaArgs a{};
@@ -658,6 +668,7 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     a.sg = P->sgtab; a.sgstride = P->sgstride; a.mmin = P->mmin; a.ctab = P->ctab;
     a.fold0 = fwd ? P->fold0 : P->fold0i;
     a.ldout = P->F_ld; a.nfull = R.nfull;
+    shard_range(P, fwd, &a.th_lo, &a.th_hi);
     a.nsm = P->nsm; a.tile = (P->opts & SHT_OPT_TILE64) ? 64 : (P->opts & SHT_OPT_TILE128) ? 128 : 0;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
@@ -696,11 +707,11 @@ sht_status inverse_poles(sht_plan* P, const double2* coef, cudaStream_t st) {
     for (int s = 0; s < P->nslab; ++s) {
         const int n = P->slab_n[s];
         double2* Fs = P->F + P->F_slab * s;
-        if (P->inv.pole) {
+        if (P->inv.pole && P->shard_rank == P->shard_n - 1) {        // the south pole belongs to the last ring shard, the north pole to the first
             const int row = (-n) < 0 ? -n + P->NB : -n;
             CK(st_pole_inverse(L, n, 0, coef + (size_t)s * L * P->M, P->scale_inv, Fs + (size_t)row * P->F_ld + P->col0 + nreg, st));
         }
-        if (P->inv.pole_n) {
+        if (P->inv.pole_n && P->shard_rank == 0) {
             const int row = n < 0 ? n + P->NB : n;
             CK(st_pole_inverse(L, n, 1, coef + (size_t)s * L * P->M, P->scale_inv, Fs + (size_t)row * P->F_ld, st));
         }
@@ -830,17 +841,19 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         CK(launch_theta_f32(a, true, NC, st));
         return SHT_OK;
     }
+    int slo, shi;
+    shard_range(P, true, &slo, &shi);
     for (auto& ph : P->pfwd) {
         int n_slab = P->slab_n[ph.p.slab];
         if (P->fold0) {
             const int NC = ph.mode == 0 ? 2 : 1;
             CK(st_weight_split_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, ph.p.m_end, P->fwd.wq, U + U_slab * ph.p.slab,
-                                     reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * 2 * NC, st));
+                                     reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * 2 * NC, slo, shi, st));
             continue;
         }
         CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo,
                            P->fwd.wq, U + U_slab * ph.p.slab,
-                           reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), st));
+                           reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), slo, shi, st));
     }
     CS(zero_async(P->H, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
@@ -1195,6 +1208,22 @@ sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
     return SHT_OK;
 }
 
+sht_status sht_plan_set_shard(sht_plan* P, int rank, int nranks) {
+    if (!P || nranks < 1 || rank < 0 || rank >= nranks) return SHT_EINVAL;
+    if (nranks > 1 && (P->batch > 1 || P->dtype != SHT_F64 || P->invsym || (P->opts & SHT_OPT_ADJOINT))) {
+        g_err = "ring shards are built for single-map fp64 plans without SHT_OPT_INVSYM / SHT_OPT_ADJOINT";
+        return SHT_EUNSUPPORTED;
+    }
+    P->shard_rank = rank; P->shard_n = nranks;
+    return SHT_OK;
+}
+sht_status sht_plan_shard_range(const sht_plan* P, int forward, int* first, int* count) {
+    if (!P || !first || !count) return SHT_EINVAL;
+    int lo, hi;
+    shard_range(P, forward != 0, &lo, &hi);
+    *first = lo; *count = hi - lo;
+    return SHT_OK;
+}
 sht_status sht_plan_stage_bytes(const sht_plan* P, double bytes[3]) {
     if (!P || !bytes) return SHT_EINVAL;
     for (int i = 0; i < 3; ++i) bytes[i] = P->sec_bytes[i];

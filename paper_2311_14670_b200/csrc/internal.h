@@ -51,6 +51,7 @@ struct ThetaArgs {
     int npass;
     int fold0;             // n = 0, northern rings only (theta_kernels.cu FOLD): forward operand rows hold the E / O sets,
                            // the inverse keeps even-l / odd-l partial sums and writes both rings of a mirror pair
+    int th_lo, th_hi;      // ring shard (sht_plan_set_shard): only kernel rings th_lo <= th < th_hi are served by this launch
     int nsm;               // SMs of the device (tile choice)
     int tile;              // 0 = automatic, 64 / 128 = forced ring-tile size (plan option SHT_OPT_TILE64 / SHT_OPT_TILE128)
 };

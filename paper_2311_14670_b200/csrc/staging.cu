@@ -303,13 +303,13 @@ __global__ void k_rows_head(int ncol, int ldin, int ldout, const double2* __rest
 // ring pi - theta (index nth-1-th), served by the same d-value up to (-1)^{l-n} (applied at the output), for m > m_s.
 __global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold,
                                const int* __restrict__ m_lo, const double* __restrict__ wq, const double2* __restrict__ U,
-                               double2* __restrict__ W) {
+                               double2* __restrict__ W, int th_lo, int th_hi) {
     int th = blockIdx.x * blockDim.x + threadIdx.x;
     int m = m_end + blockIdx.y;
     if (th >= ntp) return;
     for (int c = 0; c < NC; ++c) {
         double2 v = {0.0, 0.0};
-        bool ok = th < nth && (m < L) && (m > -L);
+        bool ok = th < nth && (m < L) && (m > -L) && th >= th_lo && th < th_hi;
         if (fold) { if (ok) ok = c == 0 ? m >= m_lo[th] : m > m_lo[th]; }
         else {
             ok = ok && !(c == 1 && m == 0);
@@ -333,13 +333,13 @@ __global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int 
 // recursed.  W[m][ntp][2][NC]: set 0 = E = q (F_m(theta) + F_m(pi - theta)), set 1 = O = q (F_m(theta) - F_m(pi - theta)); the mirror of
 // ring th is nfull-1-th (the equator ring of HEALPix is its own mirror: E = q F_m, O = 0).  Column c = 1 is order -m with (-1)^m.
 __global__ void k_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end,
-                                     const double* __restrict__ wq, const double2* __restrict__ U, double2* __restrict__ W) {
+                                     const double* __restrict__ wq, const double2* __restrict__ U, double2* __restrict__ W, int th_lo, int th_hi) {
     int th = blockIdx.x * blockDim.x + threadIdx.x;
     int m = m_end + blockIdx.y;
     if (th >= ntp) return;
     for (int c = 0; c < NC; ++c) {
         double2 e = {0.0, 0.0}, o = {0.0, 0.0};
-        if (th < nth && !(c == 1 && m == 0) && m < L && m > -L) {
+        if (th < nth && !(c == 1 && m == 0) && m < L && m > -L && th >= th_lo && th < th_hi) {
             const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
             const double2* row = U + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
             double s = wq[th];
@@ -792,9 +792,9 @@ cudaError_t st_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2*
     count_bytes(16.0 * (double)T * ((double)T + ldout)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
-                            const double* wq, const double2* U, double2* W, cudaStream_t st) {
+                            const double* wq, const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
-    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, fold, m_lo, wq, U, W);
+    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, fold, m_lo, wq, U, W, th_lo, th_hi);
     count_bytes(32.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
@@ -837,9 +837,9 @@ cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int 
     count_bytes(8.0 * SHT_MMA_NCOL * (double)ncg * (L - m_end) * Mp + 32.0 * B * NC * (double)(L - m_end) * mlim); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
-                                  const double2* U, double2* W, cudaStream_t st) {
+                                  const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
-    k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, m_end, wq, U, W);
+    k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, m_end, wq, U, W, th_lo, th_hi);
     count_bytes(64.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,

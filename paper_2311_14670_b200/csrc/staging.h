@@ -22,9 +22,9 @@ cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStr
 cudaError_t st_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st);
 cudaError_t st_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
 cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
-                            const double* wq, const double2* U, double2* W, cudaStream_t st);
+                            const double* wq, const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st);
 cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
-                                  const double2* U, double2* W, cudaStream_t st);
+                                  const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st);
 cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
                             cudaStream_t st);
 cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st);

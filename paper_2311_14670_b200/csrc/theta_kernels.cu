@@ -66,7 +66,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;     // heavy (large-l) tiles first
     const int l0 = lt * TL, th0 = tt * NTH;
     const int an = P.n < 0 ? -P.n : P.n;
-    if (l0 + TL <= an || l0 >= A.L || th0 >= A.nth) return;
+    if (l0 + TL <= an || l0 >= A.L || th0 >= A.nth || th0 + NTH <= A.th_lo || th0 >= A.th_hi) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end;
     const int npairs = (mtop - m_end + 2) / KS;       // an odd step count ends with a dummy step m_end-1 (all-zero table row)
@@ -105,7 +105,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             const int o = at + NAUX * 32 * q;
             const int th = th0 + o % NTH;             // partial sums are stored [column][ring]
             neg[q] = NC == 2 && (o / NTH);
-            valid[q] = th < A.nth && o < NOUT;
+            valid[q] = th < A.nth && o < NOUT && th >= A.th_lo && th < A.th_hi;
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
             if (mlo[q] < m_end) mlo[q] = m_end;
             obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2;
@@ -313,7 +313,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
     const int l0 = lt * TLB, th0 = tt * NTB;
     const int an = P.n < 0 ? -P.n : P.n;
-    if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth) return;
+    if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth || th0 + NTB <= A.th_lo || th0 >= A.th_hi) return;   // (rings outside the shard inside a
+                                                                                                       //  boundary tile carry zero operands)
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end;
     const int npairs = (mtop - m_end + 2) / KS;
