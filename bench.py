@@ -248,6 +248,9 @@ def main():
     ap.add_argument("--L", type=int, default=None, help="profiling only: override the band-limit of the workload")
     ap.add_argument("--spin", type=int, default=None, help="profiling only: override the spin of the workload")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="profiling only: fp32 variant (needs --spin 0)")
+    ap.add_argument("--shard", default="none", choices=["none", "rings"],
+                    help="rings: ONE transform pair per step spread over the --gpus ranks by ring shards (strong scaling; NCCL all-reduce of "
+                         "the partial flm and of the map); default: independent problems per rank (weak scaling, no data-path collective)")
     ap.add_argument("--batch", type=int, default=1, help="profiling only: transform a batch of maps together (configs[4]: --L 2048 --spin 0 --batch 16)")
     args = ap.parse_args()
     if args.L is not None:
@@ -261,6 +264,7 @@ def main():
     import torch
     from paper_2311_14670_b200 import api, synth
     from paper_2311_14670_b200.ranks import Ranks
+    from paper_2311_14670_b200.sharded import ShardedTransform
 
     R = Ranks(backend="nccl")
     rank, local_rank, world = R.rank, R.local_rank, R.world
@@ -269,9 +273,11 @@ def main():
     sync = torch.cuda.synchronize
 
     L, spin, B = WORKLOAD["L"], WORKLOAD["spin"], args.batch
-    # weak scaling: every rank transforms its own seeded field (independent problems, no data-path collective)
+    sharded = args.shard == "rings"
+    # weak scaling (default): every rank transforms its own seeded field (independent problems, no data-path collective);
+    # --shard rings: all ranks work on the SAME field, each on its share of the rings (strong scaling)
     if B == 1:
-        flm_h = synth.random_flm(L, spin, seed=R.seed(WORKLOAD["seed"]), sigma=sigma_for(spin))
+        flm_h = synth.random_flm(L, spin, seed=WORKLOAD["seed"] if sharded else R.seed(WORKLOAD["seed"]), sigma=sigma_for(spin))
     else:
         flm_h = np.stack([synth.random_flm(L, spin, seed=4 + i + 1000 * rank, sigma=synth.SIGMA_RED) for i in range(B)])
     if args.dtype == "f32":
@@ -282,9 +288,16 @@ def main():
     back = torch.empty_like(flm)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
-    def step():
-        plan.inverse(flm, out=f)
-        plan.forward(f, out=back)
+    if sharded:
+        ST = ShardedTransform(plan, R)
+
+        def step():
+            ST.inverse(flm, out=f, gather=True)     # each rank fills its rings; the MW forward needs the assembled map
+            ST.forward(f, out=back)                 # partial flm of the rank's quadrature rings, summed over ranks
+    else:
+        def step():
+            plan.inverse(flm, out=f)
+            plan.forward(f, out=back)
 
     warm = max(args.warmup, 3)
     for _ in range(warm):
@@ -303,7 +316,9 @@ def main():
     launches = api.launch_count()
     total_ms = R.max_over_ranks(sum(a.elapsed_time(b) for a, b in ev), device=dev)
     ms_per_step = total_ms / args.steps
-    value = R.throughput(B, args.steps, total_ms)
+    value = (B * args.steps / (total_ms * 1e-3)) if sharded else R.throughput(B, args.steps, total_ms)
+    if sharded:
+        plan.set_shard(0, 1)            # the stage timings / e2e / sweep below are single-GPU measurements
     err = float((back - flm).abs().max() / flm.abs().max())
 
     # per-stage device times: a separate loop of timed transforms AFTER the K timed steps (events recorded inside the library)
@@ -376,10 +391,11 @@ def main():
             cpu = {"value": 1.0 / (t_inv + t_fwd), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                    "inverse_s": t_inv, "forward_s": t_fwd}
         out = {"metric": metric_name(L, spin), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
-               "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+               "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": args.dtype,
                "data": "synthetic",
                "config": {"workload": workload_name(L, spin, B), "l2": "flushed between timed iterations (256 MiB memset, untimed)",
-                          "parallelism": f"independent x{world}"},
+                          "parallelism": (f"ring shards x{world}: one transform pair per step, NCCL all-reduce of the map ({f.numel() * f.element_size()} B) and of the "
+                                          f"partial flm ({flm.numel() * flm.element_size()} B)" if sharded else f"independent x{world}")},
                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                "stages": stages, "roundtrip_err": err,
                "paper_context": "S2FFT on 1x A100-40GB: 240 s per MW L=8192 round trip, 430 ms at L=1024 (PAPER.md:737-740, Table 3; other hardware)"}

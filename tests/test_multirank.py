@@ -52,8 +52,60 @@ def _worker(rank, world, port, q):
     R.sum_over_ranks(buf)                       # disjoint rows: the sum assembles the map
     out["map"] = torch.view_as_complex(buf).numpy()
     out["range"] = (a, b)
+    # (4) the code path of `bench.py --gpus N --shard rings`: sharded.ShardedTransform over this process group, with a CPU stand-in
+    # for the ring-sharded plan (the oracle restricted to the rank's rings; the library's share rule is ranks.split_range)
+    from paper_2311_14670_b200.sharded import ShardedTransform
+    ST = ShardedTransform(OraclePlan(oracle, L, spin), R)
+    cc = torch.from_numpy(c)
+    f_full = ST.inverse(cc, gather=True)
+    out["sharded_map"] = f_full.numpy().copy()
+    out["sharded_back"] = ST.forward(f_full).numpy().copy()
     R.finish()
     q.put(out)
+
+
+class OraclePlan:
+    """CPU stand-in for a ring-sharded api.Plan (MW): serves the ranks.split_range share of the rings with the oracle.  inverse:
+    the rank's rings of the map, zeros elsewhere; forward: Eq. 30 restricted to the rank's share of the 2L quadrature rings."""
+
+    def __init__(self, oracle, L, spin):
+        self.o, self.L, self.spin, self.rank, self.n = oracle, L, spin, 0, 1
+
+    def set_shard(self, rank, n):
+        self.rank, self.n = rank, n
+
+    def inverse(self, flm, out=None):
+        from paper_2311_14670_b200.ranks import split_range
+        L = self.L
+        a, b = split_range(L, self.n, self.rank)
+        f = torch.zeros((L, 2 * L - 1), dtype=torch.complex128)
+        rows = self.o.s2_inverse_rings(L, self.spin, self.o.MW, flm.numpy(), np.arange(a, b))
+        for i, r in enumerate(range(a, b)):
+            f[r] = torch.from_numpy(rows[i])
+        return f
+
+    def forward(self, f, out=None):
+        from paper_2311_14670_b200.ranks import split_range
+        o, L, s = self.o, self.L, self.spin
+        ms = np.arange(-(L - 1), L)
+        # full staging on every rank (ring DFT, extension, upsampling to the oracle's 2L quadrature rings), theta step on the share
+        U = np.zeros((2 * L - 1, 2 * L), complex)
+        Fm = np.fft.fft(f.numpy(), axis=1)
+        T, sg = 2 * L - 1, (-1.0) ** (ms + s)
+        t = np.arange(T)
+        u = np.arange(2 * L)
+        for i, m in enumerate(ms):
+            col = Fm[:, m % T]
+            ext = np.concatenate([col, sg[i] * col[L - 2::-1]])
+            mp = np.arange(-(L - 1), L)
+            Fmm = (ext[None, :] * np.exp(-1j * np.pi * mp[:, None] * (2 * t[None, :] + 1) / T)).sum(1) / T
+            U[i] = (Fmm[None, :] * np.exp(1j * np.pi * mp[None, :] * (2 * u[:, None] + 1) / (4 * L - 1))).sum(1)
+        tab = o.ring_table(o.MW_QUAD, L)
+        W = U * np.asarray(tab["weight"], float)[None, :]
+        a, b = split_range(2 * L, self.n, self.rank)
+        W[:, :a] = 0
+        W[:, b:] = 0
+        return torch.from_numpy(np.ascontiguousarray(o.s2_theta_forward_columns(L, s, o.MW_QUAD, W, ms).T))
 
 
 @pytest.mark.timeout(300)
@@ -83,6 +135,11 @@ def test_two_ranks_gloo():
     full = oracle.s2_inverse(12, 1, oracle.MW, synth.random_flm(12, 1, seed=3))
     for d in res:
         assert np.abs(d["map"] - full).max() <= 1e-14 * np.abs(full).max()
+    # the sharded transform pair (bench.py --shard rings): assembled map and summed partial flm on EVERY rank
+    c = synth.random_flm(12, 1, seed=3)
+    for d in res:
+        assert np.abs(d["sharded_map"] - full).max() <= 1e-14 * np.abs(full).max()
+        assert np.abs(d["sharded_back"] - c).max() <= 1e-13 * np.abs(c).max()          # sampling theorem: the round trip is exact
 
 
 def test_split_range_is_a_balanced_partition():
