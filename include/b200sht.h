@@ -122,6 +122,9 @@ sht_status sht_plan_destroy(sht_plan* plan);
  */
 sht_status s2_forward_plan(sht_plan* plan, const void* f, void* flm, sht_stream stream);
 sht_status s2_inverse_plan(sht_plan* plan, const void* flm, void* f, sht_stream stream);
+/* HEALPix forward transform with `niter` refinement iterations (HEALPix has no sampling theorem, "iterations are
+ * usually performed"): flm_0 = F f, flm_{k+1} = flm_k + F (f - F^-1 flm_k).  niter = 0 is s2_forward_plan.  HEALPix plans only. */
+sht_status s2_forward_iter_plan(sht_plan* plan, const void* f, void* flm, int niter, sht_stream stream);
 sht_status so3_forward_plan(sht_plan* plan, const void* f, void* flmn, sht_stream stream);
 sht_status so3_inverse_plan(sht_plan* plan, const void* flmn, void* f, sht_stream stream);
 

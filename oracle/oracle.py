@@ -180,6 +180,16 @@ def s2_forward(L, spin, sampling, f, nside=0, direct=False):
     return flm
 
 
+def s2_forward_iter(L, spin, sampling, f, niter, nside=0):
+    """Forward transform with `niter` refinement iterations ("iterations are usually performed" on HEALPix; reading
+    R24 of DESIGN.md): flm_0 = F f;  flm_{k+1} = flm_k + F (f - F^-1 flm_k).  A composition of the oracle's own F and F^-1."""
+    f = _c128(f, map_shape(sampling, L, nside))
+    flm = s2_forward(L, spin, sampling, f, nside)
+    for _ in range(int(niter)):
+        flm = flm + s2_forward(L, spin, sampling, f - s2_inverse(L, spin, sampling, flm, nside), nside)
+    return flm
+
+
 def s2_inverse_rings(L, spin, sampling, flm, rings, nside=0):
     """Samples of the selected rings only (list of 1-D complex arrays, one per ring)."""
     flm = _c128(flm, (L, 2 * L - 1))

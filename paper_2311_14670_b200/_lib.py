@@ -26,6 +26,7 @@ SIGNATURES = {
     "sht_plan_destroy": (_i, [_vp]),
     "s2_forward_plan": (_i, [_vp, _vp, _vp, _vp]),
     "s2_inverse_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "s2_forward_iter_plan": (_i, [_vp, _vp, _vp, _i, _vp]),
     "so3_forward_plan": (_i, [_vp, _vp, _vp, _vp]),
     "so3_inverse_plan": (_i, [_vp, _vp, _vp, _vp]),
     "s2_forward_adjoint_plan": (_i, [_vp, _vp, _vp, _vp]),

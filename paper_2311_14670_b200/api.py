@@ -94,6 +94,13 @@ class Plan:
         check(fn(self._h, _dev(f, self.map_dtype, self.map_shape, "f"), _dev(out, self.coef_dtype, self.coef_shape, "flm"), _stream()))
         return out
 
+    def forward_iter(self, f, niter, out=None):
+        """HEALPix forward with `niter` refinement iterations: flm <- flm + F (f - F^-1 flm)."""
+        out = torch.empty(self.coef_shape, dtype=self.coef_dtype, device=self.device) if out is None else out
+        check(lib().s2_forward_iter_plan(self._h, _dev(f, self.map_dtype, self.map_shape, "f"),
+                                         _dev(out, self.coef_dtype, self.coef_shape, "flm"), int(niter), _stream()))
+        return out
+
     def inverse(self, flm, out=None):
         out = torch.empty(self.map_shape, dtype=self.map_dtype, device=self.device) if out is None else out
         fn = lib().s2_inverse_plan if self.N is None else lib().so3_inverse_plan

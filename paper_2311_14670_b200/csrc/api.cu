@@ -110,6 +110,7 @@ struct sht_plan {
     sht_plan *adj_inv = nullptr, *adj_fwd = nullptr;
     bool helper = false;
     int only_dir = 0;          // helper plans: 1 = inverse-type kernel only, 2 = forward-type kernel only
+    double *it_map = nullptr, *it_coef = nullptr;   // HEALPix iterative refinement: residual map / coefficient update scratch
     double* wq_map = nullptr;  // [F_ld] quadrature weight of every ring of the map (direct-quadrature samplings; adjoints)
     double* wq_quad = nullptr; // [4L] MW / MWSS: weight of every one of the 2L quadrature rings (not folded; adjoints)
     int device = 0, nsm = 0;   // device the plan was created on and its SM count (tile choice)
@@ -378,6 +379,8 @@ void layout(sht_plan* P, char* base) {
             P->Fa = B.take<double2>(P->Fa_slab * P->nslab);
             if (P->upsampled) P->X = B.take<double2>(P->X_slab * P->nslab);
         } else {
+            P->it_map = B.take<double>(P->map_elems * (P->reality ? 1 : 2));
+            P->it_coef = B.take<double>(2 * (size_t)L * P->M);
             P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
             P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
             P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
@@ -1333,6 +1336,25 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     for (int b = 0; b < P->batch; ++b)
         CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + ncoef * b, st));
     stage(P, CAT_STAGE, st);
+    return SHT_OK;
+}
+
+// HEALPix forward transform with iterative refinement (the scheme has no sampling theorem, "iterations are usually
+// performed"): flm_0 = F f;  flm_{k+1} = flm_k + F (f - F^-1 flm_k) -- Jacobi iterations on the residual map, every F / F^-1 the fused
+// transforms above (reading R24 of DESIGN.md).  niter = 0 is s2_forward_plan.
+sht_status s2_forward_iter_plan(sht_plan* P, const void* f, void* flm, int niter, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0 || niter < 0) return SHT_EINVAL;
+    if (P->sampling != SHT_HEALPIX) { g_err = "iterative refinement is a HEALPix feature: the other samplings are exact"; return SHT_EUNSUPPORTED; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nm = P->map_elems * (P->reality ? 1 : 2), nc = 2 * (size_t)P->L * P->M;
+    CS(s2_forward_plan(P, f, flm, stream));
+    for (int it = 0; it < niter; ++it) {
+        CS(s2_inverse_plan(P, flm, P->it_map, stream));
+        CK(st_vec_sub(nm, (const double*)f, P->it_map, P->it_map, st));
+        CS(s2_forward_plan(P, P->it_map, P->it_coef, stream));
+        CK(st_vec_add(nc, P->it_coef, (double*)flm, st));
+    }
     return SHT_OK;
 }
 

@@ -463,6 +463,16 @@ __global__ void k_adj_fold(int L, int n, int mwss, int nrmap, int ldf, const dou
     F[(size_t)b * ldf + t] = v;
 }
 
+// ---- HEALPix iterative refinement: residual and update, plain vector kernels
+__global__ void k_vec_sub(size_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ out) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = a[i] - b[i];
+}
+__global__ void k_vec_add(size_t n, const double* __restrict__ x, double* __restrict__ y) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) y[i] += x[i];
+}
+
 // ---- batched path (theta_mma.cu; operand layouts in internal.h) ----------------------------------------------------
 // Complex column j = cg*16 + jc of a pass belongs to map b = j / NC and, with NC = 2 (spin 0 complex), to order +m
 // (c = 0) or -m (c = 1); columns j >= B*NC are zero padding.
@@ -908,4 +918,12 @@ cudaError_t st_adj_trunc_phase(int L, int mwss, int NB, int T2, const double2* Z
 cudaError_t st_adj_fold(int L, int n, int mwss, int NB, int nrmap, int ldf, const double2* X, double2* F, cudaStream_t st) {
     k_adj_fold<<<dim3(cdiv(nrmap, 128), NB), 128, 0, st>>>(L, n, mwss, nrmap, ldf, X, F);
     count_bytes(16.0 * (double)NB * (3.0 * nrmap)); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_vec_sub(size_t n, const double* a, const double* b, double* out, cudaStream_t st) {
+    k_vec_sub<<<cdiv(n, 256), 256, 0, st>>>(n, a, b, out);
+    count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_vec_add(size_t n, const double* x, double* y, cudaStream_t st) {
+    k_vec_add<<<cdiv(n, 256), 256, 0, st>>>(n, x, y);
+    count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }

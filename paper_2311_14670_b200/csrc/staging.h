@@ -37,6 +37,10 @@ cudaError_t st_adj_weight_pad(int L, int NBq, int ldq, const double2* Fq, const 
 cudaError_t st_adj_trunc_phase(int L, int mwss, int NB, int T2, const double2* Zf, double2* X, cudaStream_t st);
 cudaError_t st_adj_fold(int L, int n, int mwss, int NB, int nrmap, int ldf, const double2* X, double2* F, cudaStream_t st);
 
+// HEALPix iterative refinement: out = a - b; y += x (arrays of doubles)
+cudaError_t st_vec_sub(size_t n, const double* a, const double* b, double* out, cudaStream_t st);
+cudaError_t st_vec_add(size_t n, const double* x, double* y, cudaStream_t st);
+
 // MW inverse through the symmetric midpoint rings: resampling of F_m to the MW rings
 cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st);
 cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st);

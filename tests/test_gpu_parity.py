@@ -250,3 +250,32 @@ def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, sym, L, rea
     assert rel(got, ref.real if real else ref) < TOL
     F = P.theta_inverse(dev(flm)).cpu().numpy()
     assert rel(F, orc.s2_theta_inverse_columns(L, 0, orc.MW, flm, np.arange(-(L - 1), L))) < TOL
+
+
+@pytest.mark.parametrize("nside,L,spin,real", [(4, 8, 0, True), (8, 16, 0, True), (8, 20, 2, False), (16, 32, 0, False)])
+def test_healpix_iterative_refinement_vs_oracle(api, orc, nside, L, spin, real):
+    """PAPER.md:172 "iterations are usually performed": flm <- flm + F (f - F^-1 flm), against the oracle's composition of its own
+    F and F^-1, element by element; plus, at a larger size, the property that the map residual shrinks with every iteration."""
+    flm = synth.random_flm(L, spin, seed=nside + L, sigma=synth.SIGMA_RED, real=real)
+    f_ref = orc.s2_inverse(L, spin, orc.HEALPIX, flm, nside=nside)
+    f_in = f_ref.real.copy() if real else f_ref
+    P = api.Plan(L, spin, sampling=api.HEALPIX, nside=nside, reality=real)
+    for niter in (0, 1, 3):
+        got = P.forward_iter(dev(f_in), niter).cpu().numpy()
+        want = orc.s2_forward_iter(L, spin, orc.HEALPIX, f_ref, niter, nside=nside)
+        assert rel(got, want) < TOL, niter
+    with pytest.raises(Exception):
+        api.Plan(L, spin).forward_iter(dev(synth.random_map((L, 2 * L - 1), seed=1)), 1)
+
+
+def test_healpix_iterative_refinement_residual_shrinks_at_size(api):
+    nside, L = 128, 256
+    flm = dev(synth.random_flm(L, 0, seed=3, sigma=synth.SIGMA_RED, real=True))
+    P = api.Plan(L, 0, sampling=api.HEALPIX, nside=nside, reality=True)
+    f = P.inverse(flm)
+    res, err = [], []
+    for niter in range(4):
+        c = P.forward_iter(f, niter)
+        res.append(float((f - P.inverse(c)).abs().max()))
+        err.append(float((c - flm).abs().max() / flm.abs().max()))
+    assert all(b < a for a, b in zip(res, res[1:])) and err[3] < err[0] / 10, (res, err)

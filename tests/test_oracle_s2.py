@@ -217,3 +217,24 @@ def test_round_trip_error_is_below_paper_table1(orc):
             errs.append(np.abs(back - flm)[sup].mean())
         e = float(np.mean(errs))
         assert e < tab[L] / 3, (L, e, tab[L])
+
+
+def test_healpix_iterative_refinement(orc):
+    """HEALPix transforms are approximate and "iterations are usually performed".  The iteration
+    flm <- flm + F (f - F^-1 flm) (reading R24) must (a) reduce to the plain forward at niter = 0, (b) shrink the map residual
+    |f - F^-1 flm| at every step, and (c) move the coefficients of a band-limited map toward the generating ones."""
+    nside, L = 8, 16
+    flm = synth.random_flm(L, 0, seed=6, sigma=synth.SIGMA_RED, real=True)
+    f = orc.s2_inverse(L, 0, 1, flm, nside=nside)
+    assert np.array_equal(orc.s2_forward_iter(L, 0, 1, f, 0, nside=nside), orc.s2_forward(L, 0, 1, f, nside=nside))
+    errs, res = [], []
+    for it in range(4):
+        c = orc.s2_forward_iter(L, 0, 1, f, it, nside=nside)
+        errs.append(np.abs(c - flm).max() / np.abs(flm).max())
+        res.append(np.abs(f - orc.s2_inverse(L, 0, 1, c, nside=nside)).max())
+    assert all(b < a for a, b in zip(res, res[1:])) and all(b < a for a, b in zip(errs, errs[1:]))
+    assert errs[3] < errs[0] / 20
+    # one step written out by hand from the pinned F and F^-1
+    c0 = orc.s2_forward(L, 0, 1, f, nside=nside)
+    c1 = c0 + orc.s2_forward(L, 0, 1, f - orc.s2_inverse(L, 0, 1, c0, nside=nside), nside=nside)
+    assert np.abs(orc.s2_forward_iter(L, 0, 1, f, 1, nside=nside) - c1).max() < 1e-16
