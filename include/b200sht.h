@@ -63,6 +63,11 @@ enum {
                                      resampling of F_m to the MW rings (off by default: measured not faster) */
     SHT_OPT_TILE64   = 1u << 3,   /* force 64-ring block tiles in the fused kernels ...                                          */
     SHT_OPT_TILE128  = 1u << 4,   /* ... or 128-ring tiles.  Default: 64 when 128-ring tiles give fewer blocks than the device has SMs */
+    SHT_OPT_PRECOMPUTE = 1u << 6, /* the paper's full-precomputation mode (Sec. 4.3): the Wigner d-functions of every
+                                     (l, m, ring) are computed once at sht_plan_set_workspace and stored -- O(L^3) workspace (16 L^3 to
+                                     24 L^3 bytes on MW) -- and the theta steps become plain weighted sums over the stored table
+                                     (HBM-bound).  Pays at L <= 512, where the on-the-fly kernels are bound by the latency of their L
+                                     sequential recursion steps.  Single-map fp64 S^2 plans; the folds are off. */
     SHT_OPT_ADJOINT  = 1u << 5    /* also build what the adjoint entry points need (complex fp64 single-map plans; MW / MWSS plans then
                                      carry the tables of two more ring sets: about twice the workspace) */
 };

@@ -102,6 +102,7 @@ struct sht_plan {
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     bool upsampled = false;    // MW / MWSS: the forward transform extends F_m to the theta circle and upsamples to the quadrature rings
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
+    bool precomp = false;      // SHT_OPT_PRECOMPUTE: stored d-function tables (precompute.cu, Sec. 4.3)
     int shard_rank = 0, shard_n = 1;   // ring shard (sht_plan_set_shard): this plan serves share shard_rank of shard_n of the kernel rings
     unsigned opts = 0;         // SHT_OPT_* given at creation
     // Helper plans of the adjoint entry points (SHT_OPT_ADJOINT; MW / MWSS only, where the forward quadrature does not run on the
@@ -359,6 +360,10 @@ void layout(sht_plan* P, char* base) {
     for (auto& ph : P->pfwd) {
         ph.p.in = B.take<double>(pass_in_doubles(P, ph, true));
         ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->fwd.ntp);
+    }
+    if (P->precomp) {        // E[m - m_end][ntp][Lp] per pass: the O(L^3) memory of Sec. 4.3
+        for (auto& ph : P->pinv) ph.p.pre = B.take<double>((size_t)(L - ph.p.m_end) * P->inv.ntp * Lp);
+        for (auto& ph : P->pfwd) ph.p.pre = B.take<double>((size_t)(L - ph.p.m_end) * P->fwd.ntp * Lp);
     }
     if (P->batch > 1) {
         size_t oi = 0, of = 0;
@@ -783,8 +788,13 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
                            const_cast<double*>(ph.p.in) + (size_t)P->Lp * theta_inverse_rowd(ph.mode), st));
     CS(zero_async(P->F, sizeof(double2) * P->F_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
-    CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
-    CK(launch_theta_inverse(theta_args(P, false, false), 1, st));
+    if (P->precomp) {
+        CK(launch_pre_inverse(theta_args(P, false, true), 0, L - P->mmin - 1, st));
+        CK(launch_pre_inverse(theta_args(P, false, false), 1, L - P->mmin - 1, st));
+    } else {
+        CK(launch_theta_inverse(theta_args(P, false, true), 0, st));
+        CK(launch_theta_inverse(theta_args(P, false, false), 1, st));
+    }
     CS(inverse_poles(P, coef, st));
     stage(P, CAT_STAGE, st);
     if (P->reality)
@@ -860,8 +870,13 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     }
     CS(zero_async(P->H, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
-    CK(launch_theta_forward(theta_args(P, true, true), 0, st));
-    CK(launch_theta_forward(theta_args(P, true, false), 1, st));
+    if (P->precomp) {
+        CK(launch_pre_forward(theta_args(P, true, true), 0, L - P->mmin - 1, st));
+        CK(launch_pre_forward(theta_args(P, true, false), 1, L - P->mmin - 1, st));
+    } else {
+        CK(launch_theta_forward(theta_args(P, true, true), 0, st));
+        CK(launch_theta_forward(theta_args(P, true, false), 1, st));
+    }
     // pole rings of the ring set (only the adjoint helpers on the rings of an MW / MWSS map have any; unit weight): U points at
     // the first regular ring, the south pole follows the regular rings, the north pole precedes them
     const int nreg = P->fwd.nfull ? P->fwd.nfull : P->fwd.nth;
@@ -991,6 +1006,11 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if (batch > 1 && sampling != SHT_MW) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
+    if (opts & SHT_OPT_PRECOMPUTE) {
+        // stored d-functions (Sec. 4.3): single-map fp64 plans; the tables hold every ring, so the folds are off
+        if (batch != 1 || dtype != SHT_F64 || (opts & (SHT_OPT_FOLD_ON | SHT_OPT_INVSYM | SHT_OPT_ADJOINT))) return SHT_EUNSUPPORTED;
+        opts |= SHT_OPT_FOLD_OFF;
+    }
     if ((opts & SHT_OPT_FOLD_ON) && (opts & SHT_OPT_FOLD_OFF)) return SHT_EINVAL;
     if ((opts & SHT_OPT_TILE64) && (opts & SHT_OPT_TILE128)) return SHT_EINVAL;
     // fp32 variant (BASELINE config 5): spin 0, MW sampling, one map
@@ -998,6 +1018,7 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
     P->dtype = dtype; P->opts = opts; P->helper = helper; P->only_dir = only_dir;
+    P->precomp = (opts & SHT_OPT_PRECOMPUTE) != 0;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     query_device(P);
@@ -1144,6 +1165,17 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         CS(up(w, P->fwd.wq, st));
     }
     CS(upload_passes(P, st));
+    if (P->precomp) {
+        for (int dir = 0; dir < 2; ++dir) {
+            for (auto& ph : (dir ? P->pfwd : P->pinv))
+                CK(cudaMemsetAsync(const_cast<double*>(ph.p.pre), 0, sizeof(double) * (size_t)(L - ph.p.m_end) * (dir ? P->fwd.ntp : P->inv.ntp) * Lp, st));
+            for (int pm = 0; pm < 2; ++pm) {
+                ThetaArgs a = theta_args(P, dir != 0, pm != 0);
+                a.th_lo = 0; a.th_hi = a.nth;
+                CK(launch_pre_fill(a, st));
+            }
+        }
+    }
     for (sht_plan* Q : {P->adj_inv, P->adj_fwd})
         if (Q) CS(sht_plan_set_workspace(Q, Q->work, Q->need_bytes, stream));
     if (P->dtype == SHT_F32) {
@@ -1213,7 +1245,7 @@ sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
 
 sht_status sht_plan_set_shard(sht_plan* P, int rank, int nranks) {
     if (!P || nranks < 1 || rank < 0 || rank >= nranks) return SHT_EINVAL;
-    if (nranks > 1 && (P->batch > 1 || P->dtype != SHT_F64 || P->invsym || (P->opts & SHT_OPT_ADJOINT))) {
+    if (nranks > 1 && (P->batch > 1 || P->dtype != SHT_F64 || P->invsym || (P->opts & SHT_OPT_ADJOINT))) {   // (precompute plans shard too)
         g_err = "ring shards are built for single-map fp64 plans without SHT_OPT_INVSYM / SHT_OPT_ADJOINT";
         return SHT_EUNSUPPORTED;
     }

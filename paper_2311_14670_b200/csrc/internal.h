@@ -36,6 +36,7 @@ struct ThetaPass {
     const double* in;      // inverse: G[m-m_end][Lp][ROWD] rows {c*Re, c*Im (x NC), g'_m(l), s_m}
                            // forward: W[m-m_end][ntp][NC] weighted F_m samples (complex)
     double2* out;          // inverse: F[row][ntp] (row = m_out mod NB)   forward: H[m_out+L-1][Lp]
+    const double* pre;     // precompute mode (precompute.cu): E[m-m_end][ntp][Lp] stored e-form d-functions of this pass, else nullptr
 };
 
 struct ThetaArgs {
@@ -92,6 +93,10 @@ cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st);
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st);
+// precompute.cu (Sec. 4.3): fill the stored d-function tables of the passes, and the theta steps that read them
+cudaError_t launch_pre_fill(const ThetaArgs& a, cudaStream_t st);
+cudaError_t launch_pre_inverse(const ThetaArgs& a, int mode, int nrows, cudaStream_t st);
+cudaError_t launch_pre_forward(const ThetaArgs& a, int mode, int nrows, cudaStream_t st);
 // peaks.cu: register-only instruction chains; kind 0 = DFMA, 1 = DMMA (mma.sync m8n8k4 f64), 2 = FFMA.  Returns flop per launch.
 cudaError_t launch_peak(int kind, int iters, int nsm, double* sink, cudaStream_t st, double* flop);
 int theta_inverse_rowd(int mode);   // doubles per (m, l) entry of the inverse operand table

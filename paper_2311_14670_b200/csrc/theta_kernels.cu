@@ -284,8 +284,10 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 // =============================================================================================================
 // FOLD (n = 0 on a ring set symmetric about the equator): only the northern rings are recursed; d^l_{m,0}(pi - theta) =
 // (-1)^{l+m} d^l_{m,0}(theta), so a degree with l+m even contracts with E = W(theta) + W(pi-theta) and one with
-// l+m odd with O = W(theta) - W(pi-theta).  Operand rows then hold both sets: [ring][E, O][NC]; a thread's two degrees
-// l0 + 2 lane + {0, 1} have opposite, warp-uniform parities.
+// l+m odd with O = W(theta) - W(pi-theta).  Operand rows then hold both sets: [ring][E, O][NC].  A thread's two degrees
+// l0 + lane + {0, 32} have the SAME parity, which alternates with the lane: one shared-memory load with two distinct addresses
+// (even lanes one set, odd lanes the other) serves both degrees of every lane in a single wavefront -- half the operand
+// wavefronts of a mapping whose two degrees differ in parity (the r1 kernel was bound by the shared-memory pipe at 86 %).
 template <int RL, int RT, int NW, int NC, bool FOLD>
 struct FwdSmem {
     static constexpr int TLB = 32 * RL, NTB = NW * RT, NCW = FOLD ? 2 * NC : NC;
@@ -432,7 +434,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     int lr[RL];
 #pragma unroll
     for (int r = 0; r < RL; ++r) {
-        lr[r] = l0 + RL * lane + r;                    // the thread's degrees are neighbours: opposite parities
+        lr[r] = l0 + lane + 32 * r;                    // the thread's degrees share their parity (FOLD: one operand set for both)
         const bool ok = lr[r] >= an && lr[r] < A.L;
         x[r] = (double)(lr[r] - mtop) * (double)(lr[r] + mtop + 1);
 #pragma unroll
@@ -449,12 +451,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
     auto step = [&](const int m, const int slot, const int rs, const int h, double (&ca)[NI],
                     double (&cb)[NI]) -> bool {
-        // operand set of degree r: FOLD picks E (l+m even) or O (l+m odd); the parity is warp-uniform
-        const double2* T = &sm.wt[slot][h][w * RT * NCW];
-        const int par = FOLD ? ((l0 + m) & 1) : 0;
-        const double2* Tr[RL];
-#pragma unroll
-        for (int r = 0; r < RL; ++r) Tr[r] = T + (FOLD ? ((par ^ r) & 1) * NC : 0);
+        // operand set of the thread's degrees: FOLD picks E (l+m even) or O (l+m odd) by address, per lane parity
+        const double2* Tq = &sm.wt[slot][h][w * RT * NCW] + (FOLD ? ((l0 + m + lane) & 1) * NC : 0);
         const double* LM = &sm.hdr[w][h][0];
         const double G = sm.sg[slot][KS - 1 - h].y;
         bool wrote = false;
@@ -471,11 +469,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
 #pragma unroll
             for (int i = 0; i < RT; ++i) {
                 const double lm = LM[i];
+                const double2 w0 = Tq[i * NCW];
+                double2 w1 = make_double2(0.0, 0.0);
+                if (NC == 2) w1 = Tq[i * NCW + 1];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
-                    const double2 w0 = Tr[r][i * NCW];
-                    double2 w1 = make_double2(0.0, 0.0);
-                    if (NC == 2) w1 = Tr[r][i * NCW + 1];
                     const double e = ca[r * RT + i];
                     acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
                     if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
@@ -494,11 +492,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
 #pragma unroll
                 for (int ii = 0; ii < 2; ++ii) {
                     const double lm = ii ? lm2.y : lm2.x;
+                    const double2 w0 = Tq[(i + ii) * NCW];
+                    double2 w1 = make_double2(0.0, 0.0);
+                    if (NC == 2) w1 = Tq[(i + ii) * NCW + 1];
 #pragma unroll
                     for (int r = 0; r < RL; ++r) {
-                        const double2 w0 = Tr[r][(i + ii) * NCW];
-                        double2 w1 = make_double2(0.0, 0.0);
-                        if (NC == 2) w1 = Tr[r][(i + ii) * NCW + 1];
                         const double e = ca[r * RT + i + ii];
                         acc[r][0] = fma(e, w0.x, acc[r][0]); acc[r][1] = fma(e, w0.y, acc[r][1]);
                         if (NC == 2) { acc[r][2] = fma(e, w1.x, acc[r][2]); acc[r][3] = fma(e, w1.y, acc[r][3]); }
@@ -532,7 +530,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             for (int r = 0; r < RL; ++r)
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
-                    rd[c * TLB + RL * lane + r] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);
+                    rd[c * TLB + lane + 32 * r] = make_double2(acc[r][2 * c], acc[r][2 * c + 1]);      // slot = degree - l0; conflict-free
                 }
         }
         return wrote;
