@@ -90,6 +90,7 @@ __global__ void __launch_bounds__(PI_WARPS * 32) pre_inverse_kernel(const ThetaA
 
 // ---- forward, Eq. 30 with stored d-functions ----------------------------------------------------------------------------------
 constexpr int PF_T = 128;                              // degrees per block = rings per shared-memory chunk
+constexpr int PF_SPLIT = 4;                            // blocks sharing the rings of one (degree tile, m): more parallelism at moderate L
 template <int NC>
 __global__ void __launch_bounds__(PF_T) pre_forward_kernel(const ThetaArgs A) {
     __shared__ double2 sw[PF_T][NC];
@@ -97,14 +98,19 @@ __global__ void __launch_bounds__(PF_T) pre_forward_kernel(const ThetaArgs A) {
     const int m = A.L - 1 - (int)blockIdx.y, m_end = P.m_end;
     if (m < m_end) return;
     const int an = P.n < 0 ? -P.n : P.n, am = m < 0 ? -m : m, l_lo = am > an ? am : an;
-    const int l0 = blockIdx.x * PF_T, l = l0 + threadIdx.x;
+    const int l0 = (blockIdx.x / PF_SPLIT) * PF_T, l = l0 + threadIdx.x, part = blockIdx.x % PF_SPLIT;
     if (l0 + PF_T <= l_lo || l0 >= A.L) return;
     const double* E = P.pre + (size_t)(m - m_end) * A.ntp * A.Lp;
     const double2* W = reinterpret_cast<const double2*>(P.in) + (size_t)(m - m_end + 1) * A.ntp * NC;
-    double acc[2 * NC];
+    double acc[4][2 * NC];
 #pragma unroll
-    for (int c = 0; c < 2 * NC; ++c) acc[c] = 0.0;
-    const int t_lo = A.th_lo, t_hi = min(A.th_hi, A.nth);
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int c = 0; c < 2 * NC; ++c) acc[u][c] = 0.0;
+    // this block's share of the (shard's) rings, in chunks of PF_T
+    const int r_lo = A.th_lo, r_hi = min(A.th_hi, A.nth);
+    const int per = ((r_hi - r_lo + PF_SPLIT - 1) / PF_SPLIT + 3) & ~3;
+    const int t_lo = r_lo + part * per, t_hi = min(r_hi, t_lo + per);
     for (int t0 = t_lo; t0 < t_hi; t0 += PF_T) {
         __syncthreads();
         const int tt = t0 + threadIdx.x;
@@ -113,12 +119,16 @@ __global__ void __launch_bounds__(PF_T) pre_forward_kernel(const ThetaArgs A) {
         __syncthreads();
         const int nt = min(PF_T, t_hi - t0);
         const double* e = E + (size_t)t0 * A.Lp + l;
-        for (int t = 0; t < nt; ++t) {
-            const double ev = e[(size_t)t * A.Lp];
+        for (int t = 0; t < nt; t += 4) {              // (rows beyond nt inside the chunk carry zero weights; E is allocated to ntp rows)
+            double ev[4];
 #pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                acc[2 * c] = fma(ev, sw[t][c].x, acc[2 * c]); acc[2 * c + 1] = fma(ev, sw[t][c].y, acc[2 * c + 1]);
-            }
+            for (int u = 0; u < 4; ++u) ev[u] = t0 + t + u < A.ntp ? e[(size_t)(t + u) * A.Lp] : 0.0;
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    acc[u][2 * c] = fma(ev[u], sw[t + u][c].x, acc[u][2 * c]); acc[u][2 * c + 1] = fma(ev[u], sw[t + u][c].y, acc[u][2 * c + 1]);
+                }
         }
     }
     if (l < an || l >= A.L || l < m || l < -m) return;
@@ -129,21 +139,22 @@ __global__ void __launch_bounds__(PF_T) pre_forward_kernel(const ThetaArgs A) {
         const int m_out = (NC == 2) ? (neg ? -m : m) : P.sgn_out * m;
         const double f = (P.fold && neg && ((l - P.n) & 1)) ? -cm : cm;          // (-1)^{l-n} on the mirrored-ring column of a fold pass
         double* o = reinterpret_cast<double*>(P.out) + ((size_t)(m_out + A.L - 1) * A.Lp + l) * 2;
-        red_add_f64(o, acc[2 * c] * f); red_add_f64(o + 1, acc[2 * c + 1] * f);
+        red_add_f64(o, ((acc[0][2 * c] + acc[1][2 * c]) + (acc[2][2 * c] + acc[3][2 * c])) * f);
+        red_add_f64(o + 1, ((acc[0][2 * c + 1] + acc[1][2 * c + 1]) + (acc[2][2 * c + 1] + acc[3][2 * c + 1])) * f);
     }
 }
 
 }  // namespace
 
 cudaError_t launch_pre_fill(const ThetaArgs& a, cudaStream_t st) {
-    if (a.npass == 0) return cudaSuccess;
+    if (a.npass == 0 || a.nth == 0) return cudaSuccess;
     dim3 grid((a.L + 31) / 32, (a.nth + 7) / 8, a.npass), block(32, 8);
     pre_fill_kernel<<<grid, block, 0, st>>>(a);
     count_launch();
     return cudaGetLastError();
 }
 cudaError_t launch_pre_inverse(const ThetaArgs& a, int mode, int nrows, cudaStream_t st) {
-    if (a.npass == 0) return cudaSuccess;
+    if (a.npass == 0 || a.nth == 0) return cudaSuccess;
     dim3 grid((a.nth + PI_WARPS - 1) / PI_WARPS, nrows, a.npass);
     if (mode == 0) pre_inverse_kernel<2><<<grid, PI_WARPS * 32, 0, st>>>(a);
     else pre_inverse_kernel<1><<<grid, PI_WARPS * 32, 0, st>>>(a);
@@ -151,8 +162,8 @@ cudaError_t launch_pre_inverse(const ThetaArgs& a, int mode, int nrows, cudaStre
     return cudaGetLastError();
 }
 cudaError_t launch_pre_forward(const ThetaArgs& a, int mode, int nrows, cudaStream_t st) {
-    if (a.npass == 0) return cudaSuccess;
-    dim3 grid(a.Lp / PF_T, nrows, a.npass);
+    if (a.npass == 0 || a.nth == 0) return cudaSuccess;
+    dim3 grid((a.Lp / PF_T) * PF_SPLIT, nrows, a.npass);
     if (mode == 0) pre_forward_kernel<2><<<grid, PF_T, 0, st>>>(a);
     else pre_forward_kernel<1><<<grid, PF_T, 0, st>>>(a);
     count_launch();

@@ -39,15 +39,16 @@ constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on 
 // =============================================================================================================
 // FOLD (n = 0 on a ring set symmetric about the equator): only the northern rings are recursed.  d^l_{m0}(pi - theta) =
 // (-1)^{l+m} d^l_{m0}(theta), so with E = sum over l+m even and O = sum over l+m odd of G d:
-// F_m(theta) = E + O and F_m(pi - theta) = E - O.  A thread's degrees la + j alternate in parity with j (la is even), so two
-// accumulator sets (j even / j odd) are kept and the reducers emit both rings.
+// F_m(theta) = E + O and F_m(pi - theta) = E - O.  The degrees of a WARP all have one parity (warp w: degrees
+// l0 + 16 (w/2) + (w%2) + 2j), so every warp still hands over ONE partial-sum set -- the shared-memory footprint of the plain kernel,
+// 128-ring tiles included -- and the reducers add the even-degree warps and the odd-degree warps apart and emit both rings.
 template <int RL, int RT, int NW, int NC, bool FOLD>
 struct InvSmem {
-    static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2, NSET = FOLD ? 2 : 1;
-    static constexpr int NRS = (NC == 1 && !FOLD) ? 4 : 2;   // the one-column partial sums are half the size: a deeper hand-off fits
+    static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2, NSET = FOLD ? 2 : 1;   // NSET: sets the reducers keep apart
+    static constexpr int NRS = NC == 1 ? 4 : 2;   // the one-column partial sums are half the size: a deeper hand-off fits
     double op[NST][KS][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
     double lam[NST][KS][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
-    double red[NRS][KS][NW][NSET][NTH][2 * NC];   // per-warp partial sums
+    double red[NRS][KS][NW][NTH][2 * NC];   // per-warp partial sums
     int act[NRS][NW];                       // bit h: the warp wrote partial sums for step h of the pair
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
@@ -56,7 +57,7 @@ template <int RL, int RT, int NW, int NC, bool FOLD>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(const ThetaArgs A) {
     using S = InvSmem<RL, RT, NW, NC, FOLD>;
     constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS, NSET = S::NSET;
-    static_assert(!FOLD || (RL % 2 == 0), "degrees of a thread alternate in parity");
+    static_assert(!FOLD || (NW % 2 == 0), "even-degree and odd-degree warps come in pairs");
     static_assert(TL == SHT_TQ, "the block's degrees must be one kappa quantum");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
@@ -132,13 +133,16 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                 for (int ww = 0; ww < NW; ++ww) {
                     if ((actb[ww] >> h) & 1) {
                         any = true;
+                        constexpr int e = 0;
+                        const int es = FOLD ? (ww & 1) : e;       // FOLD: warp ww carries degrees of parity ww & 1
+                        const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]) + at;
 #pragma unroll
-                        for (int e = 0; e < NSET; ++e) {
-                            const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][e][0][0]) + at;
-#pragma unroll
-                            for (int q = 0; q < NQ; ++q)
-                                if (at + NAUX * 32 * q < NOUT) { const double2 t = r[NAUX * 32 * q]; v[e][q].x += t.x; v[e][q].y += t.y; }
-                        }
+                        for (int q = 0; q < NQ; ++q)
+                            if (at + NAUX * 32 * q < NOUT) {
+                                const double2 t = r[NAUX * 32 * q];
+                                if (FOLD && es) { v[NSET - 1][q].x += t.x; v[NSET - 1][q].y += t.y; }
+                                else { v[0][q].x += t.x; v[0][q].y += t.y; }
+                            }
                     }
                 }
                 if (any) {
@@ -172,7 +176,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     reg_alloc_compute();
 
     // -------------------------------------------------------------------- compute warps
-    const int la = l0 + w * RL, l_hi = la + RL - 1;   // degrees of this warp
+    // degrees of this warp: la + DS j, j < RL (FOLD: one parity per warp, DS = 2)
+    constexpr int DS = FOLD ? 2 : 1;
+    const int la = FOLD ? l0 + 2 * RL * (w >> 1) + (w & 1) : l0 + w * RL, l_hi = la + DS * (RL - 1);
     const bool warp_real = la < A.L;
     double cur[NI], prev[NI];
     KPack<NI> kp;
@@ -192,33 +198,31 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         if (m >= la) {                                // the degree l == m starts (warp-uniform): Eq. 27 start values
 #pragma unroll
             for (int j = 0; j < RL; ++j) {
-                if (m == la + j) {
+                if (m == la + DS * j) {
 #pragma unroll
                     for (int i = 0; i < RT; ++i) {
-                        ca[j * RT + i] = stv[(size_t)j * A.ntp + 32 * i];
+                        ca[j * RT + i] = stv[(size_t)(DS * j) * A.ntp + 32 * i];
                         cb[j * RT + i] = 0.0;
-                        kp.set(j * RT + i, stk[(size_t)j * A.ntp + 32 * i]);
+                        kp.set(j * RT + i, stk[(size_t)(DS * j) * A.ntp + 32 * i]);
                     }
                 }
             }
             wact = true;                              // re-evaluated at the next window check
         }
-        const double* row = &sm.op[slot][h][(w * RL) * ROWD];
+        const double* row = &sm.op[slot][h][(la - l0) * ROWD];
         const double s = row[ROWD - 1];
         double lam[RT];
 #pragma unroll
         for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][h][lane + 32 * i] * s;
         if (wact) {
-            double acc[NSET][RT][2 * NC];
+            double acc[RT][2 * NC];
 #pragma unroll
-            for (int e = 0; e < NSET; ++e)
+            for (int i = 0; i < RT; ++i)
 #pragma unroll
-                for (int i = 0; i < RT; ++i)
-#pragma unroll
-                    for (int c = 0; c < 2 * NC; ++c) acc[e][i][c] = 0.0;
+                for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.0;
 #pragma unroll
             for (int j = 0; j < RL; ++j) {
-                const double* r = row + j * ROWD;
+                const double* r = row + (DS * j) * ROWD;
                 double cf[2 * NC];
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
@@ -230,25 +234,20 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                 for (int i = 0; i < RT; ++i) {
                     const double e = ca[j * RT + i];
 #pragma unroll
-                    for (int c = 0; c < 2 * NC; ++c) acc[FOLD ? (j & 1) : 0][i][c] = fma(e, cf[c], acc[FOLD ? (j & 1) : 0][i][c]);
+                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fma(e, cf[c], acc[i][c]);
                     cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
                 }
             }
+            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
 #pragma unroll
-            for (int e = 0; e < NSET; ++e) {
-                double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][e][0][0]);
+            for (int i = 0; i < RT; ++i)
 #pragma unroll
-                for (int i = 0; i < RT; ++i)
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) {
-                        rd[c * NTH + lane + 32 * i] = make_double2(acc[e][i][2 * c], acc[e][i][2 * c + 1]);
-                    }
-            }
+                for (int c = 0; c < NC; ++c) rd[c * NTH + lane + 32 * i] = make_double2(acc[i][2 * c], acc[i][2 * c + 1]);
             wrote = true;
         } else {                                      // every item of the warp is still below 2^-340: recursion only
 #pragma unroll
             for (int j = 0; j < RL; ++j) {
-                const double g = row[j * ROWD + 2 * NC];
+                const double g = row[(DS * j) * ROWD + 2 * NC];
 #pragma unroll
                 for (int i = 0; i < RT; ++i) cb[j * RT + i] = fma(lam[i], ca[j * RT + i], -(g * cb[j * RT + i]));
             }
@@ -599,8 +598,10 @@ static bool small_tiles(const ThetaArgs& a, int big) {
 }
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
-    // folded inverse: two partial-sum sets; the two-column (PM) variant fits shared memory with 64 rings per block only
-    if (a.fold0) return mode == 0 ? launch_inv<8, 2, 8, 2, true>(a, st) : launch_inv<8, 4, 8, 1, true>(a, st);
+    if (a.fold0) {
+        if (small_tiles(a, 128)) return mode == 0 ? launch_inv<8, 2, 8, 2, true>(a, st) : launch_inv<8, 2, 8, 1, true>(a, st);
+        return mode == 0 ? launch_inv<8, 4, 8, 2, true>(a, st) : launch_inv<8, 4, 8, 1, true>(a, st);
+    }
     if (small_tiles(a, 128)) return mode == 0 ? launch_inv<8, 2, 8, 2>(a, st) : launch_inv<8, 2, 8, 1>(a, st);
     return mode == 0 ? launch_inv<8, 4, 8, 2>(a, st) : launch_inv<8, 4, 8, 1>(a, st);
 }
