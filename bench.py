@@ -283,7 +283,8 @@ def main():
     if args.dtype == "f32":
         flm_h = flm_h.astype(np.complex64)
     flm = torch.from_numpy(flm_h).to(dev)
-    plan = api.Plan(L, spin, device=dev, batch=B, dtype=args.dtype)
+    # (ring shards need the inverse on the MW rings themselves: the midpoint-ring resampling of the default plan mixes rings)
+    plan = api.Plan(L, spin, device=dev, batch=B, dtype=args.dtype, invsym=False if sharded else None)
     f = torch.empty(plan.map_shape, dtype=plan.map_dtype, device=dev)
     back = torch.empty_like(flm)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2

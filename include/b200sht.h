@@ -60,7 +60,8 @@ enum {
     SHT_OPT_FOLD_ON  = 1u << 0,   /* spin 0: run the recursion on the northern rings only (north-south fold) ...   */
     SHT_OPT_FOLD_OFF = 1u << 1,   /* ... or on all rings.  Default: folded when the northern half alone fills the GPU (MW: L >= 2048) */
     SHT_OPT_INVSYM   = 1u << 2,   /* spin-0 MW inverse on the L midpoint rings (2j+1)pi/(2L) with the fold, then an exact FFT
-                                     resampling of F_m to the MW rings (off by default: measured not faster) */
+                                     resampling of F_m to the MW rings.  Default where the fold is on (L >= 2048) ...               */
+    SHT_OPT_NO_INVSYM = 1u << 7,  /* ... this flag keeps the inverse on the MW rings themselves (needed for ring shards)            */
     SHT_OPT_TILE64   = 1u << 3,   /* force 64-ring block tiles in the fused kernels ...                                          */
     SHT_OPT_TILE128  = 1u << 4,   /* ... or 128-ring tiles.  Default: 64 when 128-ring tiles give fewer blocks than the device has SMs */
     SHT_OPT_PRECOMPUTE = 1u << 6, /* the paper's full-precomputation mode (Sec. 4.3): the Wigner d-functions of every
@@ -153,7 +154,8 @@ sht_status s2_theta_forward_plan(sht_plan* plan, const void* Wm, void* flm, sht_
  *             the transform: one all-reduce (NCCL, fp64 sum) of L (2L-1) complex numbers.
  *   inverse : the full flm in (replicated) -> a map in which only the shard's rings are filled, all others are zero.  No
  *             collective is needed (each GPU owns its rings); the sum over ranks is the full map.
- * (0, 1) restores the whole transform.  SO(3) plans shard the same way.  SHT_EUNSUPPORTED for batched / fp32 / INVSYM / ADJOINT plans.
+ * (0, 1) restores the whole transform.  SO(3) plans shard the same way.  SHT_EUNSUPPORTED for batched / fp32 / ADJOINT plans and for
+ * MW plans whose inverse runs on the midpoint rings (create the plan with SHT_OPT_NO_INVSYM: the resampling mixes rings).
  * sht_plan_shard_range() reports the share: first kernel ring and count, for the forward or the inverse ring set. */
 sht_status sht_plan_set_shard(sht_plan* plan, int rank, int nranks);
 sht_status sht_plan_shard_range(const sht_plan* plan, int forward, int* first, int* count);

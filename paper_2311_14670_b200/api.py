@@ -40,14 +40,14 @@ class Plan:
     """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
 
     def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1, dtype="f64",
-                 fold=None, invsym=False, tile=None, adjoint=False, precompute=False):
+                 fold=None, invsym=None, tile=None, adjoint=False, precompute=False):
         """fold / invsym / tile map to the SHT_OPT_* creation flags (None = the library's automatic choice)."""
         self._h = C.c_void_p()
         opts = 0
         if fold is not None:
             opts |= _lib.SHT_OPT_FOLD_ON if fold else _lib.SHT_OPT_FOLD_OFF
-        if invsym:
-            opts |= _lib.SHT_OPT_INVSYM
+        if invsym is not None:
+            opts |= _lib.SHT_OPT_INVSYM if invsym else _lib.SHT_OPT_NO_INVSYM
         if tile is not None:
             opts |= {64: _lib.SHT_OPT_TILE64, 128: _lib.SHT_OPT_TILE128}[tile]
         if adjoint:

@@ -1009,10 +1009,12 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if (opts & SHT_OPT_PRECOMPUTE) {
         // stored d-functions (Sec. 4.3): single-map fp64 plans; the tables hold every ring, so the folds are off
         if (batch != 1 || dtype != SHT_F64 || (opts & (SHT_OPT_FOLD_ON | SHT_OPT_INVSYM | SHT_OPT_ADJOINT))) return SHT_EUNSUPPORTED;
+        opts |= SHT_OPT_NO_INVSYM;
         opts |= SHT_OPT_FOLD_OFF;
     }
     if ((opts & SHT_OPT_FOLD_ON) && (opts & SHT_OPT_FOLD_OFF)) return SHT_EINVAL;
     if ((opts & SHT_OPT_TILE64) && (opts & SHT_OPT_TILE128)) return SHT_EINVAL;
+    if ((opts & SHT_OPT_INVSYM) && (opts & SHT_OPT_NO_INVSYM)) return SHT_EINVAL;
     // fp32 variant (BASELINE config 5): spin 0, MW sampling, one map
     if (dtype == SHT_F32 && (spin != 0 || sampling != SHT_MW || batch != 1)) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
@@ -1040,11 +1042,14 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
         if (opts & SHT_OPT_FOLD_ON) on = true;
         if (opts & SHT_OPT_FOLD_OFF) on = false;
         if (on && P->fwd.symmetric && only_dir != 1) { P->fold0 = 1; north_only(P->fwd); }
-        // MW inverse: the MW rings (2t+1)pi/(2L-1) are not symmetric; SHT_OPT_INVSYM evaluates F_m on the L midpoint rings instead
-        // (folded) and resamples to the MW rings with two FFT passes (resample_sym_to_mw).  Off by default: the two-column folded
-        // inverse kernel only fits shared memory with 64-ring tiles and gains 17 % on the hot kernel at L = 2048 (3.03 -> 2.53 ms)
-        // while the resampling adds 0.77 ms of FFT + staging (measured).
-        const bool isym = (opts & SHT_OPT_INVSYM) && sampling == SHT_MW && batch == 1 && dtype == SHT_F64;
+        // MW inverse: the MW rings (2t+1)pi/(2L-1) are not symmetric.  F_m is evaluated on the L midpoint rings (2j+1)pi/(2L) instead, with
+        // the north-south fold (half the d-steps), and resampled to the MW rings with two FFT passes (resample_sym_to_mw; exact).
+        // Default wherever the fold itself is worth it (L >= 2048 on 148 SMs): measured inverse totals 3.39 -> 3.13 ms at L = 2048,
+        // 23.8 -> 21.0 ms at L = 4096, 171.3 -> 131.6 ms at L = 8192.  SHT_OPT_INVSYM / SHT_OPT_NO_INVSYM override.
+        bool isym = on;
+        if (opts & SHT_OPT_INVSYM) isym = true;
+        if (opts & (SHT_OPT_NO_INVSYM | SHT_OPT_FOLD_OFF)) isym = false;
+        isym = isym && sampling == SHT_MW && batch == 1 && dtype == SHT_F64 && !helper && !(opts & SHT_OPT_ADJOINT);
         if (isym) { P->invsym = 1; P->fold0i = 1; rings_mid(P->inv, L); north_only(P->inv); }
         // the rings of the map are symmetric about the equator on every sampling but MW: fold the inverse too.  DH has 2L rings, so
         // its folded inverse does the work of an MW inverse; it is folded whatever the size.
@@ -1246,7 +1251,7 @@ sht_status sht_plan_timings(sht_plan* P, float ms[4]) {
 sht_status sht_plan_set_shard(sht_plan* P, int rank, int nranks) {
     if (!P || nranks < 1 || rank < 0 || rank >= nranks) return SHT_EINVAL;
     if (nranks > 1 && (P->batch > 1 || P->dtype != SHT_F64 || P->invsym || (P->opts & SHT_OPT_ADJOINT))) {   // (precompute plans shard too)
-        g_err = "ring shards are built for single-map fp64 plans without SHT_OPT_INVSYM / SHT_OPT_ADJOINT";
+        g_err = "ring shards need a single-map fp64 plan created with SHT_OPT_NO_INVSYM and without SHT_OPT_ADJOINT";
         return SHT_EUNSUPPORTED;
     }
     P->shard_rank = rank; P->shard_n = nranks;

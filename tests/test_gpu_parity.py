@@ -240,7 +240,7 @@ def test_spin0_forward_with_and_without_north_south_fold(api, orc, fold, samplin
 @pytest.mark.parametrize("sym", ["0", "1"])
 @pytest.mark.parametrize("L,real", [(1, False), (2, False), (8, False), (33, False), (64, False), (130, False), (200, True), (257, False)])
 def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, sym, L, real):
-    """MW spin-0 inverse either directly on the MW rings (default), or (plan option SHT_OPT_INVSYM) on the L midpoint rings (2j+1)pi/(2L) with the
+    """MW spin-0 inverse either directly on the MW rings (SHT_OPT_NO_INVSYM; default below L = 2048), or (SHT_OPT_INVSYM; default from L = 2048) on the L midpoint rings (2j+1)pi/(2L) with the
     north-south fold followed by an exact FFT resampling of F_m(theta) to the MW rings.  Both against the oracle, element by element,
     through the full transform and through the theta-stage entry point."""
     flm = synth.random_flm(L, 0, seed=5 * L, real=real)
