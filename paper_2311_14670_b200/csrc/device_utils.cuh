@@ -59,9 +59,12 @@ __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7
 #define SHT_HI_DEAD ((1023 + 500) << 20)
 
 // The register file is split over the 4 SM sub-partitions (16 K registers each, 3 warps each with 8 compute + 4 auxiliary
-// warps): compute warps take 232 registers per thread, auxiliary warps 40 (2*32*232 + 32*40 = 16128); kernels launch at 168.
-__device__ __forceinline__ void reg_dealloc_aux() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
-__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
+// warps): 2*32*RC + 32*RA <= 16384.  Default: compute warps 232 registers per thread, auxiliary warps 48 (exactly 16384); kernels
+// whose auxiliary warps carry more state (folded inverse: two sums, two output rings) take 224 / 64.  Kernels launch at 168.
+template <int RA = 48>
+__device__ __forceinline__ void reg_dealloc_aux() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(RA)); }
+template <int RC = 232>
+__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RC)); }
 
 // Window counters k (internal.h) of the NI items of a thread, one byte each.  0xff = item not started yet.
 template <int NI>
