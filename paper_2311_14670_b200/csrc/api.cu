@@ -122,6 +122,7 @@ struct sht_plan {
     double* Ob = nullptr;      // batched path: result scratch of all passes
     std::vector<size_t> ob_off_inv, ob_off_fwd;   // per-pass offsets (doubles) into Ob
     std::vector<int> slab_n;   // second index n of d^l_{m,n} per slab
+    int *d_slab_n = nullptr, *d_cslab = nullptr;   // device copies: n per slab; slab -> slab of the public coefficient array
     RingSet inv, fwd;          // rings of the inverse theta step / of the forward quadrature
     int kmin = 0, kstride = 0, krows = 0;
     int8_t* kexp = nullptr;
@@ -331,6 +332,7 @@ void layout(sht_plan* P, char* base) {
     Bump B; B.base = base;
     const int L = P->L, Lp = P->Lp, NB = P->NB;
     P->d_flag = B.take<int>(64);
+    P->d_slab_n = B.take<int>(P->nslab); P->d_cslab = B.take<int>(P->nslab);
     P->rsq = B.take<double>(2 * (size_t)Lp + 64);
     P->kexp = B.take<int8_t>((size_t)P->krows * P->kstride);
     P->ctab = B.take<double>((size_t)(L - P->mmin) * Lp);
@@ -423,11 +425,13 @@ void add_passes(sht_plan* P, int slab, int n, bool real) {
         (void)mlo_key;
         return a;
     };
-    if (n == 0) {
+    if (n == 0 && P->kind == 0) {
         PassHost a = mk(0, +1, 0, real ? 1 : 0, -1);
         P->pinv.push_back(a); P->pfwd.push_back(a);
         P->inv.start[0]; P->fwd.start[0];
     } else {
+        // (SO(3) plans send n = 0 through the same two passes as the other orders, so that ONE launch serves all 2N-1 slabs: a
+        //  separate +-m launch for the single n = 0 slab would occupy 8 blocks of the GPU for a whole recursion)
         int an = n < 0 ? -n : n;
         PassHost a = mk(n, +1, -an, 1, 2 * n), b = mk(-n, -1, 1 - an, 1, 2 * n + 1);
         P->pinv.push_back(a); P->pinv.push_back(b);
@@ -636,7 +640,7 @@ sht_status upload_passes(sht_plan* P, cudaStream_t st) {
         for (auto& ph : (dir ? P->pfwd : P->pinv)) {
             ThetaPass t = ph.p;
             t.st_val = R.start[t.n].val; t.st_k = R.start[t.n].k;
-            if (t.n != 0) {
+            if (t.n != 0 || P->kind == 1) {      // (SO(3) plans route n = 0 through the general passes too)
                 int n_slab = t.sgn_out > 0 ? t.n : -t.n;
                 t.m_lo = R.mlo[2 * n_slab + (t.sgn_out > 0 ? 0 : 1)];
             } else t.m_lo = nullptr;
@@ -712,18 +716,11 @@ sht_status zero_async(void* p, size_t bytes, cudaStream_t st) {
 sht_status inverse_poles(sht_plan* P, const double2* coef, cudaStream_t st) {
     const int L = P->L;
     const int nreg = P->inv.nfull ? P->inv.nfull : P->inv.nth;
-    for (int s = 0; s < P->nslab; ++s) {
-        const int n = P->slab_n[s];
-        double2* Fs = P->F + P->F_slab * s;
-        if (P->inv.pole && P->shard_rank == P->shard_n - 1) {        // the south pole belongs to the last ring shard, the north pole to the first
-            const int row = (-n) < 0 ? -n + P->NB : -n;
-            CK(st_pole_inverse(L, n, 0, coef + (size_t)s * L * P->M, P->scale_inv, Fs + (size_t)row * P->F_ld + P->col0 + nreg, st));
-        }
-        if (P->inv.pole_n && P->shard_rank == 0) {
-            const int row = n < 0 ? n + P->NB : n;
-            CK(st_pole_inverse(L, n, 1, coef + (size_t)s * L * P->M, P->scale_inv, Fs + (size_t)row * P->F_ld, st));
-        }
-    }
+    const size_t cs = (size_t)L * P->M;
+    if (P->inv.pole && P->shard_rank == P->shard_n - 1)        // the south pole belongs to the last ring shard, the north pole to the first
+        CK(st_pole_inverse(L, 0, P->NB, P->nslab, P->d_slab_n, P->d_cslab, coef, cs, P->scale_inv, P->F, P->F_slab, P->F_ld, P->col0 + nreg, st));
+    if (P->inv.pole_n && P->shard_rank == 0)
+        CK(st_pole_inverse(L, 1, P->NB, P->nslab, P->d_slab_n, P->d_cslab, coef, cs, P->scale_inv, P->F, P->F_slab, P->F_ld, 0, st));
     return SHT_OK;
 }
 
@@ -782,10 +779,8 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         if (P->reality) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F, st));
         return SHT_OK;
     }
-    for (auto& ph : P->pinv)
-        CK(st_prep_inverse(L, P->Lp, ph.mode == 0 ? 2 : 1, ph.p.n, ph.p.sgn_out, ph.p.m_end, P->mmin, coef + (size_t)ph.p.slab * L * P->M,
-                           P->scale_inv, P->ctab, P->sgtab, P->sgstride,
-                           const_cast<double*>(ph.p.in) + (size_t)P->Lp * theta_inverse_rowd(ph.mode), st));
+    CK(st_prep_inverse(L, P->Lp, 2, P->mmin, P->n_inv_pm, coef, (size_t)L * P->M, P->d_cslab, P->scale_inv, P->ctab, P->sgtab, P->sgstride, P->d_inv_pm, st));
+    CK(st_prep_inverse(L, P->Lp, 1, P->mmin, P->n_inv_p, coef, (size_t)L * P->M, P->d_cslab, P->scale_inv, P->ctab, P->sgtab, P->sgstride, P->d_inv_p, st));
     CS(zero_async(P->F, sizeof(double2) * P->F_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
     if (P->precomp) {
@@ -856,17 +851,15 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     }
     int slo, shi;
     shard_range(P, true, &slo, &shi);
-    for (auto& ph : P->pfwd) {
-        int n_slab = P->slab_n[ph.p.slab];
-        if (P->fold0) {
+    if (P->fold0) {         // n = 0 on the northern rings: E / O operand sets (one pass)
+        for (auto& ph : P->pfwd) {
             const int NC = ph.mode == 0 ? 2 : 1;
             CK(st_weight_split_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, ph.p.m_end, P->fwd.wq, U + U_slab * ph.p.slab,
                                      reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * 2 * NC, slo, shi, st));
-            continue;
         }
-        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, n_slab, ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo,
-                           P->fwd.wq, U + U_slab * ph.p.slab,
-                           reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * (ph.mode == 0 ? 2 : 1), slo, shi, st));
+    } else {
+        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, 2, P->mmin, P->n_fwd_pm, P->fwd.wq, U, U_slab, P->d_fwd_pm, slo, shi, st));
+        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, 1, P->mmin, P->n_fwd_p, P->fwd.wq, U, U_slab, P->d_fwd_p, slo, shi, st));
     }
     CS(zero_async(P->H, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
@@ -914,11 +907,11 @@ sht_status resample_sym_to_mw(sht_plan* P, cudaStream_t st) {
 sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
     const int L = P->L, T2 = 4 * L, mwss = P->sampling == SHT_MWSS;
     stage(P, CAT_STAGE, st);
-    for (int s = 0; s < P->nslab; ++s) CK(st_mw_extend(L, P->slab_n[s], mwss, P->Ltp, P->Tcirc, P->Fa + P->Fa_slab * s, P->X + P->X_slab * s, st));
+    CK(st_mw_extend(L, P->nslab, P->d_slab_n, mwss, P->Ltp, P->Tcirc, P->Fa, P->Fa_slab, P->X, P->X_slab, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_FORWARD, st));
     stage(P, CAT_STAGE, st);
-    for (int s = 0; s < P->nslab; ++s) CK(st_mw_pad_phase(L, mwss, P->Tcirc, T2, P->X + P->X_slab * s, P->Z + P->Z_slab * s, st));
+    CK(st_mw_pad_phase(L, P->nslab, mwss, P->Tcirc, T2, P->X, P->X_slab, P->Z, P->Z_slab, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th2, P->Z, P->Z, CUFFT_INVERSE, st));
     return SHT_OK;
@@ -1113,6 +1106,13 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     layout(P, (char*)work);
     const int L = P->L, Lp = P->Lp;
     CK(cudaMemsetAsync(P->d_flag, 0, 64 * sizeof(int), st));
+    {   // SO(3): internal slabs are in gamma-FFT bin order, the public coefficient array in n order (n + N - 1)
+        std::vector<int> cs(P->nslab);
+        for (int b = 0; b < P->nslab; ++b) cs[b] = P->kind == 1 ? P->slab_n[b] + P->N - 1 : b;
+        CK(cudaMemcpyAsync(P->d_slab_n, P->slab_n.data(), sizeof(int) * P->nslab, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(P->d_cslab, cs.data(), sizeof(int) * P->nslab, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+    }
     CK(st_rsq(2 * Lp + 64, P->rsq, st));
     CK(st_kexp(P->krows, P->kstride, P->kmin, P->kexp, st));
     CK(st_ctab(L, Lp, P->mmin, P->kstride, P->kmin, P->kexp, P->rsq, P->ctab, st));
@@ -1299,7 +1299,7 @@ sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_str
     P->fwd.wq = saved;
     if (s == SHT_OK) {
         stage(P, CAT_STAGE, st);
-        cudaError_t e = st_finalize_forward(P->L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H, (double2*)flm, st);
+        cudaError_t e = st_finalize_forward(P->L, P->Lp, 1, P->d_slab_n, P->d_cslab, P->reality, P->scale_fwd, P->H, P->H_slab, (double2*)flm, 0, st);
         if (e != cudaSuccess) s = SHT_ECUDA;
         stage(P, CAT_STAGE, st);
     }
@@ -1355,7 +1355,7 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
         CS(healpix_analysis(P, f, st));
         CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
         stage(P, CAT_STAGE, st);
-        CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H, (double2*)flm, st));
+        CK(st_finalize_forward(L, P->Lp, 1, P->d_slab_n, P->d_cslab, P->reality, P->scale_fwd, P->H, P->H_slab, (double2*)flm, 0, st));
         stage(P, CAT_STAGE, st);
         return SHT_OK;
     }
@@ -1370,8 +1370,7 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
     } else                      // DH / GL: explicit quadrature on the rings of the map (Eq. 36 / 46)
         CS(run_theta_forward(P, P->Fa, P->Fa_slab, P->Ltp, st));
     stage(P, CAT_STAGE, st);
-    for (int b = 0; b < P->batch; ++b)
-        CK(st_finalize_forward(L, P->Lp, P->slab_n[0], P->reality, P->scale_fwd, P->H + P->H_slab * b, (double2*)flm + ncoef * b, st));
+    CK(st_finalize_forward(L, P->Lp, P->batch, P->d_slab_n, P->d_cslab, P->reality, P->scale_fwd, P->H, P->H_slab, (double2*)flm, ncoef, st));
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
@@ -1406,7 +1405,7 @@ sht_status adjoint_analysis(sht_plan* P, const double2* U, size_t U_slab, int ld
     if (P->adj_inv) {           // MW / MWSS: helper plan on the rings of the map; U points at its first regular ring
         sht_plan* Q = P->adj_inv;
         CS(run_theta_forward(Q, U + P->col0, U_slab, ldu, st));
-        CK(st_finalize_forward(P->L, Q->Lp, Q->slab_n[0], 0, Q->scale_fwd, Q->H, flm, st));
+        CK(st_finalize_forward(P->L, Q->Lp, 1, Q->d_slab_n, Q->d_cslab, 0, Q->scale_fwd, Q->H, Q->H_slab, flm, 0, st));
         return SHT_OK;
     }
     double* saved = P->fwd.wq;
@@ -1414,7 +1413,7 @@ sht_status adjoint_analysis(sht_plan* P, const double2* U, size_t U_slab, int ld
     sht_status s = run_theta_forward(P, U, U_slab, ldu, st);
     P->fwd.wq = saved;
     CS(s);
-    CK(st_finalize_forward(P->L, P->Lp, P->slab_n[0], 0, P->scale_fwd, P->H, flm, st));
+    CK(st_finalize_forward(P->L, P->Lp, 1, P->d_slab_n, P->d_cslab, 0, P->scale_fwd, P->H, P->H_slab, flm, 0, st));
     return SHT_OK;
 }
 // inverse-type kernel on the quadrature rings: returns the array [bins][ld] holding F_m on ALL quadrature rings (unweighted)
@@ -1497,11 +1496,8 @@ sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream s
     const size_t slab = (size_t)L * NB;
     begin_transform(P);
     stage(P, CAT_STAGE, st);
-    // coefficient slabs from n order (n+N-1) to gamma-FFT bin order
-    for (int b = 0; b < P->nslab; ++b)
-        CK(cudaMemcpyAsync(P->fn + slab * b, (const double2*)flmn + slab * (P->slab_n[b] + N - 1), sizeof(double2) * slab, cudaMemcpyDeviceToDevice, st));
-    count_bytes(32.0 * (double)slab * P->nslab);
-    CS(run_theta_inverse(P, P->fn, st));
+    // (coefficient slabs are read in place: the staging kernels map gamma-FFT bin order to n order through d_cslab)
+    CS(run_theta_inverse(P, (const double2*)flmn, st));
     stage(P, CAT_FFT, st);
     for (int b = 0; b < P->nslab; ++b) CS(fft_exec(P, P->fft_phi_inv, P->F + P->F_slab * b, (double2*)f + slab * b, CUFFT_INVERSE, st));
     CS(fft_exec(P, P->fft_gamma, (double2*)f, (double2*)f, CUFFT_INVERSE, st));          // Eq. 17
@@ -1521,8 +1517,7 @@ sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream s
     CS(mw_upsample(P, st));
     CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
     stage(P, CAT_STAGE, st);
-    for (int b = 0; b < P->nslab; ++b)
-        CK(st_finalize_forward(L, P->Lp, P->slab_n[b], 0, P->scale_fwd, P->H + P->H_slab * b, (double2*)flmn + slab * (P->slab_n[b] + N - 1), st));
+    CK(st_finalize_forward(L, P->Lp, P->nslab, P->d_slab_n, P->d_cslab, 0, P->scale_fwd, P->H, P->H_slab, (double2*)flmn, slab, st));
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }

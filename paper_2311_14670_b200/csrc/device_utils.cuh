@@ -58,13 +58,19 @@ __device__ __forceinline__ int hi_abs(double v) { return __double2hiint(v) & 0x7
 #define SHT_HI_TWIN ((1023 + SHT_TWIN) << 20)
 #define SHT_HI_DEAD ((1023 + 500) << 20)
 
-// The register file is split over the 4 SM sub-partitions (16 K registers each, 3 warps each with 8 compute + 4 auxiliary
-// warps): 2*32*RC + 32*RA <= 16384.  Default: compute warps 232 registers per thread, auxiliary warps 48 (exactly 16384); kernels
-// whose auxiliary warps carry more state (folded inverse: two sums, two output rings) take 224 / 64.  Kernels launch at 168.
-template <int RA = 48>
+// Register budgets re-split with setmaxnreg.  The kernels launch 12 warps (8 compute + 4 auxiliary, 3 per SM sub-partition) at 168
+// registers per thread, so each sub-partition's pool is 3 * 32 * 168 = 16128 registers, and a split must satisfy
+// 2 * 32 * RC + 32 * RA <= 16128 EXACTLY within that pool -- a compute warp asking for more than the auxiliary warps released waits
+// forever.  RA = 40 -> RC = 232 (default); RA = 56 -> RC = 224 (kernels whose auxiliary warps carry more state).
+template <int RA>
+struct RegSplit {
+    static constexpr int RC = (3 * 32 * 168 - 32 * RA) / 64;
+    static_assert(RA % 8 == 0 && RC % 8 == 0 && 64 * RC + 32 * RA <= 3 * 32 * 168, "register split exceeds the CTA's pool");
+};
+template <int RA = 40>
 __device__ __forceinline__ void reg_dealloc_aux() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(RA)); }
-template <int RC = 232>
-__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RC)); }
+template <int RA = 40>
+__device__ __forceinline__ void reg_alloc_compute() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RegSplit<RA>::RC)); }
 
 // Window counters k (internal.h) of the NI items of a thread, one byte each.  0xff = item not started yet.
 template <int NI>

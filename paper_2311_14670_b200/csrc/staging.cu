@@ -159,9 +159,15 @@ __global__ void k_mw_weights(int Lq, double qphi, double* __restrict__ w) {
 // ---- per-transform staging ------------------------------------------------------------------------------------
 // inverse prep: coef[l][NB] -> operand rows G[m-m_end][Lp][ROWD] of one pass: {c Re, c Im (x NC), g'_m(l), s_m} with
 // c = scale(l) * sign * c_m(l) (internal.h), through a 32x32 shared-memory transpose (coef is l-major, G is m-major).
-__global__ void k_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* __restrict__ coef,
-                               const double* __restrict__ scale, const double* __restrict__ C, const double2* __restrict__ SG,
-                               int sgstride, double* __restrict__ G) {
+__global__ void k_prep_inverse(int L, int Lp, int NC, int mmin, const double2* __restrict__ coef_base, size_t coef_slab,
+                               const int* __restrict__ cslab, const double* __restrict__ scale, const double* __restrict__ C,
+                               const double2* __restrict__ SG, int sgstride, const ThetaPass* __restrict__ passes) {
+    // one launch serves all passes of a kernel mode: grid.z = pass (its operand rows start one row into ThetaPass::in)
+    const ThetaPass P = passes[blockIdx.z];
+    const int n = P.n, sgn_out = P.sgn_out, m_end = P.m_end;
+    const double2* coef = coef_base + (size_t)cslab[P.slab] * coef_slab;
+    double* G = const_cast<double*>(P.in) + (size_t)Lp * (2 * NC + 2);
+    if (m_end + (int)blockIdx.y * 32 >= L) return;
     __shared__ double2 tile[2][32][33];
     const int NB = 2 * L - 1, an = n < 0 ? -n : n, ROWD = 2 * NC + 2;
     const int l0 = blockIdx.x * 32, m0 = m_end + blockIdx.y * 32;
@@ -194,8 +200,12 @@ __global__ void k_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_
 }
 // pole rings, inverse.  South (theta = pi, Eq. 29): F_{-n}(pi) = sum_l scale(l) f_{l,-n} (-1)^{l-n};  north (theta = 0, Eq. 28,
 // MWSS only): F_n(0) = sum_l scale(l) f_{l,n}  (d^l_{mn}(0) = delta_mn, d^l_{mn}(pi) = (-1)^{l+m} delta_{m,-n}).  One block per slab.
-__global__ void k_pole_inverse(int L, int n, int north, const double2* __restrict__ coef, const double* __restrict__ scale, double2* __restrict__ out) {
+__global__ void k_pole_inverse(int L, int north, int NBf, const int* __restrict__ slab_n, const int* __restrict__ cslab,
+                               const double2* __restrict__ coef_base, size_t coef_slab, const double* __restrict__ scale,
+                               double2* __restrict__ F, size_t F_slab, int ldf, int col) {
     __shared__ double sre[256], sim[256];
+    const int slab = blockIdx.x, n = slab_n[slab];
+    const double2* coef = coef_base + (size_t)cslab[slab] * coef_slab;
     const int an = n < 0 ? -n : n, NB = 2 * L - 1, m = north ? n : -n;
     double re = 0, im = 0;
     for (int l = an + threadIdx.x; l < L; l += blockDim.x) {
@@ -209,7 +219,7 @@ __global__ void k_pole_inverse(int L, int n, int north, const double2* __restric
         if ((int)threadIdx.x < k) { sre[threadIdx.x] += sre[threadIdx.x + k]; sim[threadIdx.x] += sim[threadIdx.x + k]; }
         __syncthreads();
     }
-    if (threadIdx.x == 0) { out->x = sre[0]; out->y = sim[0]; }
+    if (threadIdx.x == 0) F[F_slab * slab + (size_t)(m < 0 ? m + NBf : m) * ldf + col] = make_double2(sre[0], sim[0]);
 }
 // real signals: rows m < 0 of F from rows m > 0:  F_{-m}(theta) = conj(F_m(theta))
 __global__ void k_hermitian_rows(int L, int NB, int ntp, int nth, double2* __restrict__ F) {
@@ -233,8 +243,12 @@ __global__ void k_complex_to_real(size_t n, const double2* __restrict__ in, doub
 // Rings AT a pole hold one value of a spin-s function (n = -s): at theta = pi only the order m = -n survives (Eq. 29),
 // at theta = 0 only m = n (Eq. 28).  The samples of those rings are projected onto that component (F_m := 0 for the other m), which
 // makes the transform well defined on arbitrary arrays (R21; include/b200sht.h, s2_forward).
-__global__ void k_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* __restrict__ Fa, double2* __restrict__ X) {
+__global__ void k_mw_extend(int L, const int* __restrict__ slab_n, int mwss, int ldin, int ldout, const double2* __restrict__ Fa_base,
+                            size_t Fa_slab, double2* __restrict__ X_base, size_t X_slab) {
     int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const int n = slab_n[blockIdx.z];
+    const double2* Fa = Fa_base + Fa_slab * blockIdx.z;
+    double2* X = X_base + X_slab * blockIdx.z;
     const int T = mwss ? 2 * L : 2 * L - 1, tpole = mwss ? L : L - 1;
     if (t >= T) return;
     int m = b < L ? b : b - T;
@@ -249,8 +263,11 @@ __global__ void k_mw_extend(int L, int n, int mwss, int ldin, int ldout, const d
 // MW / MWSS forward (iii)->(iv): with Y = FFT_T of the extended samples, F_{mm'} = (1/T) e^{-i m' theta_0} Y[m' mod T] (theta_0 = pi/T
 // on MW, 0 on MWSS); Z[m' mod T2] = F_{mm'} e^{+i m' pi/T2} for |m'| <= L-1, zero elsewhere, so that the inverse FFT of length T2 = 4L
 // evaluates F_m on the midpoint rings theta'_u = (2u+1) pi/T2 (T2 samples of the circle; u < 2L are the rings in (0, pi)).
-__global__ void k_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* __restrict__ Y, double2* __restrict__ Z) {
+__global__ void k_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* __restrict__ Y_base, size_t Y_slab,
+                               double2* __restrict__ Z_base, size_t Z_slab) {
     int k2 = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    const double2* Y = Y_base + Y_slab * blockIdx.z;
+    double2* Z = Z_base + Z_slab * blockIdx.z;
     const int T = mwss ? 2 * L : 2 * L - 1, T2 = ldout;
     if (k2 >= T2) return;
     int mp = k2 < L ? k2 : (k2 > T2 - L ? k2 - T2 : T2);      // |m'| <= L-1, else none
@@ -301,9 +318,15 @@ __global__ void k_rows_head(int ncol, int ldin, int ldout, const double2* __rest
 // tiles W[m-m_end][ntp][NC] of one pass; rings not served by the pass at step m get 0 (peak split, R5).
 // fold != 0 (n != 0, symmetric ring set): column 0 = order +m at the ring itself (m >= m_s), column 1 = order -m at the MIRRORED
 // ring pi - theta (index nth-1-th), served by the same d-value up to (-1)^{l-n} (applied at the output), for m > m_s.
-__global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold,
-                               const int* __restrict__ m_lo, const double* __restrict__ wq, const double2* __restrict__ U,
-                               double2* __restrict__ W, int th_lo, int th_hi) {
+__global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* __restrict__ wq,
+                               const double2* __restrict__ U_base, size_t U_slab, const ThetaPass* __restrict__ passes, int th_lo, int th_hi) {
+    // one launch serves all passes of a kernel mode: grid.z = pass (its operand rows start one row into ThetaPass::in)
+    const ThetaPass P = passes[blockIdx.z];
+    const int n = P.sgn_out > 0 ? P.n : -P.n, sgn_out = P.sgn_out, m_end = P.m_end, fold = P.fold;
+    const int* __restrict__ m_lo = P.m_lo;
+    const double2* U = U_base + U_slab * P.slab;
+    double2* W = reinterpret_cast<double2*>(const_cast<double*>(P.in)) + (size_t)ntp * NC;
+    if (m_end + (int)blockIdx.y >= L) return;
     int th = blockIdx.x * blockDim.x + threadIdx.x;
     int m = m_end + blockIdx.y;
     if (th >= ntp) return;
@@ -368,9 +391,13 @@ __global__ void k_pole_forward(int L, int Lp, int n, int north, int NBin, int ld
     h->x += s * x.x; h->y += s * x.y;
 }
 // forward finalize: H[m+L-1][Lp] -> coef[l][m+L-1] = scale(l) * H on the support, 0 elsewhere; real: fill m<0.
-__global__ void k_finalize_forward(int L, int Lp, int n, int real, const double* __restrict__ scale, const double2* __restrict__ H,
-                                   double2* __restrict__ coef) {
+__global__ void k_finalize_forward(int L, int Lp, const int* __restrict__ slab_n, const int* __restrict__ cslab, int real,
+                                   const double* __restrict__ scale, const double2* __restrict__ H_base, size_t H_slab,
+                                   double2* __restrict__ coef_base, size_t coef_slab) {
     __shared__ double2 tile[32][33];
+    const int n = slab_n[blockIdx.z];
+    const double2* H = H_base + H_slab * blockIdx.z;
+    double2* coef = coef_base + (size_t)cslab[blockIdx.z] * coef_slab;
     const int NB = 2 * L - 1, an = n < 0 ? -n : n;
     int mi0 = blockIdx.x * 32, l0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {      // read H rows (mi), coalesced along l
@@ -752,11 +779,12 @@ cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st) {
     k_mw_weights<<<cdiv(Lq, 128), 128, 0, st>>>(Lq, qphi, w);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* coef, const double* scale,
-                            const double* C, const double2* SG, int sgstride, double* G, cudaStream_t st) {
-    dim3 grid(cdiv(Lp, 32), cdiv(L - m_end, 32)), block(32, 8);
-    k_prep_inverse<<<grid, block, 0, st>>>(L, Lp, NC, n, sgn_out, m_end, mmin, coef, scale, C, SG, sgstride, G);
-    count_bytes(16.0 * NC * (double)(L - m_end) * L + 8.0 * (2 * NC + 2) * (double)(L - m_end) * Lp); LAUNCHED(); return cudaSuccess;
+cudaError_t st_prep_inverse(int L, int Lp, int NC, int mmin, int npass, const double2* coef, size_t coef_slab, const int* cslab,
+                            const double* scale, const double* C, const double2* SG, int sgstride, const ThetaPass* passes, cudaStream_t st) {
+    if (npass == 0) return cudaSuccess;
+    dim3 grid(cdiv(Lp, 32), cdiv(L - mmin - 1, 32), npass), block(32, 8);
+    k_prep_inverse<<<grid, block, 0, st>>>(L, Lp, NC, mmin, coef, coef_slab, cslab, scale, C, SG, sgstride, passes);
+    count_bytes(npass * (16.0 * NC * (double)L * L / 2 + 8.0 * (2 * NC + 2) * (double)L * Lp)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* kexp, const double* rsq, double* C, cudaStream_t st) {
     k_ctab<<<cdiv(Lp, 64), 64, 0, st>>>(L, Lp, mmin, kstride, kmin, kexp, rsq, C);
@@ -771,9 +799,10 @@ cudaError_t st_lamtab(int n, int nth, int ntp, int m_end, int nrows, const doubl
     k_lamtab<<<dim3(cdiv(ntp, 128), nrows), 128, 0, st>>>(n, nth, ntp, m_end, csc, tau, sig, lam);
     LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_pole_inverse(int L, int n, int north, const double2* coef, const double* scale, double2* out, cudaStream_t st) {
-    k_pole_inverse<<<1, 256, 0, st>>>(L, n, north, coef, scale, out);
-    count_bytes(16.0 * L); LAUNCHED(); return cudaSuccess;
+cudaError_t st_pole_inverse(int L, int north, int NBf, int nslab, const int* slab_n, const int* cslab, const double2* coef, size_t coef_slab,
+                            const double* scale, double2* F, size_t F_slab, int ldf, int col, cudaStream_t st) {
+    k_pole_inverse<<<nslab, 256, 0, st>>>(L, north, NBf, slab_n, cslab, coef, coef_slab, scale, F, F_slab, ldf, col);
+    count_bytes(16.0 * L * nslab); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st) {
     if (L < 2) return cudaSuccess;
@@ -789,33 +818,37 @@ cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStr
     k_complex_to_real<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
     count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st) {
+cudaError_t st_mw_extend(int L, int nslab, const int* slab_n, int mwss, int ldin, int ldout, const double2* Fa, size_t Fa_slab, double2* X,
+                         size_t X_slab, cudaStream_t st) {
     const int T = mwss ? 2 * L : 2 * L - 1;
-    dim3 grid(cdiv(T, 128), T);
-    k_mw_extend<<<grid, 128, 0, st>>>(L, n, mwss, ldin, ldout, Fa, X);
-    count_bytes(32.0 * (double)T * T); LAUNCHED(); return cudaSuccess;
+    dim3 grid(cdiv(T, 128), T, nslab);
+    k_mw_extend<<<grid, 128, 0, st>>>(L, slab_n, mwss, ldin, ldout, Fa, Fa_slab, X, X_slab);
+    count_bytes(32.0 * (double)T * T * nslab); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st) {
+cudaError_t st_mw_pad_phase(int L, int nslab, int mwss, int ldin, int ldout, const double2* Y, size_t Y_slab, double2* Z, size_t Z_slab,
+                            cudaStream_t st) {
     const int T = mwss ? 2 * L : 2 * L - 1;
-    dim3 grid(cdiv(ldout, 128), T);
-    k_mw_pad_phase<<<grid, 128, 0, st>>>(L, mwss, ldin, ldout, Y, Z);
-    count_bytes(16.0 * (double)T * ((double)T + ldout)); LAUNCHED(); return cudaSuccess;
+    dim3 grid(cdiv(ldout, 128), T, nslab);
+    k_mw_pad_phase<<<grid, 128, 0, st>>>(L, mwss, ldin, ldout, Y, Y_slab, Z, Z_slab);
+    count_bytes(16.0 * (double)T * ((double)T + ldout) * nslab); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
-                            const double* wq, const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st) {
-    dim3 grid(cdiv(ntp, 128), L - m_end);
-    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, n, sgn_out, m_end, fold, m_lo, wq, U, W, th_lo, th_hi);
-    count_bytes(32.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
+cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int mmin, int npass, const double* wq, const double2* U,
+                            size_t U_slab, const ThetaPass* passes, int th_lo, int th_hi, cudaStream_t st) {
+    if (npass == 0) return cudaSuccess;
+    dim3 grid(cdiv(ntp, 128), L - mmin - 1, npass);
+    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, wq, U, U_slab, passes, th_lo, th_hi);
+    count_bytes(32.0 * NC * (double)(L - mmin - 1) * ntp * npass); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
                             cudaStream_t st) {
     k_pole_forward<<<cdiv(L, 128), 128, 0, st>>>(L, Lp, n, north, NBin, ldin, col, w, U, H);
     count_bytes(32.0 * L); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st) {
-    dim3 grid(cdiv(2 * L - 1, 32), cdiv(L, 32)), block(32, 8);
-    k_finalize_forward<<<grid, block, 0, st>>>(L, Lp, n, real, scale, H, coef);
-    count_bytes(32.0 * (double)(2 * L - 1) * L); LAUNCHED(); return cudaSuccess;
+cudaError_t st_finalize_forward(int L, int Lp, int nslab, const int* slab_n, const int* cslab, int real, const double* scale, const double2* H,
+                                size_t H_slab, double2* coef, size_t coef_slab, cudaStream_t st) {
+    dim3 grid(cdiv(2 * L - 1, 32), cdiv(L, 32), nslab), block(32, 8);
+    k_finalize_forward<<<grid, block, 0, st>>>(L, Lp, slab_n, cslab, real, scale, H, H_slab, coef, coef_slab);
+    count_bytes(32.0 * (double)(2 * L - 1) * L * nslab); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st) {
     dim3 grid(cdiv(ncol, 128), 2 * L - 1);      // rows r = m + L - 1 of the m-ordered array; NB = number of phi bins of the other one

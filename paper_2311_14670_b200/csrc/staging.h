@@ -9,25 +9,29 @@ cudaError_t st_kexp(int nrows, int kstride, int kmin, int8_t* kexp, cudaStream_t
 cudaError_t st_rsq(int n, double* rsq, cudaStream_t st);
 cudaError_t st_mw_weights(int Lq, double qphi, double* w, cudaStream_t st);
 cudaError_t st_mid_weights(int L, int count, double qphi, double* w, cudaStream_t st);
-cudaError_t st_prep_inverse(int L, int Lp, int NC, int n, int sgn_out, int m_end, int mmin, const double2* coef, const double* scale,
-                            const double* C, const double2* SG, int sgstride, double* G, cudaStream_t st);
+cudaError_t st_prep_inverse(int L, int Lp, int NC, int mmin, int npass, const double2* coef, size_t coef_slab, const int* cslab,
+                            const double* scale, const double* C, const double2* SG, int sgstride, const ThetaPass* passes, cudaStream_t st);
 cudaError_t st_ctab(int L, int Lp, int mmin, int kstride, int kmin, const int8_t* kexp, const double* rsq, double* C, cudaStream_t st);
 cudaError_t st_sgtab(int nrows, int ncol, int mmin, int kstride, int kmin, const int8_t* kexp, double2* SG, cudaStream_t st);
 cudaError_t st_lamtab(int n, int nth, int ntp, int m_end, int nrows, const double* csc, const double* tau, const double* sig, double* lam,
                       cudaStream_t st);
-cudaError_t st_pole_inverse(int L, int n, int north, const double2* coef, const double* scale, double2* out, cudaStream_t st);
+cudaError_t st_pole_inverse(int L, int north, int NBf, int nslab, const int* slab_n, const int* cslab, const double2* coef, size_t coef_slab,
+                            const double* scale, double2* F, size_t F_slab, int ldf, int col, cudaStream_t st);
 cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st);
 cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStream_t st);
 cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st);
-cudaError_t st_mw_extend(int L, int n, int mwss, int ldin, int ldout, const double2* Fa, double2* X, cudaStream_t st);
-cudaError_t st_mw_pad_phase(int L, int mwss, int ldin, int ldout, const double2* Y, double2* Z, cudaStream_t st);
-cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int n, int sgn_out, int m_end, int fold, const int* m_lo,
-                            const double* wq, const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st);
+cudaError_t st_mw_extend(int L, int nslab, const int* slab_n, int mwss, int ldin, int ldout, const double2* Fa, size_t Fa_slab, double2* X,
+                         size_t X_slab, cudaStream_t st);
+cudaError_t st_mw_pad_phase(int L, int nslab, int mwss, int ldin, int ldout, const double2* Y, size_t Y_slab, double2* Z, size_t Z_slab,
+                            cudaStream_t st);
+cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int mmin, int npass, const double* wq, const double2* U,
+                            size_t U_slab, const ThetaPass* passes, int th_lo, int th_hi, cudaStream_t st);
 cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
                                   const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st);
 cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
                             cudaStream_t st);
-cudaError_t st_finalize_forward(int L, int Lp, int n, int real, const double* scale, const double2* H, double2* coef, cudaStream_t st);
+cudaError_t st_finalize_forward(int L, int Lp, int nslab, const int* slab_n, const int* cslab, int real, const double* scale, const double2* H,
+                                size_t H_slab, double2* coef, size_t coef_slab, cudaStream_t st);
 cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* src, double2* dst, cudaStream_t st);
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st);
 

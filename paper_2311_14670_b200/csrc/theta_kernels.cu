@@ -81,7 +81,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 
     if (w >= NW) {
         // ---------------------------------------------------------------- auxiliary warps: TMA producer + reducers
-        reg_dealloc_aux<(FOLD && NC == 2) ? 64 : (NC == 1 && !FOLD) ? 40 : 48>();
+        reg_dealloc_aux<(FOLD && NC == 2) ? 56 : 40>();
         const int at = tid - NW * 32;                 // 0..127: owns output pairs (re, im) at, at+128, ... of the NOUT per step
         constexpr int NOUT = NTH * NC, NQ = (NOUT + NAUX * 32 - 1) / (NAUX * 32);
         constexpr uint32_t op_bytes = TL * ROWD * sizeof(double), lam_bytes = NTH * sizeof(double);
@@ -173,7 +173,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         }
         return;
     }
-    reg_alloc_compute<(FOLD && NC == 2) ? 224 : 232>();
+    reg_alloc_compute<(FOLD && NC == 2) ? 56 : 40>();
 
     // -------------------------------------------------------------------- compute warps
     // degrees of this warp: la + DS j, j < RL (FOLD: one parity per warp, DS = 2)
@@ -329,7 +329,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
 
     if (w >= NW) {
         // ---------------------------------------------------------------- auxiliary warps
-        reg_dealloc_aux();
+        reg_dealloc_aux<(NC == 1 && RT == 16) ? 56 : 40>();
         const int at = tid - NW * 32;
         constexpr int NOUT = TLB * NC, NQ = (NOUT + NAUX * 32 - 1) / (NAUX * 32);
         constexpr uint32_t wt_bytes = NTB * NCW * sizeof(double2), lam_bytes = NTB * sizeof(double);
@@ -424,7 +424,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         }
         return;
     }
-    reg_alloc_compute();
+    reg_alloc_compute<(NC == 1 && RT == 16) ? 56 : 40>();
 
     // -------------------------------------------------------------------- compute warps
     // state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
