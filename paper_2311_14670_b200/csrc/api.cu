@@ -771,6 +771,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         stage(P, CAT_HOT, st);
         F32Args a{};
         a.L = L; a.Lp = P->Lp; a.nth = P->inv.nth; a.ntp = P->inv.ntp; a.NB = P->NB; a.ldout = P->F_ld;
+        a.fold0 = P->fold0i; a.nfull = P->inv.nfull;
         a.ab = P->ab32; a.lam32 = P->lam32_inv; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
         a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F;
         CK(launch_theta_f32(a, false, NC, st));
@@ -1042,7 +1043,7 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
         bool isym = on;
         if (opts & SHT_OPT_INVSYM) isym = true;
         if (opts & (SHT_OPT_NO_INVSYM | SHT_OPT_FOLD_OFF)) isym = false;
-        isym = isym && sampling == SHT_MW && batch == 1 && dtype == SHT_F64 && !helper && !(opts & SHT_OPT_ADJOINT);
+        isym = isym && sampling == SHT_MW && batch == 1 && !helper && !(opts & SHT_OPT_ADJOINT);      // (fp64 and fp32 plans)
         if (isym) { P->invsym = 1; P->fold0i = 1; rings_mid(P->inv, L); north_only(P->inv); }
         // the rings of the map are symmetric about the equator on every sampling but MW: fold the inverse too.  DH has 2L rings, so
         // its folded inverse does the work of an MW inverse; it is folded whatever the size.

@@ -80,7 +80,8 @@ cudaError_t launch_theta_mma(const MmaArgs& a, bool forward, cudaStream_t st);
 // ---- fp32 variant (theta_f32.cu): n = 0, MW sampling, one map ------------------------------------------------------------
 struct F32Args {
     int L, Lp, nth, ntp, NB, ldout;
-    int fold0;                // forward: northern rings only, W32 rows hold the E / O sets (as theta_kernels.cu FOLD)
+    int fold0;                // northern rings only.  forward: W32 rows hold the E / O sets; inverse: both rings of a mirror pair are written
+    int nfull;                // folded ring sets: ring th mirrors ring nfull-1-th
     const float2* ab;         // [m][Lp] {A_m(l) = a_{m-1}(l), B_m(l) = a_{m-1}(l)/a_m(l)} (Eq. 25-26), rows m = 0..L-1 (row 0 unused: zeros)
     const float* lam32;       // fp32 copy of the lambda table of the n = 0 pass, row m + 1 (layout of ThetaPass::lam with m_end = 0)
     const float* st_val;      // [Lp][ntp] Eq. 27 start values, windowed: true value = st_val * 2^(-48 st_k)

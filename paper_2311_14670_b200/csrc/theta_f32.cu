@@ -60,20 +60,23 @@ __device__ __forceinline__ void window_check_f(float (&cur)[NI], float (&prev)[N
 // inverse, Eq. 33:  F[row(+-m)][theta] += sum_l G[m][l][c] d^l_{m,0}(theta)
 // warp w: degrees l0 + 8 w + j (j < 8); lane: rings th0 + lane + 32 i (i < 4)
 // =============================================================================================================
-template <int NC>
+// FOLD (rings symmetric about the equator, northern half recursed): d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta).  The
+// degrees of a warp all have one parity (warp w: l0 + 16 (w/2) + (w%2) + 2j), the reducers add the even-degree and the odd-degree warps
+// apart (E0, E1) and write F_m(theta) = E0 + E1 and F_m(pi - theta) = (-1)^m (E0 - E1), as the fp64 kernel does.
+template <int NC, bool FOLD>
 __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
-    constexpr int RL = 8, RT = 4, NI = RL * RT;
+    constexpr int RL = 8, RT = 4, NI = RL * RT, DS = FOLD ? 2 : 1;
     __shared__ float2 s_ab[2][TLF];
     __shared__ float2 s_g[2][TLF * NC];
     __shared__ float s_lam[2][NTF];
-    __shared__ float2 s_part[NWF][NC][NTF];
+    __shared__ float2 s_part[2][NWF][NC][NTF];       // double-buffered: the sums of step m are reduced while step m-1 is computed
     const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;      // heavy tiles first
     const int l0 = lt * TLF, th0 = tt * NTF;
     if (l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int mtop = min(l0 + TLF - 1, A.L - 1);
-    const int la = l0 + w * RL;
+    const int la = FOLD ? l0 + 2 * RL * (w >> 1) + (w & 1) : l0 + w * RL;         // degrees of this warp: la + DS j
 
     // operand rows of step m, one element per thread, copied global -> shared asynchronously (cp.async): the copy of step m-1
     // is in flight while step m is computed and is awaited just before the block barrier
@@ -93,14 +96,38 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
     __pipeline_wait_prior(0);
     __syncthreads();
 
+    // cross-warp sum of the partial sums of step m (buffer pb) and RED.ADD to the output rows
+    auto reduce = [&](const int m, const int pb) {
+        for (int o = tid; o < NC * NTF; o += NWF * 32) {
+            const int c = o / NTF, t = o % NTF, th = th0 + t;
+            float ex = 0.f, ey = 0.f, ox = 0.f, oy = 0.f;
+#pragma unroll
+            for (int ww = 0; ww < NWF; ++ww) {
+                const float2 v = s_part[pb][ww][c][t];
+                if (FOLD && (ww & 1)) { ox += v.x; oy += v.y; } else { ex += v.x; ey += v.y; }
+            }
+            if (th < A.nth && !(c == 1 && m == 0)) {
+                const int m_out = c == 1 ? -m : m;
+                const int row = m_out < 0 ? m_out + A.NB : m_out;
+                double* op = reinterpret_cast<double*>(A.out) + ((size_t)row * A.ldout + th) * 2;
+                red_add_f64(op, (double)(ex + ox)); red_add_f64(op + 1, (double)(ey + oy));
+                const int tm = A.nfull - 1 - th;
+                if (FOLD && tm != th) {
+                    const float sg = (m & 1) ? -1.f : 1.f;
+                    double* os = reinterpret_cast<double*>(A.out) + ((size_t)row * A.ldout + tm) * 2;
+                    red_add_f64(os, (double)(sg * (ex - ox))); red_add_f64(os + 1, (double)(sg * (ey - oy)));
+                }
+            }
+        }
+    };
     // one step: project d_m, then advance to d_{m-1}.  `ca` holds d_m, `cb` holds d_{m+1} on entry and d_{m-1} on exit.
     auto step = [&](const int m, const int buf, float (&ca)[NI], float (&cb)[NI]) {
         if (m > 0) load_ops(m - 1, buf ^ 1);
-        bool mine = m <= la + RL - 1 && la < A.L;   // this warp has started degrees
+        bool mine = m <= la + DS * (RL - 1) && la < A.L;   // this warp has started degrees
         if (mine && m >= la) {                      // the degree l == m starts (warp-uniform)
 #pragma unroll
             for (int j = 0; j < RL; ++j)
-                if (m == la + j) {
+                if (m == la + DS * j) {
 #pragma unroll
                     for (int i = 0; i < RT; ++i) {
                         const size_t o = (size_t)m * A.ntp + th0 + lane + 32 * i;
@@ -120,10 +147,11 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
             for (int i = 0; i < RT; ++i) lam[i] = s_lam[buf][lane + 32 * i];
 #pragma unroll
             for (int j = 0; j < RL; ++j) {
-                const float2 ab = s_ab[buf][w * RL + j];
+                const int dj = la - l0 + DS * j;
+                const float2 ab = s_ab[buf][dj];
                 float cf[2 * NC];
 #pragma unroll
-                for (int c = 0; c < NC; ++c) { const float2 t = s_g[buf][(w * RL + j) * NC + c]; cf[2 * c] = t.x; cf[2 * c + 1] = t.y; }
+                for (int c = 0; c < NC; ++c) { const float2 t = s_g[buf][dj * NC + c]; cf[2 * c] = t.x; cf[2 * c + 1] = t.y; }
 #pragma unroll
                 for (int i = 0; i < RT; ++i) {
                     const float e = ca[j * RT + i];
@@ -134,25 +162,14 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
             }
             if (kp.any_nonzero()) window_check_f<NI>(cb, ca, kp);
         }
+        const int pb = buf;                         // partial-sum buffer of this step (alternates with the operand buffer)
 #pragma unroll
         for (int i = 0; i < RT; ++i)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) s_part[w][c][lane + 32 * i] = make_float2(acc[i][2 * c], acc[i][2 * c + 1]);
+            for (int c = 0; c < NC; ++c) s_part[pb][w][c][lane + 32 * i] = make_float2(acc[i][2 * c], acc[i][2 * c + 1]);
         __pipeline_wait_prior(0);
-        __syncthreads();
-        for (int o = tid; o < NC * NTF; o += NWF * 32) {
-            const int c = o / NTF, t = o % NTF, th = th0 + t;
-            float sx = 0.f, sy = 0.f;
-#pragma unroll
-            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += v.x; sy += v.y; }
-            if (th < A.nth && !(c == 1 && m == 0)) {
-                const int m_out = c == 1 ? -m : m;
-                const int row = m_out < 0 ? m_out + A.NB : m_out;
-                double* op = reinterpret_cast<double*>(A.out) + ((size_t)row * A.ldout + th) * 2;
-                red_add_f64(op, (double)sx); red_add_f64(op + 1, (double)sy);
-            }
-        }
-        __syncthreads();
+        __syncthreads();                            // the only block barrier of the step: partial sums of m and operands of m-1 are visible;
+        reduce(m, pb);                              // buffer pb is next written two steps from now, after the barrier of step m-1
     };
     for (int m = mtop; m >= 0; m -= 2) {
         step(m, (mtop - m) & 1, cur, prev);
@@ -162,9 +179,10 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
 
 // =============================================================================================================
 // forward, Eq. 30:  H[+-m + L-1][l] += sum_theta W[m][theta][c] d^l_{m,0}(theta)
-// warp w: rings th0 + 16 w + i (i < 16); lane: degrees l0 + 2 lane + r (r < 2)
-// FOLD: northern rings only; W32 rows hold E = q (F_m(theta) + F_m(pi - theta)) and O = q (F_m(theta) - F_m(pi - theta)); the degree
-// with l+m even contracts with E, the other one with O (d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta)).
+// warp w: rings th0 + 16 w + i (i < 16); lane: degrees l0 + lane + 32 r (r < 2)
+// FOLD: northern rings only; W32 rows hold E = q (F_m(theta) + F_m(pi - theta)) and O = q (F_m(theta) - F_m(pi - theta)); a degree
+// with l+m even contracts with E, one with l+m odd with O (d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta)).  A thread's two
+// degrees share their parity, which alternates with the lane: one load with two addresses serves both (as in theta_kernels.cu).
 // =============================================================================================================
 template <int NC, bool FOLD>
 __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
@@ -172,7 +190,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
     __shared__ float2 s_ab[2][TLF];
     __shared__ float2 s_w[2][NTF * NCW];
     __shared__ float s_lam[2][NTF];
-    __shared__ float2 s_part[NWF][NC][TLF];
+    __shared__ float2 s_part[2][NWF][NC][TLF];
     const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
     const int l0 = lt * TLF, th0 = tt * NTF;
@@ -195,7 +213,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
     for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
     int lr[RL];
 #pragma unroll
-    for (int r = 0; r < RL; ++r) lr[r] = l0 + RL * lane + r;
+    for (int r = 0; r < RL; ++r) lr[r] = l0 + lane + 32 * r;
     load_ops(mtop, 0);
     __pipeline_wait_prior(0);
     __syncthreads();
@@ -219,19 +237,19 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
             for (int c = 0; c < 2 * NC; ++c) acc[r][c] = 0.f;
         float2 ab[RL];
 #pragma unroll
-        for (int r = 0; r < RL; ++r) ab[r] = s_ab[buf][RL * lane + r];
-        const int par = (l0 + m) & 1;                 // FOLD: degree r uses set (par ^ r): 0 = E, 1 = O (warp-uniform)
+        for (int r = 0; r < RL; ++r) ab[r] = s_ab[buf][lane + 32 * r];
+        const int set = FOLD ? ((l0 + m + lane) & 1) * NC : 0;      // FOLD: 0 = E (l+m even), NC = O; per lane parity, same for both degrees
 #pragma unroll
         for (int i = 0; i < RT; ++i) {
             const float lam = s_lam[buf][w * RT + i];
+            float wv[2 * NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const float2 t = s_w[buf][(w * RT + i) * NCW + set + c];
+                wv[2 * c] = t.x; wv[2 * c + 1] = t.y;
+            }
 #pragma unroll
             for (int r = 0; r < RL; ++r) {
-                float wv[2 * NC];
-#pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    const float2 t = s_w[buf][(w * RT + i) * NCW + (FOLD ? ((par ^ r) & 1) * NC : 0) + c];
-                    wv[2 * c] = t.x; wv[2 * c + 1] = t.y;
-                }
                 const float e = ca[r * RT + i];
 #pragma unroll
                 for (int c = 0; c < 2 * NC; ++c) acc[r][c] = fmaf(e, wv[c], acc[r][c]);
@@ -242,21 +260,20 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
 #pragma unroll
         for (int r = 0; r < RL; ++r)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) s_part[w][c][RL * lane + r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
+            for (int c = 0; c < NC; ++c) s_part[buf][w][c][lane + 32 * r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
         __pipeline_wait_prior(0);
-        __syncthreads();
+        __syncthreads();                            // the only block barrier of the step (partial sums double-buffered, see the inverse)
         for (int o = tid; o < NC * TLF; o += NWF * 32) {
             const int c = o / TLF, t = o % TLF, l = l0 + t;
             float sx = 0.f, sy = 0.f;
 #pragma unroll
-            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[ww][c][t]; sx += v.x; sy += v.y; }
+            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[buf][ww][c][t]; sx += v.x; sy += v.y; }
             if (l < A.L && l >= m && !(c == 1 && m == 0)) {
                 const int m_out = c == 1 ? -m : m;
                 double* op = reinterpret_cast<double*>(A.out) + ((size_t)(m_out + A.L - 1) * A.Lp + l) * 2;
                 red_add_f64(op, (double)sx); red_add_f64(op + 1, (double)sy);
             }
         }
-        __syncthreads();
     };
     for (int m = mtop; m >= 0; m -= 2) {
         step(m, (mtop - m) & 1, cur, prev);
@@ -274,9 +291,12 @@ cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_
     } else if (forward) {
         if (NC == 2) theta_forward_f32<2, false><<<grid, NWF * 32, 0, st>>>(a);
         else theta_forward_f32<1, false><<<grid, NWF * 32, 0, st>>>(a);
+    } else if (a.fold0) {
+        if (NC == 2) theta_inverse_f32<2, true><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_inverse_f32<1, true><<<grid, NWF * 32, 0, st>>>(a);
     } else {
-        if (NC == 2) theta_inverse_f32<2><<<grid, NWF * 32, 0, st>>>(a);
-        else theta_inverse_f32<1><<<grid, NWF * 32, 0, st>>>(a);
+        if (NC == 2) theta_inverse_f32<2, false><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_inverse_f32<1, false><<<grid, NWF * 32, 0, st>>>(a);
     }
     count_launch();
     return cudaGetLastError();

@@ -1,0 +1,113 @@
+"""Memory-safety and race evidence that does not need compute-sanitizer (closed on this GPU pool: see profiles/r2_sanitizer.md).
+
+* Guard bands: the plan workspace and every public input / output array live INSIDE larger buffers whose margins hold a sentinel
+  pattern; after plan creation and a forward + inverse transform the margins must be bit-identical (no out-of-bounds write of any
+  kernel, bulk-TMA copy, bulk reduce or cuFFT call), and the inputs unmodified.
+* Repeatability: the fused kernels hand partial sums between warps through mbarrier pipelines and recycle shared-memory slots; a race
+  there shows up as run-to-run differences far above the 1e-15 the unordered fp64 atomics allow.  Every kernel variant (P / PM, folds,
+  64- and 128-ring tiles, batched DMMA, fp32, precompute) is run 12 times on the same input and compared."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from paper_2311_14670_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+PAD = 1 << 16          # bytes of sentinel on each side
+
+
+@pytest.fixture(scope="module")
+def api():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_14670_b200 import api as A
+    return A
+
+
+def guarded(nbytes):
+    """(whole buffer, aligned inner view) with 0xA5 sentinels around the inner region"""
+    whole = torch.full((nbytes + 2 * PAD + 512,), 0xA5, dtype=torch.uint8, device="cuda")
+    off = PAD + (-(whole.data_ptr() + PAD)) % 256
+    return whole, whole[off:off + nbytes], off
+
+
+def margins_intact(whole, off, nbytes):
+    return bool((whole[:off] == 0xA5).all()) and bool((whole[off + nbytes:] == 0xA5).all())
+
+
+CASES = [dict(L=33, spin=0), dict(L=64, spin=2), dict(L=130, spin=-1), dict(L=200, spin=0, fold=True), dict(L=96, spin=0, reality=True),
+         dict(L=130, spin=0, invsym=True), dict(L=48, spin=1, sampling="mwss"), dict(L=40, spin=0, sampling="dh"), dict(L=65, spin=2, sampling="gl"),
+         dict(L=24, spin=0, sampling="hp", nside=8, reality=True), dict(L=40, spin=2, sampling="hp", nside=16), dict(L=20, N=4),
+         dict(L=48, spin=0, batch=5), dict(L=64, spin=0, dtype="f32"), dict(L=72, spin=1, precompute=True), dict(L=50, spin=2, adjoint=True)]
+
+
+@pytest.mark.parametrize("case", CASES, ids=lambda c: "-".join(f"{k}{v}" for k, v in c.items()))
+def test_nothing_is_written_outside_the_workspace_or_the_outputs(api, case):
+    from paper_2311_14670_b200._lib import check, lib
+    kw = dict(case)
+    samp = {"mw": api.MW, "mwss": api.MWSS, "dh": api.DH, "gl": api.GL, "hp": api.HEALPIX}[kw.pop("sampling", "mw")]
+    L = kw.pop("L")
+    P = api.Plan(L, sampling=samp, **kw)                       # sizes, dtypes and shapes from the binding ...
+    nws = P.workspace.numel()
+    ws_whole, ws, ws_off = guarded(nws)
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    check(lib().sht_plan_set_workspace(P._h, C.c_void_p(ws.data_ptr()), nws, st))    # ... but the workspace inside a guarded buffer
+    P.workspace = ws
+    rng = np.random.default_rng(1)
+
+    def rand(shape, dtype):
+        real = not dtype.is_complex
+        a = rng.standard_normal(shape) if real else rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+        return torch.from_numpy(a).to(dtype)
+
+    def inside(shape, dtype, src=None):
+        n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+        whole, inner, off = guarded(n)
+        view = inner.view(dtype).view(shape)
+        if src is not None:
+            view.copy_(src)
+        return whole, view, off, n
+
+    c_in = rand(P.coef_shape, P.coef_dtype)
+    f_in = rand(P.map_shape, P.map_dtype)
+    bufs = [inside(P.coef_shape, P.coef_dtype, c_in), inside(P.map_shape, P.map_dtype), inside(P.map_shape, P.map_dtype, f_in), inside(P.coef_shape, P.coef_dtype)]
+    P.inverse(bufs[0][1], out=bufs[1][1])
+    P.forward(bufs[2][1], out=bufs[3][1])
+    if case.get("adjoint"):
+        P.forward_adjoint(bufs[0][1], out=bufs[1][1])
+        P.inverse_adjoint(bufs[2][1], out=bufs[3][1])
+    torch.cuda.synchronize()
+    assert margins_intact(ws_whole, ws_off, nws), "write outside the workspace"
+    for whole, view, off, n in bufs:
+        assert margins_intact(whole, off, n), "write outside a public array"
+    assert torch.equal(bufs[0][1].cpu(), c_in) and torch.equal(bufs[2][1].cpu(), f_in), "an input was modified"
+    assert torch.isfinite(torch.view_as_real(bufs[3][1]) if bufs[3][1].is_complex() else bufs[3][1]).all()
+
+
+REPEAT = [dict(L=130, spin=0), dict(L=130, spin=2), dict(L=257, spin=0, fold=True), dict(L=257, spin=0, fold=True, tile=64), dict(L=200, spin=0, invsym=True),
+          dict(L=200, spin=0, reality=True, invsym=True), dict(L=130, spin=0, sampling="hp", nside=64, reality=True, fold=True), dict(L=40, N=5),
+          dict(L=130, spin=0, batch=9), dict(L=130, spin=0, dtype="f32", fold=True, invsym=True), dict(L=100, spin=1, precompute=True)]
+
+
+@pytest.mark.parametrize("case", REPEAT, ids=lambda c: "-".join(f"{k}{v}" for k, v in c.items()))
+def test_repeated_runs_agree_to_rounding(api, case):
+    kw = dict(case)
+    samp = {"mw": api.MW, "hp": api.HEALPIX}[kw.pop("sampling", "mw")]
+    L = kw.pop("L")
+    P = api.Plan(L, sampling=samp, **kw)
+    rng = np.random.default_rng(2)
+    real_c = not P.coef_dtype.is_complex
+    c = torch.from_numpy(rng.standard_normal(P.coef_shape) + 1j * rng.standard_normal(P.coef_shape)).to(P.coef_dtype).cuda()
+    if kw.get("reality"):
+        flm = synth.random_flm(L, 0, seed=3, real=True)
+        c = torch.from_numpy(flm).to(P.coef_dtype).cuda()
+    g = rng.standard_normal(P.map_shape) if not P.map_dtype.is_complex else rng.standard_normal(P.map_shape) + 1j * rng.standard_normal(P.map_shape)
+    g = torch.from_numpy(g).to(P.map_dtype).cuda()
+    tol = 1e-5 if kw.get("dtype") == "f32" else 1e-13
+    f0, c0 = P.inverse(c).clone(), P.forward(g).clone()
+    for _ in range(12):
+        f1, c1 = P.inverse(c), P.forward(g)
+        assert float((f1 - f0).abs().max() / f0.abs().max()) < tol
+        assert float((c1 - c0).abs().max() / c0.abs().max()) < tol
+    del real_c
