@@ -45,8 +45,25 @@ def test_status_strings_and_argument_validation(lib):
     assert lib.sht_plan_s2(C.byref(h), 8, 2, 0, 0, 0, 1) == 2          # fp32 is built for spin 0 / MW / one map only
     assert lib.sht_plan_s2(C.byref(h), 8, 0, 0, 0, 0, 7) == 1          # unknown dtype
     assert lib.sht_plan_so3(C.byref(h), 8, 9, 0) == 1                  # N > L
+    assert lib.sht_plan_s2(C.byref(h), 8, 0, 9, 0, 0, 0) == 1          # sampling codes are 0..4 (MW, HEALPix, MWSS, DH, GL)
+    assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 0, 1, 1 | 2) == 1      # SHT_OPT_FOLD_ON with SHT_OPT_FOLD_OFF
+    assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 0, 1, 4 | 128) == 1    # SHT_OPT_INVSYM with SHT_OPT_NO_INVSYM
+    assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 1, 1, 64) == 2         # precompute is fp64 only
+    assert lib.sht_plan_set_shard(None, 0, 1) == 1
+    assert lib.sht_peak(7, 10, None, None, None) == 1
     assert lib.sht_plan_workspace_bytes(None) == 0
     assert lib.s2_forward_plan(None, None, None, None) == 1
+
+
+def test_band_limit_beyond_the_window_counter_range_is_refused(lib):
+    """Eq. 27 start values below 2^-122900 do not fit the one-byte window counter; they must never be dropped silently.
+    The range check runs on the host before any CUDA call, so it is testable without a GPU: MW plans are refused from L ~ 9100."""
+    h = C.c_void_p()
+    for L in (9300, 12000, 16384):
+        assert lib.sht_plan_s2(C.byref(h), L, 0, 0, 0, 0, 0) == 2, L                # SHT_EUNSUPPORTED
+        assert b"start values" in lib.sht_last_error()
+    assert lib.sht_plan_s2(C.byref(h), 9300, 2, 3, 0, 0, 0) == 2                    # DH: same rings as the MW quadrature
+    assert lib.sht_plan_so3(C.byref(h), 9300, 4, 0) == 2
 
 
 def test_no_cpu_fallback_without_gpu(lib):

@@ -135,3 +135,24 @@ def test_config5a_mw_L8192_spin0(api, orc):
     got32 = P32.forward(dev(g.astype(np.complex64))).cpu().numpy()
     for m, col in zip(ms, want):
         assert rel(got32[:, m + L - 1], col, sc) < 1e-4, m
+
+
+def test_near_the_band_limit_ceiling_L9000(api, orc):
+    """the one-byte window counter of the Eq. 27 start values reaches 2^-122900; on MW that is exhausted near L = 9100 (plans
+    beyond are refused, tests/test_abi.py).  Just below the ceiling the rings next to the poles use window counters up to ~250 of 254:
+    sampled polar rings of the inverse against the oracle, and the exact round trip."""
+    L = 9000
+    tol = TOL * L / 1024
+    flm = synth.random_flm(L, 0, seed=5, sigma=synth.SIGMA_RED)
+    P = api.Plan(L, 0)
+    d = dev(flm)
+    f = P.inverse(d)
+    rings = np.array([0, 1, 2, L - 3, L - 2, L - 1])
+    rows = orc.s2_inverse_rings(L, 0, orc.MW, flm, rings)
+    scale = max(np.abs(r).max() for r in rows)
+    for r, row in zip(rings, rows):
+        assert rel(f[int(r)].cpu().numpy(), row, scale) < tol, r
+    back = P.forward(f)
+    err = float((back - d).abs().max() / d.abs().max())
+    print(f"L=9000 round trip max rel err {err:.3e}")
+    assert err < tol
