@@ -131,7 +131,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                 bool any = false;
 #pragma unroll
                 for (int ww = 0; ww < NW; ++ww) {
+#ifdef SHT_EXP_NOREDUCE
+                    if (0) {
+#else
                     if ((actb[ww] >> h) & 1) {
+#endif
                         any = true;
                         constexpr int e = 0;
                         const int es = FOLD ? (ww & 1) : e;       // FOLD: warp ww carries degrees of parity ww & 1
@@ -145,7 +149,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                             }
                     }
                 }
+#ifdef SHT_EXP_NORED
+                if (any && v[0][0].x == 12345.678) {
+#else
                 if (any) {
+#endif
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
                         if (valid[q] && m >= mlo[q] && !(neg[q] && m == 0)) {
@@ -174,6 +182,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         return;
     }
     reg_alloc_compute<(FOLD && NC == 2) ? 56 : 40>();
+#ifdef SHT_EXP_STAGGER
+    if (w >= NW / 2) __nanosleep(SHT_EXP_STAGGER);
+#endif
 
     // -------------------------------------------------------------------- compute warps
     // degrees of this warp: la + DS j, j < RL (FOLD: one parity per warp, DS = 2)
@@ -425,6 +436,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         return;
     }
     reg_alloc_compute<(NC == 1 && RT == 16) ? 56 : 40>();
+#ifdef SHT_EXP_STAGGER
+    if (w >= NW / 2) __nanosleep(SHT_EXP_STAGGER);
+#endif
 
     // -------------------------------------------------------------------- compute warps
     // state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
