@@ -69,8 +69,12 @@ enum {
                                      24 L^3 bytes on MW) -- and the theta steps become plain weighted sums over the stored table
                                      (HBM-bound).  Pays at L <= 512, where the on-the-fly kernels are bound by the latency of their L
                                      sequential recursion steps.  Single-map fp64 S^2 plans; the folds are off. */
-    SHT_OPT_ADJOINT  = 1u << 5    /* also build what the adjoint entry points need (complex fp64 single-map plans; MW / MWSS plans then
+    SHT_OPT_ADJOINT  = 1u << 5,   /* also build what the adjoint entry points need (complex fp64 single-map plans; MW / MWSS plans then
                                      carry the tables of two more ring sets: about twice the workspace) */
+    SHT_OPT_NO_PAIR  = 1u << 8    /* MW / MWSS: the theta-direction FFTs of the forward upsampling and of the symmetric-ring
+                                     inverse carry TWO orders m, m+1 per column by default (their extensions to the theta circle are one even
+                                     and one odd function, separated afterwards: half the FFT work); this flag keeps one order
+                                     per column */
 };
 enum { SHT_PEAK_DFMA = 0, SHT_PEAK_DMMA = 1, SHT_PEAK_FFMA = 2 };   /* sht_peak kinds */
 

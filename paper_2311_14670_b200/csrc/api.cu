@@ -101,6 +101,8 @@ struct sht_plan {
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     bool upsampled = false;    // MW / MWSS: the forward transform extends F_m to the theta circle and upsamples to the quadrature rings
+    int pair = 0;              // MW / MWSS: the theta-circle FFTs carry two orders m per column (staging.cu u_get): prow = L rows instead of NB
+    int prow = 0;              // rows of the theta-circle arrays X / Z the upsampling (and the symmetric-ring resampling) works on
     int fold0 = 0;             // spin-0 S^2 plans: the forward recursion runs on the northern quadrature rings only
     bool precomp = false;      // SHT_OPT_PRECOMPUTE: stored d-function tables (precompute.cu, Sec. 4.3)
     int shard_rank = 0, shard_n = 1;   // ring shard (sht_plan_set_shard): this plan serves share shard_rank of shard_n of the kernel rings
@@ -306,6 +308,7 @@ void plan_dims(sht_plan* P) {
         default: P->NB = 2 * L - 1; P->nrmap = L; break;         // MW, GL; HEALPix keeps 2L-1 "bins" as its F-row convention
     }
     P->Tcirc = P->NB;
+    P->prow = P->pair ? L : P->NB;
     P->col0 = P->inv.pole_n ? 1 : 0;
     if (P->sampling == SHT_HEALPIX) {
         P->nrmap = 4 * P->nside - 1;
@@ -483,15 +486,15 @@ sht_status make_fft_plans(sht_plan* P) {
         // theta FFTs of the forward upsampling: length Tcirc on the extended samples, length 4L onto the quadrature rings
         int nt[1] = {P->Tcirc};
         CF(cufftCreate(&P->fft_th1)); CF(cufftSetAutoAllocation(P->fft_th1, 0));
-        CF(cufftMakePlanMany(P->fft_th1, 1, nt, nt, 1, P->Tcirc, nt, 1, P->Tcirc, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th1] = (double)P->Tcirc * NB * P->nslab; ws = w > ws ? w : ws;
+        CF(cufftMakePlanMany(P->fft_th1, 1, nt, nt, 1, P->Tcirc, nt, 1, P->Tcirc, CUFFT_Z2Z, P->prow * P->nslab, &w)); P->fft_elems[P->fft_th1] = (double)P->Tcirc * P->prow * P->nslab; ws = w > ws ? w : ws;
         int n2[1] = {4 * L};
         CF(cufftCreate(&P->fft_th2)); CF(cufftSetAutoAllocation(P->fft_th2, 0));
-        CF(cufftMakePlanMany(P->fft_th2, 1, n2, n2, 1, 4 * L, n2, 1, 4 * L, CUFFT_Z2Z, NB * P->nslab, &w)); P->fft_elems[P->fft_th2] = 4.0 * L * NB * P->nslab; ws = w > ws ? w : ws;
+        CF(cufftMakePlanMany(P->fft_th2, 1, n2, n2, 1, 4 * L, n2, 1, 4 * L, CUFFT_Z2Z, P->prow * P->nslab, &w)); P->fft_elems[P->fft_th2] = 4.0 * L * P->prow * P->nslab; ws = w > ws ? w : ws;
     }
     if (P->invsym) {
         int n4[1] = {2 * L};
         CF(cufftCreate(&P->fft_sym)); CF(cufftSetAutoAllocation(P->fft_sym, 0));
-        CF(cufftMakePlanMany(P->fft_sym, 1, n4, n4, 1, 2 * L, n4, 1, 2 * L, CUFFT_Z2Z, NB, &w)); P->fft_elems[P->fft_sym] = 2.0 * L * NB; ws = w > ws ? w : ws;
+        CF(cufftMakePlanMany(P->fft_sym, 1, n4, n4, 1, 2 * L, n4, 1, 2 * L, CUFFT_Z2Z, P->prow, &w)); P->fft_elems[P->fft_sym] = 2.0 * L * P->prow; ws = w > ws ? w : ws;
     }
     if (P->kind == 1) {
         int n3[1] = {2 * P->N - 1};
@@ -798,7 +801,8 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
     return SHT_OK;
 }
 // U: [slab][bin][ldu] samples of F_m on the forward ring set (weights not yet applied).  Leaves H complete.
-sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int ldu, cudaStream_t st) {
+// pair != 0: U is the paired output of mw_upsample (two orders per row, staging.cu u_get).
+sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int ldu, cudaStream_t st, int pair = 0) {
     const int L = P->L;
     stage(P, CAT_STAGE, st);
     if (P->batch > 1) {
@@ -807,13 +811,13 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
             auto& ph = P->pfwd[i];
             const size_t rows = (size_t)(L - ph.p.m_end);
             if (P->fold0) {
-                CK(st_weight_split_batch_fold0(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, ph.mode == 0 ? 2 : 1, P->batch,
+                CK(st_weight_split_batch_fold0(L, P->NB, ldu, pair, U_slab, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, ph.mode == 0 ? 2 : 1, P->batch,
                                                P->ncg_fwd, ph.p.m_end, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
                                                rows * P->fwd.ntp * SHT_MMA_ROWF, st));
                 CS(zero_async(ph.p.out, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
                 continue;
             }
-            CK(st_weight_split_batch(L, P->NB, ldu, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, P->slab_n[0],
+            CK(st_weight_split_batch(L, P->NB, ldu, pair, U_slab, P->fwd.nth, P->fwd.ntp, ph.mode == 0 ? 2 : 1, P->batch, P->ncg_fwd, P->slab_n[0],
                                      ph.p.sgn_out, ph.p.m_end, ph.p.fold, ph.p.m_lo, P->fwd.wq, ph.p.lam, U, const_cast<double*>(ph.p.in),
                                      rows * P->fwd.ntp * SHT_MMA_ROW, st));
             CS(zero_async(ph.p.out, sizeof(double) * P->ncg_fwd * rows * P->Lp * SHT_MMA_NCOL, st));
@@ -839,8 +843,8 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         auto& ph = P->pfwd[0];
         const int NC = ph.mode == 0 ? 2 : 1;
         float2* W32 = reinterpret_cast<float2*>(const_cast<double*>(ph.p.in));
-        if (P->fold0) CK(st_weight_split_f32_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, P->fwd.wq, U, W32, st));
-        else CK(st_weight_split_f32(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, W32, st));
+        if (P->fold0) CK(st_weight_split_f32_fold0(L, P->NB, ldu, pair, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, P->fwd.wq, U, W32, st));
+        else CK(st_weight_split_f32(L, P->NB, ldu, pair, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, W32, st));
         CS(zero_async(P->H, sizeof(double2) * P->H_slab, st));
         stage(P, CAT_HOT, st);
         F32Args a{};
@@ -855,12 +859,12 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
     if (P->fold0) {         // n = 0 on the northern rings: E / O operand sets (one pass)
         for (auto& ph : P->pfwd) {
             const int NC = ph.mode == 0 ? 2 : 1;
-            CK(st_weight_split_fold0(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, ph.p.m_end, P->fwd.wq, U + U_slab * ph.p.slab,
+            CK(st_weight_split_fold0(L, P->NB, ldu, pair, P->fwd.nth, P->fwd.ntp, P->fwd.nfull, NC, ph.p.m_end, P->fwd.wq, U + U_slab * ph.p.slab,
                                      reinterpret_cast<double2*>(const_cast<double*>(ph.p.in)) + (size_t)P->fwd.ntp * 2 * NC, slo, shi, st));
         }
     } else {
-        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, 2, P->mmin, P->n_fwd_pm, P->fwd.wq, U, U_slab, P->d_fwd_pm, slo, shi, st));
-        CK(st_weight_split(L, P->NB, ldu, P->fwd.nth, P->fwd.ntp, 1, P->mmin, P->n_fwd_p, P->fwd.wq, U, U_slab, P->d_fwd_p, slo, shi, st));
+        CK(st_weight_split(L, P->NB, ldu, pair, P->fwd.nth, P->fwd.ntp, 2, P->mmin, P->n_fwd_pm, P->fwd.wq, U, U_slab, P->d_fwd_pm, slo, shi, st));
+        CK(st_weight_split(L, P->NB, ldu, pair, P->fwd.nth, P->fwd.ntp, 1, P->mmin, P->n_fwd_p, P->fwd.wq, U, U_slab, P->d_fwd_p, slo, shi, st));
     }
     CS(zero_async(P->H, sizeof(double2) * P->H_slab * P->nslab, st));
     stage(P, CAT_HOT, st);
@@ -892,15 +896,16 @@ sht_status check_ready(const sht_plan* P) {
 sht_status resample_sym_to_mw(sht_plan* P, cudaStream_t st) {
     const int L = P->L, NB = P->NB;
     stage(P, CAT_STAGE, st);
-    CK(st_sym_extend(L, P->slab_n[0], P->F_ld, P->F, P->Z, st));
+    CK(st_sym_extend(L, P->slab_n[0], P->pair, P->F_ld, P->F, P->Z, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_sym, P->Z, P->Z, CUFFT_FORWARD, st));
     stage(P, CAT_STAGE, st);
-    CK(st_sym_rebin(L, P->Z, P->X, st));
+    CK(st_sym_rebin(L, P->prow, P->Z, P->X, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_INVERSE, st));
     stage(P, CAT_STAGE, st);
-    CK(st_rows_head(NB, L, NB, P->F_ld, P->X, P->F, st));
+    if (P->pair) CK(st_sym_unpair(L, P->slab_n[0], P->F_ld, P->X, P->F, st));    // two orders per column: split them by their symmetry
+    else CK(st_rows_head(NB, L, NB, P->F_ld, P->X, P->F, st));
     return SHT_OK;
 }
 
@@ -908,11 +913,13 @@ sht_status resample_sym_to_mw(sht_plan* P, cudaStream_t st) {
 sht_status mw_upsample(sht_plan* P, cudaStream_t st) {
     const int L = P->L, T2 = 4 * L, mwss = P->sampling == SHT_MWSS;
     stage(P, CAT_STAGE, st);
-    CK(st_mw_extend(L, P->nslab, P->d_slab_n, mwss, P->Ltp, P->Tcirc, P->Fa, P->Fa_slab, P->X, P->X_slab, st));
+    // (with `pair` the rows are packed: slab stride prow rows, so that one batched FFT plan serves all slabs)
+    const size_t xs = (size_t)P->prow * P->Tcirc, zs = (size_t)P->prow * T2;
+    CK(st_mw_extend(L, P->nslab, P->d_slab_n, mwss, P->pair, P->Ltp, P->Tcirc, P->Fa, P->Fa_slab, P->X, xs, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_FORWARD, st));
     stage(P, CAT_STAGE, st);
-    CK(st_mw_pad_phase(L, P->nslab, mwss, P->Tcirc, T2, P->X, P->X_slab, P->Z, P->Z_slab, st));
+    CK(st_mw_pad_phase(L, P->nslab, mwss, P->prow, P->Tcirc, T2, P->X, xs, P->Z, zs, st));
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_th2, P->Z, P->Z, CUFFT_INVERSE, st));
     return SHT_OK;
@@ -1051,6 +1058,9 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
             P->fold0i = 1; north_only(P->inv);
         }
     }
+    // MW / MWSS forward upsampling and the symmetric-ring resampling carry two orders per theta-circle column (staging.cu u_get); the
+    // adjoint entry points run the transposed chain on single orders, so plans that offer them keep one order per column
+    P->pair = (sampling == SHT_MW || sampling == SHT_MWSS) && !helper && !(opts & (SHT_OPT_ADJOINT | SHT_OPT_NO_PAIR));
     sht_status s = check_start_range(P);
     if (s == SHT_OK && (opts & SHT_OPT_ADJOINT) && !helper) {
         // adjoint entry points (Eq. 52 / 58): complex fp64 single-map plans
@@ -1081,6 +1091,7 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     for (int b = 0; b < P->nslab; ++b) P->slab_n.push_back(b < N ? b : b - (2 * N - 1));   // gamma-FFT bin order
     query_device(P);
     rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L);
+    P->pair = 1;
     sht_status s = check_start_range(P);
     if (s == SHT_OK) s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
@@ -1367,7 +1378,7 @@ sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream str
         CS(fft_exec(P, P->fft_phi_fwd, const_cast<double2*>(fin) + nmap * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
     if (P->upsampled) {         // MW / MWSS: extension to the theta circle + upsampling to the quadrature rings
         CS(mw_upsample(P, st));
-        CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
+        CS(run_theta_forward(P, P->Z, (size_t)P->prow * P->fwd_ld, P->fwd_ld, st, P->pair));
     } else                      // DH / GL: explicit quadrature on the rings of the map (Eq. 36 / 46)
         CS(run_theta_forward(P, P->Fa, P->Fa_slab, P->Ltp, st));
     stage(P, CAT_STAGE, st);
@@ -1516,7 +1527,7 @@ sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream s
     CS(fft_exec(P, P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD, st));   // Eq. 16 (q_Gamma in scale_fwd)
     for (int b = 0; b < P->nslab; ++b) CS(fft_exec(P, P->fft_phi_fwd, P->fn + slab * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
     CS(mw_upsample(P, st));
-    CS(run_theta_forward(P, P->Z, P->Z_slab, P->fwd_ld, st));
+    CS(run_theta_forward(P, P->Z, (size_t)P->prow * P->fwd_ld, P->fwd_ld, st, P->pair));
     stage(P, CAT_STAGE, st);
     CK(st_finalize_forward(L, P->Lp, P->nslab, P->d_slab_n, P->d_cslab, 0, P->scale_fwd, P->H, P->H_slab, (double2*)flmn, slab, st));
     stage(P, CAT_STAGE, st);

@@ -10,6 +10,21 @@ namespace {
 
 __device__ __forceinline__ double sgn_pow(int k) { return (k & 1) ? -1.0 : 1.0; }
 
+// F_m on quadrature ring ts, read from the forward ring-sample array U.
+//   pair = 0: U[bin(m)][ldin], one row per order.
+//   pair != 0 (MW / MWSS upsampling, api.cu mw_upsample): the extension of F_m to the theta circle has the reflection symmetry
+//   F_m(2pi - theta) = (-1)^{m-n} F_m(theta), which alternates with m.  Row j of U then holds the SUM of the theta-circle
+//   samples (ldin = 4L midpoints theta'_u; the mirror of u is ldin-1-u) of the orders m = 2j-(L-1) and 2j-(L-2) -- one even and one odd
+//   function, carried through the (linear) FFT upsampling as ONE column -- and either is recovered from its own symmetry:
+//   F_m(theta'_u) = (c[u] + (-1)^{m-n} c[ldin-1-u]) / 2.  Half the theta FFT work of the forward transform.
+__device__ __forceinline__ double2 u_get(const double2* __restrict__ U, int ldin, int NBin, int pair, int L, int n, int m, int ts) {
+    if (!pair) return U[(size_t)(m < 0 ? m + NBin : m) * ldin + ts];
+    const double2* row = U + (size_t)((m + L - 1) >> 1) * ldin;
+    const double2 a = row[ts], b = row[ldin - 1 - ts];
+    const double s = ((m - n) & 1) ? -0.5 : 0.5;
+    return make_double2(fma(s, b.x, 0.5 * a.x), fma(s, b.y, 0.5 * a.y));
+}
+
 // ---- double-double helpers for the start-value product -------------------------------------------------------
 struct dd { double hi, lo; };
 __device__ __forceinline__ dd dd_mul(dd a, dd b) {
@@ -243,21 +258,33 @@ __global__ void k_complex_to_real(size_t n, const double2* __restrict__ in, doub
 // Rings AT a pole hold one value of a spin-s function (n = -s): at theta = pi only the order m = -n survives (Eq. 29),
 // at theta = 0 only m = n (Eq. 28).  The samples of those rings are projected onto that component (F_m := 0 for the other m), which
 // makes the transform well defined on arbitrary arrays (R21; include/b200sht.h, s2_forward).
-__global__ void k_mw_extend(int L, const int* __restrict__ slab_n, int mwss, int ldin, int ldout, const double2* __restrict__ Fa_base,
+__device__ __forceinline__ double2 mw_ext_value(int L, int n, int mwss, int ldin, const double2* __restrict__ Fa, int m, int t) {
+    const int T = mwss ? 2 * L : 2 * L - 1, tpole = mwss ? L : L - 1;
+    const int b = m < 0 ? m + T : m;
+    double2 v;
+    if (t == tpole) { v = Fa[(size_t)b * ldin + t]; if (m != -n) v = make_double2(0.0, 0.0); }
+    else if (mwss && t == 0) { v = Fa[(size_t)b * ldin]; if (m != n) v = make_double2(0.0, 0.0); }
+    else if (t < tpole) v = Fa[(size_t)b * ldin + t];
+    else { v = Fa[(size_t)b * ldin + (2 * tpole - t)]; double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
+    return v;
+}
+// pair = 0: row b of X = the extension of the phi-FFT bin b (order m = b or b - T).  pair != 0: row j = the sum of the extensions of
+// the orders 2j-(L-1) and 2j-(L-2) (u_get above), L rows instead of T.
+__global__ void k_mw_extend(int L, const int* __restrict__ slab_n, int mwss, int pair, int ldin, int ldout, const double2* __restrict__ Fa_base,
                             size_t Fa_slab, double2* __restrict__ X_base, size_t X_slab) {
     int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     const int n = slab_n[blockIdx.z];
     const double2* Fa = Fa_base + Fa_slab * blockIdx.z;
     double2* X = X_base + X_slab * blockIdx.z;
-    const int T = mwss ? 2 * L : 2 * L - 1, tpole = mwss ? L : L - 1;
+    const int T = mwss ? 2 * L : 2 * L - 1;
     if (t >= T) return;
-    int m = b < L ? b : b - T;
     double2 v;
-    if (mwss && b == L) v = make_double2(0.0, 0.0);                  // phi-Nyquist bin of the 2L-point ring FFT: outside the band-limit
-    else if (t == tpole) { v = Fa[(size_t)b * ldin + t]; if (m != -n) v = make_double2(0.0, 0.0); }
-    else if (mwss && t == 0) { v = Fa[(size_t)b * ldin]; if (m != n) v = make_double2(0.0, 0.0); }
-    else if (t < tpole) v = Fa[(size_t)b * ldin + t];
-    else { v = Fa[(size_t)b * ldin + (2 * tpole - t)]; double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
+    if (pair) {
+        const int ma = 2 * b - (L - 1);
+        v = mw_ext_value(L, n, mwss, ldin, Fa, ma, t);
+        if (ma + 1 <= L - 1) { const double2 w = mw_ext_value(L, n, mwss, ldin, Fa, ma + 1, t); v.x += w.x; v.y += w.y; }
+    } else if (mwss && b == L) v = make_double2(0.0, 0.0);           // phi-Nyquist bin of the 2L-point ring FFT: outside the band-limit
+    else v = mw_ext_value(L, n, mwss, ldin, Fa, b < L ? b : b - T, t);
     X[(size_t)b * ldout + t] = v;
 }
 // MW / MWSS forward (iii)->(iv): with Y = FFT_T of the extended samples, F_{mm'} = (1/T) e^{-i m' theta_0} Y[m' mod T] (theta_0 = pi/T
@@ -288,14 +315,34 @@ __global__ void k_mw_pad_phase(int L, int mwss, int ldin, int ldout, const doubl
 // (-1)^{m+s} F_m(theta).  The theta kernel evaluates it on the L midpoint rings vartheta_j = (2j+1)pi/(2L), which are
 // symmetric about the equator (north-south fold); these kernels carry it to the MW rings theta_t = (2t+1)pi/(2L-1), exactly:
 // extend to the 2L-point circle -> FFT(2L) -> phase and re-bin -> inverse FFT(2L-1) -> keep t = 0..L-1 (t = L-1 is the ring theta = pi).
-__global__ void k_sym_extend(int L, int n, int ldin, const double2* __restrict__ F, double2* __restrict__ X) {
+__global__ void k_sym_extend(int L, int n, int pair, int ldin, const double2* __restrict__ F, double2* __restrict__ X) {
     int j = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     if (j >= 2 * L) return;
-    const int T = 2 * L - 1, m = b < L ? b : b - T;
+    const int T = 2 * L - 1;
+    auto ext = [&](int m) {
+        const double2* row = F + (size_t)(m < 0 ? m + T : m) * ldin;
+        if (j < L) return row[j];
+        double2 v = row[2 * L - 1 - j]; const double s = sgn_pow(m - n); v.x *= s; v.y *= s;
+        return v;
+    };
     double2 v;
-    if (j < L) v = F[(size_t)b * ldin + j];
-    else { v = F[(size_t)b * ldin + (2 * L - 1 - j)]; const double s = sgn_pow(m - n); v.x *= s; v.y *= s; }
+    if (pair) {               // row b = orders 2b-(L-1) and 2b-(L-2) summed (u_get above): L rows instead of 2L-1
+        const int ma = 2 * b - (L - 1);
+        v = ext(ma);
+        if (ma + 1 <= L - 1) { const double2 w = ext(ma + 1); v.x += w.x; v.y += w.y; }
+    } else v = ext(b < L ? b : b - T);
     X[(size_t)b * 2 * L + j] = v;
+}
+// paired resampling, last step: X[j][t] (t = 0..2L-2, the MW circle theta_t = (2t+1)pi/(2L-1); mirror of t is 2L-2-t) holds the sum of two
+// orders; F[bin(m)][t] = (c[t] + (-1)^{m-n} c[2L-2-t]) / 2 for the rings t = 0..L-1 of the map.
+__global__ void k_sym_unpair(int L, int n, int ldout, const double2* __restrict__ X, double2* __restrict__ F) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (t >= L) return;
+    const int T = 2 * L - 1, m = b < L ? b : b - T;
+    const double2* row = X + (size_t)((m + L - 1) >> 1) * T;
+    const double2 a = row[t], c = row[T - 1 - t];
+    const double s = ((m - n) & 1) ? -0.5 : 0.5;
+    F[(size_t)b * ldout + t] = make_double2(fma(s, c.x, 0.5 * a.x), fma(s, c.y, 0.5 * a.y));
 }
 // Y[b][k] = 2L c_{m'} e^{i m' pi/(2L)} (k = m' mod 2L)  ->  Z[b][m' mod (2L-1)] = c_{m'} e^{i m' pi/(2L-1)}
 __global__ void k_sym_rebin(int L, const double2* __restrict__ Y, double2* __restrict__ Z) {
@@ -318,7 +365,7 @@ __global__ void k_rows_head(int ncol, int ldin, int ldout, const double2* __rest
 // tiles W[m-m_end][ntp][NC] of one pass; rings not served by the pass at step m get 0 (peak split, R5).
 // fold != 0 (n != 0, symmetric ring set): column 0 = order +m at the ring itself (m >= m_s), column 1 = order -m at the MIRRORED
 // ring pi - theta (index nth-1-th), served by the same d-value up to (-1)^{l-n} (applied at the output), for m > m_s.
-__global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* __restrict__ wq,
+__global__ void k_weight_split(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* __restrict__ wq,
                                const double2* __restrict__ U_base, size_t U_slab, const ThetaPass* __restrict__ passes, int th_lo, int th_hi) {
     // one launch serves all passes of a kernel mode: grid.z = pass (its operand rows start one row into ThetaPass::in)
     const ThetaPass P = passes[blockIdx.z];
@@ -346,7 +393,7 @@ __global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int 
                 if (c == 1) s *= sgn_pow(m);
                 else if (sgn_out < 0) s *= sgn_pow(m + n);
             }
-            double2 x = U[(size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + ts];
+            double2 x = u_get(U, ldin, NBin, pair, L, n, m_out, ts);
             v.x = s * x.x; v.y = s * x.y;
         }
         W[((size_t)(m - m_end) * ntp + th) * NC + c] = v;
@@ -355,7 +402,7 @@ __global__ void k_weight_split(int L, int NBin, int ldin, int nth, int ntp, int 
 // forward split for n = 0 on a ring set symmetric about the equator (theta_kernels.cu FOLD): only the nth northern rings are
 // recursed.  W[m][ntp][2][NC]: set 0 = E = q (F_m(theta) + F_m(pi - theta)), set 1 = O = q (F_m(theta) - F_m(pi - theta)); the mirror of
 // ring th is nfull-1-th (the equator ring of HEALPix is its own mirror: E = q F_m, O = 0).  Column c = 1 is order -m with (-1)^m.
-__global__ void k_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end,
+__global__ void k_weight_split_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, int m_end,
                                      const double* __restrict__ wq, const double2* __restrict__ U, double2* __restrict__ W, int th_lo, int th_hi) {
     int th = blockIdx.x * blockDim.x + threadIdx.x;
     int m = m_end + blockIdx.y;
@@ -364,12 +411,11 @@ __global__ void k_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp
         double2 e = {0.0, 0.0}, o = {0.0, 0.0};
         if (th < nth && !(c == 1 && m == 0) && m < L && m > -L && th >= th_lo && th < th_hi) {
             const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
-            const double2* row = U + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
             double s = wq[th];
             if (c == 1) s *= sgn_pow(m);
-            const double2 a = row[th];
+            const double2 a = u_get(U, ldin, NBin, pair, L, 0, m_out, th);
             double2 b = {0.0, 0.0};
-            if (tm != th) b = row[tm];
+            if (tm != th) b = u_get(U, ldin, NBin, pair, L, 0, m_out, tm);
             e.x = s * (a.x + b.x); e.y = s * (a.y + b.y);
             if (tm != th) { o.x = s * (a.x - b.x); o.y = s * (a.y - b.y); }
         }
@@ -543,7 +589,7 @@ __global__ void k_prep_inverse_batch(int L, int Lp, int NC, int B, int n, int sg
 }
 // forward split: U[b][bin][ldu] -> Wb[cg][m-m_end][ntp][36] (weighted, masked by the peak split; [32] = lambda_m(theta)).
 // Block = 32 rings x one order x one column group.
-__global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int n, int sgn_out,
+__global__ void k_weight_split_batch(int L, int NBin, int ldin, int pair, size_t U_slab, int nth, int ntp, int NC, int B, int n, int sgn_out,
                                      int m_end, int fold, const int* __restrict__ m_lo, const double* __restrict__ wq,
                                      const double* __restrict__ lam, const double2* __restrict__ U, double* __restrict__ Wb,
                                      size_t cg_stride) {
@@ -567,7 +613,7 @@ __global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, i
                 if (c == 1) s *= sgn_pow(m);
                 else if (sgn_out < 0) s *= sgn_pow(m + n);
             }
-            const double2 x = U[(size_t)b * U_slab + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + ts];
+            const double2 x = u_get(U + (size_t)b * U_slab, ldin, NBin, pair, L, n, m_out, ts);      // (n = the slab's second index)
             v.x = s * x.x; v.y = s * x.y;
         }
         tile[tx][jc] = v;
@@ -584,7 +630,7 @@ __global__ void k_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, i
 }
 // forward split of the n = 0 fold (theta_mma.cu FOLD): Wb[cg][m-m_end][ntp north][68] = {32 columns E, 32 columns O, lambda, pad};
 // E = q (F_m(theta) + F_m(pi - theta)), O = q (F_m(theta) - F_m(pi - theta)), mirror ring index nfull-1-th.
-__global__ void k_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int m_end,
+__global__ void k_weight_split_batch_fold0(int L, int NBin, int ldin, int pair, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int m_end,
                                            const double* __restrict__ wq, const double* __restrict__ lam,
                                            const double2* __restrict__ U, double* __restrict__ Wb, size_t cg_stride) {
     __shared__ double2 tile[2][32][17];
@@ -595,12 +641,12 @@ __global__ void k_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_s
         double2 e = make_double2(0.0, 0.0), o = make_double2(0.0, 0.0);
         if (b < B && th < nth && !(c == 1 && m == 0) && m < L && m > -L) {
             const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
-            const double2* row = U + (size_t)b * U_slab + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
+            const double2* Ub = U + (size_t)b * U_slab;
             double s = wq[th];
             if (c == 1) s *= sgn_pow(m);
-            const double2 a = row[th];
+            const double2 a = u_get(Ub, ldin, NBin, pair, L, 0, m_out, th);
             double2 v = make_double2(0.0, 0.0);
-            if (tm != th) v = row[tm];
+            if (tm != th) v = u_get(Ub, ldin, NBin, pair, L, 0, m_out, tm);
             e.x = s * (a.x + v.x); e.y = s * (a.y + v.y);
             if (tm != th) { o.x = s * (a.x - v.x); o.y = s * (a.y - v.y); }
         }
@@ -705,7 +751,7 @@ __global__ void k_prep_inverse_f32(int L, int Lp, int NC, const double2* __restr
     }
 }
 // forward operands: W32[m][ntp][NC] = q(theta) F_{+m}(theta) and, for NC = 2, (-1)^m q(theta) F_{-m}(theta)
-__global__ void k_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* __restrict__ wq,
+__global__ void k_weight_split_f32(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* __restrict__ wq,
                                    const double2* __restrict__ U, float2* __restrict__ W) {
     int th = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     if (th >= ntp) return;
@@ -714,14 +760,14 @@ __global__ void k_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, 
         if (th < nth && !(c == 1 && m == 0)) {
             const int m_out = c == 1 ? -m : m;
             const double s = (c == 1 && (m & 1)) ? -wq[th] : wq[th];
-            const double2 x = U[(size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin + th];
+            const double2 x = u_get(U, ldin, NBin, pair, L, 0, m_out, th);
             v = make_float2((float)(s * x.x), (float)(s * x.y));
         }
         W[((size_t)m * ntp + th) * NC + c] = v;
     }
 }
 // the same for the north-south fold: W32[m][ntp north][2][NC], set 0 = E = q (F(theta) + F(pi - theta)), set 1 = O = q (F(theta) - F(pi - theta))
-__global__ void k_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* __restrict__ wq,
+__global__ void k_weight_split_f32_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, const double* __restrict__ wq,
                                          const double2* __restrict__ U, float2* __restrict__ W) {
     int th = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     if (th >= ntp) return;
@@ -730,10 +776,9 @@ __global__ void k_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int
         if (th < nth && !(c == 1 && m == 0)) {
             const int m_out = c == 1 ? -m : m, tm = nfull - 1 - th;
             const double s = (c == 1 && (m & 1)) ? -wq[th] : wq[th];
-            const double2* row = U + (size_t)(m_out < 0 ? m_out + NBin : m_out) * ldin;
-            const double2 a = row[th];
+            const double2 a = u_get(U, ldin, NBin, pair, L, 0, m_out, th);
             double2 b = make_double2(0.0, 0.0);
-            if (tm != th) b = row[tm];
+            if (tm != th) b = u_get(U, ldin, NBin, pair, L, 0, m_out, tm);
             e = make_float2((float)(s * (a.x + b.x)), (float)(s * (a.y + b.y)));
             if (tm != th) o = make_float2((float)(s * (a.x - b.x)), (float)(s * (a.y - b.y)));
         }
@@ -818,25 +863,25 @@ cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStr
     k_complex_to_real<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
     count_bytes(24.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mw_extend(int L, int nslab, const int* slab_n, int mwss, int ldin, int ldout, const double2* Fa, size_t Fa_slab, double2* X,
-                         size_t X_slab, cudaStream_t st) {
-    const int T = mwss ? 2 * L : 2 * L - 1;
-    dim3 grid(cdiv(T, 128), T, nslab);
-    k_mw_extend<<<grid, 128, 0, st>>>(L, slab_n, mwss, ldin, ldout, Fa, Fa_slab, X, X_slab);
-    count_bytes(32.0 * (double)T * T * nslab); LAUNCHED(); return cudaSuccess;
+cudaError_t st_mw_extend(int L, int nslab, const int* slab_n, int mwss, int pair, int ldin, int ldout, const double2* Fa, size_t Fa_slab,
+                         double2* X, size_t X_slab, cudaStream_t st) {
+    const int T = mwss ? 2 * L : 2 * L - 1, rows = pair ? L : T;
+    dim3 grid(cdiv(T, 128), rows, nslab);
+    k_mw_extend<<<grid, 128, 0, st>>>(L, slab_n, mwss, pair, ldin, ldout, Fa, Fa_slab, X, X_slab);
+    count_bytes(16.0 * (double)T * ((double)T + rows) * nslab); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_mw_pad_phase(int L, int nslab, int mwss, int ldin, int ldout, const double2* Y, size_t Y_slab, double2* Z, size_t Z_slab,
+cudaError_t st_mw_pad_phase(int L, int nslab, int mwss, int rows, int ldin, int ldout, const double2* Y, size_t Y_slab, double2* Z, size_t Z_slab,
                             cudaStream_t st) {
     const int T = mwss ? 2 * L : 2 * L - 1;
-    dim3 grid(cdiv(ldout, 128), T, nslab);
+    dim3 grid(cdiv(ldout, 128), rows, nslab);
     k_mw_pad_phase<<<grid, 128, 0, st>>>(L, mwss, ldin, ldout, Y, Y_slab, Z, Z_slab);
-    count_bytes(16.0 * (double)T * ((double)T + ldout) * nslab); LAUNCHED(); return cudaSuccess;
+    count_bytes(16.0 * (double)rows * ((double)T + ldout) * nslab); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int mmin, int npass, const double* wq, const double2* U,
+cudaError_t st_weight_split(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, int mmin, int npass, const double* wq, const double2* U,
                             size_t U_slab, const ThetaPass* passes, int th_lo, int th_hi, cudaStream_t st) {
     if (npass == 0) return cudaSuccess;
     dim3 grid(cdiv(ntp, 128), L - mmin - 1, npass);
-    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, wq, U, U_slab, passes, th_lo, th_hi);
+    k_weight_split<<<grid, 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, NC, wq, U, U_slab, passes, th_lo, th_hi);
     count_bytes(32.0 * NC * (double)(L - mmin - 1) * ntp * npass); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
@@ -866,11 +911,11 @@ cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, 
     k_prep_inverse_batch<<<grid, 128, 0, st>>>(L, Lp, NC, B, n, sgn_out, m_end, mmin, coef, scale, C, SG, sgstride, Gb, cg_stride);
     count_bytes(16.0 * B * NC * (double)(L - m_end) * L + 8.0 * SHT_MMA_ROW * (double)ncg * (L - m_end) * Lp); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
+cudaError_t st_weight_split_batch(int L, int NBin, int ldin, int pair, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
                                   int m_end, int fold, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
                                   size_t cg_stride, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
-    k_weight_split_batch<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, NC, B, n, sgn_out, m_end, fold, m_lo, wq, lam, U, Wb, cg_stride);
+    k_weight_split_batch<<<grid, 128, 0, st>>>(L, NBin, ldin, pair, U_slab, nth, ntp, NC, B, n, sgn_out, m_end, fold, m_lo, wq, lam, U, Wb, cg_stride);
     count_bytes(16.0 * B * NC * (double)(L - m_end) * ntp + 8.0 * SHT_MMA_ROW * (double)ncg * (L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
@@ -879,17 +924,17 @@ cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int 
     k_unpack_batch<<<grid, 128, 0, st>>>(L, Lp, Mp, mlim, NC, B, n, sgn_out, m_end, mmin, fwd, fold, C, Ob, cg_stride, out, out_slab, ld);
     count_bytes(8.0 * SHT_MMA_NCOL * (double)ncg * (L - m_end) * Mp + 32.0 * B * NC * (double)(L - m_end) * mlim); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
+cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
                                   const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st) {
     dim3 grid(cdiv(ntp, 128), L - m_end);
-    k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, m_end, wq, U, W, th_lo, th_hi);
+    k_weight_split_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, nfull, NC, m_end, wq, U, W, th_lo, th_hi);
     count_bytes(64.0 * NC * (double)(L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
+cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, int pair, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
                                         int m_end, const double* wq, const double* lam, const double2* U, double* Wb, size_t cg_stride,
                                         cudaStream_t st) {
     dim3 grid(cdiv(ntp, 32), L - m_end, ncg);
-    k_weight_split_batch_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, U_slab, nth, ntp, nfull, NC, B, m_end, wq, lam, U, Wb, cg_stride);
+    k_weight_split_batch_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, pair, U_slab, nth, ntp, nfull, NC, B, m_end, wq, lam, U, Wb, cg_stride);
     count_bytes(32.0 * B * NC * (double)(L - m_end) * ntp + 8.0 * SHT_MMA_ROWF * (double)ncg * (L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st) {
@@ -905,9 +950,9 @@ cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, cons
     k_prep_inverse_f32<<<grid, block, 0, st>>>(L, Lp, NC, coef, scale, G);
     count_bytes(16.0 * NC * (double)L * L + 8.0 * NC * (double)L * Lp); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
+cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
                                 cudaStream_t st) {
-    k_weight_split_f32<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, NC, wq, U, W);
+    k_weight_split_f32<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, NC, wq, U, W);
     count_bytes(24.0 * NC * (double)L * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st) {
@@ -918,18 +963,23 @@ cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t s
     k_c128_to_c64<<<cdiv(n, 256), 256, 0, st>>>(n, in, out);
     count_bytes(12.0 * (double)n); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
+cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
                                       float2* W, cudaStream_t st) {
-    k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, nth, ntp, nfull, NC, wq, U, W);
+    k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, nfull, NC, wq, U, W);
     count_bytes(48.0 * NC * (double)L * ntp); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st) {
-    k_sym_extend<<<dim3(cdiv(2 * L, 128), 2 * L - 1), 128, 0, st>>>(L, n, ldin, F, X);
-    count_bytes(32.0 * (double)(2 * L) * (2 * L - 1)); LAUNCHED(); return cudaSuccess;
+cudaError_t st_sym_extend(int L, int n, int pair, int ldin, const double2* F, double2* X, cudaStream_t st) {
+    const int rows = pair ? L : 2 * L - 1;
+    k_sym_extend<<<dim3(cdiv(2 * L, 128), rows), 128, 0, st>>>(L, n, pair, ldin, F, X);
+    count_bytes(16.0 * (double)(2 * L) * ((double)rows + 0.5 * (2 * L - 1))); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st) {
-    k_sym_rebin<<<dim3(cdiv(2 * L - 1, 128), 2 * L - 1), 128, 0, st>>>(L, Y, Z);
-    count_bytes(32.0 * (double)(2 * L - 1) * (2 * L - 1)); LAUNCHED(); return cudaSuccess;
+cudaError_t st_sym_rebin(int L, int rows, const double2* Y, double2* Z, cudaStream_t st) {
+    k_sym_rebin<<<dim3(cdiv(2 * L - 1, 128), rows), 128, 0, st>>>(L, Y, Z);
+    count_bytes(32.0 * (double)(2 * L - 1) * rows); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_sym_unpair(int L, int n, int ldout, const double2* X, double2* F, cudaStream_t st) {
+    k_sym_unpair<<<dim3(cdiv(L, 128), 2 * L - 1), 128, 0, st>>>(L, n, ldout, X, F);
+    count_bytes(16.0 * (double)(2 * L - 1) * (2.0 * L)); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st) {
     k_rows_head<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ldin, ldout, in, out);

@@ -20,13 +20,13 @@ cudaError_t st_pole_inverse(int L, int north, int NBf, int nslab, const int* sla
 cudaError_t st_hermitian_rows(int L, int NB, int ntp, int nth, double2* F, cudaStream_t st);
 cudaError_t st_real_to_complex(size_t n, const double* in, double2* out, cudaStream_t st);
 cudaError_t st_complex_to_real(size_t n, const double2* in, double* out, cudaStream_t st);
-cudaError_t st_mw_extend(int L, int nslab, const int* slab_n, int mwss, int ldin, int ldout, const double2* Fa, size_t Fa_slab, double2* X,
+cudaError_t st_mw_extend(int L, int nslab, const int* slab_n, int mwss, int pair, int ldin, int ldout, const double2* Fa, size_t Fa_slab, double2* X,
                          size_t X_slab, cudaStream_t st);
-cudaError_t st_mw_pad_phase(int L, int nslab, int mwss, int ldin, int ldout, const double2* Y, size_t Y_slab, double2* Z, size_t Z_slab,
+cudaError_t st_mw_pad_phase(int L, int nslab, int mwss, int rows, int ldin, int ldout, const double2* Y, size_t Y_slab, double2* Z, size_t Z_slab,
                             cudaStream_t st);
-cudaError_t st_weight_split(int L, int NBin, int ldin, int nth, int ntp, int NC, int mmin, int npass, const double* wq, const double2* U,
+cudaError_t st_weight_split(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, int mmin, int npass, const double* wq, const double2* U,
                             size_t U_slab, const ThetaPass* passes, int th_lo, int th_hi, cudaStream_t st);
-cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
+cudaError_t st_weight_split_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, int m_end, const double* wq,
                                   const double2* U, double2* W, int th_lo, int th_hi, cudaStream_t st);
 cudaError_t st_pole_forward(int L, int Lp, int n, int north, int NBin, int ldin, int col, double w, const double2* U, double2* H,
                             cudaStream_t st);
@@ -46,18 +46,19 @@ cudaError_t st_vec_sub(size_t n, const double* a, const double* b, double* out, 
 cudaError_t st_vec_add(size_t n, const double* x, double* y, cudaStream_t st);
 
 // MW inverse through the symmetric midpoint rings: resampling of F_m to the MW rings
-cudaError_t st_sym_extend(int L, int n, int ldin, const double2* F, double2* X, cudaStream_t st);
-cudaError_t st_sym_rebin(int L, const double2* Y, double2* Z, cudaStream_t st);
+cudaError_t st_sym_extend(int L, int n, int pair, int ldin, const double2* F, double2* X, cudaStream_t st);
+cudaError_t st_sym_rebin(int L, int rows, const double2* Y, double2* Z, cudaStream_t st);
+cudaError_t st_sym_unpair(int L, int n, int ldout, const double2* X, double2* F, cudaStream_t st);
 cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st);
 
 // batched path (operand / result layouts of theta_mma.cu, internal.h)
 cudaError_t st_prep_inverse_batch(int L, int Lp, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, const double2* coef,
                                   const double* scale, const double* C, const double2* SG, int sgstride, double* Gb, size_t cg_stride,
                                   cudaStream_t st);
-cudaError_t st_weight_split_batch(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
+cudaError_t st_weight_split_batch(int L, int NBin, int ldin, int pair, size_t U_slab, int nth, int ntp, int NC, int B, int ncg, int n, int sgn_out,
                                   int m_end, int fold, const int* m_lo, const double* wq, const double* lam, const double2* U, double* Wb,
                                   size_t cg_stride, cudaStream_t st);
-cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
+cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, int pair, size_t U_slab, int nth, int ntp, int nfull, int NC, int B, int ncg,
                                         int m_end, const double* wq, const double* lam, const double2* U, double* Wb, size_t cg_stride,
                                         cudaStream_t st);
 cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int ncg, int n, int sgn_out, int m_end, int mmin, int fwd, int fold,
@@ -67,9 +68,9 @@ cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int 
 cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st);
 cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v32, uint16_t* k16, cudaStream_t st);
 cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st);
-cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
+cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
                                 cudaStream_t st);
-cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
+cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
                                       float2* W, cudaStream_t st);
 cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st);
 cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t st);

@@ -252,6 +252,23 @@ def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, sym, L, rea
     assert rel(F, orc.s2_theta_inverse_columns(L, 0, orc.MW, flm, np.arange(-(L - 1), L))) < TOL
 
 
+@pytest.mark.parametrize("pair", [False, True])
+@pytest.mark.parametrize("L,spin,fold,real", [(1, 0, None, False), (2, 0, None, False), (9, 1, None, False), (33, 0, True, False), (64, -2, None, False),
+                                              (130, 0, True, True), (131, 3, None, False), (200, 0, False, False)])
+def test_mw_theta_ffts_with_one_or_two_orders_per_column(api, orc, pair, L, spin, fold, real):
+    """The extension of F_m to the theta circle is even or odd about the poles, alternating with m, so the theta-direction
+    FFTs of the forward upsampling and of the symmetric-ring inverse carry the orders m, m+1 as ONE column and split them afterwards
+    (default); SHT_OPT_NO_PAIR keeps one order per column.  Both against the oracle, on raw white noise (forward) and through the
+    symmetric-ring inverse (spin 0)."""
+    f = synth.random_map((L, 2 * L - 1), seed=11 + L, real=real)
+    P = api.Plan(L, spin, reality=real, fold=fold, pair=pair, invsym=True if spin == 0 else None)
+    want = orc.s2_forward(L, spin, orc.MW, project_mw_pole(f, spin).astype(np.complex128))
+    assert rel(P.forward(dev(f)).cpu().numpy(), want) < TOL
+    flm = synth.random_flm(L, spin, seed=2 * L + 1, real=real)
+    ref = orc.s2_inverse(L, spin, orc.MW, flm)
+    assert rel(P.inverse(dev(flm)).cpu().numpy(), ref.real if real else ref) < TOL
+
+
 @pytest.mark.parametrize("nside,L,spin,real", [(4, 8, 0, True), (8, 16, 0, True), (8, 20, 2, False), (16, 32, 0, False)])
 def test_healpix_iterative_refinement_vs_oracle(api, orc, nside, L, spin, real):
     """PAPER.md:172 "iterations are usually performed": flm <- flm + F (f - F^-1 flm), against the oracle's composition of its own

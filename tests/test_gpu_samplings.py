@@ -71,6 +71,15 @@ def test_forward_of_raw_white_noise_and_folds(api, orc, name, fold, L, spin, rea
         print(f"MWSS L={L} spin={spin}: departure from the oracle on the raw array {rel(got, raw):.3e}")
 
 
+@pytest.mark.parametrize("L,spin", [(2, 0), (9, 0), (40, 1), (65, -2), (128, 0)])
+def test_mwss_forward_with_one_order_per_theta_fft_column(api, orc, L, spin):
+    """MWSS forward with SHT_OPT_NO_PAIR (the default carries two orders per theta-FFT column, tested above) on raw white noise."""
+    g = synth.random_map(orc.map_shape(orc.MWSS, L), seed=7 * L + spin)
+    P = api.Plan(L, spin, sampling=api.MWSS, pair=False)
+    want = orc.s2_forward(L, spin, orc.MWSS, project_mwss_poles(g, spin).astype(np.complex128))
+    assert rel(P.forward(dev(g)).cpu().numpy(), want) < TOL
+
+
 @pytest.mark.parametrize("name", ["mwss", "dh", "gl"])
 def test_theta_stage_entry_points(api, orc, name):
     """Hot path alone on the new ring sets: Eq. 33 against the oracle's F_m(theta) columns (pole rings included)."""
