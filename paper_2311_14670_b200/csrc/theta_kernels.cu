@@ -25,10 +25,7 @@ namespace {
 
 using namespace shtdev;
 
-#ifndef SHT_NST
-#define SHT_NST 4
-#endif
-constexpr int NST = SHT_NST;   // stages of the operand ring
+constexpr int NST = 4;   // stages of the operand ring
 constexpr int NRS = 2;   // stages of the partial-sum hand-off
 constexpr int KS = 2;    // recursion steps per pipeline stage (one TMA barrier, one hand-off per KS steps)
 constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
@@ -42,22 +39,25 @@ constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on 
 // F_m(theta) = E + O and F_m(pi - theta) = E - O.  The degrees of a WARP all have one parity (warp w: degrees
 // l0 + 16 (w/2) + (w%2) + 2j), so every warp still hands over ONE partial-sum set -- the shared-memory footprint of the plain kernel,
 // 128-ring tiles included -- and the reducers add the even-degree warps and the odd-degree warps apart and emit both rings.
-template <int RL, int RT, int NW, int NC, bool FOLD>
+// WT = ring groups of warps: the NW compute warps form ND = NW / WT degree groups x WT ring groups; a warp covers RL degrees x 32 RT rings.
+// WT = 2 (16 degrees x 64 rings per warp) halves the cross-warp sum: half the partial-sum stores, half the reducers' loads and adds, and a
+// hand-off twice as deep in the same shared memory, for twice the (broadcast) operand loads per item.
+template <int RL, int RT, int NW, int NC, bool FOLD, int WT>
 struct InvSmem {
-    static constexpr int TL = NW * RL, NTH = 32 * RT, ROWD = 2 * NC + 2, NSET = FOLD ? 2 : 1;   // NSET: sets the reducers keep apart
-    static constexpr int NRS = NC == 1 ? 4 : 2;   // the one-column partial sums are half the size: a deeper hand-off fits
+    static constexpr int ND = NW / WT, TL = ND * RL, NTH = 32 * RT * WT, ROWD = 2 * NC + 2, NSET = FOLD ? 2 : 1;   // NSET: sets the reducers keep apart
+    static constexpr int NRS = (NC == 1 || WT >= 2) ? 4 : 2;   // smaller partial-sum sets: a deeper hand-off fits
     double op[NST][KS][TL * ROWD];          // operand rows {c Re, c Im (x NC), g', s} of the block's degrees (TMA ring)
     double lam[NST][KS][NTH];               // lambda_m(theta) of the block's rings (TMA ring)
-    double red[NRS][KS][NW][NTH][2 * NC];   // per-warp partial sums
+    double red[NRS][KS][ND][NTH][2 * NC];   // partial sums per degree group (the WT warps of a group own disjoint rings)
     int act[NRS][NW];                       // bit h: the warp wrote partial sums for step h of the pair
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
-template <int RL, int RT, int NW, int NC, bool FOLD>
+template <int RL, int RT, int NW, int NC, bool FOLD, int WT>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(const ThetaArgs A) {
-    using S = InvSmem<RL, RT, NW, NC, FOLD>;
-    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS, NSET = S::NSET;
-    static_assert(!FOLD || (NW % 2 == 0), "even-degree and odd-degree warps come in pairs");
+    using S = InvSmem<RL, RT, NW, NC, FOLD, WT>;
+    constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS, NSET = S::NSET, ND = S::ND;
+    static_assert(NW % WT == 0 && (!FOLD || (ND % 2 == 0)), "even-degree and odd-degree warps come in pairs");
     static_assert(TL == SHT_TQ, "the block's degrees must be one kappa quantum");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         };
         if (at == 0)
             for (int p = 0; p < NST && p < npairs; ++p) issue(p);
-        int mlo[NQ];
+        int mlo[NQ], wtq[NQ];                         // wtq: ring group of the output's ring (which warp of a degree group wrote it)
         bool valid[NQ], neg[NQ], south[NQ];
         double* obase[NQ];
         ptrdiff_t osouth[NQ];                         // FOLD: offset (doubles) from the ring's entry to its mirror ring's
@@ -105,6 +105,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         for (int q = 0; q < NQ; ++q) {
             const int o = at + NAUX * 32 * q;
             const int th = th0 + o % NTH;             // partial sums are stored [column][ring]
+            wtq[q] = (o % NTH) / (32 * RT);
             neg[q] = NC == 2 && (o / NTH);
             valid[q] = th < A.nth && o < NOUT && th >= A.th_lo && th < A.th_hi;
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
@@ -117,9 +118,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         for (int p = 0; p < npairs; ++p) {
             const int rs = p & (NRS - 1);
             mbar_wait(&sm.rfull[rs], (p / NRS) & 1);
-            int actb[NW];
+            int actb[ND][NQ];                          // flags of the warp that wrote output q of degree group ww
 #pragma unroll
-            for (int ww = 0; ww < NW; ++ww) actb[ww] = sm.act[rs][ww];
+            for (int ww = 0; ww < ND; ++ww)
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) actb[ww][q] = sm.act[rs][ww * WT + wtq[q]];
 #pragma unroll
             for (int h = 0; h < KS; ++h) {
                 const int m = mtop - KS * p - h;
@@ -130,30 +133,19 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                     for (int q = 0; q < NQ; ++q) v[e][q] = make_double2(0.0, 0.0);
                 bool any = false;
 #pragma unroll
-                for (int ww = 0; ww < NW; ++ww) {
-#ifdef SHT_EXP_NOREDUCE
-                    if (0) {
-#else
-                    if ((actb[ww] >> h) & 1) {
-#endif
-                        any = true;
-                        constexpr int e = 0;
-                        const int es = FOLD ? (ww & 1) : e;       // FOLD: warp ww carries degrees of parity ww & 1
-                        const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]) + at;
+                for (int ww = 0; ww < ND; ++ww) {
+                    const int es = FOLD ? (ww & 1) : 0;           // FOLD: degree group ww carries degrees of parity ww & 1
+                    const double2* r = reinterpret_cast<const double2*>(&sm.red[rs][h][ww][0][0]) + at;
 #pragma unroll
-                        for (int q = 0; q < NQ; ++q)
-                            if (at + NAUX * 32 * q < NOUT) {
-                                const double2 t = r[NAUX * 32 * q];
-                                if (FOLD && es) { v[NSET - 1][q].x += t.x; v[NSET - 1][q].y += t.y; }
-                                else { v[0][q].x += t.x; v[0][q].y += t.y; }
-                            }
-                    }
+                    for (int q = 0; q < NQ; ++q)
+                        if (at + NAUX * 32 * q < NOUT && ((actb[ww][q] >> h) & 1)) {
+                            any = true;
+                            const double2 t = r[NAUX * 32 * q];
+                            if (FOLD && es) { v[NSET - 1][q].x += t.x; v[NSET - 1][q].y += t.y; }
+                            else { v[0][q].x += t.x; v[0][q].y += t.y; }
+                        }
                 }
-#ifdef SHT_EXP_NORED
-                if (any && v[0][0].x == 12345.678) {
-#else
                 if (any) {
-#endif
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
                         if (valid[q] && m >= mlo[q] && !(neg[q] && m == 0)) {
@@ -182,14 +174,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         return;
     }
     reg_alloc_compute<(FOLD && NC == 2) ? 56 : 40>();
-#ifdef SHT_EXP_STAGGER
-    if (w >= NW / 2) __nanosleep(SHT_EXP_STAGGER);
-#endif
 
     // -------------------------------------------------------------------- compute warps
     // degrees of this warp: la + DS j, j < RL (FOLD: one parity per warp, DS = 2)
     constexpr int DS = FOLD ? 2 : 1;
-    const int la = FOLD ? l0 + 2 * RL * (w >> 1) + (w & 1) : l0 + w * RL, l_hi = la + DS * (RL - 1);
+    const int wd = w / WT, tho = (w % WT) * 32 * RT;  // degree group; first ring of the warp inside the block's ring tile
+    const int la = FOLD ? l0 + 2 * RL * (wd >> 1) + (wd & 1) : l0 + wd * RL, l_hi = la + DS * (RL - 1);
     const bool warp_real = la < A.L;
     double cur[NI], prev[NI];
     KPack<NI> kp;
@@ -197,8 +187,8 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
 #pragma unroll
     for (int q = 0; q < NI; ++q) { cur[q] = 0.0; prev[q] = 0.0; }
     bool wact = false;                                // some item of this warp has k == 0 (its contribution matters)
-    const double* stv = P.st_val + (size_t)la * A.ntp + th0 + lane;
-    const uint8_t* stk = P.st_k + (size_t)la * A.ntp + th0 + lane;
+    const double* stv = P.st_val + (size_t)la * A.ntp + th0 + tho + lane;
+    const uint8_t* stk = P.st_k + (size_t)la * A.ntp + th0 + tho + lane;
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step, so the
     // iterates never move between registers).  Returns true if partial sums were written.
@@ -207,14 +197,20 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         if (!(m <= l_hi && warp_real)) return false;
         bool wrote = false;
         if (m >= la) {                                // the degree l == m starts (warp-uniform): Eq. 27 start values
+            if (DS == 1 || ((m - la) & 1) == 0) {     // (one address computed here, not RL row pointers kept in registers)
+                const size_t so = (size_t)(m - la) * A.ntp;
+                double sv[RT]; uint32_t sk[RT];
 #pragma unroll
-            for (int j = 0; j < RL; ++j) {
-                if (m == la + DS * j) {
+                for (int i = 0; i < RT; ++i) { sv[i] = stv[so + 32 * i]; sk[i] = stk[so + 32 * i]; }
 #pragma unroll
-                    for (int i = 0; i < RT; ++i) {
-                        ca[j * RT + i] = stv[(size_t)(DS * j) * A.ntp + 32 * i];
-                        cb[j * RT + i] = 0.0;
-                        kp.set(j * RT + i, stk[(size_t)(DS * j) * A.ntp + 32 * i]);
+                for (int j = 0; j < RL; ++j) {
+                    if (m == la + DS * j) {
+#pragma unroll
+                        for (int i = 0; i < RT; ++i) {
+                            ca[j * RT + i] = sv[i];
+                            cb[j * RT + i] = 0.0;
+                            kp.set(j * RT + i, sk[i]);
+                        }
                     }
                 }
             }
@@ -224,7 +220,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         const double s = row[ROWD - 1];
         double lam[RT];
 #pragma unroll
-        for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][h][lane + 32 * i] * s;
+        for (int i = 0; i < RT; ++i) lam[i] = sm.lam[slot][h][tho + lane + 32 * i] * s;
         if (wact) {
             double acc[RT][2 * NC];
 #pragma unroll
@@ -249,7 +245,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                     cb[j * RT + i] = fma(lam[i], e, -(g * cb[j * RT + i]));
                 }
             }
-            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][w][0][0]);
+            double2* rd = reinterpret_cast<double2*>(&sm.red[rs][h][wd][0][0]) + tho;
 #pragma unroll
             for (int i = 0; i < RT; ++i)
 #pragma unroll
@@ -436,9 +432,6 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         return;
     }
     reg_alloc_compute<(NC == 1 && RT == 16) ? 56 : 40>();
-#ifdef SHT_EXP_STAGGER
-    if (w >= NW / 2) __nanosleep(SHT_EXP_STAGGER);
-#endif
 
     // -------------------------------------------------------------------- compute warps
     // state: start values preloaded; a lane holds still (lambda' = 1, g' = 0) until m reaches its degree
@@ -570,12 +563,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     }
 }
 
-template <int RL, int RT, int NW, int NC, bool FOLD = false>
+template <int RL, int RT, int NW, int NC, bool FOLD = false, int WT = 1>
 cudaError_t launch_inv(const ThetaArgs& a, cudaStream_t st) {
-    using S = InvSmem<RL, RT, NW, NC, FOLD>;
+    using S = InvSmem<RL, RT, NW, NC, FOLD, WT>;
     const size_t smem = sizeof(S) + 128;
     dim3 grid((a.Lp / S::TL) * (a.ntp / S::NTH), a.npass);
-    auto k = theta_inverse_kernel<RL, RT, NW, NC, FOLD>;
+    auto k = theta_inverse_kernel<RL, RT, NW, NC, FOLD, WT>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid, (NW + NAUX) * 32, smem, st>>>(a);
@@ -597,7 +590,9 @@ cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
 
 }  // namespace
 
-// Tile shapes: inverse 64 degrees x 128 rings per block (8 compute warps, 8 degrees x 4 rings per thread);
+// Tile shapes: inverse 64 degrees x 128 rings per block: 8 compute warps, 8 degrees x 4 rings per thread (one order per step, P mode) or
+//              16 degrees x 2 rings per thread with the warps split 4 degree groups x 2 ring groups (+-m per step, PM mode: measured
+//              5-6 % faster there -- L = 8192 inverse 84.7 -> 79.8 ms -- and 1-4 % slower in P mode; 4 ring groups: 15 % slower);
 //              forward 64 degrees x 128 rings per block (8 compute warps, 2 degrees x 16 rings per thread).
 int theta_inverse_rowd(int mode) { return mode == 0 ? 6 : 4; }
 // Tile choice.  A launch has (Lp/64) x (ntp/rings_per_block) x npass blocks whose step counts grow linearly with the degree
@@ -614,10 +609,12 @@ cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) 
     if (a.npass == 0) return cudaSuccess;
     if (a.fold0) {
         if (small_tiles(a, 128)) return mode == 0 ? launch_inv<8, 2, 8, 2, true>(a, st) : launch_inv<8, 2, 8, 1, true>(a, st);
-        return mode == 0 ? launch_inv<8, 4, 8, 2, true>(a, st) : launch_inv<8, 4, 8, 1, true>(a, st);
+        if (mode != 0) return launch_inv<8, 4, 8, 1, true>(a, st);
+        return a.tile == 128 ? launch_inv<8, 4, 8, 2, true>(a, st) : launch_inv<16, 2, 8, 2, true, 2>(a, st);
     }
     if (small_tiles(a, 128)) return mode == 0 ? launch_inv<8, 2, 8, 2>(a, st) : launch_inv<8, 2, 8, 1>(a, st);
-    return mode == 0 ? launch_inv<8, 4, 8, 2>(a, st) : launch_inv<8, 4, 8, 1>(a, st);
+    if (mode != 0) return launch_inv<8, 4, 8, 1>(a, st);
+    return a.tile == 128 ? launch_inv<8, 4, 8, 2>(a, st) : launch_inv<16, 2, 8, 2, false, 2>(a, st);
 }
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
