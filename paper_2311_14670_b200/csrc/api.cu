@@ -92,7 +92,7 @@ struct sht_plan {
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
     bool f32_inner = false;    // set while an fp32 transform runs its fp64-array core
     int dtype = SHT_F64;       // SHT_F32: fp32 hot kernels (theta_f32.cu) and fp32 public arrays; staging and FFTs stay fp64
-    float2* ab32 = nullptr;    // fp32: [L][Lp] recursion coefficients
+    float4* ab32 = nullptr;    // fp32: [L][Lp] recursion coefficients {A, A, -B, -B}
     float *lam32_inv = nullptr, *lam32_fwd = nullptr;
     float *st32_inv = nullptr, *st32_fwd = nullptr; uint16_t *k16_inv = nullptr, *k16_fwd = nullptr;   // fp32 start values
     double2 *io_a = nullptr, *io_b = nullptr;   // fp32: fp64 copies of the public arrays
@@ -401,7 +401,7 @@ void layout(sht_plan* P, char* base) {
     if (P->reality && P->sampling != SHT_HEALPIX) P->cplx = B.take<double2>(P->map_elems * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
     if (P->dtype == SHT_F32) {
-        P->ab32 = B.take<float2>((size_t)L * Lp);
+        P->ab32 = B.take<float4>((size_t)L * Lp);
         P->st32_inv = B.take<float>((size_t)Lp * P->inv.ntp); P->k16_inv = B.take<uint16_t>((size_t)Lp * P->inv.ntp);
         P->st32_fwd = B.take<float>((size_t)Lp * P->fwd.ntp); P->k16_fwd = B.take<uint16_t>((size_t)Lp * P->fwd.ntp);
         P->io_a = B.take<double2>((size_t)L * NB); P->io_b = B.take<double2>((size_t)L * NB);

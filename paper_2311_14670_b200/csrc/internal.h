@@ -82,11 +82,13 @@ struct F32Args {
     int L, Lp, nth, ntp, NB, ldout;
     int fold0;                // northern rings only.  forward: W32 rows hold the E / O sets; inverse: both rings of a mirror pair are written
     int nfull;                // folded ring sets: ring th mirrors ring nfull-1-th
-    const float2* ab;         // [m][Lp] {A_m(l) = a_{m-1}(l), B_m(l) = a_{m-1}(l)/a_m(l)} (Eq. 25-26), rows m = 0..L-1 (row 0 unused: zeros)
+    const float4* ab;         // [m][Lp] {A, A, -B, -B}: A_m(l) = a_{m-1}(l), B_m(l) = a_{m-1}(l)/a_m(l) (Eq. 25-26), duplicated for the packed
+                              // two-rings-per-instruction arithmetic; rows m = 0..L-1 (row 0 unused: zeros)
     const float* lam32;       // fp32 copy of the lambda table of the n = 0 pass, row m + 1 (layout of ThetaPass::lam with m_end = 0)
     const float* st_val;      // [Lp][ntp] Eq. 27 start values, windowed: true value = st_val * 2^(-48 st_k)
     const uint16_t* st_k;
-    const float2* in;         // inverse: G32[m][Lp][NC] = scale(l) f_lm; forward: W32[m][ntp][NC] = q(theta) F_m(theta)
+    const float2* in;         // inverse: G32[m][Lp][NC] float4 {Re, Re, Im, Im} of scale(l) f_lm; forward: W32[m][ntp/2][NSET][2 NC] float2 =
+                              // (ring 2p, ring 2p+1) of q(theta) F_m(theta) (staging.cu k_weight_split_f32)
     double2* out;             // inverse: F[row][ldout]; forward: H[m + L - 1][Lp]   (fp64 accumulators shared with the fp64 staging)
 };
 cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st);

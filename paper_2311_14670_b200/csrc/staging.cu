@@ -698,15 +698,16 @@ __global__ void k_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, i
 }
 
 // ---- fp32 variant (theta_f32.cu) ----------------------------------------------------------------------------------------
-// recursion coefficients of Eq. 25-26 in the paper's own form, fp32: AB[m][l] = {a_{m-1}(l), a_{m-1}(l)/a_m(l)}, a_m = 2/sqrt((l-m)(l+m+1))
-__global__ void k_ab32(int L, int Lp, float2* __restrict__ AB) {
+// recursion coefficients of Eq. 25-26 in the paper's own form, fp32, duplicated for the packed arithmetic of theta_f32.cu:
+// AB[m][l] = {A, A, -B, -B}, A = a_{m-1}(l), B = a_{m-1}(l)/a_m(l), a_m = 2/sqrt((l-m)(l+m+1))
+__global__ void k_ab32(int L, int Lp, float4* __restrict__ AB) {
     int l = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     if (l >= Lp) return;
-    float2 v = make_float2(0.f, 0.f);
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
     if (l < L && m >= 1 && l >= m) {
         const double p = (double)(l - m + 1) * (double)(l + m);
-        v.x = (float)(2.0 / sqrt(p));
-        v.y = (float)sqrt((double)(l - m) * (double)(l + m + 1) / p);
+        v.x = v.y = (float)(2.0 / sqrt(p));
+        v.z = v.w = -(float)sqrt((double)(l - m) * (double)(l + m + 1) / p);
     }
     AB[(size_t)m * Lp + l] = v;
 }
@@ -728,7 +729,7 @@ __global__ void k_start32(size_t n, const double* __restrict__ v64, const uint8_
 }
 // inverse operands: G32[m][Lp][NC] = scale(l) f_{l,+m} and, for NC = 2, (-1)^m scale(l) f_{l,-m} (32 x 32 transpose, coef is l-major)
 __global__ void k_prep_inverse_f32(int L, int Lp, int NC, const double2* __restrict__ coef, const double* __restrict__ scale,
-                                   float2* __restrict__ G) {
+                                   float4* __restrict__ G) {
     __shared__ double2 tile[2][32][33];
     const int NB = 2 * L - 1, l0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
     for (int c = 0; c < NC; ++c)
@@ -746,13 +747,20 @@ __global__ void k_prep_inverse_f32(int L, int Lp, int NC, const double2* __restr
         for (int c = 0; c < NC; ++c) {
             const double sg = (c == 1 && (m & 1)) ? -sc : sc;
             const double2 x = tile[c][threadIdx.x][q];
-            G[((size_t)m * Lp + l) * NC + c] = make_float2((float)(sg * x.x), (float)(sg * x.y));
+            const float gx = (float)(sg * x.x), gy = (float)(sg * x.y);
+            G[((size_t)m * Lp + l) * NC + c] = make_float4(gx, gx, gy, gy);       // duplicated for the packed arithmetic
         }
     }
 }
-// forward operands: W32[m][ntp][NC] = q(theta) F_{+m}(theta) and, for NC = 2, (-1)^m q(theta) F_{-m}(theta)
+// forward operands of the fp32 kernels, laid out for packed (two rings per instruction) arithmetic: per order m and ring PAIR
+// (2p, 2p+1), NSET operand sets of 2 NC components {Re +m, Im +m[, Re -m, Im -m]}, each a float2 = (ring 2p, ring 2p+1):
+//   W32[m][ntp/2][NSET][2 NC] float2.     value = q(theta) F_{+m}(theta) and, for NC = 2, (-1)^m q(theta) F_{-m}(theta)
+__device__ __forceinline__ void w32_store(float* __restrict__ W, int m, int ntp, int th, int NSET, int set, int NC, int c, float2 v) {
+    float* w = W + ((((size_t)m * (ntp / 2) + (th >> 1)) * NSET + set) * 2 * NC + 2 * c) * 2 + (th & 1);
+    w[0] = v.x; w[2] = v.y;
+}
 __global__ void k_weight_split_f32(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* __restrict__ wq,
-                                   const double2* __restrict__ U, float2* __restrict__ W) {
+                                   const double2* __restrict__ U, float* __restrict__ W) {
     int th = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     if (th >= ntp) return;
     for (int c = 0; c < NC; ++c) {
@@ -763,12 +771,12 @@ __global__ void k_weight_split_f32(int L, int NBin, int ldin, int pair, int nth,
             const double2 x = u_get(U, ldin, NBin, pair, L, 0, m_out, th);
             v = make_float2((float)(s * x.x), (float)(s * x.y));
         }
-        W[((size_t)m * ntp + th) * NC + c] = v;
+        w32_store(W, m, ntp, th, 1, 0, NC, c, v);
     }
 }
-// the same for the north-south fold: W32[m][ntp north][2][NC], set 0 = E = q (F(theta) + F(pi - theta)), set 1 = O = q (F(theta) - F(pi - theta))
+// the same for the north-south fold: NSET = 2, set 0 = E = q (F(theta) + F(pi - theta)), set 1 = O = q (F(theta) - F(pi - theta)), northern rings
 __global__ void k_weight_split_f32_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, const double* __restrict__ wq,
-                                         const double2* __restrict__ U, float2* __restrict__ W) {
+                                         const double2* __restrict__ U, float* __restrict__ W) {
     int th = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
     if (th >= ntp) return;
     for (int c = 0; c < NC; ++c) {
@@ -782,8 +790,8 @@ __global__ void k_weight_split_f32_fold0(int L, int NBin, int ldin, int pair, in
             e = make_float2((float)(s * (a.x + b.x)), (float)(s * (a.y + b.y)));
             if (tm != th) o = make_float2((float)(s * (a.x - b.x)), (float)(s * (a.y - b.y)));
         }
-        float2* w = W + ((size_t)m * ntp + th) * 2 * NC;
-        w[c] = e; w[NC + c] = o;
+        w32_store(W, m, ntp, th, 2, 0, NC, c, e);
+        w32_store(W, m, ntp, th, 2, 1, NC, c, o);
     }
 }
 __global__ void k_c64_to_c128(size_t n, const float* __restrict__ in, double* __restrict__ out) {
@@ -937,7 +945,7 @@ cudaError_t st_weight_split_batch_fold0(int L, int NBin, int ldin, int pair, siz
     k_weight_split_batch_fold0<<<grid, 128, 0, st>>>(L, NBin, ldin, pair, U_slab, nth, ntp, nfull, NC, B, m_end, wq, lam, U, Wb, cg_stride);
     count_bytes(32.0 * B * NC * (double)(L - m_end) * ntp + 8.0 * SHT_MMA_ROWF * (double)ncg * (L - m_end) * ntp); LAUNCHED(); return cudaSuccess;
 }
-cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st) {
+cudaError_t st_ab32(int L, int Lp, float4* AB, cudaStream_t st) {
     k_ab32<<<dim3(cdiv(Lp, 128), L), 128, 0, st>>>(L, Lp, AB);
     LAUNCHED(); return cudaSuccess;
 }
@@ -947,12 +955,12 @@ cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v
 }
 cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st) {
     dim3 grid(cdiv(Lp, 32), cdiv(L, 32)), block(32, 8);
-    k_prep_inverse_f32<<<grid, block, 0, st>>>(L, Lp, NC, coef, scale, G);
-    count_bytes(16.0 * NC * (double)L * L + 8.0 * NC * (double)L * Lp); LAUNCHED(); return cudaSuccess;
+    k_prep_inverse_f32<<<grid, block, 0, st>>>(L, Lp, NC, coef, scale, reinterpret_cast<float4*>(G));
+    count_bytes(16.0 * NC * (double)L * L + 16.0 * NC * (double)L * Lp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,
                                 cudaStream_t st) {
-    k_weight_split_f32<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, NC, wq, U, W);
+    k_weight_split_f32<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, NC, wq, U, reinterpret_cast<float*>(W));
     count_bytes(24.0 * NC * (double)L * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_f32_to_f64(size_t n, const float* in, double* out, cudaStream_t st) {
@@ -965,7 +973,7 @@ cudaError_t st_f64_to_f32(size_t n, const double* in, float* out, cudaStream_t s
 }
 cudaError_t st_weight_split_f32_fold0(int L, int NBin, int ldin, int pair, int nth, int ntp, int nfull, int NC, const double* wq, const double2* U,
                                       float2* W, cudaStream_t st) {
-    k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, nfull, NC, wq, U, W);
+    k_weight_split_f32_fold0<<<dim3(cdiv(ntp, 128), L), 128, 0, st>>>(L, NBin, ldin, pair, nth, ntp, nfull, NC, wq, U, reinterpret_cast<float*>(W));
     count_bytes(48.0 * NC * (double)L * ntp); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_sym_extend(int L, int n, int pair, int ldin, const double2* F, double2* X, cudaStream_t st) {

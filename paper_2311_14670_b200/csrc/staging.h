@@ -65,7 +65,7 @@ cudaError_t st_unpack_batch(int L, int Lp, int Mp, int mlim, int NC, int B, int 
                             const double* C, const double* Ob, size_t cg_stride, double2* out, size_t out_slab, int ld, cudaStream_t st);
 
 // fp32 variant (theta_f32.cu): tables, operand preparation, precision conversion of the public arrays
-cudaError_t st_ab32(int L, int Lp, float2* AB, cudaStream_t st);
+cudaError_t st_ab32(int L, int Lp, float4* AB, cudaStream_t st);
 cudaError_t st_start32(size_t n, const double* v64, const uint8_t* k64, float* v32, uint16_t* k16, cudaStream_t st);
 cudaError_t st_prep_inverse_f32(int L, int Lp, int NC, const double2* coef, const double* scale, float2* G, cudaStream_t st);
 cudaError_t st_weight_split_f32(int L, int NBin, int ldin, int pair, int nth, int ntp, int NC, const double* wq, const double2* U, float2* W,

@@ -7,6 +7,10 @@
 // (3 FP32 instructions per step) with fp32 tables A, B (plan time) and the renormalisation of Sec. 3.4 as
 // power-of-two windows sized for fp32: true value = stored * 2^(-48 k); a stored value with k > 0 stays below 2^-43 (it grows by
 // less than 2^21 per step and is checked every step against 2^-64), which is below fp32 resolution of the sums, so no masking.
+// Arithmetic is PACKED: a thread's items come in pairs of neighbouring rings held as float2, and every multiply-add is one
+// fma.rn.f32x2 / mul.f32x2 (SASS FFMA2 / FMUL2, sm_100+; __ffma2_rn, __fmul2_rn) -- 7 packed instructions per pair of items and step
+// (4 projection + 3 recursion).  A packed instruction occupies the FP32 pipe for two cycles but one issue slot, which leaves every
+// other issue slot to the loads, stores and bookkeeping that the one-instruction-per-cycle FP32 pipe otherwise has to share with them.
 // Scope: second index n = 0 (spin-0 plans), MW sampling, one map.  Everything around the two kernels (FFTs, staging, the pole
 // ring) is the fp64 code; the kernels read fp32 operand tables and add their block sums into the fp64 F / H arrays.
 #include "internal.h"
@@ -47,29 +51,32 @@ struct KPackF {
         return o != 0;
     }
 };
-template <int NI>
-__device__ __forceinline__ void window_check_f(float (&cur)[NI], float (&prev)[NI], KPackF& kp) {
+// items are stored as float2 pairs: item q = component q & 1 of pair q >> 1
+template <int NP>
+__device__ __forceinline__ void window_check_f(float2 (&cur)[NP], float2 (&prev)[NP], KPackF& kp) {
     const float s = pow2f(-FW), top = pow2f(FTOP);
 #pragma unroll
-    for (int q = 0; q < NI; ++q) {
-        if (fabsf(cur[q]) > top && kp.get(q) != 0u) { cur[q] *= s; prev[q] *= s; kp.dec(q); }
+    for (int q = 0; q < NP; ++q) {
+        if (fabsf(cur[q].x) > top && kp.get(2 * q) != 0u) { cur[q].x *= s; prev[q].x *= s; kp.dec(2 * q); }
+        if (fabsf(cur[q].y) > top && kp.get(2 * q + 1) != 0u) { cur[q].y *= s; prev[q].y *= s; kp.dec(2 * q + 1); }
     }
 }
 
+
 // =============================================================================================================
 // inverse, Eq. 33:  F[row(+-m)][theta] += sum_l G[m][l][c] d^l_{m,0}(theta)
-// warp w: degrees l0 + 8 w + j (j < 8); lane: rings th0 + lane + 32 i (i < 4)
+// warp w: degrees l0 + 8 w + j (j < 8); lane: ring pairs th0 + 2 lane + {0, 1} + 64 ip (ip < 2)
 // =============================================================================================================
 // FOLD (rings symmetric about the equator, northern half recursed): d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta).  The
 // degrees of a warp all have one parity (warp w: l0 + 16 (w/2) + (w%2) + 2j), the reducers add the even-degree and the odd-degree warps
 // apart (E0, E1) and write F_m(theta) = E0 + E1 and F_m(pi - theta) = (-1)^m (E0 - E1), as the fp64 kernel does.
 template <int NC, bool FOLD>
-__global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
-    constexpr int RL = 8, RT = 4, NI = RL * RT, DS = FOLD ? 2 : 1;
-    __shared__ float2 s_ab[2][TLF];
-    __shared__ float2 s_g[2][TLF * NC];
+__global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A) {
+    constexpr int RL = 8, RP = 2, NP = RL * RP, DS = FOLD ? 2 : 1, C4 = 2 * NC;      // RP ring pairs per thread; C4 real columns
+    __shared__ float4 s_ab[2][TLF];                  // {A, A, -B, -B} of the block's degrees: operands arrive duplicated for the packed math
+    __shared__ float4 s_g[2][TLF * NC];              // {Re, Re, Im, Im} of G[m][l][c]
     __shared__ float s_lam[2][NTF];
-    __shared__ float2 s_part[2][NWF][NC][NTF];       // double-buffered: the sums of step m are reduced while step m-1 is computed
+    __shared__ float s_part[2][NWF][C4][NTF];        // planar partial sums, double-buffered: step m is reduced while step m-1 is computed
     const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;      // heavy tiles first
     const int l0 = lt * TLF, th0 = tt * NTF;
@@ -79,19 +86,20 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
     const int la = FOLD ? l0 + 2 * RL * (w >> 1) + (w & 1) : l0 + w * RL;         // degrees of this warp: la + DS j
 
     // operand rows of step m, one element per thread, copied global -> shared asynchronously (cp.async): the copy of step m-1
-    // is in flight while step m is computed and is awaited just before the block barrier
+    // is in flight while step m is computed and is awaited just before the block barrier.  The tables hold the duplicated form.
     auto load_ops = [&](int m, int buf) {
-        if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float2));
-        if (tid < TLF * NC) __pipeline_memcpy_async(&s_g[buf][tid], &A.in[((size_t)m * A.Lp + l0) * NC + tid], sizeof(float2));
+        if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float4));
+        if (tid < TLF * NC)
+            __pipeline_memcpy_async(&s_g[buf][tid], reinterpret_cast<const float4*>(A.in) + ((size_t)m * A.Lp + l0) * NC + tid, sizeof(float4));
         if (tid >= 128 && tid < 128 + NTF)
             __pipeline_memcpy_async(&s_lam[buf][tid - 128], &A.lam32[(size_t)(m + 1) * A.ntp + th0 + tid - 128], sizeof(float));
         __pipeline_commit();
     };
-    float cur[NI], prev[NI];
+    float2 cur[NP], prev[NP];
     KPackF kp;
     kp.fill(0u);
 #pragma unroll
-    for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
+    for (int q = 0; q < NP; ++q) { cur[q] = make_float2(0.f, 0.f); prev[q] = make_float2(0.f, 0.f); }
     load_ops(mtop, 0);
     __pipeline_wait_prior(0);
     __syncthreads();
@@ -103,8 +111,8 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
             float ex = 0.f, ey = 0.f, ox = 0.f, oy = 0.f;
 #pragma unroll
             for (int ww = 0; ww < NWF; ++ww) {
-                const float2 v = s_part[pb][ww][c][t];
-                if (FOLD && (ww & 1)) { ox += v.x; oy += v.y; } else { ex += v.x; ey += v.y; }
+                const float vx = s_part[pb][ww][2 * c][t], vy = s_part[pb][ww][2 * c + 1][t];
+                if (FOLD && (ww & 1)) { ox += vx; oy += vy; } else { ex += vx; ey += vy; }
             }
             if (th < A.nth && !(c == 1 && m == 0)) {
                 const int m_out = c == 1 ? -m : m;
@@ -121,7 +129,7 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
         }
     };
     // one step: project d_m, then advance to d_{m-1}.  `ca` holds d_m, `cb` holds d_{m+1} on entry and d_{m-1} on exit.
-    auto step = [&](const int m, const int buf, float (&ca)[NI], float (&cb)[NI]) {
+    auto step = [&](const int m, const int buf, float2 (&ca)[NP], float2 (&cb)[NP]) {
         if (m > 0) load_ops(m - 1, buf ^ 1);
         bool mine = m <= la + DS * (RL - 1) && la < A.L;   // this warp has started degrees
         if (mine && m >= la) {                      // the degree l == m starts (warp-uniform)
@@ -129,44 +137,49 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
             for (int j = 0; j < RL; ++j)
                 if (m == la + DS * j) {
 #pragma unroll
-                    for (int i = 0; i < RT; ++i) {
-                        const size_t o = (size_t)m * A.ntp + th0 + lane + 32 * i;
-                        ca[j * RT + i] = A.st_val[o]; cb[j * RT + i] = 0.f;
-                        kp.set(j * RT + i, A.st_k[o]);
+                    for (int ip = 0; ip < RP; ++ip) {
+                        const size_t o = (size_t)m * A.ntp + th0 + 2 * lane + 64 * ip;
+                        ca[j * RP + ip] = *reinterpret_cast<const float2*>(A.st_val + o); cb[j * RP + ip] = make_float2(0.f, 0.f);
+                        const ushort2 k2 = *reinterpret_cast<const ushort2*>(A.st_k + o);
+                        kp.set(2 * (j * RP + ip), k2.x); kp.set(2 * (j * RP + ip) + 1, k2.y);
                     }
                 }
         }
-        float acc[RT][2 * NC];
+        float2 acc[RP][C4];
 #pragma unroll
-        for (int i = 0; i < RT; ++i)
+        for (int ip = 0; ip < RP; ++ip)
 #pragma unroll
-            for (int c = 0; c < 2 * NC; ++c) acc[i][c] = 0.f;
+            for (int c = 0; c < C4; ++c) acc[ip][c] = make_float2(0.f, 0.f);
         if (mine) {
-            float lam[RT];
+            float2 lam[RP];
 #pragma unroll
-            for (int i = 0; i < RT; ++i) lam[i] = s_lam[buf][lane + 32 * i];
+            for (int ip = 0; ip < RP; ++ip) lam[ip] = *reinterpret_cast<const float2*>(&s_lam[buf][2 * lane + 64 * ip]);
 #pragma unroll
             for (int j = 0; j < RL; ++j) {
                 const int dj = la - l0 + DS * j;
-                const float2 ab = s_ab[buf][dj];
-                float cf[2 * NC];
+                const float4 ab = s_ab[buf][dj];
+                const float2 A2 = make_float2(ab.x, ab.y), nB2 = make_float2(ab.z, ab.w);
+                float2 cf[C4];
 #pragma unroll
-                for (int c = 0; c < NC; ++c) { const float2 t = s_g[buf][dj * NC + c]; cf[2 * c] = t.x; cf[2 * c + 1] = t.y; }
+                for (int c = 0; c < NC; ++c) {
+                    const float4 t = s_g[buf][dj * NC + c];
+                    cf[2 * c] = make_float2(t.x, t.y); cf[2 * c + 1] = make_float2(t.z, t.w);
+                }
 #pragma unroll
-                for (int i = 0; i < RT; ++i) {
-                    const float e = ca[j * RT + i];
+                for (int ip = 0; ip < RP; ++ip) {
+                    const float2 e = ca[j * RP + ip];
 #pragma unroll
-                    for (int c = 0; c < 2 * NC; ++c) acc[i][c] = fmaf(e, cf[c], acc[i][c]);
-                    cb[j * RT + i] = fmaf(lam[i] * ab.x, e, -(ab.y * cb[j * RT + i]));
+                    for (int c = 0; c < C4; ++c) acc[ip][c] = __ffma2_rn(e, cf[c], acc[ip][c]);
+                    cb[j * RP + ip] = __ffma2_rn(__fmul2_rn(lam[ip], A2), e, __fmul2_rn(nB2, cb[j * RP + ip]));
                 }
             }
-            if (kp.any_nonzero()) window_check_f<NI>(cb, ca, kp);
+            if (kp.any_nonzero()) window_check_f<NP>(cb, ca, kp);
         }
         const int pb = buf;                         // partial-sum buffer of this step (alternates with the operand buffer)
 #pragma unroll
-        for (int i = 0; i < RT; ++i)
+        for (int ip = 0; ip < RP; ++ip)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) s_part[pb][w][c][lane + 32 * i] = make_float2(acc[i][2 * c], acc[i][2 * c + 1]);
+            for (int c = 0; c < C4; ++c) *reinterpret_cast<float2*>(&s_part[pb][w][c][2 * lane + 64 * ip]) = acc[ip][c];
         __pipeline_wait_prior(0);
         __syncthreads();                            // the only block barrier of the step: partial sums of m and operands of m-1 are visible;
         reduce(m, pb);                              // buffer pb is next written two steps from now, after the barrier of step m-1
@@ -179,18 +192,18 @@ __global__ void __launch_bounds__(NWF * 32) theta_inverse_f32(const F32Args A) {
 
 // =============================================================================================================
 // forward, Eq. 30:  H[+-m + L-1][l] += sum_theta W[m][theta][c] d^l_{m,0}(theta)
-// warp w: rings th0 + 16 w + i (i < 16); lane: degrees l0 + lane + 32 r (r < 2)
+// warp w: ring pairs th0 + 16 w + 2 ip + {0, 1} (ip < 8); lane: degrees l0 + lane + 32 r (r < 2)
 // FOLD: northern rings only; W32 rows hold E = q (F_m(theta) + F_m(pi - theta)) and O = q (F_m(theta) - F_m(pi - theta)); a degree
 // with l+m even contracts with E, one with l+m odd with O (d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta)).  A thread's two
 // degrees share their parity, which alternates with the lane: one load with two addresses serves both (as in theta_kernels.cu).
 // =============================================================================================================
 template <int NC, bool FOLD>
-__global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
-    constexpr int RL = 2, RT = 16, NI = RL * RT, NCW = FOLD ? 2 * NC : NC;
-    __shared__ float2 s_ab[2][TLF];
-    __shared__ float2 s_w[2][NTF * NCW];
+__global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A) {
+    constexpr int RL = 2, RP = 8, NP = RL * RP, NSET = FOLD ? 2 : 1, C4 = 2 * NC, NPB = NTF / 2;      // NPB ring pairs per block
+    __shared__ float4 s_ab[2][TLF];
+    __shared__ __align__(16) float2 s_w[2][NPB * NSET * C4];      // [pair][set][column] = (ring 2p, ring 2p+1): the layout of k_weight_split_f32
     __shared__ float s_lam[2][NTF];
-    __shared__ float2 s_part[2][NWF][NC][TLF];
+    __shared__ float s_part[2][NWF][C4][TLF];
     const int ntt = A.ntp / NTF, nlt = A.Lp / TLF;
     const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
     const int l0 = lt * TLF, th0 = tt * NTF;
@@ -199,18 +212,19 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
     const int mtop = min(l0 + TLF - 1, A.L - 1);
 
     auto load_ops = [&](int m, int buf) {
-        if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float2));
-        for (int o = tid; o < NTF * NCW; o += NWF * 32)
-            __pipeline_memcpy_async(&s_w[buf][o], &A.in[((size_t)m * A.ntp + th0) * NCW + o], sizeof(float2));
+        if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float4));
+        const float4* src = reinterpret_cast<const float4*>(A.in + ((size_t)m * A.ntp + th0) * NSET * NC);
+        for (int o = tid; o < NPB * NSET * C4 / 2; o += NWF * 32)
+            __pipeline_memcpy_async(reinterpret_cast<float4*>(&s_w[buf][0]) + o, src + o, sizeof(float4));
         if (tid >= 128 && tid < 128 + NTF)
             __pipeline_memcpy_async(&s_lam[buf][tid - 128], &A.lam32[(size_t)(m + 1) * A.ntp + th0 + tid - 128], sizeof(float));
         __pipeline_commit();
     };
-    float cur[NI], prev[NI];
+    float2 cur[NP], prev[NP];
     KPackF kp;
     kp.fill(0u);
 #pragma unroll
-    for (int q = 0; q < NI; ++q) { cur[q] = 0.f; prev[q] = 0.f; }
+    for (int q = 0; q < NP; ++q) { cur[q] = make_float2(0.f, 0.f); prev[q] = make_float2(0.f, 0.f); }
     int lr[RL];
 #pragma unroll
     for (int r = 0; r < RL; ++r) lr[r] = l0 + lane + 32 * r;
@@ -218,56 +232,59 @@ __global__ void __launch_bounds__(NWF * 32) theta_forward_f32(const F32Args A) {
     __pipeline_wait_prior(0);
     __syncthreads();
 
-    auto step = [&](const int m, const int buf, float (&ca)[NI], float (&cb)[NI]) {
+    auto step = [&](const int m, const int buf, float2 (&ca)[NP], float2 (&cb)[NP]) {
         if (m > 0) load_ops(m - 1, buf ^ 1);
 #pragma unroll
         for (int r = 0; r < RL; ++r)
             if (m == lr[r] && lr[r] < A.L) {        // this lane's degree starts
 #pragma unroll
-                for (int i = 0; i < RT; ++i) {
-                    const size_t o = (size_t)m * A.ntp + th0 + w * RT + i;
-                    ca[r * RT + i] = A.st_val[o]; cb[r * RT + i] = 0.f;
-                    kp.set(r * RT + i, A.st_k[o]);
+                for (int ip = 0; ip < RP; ++ip) {
+                    const size_t o = (size_t)m * A.ntp + th0 + w * 2 * RP + 2 * ip;
+                    ca[r * RP + ip] = *reinterpret_cast<const float2*>(A.st_val + o); cb[r * RP + ip] = make_float2(0.f, 0.f);
+                    const ushort2 k2 = *reinterpret_cast<const ushort2*>(A.st_k + o);
+                    kp.set(2 * (r * RP + ip), k2.x); kp.set(2 * (r * RP + ip) + 1, k2.y);
                 }
             }
-        float acc[RL][2 * NC];
+        float2 acc[RL][C4];
 #pragma unroll
         for (int r = 0; r < RL; ++r)
 #pragma unroll
-            for (int c = 0; c < 2 * NC; ++c) acc[r][c] = 0.f;
-        float2 ab[RL];
+            for (int c = 0; c < C4; ++c) acc[r][c] = make_float2(0.f, 0.f);
+        float2 A2[RL], nB2[RL];
 #pragma unroll
-        for (int r = 0; r < RL; ++r) ab[r] = s_ab[buf][lane + 32 * r];
-        const int set = FOLD ? ((l0 + m + lane) & 1) * NC : 0;      // FOLD: 0 = E (l+m even), NC = O; per lane parity, same for both degrees
+        for (int r = 0; r < RL; ++r) { const float4 ab = s_ab[buf][lane + 32 * r]; A2[r] = make_float2(ab.x, ab.y); nB2[r] = make_float2(ab.z, ab.w); }
+        const int set = FOLD ? ((l0 + m + lane) & 1) : 0;      // FOLD: 0 = E (l+m even), 1 = O; per lane parity, same for both degrees
+        const float2* wrow = &s_w[buf][(w * RP * NSET + set) * C4];
+        const float2* lrow = reinterpret_cast<const float2*>(&s_lam[buf][w * 2 * RP]);
 #pragma unroll
-        for (int i = 0; i < RT; ++i) {
-            const float lam = s_lam[buf][w * RT + i];
-            float wv[2 * NC];
+        for (int ip = 0; ip < RP; ++ip) {
+            const float2 lam = lrow[ip];
+            float2 wv[C4];
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
-                const float2 t = s_w[buf][(w * RT + i) * NCW + set + c];
-                wv[2 * c] = t.x; wv[2 * c + 1] = t.y;
+                const float4 t = *reinterpret_cast<const float4*>(wrow + ip * NSET * C4 + 2 * c);
+                wv[2 * c] = make_float2(t.x, t.y); wv[2 * c + 1] = make_float2(t.z, t.w);
             }
 #pragma unroll
             for (int r = 0; r < RL; ++r) {
-                const float e = ca[r * RT + i];
+                const float2 e = ca[r * RP + ip];
 #pragma unroll
-                for (int c = 0; c < 2 * NC; ++c) acc[r][c] = fmaf(e, wv[c], acc[r][c]);
-                cb[r * RT + i] = fmaf(lam * ab[r].x, e, -(ab[r].y * cb[r * RT + i]));
+                for (int c = 0; c < C4; ++c) acc[r][c] = __ffma2_rn(e, wv[c], acc[r][c]);
+                cb[r * RP + ip] = __ffma2_rn(__fmul2_rn(lam, A2[r]), e, __fmul2_rn(nB2[r], cb[r * RP + ip]));
             }
         }
-        if (kp.any_nonzero()) window_check_f<NI>(cb, ca, kp);
+        if (kp.any_nonzero()) window_check_f<NP>(cb, ca, kp);
 #pragma unroll
         for (int r = 0; r < RL; ++r)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) s_part[buf][w][c][lane + 32 * r] = make_float2(acc[r][2 * c], acc[r][2 * c + 1]);
+            for (int c = 0; c < C4; ++c) s_part[buf][w][c][lane + 32 * r] = acc[r][c].x + acc[r][c].y;      // the pair's two rings
         __pipeline_wait_prior(0);
         __syncthreads();                            // the only block barrier of the step (partial sums double-buffered, see the inverse)
         for (int o = tid; o < NC * TLF; o += NWF * 32) {
             const int c = o / TLF, t = o % TLF, l = l0 + t;
             float sx = 0.f, sy = 0.f;
 #pragma unroll
-            for (int ww = 0; ww < NWF; ++ww) { const float2 v = s_part[buf][ww][c][t]; sx += v.x; sy += v.y; }
+            for (int ww = 0; ww < NWF; ++ww) { sx += s_part[buf][ww][2 * c][t]; sy += s_part[buf][ww][2 * c + 1][t]; }
             if (l < A.L && l >= m && !(c == 1 && m == 0)) {
                 const int m_out = c == 1 ? -m : m;
                 double* op = reinterpret_cast<double*>(A.out) + ((size_t)(m_out + A.L - 1) * A.Lp + l) * 2;
