@@ -62,9 +62,11 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
-    const ThetaPass P = A.passes[blockIdx.y];
+    // blocks are dispatched in linear order: tile-major, pass-minor, so that the heavy (large-l) tiles of EVERY pass start first
+    const unsigned bid = blockIdx.x + gridDim.x * blockIdx.y, tile = bid / gridDim.y;
+    const ThetaPass P = A.passes[bid % gridDim.y];
     const int ntt = A.ntp / NTH, nlt = A.Lp / TL;
-    const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;     // heavy (large-l) tiles first
+    const int lt = nlt - 1 - (int)(tile / ntt), tt = tile % ntt;
     const int l0 = lt * TL, th0 = tt * NTH;
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TL <= an || l0 >= A.L || th0 >= A.nth || th0 + NTH <= A.th_lo || th0 >= A.th_hi) return;
@@ -316,9 +318,10 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
-    const ThetaPass P = A.passes[blockIdx.y];
+    const unsigned bid = blockIdx.x + gridDim.x * blockIdx.y, tile = bid / gridDim.y;      // tile-major, pass-minor (see the inverse kernel)
+    const ThetaPass P = A.passes[bid % gridDim.y];
     const int ntt = A.ntp / NTB, nlt = A.Lp / TLB;
-    const int lt = nlt - 1 - (int)(blockIdx.x / ntt), tt = blockIdx.x % ntt;
+    const int lt = nlt - 1 - (int)(tile / ntt), tt = tile % ntt;
     const int l0 = lt * TLB, th0 = tt * NTB;
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth || th0 + NTB <= A.th_lo || th0 >= A.th_hi) return;   // (rings outside the shard inside a
