@@ -32,9 +32,11 @@ UNIT = "transform_pairs/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of the forward theta kernel, per launch, from the ncu --set full captures under
 # profiles/ (file named beside each); key (L, spin, batch).  Not measurable inside this process: null for other workloads.
 NCU_TRAFFIC_BYTES = {
-    (1024, 2, 1): (128.008e6 + 11.222e6, "profiles/r1_v7_theta_kernels.md"),
-    (2048, 0, 1): (1.516876e9 + 155.507e6, "profiles/r1_v7_theta_kernels.md"),
-    (2048, 0, 16): (46.314083e9 + 11.453921e9, "profiles/r1_v7_theta_kernels.md"),
+    (1024, 2, 1): (127.888128e6 + 10.841600e6, "profiles/r2b_theta_kernels.md"),
+    (2048, 0, 1): (1.329291e9 + 126.638336e6, "profiles/r2b_theta_kernels.md"),
+    (4096, 0, 1): (37.860121e9 + 1.936975e9, "profiles/r2b_theta_kernels.md"),
+    (8192, 0, 1): (337.503584e9 + 24.737303e9, "profiles/r2b_theta_kernels.md"),
+    (2048, 0, 16): (46.052300e9 + 11.329958e9, "profiles/r2_theta_kernels.md"),
 }
 
 
