@@ -177,6 +177,23 @@ def time_stages(plan, x, flush, reps=5):
     return med(ti), med(tf), bi, bf, err
 
 
+def time_pairs(plan, x, torch, target_ms=40.0):
+    """ms per inverse + forward pair through the normal call path (stage timing off, so plans with L <= 512 replay their captured CUDA
+    graphs), back to back on the same buffers, CUDA events around the whole loop."""
+    f = plan.inverse(x)
+    b = plan.forward(f)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def loop(n):
+        e0.record()
+        for _ in range(n):
+            plan.inverse(x, out=f); plan.forward(f, out=b)
+        e1.record(); e1.synchronize()
+        return e0.elapsed_time(e1) / n
+    t = loop(3)
+    return loop(max(3, min(400, int(target_ms / max(t, 1e-3)))))
+
+
 def compact(ms, nbytes, flops, peak_tf):
     """One direction of a sweep row: ms per stage, fraction of the arithmetic peak in the hot kernels, GB/s of the HBM-bound stages."""
     gbs = lambda b, t: round(b / (t * 1e-3) / 1e9, 1) if t > 0 else None
@@ -193,7 +210,7 @@ def sweep(api, synth, torch, dev, flush, pk):
     def add(name, plan, x, peak_tf, extra=None):
         mi, mf, bi, bf, err = time_stages(plan, x, flush, reps=3)
         r = {"config": name, "inverse": compact(mi, bi, plan.flops(False), peak_tf), "forward": compact(mf, bf, plan.flops(True), peak_tf),
-             "roundtrip_err": float(f"{err:.3e}")}
+             "pair_ms": round(time_pairs(plan, x, torch), 4), "roundtrip_err": float(f"{err:.3e}")}
         if extra:
             r.update(extra)
         rows.append(r)
@@ -408,7 +425,8 @@ def main():
             out["sweep"] = sweep(api, synth, torch, dev, flush, pk)
             out["sweep_is"] = ("per direction: hot / fft / staging ms (median of 3, CUDA events inside the library), frac = algorithmic flop / hot ms / "
                                "measured peak (DFMA unless 'peak' says ffma), GB/s = algorithmic bytes of the stage / its time "
-                               f"(HBM peak {hbm.get('hbm_gbs')} GB/s {hbm_kind})")
+                               f"(HBM peak {hbm.get('hbm_gbs')} GB/s {hbm_kind}); pair_ms = one inverse + forward through the normal call path "
+                               "(stage timing off: plans with L <= 512 replay captured CUDA graphs), back to back, no L2 flush")
         print(json.dumps(out))
     R.finish()
 

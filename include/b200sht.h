@@ -71,6 +71,10 @@ enum {
                                      sequential recursion steps.  Single-map fp64 S^2 plans; the folds are off. */
     SHT_OPT_ADJOINT  = 1u << 5,   /* also build what the adjoint entry points need (complex fp64 single-map plans; MW / MWSS plans then
                                      carry the tables of two more ring sets: about twice the workspace) */
+    SHT_OPT_GRAPH    = 1u << 9,   /* replay each whole transform as ONE captured CUDA graph (one capture per direction and pair of buffers; an
+                                     internal capture stream, so the caller's stream may be the default stream).  Default for L <= 512, where a
+                                     transform is a chain of 10-50 short launches and bound by launch overhead ...                          */
+    SHT_OPT_NO_GRAPH = 1u << 10,  /* ... this flag launches the kernels one by one.  (Stage timing always does.)                          */
     SHT_OPT_NO_PAIR  = 1u << 8    /* MW / MWSS: the theta-direction FFTs of the forward upsampling and of the symmetric-ring
                                      inverse carry TWO orders m, m+1 per column by default (their extensions to the theta circle are one even
                                      and one odd function, separated afterwards: half the FFT work); this flag keeps one order

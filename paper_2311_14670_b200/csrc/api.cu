@@ -117,6 +117,12 @@ struct sht_plan {
     double* wq_map = nullptr;  // [F_ld] quadrature weight of every ring of the map (direct-quadrature samplings; adjoints)
     double* wq_quad = nullptr; // [4L] MW / MWSS: weight of every one of the 2L quadrature rings (not folded; adjoints)
     int device = 0, nsm = 0;   // device the plan was created on and its SM count (tile choice)
+    // CUDA graphs (launch-bound sizes): a whole transform is captured once per (direction, input, output) and replayed with one launch
+    struct GraphEntry { int kind; const void* in; void* out; cudaGraphExec_t exec; long launches; };
+    std::vector<GraphEntry> graphs;
+    cudaStream_t cap_stream = nullptr;   // capture stream (the caller's stream may be the legacy default stream, which cannot capture)
+    bool use_graph = false;
+    int graph_hits = 0, graph_misses = 0;
     int* d_flag = nullptr;     // device flag raised by table kernels (start value outside the window-counter range)
     double sec_bytes[3] = {0, 0, 0};   // algorithmic bytes moved by the FFT / staging sections of the last transform (stage timing)
     int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
@@ -1016,6 +1022,7 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if ((opts & SHT_OPT_FOLD_ON) && (opts & SHT_OPT_FOLD_OFF)) return SHT_EINVAL;
     if ((opts & SHT_OPT_TILE64) && (opts & SHT_OPT_TILE128)) return SHT_EINVAL;
     if ((opts & SHT_OPT_INVSYM) && (opts & SHT_OPT_NO_INVSYM)) return SHT_EINVAL;
+    if ((opts & SHT_OPT_GRAPH) && (opts & SHT_OPT_NO_GRAPH)) return SHT_EINVAL;
     // fp32 variant (BASELINE config 5): spin 0, MW sampling, one map
     if (dtype == SHT_F32 && (spin != 0 || sampling != SHT_MW || batch != 1)) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
@@ -1061,6 +1068,8 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     // MW / MWSS forward upsampling and the symmetric-ring resampling carry two orders per theta-circle column (staging.cu u_get); the
     // adjoint entry points run the transposed chain on single orders, so plans that offer them keep one order per column
     P->pair = (sampling == SHT_MW || sampling == SHT_MWSS) && !helper && !(opts & (SHT_OPT_ADJOINT | SHT_OPT_NO_PAIR));
+    // launch-bound sizes replay a captured CUDA graph (run_transform below)
+    P->use_graph = !helper && ((L <= 512 && !(opts & SHT_OPT_NO_GRAPH)) || (opts & SHT_OPT_GRAPH));
     sht_status s = check_start_range(P);
     if (s == SHT_OK && (opts & SHT_OPT_ADJOINT) && !helper) {
         // adjoint entry points (Eq. 52 / 58): complex fp64 single-map plans
@@ -1092,6 +1101,7 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     query_device(P);
     rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L);
     P->pair = 1;
+    P->use_graph = L <= 512;
     sht_status s = check_start_range(P);
     if (s == SHT_OK) s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
@@ -1114,6 +1124,8 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     if (work_bytes < P->need_bytes) { g_err = "workspace too small"; return SHT_EWORKSPACE; }
     if (reinterpret_cast<uintptr_t>(work) % 256 != 0) { g_err = "workspace must be 256-byte aligned (bulk-TMA operand rows)"; return SHT_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
+    for (auto& g : P->graphs) cudaGraphExecDestroy(g.exec);      // captured transforms point into the old workspace
+    P->graphs.clear();
     P->work = work; P->work_bytes = work_bytes;
     layout(P, (char*)work);
     const int L = P->L, Lp = P->Lp;
@@ -1233,6 +1245,8 @@ sht_status sht_plan_destroy(sht_plan* P) {
             if (h) cufftDestroy(h);
     }
     for (auto e : P->ev) cudaEventDestroy(e);
+    for (auto& g : P->graphs) cudaGraphExecDestroy(g.exec);
+    if (P->cap_stream) cudaStreamDestroy(P->cap_stream);
     sht_plan_destroy(P->adj_inv); sht_plan_destroy(P->adj_fwd);
     delete P;
     return SHT_OK;
@@ -1267,6 +1281,8 @@ sht_status sht_plan_set_shard(sht_plan* P, int rank, int nranks) {
         return SHT_EUNSUPPORTED;
     }
     P->shard_rank = rank; P->shard_n = nranks;
+    for (auto& g : P->graphs) cudaGraphExecDestroy(g.exec);      // captured transforms carry the old share
+    P->graphs.clear();
     return SHT_OK;
 }
 sht_status sht_plan_shard_range(const sht_plan* P, int forward, int* first, int* count) {
@@ -1318,16 +1334,14 @@ sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_str
     return s;
 }
 
-sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream stream) {
-    CS(check_ready(P));
-    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+static sht_status s2_inverse_body(sht_plan* P, const void* flm, void* f, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L;
     const size_t ncoef = (size_t)L * P->M, nmap = P->map_elems;
     if (P->dtype == SHT_F32 && !P->f32_inner) {      // fp32 public arrays: fp64 copies around the core (staging and FFTs are fp64)
         CK(st_f32_to_f64(2 * ncoef, (const float*)flm, (double*)P->io_a, st));
         P->f32_inner = true;
-        sht_status s = s2_inverse_plan(P, P->io_a, P->io_b, stream);
+        sht_status s = s2_inverse_body(P, P->io_a, P->io_b, stream);
         P->f32_inner = false;
         if (s != SHT_OK) return s;
         CK(st_f64_to_f32(P->reality ? nmap : 2 * nmap, (const double*)P->io_b, (float*)f, st));
@@ -1346,16 +1360,14 @@ sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream str
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
-sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream stream) {
-    CS(check_ready(P));
-    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+static sht_status s2_forward_body(sht_plan* P, const void* f, void* flm, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L;
     const size_t ncoef = (size_t)L * P->M, nmap = P->map_elems;
     if (P->dtype == SHT_F32 && !P->f32_inner) {
         CK(st_f32_to_f64(P->reality ? nmap : 2 * nmap, (const float*)f, (double*)P->io_a, st));
         P->f32_inner = true;
-        sht_status s = s2_forward_plan(P, P->io_a, P->io_b, stream);
+        sht_status s = s2_forward_body(P, P->io_a, P->io_b, stream);
         P->f32_inner = false;
         if (s != SHT_OK) return s;
         CK(st_f64_to_f32(2 * ncoef, (const double*)P->io_b, (float*)flm, st));
@@ -1500,9 +1512,7 @@ sht_status s2_forward_adjoint_plan(sht_plan* P, const void* flm, void* f, sht_st
 }
 
 // ---- SO(3) (Eq. 15-18) ----------------------------------------------------------------------------
-sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream stream) {
-    CS(check_ready(P));
-    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+static sht_status so3_inverse_body(sht_plan* P, const void* flmn, void* f, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB, N = P->N;
     const size_t slab = (size_t)L * NB;
@@ -1516,9 +1526,7 @@ sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream s
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
-sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream stream) {
-    CS(check_ready(P));
-    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+static sht_status so3_forward_body(sht_plan* P, const void* f, void* flmn, sht_stream stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB, N = P->N;
     const size_t slab = (size_t)L * NB;
@@ -1534,8 +1542,84 @@ sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream s
     return SHT_OK;
 }
 
-// ---- cached convenience calls ------------------------------------------------------------------------------------------
 }  // extern "C"
+
+// ---- public transform calls: direct, or through a captured CUDA graph -----------------------------------------------------------
+// At small band-limits a transform is a chain of 10-50 short launches (staging kernels, cuFFT passes, the fused kernels) and is bound
+// by launch overhead, not by the GPU.  Plans with use_graph (default L <= 512; SHT_OPT_GRAPH / SHT_OPT_NO_GRAPH) capture the chain once
+// per (direction, input pointer, output pointer) on an internal stream and replay it with ONE cudaGraphLaunch on the caller's stream.
+// Stage timing, a caller that is itself capturing, and plans whose buffers change on every call (the cache misses) take the direct path.
+namespace {
+typedef sht_status (*transform_body)(sht_plan*, const void*, void*, sht_stream);
+void drop_graphs(sht_plan* P) {
+    for (auto& g : P->graphs) cudaGraphExecDestroy(g.exec);
+    P->graphs.clear();
+}
+sht_status run_transform(sht_plan* P, int kind, const void* in, void* out, sht_stream stream, transform_body body) {
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!P->use_graph || P->timing) return body(P, in, out, stream);
+    cudaStreamCaptureStatus cst = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cst) != cudaSuccess || cst != cudaStreamCaptureStatusNone) { (void)cudaGetLastError(); return body(P, in, out, stream); }
+    for (auto& g : P->graphs)
+        if (g.kind == kind && g.in == in && g.out == out) {
+            CK(cudaGraphLaunch(g.exec, st));
+            count_launch((int)g.launches);
+            P->graph_hits++;
+            return SHT_OK;
+        }
+    // buffers that change on every call would be re-captured every time: give up on graphs for this plan
+    if (++P->graph_misses > 16 && P->graph_hits < P->graph_misses) { P->use_graph = false; drop_graphs(P); return body(P, in, out, stream); }
+    if (!P->cap_stream) CK(cudaStreamCreateWithFlags(&P->cap_stream, cudaStreamNonBlocking));
+    const long before = sht_launch_count(0);
+    CK(cudaStreamBeginCapture(P->cap_stream, cudaStreamCaptureModeThreadLocal));
+    sht_status s = body(P, in, out, (sht_stream)P->cap_stream);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(P->cap_stream, &graph);
+    const long nl = sht_launch_count(0) - before;
+    count_launch(-(int)nl);                                   // nothing ran yet
+    if (s != SHT_OK || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        (void)cudaGetLastError();
+        if (s != SHT_OK) return s;
+        P->use_graph = false;                                 // capture not possible here: direct launches from now on
+        return body(P, in, out, stream);
+    }
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); P->use_graph = false; return body(P, in, out, stream); }
+    if (P->graphs.size() >= 8) { cudaGraphExecDestroy(P->graphs.front().exec); P->graphs.erase(P->graphs.begin()); }
+    P->graphs.push_back({kind, in, out, exec, nl});
+    CK(cudaGraphLaunch(exec, st));
+    count_launch((int)nl);
+    return SHT_OK;
+}
+}  // namespace
+
+extern "C" {
+sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+    return run_transform(P, 0, flm, f, stream, s2_inverse_body);
+}
+sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flm || !f || P->kind != 0) return SHT_EINVAL;
+    return run_transform(P, 1, f, flm, stream, s2_forward_body);
+}
+sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+    return run_transform(P, 0, flmn, f, stream, so3_inverse_body);
+}
+sht_status so3_forward_plan(sht_plan* P, const void* f, void* flmn, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+    return run_transform(P, 1, f, flmn, stream, so3_forward_body);
+}
+}  // extern "C"
+
+// ---- cached convenience calls ------------------------------------------------------------------------------------------
 
 namespace {
 // One entry per (device, problem).  The entry's mutex is held from lookup until the transform (and, for the *_host calls, the
