@@ -101,32 +101,38 @@ __global__ void k_hp_unpack_fwd(int nside, int L, int NB, int mlo, int nth, int 
         if (m < L && i < nth) U[(size_t)(m < 0 ? m + NB : m) * ldu + i] = tile[threadIdx.x][q];
     }
 }
-// inverse fold: Y_ring[k] = sum_{m = k mod n, |m| < L} F[bin(m)][ring] e^{+i m phi0}.  Cap rings are written into the
-// Bluestein batch as conj(Y_k) conj(b_k) (synthesis = conj(DFT(conj Y))), belt rings into E.
+// inverse fold: Y_ring[k] = sum_{m = k mod n, |m| < L} F[bin(m)][ring] e^{+i m phi0}.  Cap rings go into the Bluestein batch as
+// conj(Y_k) conj(b_k) (synthesis = conj(DFT(conj Y))), belt rings into E.  F is bin-major (rows m, rings contiguous) and the targets are
+// ring-major, so a 32 x 32 tile is read along the rings and, transposed through shared memory, added along k: C and E are zeroed
+// first and every term is added with RED.ADD.F64 (the map is linear; several m fold onto one k wherever n < 2L-1).
 __global__ void k_hp_fold_inv(int nside, int L, int NB, int nth, int ldf, int M, const double2* __restrict__ F,
                               double2* __restrict__ C, double2* __restrict__ E) {
-    const int i = blockIdx.y, k = blockIdx.x * blockDim.x + threadIdx.x;
-    const HpRing g = hp_ring(nside, i);
-    const int width = g.cap >= 0 ? M : g.n;
-    if (k >= width) return;
-    double2 acc = make_double2(0.0, 0.0);
-    if (k < g.n) {
-        int m = k - ((k + (L - 1)) / g.n) * g.n;                  // smallest m >= -(L-1) congruent to k
-        for (; m <= L - 1; m += g.n) {
-            double2 x = F[(size_t)(m < 0 ? m + NB : m) * ldf + i];
-            if (g.shifted) {
-                long long r = ((long long)m) % (2LL * g.n); if (r < 0) r += 2LL * g.n;
-                double s, c; sincospi((double)r / (double)g.n, &s, &c);
-                x = cmul(x, make_double2(c, s));
-            }
-            acc.x += x.x; acc.y += x.y;
-        }
-    }
-    if (g.cap >= 0) {
+    __shared__ double2 tile[32][33];
+    const int i0 = blockIdx.x * 32, mi0 = blockIdx.y * 32;        // mi = m + L - 1
+    for (int q = threadIdx.y; q < 32; q += blockDim.y) {
+        const int mi = mi0 + q, i = i0 + threadIdx.x, m = mi - (L - 1);
         double2 v = make_double2(0.0, 0.0);
-        if (k < g.n) { double2 b = chirp(k, g.n); v = cmulc(make_double2(acc.x, -acc.y), b); }
-        C[(size_t)g.cap * M + k] = v;
-    } else E[(size_t)(i - (nside - 1)) * g.n + k] = acc;
+        if (mi < 2 * L - 1 && i < nth) v = F[(size_t)(m < 0 ? m + NB : m) * ldf + i];
+        tile[q][threadIdx.x] = v;
+    }
+    __syncthreads();
+    for (int q = threadIdx.y; q < 32; q += blockDim.y) {
+        const int i = i0 + q, mi = mi0 + threadIdx.x, m = mi - (L - 1);
+        if (i >= nth || mi >= 2 * L - 1) continue;
+        const HpRing g = hp_ring(nside, i);
+        double2 x = tile[threadIdx.x][q];
+        int k = m % g.n; if (k < 0) k += g.n;
+        if (g.shifted) {
+            long long r = ((long long)m) % (2LL * g.n); if (r < 0) r += 2LL * g.n;
+            double s, c; sincospi((double)r / (double)g.n, &s, &c);
+            x = cmul(x, make_double2(c, s));
+        }
+        double* dst;
+        if (g.cap >= 0) { x = cmulc(make_double2(x.x, -x.y), chirp(k, g.n)); dst = reinterpret_cast<double*>(C + (size_t)g.cap * M + k); }
+        else dst = reinterpret_cast<double*>(E + (size_t)(i - (nside - 1)) * g.n + k);
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(dst), "d"(x.x) : "memory");
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(dst + 1), "d"(x.y) : "memory");
+    }
 }
 // inverse unpack of the cap rings: f_j = conj( conj(b_j) * conv_j ) = b_j * conj(conv_j)
 __global__ void k_hp_unpack_inv(int nside, int M, int real_out, const double2* __restrict__ C, void* __restrict__ map) {
@@ -177,9 +183,13 @@ cudaError_t st_hp_unpack_fwd(int nside, int L, int NB, int mlo, int ldu, int M, 
     count_bytes(16.0 * (double)nth * (L - mlo) + 16.0 * 12.0 * (double)nside * nside); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_fold_inv(int nside, int L, int NB, int ldf, int M, const double2* F, double2* C, double2* E, cudaStream_t st) {
-    const int nth = 4 * nside - 1, width = M > 4 * nside ? M : 4 * nside;
-    k_hp_fold_inv<<<dim3(cdiv(width, 128), nth), 128, 0, st>>>(nside, L, NB, nth, ldf, M, F, C, E);
-    count_bytes(16.0 * (double)nth * NB + 16.0 * ((double)M * 2 * (nside - 1) + 4.0 * nside * (2 * nside + 1))); LAUNCHED(); return cudaSuccess;
+    const int nth = 4 * nside - 1;
+    const size_t cb = sizeof(double2) * (size_t)M * 2 * (nside > 1 ? nside - 1 : 0), eb = sizeof(double2) * 4 * (size_t)nside * (2 * nside + 1);
+    cudaError_t e = cb ? cudaMemsetAsync(C, 0, cb, st) : cudaSuccess;
+    if (e == cudaSuccess) e = cudaMemsetAsync(E, 0, eb, st);
+    if (e != cudaSuccess) return e;
+    k_hp_fold_inv<<<dim3(cdiv(nth, 32), cdiv(2 * L - 1, 32)), dim3(32, 8), 0, st>>>(nside, L, NB, nth, ldf, M, F, C, E);
+    count_bytes(32.0 * (double)nth * (2 * L - 1) + (double)cb + (double)eb); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_hp_unpack_inv(int nside, int M, int real_out, const double2* C, void* map, cudaStream_t st) {
     if (nside < 2) return cudaSuccess;
