@@ -157,6 +157,7 @@ struct sht_plan {
     cufftHandle fft_hp_cap = 0, fft_hp_eq = 0;
     void* fft_work = nullptr; size_t fft_work_bytes = 0;
     cufftHandle fft_phi_inv = 0, fft_phi_fwd = 0, fft_th1 = 0, fft_th2 = 0, fft_gamma = 0;
+    cufftHandle fft_alpha = 0; // SO(3): the ring FFTs of all (gamma / n, beta) rows in ONE batch, on the [slab][ring][phi] layout
     bool have_fft = false;
     std::map<cufftHandle, double> fft_elems;   // complex elements one execution of each handle transforms (byte accounting)
     // workspace
@@ -507,6 +508,8 @@ sht_status make_fft_plans(sht_plan* P) {
         CF(cufftCreate(&P->fft_gamma)); CF(cufftSetAutoAllocation(P->fft_gamma, 0));
         int emb[1] = {2 * P->N - 1};
         CF(cufftMakePlanMany(P->fft_gamma, 1, n3, emb, L * NB, 1, emb, L * NB, 1, CUFFT_Z2Z, L * NB, &w)); P->fft_elems[P->fft_gamma] = (double)(2 * P->N - 1) * L * NB; ws = w > ws ? w : ws;
+        CF(cufftCreate(&P->fft_alpha)); CF(cufftSetAutoAllocation(P->fft_alpha, 0));
+        CF(cufftMakePlanMany(P->fft_alpha, 1, n1, n1, 1, NB, n1, 1, NB, CUFFT_Z2Z, L * P->nslab, &w)); P->fft_elems[P->fft_alpha] = (double)P->nslab * L * NB; ws = w > ws ? w : ws;
     }
     P->fft_work_bytes = ws + 256;
     P->have_fft = true;
@@ -1218,7 +1221,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2})
             if (h) CF(cufftSetWorkArea(h, P->fft_work));
         if (P->invsym) CF(cufftSetWorkArea(P->fft_sym, P->fft_work));
-        if (P->kind == 1) CF(cufftSetWorkArea(P->fft_gamma, P->fft_work));
+        if (P->kind == 1) { CF(cufftSetWorkArea(P->fft_gamma, P->fft_work)); CF(cufftSetWorkArea(P->fft_alpha, P->fft_work)); }
     } else {
         CF(cufftSetWorkArea(P->fft_hp_eq, P->fft_work));
         if (P->hp_ncap > 0) {
@@ -1241,7 +1244,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
 sht_status sht_plan_destroy(sht_plan* P) {
     if (!P) return SHT_OK;
     if (P->have_fft || P->fft_phi_inv) {
-        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_hp_cap, P->fft_hp_eq, P->fft_sym})
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_alpha, P->fft_hp_cap, P->fft_hp_eq, P->fft_sym})
             if (h) cufftDestroy(h);
     }
     for (auto e : P->ev) cudaEventDestroy(e);
@@ -1520,9 +1523,12 @@ static sht_status so3_inverse_body(sht_plan* P, const void* flmn, void* f, sht_s
     stage(P, CAT_STAGE, st);
     // (coefficient slabs are read in place: the staging kernels map gamma-FFT bin order to n order through d_cslab)
     CS(run_theta_inverse(P, (const double2*)flmn, st));
+    // F[n][bin][ring] -> f[n][ring][bin] (one transpose for all slabs), then the gamma transform (Eq. 17) and the ring synthesis of all
+    // (gamma, beta) rows as ONE batched FFT each, in place in the output: 3 FFT launches instead of 2N per direction
+    CK(st_transpose_slabs(P->nslab, NB, L, P->F_ld, NB, P->F, P->F_slab, (double2*)f, slab, st));
     stage(P, CAT_FFT, st);
-    for (int b = 0; b < P->nslab; ++b) CS(fft_exec(P, P->fft_phi_inv, P->F + P->F_slab * b, (double2*)f + slab * b, CUFFT_INVERSE, st));
     CS(fft_exec(P, P->fft_gamma, (double2*)f, (double2*)f, CUFFT_INVERSE, st));          // Eq. 17
+    CS(fft_exec(P, P->fft_alpha, (double2*)f, (double2*)f, CUFFT_INVERSE, st));          // Eq. 32 on every row
     stage(P, CAT_STAGE, st);
     return SHT_OK;
 }
@@ -1533,7 +1539,9 @@ static sht_status so3_forward_body(sht_plan* P, const void* f, void* flmn, sht_s
     begin_transform(P);
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD, st));   // Eq. 16 (q_Gamma in scale_fwd)
-    for (int b = 0; b < P->nslab; ++b) CS(fft_exec(P, P->fft_phi_fwd, P->fn + slab * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
+    CS(fft_exec(P, P->fft_alpha, P->fn, P->fn, CUFFT_FORWARD, st));                            // ring DFTs of all (n, beta) rows, one batch
+    stage(P, CAT_STAGE, st);
+    CK(st_transpose_slabs(P->nslab, L, NB, NB, P->Ltp, P->fn, slab, P->Fa, P->Fa_slab, st));   // fn[n][ring][bin] -> Fa[n][bin][ring]
     CS(mw_upsample(P, st));
     CS(run_theta_forward(P, P->Z, (size_t)P->prow * P->fwd_ld, P->fwd_ld, st, P->pair));
     stage(P, CAT_STAGE, st);

@@ -464,6 +464,22 @@ __global__ void k_finalize_forward(int L, int Lp, const int* __restrict__ slab_n
         if (l < L && mi < NB) coef[(size_t)l * NB + mi] = tile[threadIdx.x][r];
     }
 }
+// 32 x 32 tile transpose of nslab matrices: out[slab][c][r] = in[slab][r][c] (r < nrow, c < ncol; row lengths ldin / ldout)
+__global__ void k_transpose_slabs(int nrow, int ncol, int ldin, int ldout, const double2* __restrict__ in, size_t in_slab,
+                                  double2* __restrict__ out, size_t out_slab) {
+    __shared__ double2 tile[32][33];
+    in += in_slab * blockIdx.z; out += out_slab * blockIdx.z;
+    const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+    for (int q = threadIdx.y; q < 32; q += blockDim.y) {
+        const int r = r0 + q, c = c0 + threadIdx.x;
+        tile[q][threadIdx.x] = (r < nrow && c < ncol) ? in[(size_t)r * ldin + c] : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    for (int q = threadIdx.y; q < 32; q += blockDim.y) {
+        const int c = c0 + q, r = r0 + threadIdx.x;
+        if (c < ncol && r < nrow) out[(size_t)c * ldout + r] = tile[threadIdx.x][q];
+    }
+}
 // generic strided row copy used by the theta-stage entry points: dst[r][c] = src[map(r)][c]
 __global__ void k_rows_bin_to_mi(int L, int NB, int ncol, int ldsrc, int lddst, int to_mi, const double2* __restrict__ src,
                                  double2* __restrict__ dst) {
@@ -907,6 +923,11 @@ cudaError_t st_rows_reorder(int L, int NB, int ncol, int ldsrc, int lddst, int t
     dim3 grid(cdiv(ncol, 128), 2 * L - 1);      // rows r = m + L - 1 of the m-ordered array; NB = number of phi bins of the other one
     k_rows_bin_to_mi<<<grid, 128, 0, st>>>(L, NB, ncol, ldsrc, lddst, to_mi, src, dst);
     count_bytes(32.0 * (double)(2 * L - 1) * ncol); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_transpose_slabs(int nslab, int nrow, int ncol, int ldin, int ldout, const double2* in, size_t in_slab, double2* out,
+                               size_t out_slab, cudaStream_t st) {
+    k_transpose_slabs<<<dim3(cdiv(ncol, 32), cdiv(nrow, 32), nslab), dim3(32, 8), 0, st>>>(nrow, ncol, ldin, ldout, in, in_slab, out, out_slab);
+    count_bytes(32.0 * (double)nrow * ncol * nslab); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_scale_copy(size_t n, double s, const double2* in, double2* out, cudaStream_t st) {
     k_scale_copy<<<cdiv(n, 256), 256, 0, st>>>(n, s, in, out);
