@@ -348,7 +348,7 @@ def main():
     out = None
     if rank == 0:
         hbm, hbm_kind = peaks()
-        pk = {k: api.peak(k, 20000)[0] for k in ("dfma", "dmma", "ffma")}
+        pk = {k: api.peak(k, 20000)[0] for k in ("dfma", "dmma", "ffma", "ffma2")}
         nsm = torch.cuda.get_device_properties(dev).multi_processor_count
         peak_tf = pk["ffma"] if args.dtype == "f32" else pk["dfma"]
         # algorithmic flop: per d-step 6 (recursion) + 4 per order and map served
@@ -369,7 +369,7 @@ def main():
                 "frac_executed_is": f"FP64 instructions the e-form kernel executes ({instr:.0f} per d-step, 2 flop each) / hot time / measured peak: 1.0 = pipe-bound",
                 "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
                 "time_source": "CUDA events recorded inside the library around the hot kernels; median of 5 transforms timed after the K timed steps",
-                "peak_kind": f"measured in this run by register-only chains (sht_peak): DFMA {pk['dfma']:.2f}, DMMA {pk['dmma']:.2f}, FFMA {pk['ffma']:.2f} "
+                "peak_kind": f"measured in this run by register-only chains (sht_peak): DFMA {pk['dfma']:.2f}, DMMA {pk['dmma']:.2f}, FFMA {pk['ffma']:.2f}, FFMA2 (packed f32x2) {pk['ffma2']:.2f} "
                              f"TFLOP/s; nominal {nsm} SM x 64 DFMA/clk x 2 x 1.965 GHz = {nsm * 64 * 2 * 1.965e-3:.1f}",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
                 "inverse_kernel": {"achieved": ach_inv, "frac": ach_inv / peak_tf, "frac_executed": ach_inv * (2.0 * instr / fl) / peak_tf},

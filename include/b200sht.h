@@ -80,7 +80,7 @@ enum {
                                      and one odd function, separated afterwards: half the FFT work); this flag keeps one order
                                      per column */
 };
-enum { SHT_PEAK_DFMA = 0, SHT_PEAK_DMMA = 1, SHT_PEAK_FFMA = 2 };   /* sht_peak kinds */
+enum { SHT_PEAK_DFMA = 0, SHT_PEAK_DMMA = 1, SHT_PEAK_FFMA = 2, SHT_PEAK_FFMA2 = 3 };   /* sht_peak kinds */
 
 typedef struct sht_plan sht_plan;       /* opaque; host object holding sizes, cuFFT handles and table pointers */
 typedef void* sht_stream;               /* a cudaStream_t */
@@ -224,7 +224,8 @@ sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, s
 
 /* ---- measurement helpers: register-only instruction chains, return achieved TFLOP/s and kernel ms (used by bench.py for the
  * roofline denominators, since MEASURED_PEAKS.json has no FP64 / FP32 ALU entries).  kind: SHT_PEAK_DFMA (fma.f64),
- * SHT_PEAK_DMMA (mma.sync.m8n8k4.f64, the FP64 tensor-core path of the batched kernels), SHT_PEAK_FFMA (fma.f32).
+ * SHT_PEAK_DMMA (mma.sync.m8n8k4.f64, the FP64 tensor-core path of the batched kernels), SHT_PEAK_FFMA (fma.f32),
+ * SHT_PEAK_FFMA2 (packed fma.rn.f32x2, the arithmetic of the fp32 kernels: same peak as FFMA, half the issue slots).
  * sht_fp64_peak() is sht_peak(SHT_PEAK_DFMA, ...). */
 sht_status sht_peak(int kind, int iters, double* tflops, float* ms, sht_stream stream);
 sht_status sht_fp64_peak(int iters, double* tflops, float* ms, sht_stream stream);

@@ -274,8 +274,8 @@ def fp64_peak(iters=20000):
 
 
 def peak(kind, iters=20000):
-    """Measured instruction-chain peak: kind 'dfma' | 'dmma' | 'ffma' -> (TFLOP/s, ms)."""
-    code = {"dfma": _lib.SHT_PEAK_DFMA, "dmma": _lib.SHT_PEAK_DMMA, "ffma": _lib.SHT_PEAK_FFMA}[kind]
+    """Measured instruction-chain peak: kind 'dfma' | 'dmma' | 'ffma' | 'ffma2' -> (TFLOP/s, ms)."""
+    code = {"dfma": _lib.SHT_PEAK_DFMA, "dmma": _lib.SHT_PEAK_DMMA, "ffma": _lib.SHT_PEAK_FFMA, "ffma2": _lib.SHT_PEAK_FFMA2}[kind]
     tf, ms = C.c_double(), C.c_float()
     check(lib().sht_peak(code, iters, C.byref(tf), C.byref(ms), _stream()))
     return tf.value, ms.value

@@ -1779,7 +1779,7 @@ sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, s
 }
 
 sht_status sht_peak(int kind, int iters, double* tflops, float* ms, sht_stream stream) {
-    if (!tflops || !ms || iters < 1 || kind < 0 || kind > 2) return SHT_EINVAL;
+    if (!tflops || !ms || iters < 1 || kind < 0 || kind > 3) return SHT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, nsm = 0;
     CK(cudaGetDevice(&dev));

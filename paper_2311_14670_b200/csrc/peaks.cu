@@ -4,6 +4,7 @@
 //   kind 0: DFMA   -- 16 independent fma.rn.f64 chains per thread            (2 flop per instruction and lane)
 //   kind 1: DMMA   -- 8 independent mma.sync.m8n8k4.f64 accumulator chains   (512 flop per warp instruction)
 //   kind 2: FFMA   -- 16 independent fma.rn.f32 chains per thread
+//   kind 3: FFMA2  -- 16 independent fma.rn.f32x2 chains per thread (packed: 4 flop per instruction and lane; theta_f32.cu)
 #include "internal.h"
 
 #include <cuda_runtime.h>
@@ -58,6 +59,21 @@ __global__ void __launch_bounds__(256) peak_ffma_kernel(int iters, double* sink)
     if (s == 123.456f) sink[0] = s;
 }
 
+__global__ void __launch_bounds__(256) peak_ffma2_kernel(int iters, double* sink) {
+    float2 a[16];
+    const float2 x = make_float2(1.0f + 1e-6f * threadIdx.x, 1.0f - 1e-6f * threadIdx.x), y = make_float2(1e-6f * (blockIdx.x + 1), -1e-6f);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = make_float2((float)i, (float)-i);
+    for (int k = 0; k < iters; ++k) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = __ffma2_rn(a[i], x, y);
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i].x + a[i].y;
+    if (s == 123.456f) sink[0] = s;
+}
+
 }  // namespace
 
 cudaError_t launch_peak(int kind, int iters, int nsm, double* sink, cudaStream_t st, double* flop) {
@@ -71,6 +87,9 @@ cudaError_t launch_peak(int kind, int iters, int nsm, double* sink, cudaStream_t
     } else if (kind == 2) {
         peak_ffma_kernel<<<blocks, threads, 0, st>>>(iters, sink);
         *flop = 2.0 * 16 * (double)iters * blocks * threads;
+    } else if (kind == 3) {
+        peak_ffma2_kernel<<<blocks, threads, 0, st>>>(iters, sink);
+        *flop = 4.0 * 16 * (double)iters * blocks * threads;
     } else
         return cudaErrorInvalidValue;
     count_launch();
