@@ -59,9 +59,11 @@ enum { SHT_F64 = 0, SHT_F32 = 1 };      /* dtype    */
 enum {
     SHT_OPT_FOLD_ON  = 1u << 0,   /* spin 0: run the recursion on the northern rings only (north-south fold) ...   */
     SHT_OPT_FOLD_OFF = 1u << 1,   /* ... or on all rings.  Default: folded when the northern half alone fills the GPU (MW: L >= 2048) */
-    SHT_OPT_INVSYM   = 1u << 2,   /* spin-0 MW inverse on the L midpoint rings (2j+1)pi/(2L) with the fold, then an exact FFT
-                                     resampling of F_m to the MW rings.  Default where the fold is on (L >= 2048) ...               */
-    SHT_OPT_NO_INVSYM = 1u << 7,  /* ... this flag keeps the inverse on the MW rings themselves (needed for ring shards)            */
+    SHT_OPT_INVSYM   = 1u << 2,   /* MW inverse on the L midpoint rings (2j+1)pi/(2L), which are symmetric about the equator -- spin 0: north-south
+                                     fold; spin != 0: ONE pass serves order +m at a ring and -m at its mirror ring instead of two passes
+                                      -- then an exact FFT resampling of F_m to the MW rings.  Default from L >= 2048 ...       */
+    SHT_OPT_NO_INVSYM = 1u << 7,  /* ... this flag keeps the inverse on the rings of the map, every kernel ring written by its own recursion only
+                                     (needed for ring shards; on MWSS / DH / GL / HEALPix it selects two passes for spin != 0)             */
     SHT_OPT_TILE64   = 1u << 3,   /* force 64-ring block tiles in the fused kernels ...                                          */
     SHT_OPT_TILE128  = 1u << 4,   /* ... or 128-ring tiles.  Default: 64 when 128-ring tiles give fewer blocks than the device has SMs */
     SHT_OPT_PRECOMPUTE = 1u << 6, /* the paper's full-precomputation mode (Sec. 4.3): the Wigner d-functions of every

@@ -179,7 +179,7 @@ __global__ void k_prep_inverse(int L, int Lp, int NC, int mmin, const double2* _
                                const double2* __restrict__ SG, int sgstride, const ThetaPass* __restrict__ passes) {
     // one launch serves all passes of a kernel mode: grid.z = pass (its operand rows start one row into ThetaPass::in)
     const ThetaPass P = passes[blockIdx.z];
-    const int n = P.n, sgn_out = P.sgn_out, m_end = P.m_end;
+    const int n = P.n, sgn_out = P.sgn_out, m_end = P.m_end, fold = P.fold;
     const double2* coef = coef_base + (size_t)cslab[P.slab] * coef_slab;
     double* G = const_cast<double*>(P.in) + (size_t)Lp * (2 * NC + 2);
     if (m_end + (int)blockIdx.y * 32 >= L) return;
@@ -192,7 +192,7 @@ __global__ void k_prep_inverse(int L, int Lp, int NC, int mmin, const double2* _
             const int m_out = (c == 1 || sgn_out < 0) ? -m : m;
             double2 v = make_double2(0.0, 0.0);
             const int am = m < 0 ? -m : m;
-            if (l < L && m < L && l >= an && l >= am && !(c == 1 && m == 0)) v = coef[(size_t)l * NB + m_out + L - 1];
+            if (l < L && m < L && l >= an && l >= am && !(c == 1 && m == 0 && !fold)) v = coef[(size_t)l * NB + m_out + L - 1];
             tile[c][q][threadIdx.x] = v;
         }
     __syncthreads();
@@ -204,7 +204,7 @@ __global__ void k_prep_inverse(int L, int Lp, int NC, int mmin, const double2* _
         const double cm = l < L ? scale[l] * C[(size_t)(m - mmin) * Lp + l] : 0.0;
         for (int c = 0; c < NC; ++c) {
             double sgn = 1.0;
-            if (c == 1) sgn = sgn_pow(m);
+            if (c == 1) sgn = fold ? sgn_pow(l - n) : sgn_pow(m);      // fold pass: F_{-m}(pi - theta) = sum_l (-1)^{l-n} f_{l,-m} d^l_{m,n}(theta)
             else if (sgn_out < 0) sgn = sgn_pow(m + n);
             const double2 x = tile[c][threadIdx.x][q];
             g[2 * c] = sgn * cm * x.x; g[2 * c + 1] = sgn * cm * x.y;

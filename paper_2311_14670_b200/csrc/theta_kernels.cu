@@ -112,7 +112,10 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             valid[q] = th < A.nth && o < NOUT && th >= A.th_lo && th < A.th_hi;
             mlo[q] = P.m_lo ? P.m_lo[th] : -(1 << 30);
             if (mlo[q] < m_end) mlo[q] = m_end;
-            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)th * 2;
+            // fold pass (n != 0, ring set symmetric about the equator): the -m column is F_{-m} of the MIRRORED ring pi - theta, served by the
+            // same d-value (d^l_{-m,n}(pi - theta) = (-1)^{l-n} d^l_{m,n}(theta); the sign rides on the operand) for m > m_s(theta)
+            if (NC == 2 && P.fold && neg[q]) mlo[q] += 1;
+            obase[q] = reinterpret_cast<double*>(P.out) + (size_t)((NC == 2 && P.fold && neg[q] && th < A.nth) ? A.nth - 1 - th : th) * 2;
             const int tm = A.nfull - 1 - th;
             south[q] = FOLD && tm != th;              // the equator ring of an odd ring count mirrors itself
             osouth[q] = ((ptrdiff_t)tm - th) * 2;
@@ -150,7 +153,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
                 if (any) {
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
-                        if (valid[q] && m >= mlo[q] && !(neg[q] && m == 0)) {
+                        if (valid[q] && m >= mlo[q] && !(neg[q] && m == 0 && !P.fold)) {
                             const int m_out = (NC == 2) ? (neg[q] ? -m : m) : P.sgn_out * m;
                             const int row = m_out < 0 ? m_out + A.NB : m_out;
                             double* o = obase[q] + (size_t)row * A.ldout * 2;

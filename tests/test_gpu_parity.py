@@ -252,6 +252,20 @@ def test_mw_spin0_inverse_with_and_without_symmetric_rings(api, orc, sym, L, rea
     assert rel(F, orc.s2_theta_inverse_columns(L, 0, orc.MW, flm, np.arange(-(L - 1), L))) < TOL
 
 
+@pytest.mark.parametrize("sym", [False, True])
+@pytest.mark.parametrize("L,spin", [(2, 1), (3, -2), (9, 1), (33, 2), (64, -1), (65, 3), (130, -2), (200, 1), (257, 2)])
+def test_mw_spin_inverse_with_two_passes_or_one_fold_pass_on_symmetric_rings(api, orc, sym, L, spin):
+    """spin != 0 MW inverse: two passes (second index n and -n) on the MW rings (SHT_OPT_NO_INVSYM; default below L = 2048), or ONE fold pass
+    on the L midpoint rings -- order +m at a ring, order -m at its mirror ring, d^l_{-m,n}(pi - theta) = (-1)^{l-n} d^l_{m,n}(theta), PAPER.md:236 --
+    followed by the exact FFT resampling to the MW rings (SHT_OPT_INVSYM; default from L = 2048).  Both against the oracle, element by element,
+    through the full transform and through the theta-stage entry point."""
+    flm = synth.random_flm(L, spin, seed=3 * L + spin)
+    P = api.Plan(L, spin, invsym=sym)
+    assert rel(P.inverse(dev(flm)).cpu().numpy(), orc.s2_inverse(L, spin, orc.MW, flm)) < TOL
+    F = P.theta_inverse(dev(flm)).cpu().numpy()
+    assert rel(F, orc.s2_theta_inverse_columns(L, spin, orc.MW, flm, np.arange(-(L - 1), L))) < TOL
+
+
 @pytest.mark.parametrize("pair", [False, True])
 @pytest.mark.parametrize("L,spin,fold,real", [(1, 0, None, False), (2, 0, None, False), (9, 1, None, False), (33, 0, True, False), (64, -2, None, False),
                                               (130, 0, True, True), (131, 3, None, False), (200, 0, False, False)])
@@ -261,7 +275,7 @@ def test_mw_theta_ffts_with_one_or_two_orders_per_column(api, orc, pair, L, spin
     (default); SHT_OPT_NO_PAIR keeps one order per column.  Both against the oracle, on raw white noise (forward) and through the
     symmetric-ring inverse (spin 0)."""
     f = synth.random_map((L, 2 * L - 1), seed=11 + L, real=real)
-    P = api.Plan(L, spin, reality=real, fold=fold, pair=pair, invsym=True if spin == 0 else None)
+    P = api.Plan(L, spin, reality=real, fold=fold, pair=pair, invsym=True)
     want = orc.s2_forward(L, spin, orc.MW, project_mw_pole(f, spin).astype(np.complex128))
     assert rel(P.forward(dev(f)).cpu().numpy(), want) < TOL
     flm = synth.random_flm(L, spin, seed=2 * L + 1, real=real)
