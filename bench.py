@@ -219,7 +219,7 @@ def sweep(api, synth, torch, dev, flush, pk):
         return torch.from_numpy(synth.random_flm(L, spin, seed=seed, sigma=sigma)).to(dev)
 
     for L, spin, sigma, seed, tag in ((64, 0, synth.SIGMA_UNIT, 0, "configs[0] "), (1024, 2, synth.SIGMA_CMB, 1, "configs[1] "),
-                                      (2048, 0, synth.SIGMA_RED, 4, ""), (4096, 0, synth.SIGMA_RED, 4, "")):
+                                      (2048, 0, synth.SIGMA_RED, 4, ""), (2048, 2, synth.SIGMA_CMB, 1, ""), (4096, 0, synth.SIGMA_RED, 4, "")):
         x = mw(L, spin, sigma, seed)
         P = api.Plan(L, spin, device=dev)
         add(f"{tag}MW spin-{spin} L={L} fp64", P, x, pk["dfma"])

@@ -34,9 +34,10 @@
 //
 // Parity pins (tests, -m "not gpu"): closed-form Y_lm / sY_lm, scipy sph_harm_y, Jacobi form (Eq. 22) through
 // scipy/mpmath, d(0)=I, d(pi), symmetries, orthogonality, E==R==T, un-separated sums, quadrature exactness,
-// exact MW / SO(3) round trips (sampling theorem).  HEALPix forward: "parity unpinned" in the absolute beyond
-// normalisation (constant map), geometry and the shared, pinned, Y_lm -- the scheme has no sampling theorem
-// (PAPER.md:172); see DESIGN.md.
+// exact MW / SO(3) round trips (sampling theorem).  HEALPix forward: the scheme has no sampling theorem, so it is
+// pinned by normalisation (constant map), geometry, the shared, pinned, Y_lm, and by CONVERGENCE: the forward of a synthesised
+// band-limited map converges to the generating coefficients at second order in the pixel size (error / 4 per doubling of nside),
+// test_oracle_s2.py::test_healpix_forward_converges_to_the_generating_coefficients; see DESIGN.md.
 //
 // Build: python oracle/build.py   (g++ -O2 -fopenmp -shared -fPIC)
 #include <cmath>
