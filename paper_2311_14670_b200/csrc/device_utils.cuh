@@ -36,6 +36,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
             : "memory");
     } while (!ok);
 }
+// the same for a warp with slack (the reducers waiting for the compute warps): back off between polls instead of spinning, so that the
+// polling loop does not compete with the compute warps of the same scheduler for issue slots
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    for (;;) {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+        if (ok) break;
+        __nanosleep(100);
+    }
+}
 // fire-and-forget fp64 add to GLOBAL memory (SASS RED.E.ADD.F64)
 __device__ __forceinline__ void red_add_f64(double* gptr, double v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gptr), "d"(v) : "memory");

@@ -26,7 +26,8 @@ namespace {
 using namespace shtdev;
 
 constexpr int NST = 4;   // stages of the operand ring
-constexpr int NRS = 2;   // stages of the partial-sum hand-off
+constexpr int NRS = 4;   // stages of the partial-sum hand-off of the forward kernel (131 KB; 2 -> 4: config 2 forward 0.814 -> 0.796 ms, L = 4096 19.34 -> 19.23 ms;
+                         // starting half of the compute warps half a pair late, so that the two warps of a scheduler interleave, LOSES 7 % at either depth)
 constexpr int KS = 2;    // recursion steps per pipeline stage (one TMA barrier, one hand-off per KS steps)
 constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
 
@@ -395,7 +396,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) cn[h][q] = crow[-(ptrdiff_t)h * A.Lp + lq[q]];
             }
-            mbar_wait(&sm.rfull[rs], (p / NRS) & 1);
+            mbar_wait_relaxed(&sm.rfull[rs], (p / NRS) & 1);      // (forward: -0.7 ... -1.5 % with the back-off; the inverse reducers are on the critical path: +2 %)
             int actb[NW];
 #pragma unroll
             for (int ww = 0; ww < NW; ++ww) actb[ww] = sm.act[rs][ww];

@@ -49,6 +49,7 @@ def test_status_strings_and_argument_validation(lib):
     assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 0, 1, 1 | 2) == 1      # SHT_OPT_FOLD_ON with SHT_OPT_FOLD_OFF
     assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 0, 1, 4 | 128) == 1    # SHT_OPT_INVSYM with SHT_OPT_NO_INVSYM
     assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 1, 1, 64) == 2         # precompute is fp64 only
+    assert lib.sht_plan_s2_opts(C.byref(h), 8, 0, 0, 0, 0, 0, 1, 512 | 1024) == 1 # SHT_OPT_GRAPH with SHT_OPT_NO_GRAPH
     assert lib.sht_plan_set_shard(None, 0, 1) == 1
     assert lib.sht_peak(7, 10, None, None, None) == 1
     assert lib.sht_plan_workspace_bytes(None) == 0
