@@ -41,12 +41,12 @@ def test_random_plan_options_vs_oracle(orc, samp, L, spin, real, nside, kw):
     gs, os_ = {"mw": (api.MW, orc.MW), "mwss": (api.MWSS, orc.MWSS), "dh": (api.DH, orc.DH), "gl": (api.GL, orc.GL), "hp": (api.HEALPIX, orc.HEALPIX)}[samp]
     P = api.Plan(L, spin, sampling=gs, nside=nside, reality=real, **kw)
     okw = dict(nside=nside) if samp == "hp" else {}
-    flm = synth.random_flm(L, spin, seed=L + 11 * spin, real=real)
+    flm = synth.random_flm(L, spin, seed=100 + L + 11 * spin, real=real)
     ref = orc.s2_inverse(L, spin, os_, flm, **okw)
     got = P.inverse(torch.from_numpy(flm).cuda()).cpu().numpy()
     assert rel(got, ref.real if real else ref) < TOL
     shape = (12 * nside * nside,) if samp == "hp" else orc.map_shape(os_, L)
-    g = synth.random_map(shape, seed=3 * L + spin, real=real)
+    g = synth.random_map(shape, seed=100 + 3 * L + spin, real=real)
     gp = project_mw_pole(g, spin) if samp == "mw" else project_mwss_poles(g, spin) if samp == "mwss" else g
     want = orc.s2_forward(L, spin, os_, gp.astype(np.complex128), **okw)
     back = P.forward(torch.from_numpy(g).cuda()).cpu().numpy()
