@@ -102,6 +102,8 @@ const char* sht_last_error(void);       /* text of the last CUDA / cuFFT failure
  */
 sht_status sht_plan_s2(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype);
 sht_status sht_plan_so3(sht_plan** plan, int L, int N, int dtype);
+/* the same with option flags: SHT_OPT_ADJOINT (the Wigner adjoints below), SHT_OPT_GRAPH / SHT_OPT_NO_GRAPH; others are ignored */
+sht_status sht_plan_so3_opts(sht_plan** plan, int L, int N, int dtype, unsigned opts);
 /* A batch of `batch` S^2 problems with identical (L, spin, sampling, reality) transformed together (BASELINE config 5b):
  * the Wigner-d recursion is run once and shared by all maps, which turns the theta / l contraction of Eq. 30 / 33
  * into a dense GEMM per harmonic order m (the einsum of Sec. 4.3, without storing the d-functions); it
@@ -188,6 +190,12 @@ sht_status s2_forward_adjoint_plan(sht_plan* plan, const void* flm, void* f, sht
 sht_status s2_inverse_adjoint_plan(sht_plan* plan, const void* f, void* flm, sht_stream stream);
 sht_status s2_theta_forward_adjoint_plan(sht_plan* plan, const void* flm, void* Wm, sht_stream stream);
 sht_status s2_theta_inverse_adjoint_plan(sht_plan* plan, const void* Fm, void* flm, sht_stream stream);
+/* Wigner transforms (plans from sht_plan_so3_opts with SHT_OPT_ADJOINT): W^H (flmn -> f) and (W^-1)^H (f -> flmn).  Per order n of the
+ * gamma transform the Wigner transform is a spin transform with second index n (Eq. 15-18), so its adjoint is the
+ * transposed chain: the l-scaling, the S^2 adjoint above for s = -n (one internal S^2 adjoint plan per n, inside the same workspace),
+ * the transposed gamma DFT.  Identities (tests): <W x, y> = <x, W^H y>, <W^-1 c, g> = <c, (W^-1)^H g>. */
+sht_status so3_forward_adjoint_plan(sht_plan* plan, const void* flmn, void* f, sht_stream stream);
+sht_status so3_inverse_adjoint_plan(sht_plan* plan, const void* f, void* flmn, sht_stream stream);
 
 /* Stage timing.  After sht_plan_enable_timing(plan, 1) every transform records CUDA events between its stages;
  * sht_plan_timings() synchronises on the last transform's final event and returns milliseconds:

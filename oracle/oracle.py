@@ -273,3 +273,45 @@ def so3_forward(L, N, f):
     flmn = np.zeros((2 * N - 1, L, 2 * L - 1), dtype=np.complex128)
     _check(lib().orc_so3_forward(L, N, _pd(f), _pd(flmn)), "so3_forward")
     return flmn
+
+
+# ---- SO(3) adjoints: the transposed chains of Eq. 15-18, step by step in reverse order ----
+# The Wigner transform is, per order n of the gamma transform (Eq. 16), a spin transform with second index n (Eq. 15 / 18): with
+# s = -n, W_n = (2 pi / (2N-1)) / p_s(l) * F_s and (W^-1)_n = F_s^-1 * ((2l+1)/(8 pi^2)) / p_s(l), p_s(l) = (-1)^s sqrt((2l+1)/(4 pi)) the
+# prefactor of Eq. 30 / 33 (that relation is pinned in tests/test_oracle_so3.py).  The adjoints below transpose exactly that chain with
+# the oracle's own (pinned) S^2 adjoints and plain gamma sums; they are pinned by the dot-product identity against so3_forward /
+# so3_inverse (tests/test_oracle_adjoint.py).
+def _so3_diag(L, n, num):
+    l = np.arange(L, dtype=np.float64)
+    p = (-1.0) ** n * np.sqrt((2 * l + 1) / (4 * np.pi))
+    return (num(l) / p)[:, None]
+
+
+def so3_forward_adjoint(L, N, flmn):
+    """W^H: coefficients flmn[2N-1, L, 2L-1] -> f[2N-1 (gamma), L (beta), 2L-1 (alpha)], the conjugate transpose of so3_forward."""
+    flmn = _c128(flmn, (2 * N - 1, L, 2 * L - 1))
+    NG = 2 * N - 1
+    g_n = np.zeros((NG, L, 2 * L - 1), dtype=np.complex128)
+    for ni in range(NG):
+        n = ni - (N - 1)
+        y = flmn[ni] * _so3_diag(L, n, lambda l: np.full_like(l, 2 * np.pi / NG))       # transpose of the l-scaling (real, diagonal)
+        g_n[ni] = s2_forward_adjoint(L, -n, 0, y)                                            # transpose of the spin transform with s = -n
+    gam = 2 * np.pi * np.arange(NG) / NG
+    ns = np.arange(NG) - (N - 1)
+    # transpose of f_n = sum_g f e^{-i n gamma_g}:  f[g] = sum_n e^{+i n gamma_g} g_n
+    return np.einsum("gn,nba->gba", np.exp(1j * np.outer(gam, ns)), g_n)
+
+
+def so3_inverse_adjoint(L, N, f):
+    """(W^-1)^H: f[2N-1, L, 2L-1] -> coefficients flmn[2N-1, L, 2L-1], the conjugate transpose of so3_inverse."""
+    f = _c128(f, (2 * N - 1, L, 2 * L - 1))
+    NG = 2 * N - 1
+    gam = 2 * np.pi * np.arange(NG) / NG
+    ns = np.arange(NG) - (N - 1)
+    h_n = np.einsum("ng,gba->nba", np.exp(-1j * np.outer(ns, gam)), f)                       # transpose of f = sum_n e^{+i n gamma_g} (...)
+    out = np.zeros((NG, L, 2 * L - 1), dtype=np.complex128)
+    for ni in range(NG):
+        n = ni - (N - 1)
+        c = s2_inverse_adjoint(L, -n, 0, h_n[ni])
+        out[ni] = c * _so3_diag(L, n, lambda l: (2 * l + 1) / (8 * np.pi ** 2))
+    return out

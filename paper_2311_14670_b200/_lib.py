@@ -19,6 +19,9 @@ SIGNATURES = {
     "sht_last_error": (C.c_char_p, []),
     "sht_plan_s2": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i]),
     "sht_plan_so3": (_i, [C.POINTER(_vp), _i, _i, _i]),
+    "sht_plan_so3_opts": (_i, [C.POINTER(_vp), _i, _i, _i, C.c_uint]),
+    "so3_forward_adjoint_plan": (_i, [_vp, _vp, _vp, _vp]),
+    "so3_inverse_adjoint_plan": (_i, [_vp, _vp, _vp, _vp]),
     "sht_plan_s2_batch": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i, _i]),
     "sht_plan_s2_opts": (_i, [C.POINTER(_vp), _i, _i, _i, _i, _i, _i, _i, C.c_uint]),
     "sht_plan_batch": (_i, [_vp]),

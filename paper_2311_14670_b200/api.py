@@ -70,7 +70,7 @@ class Plan:
             if N is None:
                 check(L_.sht_plan_s2_opts(C.byref(self._h), L, spin, sampling, nside, int(self.reality), code, self.batch, opts))
             else:
-                check(L_.sht_plan_so3(C.byref(self._h), L, N, code))
+                check(L_.sht_plan_so3_opts(C.byref(self._h), L, N, code, opts))
             nbytes = L_.sht_plan_workspace_bytes(self._h)
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             check(L_.sht_plan_set_workspace(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes, _stream()))
@@ -117,14 +117,16 @@ class Plan:
     def forward_adjoint(self, flm, out=None):
         """F^H: coefficients -> map (the conjugate transpose of forward)."""
         out = torch.empty(self.map_shape, dtype=self.map_dtype, device=self.device) if out is None else out
-        check(lib().s2_forward_adjoint_plan(self._h, _dev(flm, self.coef_dtype, self.coef_shape, "flm"),
+        fn = lib().s2_forward_adjoint_plan if self.N is None else lib().so3_forward_adjoint_plan
+        check(fn(self._h, _dev(flm, self.coef_dtype, self.coef_shape, "flm"),
                                             _dev(out, self.map_dtype, self.map_shape, "f"), _stream()))
         return out
 
     def inverse_adjoint(self, f, out=None):
         """(F^-1)^H: map -> coefficients (the conjugate transpose of inverse)."""
         out = torch.empty(self.coef_shape, dtype=self.coef_dtype, device=self.device) if out is None else out
-        check(lib().s2_inverse_adjoint_plan(self._h, _dev(f, self.map_dtype, self.map_shape, "f"),
+        fn = lib().s2_inverse_adjoint_plan if self.N is None else lib().so3_inverse_adjoint_plan
+        check(fn(self._h, _dev(f, self.map_dtype, self.map_shape, "f"),
                                             _dev(out, self.coef_dtype, self.coef_shape, "flm"), _stream()))
         return out
 

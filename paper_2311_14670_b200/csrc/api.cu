@@ -112,6 +112,11 @@ struct sht_plan {
     // rings of the map): adj_inv runs the FORWARD-type kernel on the rings of the map ((F^-1)^H, Eq. 58), adj_fwd runs the
     // INVERSE-type kernel on the 2L quadrature rings (F^H, Eq. 52).  A helper owns only the tables / buffers of its one direction.
     sht_plan *adj_inv = nullptr, *adj_fwd = nullptr;
+    // SO(3) plans with SHT_OPT_ADJOINT: one S^2 adjoint plan per order n (spin -n), the l-scalings between the Wigner and the spin
+    // normalisations (for even n; odd n flips the sign), one coefficient slab of scratch
+    std::vector<sht_plan*> sub;
+    double *so3_dfwd = nullptr, *so3_dinv = nullptr;
+    double2* adj_tmp = nullptr;
     bool helper = false;
     int only_dir = 0;          // helper plans: 1 = inverse-type kernel only, 2 = forward-type kernel only
     double *it_map = nullptr, *it_coef = nullptr;   // HEALPix iterative refinement: residual map / coefficient update scratch
@@ -423,9 +428,14 @@ void layout(sht_plan* P, char* base) {
         for (size_t i = 0; i < P->pinv.size(); ++i) P->pinv[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_inv[i]);
         for (size_t i = 0; i < P->pfwd.size(); ++i) P->pfwd[i].p.out = reinterpret_cast<double2*>(P->Ob + P->ob_off_fwd[i]);
     }
+    if (!P->sub.empty()) {
+        P->so3_dfwd = B.take<double>(L); P->so3_dinv = B.take<double>(L);
+        P->adj_tmp = B.take<double2>((size_t)L * P->M);
+    }
     // the helper plans of the adjoints live at the end of the same workspace
     for (sht_plan* Q : {P->adj_inv, P->adj_fwd})
         if (Q) { B.off = rup(B.off, 256); Q->work = base ? base + B.off : nullptr; B.off += Q->need_bytes; }
+    for (sht_plan* Q : P->sub) { B.off = rup(B.off, 256); Q->work = base ? base + B.off : nullptr; B.off += Q->need_bytes; }
     P->need_bytes = rup(B.off, 256);
 }
 
@@ -1111,7 +1121,8 @@ sht_status sht_plan_s2_opts(sht_plan** out, int L, int spin, int sampling, int n
     return make_s2_plan(out, L, spin, sampling, nside, reality, dtype, batch, opts, 0, false);
 }
 
-sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
+sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) { return sht_plan_so3_opts(out, L, N, dtype, 0u); }
+sht_status sht_plan_so3_opts(sht_plan** out, int L, int N, int dtype, unsigned opts) {
     if (!out) return SHT_EINVAL;
     *out = nullptr;
     if (L < 1 || L > 16384 || N < 1 || N > L) return SHT_EINVAL;
@@ -1123,8 +1134,17 @@ sht_status sht_plan_so3(sht_plan** out, int L, int N, int dtype) {
     query_device(P);
     rings_mw(P->inv, L); rings_mid(P->fwd, 2 * L);
     P->pair = 1;
-    P->use_graph = L <= 512;
-    sht_status s = check_start_range(P);
+    P->opts = opts & (SHT_OPT_ADJOINT | SHT_OPT_GRAPH | SHT_OPT_NO_GRAPH);
+    P->use_graph = (L <= 512 && !(opts & SHT_OPT_NO_GRAPH)) || (opts & SHT_OPT_GRAPH);
+    sht_status s = ((opts & SHT_OPT_GRAPH) && (opts & SHT_OPT_NO_GRAPH)) ? SHT_EINVAL : check_start_range(P);
+    if (s == SHT_OK && (opts & SHT_OPT_ADJOINT)) {
+        // Wigner adjoints: per order n the transposed spin transform with s = -n (Eq. 15-18), through one S^2 adjoint plan each
+        for (int b = 0; b < P->nslab && s == SHT_OK; ++b) {
+            sht_plan* Q = nullptr;
+            s = make_s2_plan(&Q, L, -P->slab_n[b], SHT_MW, 0, 0, SHT_F64, 1, SHT_OPT_ADJOINT | SHT_OPT_NO_GRAPH, 0, false);
+            if (Q) P->sub.push_back(Q);
+        }
+    }
     if (s == SHT_OK) s = plan_common(P);
     if (s != SHT_OK) { sht_plan_destroy(P); return s; }
     *out = P;
@@ -1229,6 +1249,17 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     }
     for (sht_plan* Q : {P->adj_inv, P->adj_fwd})
         if (Q) CS(sht_plan_set_workspace(Q, Q->work, Q->need_bytes, stream));
+    if (!P->sub.empty()) {
+        // Wigner vs spin normalisation (n even): W_n = (q_Gamma / p(l)) F_s, (W^-1)_n = F_s^-1 ((2l+1)/(8 pi^2) / p(l)), p(l) = sqrt((2l+1)/(4 pi))
+        std::vector<double> df(L), di(L);
+        for (int l = 0; l < L; ++l) {
+            const ld p = sqrtl((ld)(2 * l + 1) / (4 * PI_L));
+            df[l] = (double)((2 * PI_L / (ld)(2 * P->N - 1)) / p);
+            di[l] = (double)(((ld)(2 * l + 1) / (8 * PI_L * PI_L)) / p);
+        }
+        CS(up(df, P->so3_dfwd, st)); CS(up(di, P->so3_dinv, st));
+        for (sht_plan* Q : P->sub) CS(sht_plan_set_workspace(Q, Q->work, Q->need_bytes, stream));
+    }
     if (P->dtype == SHT_F32) {
         CK(st_ab32(L, Lp, P->ab32, st));
         CK(st_start32((size_t)Lp * P->inv.ntp, P->inv.start[0].val, P->inv.start[0].k, P->st32_inv, P->k16_inv, st));
@@ -1270,6 +1301,7 @@ sht_status sht_plan_destroy(sht_plan* P) {
     for (auto& g : P->graphs) cudaGraphExecDestroy(g.exec);
     if (P->cap_stream) cudaStreamDestroy(P->cap_stream);
     sht_plan_destroy(P->adj_inv); sht_plan_destroy(P->adj_fwd);
+    for (sht_plan* Q : P->sub) sht_plan_destroy(Q);
     delete P;
     return SHT_OK;
 }
@@ -1533,6 +1565,35 @@ sht_status s2_forward_adjoint_plan(sht_plan* P, const void* flm, void* f, sht_st
     CS(fft_exec(P, P->fft_th1, P->X, P->X, CUFFT_INVERSE, st));
     CK(st_adj_fold(L, P->slab_n[0], mwss, P->NB, P->nrmap, P->F_ld, P->X, P->F, st));
     return fft_exec(P, P->fft_phi_inv, P->F, (double2*)f, CUFFT_INVERSE, st);
+}
+
+// ---- Wigner adjoints -------------------------------------------------------------------------------------------------
+sht_status so3_forward_adjoint_plan(sht_plan* P, const void* flmn, void* f, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+    if (P->sub.empty()) { g_err = "plan was not created with SHT_OPT_ADJOINT"; return SHT_EUNSUPPORTED; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t slab = (size_t)P->L * P->NB;
+    for (int b = 0; b < P->nslab; ++b) {             // internal slabs are in gamma-FFT bin order, the coefficient array in n order
+        const int n = P->slab_n[b];
+        CK(st_scale_rows(P->L, P->M, (n & 1) ? -1.0 : 1.0, P->so3_dfwd, (const double2*)flmn + (size_t)(n + P->N - 1) * slab, P->adj_tmp, st));
+        CS(s2_forward_adjoint_plan(P->sub[b], P->adj_tmp, (double2*)f + slab * b, stream));
+    }
+    return fft_exec(P, P->fft_gamma, (double2*)f, (double2*)f, CUFFT_INVERSE, st);      // transpose of f_n = sum_g f e^{-i n gamma_g}
+}
+sht_status so3_inverse_adjoint_plan(sht_plan* P, const void* f, void* flmn, sht_stream stream) {
+    CS(check_ready(P));
+    if (!flmn || !f || P->kind != 1) return SHT_EINVAL;
+    if (P->sub.empty()) { g_err = "plan was not created with SHT_OPT_ADJOINT"; return SHT_EUNSUPPORTED; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t slab = (size_t)P->L * P->NB;
+    CS(fft_exec(P, P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD, st));   // transpose of f = sum_n e^{+i n gamma_g} (...)
+    for (int b = 0; b < P->nslab; ++b) {
+        const int n = P->slab_n[b];
+        CS(s2_inverse_adjoint_plan(P->sub[b], P->fn + slab * b, P->adj_tmp, stream));
+        CK(st_scale_rows(P->L, P->M, (n & 1) ? -1.0 : 1.0, P->so3_dinv, P->adj_tmp, (double2*)flmn + (size_t)(n + P->N - 1) * slab, st));
+    }
+    return SHT_OK;
 }
 
 // ---- SO(3) (Eq. 15-18) ----------------------------------------------------------------------------

@@ -498,6 +498,14 @@ __global__ void k_scale_copy(size_t n, double s, const double2* __restrict__ in,
 
 // ---- adjoint transforms (Sec. 5.3): conjugate transposes of the staging steps above -------------------------------
 // F[row][c] *= w[c]: the diagonal operator Q of Eq. 52 on the rings of the map (direct-quadrature samplings)
+// out[l][c] = sgn * d[l] * in[l][c]  (row-wise l-scaling of a coefficient slab; SO(3) adjoints)
+__global__ void k_scale_rows(int nrow, int ncol, double sgn, const double* __restrict__ d, const double2* __restrict__ in, double2* __restrict__ out) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x, l = blockIdx.y;
+    if (c >= ncol) return;
+    const double s = sgn * d[l];
+    const double2 v = in[(size_t)l * ncol + c];
+    out[(size_t)l * ncol + c] = make_double2(s * v.x, s * v.y);
+}
 __global__ void k_scale_cols(int ncol, int ld, const double* __restrict__ w, double2* __restrict__ F) {
     int c = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y;
     if (c >= ncol) return;
@@ -1013,6 +1021,10 @@ cudaError_t st_sym_unpair(int L, int n, int ldout, const double2* X, double2* F,
 cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st) {
     k_rows_head<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ldin, ldout, in, out);
     count_bytes(32.0 * (double)nrows * ncol); LAUNCHED(); return cudaSuccess;
+}
+cudaError_t st_scale_rows(int nrow, int ncol, double sgn, const double* d, const double2* in, double2* out, cudaStream_t st) {
+    k_scale_rows<<<dim3(cdiv(ncol, 128), nrow), 128, 0, st>>>(nrow, ncol, sgn, d, in, out);
+    count_bytes(32.0 * (double)nrow * ncol); LAUNCHED(); return cudaSuccess;
 }
 cudaError_t st_scale_cols(int nrows, int ncol, int ld, const double* w, double2* F, cudaStream_t st) {
     k_scale_cols<<<dim3(cdiv(ncol, 128), nrows), 128, 0, st>>>(ncol, ld, w, F);

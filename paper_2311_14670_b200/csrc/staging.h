@@ -49,6 +49,7 @@ cudaError_t st_vec_add(size_t n, const double* x, double* y, cudaStream_t st);
 cudaError_t st_sym_extend(int L, int n, int pair, int ldin, const double2* F, double2* X, cudaStream_t st);
 cudaError_t st_sym_rebin(int L, int rows, const double2* Y, double2* Z, cudaStream_t st);
 cudaError_t st_sym_unpair(int L, int n, int ldout, const double2* X, double2* F, cudaStream_t st);
+cudaError_t st_scale_rows(int nrow, int ncol, double sgn, const double* d, const double2* in, double2* out, cudaStream_t st);
 cudaError_t st_transpose_slabs(int nslab, int nrow, int ncol, int ldin, int ldout, const double2* in, size_t in_slab, double2* out,
                                size_t out_slab, cudaStream_t st);
 cudaError_t st_rows_head(int nrows, int ncol, int ldin, int ldout, const double2* in, double2* out, cudaStream_t st);

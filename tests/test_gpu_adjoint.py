@@ -116,3 +116,28 @@ def test_eq52_on_dh_and_errors_without_the_option(api, orc):
         P0.forward_adjoint(dev(y))
     with pytest.raises(ShtError):
         api.Plan(L, 0, reality=True, adjoint=True)
+
+
+@pytest.mark.parametrize("L,N", [(6, 3), (24, 4), (40, 8), (65, 5)])
+def test_so3_adjoints_dot_products_and_oracle(api, orc, L, N):
+    """Wigner adjoints (so3_forward_adjoint_plan / so3_inverse_adjoint_plan): <W x, y> = <x, W^H y> and <W^-1 c, g> = <c, W^-H g> on random
+    arrays against the library's own transforms, and element-wise parity with the oracle's transposed chains (the library's forward is
+    W_oracle P with the pole-ring projection P of R21, so its adjoint is P W_oracle^H: the test applies P to the oracle's output)."""
+    from mwpole import project_so3_pole
+    shape = (2 * N - 1, L, 2 * L - 1)
+    P = api.Plan(L, N=N, adjoint=True)
+    x = synth.random_map(shape, seed=1); y = synth.random_flmn(L, N, seed=2)
+    c = synth.random_flmn(L, N, seed=3); g = synth.random_map(shape, seed=4)
+    Wx = P.forward(dev(x)).cpu().numpy()
+    WHy = P.forward_adjoint(dev(y)).cpu().numpy()
+    a, b = np.vdot(y, Wx), np.vdot(WHy, x)
+    assert abs(a - b) < 1e-12 * abs(a)
+    Vc = P.inverse(dev(c)).cpu().numpy()
+    VHg = P.inverse_adjoint(dev(g)).cpu().numpy()
+    a, b = np.vdot(g, Vc), np.vdot(VHg, c)
+    assert abs(a - b) < 1e-12 * abs(a)
+    if L <= 40:
+        assert rel(WHy, project_so3_pole(orc.so3_forward_adjoint(L, N, y))) < TOL
+        assert rel(VHg, orc.so3_inverse_adjoint(L, N, g)) < TOL
+    with pytest.raises(Exception):
+        api.Plan(8, N=2).forward_adjoint(dev(synth.random_flmn(8, 2, seed=1)))       # plan without SHT_OPT_ADJOINT

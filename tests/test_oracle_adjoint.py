@@ -81,3 +81,26 @@ def test_adjoint_is_the_conjugate_transpose_of_the_explicit_matrix(orc, sampling
     el = np.repeat(np.arange(L), 2 * L - 1); m = np.tile(np.arange(-(L - 1), L), L)
     sup = (np.abs(m) <= el) & (el >= abs(spin))
     assert np.abs(got - want)[sup].max() < 1e-14 and np.all(got[~sup] == 0)
+
+
+@pytest.mark.parametrize("L,N", [(5, 1), (6, 3), (9, 4), (8, 8)])
+def test_so3_dot_product_identities(orc, L, N):
+    """Wigner transforms (Eq. 15-18): <W x, y> = <x, W^H y> and <W^-1 c, g> = <c, W^-H g> on random (not band-limited) arrays, against the
+    separately pinned so3_forward / so3_inverse.  A wrong l-scaling, gamma sign, spin sign or slab order in the transposed chain breaks it."""
+    shape = (2 * N - 1, L, 2 * L - 1)
+    x = synth.random_map(shape, seed=1)
+    y = synth.random_flmn(L, N, seed=2)
+    a = np.vdot(y, orc.so3_forward(L, N, x))
+    b = np.vdot(orc.so3_forward_adjoint(L, N, y), x)
+    assert abs(a - b) < 1e-13 * abs(a)
+    c = synth.random_flmn(L, N, seed=3)
+    g = synth.random_map(shape, seed=4)
+    a = np.vdot(g, orc.so3_inverse(L, N, c))
+    b = np.vdot(orc.so3_inverse_adjoint(L, N, g), c)
+    assert abs(a - b) < 1e-13 * abs(a)
+    # coefficients outside the support (l < |n|, l < |m|) of the inverse's adjoint are zero
+    out = orc.so3_inverse_adjoint(L, N, g)
+    el = np.arange(L)[None, :, None]
+    m = np.arange(-(L - 1), L)[None, None, :]
+    n = (np.arange(2 * N - 1) - (N - 1))[:, None, None]
+    assert np.all(out[(np.abs(m) > el) | (np.abs(n) > el)] == 0)
