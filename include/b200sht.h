@@ -108,7 +108,8 @@ sht_status sht_plan_so3_opts(sht_plan** plan, int L, int N, int dtype, unsigned 
  * the Wigner-d recursion is run once and shared by all maps, which turns the theta / l contraction of Eq. 30 / 33
  * into a dense GEMM per harmonic order m (the einsum of Sec. 4.3, without storing the d-functions); it
  * runs on the FP64 tensor cores.  Arrays gain a leading [batch] axis: f[batch][L][2L-1], flm[batch][L][2L-1].
- * batch = 1 is sht_plan_s2().  MW sampling only (HEALPix with batch > 1: SHT_EUNSUPPORTED).  The theta-stage entry
+ * batch = 1 is sht_plan_s2().  The shared-recursion kernels serve MW fp64 plans; on the other samplings and in fp32 a batch is accepted
+ * and transformed map by map through the single-map kernels (same arrays, same results, no shared recursion).  The theta-stage entry
  * points below are single-map only. */
 sht_status sht_plan_s2_batch(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype, int batch);
 sht_status sht_plan_s2_opts(sht_plan** plan, int L, int spin, int sampling, int nside, int reality, int dtype, int batch, unsigned opts);

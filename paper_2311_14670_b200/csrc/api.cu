@@ -132,6 +132,7 @@ struct sht_plan {
     int* d_flag = nullptr;     // device flag raised by table kernels (start value outside the window-counter range)
     double sec_bytes[3] = {0, 0, 0};   // algorithmic bytes moved by the FFT / staging sections of the last transform (stage timing)
     int batch = 1;             // > 1: a batch of S^2 maps sharing one recursion (theta_mma.cu); then nslab = batch
+    int loop = 1;              // > 1: a batch on a sampling / dtype without the batched kernels: the single-map plan runs map by map
     int ncg = 0, ncg_fwd = 0;  // batched path: column groups of 16 complex columns (inverse / forward passes)
     double* Ob = nullptr;      // batched path: result scratch of all passes
     std::vector<size_t> ob_off_inv, ob_off_fwd;   // per-pass offsets (doubles) into Ob
@@ -1031,6 +1032,10 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if (batch < 1 || batch > 1024) return SHT_EINVAL;
     const bool internal = helper && (sampling == SHT_INT_MWRINGS || sampling == SHT_INT_MWSSRINGS);
     if (L < 1 || L > 16384 || abs(spin) >= L || (reality && spin != 0) || ((sampling < SHT_MW || sampling > SHT_GL) && !internal)) return SHT_EINVAL;
+    // batches run through the shared-recursion DMMA kernels on MW fp64 plans; on the other samplings and in fp32 the single-map path
+    // runs map by map (same results, no shared recursion)
+    int loop = 1;
+    if (batch > 1 && (sampling != SHT_MW || dtype == SHT_F32) && !helper && !(opts & (SHT_OPT_PRECOMPUTE | SHT_OPT_ADJOINT))) { loop = batch; batch = 1; }
     if (batch > 1 && sampling != SHT_MW) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside < 1) return SHT_EINVAL;
     if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
@@ -1051,6 +1056,7 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     P->dtype = dtype; P->opts = opts; P->helper = helper; P->only_dir = only_dir;
     P->precomp = (opts & SHT_OPT_PRECOMPUTE) != 0;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
+    P->loop = loop;
     P->batch = batch; P->nslab = batch; P->slab_n.assign(batch, -spin);        // sY_lm ~ d^l_{m,-s}  (Eq. 9+10)
     query_device(P);
     // ring sets: `inv` = the rings of the map (inverse theta step), `fwd` = the rings the forward quadrature runs on
@@ -1090,7 +1096,7 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     // adjoint entry points run the transposed chain on single orders, so plans that offer them keep one order per column
     P->pair = (sampling == SHT_MW || sampling == SHT_MWSS) && !helper && !(opts & (SHT_OPT_ADJOINT | SHT_OPT_NO_PAIR));
     // launch-bound sizes replay a captured CUDA graph (run_transform below)
-    P->use_graph = !helper && ((L <= 512 && !(opts & SHT_OPT_NO_GRAPH)) || (opts & SHT_OPT_GRAPH));
+    P->use_graph = !helper && loop == 1 && ((L <= 512 && !(opts & SHT_OPT_NO_GRAPH)) || (opts & SHT_OPT_GRAPH));
     if (spin != 0 && batch == 1 && dtype == SHT_F64 && !(opts & SHT_OPT_NO_INVSYM)) {
         // spin != 0: d^l_{-m,n}(pi - theta) = (-1)^{l-n} d^l_{m,n}(theta) lets ONE pass of the inverse serve order +m at a ring and
         // order -m at its mirror ring -- 6 FP64 instructions per d-step instead of 2 x 4, half the recursions -- wherever the inverse rings are
@@ -1151,7 +1157,7 @@ sht_status sht_plan_so3_opts(sht_plan** out, int L, int N, int dtype, unsigned o
     return SHT_OK;
 }
 size_t sht_plan_workspace_bytes(const sht_plan* P) { return P ? P->need_bytes : 0; }
-int sht_plan_batch(const sht_plan* P) { return P ? P->batch : 0; }
+int sht_plan_batch(const sht_plan* P) { return P ? (P->loop > 1 ? P->loop : P->batch) : 0; }
 int sht_plan_ntheta(const sht_plan* P, int forward) {
     if (!P) return 0;
     if (!forward) return P->F_nrings;
@@ -1332,7 +1338,7 @@ sht_status sht_plan_set_shard(sht_plan* P, int rank, int nranks) {
     if (!P || nranks < 1 || rank < 0 || rank >= nranks) return SHT_EINVAL;
     bool mirror_writes = false;      // an inverse fold pass writes the -m orders of the MIRRORED rings: not confined to a ring share
     for (auto& ph : P->pinv) mirror_writes = mirror_writes || ph.p.fold;
-    if (nranks > 1 && (P->batch > 1 || P->dtype != SHT_F64 || P->invsym || mirror_writes || (P->opts & SHT_OPT_ADJOINT))) {   // (precompute plans shard too)
+    if (nranks > 1 && (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64 || P->invsym || mirror_writes || (P->opts & SHT_OPT_ADJOINT))) {   // (precompute plans shard too)
         g_err = "ring shards need a single-map fp64 plan created with SHT_OPT_NO_INVSYM and without SHT_OPT_ADJOINT";
         return SHT_EUNSUPPORTED;
     }
@@ -1358,7 +1364,7 @@ sht_status sht_plan_stage_bytes(const sht_plan* P, double bytes[3]) {
 sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
-    if (P->batch > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     begin_transform(P);
     CS(run_theta_inverse(P, (const double2*)flm, st));
@@ -1371,7 +1377,7 @@ sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_str
 sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_stream stream) {
     CS(check_ready(P));
     if (!Wm || !flm || P->kind != 0) return SHT_EINVAL;
-    if (P->batch > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     begin_transform(P);
     // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
@@ -1462,6 +1468,7 @@ sht_status s2_forward_iter_plan(sht_plan* P, const void* f, void* flm, int niter
     CS(check_ready(P));
     if (!flm || !f || P->kind != 0 || niter < 0) return SHT_EINVAL;
     if (P->sampling != SHT_HEALPIX) { g_err = "iterative refinement is a HEALPix feature: the other samplings are exact"; return SHT_EUNSUPPORTED; }
+    if (P->loop > 1) { g_err = "iterative refinement is a single-map call"; return SHT_EUNSUPPORTED; }
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nm = P->map_elems * (P->reality ? 1 : 2), nc = 2 * (size_t)P->L * P->M;
     CS(s2_forward_plan(P, f, flm, stream));
@@ -1687,15 +1694,22 @@ sht_status run_transform(sht_plan* P, int kind, const void* in, void* out, sht_s
 }  // namespace
 
 extern "C" {
+// bytes of one map / one coefficient array of the public arrays (plans that run a batch map by map step through them)
+static size_t map_bytes(const sht_plan* P) { return P->map_elems * (P->reality ? 1 : 2) * (P->dtype == SHT_F32 ? 4 : 8); }
+static size_t coef_bytes(const sht_plan* P) { return (size_t)P->L * P->M * 2 * (P->dtype == SHT_F32 ? 4 : 8); }
 sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;
-    return run_transform(P, 0, flm, f, stream, s2_inverse_body);
+    for (int b = 0; b < P->loop; ++b)
+        CS(run_transform(P, 0, (const char*)flm + b * coef_bytes(P), (char*)f + b * map_bytes(P), stream, s2_inverse_body));
+    return SHT_OK;
 }
 sht_status s2_forward_plan(sht_plan* P, const void* f, void* flm, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;
-    return run_transform(P, 1, f, flm, stream, s2_forward_body);
+    for (int b = 0; b < P->loop; ++b)
+        CS(run_transform(P, 1, (const char*)f + b * map_bytes(P), (char*)flm + b * coef_bytes(P), stream, s2_forward_body));
+    return SHT_OK;
 }
 sht_status so3_inverse_plan(sht_plan* P, const void* flmn, void* f, sht_stream stream) {
     CS(check_ready(P));
