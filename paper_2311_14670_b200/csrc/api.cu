@@ -418,7 +418,8 @@ void layout(sht_plan* P, char* base) {
         P->ab32 = B.take<float4>((size_t)L * Lp);
         P->st32_inv = B.take<float>((size_t)Lp * P->inv.ntp); P->k16_inv = B.take<uint16_t>((size_t)Lp * P->inv.ntp);
         P->st32_fwd = B.take<float>((size_t)Lp * P->fwd.ntp); P->k16_fwd = B.take<uint16_t>((size_t)Lp * P->fwd.ntp);
-        P->io_a = B.take<double2>((size_t)L * NB); P->io_b = B.take<double2>((size_t)L * NB);
+        const size_t ioe = P->map_elems > (size_t)L * P->M ? P->map_elems : (size_t)L * P->M;      // a map or a coefficient array
+        P->io_a = B.take<double2>(ioe); P->io_b = B.take<double2>(ioe);
         P->lam32_inv = B.take<float>((size_t)(L + 1) * P->inv.ntp); P->lam32_fwd = B.take<float>((size_t)(L + 1) * P->fwd.ntp);
     }
     P->fft_work = B.take<char>(P->fft_work_bytes);
@@ -804,7 +805,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         a.L = L; a.Lp = P->Lp; a.nth = P->inv.nth; a.ntp = P->inv.ntp; a.NB = P->NB; a.ldout = P->F_ld;
         a.fold0 = P->fold0i; a.nfull = P->inv.nfull;
         a.ab = P->ab32; a.lam32 = P->lam32_inv; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
-        a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F;
+        a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F + P->col0;       // regular ring th -> map ring col0 + th
         CK(launch_theta_f32(a, false, NC, st));
         CS(inverse_poles(P, coef, st));
         stage(P, CAT_STAGE, st);
@@ -1049,8 +1050,8 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if ((opts & SHT_OPT_TILE64) && (opts & SHT_OPT_TILE128)) return SHT_EINVAL;
     if ((opts & SHT_OPT_INVSYM) && (opts & SHT_OPT_NO_INVSYM)) return SHT_EINVAL;
     if ((opts & SHT_OPT_GRAPH) && (opts & SHT_OPT_NO_GRAPH)) return SHT_EINVAL;
-    // fp32 variant (BASELINE config 5): spin 0, MW sampling, one map
-    if (dtype == SHT_F32 && (spin != 0 || sampling != SHT_MW || batch != 1)) return SHT_EUNSUPPORTED;
+    // fp32 variant (BASELINE config 5): spin 0 (the fp32 kernels recurse the second index n = 0), one map at a time, any sampling
+    if (dtype == SHT_F32 && (spin != 0 || batch != 1 || helper)) return SHT_EUNSUPPORTED;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
     P->dtype = dtype; P->opts = opts; P->helper = helper; P->only_dir = only_dir;

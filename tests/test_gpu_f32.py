@@ -49,7 +49,7 @@ def test_f32_inverse_forward_vs_oracle(api, orc, L, real):
 
 def test_f32_unsupported_requests_are_refused(api):
     from paper_2311_14670_b200._lib import ShtError
-    for kw in (dict(spin=2), dict(sampling=api.HEALPIX, nside=4), dict(N=3)):       # (a batch is accepted: it runs map by map)
+    for kw in (dict(spin=2), dict(N=3)):       # (a batch is accepted: it runs map by map; every sampling is served for spin 0)
         with pytest.raises(ShtError):
             api.Plan(16, dtype="f32", **kw)
 
@@ -83,3 +83,21 @@ def test_f32_forward_with_north_south_fold(api, orc, L, real):
     P = api.Plan(L, 0, reality=real, dtype="f32", fold=True)
     got = P.forward(dev(g.astype(np.float32 if real else np.complex64))).cpu().numpy()
     assert rel(got, orc.s2_forward(L, 0, orc.MW, project_mw_pole(g, 0).astype(np.complex128))) < TOL32
+
+
+@pytest.mark.parametrize("name,nside,real", [("mwss", 0, False), ("dh", 0, False), ("gl", 0, True), ("hp", 16, True), ("hp", 32, False)])
+@pytest.mark.parametrize("L,fold", [(40, None), (130, True), (130, False)])
+def test_f32_other_samplings_vs_oracle(api, orc, name, nside, real, L, fold):
+    """The fp32 kernels recurse the second index n = 0 on any ring set: spin-0 plans of every sampling, folded or not, within 1e-4 of the
+    oracle (inverse, and forward of the oracle's map)."""
+    gs, os_ = {"mwss": (api.MWSS, orc.MWSS), "dh": (api.DH, orc.DH), "gl": (api.GL, orc.GL), "hp": (api.HEALPIX, orc.HEALPIX)}[name]
+    okw = dict(nside=nside) if name == "hp" else {}
+    P = api.Plan(L, 0, sampling=gs, nside=nside, reality=real, dtype="f32", fold=fold)
+    flm = synth.random_flm(L, 0, seed=7 + L, sigma=synth.SIGMA_RED, real=real)
+    ref = orc.s2_inverse(L, 0, os_, flm, **okw)
+    ref = ref.real if real else ref
+    got = P.inverse(torch.from_numpy(flm.astype(np.complex64)).cuda()).cpu().numpy()
+    assert float(np.abs(got - ref).max() / np.abs(ref).max()) < 1e-4
+    want = orc.s2_forward(L, 0, os_, ref.astype(np.complex128), **okw)
+    back = P.forward(torch.from_numpy(ref.astype(np.float32 if real else np.complex64)).cuda()).cpu().numpy()
+    assert float(np.abs(back - want).max() / np.abs(want).max()) < 1e-4
