@@ -164,6 +164,10 @@ struct sht_plan {
     cufftHandle fft_hp_cap = 0, fft_hp_eq = 0;
     void* fft_work = nullptr; size_t fft_work_bytes = 0;
     cufftHandle fft_phi_inv = 0, fft_phi_fwd = 0, fft_th1 = 0, fft_th2 = 0, fft_gamma = 0;
+    // host-buffer calls (s2_*_host): ring FFTs in `nchunk` ring chunks, so that the PCIe copy of chunk k+1 overlaps the FFT of chunk k
+    cufftHandle fft_phi_inv_c = 0, fft_phi_fwd_c = 0; int nchunk = 0;
+    cudaStream_t copy_stream = nullptr; cudaEvent_t ev_copy[8] = {}, ev_begin = nullptr;
+    bool skip_phi = false;     // set while a host-buffer call runs the ring FFT stage itself
     cufftHandle fft_alpha = 0; // SO(3): the ring FFTs of all (gamma / n, beta) rows in ONE batch, on the [slab][ring][phi] layout
     bool have_fft = false;
     std::map<cufftHandle, double> fft_elems;   // complex elements one execution of each handle transforms (byte accounting)
@@ -509,6 +513,16 @@ sht_status make_fft_plans(sht_plan* P) {
     CF(cufftCreate(&P->fft_phi_fwd)); CF(cufftSetAutoAllocation(P->fft_phi_fwd, 0));
     { int inembed[1] = {NB}, onembed[1] = {NB};
       CF(cufftMakePlanMany(P->fft_phi_fwd, 1, n1, inembed, 1, NB, onembed, P->Ltp, 1, CUFFT_Z2Z, nr, &w)); P->fft_elems[P->fft_phi_fwd] = (double)nr * NB; ws = w > ws ? w : ws; }
+    if (P->kind == 0 && P->batch == 1 && P->loop == 1 && !P->reality && !P->helper && L >= 1024) {
+        for (int k : {8, 4, 2}) if (nr % k == 0) { P->nchunk = k; break; }
+        if (P->nchunk) {
+            int inembed[1] = {NB}, onembed[1] = {NB};
+            CF(cufftCreate(&P->fft_phi_inv_c)); CF(cufftSetAutoAllocation(P->fft_phi_inv_c, 0));
+            CF(cufftMakePlanMany(P->fft_phi_inv_c, 1, n1, inembed, P->F_ld, 1, onembed, 1, NB, CUFFT_Z2Z, nr / P->nchunk, &w)); P->fft_elems[P->fft_phi_inv_c] = (double)(nr / P->nchunk) * NB; ws = w > ws ? w : ws;
+            CF(cufftCreate(&P->fft_phi_fwd_c)); CF(cufftSetAutoAllocation(P->fft_phi_fwd_c, 0));
+            CF(cufftMakePlanMany(P->fft_phi_fwd_c, 1, n1, inembed, 1, NB, onembed, P->Ltp, 1, CUFFT_Z2Z, nr / P->nchunk, &w)); P->fft_elems[P->fft_phi_fwd_c] = (double)(nr / P->nchunk) * NB; ws = w > ws ? w : ws;
+        }
+    }
     if (P->upsampled) {
         // theta FFTs of the forward upsampling: length Tcirc on the extended samples, length 4L onto the quadrature rings
         int nt[1] = {P->Tcirc};
@@ -1275,7 +1289,7 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
         CK(st_f64_to_f32((size_t)(L + 1) * P->fwd.ntp, P->pfwd[0].p.lam, P->lam32_fwd, st));
     }
     if (P->sampling != SHT_HEALPIX) {
-        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2})
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_phi_inv_c, P->fft_phi_fwd_c})
             if (h) CF(cufftSetWorkArea(h, P->fft_work));
         if (P->invsym) CF(cufftSetWorkArea(P->fft_sym, P->fft_work));
         if (P->kind == 1) { CF(cufftSetWorkArea(P->fft_gamma, P->fft_work)); CF(cufftSetWorkArea(P->fft_alpha, P->fft_work)); }
@@ -1301,12 +1315,16 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
 sht_status sht_plan_destroy(sht_plan* P) {
     if (!P) return SHT_OK;
     if (P->have_fft || P->fft_phi_inv) {
-        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_alpha, P->fft_hp_cap, P->fft_hp_eq, P->fft_sym})
+        for (cufftHandle h : {P->fft_phi_inv, P->fft_phi_fwd, P->fft_th1, P->fft_th2, P->fft_gamma, P->fft_alpha, P->fft_hp_cap, P->fft_hp_eq, P->fft_sym,
+                              P->fft_phi_inv_c, P->fft_phi_fwd_c})
             if (h) cufftDestroy(h);
     }
     for (auto e : P->ev) cudaEventDestroy(e);
     for (auto& g : P->graphs) cudaGraphExecDestroy(g.exec);
     if (P->cap_stream) cudaStreamDestroy(P->cap_stream);
+    if (P->copy_stream) cudaStreamDestroy(P->copy_stream);
+    for (auto e : P->ev_copy) if (e) cudaEventDestroy(e);
+    if (P->ev_begin) cudaEventDestroy(P->ev_begin);
     sht_plan_destroy(P->adj_inv); sht_plan_destroy(P->adj_fwd);
     for (sht_plan* Q : P->sub) sht_plan_destroy(Q);
     delete P;
@@ -1415,6 +1433,7 @@ static sht_status s2_inverse_body(sht_plan* P, const void* flm, void* f, sht_str
     CS(run_theta_inverse(P, (const double2*)flm, st));
     if (P->sampling == SHT_HEALPIX) return healpix_synthesis(P, f, st);
     if (P->invsym) CS(resample_sym_to_mw(P, st));
+    if (P->skip_phi) return SHT_OK;                  // (host-buffer call: the ring synthesis runs chunk by chunk, overlapped with the copies out)
     stage(P, CAT_FFT, st);
     double2* outc = P->reality ? P->cplx : (double2*)f;
     for (int b = 0; b < P->batch; ++b)
@@ -1449,7 +1468,7 @@ static sht_status s2_forward_body(sht_plan* P, const void* f, void* flm, sht_str
     const double2* fin = (const double2*)f;
     if (P->reality) { stage(P, CAT_STAGE, st); CK(st_real_to_complex(nmap * P->batch, (const double*)f, P->cplx, st)); fin = P->cplx; }
     stage(P, CAT_FFT, st);
-    for (int b = 0; b < P->batch; ++b)                                                 // Eq. 31 (weight folded into q_u)
+    for (int b = 0; b < P->batch && !P->skip_phi; ++b)                                 // Eq. 31 (weight folded into q_u)
         CS(fft_exec(P, P->fft_phi_fwd, const_cast<double2*>(fin) + nmap * b, P->Fa + P->Fa_slab * b, CUFFT_FORWARD, st));
     if (P->upsampled) {         // MW / MWSS: extension to the theta circle + upsampling to the quadrature rings
         CS(mw_upsample(P, st));
@@ -1787,6 +1806,14 @@ size_t s2_map_bytes(int L, int sampling, int nside, int reality) {
     }
     return n * (reality ? 8 : 16);
 }
+// copy stream and events of the chunked host-buffer calls (created on first use)
+sht_status host_pipe_init(sht_plan* P) {
+    if (P->copy_stream) return SHT_OK;
+    CK(cudaStreamCreateWithFlags(&P->copy_stream, cudaStreamNonBlocking));
+    for (auto& ev : P->ev_copy) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&P->ev_begin, cudaEventDisableTiming));
+    return SHT_OK;
+}
 sht_status host_io(CacheEntry* e, size_t in_bytes, size_t out_bytes) {
     if (e->in_bytes < in_bytes) { if (e->d_in) cudaFree(e->d_in); CK(cudaMalloc(&e->d_in, in_bytes)); e->in_bytes = in_bytes; }
     if (e->out_bytes < out_bytes) { if (e->d_out) cudaFree(e->d_out); CK(cudaMalloc(&e->d_out, out_bytes)); e->out_bytes = out_bytes; }
@@ -1834,8 +1861,26 @@ sht_status s2_forward_host(int L, int spin, int sampling, int reality, const voi
     CacheLease lease; CS(cache_get(0, L, spin, sampling, nside, reality, st, &lease));
     size_t mb = s2_map_bytes(L, sampling, nside, reality), cb = (size_t)L * (2 * L - 1) * 16;
     CacheEntry* e = lease.e; CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
-    CK(cudaMemcpyAsync(e->d_in, f_host, mb, cudaMemcpyHostToDevice, st));
-    CS(s2_forward_plan(e->plan, e->d_in, e->d_out, stream));
+    sht_plan* P = e->plan;
+    if (P->nchunk && !P->timing) {
+        // ring chunks: the host -> device copy of chunk k+1 (copy stream) overlaps the ring FFT of chunk k (Eq. 31)
+        CS(host_pipe_init(P));
+        const size_t cbytes = mb / P->nchunk; const int crings = P->nrmap / P->nchunk;
+        CK(cudaEventRecord(P->ev_begin, st)); CK(cudaStreamWaitEvent(P->copy_stream, P->ev_begin, 0));   // d_in is free once earlier work on st is done
+        begin_transform(P);
+        for (int k = 0; k < P->nchunk; ++k) {
+            CK(cudaMemcpyAsync((char*)e->d_in + k * cbytes, (const char*)f_host + k * cbytes, cbytes, cudaMemcpyHostToDevice, P->copy_stream));
+            CK(cudaEventRecord(P->ev_copy[k], P->copy_stream)); CK(cudaStreamWaitEvent(st, P->ev_copy[k], 0));
+            CS(fft_exec(P, P->fft_phi_fwd_c, (double2*)((char*)e->d_in + k * cbytes), P->Fa + (size_t)k * crings, CUFFT_FORWARD, st));
+        }
+        P->skip_phi = true;
+        sht_status s = s2_forward_plan(P, e->d_in, e->d_out, stream);
+        P->skip_phi = false;
+        CS(s);
+    } else {
+        CK(cudaMemcpyAsync(e->d_in, f_host, mb, cudaMemcpyHostToDevice, st));
+        CS(s2_forward_plan(P, e->d_in, e->d_out, stream));
+    }
     CK(cudaMemcpyAsync(flm_host, e->d_out, cb, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return SHT_OK;
@@ -1847,8 +1892,25 @@ sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const voi
     size_t mb = s2_map_bytes(L, sampling, nside, reality), cb = (size_t)L * (2 * L - 1) * 16;
     CacheEntry* e = lease.e; CS(host_io(e, mb > cb ? mb : cb, mb > cb ? mb : cb));
     CK(cudaMemcpyAsync(e->d_in, flm_host, cb, cudaMemcpyHostToDevice, st));
-    CS(s2_inverse_plan(e->plan, e->d_in, e->d_out, stream));
-    CK(cudaMemcpyAsync(f_host, e->d_out, mb, cudaMemcpyDeviceToHost, st));
+    sht_plan* P = e->plan;
+    if (P->nchunk && !P->timing) {
+        // ring chunks: the device -> host copy of chunk k (copy stream) overlaps the ring synthesis of chunk k+1 (Eq. 32)
+        CS(host_pipe_init(P));
+        const size_t cbytes = mb / P->nchunk; const int crings = P->nrmap / P->nchunk;
+        P->skip_phi = true;
+        sht_status s = s2_inverse_plan(P, e->d_in, e->d_out, stream);
+        P->skip_phi = false;
+        CS(s);
+        for (int k = 0; k < P->nchunk; ++k) {
+            CS(fft_exec(P, P->fft_phi_inv_c, P->F + (size_t)k * crings, (double2*)((char*)e->d_out + k * cbytes), CUFFT_INVERSE, st));
+            CK(cudaEventRecord(P->ev_copy[k], st)); CK(cudaStreamWaitEvent(P->copy_stream, P->ev_copy[k], 0));
+            CK(cudaMemcpyAsync((char*)f_host + k * cbytes, (char*)e->d_out + k * cbytes, cbytes, cudaMemcpyDeviceToHost, P->copy_stream));
+        }
+        CK(cudaStreamSynchronize(P->copy_stream));
+    } else {
+        CS(s2_inverse_plan(P, e->d_in, e->d_out, stream));
+        CK(cudaMemcpyAsync(f_host, e->d_out, mb, cudaMemcpyDeviceToHost, st));
+    }
     CK(cudaStreamSynchronize(st));
     return SHT_OK;
 }

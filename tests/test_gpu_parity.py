@@ -165,6 +165,23 @@ def test_host_buffer_calls_match_device_calls(api):
     assert rel(api.so3_forward_host(api.so3_inverse_host(c, 12, 3), 12, 3), c) < TOL
 
 
+@pytest.mark.parametrize("L,spin,sampling", [(1024, 2, "mw"), (1030, 0, "mw"), (1031, 1, "mwss"), (1025, 0, "mw")])
+def test_host_buffer_calls_overlap_copies_in_ring_chunks(api, L, spin, sampling):
+    """From L = 1024 the host-buffer calls run the ring FFT stage in 8 / 4 / 2 ring chunks on the transform's stream while a copy stream
+    moves the next (forward) or the previous (inverse) chunk over PCIe; ring counts that no such chunk count divides (L = 1025) take
+    the plain path.  Same numbers as the device-buffer calls, pinned and pageable host memory alike, and twice in a row (buffer reuse)."""
+    samp = api.MW if sampling == "mw" else api.MWSS
+    flm = synth.random_flm(L, spin, seed=L)
+    f_dev = api.s2_inverse(dev(flm), L, spin, sampling=samp).cpu().numpy()
+    for rep in range(2):
+        f_host = api.s2_inverse_host(flm, L, spin, sampling=samp)
+        assert np.abs(f_host - f_dev).max() < 1e-13 * np.abs(f_dev).max()
+        back = api.s2_forward_host(f_host, L, spin, sampling=samp)
+        assert rel(back, flm) < TOL
+    pinned = torch.from_numpy(f_dev).pin_memory().numpy()
+    assert rel(api.s2_forward_host(pinned, L, spin, sampling=samp), flm) < TOL
+
+
 def test_inputs_are_not_modified_and_errors_are_loud(api):
     L = 20
     flm = synth.random_flm(L, 0, seed=1)
