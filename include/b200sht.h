@@ -77,6 +77,10 @@ enum {
                                      internal capture stream, so the caller's stream may be the default stream).  Default for L <= 512, where a
                                      transform is a chain of 10-50 short launches and bound by launch overhead ...                          */
     SHT_OPT_NO_GRAPH = 1u << 10,  /* ... this flag launches the kernels one by one.  (Stage timing always does.)                          */
+    SHT_OPT_NO_SKIP  = 1u << 11,  /* from L >= 1024 the fused kernels skip the "silent head" of a block tile: near the poles every iterate of a tile
+                                     stays below the window top for its first p0 steps (nothing is projected there), so the register state after
+                                     those steps is computed once at sht_plan_set_workspace and loaded by every transform (about 140 KB of
+                                     workspace per tile).  Same results.  This flag runs every step in every transform.                    */
     SHT_OPT_NO_PAIR  = 1u << 8    /* MW / MWSS: the theta-direction FFTs of the forward upsampling and of the symmetric-ring
                                      inverse carry TWO orders m, m+1 per column by default (their extensions to the theta circle are one even
                                      and one odd function, separated afterwards: half the FFT work); this flag keeps one order

@@ -9,7 +9,7 @@ LIB_PATH = os.path.join(HERE, "libb200sht.so")
 SHT_MW, SHT_HEALPIX, SHT_MWSS, SHT_DH, SHT_GL = 0, 1, 2, 3, 4
 SHT_F64, SHT_F32 = 0, 1
 SHT_OPT_FOLD_ON, SHT_OPT_FOLD_OFF, SHT_OPT_INVSYM, SHT_OPT_TILE64, SHT_OPT_TILE128, SHT_OPT_ADJOINT, SHT_OPT_PRECOMPUTE, SHT_OPT_NO_INVSYM = 1, 2, 4, 8, 16, 32, 64, 128
-SHT_OPT_NO_PAIR, SHT_OPT_GRAPH, SHT_OPT_NO_GRAPH = 256, 512, 1024
+SHT_OPT_NO_PAIR, SHT_OPT_GRAPH, SHT_OPT_NO_GRAPH, SHT_OPT_NO_SKIP = 256, 512, 1024, 2048
 SHT_PEAK_DFMA, SHT_PEAK_DMMA, SHT_PEAK_FFMA, SHT_PEAK_FFMA2 = 0, 1, 2, 3
 
 # every symbol include/b200sht.h declares: name -> (restype, argtypes)

@@ -40,7 +40,7 @@ class Plan:
     """A transform plan (sht_plan): fixes the problem, owns one workspace tensor allocated through PyTorch."""
 
     def __init__(self, L, spin=0, sampling=MW, nside=0, reality=False, N=None, device="cuda:0", batch=1, dtype="f64",
-                 fold=None, invsym=None, tile=None, adjoint=False, precompute=False, pair=None, graph=None):
+                 fold=None, invsym=None, tile=None, adjoint=False, precompute=False, pair=None, graph=None, skip=None):
         """fold / invsym / tile map to the SHT_OPT_* creation flags (None = the library's automatic choice)."""
         self._h = C.c_void_p()
         opts = 0
@@ -58,6 +58,8 @@ class Plan:
             opts |= _lib.SHT_OPT_NO_PAIR
         if graph is not None:
             opts |= _lib.SHT_OPT_GRAPH if graph else _lib.SHT_OPT_NO_GRAPH
+        if skip is not None and not skip:
+            opts |= _lib.SHT_OPT_NO_SKIP
         self.L, self.spin, self.sampling, self.nside, self.reality, self.N = L, spin, sampling, nside, bool(reality), N
         self.batch = int(batch)
         if dtype not in ("f64", "f32"):

@@ -101,6 +101,11 @@ struct sht_plan {
     int fold0i = 0;            // spin-0 plans on ring sets symmetric about the equator (HEALPix): the inverse recursion too
     int F_ld = 0, F_nrings = 0;   // row length of F[bin][F_ld] and the number of rings it holds (incl. a pole ring)
     bool upsampled = false;    // MW / MWSS: the forward transform extends F_m to the theta circle and upsamples to the quadrature rings
+    // silent-head skip tables (ThetaArgs::skip_*): [direction 0 inverse / 1 forward][kernel mode 0 PM / 1 P]
+    bool skip = false, skip_ready = false;
+    int* skip_p0[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
+    double* skip_state[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
+    int skip_nb[2][2] = {{0, 0}, {0, 0}};
     bool inv_fold = false;     // n != 0 S^2 plans: the inverse runs ONE fold pass (+m at a ring, -m at its mirror ring) where its rings are symmetric
     int pair = 0;              // MW / MWSS: the theta-circle FFTs carry two orders m per column (staging.cu u_get): prow = L rows instead of NB
     int prow = 0;              // rows of the theta-circle arrays X / Z the upsampling (and the symmetric-ring resampling) works on
@@ -383,6 +388,23 @@ void layout(sht_plan* P, char* base) {
     for (auto& ph : P->pfwd) {
         ph.p.in = B.take<double>(pass_in_doubles(P, ph, true));
         ph.p.lam = B.take<double>((size_t)(L - ph.p.m_end + 1) * P->fwd.ntp);
+    }
+    if (P->skip) {           // per block of every fused launch: pairs to skip + the register state to start from
+        for (int dir = 0; dir < 2; ++dir)
+            for (int md = 0; md < 2; ++md) {
+                const RingSet& R = dir ? P->fwd : P->inv;
+                int np = 0;
+                for (auto& ph : (dir ? P->pfwd : P->pinv)) np += ph.mode == md;
+                P->skip_nb[dir][md] = 0;
+                if (!np) continue;
+                ThetaArgs t{};
+                t.Lp = P->Lp; t.ntp = R.ntp; t.npass = np; t.nsm = P->nsm;
+                t.tile = (P->opts & SHT_OPT_TILE64) ? 64 : (P->opts & SHT_OPT_TILE128) ? 128 : 0;
+                const int nb = (P->Lp / SHT_TQ) * (R.ntp / theta_tile_rings(t)) * np;
+                P->skip_nb[dir][md] = nb;
+                P->skip_p0[dir][md] = B.take<int>(nb);
+                P->skip_state[dir][md] = reinterpret_cast<double*>(B.take<char>((size_t)nb * SHT_SKIP_STATE_BYTES));
+            }
     }
     if (P->precomp) {        // E[m - m_end][ntp][Lp] per pass: the O(L^3) memory of Sec. 4.3
         for (auto& ph : P->pinv) ph.p.pre = B.take<double>((size_t)(L - ph.p.m_end) * P->inv.ntp * Lp);
@@ -730,7 +752,63 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     a.nsm = P->nsm; a.tile = (P->opts & SHT_OPT_TILE64) ? 64 : (P->opts & SHT_OPT_TILE128) ? 128 : 0;
     a.passes = fwd ? (pm ? P->d_fwd_pm : P->d_fwd_p) : (pm ? P->d_inv_pm : P->d_inv_p);
     a.npass = fwd ? (pm ? P->n_fwd_pm : P->n_fwd_p) : (pm ? P->n_inv_pm : P->n_inv_p);
+    if (P->skip_ready) { a.skip_p0 = P->skip_p0[fwd ? 1 : 0][pm ? 0 : 1]; a.skip_state = P->skip_state[fwd ? 1 : 0][pm ? 0 : 1]; }
     return a;
+}
+
+// Silent-head skip tables (internal.h ThetaArgs::skip_*), built once at sht_plan_set_workspace with the plan's own
+// kernels: (1) PROBE -- one full recursion per launch on the zeroed operand tables; every block records the first pair of steps (at least 8
+// steps below its ramp) in which any warp contributed; (2) the host turns that into p0 = the pairs a transform may skip: 8 steps of margin
+// before the first contribution, a multiple of 8 pairs (the mbarrier phases of the operand ring and of the hand-off repeat every 8 pairs),
+// and only if p0 lies below the ramp and its first window check; (3) DUMP -- the blocks with p0 > 0 run pairs [0, p0) and store their
+// register state.  The tables depend on the ring set and the passes only, not on the data.
+sht_status build_skip_tables(sht_plan* P, cudaStream_t st) {
+    const int L = P->L, nlt = P->Lp / SHT_TQ;
+    if (P->only_dir != 2 && P->H) {
+        // the inverse kernels read their recursion coefficients g'_m(l), s_m from the operand rows that k_prep_inverse writes with every
+        // transform: fill them once here, from all-zero harmonic coefficients (H serves as the zero array; the next transform zeroes it anyway)
+        CK(cudaMemsetAsync(P->H, 0, sizeof(double2) * P->H_slab * P->nslab, st));
+        CK(st_prep_inverse(L, P->Lp, 2, P->mmin, P->n_inv_pm, P->H, (size_t)L * P->M, P->d_cslab, P->scale_inv, P->ctab, P->sgtab, P->sgstride, P->d_inv_pm, st));
+        CK(st_prep_inverse(L, P->Lp, 1, P->mmin, P->n_inv_p, P->H, (size_t)L * P->M, P->d_cslab, P->scale_inv, P->ctab, P->sgtab, P->sgstride, P->d_inv_p, st));
+    }
+    for (int dir = 0; dir < 2; ++dir) {
+        if ((dir == 0 && P->only_dir == 2) || (dir == 1 && P->only_dir == 1)) continue;
+        for (int md = 0; md < 2; ++md) {
+            const int nb = P->skip_nb[dir][md];
+            if (!nb) continue;
+            ThetaArgs a = theta_args(P, dir != 0, md == 0);
+            if (a.npass == 0) continue;
+            const int rings = theta_tile_rings(a), ntt = a.ntp / rings;
+            if (nlt * ntt * a.npass != nb) { g_err = "skip tables: block count mismatch"; return SHT_ECUDA; }
+            a.skip_p0 = P->skip_p0[dir][md]; a.skip_state = P->skip_state[dir][md];
+            CK(cudaMemsetAsync(a.skip_p0, 0, sizeof(int) * nb, st));
+            a.skip_mode = 1;
+            CK(dir ? launch_theta_forward(a, md, st) : launch_theta_inverse(a, md, st));
+            std::vector<int> h(nb);
+            CK(cudaMemcpyAsync(h.data(), a.skip_p0, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            std::vector<ThetaPass> passes(a.npass);
+            CK(cudaMemcpy(passes.data(), a.passes, sizeof(ThetaPass) * a.npass, cudaMemcpyDeviceToHost));
+            for (int b = 0; b < nb; ++b) {
+                const int tile = b / a.npass, lt = nlt - 1 - tile / ntt, l0 = lt * SHT_TQ;
+                const int mtop = l0 + SHT_TQ - 1 < L - 1 ? l0 + SHT_TQ - 1 : L - 1;
+                const int npairs = (mtop - passes[b % a.npass].m_end + 2) / 2;
+                int p0 = 0;
+                if (h[b] > 0) {                              // (0: the block did not run)
+                    const int first = h[b] == (1 << 30) ? npairs : h[b];
+                    p0 = (first - 4) & ~7;
+                    if (p0 < 8 || mtop - 2 * p0 >= l0 - 8) p0 = 0;
+                }
+                h[b] = p0;
+            }
+            CK(cudaMemcpyAsync(a.skip_p0, h.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
+            a.skip_mode = 2;
+            CK(dir ? launch_theta_forward(a, md, st) : launch_theta_inverse(a, md, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    P->skip_ready = true;
+    return SHT_OK;
 }
 
 MmaArgs mma_args(const sht_plan* P, bool fwd) {
@@ -1110,6 +1188,8 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     // MW / MWSS forward upsampling and the symmetric-ring resampling carry two orders per theta-circle column (staging.cu u_get); the
     // adjoint entry points run the transposed chain on single orders, so plans that offer them keep one order per column
     P->pair = (sampling == SHT_MW || sampling == SHT_MWSS) && !helper && !(opts & (SHT_OPT_ADJOINT | SHT_OPT_NO_PAIR));
+    // silent-head skip of the fused kernels (build_skip_tables): single-map fp64 on-the-fly plans from L >= 1024
+    P->skip = !helper && batch == 1 && dtype == SHT_F64 && !(opts & (SHT_OPT_PRECOMPUTE | SHT_OPT_NO_SKIP)) && L >= 1024;
     // launch-bound sizes replay a captured CUDA graph (run_transform below)
     P->use_graph = !helper && loop == 1 && ((L <= 512 && !(opts & SHT_OPT_NO_GRAPH)) || (opts & SHT_OPT_GRAPH));
     if (spin != 0 && batch == 1 && dtype == SHT_F64 && !(opts & SHT_OPT_NO_INVSYM)) {
@@ -1308,6 +1388,8 @@ sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sh
     int flag = 0;
     CK(cudaMemcpy(&flag, P->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
     if (flag) { g_err = "Eq. 27 start values fall below the window-counter range on this ring set"; return SHT_EUNSUPPORTED; }
+    P->skip_ready = false;
+    if (P->skip) CS(build_skip_tables(P, st));
     P->ready = true;
     return SHT_OK;
 }

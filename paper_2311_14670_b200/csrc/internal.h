@@ -20,6 +20,7 @@
 #define SHT_TWIN (-500)   // window top: stored start values with k > 0 are <= 2^TWIN
 #define SHT_SWIN 480      // window stride: true value = stored * 2^(-SWIN*k)
 #define SHT_JCHK 8        // steps between window checks
+#define SHT_SKIP_STATE_BYTES (64 * 256 * 8 + 9 * 256 * 4)   // per block: 64 doubles + 9 words per compute thread
 #define SHT_TQ 64         // quantum of the kappa tables = degrees per block tile of both hot kernels
 
 struct ThetaPass {
@@ -54,6 +55,13 @@ struct ThetaArgs {
                            // the inverse keeps even-l / odd-l partial sums and writes both rings of a mirror pair
     int th_lo, th_hi;      // ring shard (sht_plan_set_shard): only kernel rings th_lo <= th < th_hi are served by this launch
     int nsm;               // SMs of the device (tile choice)
+    // Skipping the silent head of a tile.  For rings near a pole the iterates of a whole tile stay below the
+    // window top (every counter k > 0) for the first p0 pairs of steps: nothing is projected there, the recursion merely carries the
+    // state.  At plan time the kernels run once in PROBE mode (record, per block, the first pair in which any warp contributed) and once in
+    // DUMP mode (run pairs [0, p0) and store the register state); transforms then LOAD that state and start at pair p0.
+    int skip_mode;         // 0 = transform (loads the state where skip_p0 > 0), 1 = probe, 2 = dump
+    int* skip_p0;          // [block] pairs to skip (multiple of 8), 0 = none; PROBE writes the first contributing pair here
+    double* skip_state;    // [block][SHT_SKIP_STATE_BYTES]: e_m, e_{m+1} of the 32 items of the 256 compute threads, window counters, wact
     int tile;              // 0 = automatic, 64 / 128 = forced ring-tile size (plan option SHT_OPT_TILE64 / SHT_OPT_TILE128)
 };
 
@@ -94,6 +102,7 @@ struct F32Args {
 cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st);
 
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)
+int theta_tile_rings(const ThetaArgs& a);
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st);
 cudaError_t launch_theta_forward(const ThetaArgs& a, int mode, cudaStream_t st);
 // precompute.cu (Sec. 4.3): fill the stored d-function tables of the passes, and the theta steps that read them

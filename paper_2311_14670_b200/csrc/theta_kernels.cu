@@ -31,6 +31,40 @@ constexpr int NRS = 4;   // stages of the partial-sum hand-off of the forward ke
 constexpr int KS = 2;    // recursion steps per pipeline stage (one TMA barrier, one hand-off per KS steps)
 constexpr int NAUX = 4;  // auxiliary warps (one warpgroup: setmaxnreg works on aligned groups of 4 warps)
 
+// ---- skipping the silent head of a tile (internal.h, ThetaArgs::skip_*) ------------------------------------------------------------
+// [pbeg, pend): the pairs this launch runs for the block `bid`; returns false if the block has nothing to do in this mode
+template <int SM>
+__device__ __forceinline__ bool skip_range(const ThetaArgs& A, unsigned bid, int npairs, int& pbeg, int& pend) {
+    pbeg = 0; pend = npairs;
+    if (SM == 1 || !A.skip_p0) return true;                   // probe: the whole recursion
+    const int p0 = A.skip_p0[bid];
+    if (SM == 2) { pend = p0; return p0 > 0; }                // dump: the silent head only
+    pbeg = p0;                                                // transform: start where the head ends
+    return true;
+}
+template <int NI>
+__device__ __forceinline__ void skip_store(const ThetaArgs& A, unsigned bid, int ctid, const double (&cur)[NI], const double (&prev)[NI],
+                                           const KPack<NI>& kp, bool wact) {
+    static_assert(NI <= 32, "state layout: room for 32 items per thread");
+    double* d = reinterpret_cast<double*>(reinterpret_cast<char*>(A.skip_state) + (size_t)bid * SHT_SKIP_STATE_BYTES);
+    uint32_t* u = reinterpret_cast<uint32_t*>(d + 64 * 256);
+#pragma unroll
+    for (int q = 0; q < NI; ++q) { d[q * 256 + ctid] = cur[q]; d[(NI + q) * 256 + ctid] = prev[q]; }
+#pragma unroll
+    for (int i = 0; i < (NI + 3) / 4; ++i) u[i * 256 + ctid] = kp.w[i];
+    u[8 * 256 + ctid] = wact ? 1u : 0u;
+}
+template <int NI>
+__device__ __forceinline__ void skip_load(const ThetaArgs& A, unsigned bid, int ctid, double (&cur)[NI], double (&prev)[NI], KPack<NI>& kp, bool& wact) {
+    const double* d = reinterpret_cast<const double*>(reinterpret_cast<const char*>(A.skip_state) + (size_t)bid * SHT_SKIP_STATE_BYTES);
+    const uint32_t* u = reinterpret_cast<const uint32_t*>(d + 64 * 256);
+#pragma unroll
+    for (int q = 0; q < NI; ++q) { cur[q] = d[q * 256 + ctid]; prev[q] = d[(NI + q) * 256 + ctid]; }
+#pragma unroll
+    for (int i = 0; i < (NI + 3) / 4; ++i) kp.w[i] = u[i * 256 + ctid];
+    wact = u[8 * 256 + ctid] != 0u;
+}
+
 // =============================================================================================================
 // inverse theta step, Eq. 33:  F[row(m_out)][theta] += sum_l G[m][l] * e^l_m(theta)      (G carries c_m(l))
 // block tile: TL = NW*RL degrees x NTH = 32*RT rings; KS = 2 recursion steps per pipeline stage
@@ -54,7 +88,8 @@ struct InvSmem {
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
-template <int RL, int RT, int NW, int NC, bool FOLD, int WT>
+// SM: 0 = transform, 1 = probe, 2 = dump (ThetaArgs::skip_mode; separate instantiations keep the transform kernels free of the plan-time code)
+template <int RL, int RT, int NW, int NC, bool FOLD, int WT, int SM>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(const ThetaArgs A) {
     using S = InvSmem<RL, RT, NW, NC, FOLD, WT>;
     constexpr int TL = S::TL, NTH = S::NTH, NI = RL * RT, ROWD = S::ROWD, NRS = S::NRS, NSET = S::NSET, ND = S::ND;
@@ -72,8 +107,14 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
     const int an = P.n < 0 ? -P.n : P.n;
     if (l0 + TL <= an || l0 >= A.L || th0 >= A.nth || th0 + NTH <= A.th_lo || th0 >= A.th_hi) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + TL - 1, A.L - 1), m_end = P.m_end;
-    const int npairs = (mtop - m_end + 2) / KS;       // an odd step count ends with a dummy step m_end-1 (all-zero table row)
+    int mtop = min(l0 + TL - 1, A.L - 1);
+    const int m_end = P.m_end;
+    int npairs = (mtop - m_end + 2) / KS;             // an odd step count ends with a dummy step m_end-1 (all-zero table row)
+    int pbeg, pend;
+    if (!skip_range<SM>(A, bid, npairs, pbeg, pend)) return;
+    // the loops below count pairs from 0 at step mtop, as if the tile started where its silent head ends (pbeg is a multiple of 8, so the
+    // ring slots and mbarrier phases derived from the pair counter are the same)
+    mtop -= KS * pbeg; npairs = pend - pbeg;
 
     if (tid == 0) {
         for (int i = 0; i < NST; ++i) mbar_init(&sm.full[i], 1);
@@ -124,6 +165,13 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         for (int p = 0; p < npairs; ++p) {
             const int rs = p & (NRS - 1);
             mbar_wait(&sm.rfull[rs], (p / NRS) & 1);
+            if (SM == 1 && at == 0) {                  // probe: first pair, 8 steps below the ramp or later, in which any warp contributed
+                int fl = 0;
+#pragma unroll
+                for (int ww = 0; ww < NW; ++ww) fl |= sm.act[rs][ww];
+                if (p == 0) A.skip_p0[bid] = 1 << 30;
+                if (fl && mtop - KS * p < l0 - 8 && A.skip_p0[bid] == (1 << 30)) A.skip_p0[bid] = p;
+            }
             int actb[ND][NQ];                          // flags of the warp that wrote output q of degree group ww
 #pragma unroll
             for (int ww = 0; ww < ND; ++ww)
@@ -272,6 +320,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         }
         return wrote;
     };
+    if (SM == 0 && pbeg > 0) skip_load<NI>(A, bid, tid, cur, prev, kp, wact);      // transform: the state the silent head would have produced
     for (int p = 0; p < npairs; ++p) {
         const int m = mtop - KS * p, slot = p & (NST - 1), rs = p & (NRS - 1);
         const uint32_t rparity = ((p / NRS) & 1) ^ 1;
@@ -288,6 +337,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             mbar_arrive(&sm.rfull[rs]);
         }
     }
+    if (SM == 2) skip_store<NI>(A, bid, tid, cur, prev, kp, wact);
 }
 
 // =============================================================================================================
@@ -312,7 +362,7 @@ struct FwdSmem {
     uint64_t full[NST], rfull[NRS], rempty[NRS];
 };
 
-template <int RL, int RT, int NW, int NC, bool FOLD>
+template <int RL, int RT, int NW, int NC, bool FOLD, int SM>
 __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(const ThetaArgs A) {
     using S = FwdSmem<RL, RT, NW, NC, FOLD>;
     constexpr int TLB = S::TLB, NTB = S::NTB, NI = RL * RT, NCW = S::NCW;
@@ -331,8 +381,12 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     if (l0 + TLB <= an || l0 >= A.L || th0 >= A.nth || th0 + NTB <= A.th_lo || th0 >= A.th_hi) return;   // (rings outside the shard inside a
                                                                                                        //  boundary tile carry zero operands)
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int mtop = min(l0 + TLB - 1, A.L - 1), m_end = P.m_end;
-    const int npairs = (mtop - m_end + 2) / KS;
+    int mtop = min(l0 + TLB - 1, A.L - 1);
+    const int m_end = P.m_end;
+    int npairs = (mtop - m_end + 2) / KS;
+    int pbeg, pend;
+    if (!skip_range<SM>(A, bid, npairs, pbeg, pend)) return;
+    mtop -= KS * pbeg; npairs = pend - pbeg;           // pairs count from 0 at the step the silent head ends (see the inverse kernel)
 
     if (tid == 0) {
         for (int i = 0; i < NST; ++i) mbar_init(&sm.full[i], 1);
@@ -400,6 +454,13 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             int actb[NW];
 #pragma unroll
             for (int ww = 0; ww < NW; ++ww) actb[ww] = sm.act[rs][ww];
+            if (SM == 1 && at == 0) {                  // probe (see the inverse kernel)
+                int fl = 0;
+#pragma unroll
+                for (int ww = 0; ww < NW; ++ww) fl |= actb[ww];
+                if (p == 0) A.skip_p0[bid] = 1 << 30;
+                if (fl && mtop - KS * p < l0 - 8 && A.skip_p0[bid] == (1 << 30)) A.skip_p0[bid] = p;
+            }
 #pragma unroll
             for (int h = 0; h < KS; ++h) {
                 const int m = mtop - KS * p - h;
@@ -460,6 +521,9 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
     }
     double tm = 2.0 * (double)mtop;                    // x_{m-1} = x_m + 2m
     bool wact = true;
+    if (SM == 0 && pbeg > 0) {                         // transform: the state the silent head would have produced, at step m0
+        skip_load<NI>(A, bid, tid, cur, prev, kp, wact);   // (x and tm above are already those of the step the head ends at)
+    }
 
     // one recursion step; `ca` holds e_m, `cb` holds e_{m+1} on entry and e_{m-1} on exit (roles swap every step)
     auto step = [&](const int m, const int slot, const int rs, const int h, double (&ca)[NI],
@@ -568,6 +632,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             mbar_arrive(&sm.rfull[rs]);
         }
     }
+    if (SM == 2) skip_store<NI>(A, bid, tid, cur, prev, kp, wact);
 }
 
 template <int RL, int RT, int NW, int NC, bool FOLD = false, int WT = 1>
@@ -575,7 +640,8 @@ cudaError_t launch_inv(const ThetaArgs& a, cudaStream_t st) {
     using S = InvSmem<RL, RT, NW, NC, FOLD, WT>;
     const size_t smem = sizeof(S) + 128;
     dim3 grid((a.Lp / S::TL) * (a.ntp / S::NTH), a.npass);
-    auto k = theta_inverse_kernel<RL, RT, NW, NC, FOLD, WT>;
+    auto k = a.skip_mode == 1 ? theta_inverse_kernel<RL, RT, NW, NC, FOLD, WT, 1>
+           : a.skip_mode == 2 ? theta_inverse_kernel<RL, RT, NW, NC, FOLD, WT, 2> : theta_inverse_kernel<RL, RT, NW, NC, FOLD, WT, 0>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid, (NW + NAUX) * 32, smem, st>>>(a);
@@ -586,7 +652,8 @@ template <int RL, int RT, int NW, int NC, bool FOLD>
 cudaError_t launch_fwd(const ThetaArgs& a, cudaStream_t st) {
     using S = FwdSmem<RL, RT, NW, NC, FOLD>;
     const size_t smem = sizeof(S) + 128;
-    auto k = theta_forward_kernel<RL, RT, NW, NC, FOLD>;
+    auto k = a.skip_mode == 1 ? theta_forward_kernel<RL, RT, NW, NC, FOLD, 1>
+           : a.skip_mode == 2 ? theta_forward_kernel<RL, RT, NW, NC, FOLD, 2> : theta_forward_kernel<RL, RT, NW, NC, FOLD, 0>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((a.Lp / S::TLB) * (a.ntp / S::NTB), a.npass);
@@ -612,6 +679,8 @@ static bool small_tiles(const ThetaArgs& a, int big) {
     const long blocks = (long)(a.Lp / SHT_TQ) * (a.ntp / big) * a.npass;
     return blocks <= a.nsm;
 }
+// rings per block tile the launchers below choose for these arguments (the plan sizes its per-block skip tables with it)
+int theta_tile_rings(const ThetaArgs& a) { return small_tiles(a, 128) ? 64 : 128; }
 cudaError_t launch_theta_inverse(const ThetaArgs& a, int mode, cudaStream_t st) {
     if (a.npass == 0) return cudaSuccess;
     if (a.fold0) {
