@@ -358,6 +358,7 @@ def main():
         # issue slots): frac_executed = 1.0 means the FP64 pipe issues every cycle (`frac` alone is unbounded by 1)
         orders = (fl - 6.0) / 4.0
         instr = 2.0 + 2.0 * orders
+        skf, ski = plan.skip_fraction(True), plan.skip_fraction(False)
         ach = flops_fwd / (stages["forward_ms"]["hot"] * 1e-3) / 1e12
         ach_inv = flops_inv / (stages["inverse_ms"]["hot"] * 1e-3) / 1e12
         kname = ("theta_forward_f32" if args.dtype == "f32" else "theta_forward_kernel" if B == 1 else "theta_mma_kernel<forward>")
@@ -365,14 +366,19 @@ def main():
         roof = {"bound": "alu", "kernel": kname + " (fused m-recursion + theta contraction, Eq. 25+30)",
                 "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
                 "frac_is": "ALGORITHMIC flop (6 per d-step of Eq. 25 as the paper states it + 4 per order served) / hot time / measured peak",
-                "frac_executed": ach * (2.0 * instr / fl) / peak_tf,
-                "frac_executed_is": f"FP64 instructions the e-form kernel executes ({instr:.0f} per d-step, 2 flop each) / hot time / measured peak: 1.0 = pipe-bound",
+                "frac_executed": ach * (2.0 * instr / fl) / peak_tf * (1.0 - skf),
+                "frac_executed_is": f"FP64 instructions the e-form kernel executes ({instr:.0f} per d-step, 2 flop each; the d-steps of the skipped silent "
+                                    "heads excluded) / hot time / measured peak: 1.0 = pipe-bound",
+                "skipped_dsteps": {"forward": skf, "inverse": ski,
+                                   "is": "share of the block-steps the fused kernels skip (tiles near the poles project nothing in their first steps; "
+                                         "the state those steps leave is stored at plan time, DESIGN.md section 22); `frac` counts ALL d-steps of the "
+                                         "recursion as algorithmic work"},
                 "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
                 "time_source": "CUDA events recorded inside the library around the hot kernels; median of 5 transforms timed after the K timed steps",
                 "peak_kind": f"measured in this run by register-only chains (sht_peak): DFMA {pk['dfma']:.2f}, DMMA {pk['dmma']:.2f}, FFMA {pk['ffma']:.2f}, FFMA2 (packed f32x2) {pk['ffma2']:.2f} "
                              f"TFLOP/s; nominal {nsm} SM x 64 DFMA/clk x 2 x 1.965 GHz = {nsm * 64 * 2 * 1.965e-3:.1f}",
                 "flop_per_dstep": fl, "dsteps_per_launch": plan.dsteps(True),
-                "inverse_kernel": {"achieved": ach_inv, "frac": ach_inv / peak_tf, "frac_executed": ach_inv * (2.0 * instr / fl) / peak_tf},
+                "inverse_kernel": {"achieved": ach_inv, "frac": ach_inv / peak_tf, "frac_executed": ach_inv * (2.0 * instr / fl) / peak_tf * (1.0 - ski)},
                 "hbm_peak_gbs": hbm.get("hbm_gbs"), "hbm_peak_kind": hbm_kind,
                 "stage_gbs": {"inverse": {"fft": inv_b["fft"] / (inv_ms["fft"] * 1e-3) / 1e9 if inv_ms["fft"] > 0 else None,
                                           "staging": inv_b["staging"] / (inv_ms["staging"] * 1e-3) / 1e9 if inv_ms["staging"] > 0 else None},

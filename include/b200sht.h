@@ -253,6 +253,9 @@ double     sht_plan_dsteps(const sht_plan* plan, int forward);
 /* algorithmic flop of the hot kernels of one transform of this plan: per d-step 6 (Eq. 25 as the paper states it:
  * 1 FMA + 2 MUL + 1 FMA) + 4 per (harmonic order, map) served (Eq. 30 / 33: complex x real multiply-add) */
 double     sht_plan_flops(const sht_plan* plan, int forward);
+/* share of the block-steps of the fused kernels that a transform of this plan skips (the "silent head" of the block tiles near the poles,
+ * SHT_OPT_NO_SKIP; 0 for plans that run every step): those steps project nothing, their effect on the recursion state is loaded from a table */
+double     sht_plan_skip_fraction(const sht_plan* plan, int forward);
 const char* sht_version(void);
 
 #ifdef __cplusplus

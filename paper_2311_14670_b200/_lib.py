@@ -59,6 +59,7 @@ SIGNATURES = {
     "sht_launch_count": (C.c_long, [_i]),
     "sht_plan_dsteps": (C.c_double, [_vp, _i]),
     "sht_plan_flops": (C.c_double, [_vp, _i]),
+    "sht_plan_skip_fraction": (C.c_double, [_vp, _i]),
     "sht_version": (C.c_char_p, []),
 }
 

@@ -190,6 +190,10 @@ class Plan:
     def dsteps(self, forward):
         return float(lib().sht_plan_dsteps(self._h, int(forward)))
 
+    def skip_fraction(self, forward):
+        """Share of the fused kernels' block-steps this plan skips (silent head of the polar tiles); 0 if every step runs."""
+        return float(lib().sht_plan_skip_fraction(self._h, int(forward)))
+
     def flops(self, forward):
         """Algorithmic flop of the hot kernels of one transform (6 per d-step + 4 per order and map served)."""
         return float(lib().sht_plan_flops(self._h, int(forward)))

@@ -106,6 +106,7 @@ struct sht_plan {
     int* skip_p0[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
     double* skip_state[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
     int skip_nb[2][2] = {{0, 0}, {0, 0}};
+    double skip_pairs[2] = {0, 0}, all_pairs[2] = {0, 0};     // block-pairs skipped / in total, per direction (sht_plan_skip_fraction)
     bool inv_fold = false;     // n != 0 S^2 plans: the inverse runs ONE fold pass (+m at a ring, -m at its mirror ring) where its rings are symmetric
     int pair = 0;              // MW / MWSS: the theta-circle FFTs carry two orders m per column (staging.cu u_get): prow = L rows instead of NB
     int prow = 0;              // rows of the theta-circle arrays X / Z the upsampling (and the symmetric-ring resampling) works on
@@ -764,6 +765,7 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
 // register state.  The tables depend on the ring set and the passes only, not on the data.
 sht_status build_skip_tables(sht_plan* P, cudaStream_t st) {
     const int L = P->L, nlt = P->Lp / SHT_TQ;
+    P->skip_pairs[0] = P->skip_pairs[1] = P->all_pairs[0] = P->all_pairs[1] = 0;
     if (P->only_dir != 2 && P->H) {
         // the inverse kernels read their recursion coefficients g'_m(l), s_m from the operand rows that k_prep_inverse writes with every
         // transform: fill them once here, from all-zero harmonic coefficients (H serves as the zero array; the next transform zeroes it anyway)
@@ -800,6 +802,7 @@ sht_status build_skip_tables(sht_plan* P, cudaStream_t st) {
                     if (p0 < 8 || mtop - 2 * p0 >= l0 - 8) p0 = 0;
                 }
                 h[b] = p0;
+                if (l0 < L) { P->all_pairs[dir] += npairs; P->skip_pairs[dir] += p0; }
             }
             CK(cudaMemcpyAsync(a.skip_p0, h.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
             a.skip_mode = 2;
@@ -1260,6 +1263,11 @@ int sht_plan_ntheta(const sht_plan* P, int forward) {
     return (R.nfull ? R.nfull : R.nth) + (R.pole ? 1 : 0);
 }
 double sht_plan_dsteps(const sht_plan* P, int forward) { return P ? (forward ? P->dsteps_fwd : P->dsteps_inv) : 0.0; }
+double sht_plan_skip_fraction(const sht_plan* P, int forward) {
+    if (!P || !P->skip_ready) return 0.0;
+    const int d = forward ? 1 : 0;
+    return P->all_pairs[d] > 0 ? P->skip_pairs[d] / P->all_pairs[d] : 0.0;
+}
 double sht_plan_flops(const sht_plan* P, int forward) { return P ? (forward ? P->flops_fwd : P->flops_inv) : 0.0; }
 
 sht_status sht_plan_set_workspace(sht_plan* P, void* work, size_t work_bytes, sht_stream stream) {
