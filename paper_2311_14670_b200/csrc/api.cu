@@ -398,6 +398,14 @@ void layout(sht_plan* P, char* base) {
                 for (auto& ph : (dir ? P->pfwd : P->pinv)) np += ph.mode == md;
                 P->skip_nb[dir][md] = 0;
                 if (!np) continue;
+                if (P->dtype == SHT_F32) {            // the fp32 kernels use 64 x 128 tiles and a smaller state
+                    if (md != (dir ? P->pfwd[0].mode : P->pinv[0].mode)) continue;
+                    const int nb32 = (P->Lp / SHT_TQ) * (R.ntp / 128);
+                    P->skip_nb[dir][0] = nb32;
+                    P->skip_p0[dir][0] = B.take<int>(nb32);
+                    P->skip_state[dir][0] = reinterpret_cast<double*>(B.take<char>((size_t)nb32 * SHT_SKIP_STATE_BYTES_F32));
+                    continue;
+                }
                 ThetaArgs t{};
                 t.Lp = P->Lp; t.ntp = R.ntp; t.npass = np; t.nsm = P->nsm;
                 t.tile = (P->opts & SHT_OPT_TILE64) ? 64 : (P->opts & SHT_OPT_TILE128) ? 128 : 0;
@@ -757,6 +765,20 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
     return a;
 }
 
+// arguments of the fp32 kernels (theta_f32.cu) for one direction
+F32Args f32_args(const sht_plan* P, bool fwd) {
+    F32Args a{};
+    const RingSet& R = fwd ? P->fwd : P->inv;
+    const PassHost& ph = fwd ? P->pfwd[0] : P->pinv[0];
+    a.L = P->L; a.Lp = P->Lp; a.nth = R.nth; a.ntp = R.ntp; a.NB = P->NB; a.ldout = fwd ? 0 : P->F_ld;
+    a.fold0 = fwd ? P->fold0 : P->fold0i; a.nfull = R.nfull;
+    a.ab = P->ab32; a.lam32 = fwd ? P->lam32_fwd : P->lam32_inv;
+    a.st_val = fwd ? P->st32_fwd : P->st32_inv; a.st_k = fwd ? P->k16_fwd : P->k16_inv;
+    a.in = reinterpret_cast<const float2*>(ph.p.in);
+    a.out = fwd ? P->H : P->F + P->col0;             // (inverse: regular ring th -> map ring col0 + th)
+    if (P->skip_ready) { a.skip_p0 = P->skip_p0[fwd ? 1 : 0][0]; a.skip_state = reinterpret_cast<float*>(P->skip_state[fwd ? 1 : 0][0]); }
+    return a;
+}
 // Silent-head skip tables (internal.h ThetaArgs::skip_*), built once at sht_plan_set_workspace with the plan's own
 // kernels: (1) PROBE -- one full recursion per launch on the zeroed operand tables; every block records the first pair of steps (at least 8
 // steps below its ramp) in which any warp contributed; (2) the host turns that into p0 = the pairs a transform may skip: 8 steps of margin
@@ -766,6 +788,40 @@ ThetaArgs theta_args(const sht_plan* P, bool fwd, bool pm) {
 sht_status build_skip_tables(sht_plan* P, cudaStream_t st) {
     const int L = P->L, nlt = P->Lp / SHT_TQ;
     P->skip_pairs[0] = P->skip_pairs[1] = P->all_pairs[0] = P->all_pairs[1] = 0;
+    if (P->dtype == SHT_F32) {
+        // fp32 kernels (theta_f32.cu): every step projects every item there, so a skipped pair saves a whole pair.  Their recursion
+        // coefficients are plan-time tables; the operand tables are still all zero at this point.
+        for (int dir = 0; dir < 2; ++dir) {
+            const int nb = P->skip_nb[dir][0];
+            if (!nb) continue;
+            F32Args a = f32_args(P, dir != 0);
+            const int NC = (dir ? P->pfwd[0] : P->pinv[0]).mode == 0 ? 2 : 1, ntt = a.ntp / 128;
+            a.skip_p0 = P->skip_p0[dir][0]; a.skip_state = reinterpret_cast<float*>(P->skip_state[dir][0]);
+            CK(cudaMemsetAsync(a.skip_p0, 0, sizeof(int) * nb, st));
+            a.skip_mode = 1;
+            CK(launch_theta_f32(a, dir != 0, NC, st));
+            std::vector<int> h(nb);
+            CK(cudaMemcpyAsync(h.data(), a.skip_p0, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            for (int b = 0; b < nb; ++b) {
+                const int lt = nlt - 1 - b / ntt, l0 = lt * SHT_TQ;
+                const int mtop = l0 + SHT_TQ - 1 < L - 1 ? l0 + SHT_TQ - 1 : L - 1, npairs = (mtop + 2) / 2;
+                int p0 = 0;
+                if (h[b] > 0) {
+                    p0 = (h[b] == (1 << 30) ? npairs : h[b]) - 4;
+                    if (p0 < 4 || mtop - 2 * p0 >= l0 - 8) p0 = 0;
+                }
+                h[b] = p0;
+                if (l0 < L) { P->all_pairs[dir] += npairs; P->skip_pairs[dir] += p0; }
+            }
+            CK(cudaMemcpyAsync(a.skip_p0, h.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
+            a.skip_mode = 2;
+            CK(launch_theta_f32(a, dir != 0, NC, st));
+            CK(cudaStreamSynchronize(st));
+        }
+        P->skip_ready = true;
+        return SHT_OK;
+    }
     if (P->only_dir != 2 && P->H) {
         // the inverse kernels read their recursion coefficients g'_m(l), s_m from the operand rows that k_prep_inverse writes with every
         // transform: fill them once here, from all-zero harmonic coefficients (H serves as the zero array; the next transform zeroes it anyway)
@@ -896,12 +952,7 @@ sht_status run_theta_inverse(sht_plan* P, const double2* coef, cudaStream_t st) 
         CK(st_prep_inverse_f32(L, P->Lp, NC, coef, P->scale_inv, reinterpret_cast<float2*>(const_cast<double*>(ph.p.in)), st));
         CS(zero_async(P->F, sizeof(double2) * P->F_slab, st));
         stage(P, CAT_HOT, st);
-        F32Args a{};
-        a.L = L; a.Lp = P->Lp; a.nth = P->inv.nth; a.ntp = P->inv.ntp; a.NB = P->NB; a.ldout = P->F_ld;
-        a.fold0 = P->fold0i; a.nfull = P->inv.nfull;
-        a.ab = P->ab32; a.lam32 = P->lam32_inv; a.st_val = P->st32_inv; a.st_k = P->k16_inv;
-        a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->F + P->col0;       // regular ring th -> map ring col0 + th
-        CK(launch_theta_f32(a, false, NC, st));
+        CK(launch_theta_f32(f32_args(P, false), false, NC, st));
         CS(inverse_poles(P, coef, st));
         stage(P, CAT_STAGE, st);
         if (P->reality) CK(st_hermitian_rows(L, P->NB, P->F_ld, P->F_nrings, P->F, st));
@@ -971,11 +1022,7 @@ sht_status run_theta_forward(sht_plan* P, const double2* U, size_t U_slab, int l
         else CK(st_weight_split_f32(L, P->NB, ldu, pair, P->fwd.nth, P->fwd.ntp, NC, P->fwd.wq, U, W32, st));
         CS(zero_async(P->H, sizeof(double2) * P->H_slab, st));
         stage(P, CAT_HOT, st);
-        F32Args a{};
-        a.L = L; a.Lp = P->Lp; a.nth = P->fwd.nth; a.ntp = P->fwd.ntp; a.NB = P->NB; a.ldout = 0; a.fold0 = P->fold0;
-        a.ab = P->ab32; a.lam32 = P->lam32_fwd; a.st_val = P->st32_fwd; a.st_k = P->k16_fwd;
-        a.in = reinterpret_cast<const float2*>(ph.p.in); a.out = P->H;
-        CK(launch_theta_f32(a, true, NC, st));
+        CK(launch_theta_f32(f32_args(P, true), true, NC, st));
         return SHT_OK;
     }
     int slo, shi;
@@ -1192,7 +1239,7 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     // adjoint entry points run the transposed chain on single orders, so plans that offer them keep one order per column
     P->pair = (sampling == SHT_MW || sampling == SHT_MWSS) && !helper && !(opts & (SHT_OPT_ADJOINT | SHT_OPT_NO_PAIR));
     // silent-head skip of the fused kernels (build_skip_tables): single-map fp64 on-the-fly plans from L >= 1024
-    P->skip = !helper && batch == 1 && dtype == SHT_F64 && !(opts & (SHT_OPT_PRECOMPUTE | SHT_OPT_NO_SKIP)) && L >= 1024;
+    P->skip = !helper && batch == 1 && !(opts & (SHT_OPT_PRECOMPUTE | SHT_OPT_NO_SKIP)) && L >= 1024;      // (fp64 and fp32 kernels)
     // launch-bound sizes replay a captured CUDA graph (run_transform below)
     P->use_graph = !helper && loop == 1 && ((L <= 512 && !(opts & SHT_OPT_NO_GRAPH)) || (opts & SHT_OPT_GRAPH));
     if (spin != 0 && batch == 1 && dtype == SHT_F64 && !(opts & SHT_OPT_NO_INVSYM)) {

@@ -98,7 +98,11 @@ struct F32Args {
     const float2* in;         // inverse: G32[m][Lp][NC] float4 {Re, Re, Im, Im} of scale(l) f_lm; forward: W32[m][ntp/2][NSET][2 NC] float2 =
                               // (ring 2p, ring 2p+1) of q(theta) F_m(theta) (staging.cu k_weight_split_f32)
     double2* out;             // inverse: F[row][ldout]; forward: H[m + L - 1][Lp]   (fp64 accumulators shared with the fp64 staging)
+    int skip_mode;            // silent-head skip (see ThetaArgs): 0 = transform, 1 = probe, 2 = dump
+    int* skip_p0;             // [block] pairs of steps to skip
+    float* skip_state;        // [block][SHT_SKIP_STATE_BYTES_F32]: d_m, d_{m+1} pairs and window counters of the 256 threads
 };
+#define SHT_SKIP_STATE_BYTES_F32 (80 * 256 * 4)   // per block: 32 + 32 floats + 16 counter words per thread
 cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st);
 
 // launchers (theta_kernels.cu); mode 0 = PM (spin 0 complex: +m and -m from one pass), 1 = P (one order per step)

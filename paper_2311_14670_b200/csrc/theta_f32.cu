@@ -52,14 +52,50 @@ struct KPackF {
     }
 };
 // items are stored as float2 pairs: item q = component q & 1 of pair q >> 1
-template <int NP>
-__device__ __forceinline__ void window_check_f(float2 (&cur)[NP], float2 (&prev)[NP], KPackF& kp) {
+// `contrib` (probe instantiations only) is raised when an item reaches its last window: from then on it contributes to the sums
+template <int NP, bool TRACK>
+__device__ __forceinline__ void window_check_f(float2 (&cur)[NP], float2 (&prev)[NP], KPackF& kp, bool& contrib) {
     const float s = pow2f(-FW), top = pow2f(FTOP);
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
-        if (fabsf(cur[q].x) > top && kp.get(2 * q) != 0u) { cur[q].x *= s; prev[q].x *= s; kp.dec(2 * q); }
-        if (fabsf(cur[q].y) > top && kp.get(2 * q + 1) != 0u) { cur[q].y *= s; prev[q].y *= s; kp.dec(2 * q + 1); }
+        if (fabsf(cur[q].x) > top && kp.get(2 * q) != 0u) { cur[q].x *= s; prev[q].x *= s; kp.dec(2 * q); if (TRACK && kp.get(2 * q) == 0u) contrib = true; }
+        if (fabsf(cur[q].y) > top && kp.get(2 * q + 1) != 0u) { cur[q].y *= s; prev[q].y *= s; kp.dec(2 * q + 1); if (TRACK && kp.get(2 * q + 1) == 0u) contrib = true; }
     }
+}
+// ---- silent-head skip (internal.h ThetaArgs::skip_*): the state of a block at pair p0, thread-minor
+template <int NP>
+__device__ __forceinline__ void f32_state_store(const F32Args& A, int tid, const float2 (&cur)[NP], const float2 (&prev)[NP], const KPackF& kp) {
+    float* d = reinterpret_cast<float*>(reinterpret_cast<char*>(A.skip_state) + (size_t)blockIdx.x * SHT_SKIP_STATE_BYTES_F32);
+    uint32_t* u = reinterpret_cast<uint32_t*>(d + 64 * 256);
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        d[(2 * q) * 256 + tid] = cur[q].x; d[(2 * q + 1) * 256 + tid] = cur[q].y;
+        d[(32 + 2 * q) * 256 + tid] = prev[q].x; d[(32 + 2 * q + 1) * 256 + tid] = prev[q].y;
+    }
+#pragma unroll
+    for (int i = 0; i < 16; ++i) u[i * 256 + tid] = kp.w[i];
+}
+template <int NP>
+__device__ __forceinline__ void f32_state_load(const F32Args& A, int tid, float2 (&cur)[NP], float2 (&prev)[NP], KPackF& kp) {
+    const float* d = reinterpret_cast<const float*>(reinterpret_cast<const char*>(A.skip_state) + (size_t)blockIdx.x * SHT_SKIP_STATE_BYTES_F32);
+    const uint32_t* u = reinterpret_cast<const uint32_t*>(d + 64 * 256);
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        cur[q] = make_float2(d[(2 * q) * 256 + tid], d[(2 * q + 1) * 256 + tid]);
+        prev[q] = make_float2(d[(32 + 2 * q) * 256 + tid], d[(32 + 2 * q + 1) * 256 + tid]);
+    }
+#pragma unroll
+    for (int i = 0; i < 16; ++i) kp.w[i] = u[i * 256 + tid];
+}
+// pairs this launch skips / runs: SM 0 transform (skip p0), 1 probe (all), 2 dump (the first p0 pairs only; false if there are none)
+template <int SM>
+__device__ __forceinline__ bool f32_skip_range(const F32Args& A, int mtop, int& m_first, int& m_last) {
+    m_first = mtop; m_last = 0;
+    if (SM == 1 || !A.skip_p0) return true;
+    const int p0 = A.skip_p0[blockIdx.x];
+    if (SM == 2) { m_last = mtop - 2 * p0 + 1; return p0 > 0; }
+    m_first = mtop - 2 * p0;
+    return true;
 }
 
 
@@ -70,7 +106,7 @@ __device__ __forceinline__ void window_check_f(float2 (&cur)[NP], float2 (&prev)
 // FOLD (rings symmetric about the equator, northern half recursed): d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta).  The
 // degrees of a warp all have one parity (warp w: l0 + 16 (w/2) + (w%2) + 2j), the reducers add the even-degree and the odd-degree warps
 // apart (E0, E1) and write F_m(theta) = E0 + E1 and F_m(pi - theta) = (-1)^m (E0 - E1), as the fp64 kernel does.
-template <int NC, bool FOLD>
+template <int NC, bool FOLD, int SM>
 __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A) {
     constexpr int RL = 8, RP = 2, NP = RL * RP, DS = FOLD ? 2 : 1, C4 = 2 * NC;      // RP ring pairs per thread; C4 real columns
     __shared__ float4 s_ab[2][TLF];                  // {A, A, -B, -B} of the block's degrees: operands arrive duplicated for the packed math
@@ -83,6 +119,9 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
     if (l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int mtop = min(l0 + TLF - 1, A.L - 1);
+    int m_first, m_last;                              // steps m_first .. m_last of the recursion run in this launch (silent-head skip)
+    if (!f32_skip_range<SM>(A, mtop, m_first, m_last)) return;
+    bool contrib = false;                             // (probe) some item of this thread is in its last window
     const int la = FOLD ? l0 + 2 * RL * (w >> 1) + (w & 1) : l0 + w * RL;         // degrees of this warp: la + DS j
 
     // operand rows of step m, one element per thread, copied global -> shared asynchronously (cp.async): the copy of step m-1
@@ -100,7 +139,9 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
     kp.fill(0u);
 #pragma unroll
     for (int q = 0; q < NP; ++q) { cur[q] = make_float2(0.f, 0.f); prev[q] = make_float2(0.f, 0.f); }
-    load_ops(mtop, 0);
+    if (SM == 0 && m_first < mtop) f32_state_load<NP>(A, tid, cur, prev, kp);
+    if (SM == 1 && tid == 0) A.skip_p0[blockIdx.x] = 1 << 30;
+    load_ops(m_first, 0);
     __pipeline_wait_prior(0);
     __syncthreads();
 
@@ -142,6 +183,7 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
                         ca[j * RP + ip] = *reinterpret_cast<const float2*>(A.st_val + o); cb[j * RP + ip] = make_float2(0.f, 0.f);
                         const ushort2 k2 = *reinterpret_cast<const ushort2*>(A.st_k + o);
                         kp.set(2 * (j * RP + ip), k2.x); kp.set(2 * (j * RP + ip) + 1, k2.y);
+                        if (SM == 1 && (k2.x == 0 || k2.y == 0)) contrib = true;
                     }
                 }
         }
@@ -173,7 +215,7 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
                     cb[j * RP + ip] = __ffma2_rn(__fmul2_rn(lam[ip], A2), e, __fmul2_rn(nB2, cb[j * RP + ip]));
                 }
             }
-            if (kp.any_nonzero()) window_check_f<NP>(cb, ca, kp);
+            if (kp.any_nonzero()) window_check_f<NP, SM == 1>(cb, ca, kp, contrib);
         }
         const int pb = buf;                         // partial-sum buffer of this step (alternates with the operand buffer)
 #pragma unroll
@@ -181,13 +223,18 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
 #pragma unroll
             for (int c = 0; c < C4; ++c) *reinterpret_cast<float2*>(&s_part[pb][w][c][2 * lane + 64 * ip]) = acc[ip][c];
         __pipeline_wait_prior(0);
-        __syncthreads();                            // the only block barrier of the step: partial sums of m and operands of m-1 are visible;
+        if (SM == 1) {                              // probe: first pair, 8 steps below the ramp or later, in which any thread contributes
+            const int any = __syncthreads_or(contrib);
+            if (tid == 0 && any && m < l0 - 8 && A.skip_p0[blockIdx.x] == (1 << 30)) A.skip_p0[blockIdx.x] = (mtop - m) / 2;
+        } else
+            __syncthreads();                        // the only block barrier of the step: partial sums of m and operands of m-1 are visible;
         reduce(m, pb);                              // buffer pb is next written two steps from now, after the barrier of step m-1
     };
-    for (int m = mtop; m >= 0; m -= 2) {
-        step(m, (mtop - m) & 1, cur, prev);
-        if (m - 1 >= 0) step(m - 1, (mtop - m + 1) & 1, prev, cur);
+    for (int m = m_first; m >= m_last; m -= 2) {
+        step(m, (m_first - m) & 1, cur, prev);
+        if (m - 1 >= m_last) step(m - 1, (m_first - m + 1) & 1, prev, cur);
     }
+    if (SM == 2) f32_state_store<NP>(A, tid, cur, prev, kp);
 }
 
 // =============================================================================================================
@@ -197,7 +244,7 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
 // with l+m even contracts with E, one with l+m odd with O (d^l_{m0}(pi - theta) = (-1)^{l+m} d^l_{m0}(theta)).  A thread's two
 // degrees share their parity, which alternates with the lane: one load with two addresses serves both (as in theta_kernels.cu).
 // =============================================================================================================
-template <int NC, bool FOLD>
+template <int NC, bool FOLD, int SM>
 __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A) {
     constexpr int RL = 2, RP = 8, NP = RL * RP, NSET = FOLD ? 2 : 1, C4 = 2 * NC, NPB = NTF / 2;      // NPB ring pairs per block
     __shared__ float4 s_ab[2][TLF];
@@ -210,6 +257,9 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A
     if (l0 >= A.L || th0 >= A.nth) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int mtop = min(l0 + TLF - 1, A.L - 1);
+    int m_first, m_last;
+    if (!f32_skip_range<SM>(A, mtop, m_first, m_last)) return;
+    bool contrib = false;
 
     auto load_ops = [&](int m, int buf) {
         if (tid < TLF) __pipeline_memcpy_async(&s_ab[buf][tid], &A.ab[(size_t)m * A.Lp + l0 + tid], sizeof(float4));
@@ -228,7 +278,9 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A
     int lr[RL];
 #pragma unroll
     for (int r = 0; r < RL; ++r) lr[r] = l0 + lane + 32 * r;
-    load_ops(mtop, 0);
+    if (SM == 0 && m_first < mtop) f32_state_load<NP>(A, tid, cur, prev, kp);
+    if (SM == 1 && tid == 0) A.skip_p0[blockIdx.x] = 1 << 30;
+    load_ops(m_first, 0);
     __pipeline_wait_prior(0);
     __syncthreads();
 
@@ -243,6 +295,7 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A
                     ca[r * RP + ip] = *reinterpret_cast<const float2*>(A.st_val + o); cb[r * RP + ip] = make_float2(0.f, 0.f);
                     const ushort2 k2 = *reinterpret_cast<const ushort2*>(A.st_k + o);
                     kp.set(2 * (r * RP + ip), k2.x); kp.set(2 * (r * RP + ip) + 1, k2.y);
+                    if (SM == 1 && (k2.x == 0 || k2.y == 0)) contrib = true;
                 }
             }
         float2 acc[RL][C4];
@@ -273,13 +326,17 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A
                 cb[r * RP + ip] = __ffma2_rn(__fmul2_rn(lam, A2[r]), e, __fmul2_rn(nB2[r], cb[r * RP + ip]));
             }
         }
-        if (kp.any_nonzero()) window_check_f<NP>(cb, ca, kp);
+        if (kp.any_nonzero()) window_check_f<NP, SM == 1>(cb, ca, kp, contrib);
 #pragma unroll
         for (int r = 0; r < RL; ++r)
 #pragma unroll
             for (int c = 0; c < C4; ++c) s_part[buf][w][c][lane + 32 * r] = acc[r][c].x + acc[r][c].y;      // the pair's two rings
         __pipeline_wait_prior(0);
-        __syncthreads();                            // the only block barrier of the step (partial sums double-buffered, see the inverse)
+        if (SM == 1) {
+            const int any = __syncthreads_or(contrib);
+            if (tid == 0 && any && m < l0 - 8 && A.skip_p0[blockIdx.x] == (1 << 30)) A.skip_p0[blockIdx.x] = (mtop - m) / 2;
+        } else
+            __syncthreads();                        // the only block barrier of the step (partial sums double-buffered, see the inverse)
         for (int o = tid; o < NC * TLF; o += NWF * 32) {
             const int c = o / TLF, t = o % TLF, l = l0 + t;
             float sx = 0.f, sy = 0.f;
@@ -292,29 +349,36 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A
             }
         }
     };
-    for (int m = mtop; m >= 0; m -= 2) {
-        step(m, (mtop - m) & 1, cur, prev);
-        if (m - 1 >= 0) step(m - 1, (mtop - m + 1) & 1, prev, cur);
+    for (int m = m_first; m >= m_last; m -= 2) {
+        step(m, (m_first - m) & 1, cur, prev);
+        if (m - 1 >= m_last) step(m - 1, (m_first - m + 1) & 1, prev, cur);
     }
+    if (SM == 2) f32_state_store<NP>(A, tid, cur, prev, kp);
 }
 
 }  // namespace
 
+template <int SM>
+static void launch_f32_mode(const F32Args& a, bool forward, int NC, dim3 grid, cudaStream_t st) {
+    if (forward && a.fold0) {
+        if (NC == 2) theta_forward_f32<2, true, SM><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_forward_f32<1, true, SM><<<grid, NWF * 32, 0, st>>>(a);
+    } else if (forward) {
+        if (NC == 2) theta_forward_f32<2, false, SM><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_forward_f32<1, false, SM><<<grid, NWF * 32, 0, st>>>(a);
+    } else if (a.fold0) {
+        if (NC == 2) theta_inverse_f32<2, true, SM><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_inverse_f32<1, true, SM><<<grid, NWF * 32, 0, st>>>(a);
+    } else {
+        if (NC == 2) theta_inverse_f32<2, false, SM><<<grid, NWF * 32, 0, st>>>(a);
+        else theta_inverse_f32<1, false, SM><<<grid, NWF * 32, 0, st>>>(a);
+    }
+}
 cudaError_t launch_theta_f32(const F32Args& a, bool forward, int NC, cudaStream_t st) {
     dim3 grid((a.Lp / TLF) * (a.ntp / NTF));
-    if (forward && a.fold0) {
-        if (NC == 2) theta_forward_f32<2, true><<<grid, NWF * 32, 0, st>>>(a);
-        else theta_forward_f32<1, true><<<grid, NWF * 32, 0, st>>>(a);
-    } else if (forward) {
-        if (NC == 2) theta_forward_f32<2, false><<<grid, NWF * 32, 0, st>>>(a);
-        else theta_forward_f32<1, false><<<grid, NWF * 32, 0, st>>>(a);
-    } else if (a.fold0) {
-        if (NC == 2) theta_inverse_f32<2, true><<<grid, NWF * 32, 0, st>>>(a);
-        else theta_inverse_f32<1, true><<<grid, NWF * 32, 0, st>>>(a);
-    } else {
-        if (NC == 2) theta_inverse_f32<2, false><<<grid, NWF * 32, 0, st>>>(a);
-        else theta_inverse_f32<1, false><<<grid, NWF * 32, 0, st>>>(a);
-    }
+    if (a.skip_mode == 1) launch_f32_mode<1>(a, forward, NC, grid, st);
+    else if (a.skip_mode == 2) launch_f32_mode<2>(a, forward, NC, grid, st);
+    else launch_f32_mode<0>(a, forward, NC, grid, st);
     count_launch();
     return cudaGetLastError();
 }

@@ -158,7 +158,7 @@ def test_graph_replay_equals_direct_launches(kind):
         assert float((keep[-1] - second).abs().max()) <= tol * float(second.abs().max())
 
 
-@pytest.mark.parametrize("kind", ["mw0", "mw2", "hp", "dh1", "so3"])
+@pytest.mark.parametrize("kind", ["mw0", "mw2", "hp", "dh1", "f32", "so3"])
 def test_silent_head_skip_equals_running_every_step(kind):
     """From L = 1024 the fused kernels start each block tile from a register state stored at plan time, skipping the pairs of steps in
     which no iterate of the tile has left its first window (include/b200sht.h SHT_OPT_NO_SKIP).  Those steps
@@ -167,14 +167,19 @@ def test_silent_head_skip_equals_running_every_step(kind):
     if kind == "so3":
         pytest.skip("SO(3) plans of L >= 1024 need tens of GB of tables: covered by the S^2 cases (same kernels, same passes)")
     L = 1100 if kind != "hp" else 1024
-    kw = dict(mw0=dict(spin=0), mw2=dict(spin=2), hp=dict(spin=0, sampling=A.HEALPIX, nside=512, reality=True), dh1=dict(spin=-1, sampling=A.DH))[kind]
+    kw = dict(mw0=dict(spin=0), mw2=dict(spin=2), hp=dict(spin=0, sampling=A.HEALPIX, nside=512, reality=True), dh1=dict(spin=-1, sampling=A.DH),
+              f32=dict(spin=0, dtype="f32"))[kind]
+    tol = 1e-4 if kind == "f32" else 1e-13       # (fp32: agreement at the level of the fp32 rounding of the transform, north_star tolerance)
     Ps, Pn = A.Plan(L, **kw), A.Plan(L, skip=False, **kw)
-    flm = torch.from_numpy(synth.random_flm(L, kw["spin"], seed=3, real=kind == "hp")).cuda()
+    assert Ps.skip_fraction(True) > 0.01 and Pn.skip_fraction(True) == 0.0
+    flm = synth.random_flm(L, kw["spin"], seed=3, real=kind == "hp")
+    flm = torch.from_numpy(flm.astype(np.complex64) if kind == "f32" else flm).cuda()
     f1, f2 = Ps.inverse(flm), Pn.inverse(flm)
-    assert float((f1 - f2).abs().max()) <= 1e-13 * float(f2.abs().max())
-    g = torch.from_numpy(synth.random_map(tuple(f2.shape), seed=4, real=kind == "hp")).cuda()
+    assert float((f1 - f2).abs().max()) <= tol * float(f2.abs().max())
+    g = synth.random_map(tuple(f2.shape), seed=4, real=kind == "hp")
+    g = torch.from_numpy(g.astype(np.complex64) if kind == "f32" else g).cuda()
     c1, c2 = Ps.forward(g), Pn.forward(g)
-    assert float((c1 - c2).abs().max()) <= 1e-13 * float(c2.abs().max())
-    # twelve repetitions with the skip: the loaded state is read-only
+    assert float((c1 - c2).abs().max()) <= tol * float(c2.abs().max())
+    # repetitions with the skip: the loaded state is read-only
     for _ in range(3):
-        assert float((Ps.inverse(flm) - f2).abs().max()) <= 1e-13 * float(f2.abs().max())
+        assert float((Ps.inverse(flm) - f2).abs().max()) <= tol * float(f2.abs().max())
