@@ -42,6 +42,16 @@ __device__ __forceinline__ bool skip_range(const ThetaArgs& A, unsigned bid, int
     pbeg = p0;                                                // transform: start where the head ends
     return true;
 }
+// probe: does any item of the warp matter yet?  An iterate contributes to the sums through c_m(l) e (internal.h), c <= 2^250; one whose
+// last window is reached (k = 0) but whose magnitude is still below 2^-330 adds less than 2^-80 of an O(1) sum: as silent as one with k > 0.
+#define SHT_HI_SIGNIF ((1023 - 330) << 20)
+template <int NI>
+__device__ __forceinline__ bool warp_matters(const double (&cur)[NI], const KPack<NI>& kp) {
+    bool big = false;
+#pragma unroll
+    for (int q = 0; q < NI; ++q) big = big || (kp.get(q) == 0u && hi_abs(cur[q]) > SHT_HI_SIGNIF);
+    return __any_sync(0xffffffffu, big);
+}
 template <int NI>
 __device__ __forceinline__ void skip_store(const ThetaArgs& A, unsigned bid, int ctid, const double (&cur)[NI], const double (&prev)[NI],
                                            const KPack<NI>& kp, bool wact) {
@@ -168,7 +178,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
             if (SM == 1 && at == 0) {                  // probe: first pair, 8 steps below the ramp or later, in which any warp contributed
                 int fl = 0;
 #pragma unroll
-                for (int ww = 0; ww < NW; ++ww) fl |= sm.act[rs][ww];
+                for (int ww = 0; ww < NW; ++ww) fl |= sm.act[rs][ww] & 4;
                 if (p == 0) A.skip_p0[bid] = 1 << 30;
                 if (fl && mtop - KS * p < l0 - 8 && A.skip_p0[bid] == (1 << 30)) A.skip_p0[bid] = p;
             }
@@ -331,6 +341,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_inverse_kernel(cons
         int flags = 0;
         if (step(m, slot, rs, 0, cur, prev)) flags |= 1;
         if (step(m - 1, slot, rs, 1, prev, cur)) flags |= 2;
+        if (SM == 1 && warp_matters<NI>(cur, kp)) flags |= 4;
         __syncwarp();
         if (lane == 0) {
             sm.act[rs][w] = flags;
@@ -457,7 +468,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
             if (SM == 1 && at == 0) {                  // probe (see the inverse kernel)
                 int fl = 0;
 #pragma unroll
-                for (int ww = 0; ww < NW; ++ww) fl |= actb[ww];
+                for (int ww = 0; ww < NW; ++ww) fl |= actb[ww] & 4;
                 if (p == 0) A.skip_p0[bid] = 1 << 30;
                 if (fl && mtop - KS * p < l0 - 8 && A.skip_p0[bid] == (1 << 30)) A.skip_p0[bid] = p;
             }
@@ -626,6 +637,7 @@ __global__ void __launch_bounds__((NW + NAUX) * 32, 1) theta_forward_kernel(cons
         int flags = 0;
         if (step(m, slot, rs, 0, cur, prev)) flags |= 1;
         if (step(m - 1, slot, rs, 1, prev, cur)) flags |= 2;
+        if (SM == 1 && warp_matters<NI>(cur, kp)) flags |= 4;
         __syncwarp();
         if (lane == 0) {
             sm.act[rs][w] = flags;
