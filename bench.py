@@ -33,9 +33,9 @@ UNIT = "transform_pairs/s"
 # profiles/ (file named beside each); key (L, spin, batch).  Not measurable inside this process: null for other workloads.
 NCU_TRAFFIC_BYTES = {
     (1024, 2, 1): (127.888128e6 + 10.841600e6, "profiles/r2b_theta_kernels.md"),
-    (2048, 0, 1): (1.329291e9 + 126.638336e6, "profiles/r2b_theta_kernels.md"),
-    (4096, 0, 1): (37.860121e9 + 1.936975e9, "profiles/r2b_theta_kernels.md"),
-    (8192, 0, 1): (337.503584e9 + 24.737303e9, "profiles/r2b_theta_kernels.md"),
+    (2048, 0, 1): (1.801608e9 + 336.916480e6, "profiles/r2d_theta_kernels.md"),
+    (4096, 0, 1): (31.937931e9 + 3.441399e9, "profiles/r2d_theta_kernels.md"),
+    (8192, 0, 1): (260.120313e9 + 31.275355e9, "profiles/r2d_theta_kernels.md"),
     (2048, 0, 16): (46.052300e9 + 11.329958e9, "profiles/r2_theta_kernels.md"),
 }
 

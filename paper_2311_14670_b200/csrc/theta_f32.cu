@@ -62,6 +62,17 @@ __device__ __forceinline__ void window_check_f(float2 (&cur)[NP], float2 (&prev)
         if (fabsf(cur[q].y) > top && kp.get(2 * q + 1) != 0u) { cur[q].y *= s; prev[q].y *= s; kp.dec(2 * q + 1); if (TRACK && kp.get(2 * q + 1) == 0u) contrib = true; }
     }
 }
+// probe: does any item of this thread matter yet?  One in its last window (k = 0) whose magnitude is still below 2^-40 adds less than fp32
+// resolution of an O(1) sum by a factor 2^16: as silent as one with k > 0.  (Items that have not started hold 0.)
+template <int NP>
+__device__ __forceinline__ bool f32_matters(const float2 (&cur)[NP], const KPackF& kp) {
+    const float thr = pow2f(-40);
+    bool big = false;
+#pragma unroll
+    for (int q = 0; q < NP; ++q)
+        big = big || (kp.get(2 * q) == 0u && fabsf(cur[q].x) > thr) || (kp.get(2 * q + 1) == 0u && fabsf(cur[q].y) > thr);
+    return big;
+}
 // ---- silent-head skip (internal.h ThetaArgs::skip_*): the state of a block at pair p0, thread-minor
 template <int NP>
 __device__ __forceinline__ void f32_state_store(const F32Args& A, int tid, const float2 (&cur)[NP], const float2 (&prev)[NP], const KPackF& kp) {
@@ -224,7 +235,7 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_inverse_f32(const F32Args A
             for (int c = 0; c < C4; ++c) *reinterpret_cast<float2*>(&s_part[pb][w][c][2 * lane + 64 * ip]) = acc[ip][c];
         __pipeline_wait_prior(0);
         if (SM == 1) {                              // probe: first pair, 8 steps below the ramp or later, in which any thread contributes
-            const int any = __syncthreads_or(contrib);
+            const int any = __syncthreads_or(f32_matters<NP>(cb, kp));
             if (tid == 0 && any && m < l0 - 8 && A.skip_p0[blockIdx.x] == (1 << 30)) A.skip_p0[blockIdx.x] = (mtop - m) / 2;
         } else
             __syncthreads();                        // the only block barrier of the step: partial sums of m and operands of m-1 are visible;
@@ -333,7 +344,7 @@ __global__ void __launch_bounds__(NWF * 32, 2) theta_forward_f32(const F32Args A
             for (int c = 0; c < C4; ++c) s_part[buf][w][c][lane + 32 * r] = acc[r][c].x + acc[r][c].y;      // the pair's two rings
         __pipeline_wait_prior(0);
         if (SM == 1) {
-            const int any = __syncthreads_or(contrib);
+            const int any = __syncthreads_or(f32_matters<NP>(cb, kp));
             if (tid == 0 && any && m < l0 - 8 && A.skip_p0[blockIdx.x] == (1 << 30)) A.skip_p0[blockIdx.x] = (mtop - m) / 2;
         } else
             __syncthreads();                        // the only block barrier of the step (partial sums double-buffered, see the inverse)
