@@ -39,7 +39,7 @@ CASES = [("mw", 0), ("mwss", 0), ("dh", 0), ("gl", 0), ("hp", 8)]
 
 
 @pytest.mark.parametrize("name,nside", CASES)
-@pytest.mark.parametrize("L,spin", [(8, 0), (33, 0), (40, 2), (64, -1), (130, 2), (200, 0), (257, 2)])
+@pytest.mark.parametrize("L,spin", [(8, 0), (33, 0), (40, 2), (64, -1), (130, 2), (200, 0), (257, 2), (1030, 1)])     # (1030: transforms start from the silent-head state)
 def test_dot_product_identities(api, orc, name, nside, L, spin):
     P, os_ = plan_for(api, orc, name, L, spin, nside=nside)
     x = synth.random_map(P.map_shape, seed=L)

@@ -31,7 +31,8 @@ def relt(a, b):
 @pytest.mark.parametrize("K", [2, 3, 8])
 @pytest.mark.parametrize("kind,L,spin,kw", [("mw", 130, 0, {}), ("mw", 200, 2, {}), ("mw", 257, 0, dict(fold=True)), ("mw", 96, 0, dict(reality=True)),
                                             ("mwss", 130, 1, {}), ("dh", 64, 0, {}), ("gl", 131, -2, {}), ("hp", 64, 0, dict(nside=32, reality=True)),
-                                            ("hp", 40, 2, dict(nside=16))])
+                                            ("hp", 40, 2, dict(nside=16)),
+                                            ("mw", 1100, 0, {}), ("dh", 1030, 1, {})])      # (L >= 1024: blocks start from the stored silent-head state)
 def test_sum_over_ring_shards_is_the_transform(api, kind, L, spin, kw, K):
     samp = {"mw": api.MW, "mwss": api.MWSS, "dh": api.DH, "gl": api.GL, "hp": api.HEALPIX}[kind]
     real = kw.get("reality", False)
