@@ -237,6 +237,27 @@ sht_status s2_inverse_host(int L, int spin, int sampling, int reality, const voi
 sht_status so3_forward_host(int L, int N, const void* f_host, void* flmn_host, sht_stream stream);
 sht_status so3_inverse_host(int L, int N, const void* flmn_host, void* f_host, sht_stream stream);
 
+/* ---- allocation-free entry point -----------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): the theta
+ * step of the inverse transform, Eq. 33 with the Wigner d-functions of Eq. 25-29, on caller-given rings -- what
+ * s2_theta_inverse_plan computes -- with no plan, no workspace and no cudaMalloc / cudaFree / cuFFT call.  A variant of the stored-table
+ * kernels of SHT_OPT_PRECOMPUTE (Sec. 4.3) whose d-function table E[2L-1][ntheta][L] lives in one static device array of
+ * SHT_NOALLOC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until the process exits).
+ *   L, spin : band-limit and spin, |spin| < L.
+ *   theta   : HOST array of ntheta ring colatitudes in [0, pi] (read before the call returns; pole rings take Eq. 28 / 29).
+ *   flm     : DEVICE, complex128 [L][2L-1] (column m + L - 1), read only.
+ *   Fm      : DEVICE, complex128 [2L-1][ntheta] (row m + L - 1), every entry written; need not be cleared.
+ *   err     : optional HOST buffer of err_len bytes that receives the text of a failure ("" on success); may be NULL.
+ * Limits: 1 <= ntheta <= SHT_NOALLOC_MAX_RINGS and (2L-1) * ntheta * L * 8 bytes <= SHT_NOALLOC_SCRATCH_BYTES (e.g. L = 64 on
+ * 2L = 128 rings, L = 80 on L rings); beyond them SHT_EUNSUPPORTED with the reason in err, nothing launched.  The two kernels are
+ * enqueued on `stream`; the call does not synchronise.  Every call shares the static table (its first kernel rewrites every entry
+ * the second reads, so no state carries over between calls): calls that may overlap on the GPU -- different streams without an
+ * event between them, or host threads on one device -- race on it and must be ordered by the caller.  fp64, single map. */
+#define SHT_NOALLOC_SCRATCH_BYTES (8 << 20)
+#define SHT_NOALLOC_MAX_RINGS 128
+sht_status s2_theta_inverse_noalloc(int L, int spin, int ntheta, const double* theta, const void* flm, void* Fm, sht_stream stream,
+                                    char* err, size_t err_len);
+
 /* ---- measurement helpers: register-only instruction chains, return achieved TFLOP/s and kernel ms (used by bench.py for the
  * roofline denominators, since MEASURED_PEAKS.json has no FP64 / FP32 ALU entries).  kind: SHT_PEAK_DFMA (fma.f64),
  * SHT_PEAK_DMMA (mma.sync.m8n8k4.f64, the FP64 tensor-core path of the batched kernels), SHT_PEAK_FFMA (fma.f32),

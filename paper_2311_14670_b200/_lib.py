@@ -11,6 +11,7 @@ SHT_F64, SHT_F32 = 0, 1
 SHT_OPT_FOLD_ON, SHT_OPT_FOLD_OFF, SHT_OPT_INVSYM, SHT_OPT_TILE64, SHT_OPT_TILE128, SHT_OPT_ADJOINT, SHT_OPT_PRECOMPUTE, SHT_OPT_NO_INVSYM = 1, 2, 4, 8, 16, 32, 64, 128
 SHT_OPT_NO_PAIR, SHT_OPT_GRAPH, SHT_OPT_NO_GRAPH, SHT_OPT_NO_SKIP = 256, 512, 1024, 2048
 SHT_PEAK_DFMA, SHT_PEAK_DMMA, SHT_PEAK_FFMA, SHT_PEAK_FFMA2 = 0, 1, 2, 3
+SHT_NOALLOC_SCRATCH_BYTES, SHT_NOALLOC_MAX_RINGS = 8 << 20, 128
 
 # every symbol include/b200sht.h declares: name -> (restype, argtypes)
 _vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
@@ -61,6 +62,7 @@ SIGNATURES = {
     "sht_plan_flops": (C.c_double, [_vp, _i]),
     "sht_plan_skip_fraction": (C.c_double, [_vp, _i]),
     "sht_version": (C.c_char_p, []),
+    "s2_theta_inverse_noalloc": (_i, [_i, _i, _i, C.POINTER(C.c_double), _vp, _vp, _vp, C.c_char_p, _sz]),
 }
 
 _lib = None

@@ -295,3 +295,22 @@ def launch_count(reset=False):
 
 def cache_clear():
     check(lib().sht_cache_clear())
+
+
+def theta_inverse_noalloc(flm, L, spin, theta, out=None):
+    """Allocation-free theta step of the inverse transform (Eq. 33) on the rings `theta` (host sequence of colatitudes): flm[L, 2L-1]
+    -> F[2L-1, len(theta)].  The library call allocates nothing (d-function table in a static device array of
+    SHT_NOALLOC_SCRATCH_BYTES); pass `out` to keep this wrapper from allocating the result too.  Calls share the static table:
+    do not overlap them on the GPU."""
+    th = np.ascontiguousarray(np.asarray(theta, dtype=np.float64).ravel())
+    nt = int(th.size)
+    shape = (2 * L - 1, nt)
+    if out is None:
+        out = torch.empty(shape, dtype=torch.complex128, device=flm.device)
+    err = C.create_string_buffer(512)
+    rc = lib().s2_theta_inverse_noalloc(int(L), int(spin), nt, th.ctypes.data_as(C.POINTER(C.c_double)),
+                                        _dev(flm, torch.complex128, (L, 2 * L - 1), "flm"), _dev(out, torch.complex128, shape, "F"),
+                                        _stream(), err, len(err))
+    if rc != 0:
+        raise _lib.ShtError(f"{lib().sht_status_string(rc).decode()} [{err.value.decode()}]")
+    return out

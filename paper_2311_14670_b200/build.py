@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libb200sht.so")
-SOURCES = ["api.cu", "staging.cu", "healpix.cu", "theta_kernels.cu", "theta_mma.cu", "theta_f32.cu", "peaks.cu", "precompute.cu"]
+SOURCES = ["api.cu", "staging.cu", "healpix.cu", "theta_kernels.cu", "theta_mma.cu", "theta_f32.cu", "peaks.cu", "precompute.cu", "noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-Xptxas", "-v"]
