@@ -112,27 +112,42 @@ class ClockSampler:
                     reasons=sorted(reasons), samples=len(sm), power_w_max=max(pw) if pw else None)
 
 
+_QUAD_TABLE_S = {}     # L -> seconds the oracle takes to build the ring table of its 2L quadrature rings (measured once per process)
+
+
 def oracle_sample(L, spin, flm, n_cols):
     """Time the CPU oracle (as it stands) on a bounded sample of the workload and extrapolate to one inverse + one forward.
 
-    Sample: the theta steps (Eq. 33 and Eq. 30, the O(L^3) part) of n_cols harmonic orders m spread over [-(L-1), L-1], all rings.
+    Sample: the theta steps (Eq. 33 and Eq. 30, the O(L^3) part) of n_cols harmonic orders m spread over [-(L-1), L-1].
     The cost of a column is proportional to L - |m| (the l-recurrence of the oracle's d-functions starts at l = |m|), so the
-    sample is scaled by sum_m (L - |m|) / sum_sample (L - |m|).  The oracle's ring DFTs are deliberately naive O(n^2) sums and are
-    NOT part of the sample (they would take 13 s per ring at L = 8192); the extrapolated time therefore flatters the oracle."""
+    sample is scaled by sum_m (L - |m|) / sum_sample (L - |m|).  The inverse runs on all L MW rings.  The oracle's forward runs on
+    its 2L quadrature rings, whose ring table (an O(L^2) long-double sum for the weights: 30-120 s at L = 8192) it rebuilds in every
+    call: that table is timed ONCE per process (it is needed once per transform, not once per sampled column -- scaling it with the
+    columns, as this function did before, overstated the oracle's forward time about five-fold), and the columns are timed on the L
+    MW rings (a per-ring cost, so x 2 for the 2L quadrature rings).  forward = table + 2 x scaled columns.  The oracle's ring DFTs are
+    deliberately naive O(n^2) sums and are NOT part of the sample (they would take 13 s per ring at L = 8192); the extrapolated time
+    therefore flatters the oracle."""
     import oracle as O
     ms = np.unique(np.linspace(-(L - 1), L - 1, n_cols).astype(int))
     scale = float(L * L) / float(np.sum(L - np.abs(ms)))          # sum_{|m| < L} (L - |m|) = L^2
     t0 = time.perf_counter()
     F = O.s2_theta_inverse_columns(L, spin, O.MW, flm, ms)
     t_inv = (time.perf_counter() - t0) * scale
-    # forward theta step on the oracle's 2L quadrature rings: the values do not matter for timing
-    W = np.zeros((len(ms), 2 * L), np.complex128)
-    W[:, :F.shape[1]] = F
+    if L not in _QUAD_TABLE_S:
+        t0 = time.perf_counter()
+        O.ring_table(O.MW_QUAD, L)
+        _QUAD_TABLE_S[L] = time.perf_counter() - t0
+    # forward theta step: the values do not matter for timing
     t0 = time.perf_counter()
-    O.s2_theta_forward_columns(L, spin, O.MW_QUAD, W, ms)
-    t_fwd = (time.perf_counter() - t0) * scale
-    return t_inv, t_fwd, O.threads(), (f"theta steps (Eq. 33 on the {L} MW rings, Eq. 30 on the {2 * L} quadrature rings) of {len(ms)} of "
-                                       f"{2 * L - 1} orders m, scaled by sum(L-|m|); naive O(n^2) ring DFTs of the oracle excluded")
+    O.s2_theta_forward_columns(L, spin, O.MW, np.ascontiguousarray(F), ms)
+    t_fwd = _QUAD_TABLE_S[L] + 2.0 * (time.perf_counter() - t0) * scale
+    return t_inv, t_fwd, O.threads(), (f"theta steps of {len(ms)} of {2 * L - 1} orders m, scaled by sum(L-|m|): Eq. 33 on the {L} MW rings; Eq. 30 on "
+                                       f"the {L} MW rings x 2 (the oracle's forward uses {2 * L} quadrature rings) + its quadrature ring table "
+                                       f"({_QUAD_TABLE_S[L]:.1f} s, timed once); naive O(n^2) ring DFTs of the oracle excluded")
+
+
+REF_COLS = 16          # orders m per step of `--impl reference`: one per thread on the 16-thread GPU box, about 5 s per step at L = 8192, so that
+                       # the driver's --steps 20 --warmup 5 run ends in about 3 minutes (plus the quadrature table, once)
 
 
 def run_reference(args):
@@ -146,7 +161,7 @@ def run_reference(args):
     times = []
     sample = ""
     for i in range(args.warmup + args.steps):
-        t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm, n_cols=16)
+        t_inv, t_fwd, cores, sample = oracle_sample(L, spin, flm, n_cols=REF_COLS)
         if i >= args.warmup:
             times.append(t_inv + t_fwd)
     t = float(np.mean(times))
