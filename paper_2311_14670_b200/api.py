@@ -64,7 +64,7 @@ class Plan:
         self.batch = int(batch)
         if dtype not in ("f64", "f32"):
             raise ValueError("dtype must be 'f64' or 'f32'")
-        self.dtype = dtype          # 'f32': fp32 hot kernels and complex64 / float32 arrays (spin 0, MW, batch 1)
+        self.dtype = dtype          # 'f32': complex64 / float32 arrays; fp32 hot kernels for spin 0, the fp64 kernels between fp32 arrays for spin != 0
         code = SHT_F32 if dtype == "f32" else SHT_F64
         self.device = torch.device(device)
         L_ = lib()

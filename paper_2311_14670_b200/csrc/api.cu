@@ -91,7 +91,9 @@ struct sht_plan {
     std::vector<ld> gl_w;      // GL: Gauss weights of the rings
     int nslab = 1;             // number of second-index values (1 for S^2, 2N-1 for SO(3), in gamma-FFT bin order)
     bool f32_inner = false;    // set while an fp32 transform runs its fp64-array core
-    int dtype = SHT_F64;       // SHT_F32: fp32 hot kernels (theta_f32.cu) and fp32 public arrays; staging and FFTs stay fp64
+    int dtype = SHT_F64;       // arithmetic of the hot kernels.  SHT_F32: fp32 kernels (theta_f32.cu); staging and FFTs stay fp64
+    bool io_f32 = false;       // the public arrays are fp32 (plan created with SHT_F32): fp64 copies around the core.  spin != 0 plans created
+                               // with SHT_F32 have io_f32 with dtype == SHT_F64 (the fp32 kernels recurse the second index n = 0 only)
     float4* ab32 = nullptr;    // fp32: [L][Lp] recursion coefficients {A, A, -B, -B}
     float *lam32_inv = nullptr, *lam32_fwd = nullptr;
     float *st32_inv = nullptr, *st32_fwd = nullptr; uint16_t *k16_inv = nullptr, *k16_fwd = nullptr;   // fp32 start values
@@ -449,12 +451,14 @@ void layout(sht_plan* P, char* base) {
     if (P->only_dir != 1) P->H = B.take<double2>(P->H_slab * P->nslab);
     if (P->reality && P->sampling != SHT_HEALPIX) P->cplx = B.take<double2>(P->map_elems * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
+    if (P->io_f32) {
+        const size_t ioe = P->map_elems > (size_t)L * P->M ? P->map_elems : (size_t)L * P->M;      // a map or a coefficient array
+        P->io_a = B.take<double2>(ioe); P->io_b = B.take<double2>(ioe);
+    }
     if (P->dtype == SHT_F32) {
         P->ab32 = B.take<float4>((size_t)L * Lp);
         P->st32_inv = B.take<float>((size_t)Lp * P->inv.ntp); P->k16_inv = B.take<uint16_t>((size_t)Lp * P->inv.ntp);
         P->st32_fwd = B.take<float>((size_t)Lp * P->fwd.ntp); P->k16_fwd = B.take<uint16_t>((size_t)Lp * P->fwd.ntp);
-        const size_t ioe = P->map_elems > (size_t)L * P->M ? P->map_elems : (size_t)L * P->M;      // a map or a coefficient array
-        P->io_a = B.take<double2>(ioe); P->io_b = B.take<double2>(ioe);
         P->lam32_inv = B.take<float>((size_t)(L + 1) * P->inv.ntp); P->lam32_fwd = B.take<float>((size_t)(L + 1) * P->fwd.ntp);
     }
     P->fft_work = B.take<char>(P->fft_work_bytes);
@@ -1192,11 +1196,14 @@ static sht_status make_s2_plan(sht_plan** out, int L, int spin, int sampling, in
     if ((opts & SHT_OPT_TILE64) && (opts & SHT_OPT_TILE128)) return SHT_EINVAL;
     if ((opts & SHT_OPT_INVSYM) && (opts & SHT_OPT_NO_INVSYM)) return SHT_EINVAL;
     if ((opts & SHT_OPT_GRAPH) && (opts & SHT_OPT_NO_GRAPH)) return SHT_EINVAL;
-    // fp32 variant (BASELINE config 5): spin 0 (the fp32 kernels recurse the second index n = 0), one map at a time, any sampling
-    if (dtype == SHT_F32 && (spin != 0 || batch != 1 || helper)) return SHT_EUNSUPPORTED;
+    // fp32 variant (BASELINE config 5): one map at a time, any sampling.  spin 0: the fp32 kernels; spin != 0: fp32 public arrays around the
+    // fp64 kernels (the fp32 kernels recurse the second index n = 0 only)
+    if (dtype == SHT_F32 && (batch != 1 || helper || (opts & SHT_OPT_ADJOINT))) return SHT_EUNSUPPORTED;
+    const bool io_f32 = dtype == SHT_F32;
+    if (io_f32 && spin != 0) dtype = SHT_F64;
     if (sampling == SHT_HEALPIX && nside > 8192) return SHT_EINVAL;
     sht_plan* P = new sht_plan();
-    P->dtype = dtype; P->opts = opts; P->helper = helper; P->only_dir = only_dir;
+    P->dtype = dtype; P->io_f32 = io_f32; P->opts = opts; P->helper = helper; P->only_dir = only_dir;
     P->precomp = (opts & SHT_OPT_PRECOMPUTE) != 0;
     P->kind = 0; P->L = L; P->spin = spin; P->sampling = sampling; P->nside = sampling == SHT_HEALPIX ? nside : 0; P->reality = reality ? 1 : 0;
     P->loop = loop;
@@ -1494,7 +1501,7 @@ sht_status sht_plan_set_shard(sht_plan* P, int rank, int nranks) {
     if (!P || nranks < 1 || rank < 0 || rank >= nranks) return SHT_EINVAL;
     bool mirror_writes = false;      // an inverse fold pass writes the -m orders of the MIRRORED rings: not confined to a ring share
     for (auto& ph : P->pinv) mirror_writes = mirror_writes || ph.p.fold;
-    if (nranks > 1 && (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64 || P->invsym || mirror_writes || (P->opts & SHT_OPT_ADJOINT))) {   // (precompute plans shard too)
+    if (nranks > 1 && (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64 || P->io_f32 || P->invsym || mirror_writes || (P->opts & SHT_OPT_ADJOINT))) {   // (precompute plans shard too)
         g_err = "ring shards need a single-map fp64 plan created with SHT_OPT_NO_INVSYM and without SHT_OPT_ADJOINT";
         return SHT_EUNSUPPORTED;
     }
@@ -1520,7 +1527,7 @@ sht_status sht_plan_stage_bytes(const sht_plan* P, double bytes[3]) {
 sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !Fm || P->kind != 0) return SHT_EINVAL;
-    if (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64 || P->io_f32) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     begin_transform(P);
     CS(run_theta_inverse(P, (const double2*)flm, st));
@@ -1533,7 +1540,7 @@ sht_status s2_theta_inverse_plan(sht_plan* P, const void* flm, void* Fm, sht_str
 sht_status s2_theta_forward_plan(sht_plan* P, const void* Wm, void* flm, sht_stream stream) {
     CS(check_ready(P));
     if (!Wm || !flm || P->kind != 0) return SHT_EINVAL;
-    if (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (P->batch > 1 || P->loop > 1 || P->dtype != SHT_F64 || P->io_f32) return SHT_EUNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     begin_transform(P);
     // this entry point takes rows that already carry the quadrature weight, so the split runs with unit weights
@@ -1556,7 +1563,7 @@ static sht_status s2_inverse_body(sht_plan* P, const void* flm, void* f, sht_str
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L;
     const size_t ncoef = (size_t)L * P->M, nmap = P->map_elems;
-    if (P->dtype == SHT_F32 && !P->f32_inner) {      // fp32 public arrays: fp64 copies around the core (staging and FFTs are fp64)
+    if (P->io_f32 && !P->f32_inner) {      // fp32 public arrays: fp64 copies around the core (staging and FFTs are fp64)
         CK(st_f32_to_f64(2 * ncoef, (const float*)flm, (double*)P->io_a, st));
         P->f32_inner = true;
         sht_status s = s2_inverse_body(P, P->io_a, P->io_b, stream);
@@ -1583,7 +1590,7 @@ static sht_status s2_forward_body(sht_plan* P, const void* f, void* flm, sht_str
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L;
     const size_t ncoef = (size_t)L * P->M, nmap = P->map_elems;
-    if (P->dtype == SHT_F32 && !P->f32_inner) {
+    if (P->io_f32 && !P->f32_inner) {
         CK(st_f32_to_f64(P->reality ? nmap : 2 * nmap, (const float*)f, (double*)P->io_a, st));
         P->f32_inner = true;
         sht_status s = s2_forward_body(P, P->io_a, P->io_b, stream);
@@ -1626,6 +1633,7 @@ sht_status s2_forward_iter_plan(sht_plan* P, const void* f, void* flm, int niter
     if (!flm || !f || P->kind != 0 || niter < 0) return SHT_EINVAL;
     if (P->sampling != SHT_HEALPIX) { g_err = "iterative refinement is a HEALPix feature: the other samplings are exact"; return SHT_EUNSUPPORTED; }
     if (P->loop > 1) { g_err = "iterative refinement is a single-map call"; return SHT_EUNSUPPORTED; }
+    if (P->io_f32) { g_err = "iterative refinement needs an fp64 plan (the residual is formed in fp64 arrays)"; return SHT_EUNSUPPORTED; }
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nm = P->map_elems * (P->reality ? 1 : 2), nc = 2 * (size_t)P->L * P->M;
     CS(s2_forward_plan(P, f, flm, stream));
@@ -1852,8 +1860,8 @@ sht_status run_transform(sht_plan* P, int kind, const void* in, void* out, sht_s
 
 extern "C" {
 // bytes of one map / one coefficient array of the public arrays (plans that run a batch map by map step through them)
-static size_t map_bytes(const sht_plan* P) { return P->map_elems * (P->reality ? 1 : 2) * (P->dtype == SHT_F32 ? 4 : 8); }
-static size_t coef_bytes(const sht_plan* P) { return (size_t)P->L * P->M * 2 * (P->dtype == SHT_F32 ? 4 : 8); }
+static size_t map_bytes(const sht_plan* P) { return P->map_elems * (P->reality ? 1 : 2) * (P->io_f32 ? 4 : 8); }
+static size_t coef_bytes(const sht_plan* P) { return (size_t)P->L * P->M * 2 * (P->io_f32 ? 4 : 8); }
 sht_status s2_inverse_plan(sht_plan* P, const void* flm, void* f, sht_stream stream) {
     CS(check_ready(P));
     if (!flm || !f || P->kind != 0) return SHT_EINVAL;

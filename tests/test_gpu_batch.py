@@ -108,14 +108,15 @@ def test_batched_spin0_forward_with_and_without_fold(api, orc, fold, L, batch, r
         assert rel(got[b], orc.s2_forward(L, 0, orc.MW, g[b].astype(np.complex128))) < TOL, b
 
 
-@pytest.mark.parametrize("kind", ["hp", "mwss", "dh", "gl", "f32"])
+@pytest.mark.parametrize("kind", ["hp", "mwss", "dh", "gl", "f32", "f32s2"])
 def test_batches_without_batched_kernels_run_map_by_map(api, orc, kind):
     """A batch on a sampling (or dtype) the shared-recursion DMMA kernels do not serve is accepted and transformed map by map through the
     single-map kernels: same array layout (leading [batch] axis), every map against the oracle."""
     L, B = 40, 3
-    if kind == "f32":
-        P = api.Plan(L, 0, batch=B, dtype="f32")
-        os_, okw, spin, tol = orc.MW, {}, 0, 1e-4
+    if kind in ("f32", "f32s2"):               # (f32s2: fp32 arrays around the fp64 kernels, spin 2)
+        spin = 2 if kind == "f32s2" else 0
+        P = api.Plan(L, spin, batch=B, dtype="f32")
+        os_, okw, tol = orc.MW, {}, 1e-4
     else:
         gs, os_ = {"hp": (api.HEALPIX, orc.HEALPIX), "mwss": (api.MWSS, orc.MWSS), "dh": (api.DH, orc.DH), "gl": (api.GL, orc.GL)}[kind]
         nside = 8 if kind == "hp" else 0
@@ -123,7 +124,7 @@ def test_batches_without_batched_kernels_run_map_by_map(api, orc, kind):
         P = api.Plan(L, spin, sampling=gs, nside=nside, batch=B)
         okw = dict(nside=nside) if kind == "hp" else {}
     flm = np.stack([synth.random_flm(L, spin, seed=50 + b) for b in range(B)])
-    x = flm.astype(np.complex64) if kind == "f32" else flm
+    x = flm.astype(np.complex64) if kind in ("f32", "f32s2") else flm
     f = P.inverse(dev(x))
     assert tuple(f.shape)[0] == B
     for b in range(B):

@@ -49,9 +49,36 @@ def test_f32_inverse_forward_vs_oracle(api, orc, L, real):
 
 def test_f32_unsupported_requests_are_refused(api):
     from paper_2311_14670_b200._lib import ShtError
-    for kw in (dict(spin=2), dict(N=3)):       # (a batch is accepted: it runs map by map; every sampling is served for spin 0)
+    # (a batch is accepted: it runs map by map; every sampling and every spin is served)
+    for kw in (dict(N=3), dict(spin=2, adjoint=True), dict(spin=0, adjoint=True), dict(spin=0, precompute=True), dict(spin=1, precompute=True)):
         with pytest.raises(ShtError):
             api.Plan(16, dtype="f32", **kw)
+    P = api.Plan(16, 2, dtype="f32")
+    with pytest.raises(ShtError):                # the theta-stage entry points take fp64 arrays: fp64 plans only
+        P.theta_inverse(torch.zeros((16, 31), dtype=torch.complex128, device="cuda"))
+    H = api.Plan(16, 2, sampling=api.HEALPIX, nside=8, dtype="f32")
+    with pytest.raises(ShtError):
+        H.forward_iter(torch.zeros(H.map_shape, dtype=torch.complex64, device="cuda"), 1)
+
+
+@pytest.mark.parametrize("L,spin,sampling", [(33, 1, "mw"), (130, -2, "mw"), (257, 2, "mw"), (64, 2, "dh"), (48, -1, "mwss"), (40, 2, "gl")])
+def test_f32_arrays_with_spin_run_the_fp64_kernels(api, orc, L, spin, sampling):
+    """SHT_F32 with spin != 0: fp32 public arrays around the fp64 kernels (the fp32 kernels recurse n = 0 only).  The result is the fp64
+    transform of the fp32-rounded input, rounded to fp32: well inside the fp32 tolerance, asserted at 2e-6."""
+    code = {"mw": api.MW, "dh": api.DH, "mwss": api.MWSS, "gl": api.GL}[sampling]
+    oc = {"mw": orc.MW, "dh": orc.DH, "mwss": orc.MWSS, "gl": orc.GL}[sampling]
+    flm = synth.random_flm(L, spin, seed=3 * L + spin, sigma=synth.SIGMA_RED)
+    P = api.Plan(L, spin, sampling=code, dtype="f32")
+    f = P.inverse(dev(flm.astype(np.complex64))).cpu().numpy()
+    assert f.dtype == np.complex64 and f.shape == tuple(P.map_shape)
+    f_ref = orc.s2_inverse(L, spin, oc, flm)
+    assert rel(f, f_ref) < 2e-6
+    back = P.forward(dev(f_ref.astype(np.complex64))).cpu().numpy()
+    assert back.dtype == np.complex64
+    assert rel(back, flm) < 2e-6
+    P64 = api.Plan(L, spin, sampling=code)
+    f64 = P64.inverse(dev(flm.astype(np.complex64).astype(np.complex128))).cpu().numpy()
+    assert np.array_equal(f, f64.astype(np.complex64)) or rel(f, f64) < 1e-7      # same kernels, rounded once on the way out
 
 
 def test_f32_config5a_scale_L2048_sampled(api, orc):
