@@ -452,7 +452,7 @@ void layout(sht_plan* P, char* base) {
     if (P->reality && P->sampling != SHT_HEALPIX) P->cplx = B.take<double2>(P->map_elems * P->batch);
     if (P->kind == 1) P->fn = B.take<double2>((size_t)P->nslab * L * NB);
     if (P->io_f32) {
-        const size_t ioe = P->map_elems > (size_t)L * P->M ? P->map_elems : (size_t)L * P->M;      // a map or a coefficient array
+        const size_t ioe = (P->map_elems > (size_t)L * P->M ? P->map_elems : (size_t)L * P->M) * (P->kind == 1 ? P->nslab : 1);   // a map or a coefficient array
         P->io_a = B.take<double2>(ioe); P->io_b = B.take<double2>(ioe);
     }
     if (P->dtype == SHT_F32) {
@@ -1284,8 +1284,10 @@ sht_status sht_plan_so3_opts(sht_plan** out, int L, int N, int dtype, unsigned o
     if (!out) return SHT_EINVAL;
     *out = nullptr;
     if (L < 1 || L > 16384 || N < 1 || N > L) return SHT_EINVAL;
-    if (dtype != SHT_F64) return SHT_EUNSUPPORTED;
+    if (dtype != SHT_F64 && dtype != SHT_F32) return SHT_EINVAL;
+    if (dtype == SHT_F32 && (opts & SHT_OPT_ADJOINT)) return SHT_EUNSUPPORTED;
     sht_plan* P = new sht_plan();
+    P->io_f32 = dtype == SHT_F32;          // fp32 public arrays around the fp64 kernels (the orders n != 0 need them, see make_s2_plan)
     P->kind = 1; P->L = L; P->N = N; P->sampling = SHT_MW;
     P->nslab = 2 * N - 1;
     for (int b = 0; b < P->nslab; ++b) P->slab_n.push_back(b < N ? b : b - (2 * N - 1));   // gamma-FFT bin order
@@ -1773,6 +1775,16 @@ static sht_status so3_inverse_body(sht_plan* P, const void* flmn, void* f, sht_s
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB, N = P->N;
     const size_t slab = (size_t)L * NB;
+    if (P->io_f32 && !P->f32_inner) {      // fp32 public arrays: fp64 copies around the core
+        CK(st_f32_to_f64(2 * slab * P->nslab, (const float*)flmn, (double*)P->io_a, st));
+        P->f32_inner = true;
+        sht_status s = so3_inverse_body(P, P->io_a, P->io_b, stream);
+        P->f32_inner = false;
+        if (s != SHT_OK) return s;
+        CK(st_f64_to_f32(2 * slab * P->nslab, (const double*)P->io_b, (float*)f, st));
+        stage(P, CAT_STAGE, st);
+        return SHT_OK;
+    }
     begin_transform(P);
     stage(P, CAT_STAGE, st);
     // (coefficient slabs are read in place: the staging kernels map gamma-FFT bin order to n order through d_cslab)
@@ -1790,6 +1802,16 @@ static sht_status so3_forward_body(sht_plan* P, const void* f, void* flmn, sht_s
     cudaStream_t st = (cudaStream_t)stream;
     const int L = P->L, NB = P->NB, N = P->N;
     const size_t slab = (size_t)L * NB;
+    if (P->io_f32 && !P->f32_inner) {
+        CK(st_f32_to_f64(2 * slab * P->nslab, (const float*)f, (double*)P->io_a, st));
+        P->f32_inner = true;
+        sht_status s = so3_forward_body(P, P->io_a, P->io_b, stream);
+        P->f32_inner = false;
+        if (s != SHT_OK) return s;
+        CK(st_f64_to_f32(2 * slab * P->nslab, (const double*)P->io_b, (float*)flmn, st));
+        stage(P, CAT_STAGE, st);
+        return SHT_OK;
+    }
     begin_transform(P);
     stage(P, CAT_FFT, st);
     CS(fft_exec(P, P->fft_gamma, (double2*)const_cast<void*>(f), P->fn, CUFFT_FORWARD, st));   // Eq. 16 (q_Gamma in scale_fwd)

@@ -42,8 +42,9 @@ def test_status_strings_and_argument_validation(lib):
     assert lib.sht_plan_s2(C.byref(h), 8, 2, 0, 0, 1, 0) == 1          # reality needs spin 0 (R15)
     assert lib.sht_plan_s2(C.byref(h), 8, 0, 7, 0, 0, 0) == 1          # unknown sampling
     assert lib.sht_plan_s2(C.byref(h), 8, 0, 1, 0, 0, 0) == 1          # HEALPix needs nside >= 1
-    assert lib.sht_plan_so3(C.byref(h), 8, 3, 1) == 2                  # fp32 arrays: S^2 plans only ...
-    assert lib.sht_plan_s2_opts(C.byref(h), 8, 2, 0, 0, 0, 1, 1, 32) == 2         # ... and not with SHT_OPT_ADJOINT
+    assert lib.sht_plan_so3_opts(C.byref(h), 8, 3, 1, 32) == 2                    # fp32 arrays: not with SHT_OPT_ADJOINT
+    assert lib.sht_plan_s2_opts(C.byref(h), 8, 2, 0, 0, 0, 1, 1, 32) == 2
+    assert lib.sht_plan_so3(C.byref(h), 8, 3, 7) == 1                  # unknown dtype
     assert lib.sht_plan_s2(C.byref(h), 8, 0, 0, 0, 0, 7) == 1          # unknown dtype
     assert lib.sht_plan_so3(C.byref(h), 8, 9, 0) == 1                  # N > L
     assert lib.sht_plan_s2(C.byref(h), 8, 0, 9, 0, 0, 0) == 1          # sampling codes are 0..4 (MW, HEALPix, MWSS, DH, GL)

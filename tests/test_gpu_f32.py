@@ -50,7 +50,7 @@ def test_f32_inverse_forward_vs_oracle(api, orc, L, real):
 def test_f32_unsupported_requests_are_refused(api):
     from paper_2311_14670_b200._lib import ShtError
     # (a batch is accepted: it runs map by map; every sampling and every spin is served)
-    for kw in (dict(N=3), dict(spin=2, adjoint=True), dict(spin=0, adjoint=True), dict(spin=0, precompute=True), dict(spin=1, precompute=True)):
+    for kw in (dict(N=3, adjoint=True), dict(spin=2, adjoint=True), dict(spin=0, adjoint=True), dict(spin=0, precompute=True), dict(spin=1, precompute=True)):
         with pytest.raises(ShtError):
             api.Plan(16, dtype="f32", **kw)
     P = api.Plan(16, 2, dtype="f32")
@@ -128,3 +128,16 @@ def test_f32_other_samplings_vs_oracle(api, orc, name, nside, real, L, fold):
     want = orc.s2_forward(L, 0, os_, ref.astype(np.complex128), **okw)
     back = P.forward(torch.from_numpy(ref.astype(np.float32 if real else np.complex64)).cuda()).cpu().numpy()
     assert float(np.abs(back - want).max() / np.abs(want).max()) < 1e-4
+
+
+@pytest.mark.parametrize("L,N", [(16, 3), (40, 8), (130, 2)])
+def test_f32_arrays_so3_run_the_fp64_kernels(api, orc, L, N):
+    """sht_plan_so3 with SHT_F32: complex64 arrays around the fp64 kernels (Eq. 15-18 need the orders n != 0)."""
+    flmn = synth.random_flmn(L, N, seed=L + N)
+    P = api.Plan(L, N=N, dtype="f32")
+    f = P.inverse(dev(flmn.astype(np.complex64))).cpu().numpy()
+    assert f.dtype == np.complex64 and f.shape == (2 * N - 1, L, 2 * L - 1)
+    f_ref = orc.so3_inverse(L, N, flmn)
+    assert rel(f, f_ref) < 2e-6
+    back = P.forward(dev(f_ref.astype(np.complex64))).cpu().numpy()
+    assert back.dtype == np.complex64 and rel(back, flmn) < 2e-6
