@@ -31,7 +31,7 @@
  *     2^-122900.  Plan creation returns SHT_EUNSUPPORTED when the smallest start value of the plan's ring sets falls below that
  *     (MW sampling: L above ~9090; HEALPix with L = 2 nside: far beyond nside = 8192).  Nothing is ever silently dropped.
  *   - dtype: SHT_F64, or SHT_F32 (S^2 plans of any sampling and spin, SO(3) plans; BASELINE config 5; adjoints, precompute, the
- *     theta-stage entry points, ring shards and s2_forward_iter_plan return SHT_EUNSUPPORTED with SHT_F32).  With SHT_F32 every public
+ *     theta-stage entry points and ring shards return SHT_EUNSUPPORTED with SHT_F32).  With SHT_F32 every public
  *     array is interleaved floats (complex64 / float32); FFTs and staging run in fp64 on internal copies.  S^2, spin 0: the fused
  *     recursion + contraction kernels compute in fp32 (Eq. 25 in the paper's own form, windows of 2^48).  spin != 0 and SO(3): the fp32
  *     kernels recurse the second index n = 0 only, so the fp64 kernels run between the fp32 arrays (fp32 storage, fp64 arithmetic:

@@ -128,6 +128,7 @@ struct sht_plan {
     bool helper = false;
     int only_dir = 0;          // helper plans: 1 = inverse-type kernel only, 2 = forward-type kernel only
     double *it_map = nullptr, *it_coef = nullptr;   // HEALPix iterative refinement: residual map / coefficient update scratch
+    double *it_f = nullptr, *it_acc = nullptr;      // ... of plans with fp32 public arrays: fp64 copies of the map and of the running coefficients
     double* wq_map = nullptr;  // [F_ld] quadrature weight of every ring of the map (direct-quadrature samplings; adjoints)
     double* wq_quad = nullptr; // [4L] MW / MWSS: weight of every one of the 2L quadrature rings (not folded; adjoints)
     int device = 0, nsm = 0;   // device the plan was created on and its SM count (tile choice)
@@ -442,6 +443,7 @@ void layout(sht_plan* P, char* base) {
         } else {
             P->it_map = B.take<double>(P->map_elems * (P->reality ? 1 : 2));
             P->it_coef = B.take<double>(2 * (size_t)L * P->M);
+            if (P->io_f32) { P->it_f = B.take<double>(P->map_elems * (P->reality ? 1 : 2)); P->it_acc = B.take<double>(2 * (size_t)L * P->M); }
             P->hp_C = B.take<double2>((size_t)P->hp_ncap * P->hp_M);
             P->hp_BF = B.take<double2>((size_t)(P->hp_ncap / 2) * P->hp_M);
             P->hp_E = B.take<double2>((size_t)P->hp_neq * 4 * P->nside);
@@ -1635,9 +1637,25 @@ sht_status s2_forward_iter_plan(sht_plan* P, const void* f, void* flm, int niter
     if (!flm || !f || P->kind != 0 || niter < 0) return SHT_EINVAL;
     if (P->sampling != SHT_HEALPIX) { g_err = "iterative refinement is a HEALPix feature: the other samplings are exact"; return SHT_EUNSUPPORTED; }
     if (P->loop > 1) { g_err = "iterative refinement is a single-map call"; return SHT_EUNSUPPORTED; }
-    if (P->io_f32) { g_err = "iterative refinement needs an fp64 plan (the residual is formed in fp64 arrays)"; return SHT_EUNSUPPORTED; }
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nm = P->map_elems * (P->reality ? 1 : 2), nc = 2 * (size_t)P->L * P->M;
+    if (P->io_f32) {
+        // fp32 public arrays: the map, the running coefficients and the residual are kept in fp64 between the transforms (whose hot kernels
+        // compute in fp32 for spin 0), so the iteration converges to what the transforms resolve, not to the rounding of the arrays
+        CK(st_f32_to_f64(nm, (const float*)f, P->it_f, st));
+        P->f32_inner = true;
+        sht_status s = s2_forward_body(P, P->it_f, P->it_acc, stream);
+        for (int it = 0; it < niter && s == SHT_OK; ++it) {
+            s = s2_inverse_body(P, P->it_acc, P->it_map, stream);
+            if (s == SHT_OK) s = st_vec_sub(nm, P->it_f, P->it_map, P->it_map, st) == cudaSuccess ? SHT_OK : SHT_ECUDA;
+            if (s == SHT_OK) s = s2_forward_body(P, P->it_map, P->it_coef, stream);
+            if (s == SHT_OK) s = st_vec_add(nc, P->it_coef, P->it_acc, st) == cudaSuccess ? SHT_OK : SHT_ECUDA;
+        }
+        P->f32_inner = false;
+        if (s != SHT_OK) return s;
+        CK(st_f64_to_f32(nc, P->it_acc, (float*)flm, st));
+        return SHT_OK;
+    }
     CS(s2_forward_plan(P, f, flm, stream));
     for (int it = 0; it < niter; ++it) {
         CS(s2_inverse_plan(P, flm, P->it_map, stream));

@@ -56,9 +56,6 @@ def test_f32_unsupported_requests_are_refused(api):
     P = api.Plan(16, 2, dtype="f32")
     with pytest.raises(ShtError):                # the theta-stage entry points take fp64 arrays: fp64 plans only
         P.theta_inverse(torch.zeros((16, 31), dtype=torch.complex128, device="cuda"))
-    H = api.Plan(16, 2, sampling=api.HEALPIX, nside=8, dtype="f32")
-    with pytest.raises(ShtError):
-        H.forward_iter(torch.zeros(H.map_shape, dtype=torch.complex64, device="cuda"), 1)
 
 
 @pytest.mark.parametrize("L,spin,sampling", [(33, 1, "mw"), (130, -2, "mw"), (257, 2, "mw"), (64, 2, "dh"), (48, -1, "mwss"), (40, 2, "gl")])
@@ -141,3 +138,21 @@ def test_f32_arrays_so3_run_the_fp64_kernels(api, orc, L, N):
     assert rel(f, f_ref) < 2e-6
     back = P.forward(dev(f_ref.astype(np.complex64))).cpu().numpy()
     assert back.dtype == np.complex64 and rel(back, flmn) < 2e-6
+
+
+@pytest.mark.parametrize("spin,real,tol", [(0, False, 1e-4), (0, True, 1e-4), (2, False, 2e-6)])
+def test_f32_healpix_refinement_keeps_fp64_state(api, spin, real, tol):
+    """s2_forward_iter_plan on a plan with fp32 arrays: the running coefficients and the residual stay in fp64 between the transforms, so the
+    result follows the fp64 plan's iteration on the same (fp32-rounded) map."""
+    nside, L, niter = 16, 32, 3
+    rng = np.random.default_rng(7 + spin)
+    g = rng.standard_normal(12 * nside * nside) + (0 if real else 1j * rng.standard_normal(12 * nside * nside))
+    g32 = g.astype(np.float32 if real else np.complex64)
+    P32 = api.Plan(L, spin, sampling=api.HEALPIX, nside=nside, reality=real, dtype="f32")
+    P64 = api.Plan(L, spin, sampling=api.HEALPIX, nside=nside, reality=real)
+    want = P64.forward_iter(dev(g32.astype(np.float64 if real else np.complex128)), niter).cpu().numpy()
+    got = P32.forward_iter(dev(g32), niter).cpu().numpy()
+    assert got.dtype == np.complex64
+    assert rel(got, want) < tol
+    zero = P32.forward_iter(dev(g32), 0).cpu().numpy()
+    assert rel(zero, P32.forward(dev(g32)).cpu().numpy()) < 1e-6       # niter = 0 is the forward transform
