@@ -53,7 +53,7 @@ __device__ void na_seed(int l, int n, double sh, double ch, double& mant, int& e
     for (int j = 1; j <= l + n; ++j) { mant *= ch; na_norm(mant, ex); }
 }
 
-// Eq. 25 / 26 from m = l down to m_stop (>= -l) with second index n; stores sign(m) * d^l_{m,n} at column flip * m.
+// Eq. 25 / 26 from m = l down to m_stop (>= -l) with second index n; the iterate of step m is stored at order flip * m:
 //   flip = +1: E[m] = d^l_{m,n}                      (pass A)
 //   flip = -1: E[-m] = (-1)^{m+n} d^l_{m,n}         (pass B: d^l_{-m,-n} = (-1)^{m-n} d^l_{m,n}, called with the negated index)
 __device__ void na_recurse(int l, int n, int m_stop, int flip, double sh, double ch, double* E, size_t mstride, int L) {
