@@ -156,3 +156,19 @@ def test_f32_healpix_refinement_keeps_fp64_state(api, spin, real, tol):
     assert rel(got, want) < tol
     zero = P32.forward_iter(dev(g32), 0).cpu().numpy()
     assert rel(zero, P32.forward(dev(g32)).cpu().numpy()) < 1e-6       # niter = 0 is the forward transform
+
+
+def test_f32_arrays_with_spin_at_a_size_with_the_silent_head_skip(api, orc):
+    """fp32 arrays around the fp64 kernels at L >= 1024, where the fp64 kernels start from the stored silent-head state: sampled rings and a
+    round trip."""
+    L, spin = 1030, 1
+    flm = synth.random_flm(L, spin, seed=21, sigma=synth.SIGMA_RED)
+    P = api.Plan(L, spin, dtype="f32")
+    f = P.inverse(dev(flm.astype(np.complex64))).cpu().numpy()
+    rings = np.array([0, 1, 7, 500, 1028, 1029])
+    rows = orc.s2_inverse_rings(L, spin, orc.MW, flm, rings)
+    scale = max(np.abs(r).max() for r in rows)
+    for r, row in zip(rings, rows):
+        assert rel(f[r], row, scale) < 2e-6, r
+    back = P.forward(dev(f)).cpu().numpy()
+    assert rel(back, flm) < 2e-6
